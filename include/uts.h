@@ -1,0 +1,189 @@
+/* uts.h — C ABI of the B200-native HEALPix spherical Gaussian-splat rasteriser (libuts.so).
+ *
+ * One entry point per stage of UniTriSplat's Alg.1 and of its backward:
+ *
+ *   uts_preprocess      Alg.1 l.2-8   (Eq.1-2): projection to the unit sphere, Sigma_arc, conic, r_s, colour
+ *   uts_tile_query      Alg.1 l.9-14  (Alg.2): NESTED tile query, emits ((tile,rho),i) pairs
+ *   uts_sort            Alg.1 l.15: stable radix sort of the pairs by (tile, radial depth)
+ *   uts_tile_ranges     Alg.1 l.16: per-tile [start,end)
+ *   uts_render_fwd      Alg.1 l.17-30 (Eq.6) + FoV mask
+ *   uts_render_bwd      backward of Eq.6
+ *   uts_preprocess_bwd  Eq.3-4: to means, scales, rotations, SH
+ *
+ * Conventions
+ *   - extern "C"; every call returns an int status (UTS_OK = 0).  Nothing throws, aborts, allocates or frees
+ *     caller-visible memory: THE CALLER OWNS EVERY BUFFER, including scratch (sizes from uts_*_scratch_bytes).
+ *   - Every pointer is a DEVICE pointer unless its name starts with h_ (host; pinned where it is written
+ *     asynchronously).  uts_config is read on the host.  The only calls taking host data arrays are the
+ *     uts_host_* calls at the end.
+ *   - All work is enqueued on `stream` (a cudaStream_t passed as void*); calls are asynchronous.  Where a host
+ *     count is returned (h_n_pairs) the call synchronises the stream before returning, as documented there.
+ *   - No global state except the last CUDA error code; no CPU fallback; sm_100 only.
+ *   - Inputs are ACTIVATED values: scales > 0, opacity in (0,1), quaternion (w,x,y,z) used as given
+ *     (reading A14).  Arrays are dense row-major float32 unless stated.
+ *   - Index conventions: NESTED pixel p = f*4^k + interleave(x,y); tile of p = p >> (2*tile_log2); pixel slot
+ *     inside a tile = p & (4^tile_log2 - 1)  (Alg.1 l.18 PAPER.md:564).
+ */
+#ifndef UTS_H_
+#define UTS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  UTS_OK = 0,
+  UTS_ERR_INVALID_ARG = 1, /* null pointer, out-of-range config field, misaligned buffer */
+  UTS_ERR_CAPACITY = 2,    /* a caller buffer is too small; the needed size is written to the documented out-param */
+  UTS_ERR_CUDA = 3,        /* a CUDA runtime call failed; uts_last_cuda_error() returns the cudaError_t */
+  UTS_ERR_UNSUPPORTED = 4  /* device is not sm_100, or a config combination that is not implemented */
+};
+
+/* POD, host memory, passed by const pointer.  Field meaning follows Alg.1's Require line. */
+typedef struct {
+  int   order;             /* k; Nside = 1<<k; tile_log2 <= k <= 13 */
+  int   tile_log2;         /* l; B = 1<<l pixels per tile side; only 4 (16x16) is implemented     Table 6 */
+  int   query_refine_log2; /* log2 f; query pixels are at order k_q = k - l + log2 f; 0..l */
+  int   sh_degree;         /* 0..3; M = (sh_degree+1)^2 coefficients per channel */
+  int   n_gauss;           /* P */
+  int   n_views;           /* V >= 1 */
+  float r_near;            /* cull rho <= r_near                                                   reading A5 */
+  float cov_dilation_px2;  /* h = value * 4pi/N_pix added to diag(Sigma_arc); 0 disables           reading A3 */
+  float alpha_min;         /* skip alpha < alpha_min                                               reading A7 */
+  float alpha_max;         /* alpha = min(alpha_max, o*exp(power)); gradient zero when clamped     reading A7 */
+  float t_eps;             /* stop after the update when T < t_eps                                 Alg.1 l.27 PAPER.md:578 */
+  float bg[3];             /* out = C + T*bg                                                       reading A8 */
+} uts_config;
+
+/* Gaussian set G = {mu, s, q, o, c} (Alg.1 Require), SoA. */
+typedef struct {
+  const float* means;  /* [P,3] world space */
+  const float* scales; /* [P,3] */
+  const float* quats;  /* [P,4] (w,x,y,z) */
+  const float* opac;   /* [P]   */
+  const float* sh;     /* [P,M,3] */
+} uts_gaussians;
+
+/* Views V = [W|b], t = W mu + b. */
+typedef struct {
+  const float* W; /* [V,9] row-major 3x3 */
+  const float* b; /* [V,3] */
+} uts_views;
+
+/* Projected Gaussian records written by uts_preprocess, read by every later stage. */
+typedef struct {
+  float*   dir;        /* [V,P,3] unit direction t/rho in the camera frame                        Eq.1 */
+  float*   lonlat;     /* [V,P,2] (omega, phi) = (atan2(tx,tz), atan2(ty, hypot(tx,tz)))          Eq.1 */
+  float*   rho;        /* [V,P]   radial depth ||t||; its fp32 bit pattern is the sort depth      PAPER.md:112, reading A10 */
+  float*   conic_opac; /* [V,P,4] (A,B,C,o): power = -1/2 (A dx^2 + C dy^2) - B dx dy             Eq.2 inverse, Alg.1 l.23 */
+  float*   rs;         /* [V,P]   r_s = min(pi, 3 sqrt(lambda_max(Sigma_arc))) */
+  float*   rgb;        /* [V,P,3] max(0, 0.5 + sum_m Y_m sh_m)                                    reading A13 */
+  uint8_t* flags;      /* [V,P]   bit0 culled (no tiles, no gradient); bits1-3 R,G,B clamped at 0 */
+} uts_proj;
+
+/* FoV mask M_C (reading A19).  All NULL and n_active = -1  =>  full sphere, slot == tile.
+ * Otherwise all four are required. */
+typedef struct {
+  const uint32_t* active_tiles;    /* [n_active] ascending tile ids that contain at least one visible pixel */
+  int             n_active;
+  const int32_t*  slot_of_tile;    /* [N_tile] index into active_tiles, or -1 */
+  const uint32_t* pixel_mask_bits; /* [N_pix/32] bit (p & 31) of word p>>5 is M_C(p), NESTED order */
+} uts_mask;
+
+/* ---------------------------------------------------------------------------------------------- forward */
+
+/* Alg.1 l.2-8.  For each view v and Gaussian i fills every array of `out` at index v*P+i.  Culled records
+ * (rho <= r_near, non-finite input, det(Sigma_arc) <= 0) are written as zeros with flags bit0 set. */
+int uts_preprocess(const uts_config* cfg, uts_gaussians g, uts_views views, uts_proj out, void* stream);
+
+/* Alg.1 l.9-14 with Alg.2 (reading A6).  The tile set of (v,i) is
+ *     { q >> 2(k_q-k_t) : q an order-k_q NESTED pixel with  u . centre(q) >= cos(min(pi, r_s + rho_max(k_q))) } ∩ active tiles,
+ * evaluated in double precision.  Pairs are written in (view, Gaussian, tile) ascending order:
+ *     keys[j] = ((v*N_tile + tile) << 32) | float_bits(rho[v,i]),   vals[j] = i.
+ * offsets[V*P+1] (exclusive scan of the per-(v,i) counts) is always written.  The call synchronises `stream`
+ * and writes the pair count to *h_n_pairs (host).  keys == NULL: count only.  If the count exceeds `capacity`
+ * nothing is emitted and UTS_ERR_CAPACITY is returned (*h_n_pairs holds the needed capacity).
+ * scratch: uts_tile_query_scratch_bytes(cfg) bytes, 256-byte aligned. */
+int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, uint64_t* offsets, uint64_t* keys,
+                   uint32_t* vals, uint64_t capacity, uint64_t* h_n_pairs, void* scratch, size_t scratch_bytes,
+                   void* stream);
+size_t uts_tile_query_scratch_bytes(const uts_config* cfg);
+
+/* Alg.1 l.15.  Stable ascending LSD radix sort on the 64-bit key (ties keep emission order = ascending
+ * Gaussian id, reading A9).  Result is left in keys/vals; keys_tmp/vals_tmp are ping-pong buffers of the same
+ * size.  scratch: uts_sort_scratch_bytes(n_pairs) bytes, 256-byte aligned. */
+int uts_sort(const uts_config* cfg, uint64_t n_pairs, uint64_t* keys, uint32_t* vals, uint64_t* keys_tmp,
+             uint32_t* vals_tmp, void* scratch, size_t scratch_bytes, void* stream);
+size_t uts_sort_scratch_bytes(uint64_t n_pairs);
+
+/* Alg.1 l.16.  ranges[(v*N_tile + tile)*2 + {0,1}] = [start,end) in the sorted arrays; empty tiles get (0,0). */
+int uts_tile_ranges(const uts_config* cfg, uint64_t n_pairs, const uint64_t* keys, uint64_t* ranges, void* stream);
+
+/* Alg.1 l.17-30 + mask.  S = n_active (or N_tile on the full sphere); pixel index inside a slot is p & 255.
+ * color [V,S*256,3], alpha [V,S*256] (= 1 - T), trans [V,S*256] (the final transmittance T itself, kept for the
+ * backward because 1 - alpha loses it to rounding when T is small), n_last [V,S*256] (1 + list position of the
+ * last contributing entry, 0 if none).  Masked-out pixels get color 0, alpha 0, trans 1, n_last 0.
+ * Entry order inside a tile is the order of `vals`. */
+int uts_render_fwd(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
+                   float* color, float* alpha, float* trans, uint32_t* n_last, void* stream);
+
+/* --------------------------------------------------------------------------------------------- backward */
+
+/* Backward of the blend.  trans and n_last are uts_render_fwd's outputs.  dL_dalpha may be NULL.  Outputs are zeroed by the call, then accumulated with
+ * warp-reduced atomics (summation order is not deterministic):
+ * dL_drgb [V,P,3], dL_dconic [V,P,3] (off-diagonal stored once, reading A15), dL_dmu2 [V,P,2] (gradient
+ * w.r.t. the projected mean mu' = (omega, phi)), dL_dopac [P] (summed over views). */
+int uts_render_bwd(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
+                   const float* trans, const uint32_t* n_last, const float* dL_dcolor, const float* dL_dalpha,
+                   float* dL_drgb, float* dL_dconic, float* dL_dmu2, float* dL_dopac, void* stream);
+
+/* Eq.3-4 and the rest of the chain: every output is overwritten with the sum over views.
+ * dL_dmeans [P,3], dL_dscales [P,3], dL_dquats [P,4] (gradient of the R(q) polynomial), dL_dsh [P,M,3]. */
+int uts_preprocess_bwd(const uts_config* cfg, uts_gaussians g, uts_views views, const uint8_t* flags,
+                       const float* dL_drgb, const float* dL_dconic, const float* dL_dmu2, float* dL_dmeans,
+                       float* dL_dscales, float* dL_dquats, float* dL_dsh, void* stream);
+
+/* ------------------------------------------------------------------------------------------------- mask */
+
+/* Builds M_C on the device: kind 0 = spherical cap, h_params = axis[3], half_angle;
+ * kind 1 = pinhole frustum in the frame (right,up,fwd), h_params = right[3], up[3], fwd[3], tan_x, tan_y.
+ * pixel_mask_bits [N_pix/32], slot_of_tile [N_tile], active_tiles [N_tile] (first n_active entries valid).
+ * Synchronises `stream` and writes n_active to *h_n_active. */
+int uts_build_mask(const uts_config* cfg, int kind, const double* h_params, uint32_t* pixel_mask_bits,
+                   int32_t* slot_of_tile, uint32_t* active_tiles, int* h_n_active, void* stream);
+
+/* NESTED pixel centres as camera-frame unit vectors, double [n,3], pixels first..first+n-1 at `order`
+ * (exposes the library's HEALPix indexing for tests). */
+int uts_pixel_centers(int order, uint64_t first, uint64_t n, double* out_xyz, void* stream);
+/* rho_max(o), o = 0..13: largest centre-to-corner angle of an order-o pixel (Alg.2's PixRad, reading A6). Host. */
+int uts_rho_max_table(double* h_out14);
+
+/* ------------------------------------------------------------------------------------- whole path, host */
+
+/* Device workspace needed by uts_host_forward_backward for at most `pair_capacity` pairs. */
+size_t uts_host_workspace_bytes(const uts_config* cfg, int n_active, uint64_t pair_capacity);
+
+/* The whole hot path with HOST buffers: copies the Gaussians, views and upstream gradient to the device,
+ * runs preprocess -> tile query -> sort -> ranges -> blend forward -> blend backward -> preprocess backward,
+ * and copies image and gradients back.  Host arrays have the shapes of the device calls above; the mask
+ * arrays in `mask` are DEVICE pointers (built once by uts_build_mask).  h_dL_dcolor may be NULL (forward only).
+ * workspace: device memory of uts_host_workspace_bytes(); returns UTS_ERR_CAPACITY (needed pairs in *h_n_pairs)
+ * if it is too small.  Synchronises `stream` before returning. */
+int uts_host_forward_backward(const uts_config* cfg, const float* h_means, const float* h_scales, const float* h_quats,
+                              const float* h_opac, const float* h_sh, const float* h_W, const float* h_b, uts_mask mask,
+                              const float* h_dL_dcolor, float* h_color, float* h_alpha, float* h_dL_dmeans,
+                              float* h_dL_dscales, float* h_dL_dquats, float* h_dL_dopac, float* h_dL_dsh,
+                              uint64_t pair_capacity, uint64_t* h_n_pairs, void* workspace, size_t workspace_bytes,
+                              void* stream);
+
+int         uts_last_cuda_error(void);
+const char* uts_strerror(int status);
+const char* uts_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* UTS_H_ */

@@ -1,0 +1,295 @@
+"""Thin ctypes binding of libuts.so (include/uts.h): same names, argument marshalling only.
+
+torch is used for device memory and streams; every step of the path runs in the library's CUDA kernels.  There is no
+CPU fallback: importing works without a GPU (so that the symbol table can be checked), but any compute call needs the
+CUDA library and CUDA tensors and fails loudly otherwise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libuts.so")
+
+UTS_OK, UTS_ERR_INVALID_ARG, UTS_ERR_CAPACITY, UTS_ERR_CUDA, UTS_ERR_UNSUPPORTED = 0, 1, 2, 3, 4
+
+# every symbol include/uts.h declares
+SYMBOLS = [
+    "uts_preprocess", "uts_tile_query", "uts_tile_query_scratch_bytes", "uts_sort", "uts_sort_scratch_bytes",
+    "uts_tile_ranges", "uts_render_fwd", "uts_render_bwd", "uts_preprocess_bwd", "uts_build_mask", "uts_pixel_centers",
+    "uts_rho_max_table", "uts_host_workspace_bytes", "uts_host_forward_backward", "uts_last_cuda_error", "uts_strerror",
+    "uts_version",
+]
+
+
+class UtsError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = status
+        msg = lib().uts_strerror(status).decode()
+        extra = f" (cudaError {lib().uts_last_cuda_error()})" if status == UTS_ERR_CUDA else ""
+        super().__init__(f"{where}: {msg}{extra}")
+
+
+class CConfig(C.Structure):
+    _fields_ = [("order", C.c_int), ("tile_log2", C.c_int), ("query_refine_log2", C.c_int), ("sh_degree", C.c_int),
+                ("n_gauss", C.c_int), ("n_views", C.c_int), ("r_near", C.c_float), ("cov_dilation_px2", C.c_float),
+                ("alpha_min", C.c_float), ("alpha_max", C.c_float), ("t_eps", C.c_float), ("bg", C.c_float * 3)]
+
+
+class CGaussians(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("means", "scales", "quats", "opac", "sh")]
+
+
+class CViews(C.Structure):
+    _fields_ = [("W", C.c_void_p), ("b", C.c_void_p)]
+
+
+class CProj(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("dir", "lonlat", "rho", "conic_opac", "rs", "rgb", "flags")]
+
+
+class CMask(C.Structure):
+    _fields_ = [("active_tiles", C.c_void_p), ("n_active", C.c_int), ("slot_of_tile", C.c_void_p), ("pixel_mask_bits", C.c_void_p)]
+
+
+@dataclass
+class Config:
+    """uts_config (include/uts.h).  Defaults follow DESIGN.md readings A3, A5, A7, A8."""
+    order: int
+    n_gauss: int
+    n_views: int = 1
+    sh_degree: int = 0
+    tile_log2: int = 4
+    query_refine_log2: int = 2
+    r_near: float = 0.2
+    cov_dilation_px2: float = 0.3
+    alpha_min: float = 1.0 / 255.0
+    alpha_max: float = 0.99
+    t_eps: float = 1e-4
+    bg: tuple = (0.0, 0.0, 0.0)
+
+    @property
+    def n_pix(self): return 12 << (2 * self.order)
+    @property
+    def n_tiles(self): return 12 << (2 * (self.order - self.tile_log2))
+    @property
+    def ppt(self): return 1 << (2 * self.tile_log2)
+    @property
+    def n_sh(self): return (self.sh_degree + 1) ** 2
+
+    def c(self) -> CConfig:
+        return CConfig(self.order, self.tile_log2, self.query_refine_log2, self.sh_degree, self.n_gauss, self.n_views,
+                       self.r_near, self.cov_dilation_px2, self.alpha_min, self.alpha_max, self.t_eps, (C.c_float * 3)(*self.bg))
+
+
+_lib = None
+
+
+def lib():
+    """Loads libuts.so; raises if it has not been built (python -m paper_2606_29794_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2606_29794_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.uts_strerror.restype = C.c_char_p
+        L.uts_version.restype = C.c_char_p
+        for n in ("uts_tile_query_scratch_bytes", "uts_sort_scratch_bytes", "uts_host_workspace_bytes"):
+            getattr(L, n).restype = C.c_size_t
+        L.uts_sort_scratch_bytes.argtypes = [C.c_uint64]
+        L.uts_host_workspace_bytes.argtypes = [C.POINTER(CConfig), C.c_int, C.c_uint64]
+        _lib = L
+    return _lib
+
+
+def _ptr(t, dtype=None):
+    if t is None:
+        return None
+    if not t.is_cuda:
+        raise RuntimeError("uts: device tensor expected (no CPU fallback)")
+    if not t.is_contiguous():
+        raise RuntimeError("uts: contiguous tensor expected")
+    if dtype is not None and t.dtype != dtype:
+        raise RuntimeError(f"uts: expected {dtype}, got {t.dtype}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _check(st, where):
+    if st != UTS_OK:
+        raise UtsError(st, where)
+
+
+@dataclass
+class Gaussians:
+    means: torch.Tensor; scales: torch.Tensor; quats: torch.Tensor; opac: torch.Tensor; sh: torch.Tensor
+
+    def c(self): return CGaussians(*[_ptr(t, torch.float32) for t in (self.means, self.scales, self.quats, self.opac, self.sh)])
+
+
+@dataclass
+class Views:
+    W: torch.Tensor; b: torch.Tensor
+
+    def c(self): return CViews(_ptr(self.W, torch.float32), _ptr(self.b, torch.float32))
+
+
+@dataclass
+class Proj:
+    dir: torch.Tensor; lonlat: torch.Tensor; rho: torch.Tensor; conic_opac: torch.Tensor; rs: torch.Tensor
+    rgb: torch.Tensor; flags: torch.Tensor
+
+    @staticmethod
+    def empty(cfg: Config, device="cuda"):
+        V, P = cfg.n_views, cfg.n_gauss
+        f = lambda *s: torch.empty(*s, dtype=torch.float32, device=device)
+        return Proj(f(V, P, 3), f(V, P, 2), f(V, P), f(V, P, 4), f(V, P), f(V, P, 3), torch.empty(V, P, dtype=torch.uint8, device=device))
+
+    def c(self):
+        return CProj(*[_ptr(t, torch.float32) for t in (self.dir, self.lonlat, self.rho, self.conic_opac, self.rs, self.rgb)],
+                     _ptr(self.flags, torch.uint8))
+
+
+@dataclass
+class Mask:
+    """FoV mask arrays (device).  Mask.full() = whole sphere."""
+    active_tiles: torch.Tensor | None = None      # int32 storage of uint32 tile ids
+    n_active: int = -1
+    slot_of_tile: torch.Tensor | None = None      # int32
+    pixel_mask_bits: torch.Tensor | None = None   # int32 storage of uint32 words
+
+    @staticmethod
+    def full(): return Mask()
+
+    def n_slots(self, cfg: Config): return cfg.n_tiles if self.active_tiles is None else self.n_active
+
+    def c(self):
+        return CMask(_ptr(self.active_tiles), self.n_active, _ptr(self.slot_of_tile), _ptr(self.pixel_mask_bits))
+
+
+# ---------------------------------------------------------------------------------------------- the ABI calls
+def uts_preprocess(cfg: Config, g: Gaussians, views: Views, out: Proj, stream=None):
+    c = cfg.c()
+    _check(lib().uts_preprocess(C.byref(c), g.c(), views.c(), out.c(), _stream(stream)), "uts_preprocess")
+
+
+def uts_tile_query_scratch_bytes(cfg: Config) -> int:
+    c = cfg.c()
+    return int(lib().uts_tile_query_scratch_bytes(C.byref(c)))
+
+
+def uts_tile_query(cfg: Config, proj: Proj, mask: Mask, offsets, keys, vals, capacity: int, scratch, stream=None) -> int:
+    """Returns the pair count.  keys=None: count only.  Raises UtsError(UTS_ERR_CAPACITY) with .needed set."""
+    c = cfg.c()
+    n = C.c_uint64(0)
+    st = lib().uts_tile_query(C.byref(c), proj.c(), mask.c(), _ptr(offsets, torch.int64), _ptr(keys, torch.int64), _ptr(vals, torch.int32),
+                              C.c_uint64(capacity), C.byref(n), _ptr(scratch), C.c_size_t(scratch.numel() * scratch.element_size()),
+                              _stream(stream))
+    if st == UTS_ERR_CAPACITY:
+        e = UtsError(st, "uts_tile_query"); e.needed = int(n.value); raise e
+    _check(st, "uts_tile_query")
+    return int(n.value)
+
+
+def uts_sort_scratch_bytes(n_pairs: int) -> int:
+    return int(lib().uts_sort_scratch_bytes(C.c_uint64(n_pairs)))
+
+
+def uts_sort(cfg: Config, n_pairs: int, keys, vals, keys_tmp, vals_tmp, scratch, stream=None):
+    c = cfg.c()
+    _check(lib().uts_sort(C.byref(c), C.c_uint64(n_pairs), _ptr(keys, torch.int64), _ptr(vals, torch.int32), _ptr(keys_tmp, torch.int64),
+                          _ptr(vals_tmp, torch.int32), _ptr(scratch), C.c_size_t(scratch.numel() * scratch.element_size()),
+                          _stream(stream)), "uts_sort")
+
+
+def uts_tile_ranges(cfg: Config, n_pairs: int, keys, ranges, stream=None):
+    c = cfg.c()
+    _check(lib().uts_tile_ranges(C.byref(c), C.c_uint64(n_pairs), _ptr(keys, torch.int64), _ptr(ranges, torch.int64), _stream(stream)),
+           "uts_tile_ranges")
+
+
+def uts_render_fwd(cfg: Config, proj: Proj, mask: Mask, ranges, vals, color, alpha, trans, n_last, stream=None):
+    c = cfg.c()
+    _check(lib().uts_render_fwd(C.byref(c), proj.c(), mask.c(), _ptr(ranges, torch.int64), _ptr(vals, torch.int32),
+                                _ptr(color, torch.float32), _ptr(alpha, torch.float32), _ptr(trans, torch.float32),
+                                _ptr(n_last, torch.int32), _stream(stream)), "uts_render_fwd")
+
+
+def uts_render_bwd(cfg: Config, proj: Proj, mask: Mask, ranges, vals, trans, n_last, dL_dcolor, dL_dalpha, dL_drgb, dL_dconic,
+                   dL_dmu2, dL_dopac, stream=None):
+    c = cfg.c()
+    _check(lib().uts_render_bwd(C.byref(c), proj.c(), mask.c(), _ptr(ranges, torch.int64), _ptr(vals, torch.int32),
+                                _ptr(trans, torch.float32), _ptr(n_last, torch.int32), _ptr(dL_dcolor, torch.float32),
+                                _ptr(dL_dalpha, torch.float32), _ptr(dL_drgb, torch.float32), _ptr(dL_dconic, torch.float32),
+                                _ptr(dL_dmu2, torch.float32), _ptr(dL_dopac, torch.float32), _stream(stream)), "uts_render_bwd")
+
+
+def uts_preprocess_bwd(cfg: Config, g: Gaussians, views: Views, flags, dL_drgb, dL_dconic, dL_dmu2, dL_dmeans, dL_dscales,
+                       dL_dquats, dL_dsh, stream=None):
+    c = cfg.c()
+    _check(lib().uts_preprocess_bwd(C.byref(c), g.c(), views.c(), _ptr(flags, torch.uint8), _ptr(dL_drgb, torch.float32),
+                                    _ptr(dL_dconic, torch.float32), _ptr(dL_dmu2, torch.float32), _ptr(dL_dmeans, torch.float32),
+                                    _ptr(dL_dscales, torch.float32), _ptr(dL_dquats, torch.float32), _ptr(dL_dsh, torch.float32),
+                                    _stream(stream)), "uts_preprocess_bwd")
+
+
+def uts_build_mask(cfg: Config, kind: str, params, device="cuda", stream=None) -> Mask:
+    """kind 'cap': params = axis[3], half_angle; 'frustum': right[3], up[3], fwd[3], tan_x, tan_y."""
+    c = cfg.c()
+    bits = torch.empty(cfg.n_pix // 32, dtype=torch.int32, device=device)
+    slot = torch.empty(cfg.n_tiles, dtype=torch.int32, device=device)
+    act = torch.empty(cfg.n_tiles, dtype=torch.int32, device=device)
+    prm = (C.c_double * len(params))(*[float(x) for x in params])
+    n = C.c_int(0)
+    _check(lib().uts_build_mask(C.byref(c), C.c_int(0 if kind == "cap" else 1), prm, _ptr(bits), _ptr(slot), _ptr(act), C.byref(n),
+                                _stream(stream)), "uts_build_mask")
+    return Mask(act[: n.value].contiguous(), int(n.value), slot, bits)
+
+
+def uts_pixel_centers(order: int, first: int, n: int, device="cuda", stream=None):
+    out = torch.empty(n, 3, dtype=torch.float64, device=device)
+    _check(lib().uts_pixel_centers(C.c_int(order), C.c_uint64(first), C.c_uint64(n), _ptr(out), _stream(stream)), "uts_pixel_centers")
+    return out
+
+
+def uts_rho_max_table():
+    t = (C.c_double * 14)()
+    _check(lib().uts_rho_max_table(t), "uts_rho_max_table")
+    return list(t)
+
+
+def uts_host_workspace_bytes(cfg: Config, n_active: int, pair_capacity: int) -> int:
+    c = cfg.c()
+    return int(lib().uts_host_workspace_bytes(C.byref(c), C.c_int(n_active), C.c_uint64(pair_capacity)))
+
+
+def uts_host_forward_backward(cfg: Config, h, mask: Mask, h_dL_dcolor, h_out, pair_capacity: int, workspace, stream=None) -> int:
+    """h: dict of pinned/pageable HOST float32 tensors means, scales, quats, opac, sh, W, b.  h_out: dict of host tensors
+    color, alpha and (if h_dL_dcolor is given) dL_dmeans, dL_dscales, dL_dquats, dL_dopac, dL_dsh.  Returns the pair count."""
+    c = cfg.c()
+
+    def hp(t):
+        if t is None:
+            return None
+        assert (not t.is_cuda) and t.is_contiguous() and t.dtype == torch.float32
+        return C.c_void_p(t.data_ptr())
+
+    n = C.c_uint64(0)
+    st = lib().uts_host_forward_backward(
+        C.byref(c), hp(h["means"]), hp(h["scales"]), hp(h["quats"]), hp(h["opac"]), hp(h["sh"]), hp(h["W"]), hp(h["b"]), mask.c(),
+        hp(h_dL_dcolor), hp(h_out["color"]), hp(h_out.get("alpha")), hp(h_out.get("dL_dmeans")), hp(h_out.get("dL_dscales")),
+        hp(h_out.get("dL_dquats")), hp(h_out.get("dL_dopac")), hp(h_out.get("dL_dsh")), C.c_uint64(pair_capacity), C.byref(n),
+        _ptr(workspace), C.c_size_t(workspace.numel() * workspace.element_size()), _stream(stream))
+    if st == UTS_ERR_CAPACITY:
+        e = UtsError(st, "uts_host_forward_backward"); e.needed = int(n.value); raise e
+    _check(st, "uts_host_forward_backward")
+    return int(n.value)

@@ -1,0 +1,123 @@
+// uts_host.cu — the whole hot path behind one call that takes HOST buffers (bench.py's end-to-end leg and the
+// simplest way to use the library): H2D copies, the seven stages in Alg.1's order followed by the
+// backward, D2H copies.  All device memory comes from the caller's workspace.
+#include "uts_internal.cuh"
+
+namespace uts {
+
+struct Bump {
+  char* base; size_t off;
+  template <typename T> T* take(size_t n) {
+    off = (off + 255) & ~(size_t)255;
+    T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+    off += n * sizeof(T);
+    return p;
+  }
+};
+
+struct HostLayout {
+  float *means, *scales, *quats, *opac, *sh, *W, *b;
+  uts_proj proj;
+  uint64_t *offsets, *keys, *keys_tmp, *ranges;
+  uint32_t *vals, *vals_tmp, *n_last;
+  void *tq_scratch, *sort_scratch;
+  size_t tq_bytes, sort_bytes;
+  float *color, *alpha, *trans, *g_color;
+  float *g_rgb, *g_conic, *g_mu2, *g_opac, *g_means, *g_scales, *g_quats, *g_sh;
+  size_t total;
+};
+
+static HostLayout layout(const uts_config* cfg, int64_t n_slot, uint64_t cap, char* base) {
+  HostLayout L;
+  Bump B{base, 0};
+  const size_t P = cfg->n_gauss, V = cfg->n_views, M = (size_t)(cfg->sh_degree + 1) * (cfg->sh_degree + 1);
+  const size_t VP = V * P, npx = V * (size_t)n_slot * kTilePix;
+  const size_t ids = ((size_t)12 << (2 * (cfg->order - cfg->tile_log2))) * V;
+  L.means = B.take<float>(3 * P); L.scales = B.take<float>(3 * P); L.quats = B.take<float>(4 * P);
+  L.opac = B.take<float>(P); L.sh = B.take<float>(3 * M * P); L.W = B.take<float>(9 * V); L.b = B.take<float>(3 * V);
+  L.proj.dir = B.take<float>(3 * VP); L.proj.lonlat = B.take<float>(2 * VP); L.proj.rho = B.take<float>(VP);
+  L.proj.conic_opac = B.take<float>(4 * VP); L.proj.rs = B.take<float>(VP); L.proj.rgb = B.take<float>(3 * VP);
+  L.proj.flags = B.take<uint8_t>(VP);
+  L.offsets = B.take<uint64_t>(VP + 1);
+  L.tq_bytes = uts_tile_query_scratch_bytes(cfg); L.tq_scratch = B.take<char>(L.tq_bytes);
+  L.keys = B.take<uint64_t>(cap); L.keys_tmp = B.take<uint64_t>(cap);
+  L.vals = B.take<uint32_t>(cap); L.vals_tmp = B.take<uint32_t>(cap);
+  L.sort_bytes = uts_sort_scratch_bytes(cap); L.sort_scratch = B.take<char>(L.sort_bytes);
+  L.ranges = B.take<uint64_t>(2 * ids);
+  L.color = B.take<float>(3 * npx); L.alpha = B.take<float>(npx); L.trans = B.take<float>(npx); L.n_last = B.take<uint32_t>(npx);
+  L.g_color = B.take<float>(3 * npx);
+  L.g_rgb = B.take<float>(3 * VP); L.g_conic = B.take<float>(3 * VP); L.g_mu2 = B.take<float>(2 * VP); L.g_opac = B.take<float>(P);
+  L.g_means = B.take<float>(3 * P); L.g_scales = B.take<float>(3 * P); L.g_quats = B.take<float>(4 * P); L.g_sh = B.take<float>(3 * M * P);
+  L.total = B.off + 256;
+  return L;
+}
+
+}  // namespace uts
+
+using namespace uts;
+
+extern "C" {
+
+size_t uts_host_workspace_bytes(const uts_config* cfg, int n_active, uint64_t pair_capacity) {
+  if (check_config(cfg) != UTS_OK) return 0;
+  const int64_t n_tile = (int64_t)12 << (2 * (cfg->order - cfg->tile_log2));
+  return layout(cfg, n_active >= 0 ? n_active : n_tile, pair_capacity, nullptr).total;
+}
+
+int uts_host_forward_backward(const uts_config* cfg, const float* h_means, const float* h_scales, const float* h_quats,
+                              const float* h_opac, const float* h_sh, const float* h_W, const float* h_b, uts_mask mask,
+                              const float* h_dL_dcolor, float* h_color, float* h_alpha, float* h_dL_dmeans,
+                              float* h_dL_dscales, float* h_dL_dquats, float* h_dL_dopac, float* h_dL_dsh,
+                              uint64_t pair_capacity, uint64_t* h_n_pairs, void* workspace, size_t workspace_bytes,
+                              void* stream) {
+  int st = check_config(cfg);
+  if (st) return st;
+  if ((st = check_mask(cfg, mask))) return st;
+  if (!h_means || !h_scales || !h_quats || !h_opac || !h_sh || !h_W || !h_b || !h_color || !h_n_pairs || !workspace)
+    return UTS_ERR_INVALID_ARG;
+  const bool bwd = h_dL_dcolor != nullptr;
+  if (bwd && (!h_dL_dmeans || !h_dL_dscales || !h_dL_dquats || !h_dL_dopac || !h_dL_dsh)) return UTS_ERR_INVALID_ARG;
+  if ((uintptr_t)workspace & 255) return UTS_ERR_INVALID_ARG;
+  Dims d = dims_of(cfg, &mask);
+  HostLayout L = layout(cfg, d.n_slot, pair_capacity, reinterpret_cast<char*>(workspace));
+  if (L.total > workspace_bytes) return UTS_ERR_INVALID_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t P = d.P, V = d.V, M = d.M, npx = V * (size_t)d.n_slot * kTilePix;
+  const size_t f = sizeof(float);
+  UTS_CUDA(cudaMemcpyAsync(L.means, h_means, 3 * P * f, cudaMemcpyHostToDevice, s));
+  UTS_CUDA(cudaMemcpyAsync(L.scales, h_scales, 3 * P * f, cudaMemcpyHostToDevice, s));
+  UTS_CUDA(cudaMemcpyAsync(L.quats, h_quats, 4 * P * f, cudaMemcpyHostToDevice, s));
+  UTS_CUDA(cudaMemcpyAsync(L.opac, h_opac, P * f, cudaMemcpyHostToDevice, s));
+  UTS_CUDA(cudaMemcpyAsync(L.sh, h_sh, 3 * M * P * f, cudaMemcpyHostToDevice, s));
+  UTS_CUDA(cudaMemcpyAsync(L.W, h_W, 9 * V * f, cudaMemcpyHostToDevice, s));
+  UTS_CUDA(cudaMemcpyAsync(L.b, h_b, 3 * V * f, cudaMemcpyHostToDevice, s));
+  if (bwd) UTS_CUDA(cudaMemcpyAsync(L.g_color, h_dL_dcolor, 3 * npx * f, cudaMemcpyHostToDevice, s));
+
+  uts_gaussians g{L.means, L.scales, L.quats, L.opac, L.sh};
+  uts_views vw{L.W, L.b};
+  if ((st = uts_preprocess(cfg, g, vw, L.proj, stream))) return st;
+  if ((st = uts_tile_query(cfg, L.proj, mask, L.offsets, L.keys, L.vals, pair_capacity, h_n_pairs, L.tq_scratch, L.tq_bytes, stream)))
+    return st;
+  const uint64_t n = *h_n_pairs;
+  if ((st = uts_sort(cfg, n, L.keys, L.vals, L.keys_tmp, L.vals_tmp, L.sort_scratch, L.sort_bytes, stream))) return st;
+  if ((st = uts_tile_ranges(cfg, n, L.keys, L.ranges, stream))) return st;
+  if ((st = uts_render_fwd(cfg, L.proj, mask, L.ranges, L.vals, L.color, L.alpha, L.trans, L.n_last, stream))) return st;
+  UTS_CUDA(cudaMemcpyAsync(h_color, L.color, 3 * npx * f, cudaMemcpyDeviceToHost, s));
+  if (h_alpha) UTS_CUDA(cudaMemcpyAsync(h_alpha, L.alpha, npx * f, cudaMemcpyDeviceToHost, s));
+  if (bwd) {
+    if ((st = uts_render_bwd(cfg, L.proj, mask, L.ranges, L.vals, L.trans, L.n_last, L.g_color, nullptr, L.g_rgb, L.g_conic,
+                             L.g_mu2, L.g_opac, stream)))
+      return st;
+    if ((st = uts_preprocess_bwd(cfg, g, vw, L.proj.flags, L.g_rgb, L.g_conic, L.g_mu2, L.g_means, L.g_scales, L.g_quats, L.g_sh, stream)))
+      return st;
+    UTS_CUDA(cudaMemcpyAsync(h_dL_dmeans, L.g_means, 3 * P * f, cudaMemcpyDeviceToHost, s));
+    UTS_CUDA(cudaMemcpyAsync(h_dL_dscales, L.g_scales, 3 * P * f, cudaMemcpyDeviceToHost, s));
+    UTS_CUDA(cudaMemcpyAsync(h_dL_dquats, L.g_quats, 4 * P * f, cudaMemcpyDeviceToHost, s));
+    UTS_CUDA(cudaMemcpyAsync(h_dL_dopac, L.g_opac, P * f, cudaMemcpyDeviceToHost, s));
+    UTS_CUDA(cudaMemcpyAsync(h_dL_dsh, L.g_sh, 3 * M * P * f, cudaMemcpyDeviceToHost, s));
+  }
+  UTS_CUDA(cudaStreamSynchronize(s));
+  return UTS_OK;
+}
+
+}  // extern "C"

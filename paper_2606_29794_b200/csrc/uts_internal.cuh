@@ -1,0 +1,112 @@
+// uts_internal.cuh — shared by the CUDA translation units of libuts.so (not part of the ABI).
+// Holds: status / launch helpers, derived sizes of a uts_config, and the library's own HEALPix NESTED indexing
+// (§3.1; Gorski et al. as cited at PAPER.md:23).  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <math.h>
+#include "uts.h"
+
+namespace uts {
+
+constexpr double kPi = 3.14159265358979323846264338327950288;
+constexpr int kMaxOrder = 13;
+constexpr int kTileLog2 = 4;          // B = 16 (Table 6): the only tile size implemented
+constexpr int kTilePix = 256;         // B*B pixels per tile == threads per blend block
+
+// ------------------------------------------------------------------------------------------------ status
+void set_last_cuda_error(cudaError_t e);
+#define UTS_CUDA(call)                                                      \
+  do {                                                                      \
+    cudaError_t e__ = (call);                                               \
+    if (e__ != cudaSuccess) { ::uts::set_last_cuda_error(e__); return UTS_ERR_CUDA; } \
+  } while (0)
+#define UTS_LAUNCH_CHECK() UTS_CUDA(cudaGetLastError())
+
+int check_config(const uts_config* c);   // UTS_OK / UTS_ERR_INVALID_ARG / UTS_ERR_UNSUPPORTED
+int check_mask(const uts_config* c, const uts_mask& m);
+int sm_count();
+
+// --------------------------------------------------------------------------------------------- derived
+struct Dims {
+  int k, kt, kq, P, V, M;
+  int64_t n_pix, n_tile;
+  int64_t n_slot;       // tiles that get a thread block: n_active or n_tile
+};
+inline Dims dims_of(const uts_config* c, const uts_mask* m) {
+  Dims d;
+  d.k = c->order; d.kt = c->order - c->tile_log2; d.kq = d.kt + c->query_refine_log2;
+  d.P = c->n_gauss; d.V = c->n_views; d.M = (c->sh_degree + 1) * (c->sh_degree + 1);
+  d.n_pix = (int64_t)12 << (2 * d.k);
+  d.n_tile = (int64_t)12 << (2 * d.kt);
+  d.n_slot = (m && m->active_tiles) ? m->n_active : d.n_tile;
+  return d;
+}
+
+// rho_max(o) table (host, computed once): see uts_healpix.cu
+const double* rho_max_table_host();
+
+// ------------------------------------------------------------------------------------- HEALPix (device)
+// NESTED index p at order o  ->  face f and in-face integer coordinates (x,y): x in the even bits, y in the odd
+// bits of p mod 4^o.
+__host__ __device__ __forceinline__ uint32_t squeeze_even_bits(uint64_t v) {
+  v &= 0x5555555555555555ull;
+  v = (v | (v >> 1)) & 0x3333333333333333ull;
+  v = (v | (v >> 2)) & 0x0f0f0f0f0f0f0f0full;
+  v = (v | (v >> 4)) & 0x00ff00ff00ff00ffull;
+  v = (v | (v >> 8)) & 0x0000ffff0000ffffull;
+  v = (v | (v >> 16)) & 0x00000000ffffffffull;
+  return (uint32_t)v;
+}
+
+struct PixGeom {        // what fixes a pixel centre: z (or 1-|z| in the caps) and longitude in quarter-turn units
+  double z;             // sin(latitude) = HEALPix polar coordinate
+  double sth;           // cos(latitude)
+  double lam;           // longitude (radians), not wrapped
+};
+
+// Centre of NESTED pixel p at order o.
+// Derivation used here: inside face f = 4*r + c the centre sits at v = x + y - (N-1) half-rings above the face's
+// middle ring and h = x - y half-steps east of the face's central meridian.  Ring number from the north pole is
+// i = (r+1) N - v.  A ring holds 4*n pixels with n = min(i, N, 4N - i); the z of a ring is 1 - i^2/(3N^2) in the north
+// cap (i < N), 2(2N - i)/(3N) in the equatorial belt, and mirrored in the south cap.  The face's central meridian is
+// at (2c + 1 - (r & 1)) quarter-turns/2, and one half-step in a ring of 4n pixels is pi/(4n), so
+//      lambda = (pi/4) * ((2c + 1 - (r&1)) + h / n).
+__host__ __device__ __forceinline__ PixGeom pix_geom(int o, uint64_t p) {
+  const int64_t N = (int64_t)1 << o;
+  const int f = (int)(p >> (2 * o));
+  const uint64_t m = p & (((uint64_t)1 << (2 * o)) - 1);
+  const int64_t x = squeeze_even_bits(m), y = squeeze_even_bits(m >> 1);
+  const int r = f >> 2, c = f & 3;
+  const int64_t i = (int64_t)(r + 1) * N - (x + y - (N - 1));
+  const int64_t h = x - y;
+  PixGeom g;
+  int64_t n;
+  const double inv3N2 = 1.0 / (3.0 * (double)N * (double)N);
+  if (i < N) {                       // north polar cap
+    n = i;
+    const double w = (double)(n * n) * inv3N2;        // 1 - z
+    g.z = 1.0 - w; g.sth = sqrt(w * (2.0 - w));
+  } else if (i > 3 * N) {            // south polar cap
+    n = 4 * N - i;
+    const double w = (double)(n * n) * inv3N2;        // 1 + z
+    g.z = w - 1.0; g.sth = sqrt(w * (2.0 - w));
+  } else {                           // equatorial belt
+    n = N;
+    g.z = (double)(2 * (2 * N - i)) / (double)(3 * N);
+    g.sth = sqrt((1.0 - g.z) * (1.0 + g.z));
+  }
+  g.lam = (kPi / 4) * ((double)(2 * c + 1 - (r & 1)) + (double)h / (double)n);
+  return g;
+}
+
+// Camera-frame unit vector of a pixel centre.  Frame (reading A1): polar axis = camera +y, longitude 0 at camera +z,
+// longitude = omega = atan2(t_x, t_z)  =>  (x,y,z)_cam = (cos(lat) sin(lam), sin(lat), cos(lat) cos(lam)).
+__device__ __forceinline__ void pix_center_cam(int o, uint64_t p, double& vx, double& vy, double& vz) {
+  PixGeom g = pix_geom(o, p);
+  double s, c;
+  sincos(g.lam, &s, &c);
+  vx = g.sth * s; vy = g.z; vz = g.sth * c;
+}
+
+}  // namespace uts

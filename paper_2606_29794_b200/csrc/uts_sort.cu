@@ -1,0 +1,220 @@
+// uts_sort.cu — F3: stable LSD radix sort of ((tile, rho), i) pairs (Alg.1 l.15 PAPER.md:560; radial-depth ordering
+// PAPER.md:112; reading A9/A10) and F4: per-tile ranges (Alg.1 l.16 PAPER.md:561).
+//
+// Key = (view*N_tile + tile) << 32 | float_bits(rho); rho > 0 so the IEEE-754 pattern orders as an unsigned integer.
+// 8-bit digits, least significant first; only the bytes that can differ are sorted: 4 depth bytes plus
+// ceil(log2(V*N_tile)/8) tile bytes.  Each pass is reduce-then-scan (no inter-block spinning):
+//   upsweep   : per-block digit histogram                              reads  8 B/pair
+//   scan      : exclusive scan over [digit][block]                     ~1 KB per block
+//   downsweep : stable in-block ranking (warp match), reorder in shared memory, scatter in digit runs
+//                                                                      reads 12 B/pair, writes 12 B/pair
+// Stability: inside a block keys are ranked in (warp, item, lane) order, which is their memory order; blocks are
+// ordered by the scan.  So equal keys keep their emission order = ascending Gaussian id.
+#include "uts_internal.cuh"
+#include "uts_scan.cuh"
+
+namespace uts {
+
+constexpr int kSortThreads = 256;
+constexpr int kSortItems = 12;
+constexpr int kSortTile = kSortThreads * kSortItems;     // 3072 pairs per block (47 KB of static shared memory)
+constexpr int kSortWarps = kSortThreads / 32;
+constexpr int kRadix = 256;
+
+__device__ __forceinline__ uint32_t digit_of(uint64_t key, int shift) { return (uint32_t)(key >> shift) & (kRadix - 1); }
+
+// counts[digit * nb + block]
+__global__ void __launch_bounds__(kSortThreads)
+sort_upsweep(const uint64_t* __restrict__ keys, uint64_t n, int shift, uint32_t nb, uint32_t* __restrict__ counts) {
+  __shared__ uint32_t hist[kSortWarps][kRadix];
+  const int wid = threadIdx.x >> 5;
+  for (int i = threadIdx.x; i < kSortWarps * kRadix; i += kSortThreads) (&hist[0][0])[i] = 0;
+  __syncthreads();
+  const uint64_t base = (uint64_t)blockIdx.x * kSortTile;
+#pragma unroll 4
+  for (int j = 0; j < kSortItems; ++j) {
+    const uint64_t idx = base + (uint64_t)j * kSortThreads + threadIdx.x;
+    if (idx < n) atomicAdd(&hist[wid][digit_of(__ldg(keys + idx), shift)], 1u);
+  }
+  __syncthreads();
+  for (int d = threadIdx.x; d < kRadix; d += kSortThreads) {
+    uint32_t s = 0;
+#pragma unroll
+    for (int w = 0; w < kSortWarps; ++w) s += hist[w][d];
+    counts[(uint64_t)d * nb + blockIdx.x] = s;
+  }
+}
+
+__global__ void __launch_bounds__(kSortThreads)
+sort_downsweep(const uint64_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in, uint64_t* __restrict__ keys_out,
+               uint32_t* __restrict__ vals_out, uint64_t n, int shift, uint32_t nb, const uint64_t* __restrict__ offsets) {
+  __shared__ uint32_t whist[kSortWarps][kRadix];      // per-warp digit counts, then per-warp exclusive bases
+  __shared__ uint32_t dstart[kRadix];                 // start of each digit's run inside the block
+  __shared__ uint64_t gbase[kRadix];                  // global start of this block's run of each digit
+  __shared__ uint64_t skeys[kSortTile];
+  __shared__ uint32_t svals[kSortTile];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const uint32_t lt_mask = (1u << lane) - 1u;
+  for (int i = threadIdx.x; i < kSortWarps * kRadix; i += kSortThreads) (&whist[0][0])[i] = 0;
+  for (int d = threadIdx.x; d < kRadix; d += kSortThreads) gbase[d] = offsets[(uint64_t)d * nb + blockIdx.x];
+  __syncthreads();
+
+  // Memory order inside the block: warp-major, then item, then lane (each warp owns a contiguous 512-pair segment).
+  const uint64_t wbase = (uint64_t)blockIdx.x * kSortTile + (uint64_t)wid * (32 * kSortItems);
+  uint64_t key[kSortItems];
+  uint32_t val[kSortItems];
+  uint16_t rank[kSortItems];
+#pragma unroll
+  for (int j = 0; j < kSortItems; ++j) {
+    const uint64_t idx = wbase + (uint64_t)j * 32 + lane;
+    const bool ok = idx < n;
+    key[j] = ok ? __ldg(keys_in + idx) : ~0ull;
+    val[j] = ok ? __ldg(vals_in + idx) : 0u;
+  }
+#pragma unroll
+  for (int j = 0; j < kSortItems; ++j) {
+    const uint64_t idx = wbase + (uint64_t)j * 32 + lane;
+    const bool ok = idx < n;
+    const uint32_t d = digit_of(key[j], shift);
+    const uint32_t peers = __match_any_sync(0xffffffffu, ok ? d : 0xffffffffu);
+    const uint32_t before = whist[wid][d & (kRadix - 1)];
+    rank[j] = (uint16_t)(before + __popc(peers & lt_mask));
+    __syncwarp();
+    if (ok && (peers & lt_mask) == 0) whist[wid][d] = before + __popc(peers);   // leader of each digit group
+    __syncwarp();
+  }
+  __syncthreads();
+  // per digit: exclusive scan over warps; block totals -> dstart
+  uint32_t my_total = 0;
+  if (threadIdx.x < kRadix) {
+    const int d = threadIdx.x;
+    uint32_t run = 0;
+#pragma unroll
+    for (int w = 0; w < kSortWarps; ++w) { const uint32_t c = whist[w][d]; whist[w][d] = run; run += c; }
+    my_total = run;
+  }
+  {  // exclusive scan of the 256 digit totals (kSortThreads == kRadix)
+    __shared__ uint32_t wsum[kSortWarps];
+    uint32_t incl = my_total;
+#pragma unroll
+    for (int dlt = 1; dlt < 32; dlt <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, incl, dlt); if (lane >= dlt) incl += y; }
+    if (lane == 31) wsum[wid] = incl;
+    __syncthreads();
+    uint32_t before = 0;
+#pragma unroll
+    for (int w = 0; w < kSortWarps; ++w) if (w < wid) before += wsum[w];
+    dstart[threadIdx.x] = before + incl - my_total;
+  }
+  __syncthreads();
+  // reorder in shared memory so that each digit's keys are contiguous and in stable order
+#pragma unroll
+  for (int j = 0; j < kSortItems; ++j) {
+    const uint64_t idx = wbase + (uint64_t)j * 32 + lane;
+    if (idx < n) {
+      const uint32_t d = digit_of(key[j], shift);
+      const uint32_t pos = dstart[d] + whist[wid][d] + rank[j];
+      skeys[pos] = key[j]; svals[pos] = val[j];
+    }
+  }
+  __syncthreads();
+  const uint64_t tile_base = (uint64_t)blockIdx.x * kSortTile;
+  const uint32_t cnt = (uint32_t)((n - tile_base) < (uint64_t)kSortTile ? (n - tile_base) : (uint64_t)kSortTile);
+#pragma unroll 4
+  for (int j = 0; j < kSortItems; ++j) {
+    const uint32_t pos = j * kSortThreads + threadIdx.x;
+    if (pos < cnt) {
+      const uint64_t kk = skeys[pos];
+      const uint32_t d = digit_of(kk, shift);
+      const uint64_t dst = gbase[d] + (pos - dstart[d]);
+      keys_out[dst] = kk; vals_out[dst] = svals[pos];
+    }
+  }
+}
+
+__global__ void copy_pairs(const uint64_t* __restrict__ ki, const uint32_t* __restrict__ vi, uint64_t* __restrict__ ko,
+                           uint32_t* __restrict__ vo, uint64_t n) {
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+    ko[i] = ki[i]; vo[i] = vi[i];
+  }
+}
+
+// F4.  One thread per pair: a pair that differs from its predecessor in the (view,tile) field opens a range, one that
+// differs from its successor closes it.  `ranges` is zeroed first so that empty tiles read (0,0).
+__global__ void __launch_bounds__(256)
+tile_ranges_kernel(const uint64_t* __restrict__ keys, uint64_t n, uint64_t* __restrict__ ranges) {
+  const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n) return;
+  const uint32_t id = (uint32_t)(__ldg(keys + j) >> 32);
+  const uint32_t prev = j > 0 ? (uint32_t)(__ldg(keys + j - 1) >> 32) : ~id;
+  const uint32_t next = j + 1 < n ? (uint32_t)(__ldg(keys + j + 1) >> 32) : ~id;
+  if (prev != id) ranges[2 * (uint64_t)id] = j;
+  if (next != id) ranges[2 * (uint64_t)id + 1] = j + 1;
+}
+
+static int tile_bits_of(const uts_config* cfg) {
+  const uint64_t ids = ((uint64_t)12 << (2 * (cfg->order - cfg->tile_log2))) * (uint64_t)cfg->n_views;
+  int b = 0;
+  while (((uint64_t)1 << b) < ids) ++b;
+  return b;
+}
+
+}  // namespace uts
+
+using namespace uts;
+
+extern "C" {
+
+size_t uts_sort_scratch_bytes(uint64_t n_pairs) {
+  const uint64_t nb = (n_pairs + kSortTile - 1) / kSortTile;
+  const uint64_t m = nb * kRadix;                     // histogram entries
+  return (size_t)(((m * 4 + 255) / 256) * 256 + ((m + 1) * 8 + 255) / 256 * 256) + scan_scratch_bytes((int64_t)m);
+}
+
+int uts_sort(const uts_config* cfg, uint64_t n_pairs, uint64_t* keys, uint32_t* vals, uint64_t* keys_tmp, uint32_t* vals_tmp,
+             void* scratch, size_t scratch_bytes, void* stream) {
+  int st = check_config(cfg);
+  if (st) return st;
+  if (n_pairs == 0) return UTS_OK;
+  if (!keys || !vals || !keys_tmp || !vals_tmp || !scratch) return UTS_ERR_INVALID_ARG;
+  if (scratch_bytes < uts_sort_scratch_bytes(n_pairs) || ((uintptr_t)scratch & 255)) return UTS_ERR_INVALID_ARG;
+  if (n_pairs > ((uint64_t)1 << 40)) return UTS_ERR_UNSUPPORTED;
+  cudaStream_t s = (cudaStream_t)stream;
+  const uint32_t nb = (uint32_t)((n_pairs + kSortTile - 1) / kSortTile);
+  const uint64_t m = (uint64_t)nb * kRadix;
+  char* sp = reinterpret_cast<char*>(scratch);
+  uint32_t* counts = reinterpret_cast<uint32_t*>(sp);            sp += ((m * 4 + 255) / 256) * 256;
+  uint64_t* offs = reinterpret_cast<uint64_t*>(sp);              sp += (((m + 1) * 8 + 255) / 256) * 256;
+  uint64_t* block_sums = reinterpret_cast<uint64_t*>(sp);
+  const int n_pass = 4 + (tile_bits_of(cfg) + 7) / 8;
+  uint64_t* kin = keys; uint32_t* vin = vals; uint64_t* kout = keys_tmp; uint32_t* vout = vals_tmp;
+  for (int pass = 0; pass < n_pass; ++pass) {
+    const int shift = 8 * pass;
+    sort_upsweep<<<nb, kSortThreads, 0, s>>>(kin, n_pairs, shift, nb, counts);
+    UTS_LAUNCH_CHECK();
+    if ((st = exclusive_scan_u32(counts, (int64_t)m, offs, block_sums, s))) return st;
+    sort_downsweep<<<nb, kSortThreads, 0, s>>>(kin, vin, kout, vout, n_pairs, shift, nb, offs);
+    UTS_LAUNCH_CHECK();
+    uint64_t* tk = kin; kin = kout; kout = tk;
+    uint32_t* tv = vin; vin = vout; vout = tv;
+  }
+  if (kin != keys) {
+    copy_pairs<<<sm_count() * 8, 256, 0, s>>>(kin, vin, keys, vals, n_pairs);
+    UTS_LAUNCH_CHECK();
+  }
+  return UTS_OK;
+}
+
+int uts_tile_ranges(const uts_config* cfg, uint64_t n_pairs, const uint64_t* keys, uint64_t* ranges, void* stream) {
+  int st = check_config(cfg);
+  if (st) return st;
+  if (!ranges || (n_pairs && !keys)) return UTS_ERR_INVALID_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  const uint64_t ids = ((uint64_t)12 << (2 * (cfg->order - cfg->tile_log2))) * (uint64_t)cfg->n_views;
+  UTS_CUDA(cudaMemsetAsync(ranges, 0, ids * 2 * sizeof(uint64_t), s));
+  if (n_pairs == 0) return UTS_OK;
+  tile_ranges_kernel<<<(unsigned)((n_pairs + 255) / 256), 256, 0, s>>>(keys, n_pairs, ranges);
+  UTS_LAUNCH_CHECK();
+  return UTS_OK;
+}
+
+}  // extern "C"

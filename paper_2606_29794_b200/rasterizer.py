@@ -1,0 +1,105 @@
+"""Buffer management around the seven ABI calls: allocates the caller-owned buffers with torch and runs the stages in
+Alg.1's order and the backward.  No arithmetic of the method lives here."""
+from __future__ import annotations
+
+import torch
+
+from . import binding as B
+
+
+def _i64(n, dev): return torch.empty(n, dtype=torch.int64, device=dev)
+def _i32(n, dev): return torch.empty(n, dtype=torch.int32, device=dev)
+def _f32(*s, dev): return torch.empty(*s, dtype=torch.float32, device=dev)
+def _bytes(n, dev): return torch.empty((n + 255) // 256 * 32, dtype=torch.int64, device=dev)   # 256-byte granular, 256-aligned by the allocator
+
+
+class Rasterizer:
+    """Holds every buffer of one configuration.  forward() / backward() enqueue on torch's current stream; the only host
+    synchronisation is the pair count returned by uts_tile_query."""
+
+    def __init__(self, cfg: B.Config, mask: B.Mask | None = None, device="cuda", pair_capacity: int = 0):
+        B.lib()
+        if not torch.cuda.is_available():
+            raise RuntimeError("uts: a CUDA device is required (no CPU fallback)")
+        self.cfg, self.mask, self.dev = cfg, (mask or B.Mask.full()), device
+        V, P = cfg.n_views, cfg.n_gauss
+        self.S = self.mask.n_slots(cfg)
+        npx = self.S * cfg.ppt
+        self.proj = B.Proj.empty(cfg, device)
+        self.offsets = _i64(V * P + 1, device)
+        self.tq_scratch = _bytes(B.uts_tile_query_scratch_bytes(cfg), device)
+        self.ranges = _i64(V * cfg.n_tiles * 2, device).view(V * cfg.n_tiles, 2)
+        self.color = _f32(V, npx, 3, dev=device); self.alpha = _f32(V, npx, dev=device)
+        self.trans = _f32(V, npx, dev=device); self.n_last = _i32(V * npx, device).view(V, npx)
+        self.capacity = 0
+        self.n_pairs = 0
+        self._alloc_pairs(max(int(pair_capacity), 1024))
+        self.grads = None
+
+    def _alloc_pairs(self, cap):
+        self.keys = self.vals = self.keys_tmp = self.vals_tmp = self.sort_scratch = None
+        self.capacity = int(cap)
+        d = self.dev
+        self.keys, self.keys_tmp = _i64(cap, d), _i64(cap, d)
+        self.vals, self.vals_tmp = _i32(cap, d), _i32(cap, d)
+        self.sort_scratch = _bytes(B.uts_sort_scratch_bytes(cap), d)
+
+    # ---- stages (each is one ABI call) -------------------------------------------------------------
+    def preprocess(self, g, views): B.uts_preprocess(self.cfg, g, views, self.proj)
+
+    def tile_query(self):
+        try:
+            self.n_pairs = B.uts_tile_query(self.cfg, self.proj, self.mask, self.offsets, self.keys, self.vals, self.capacity, self.tq_scratch)
+        except B.UtsError as e:
+            if e.status != B.UTS_ERR_CAPACITY:
+                raise
+            self._alloc_pairs(int(e.needed * 1.05) + 1024)
+            self.n_pairs = B.uts_tile_query(self.cfg, self.proj, self.mask, self.offsets, self.keys, self.vals, self.capacity, self.tq_scratch)
+        return self.n_pairs
+
+    def sort(self): B.uts_sort(self.cfg, self.n_pairs, self.keys, self.vals, self.keys_tmp, self.vals_tmp, self.sort_scratch)
+    def tile_ranges(self): B.uts_tile_ranges(self.cfg, self.n_pairs, self.keys, self.ranges)
+
+    def render_fwd(self):
+        B.uts_render_fwd(self.cfg, self.proj, self.mask, self.ranges, self.vals, self.color, self.alpha, self.trans, self.n_last)
+
+    def _alloc_grads(self):
+        if self.grads is None:
+            V, P, M, d = self.cfg.n_views, self.cfg.n_gauss, self.cfg.n_sh, self.dev
+            self.grads = dict(rgb=_f32(V, P, 3, dev=d), conic=_f32(V, P, 3, dev=d), mu2=_f32(V, P, 2, dev=d), opac=_f32(P, dev=d),
+                              means=_f32(P, 3, dev=d), scales=_f32(P, 3, dev=d), quats=_f32(P, 4, dev=d), sh=_f32(P, M, 3, dev=d))
+        return self.grads
+
+    def render_bwd(self, dL_dcolor, dL_dalpha=None):
+        G = self._alloc_grads()
+        B.uts_render_bwd(self.cfg, self.proj, self.mask, self.ranges, self.vals, self.trans, self.n_last, dL_dcolor, dL_dalpha,
+                         G["rgb"], G["conic"], G["mu2"], G["opac"])
+
+    def preprocess_bwd(self, g, views):
+        G = self._alloc_grads()
+        B.uts_preprocess_bwd(self.cfg, g, views, self.proj.flags, G["rgb"], G["conic"], G["mu2"], G["means"], G["scales"], G["quats"], G["sh"])
+
+    # ---- whole path --------------------------------------------------------------------------------
+    def forward(self, g, views):
+        self.preprocess(g, views)
+        self.tile_query()
+        self.sort()
+        self.tile_ranges()
+        self.render_fwd()
+        return self.color, self.alpha
+
+    def backward(self, g, views, dL_dcolor, dL_dalpha=None):
+        self.render_bwd(dL_dcolor, dL_dalpha)
+        self.preprocess_bwd(g, views)
+        return self.grads
+
+
+def scene_to_device(scene, device="cuda"):
+    """numpy scene dict (scenes.make_scene) -> (Gaussians, Views) on the device."""
+    t = lambda a: torch.from_numpy(a).to(device).contiguous()
+    return (B.Gaussians(t(scene["means"]), t(scene["scales"]), t(scene["quats"]), t(scene["opac"]), t(scene["sh"])),
+            B.Views(t(scene["W"]), t(scene["b"])))
+
+
+def config_of(scene, **kw) -> B.Config:
+    return B.Config(order=scene["order"], n_gauss=scene["n_gauss"], n_views=scene["n_views"], sh_degree=scene["sh_degree"], **kw)

@@ -1,0 +1,466 @@
+"""GPU parity: every stage of the CUDA path (through the C ABI) against the oracle, element by element, on the same
+seeded inputs.  Stage-wise protocol: GPU stage n runs on the ORACLE's output of stage n-1,
+so integer stages must be bit-identical and float stages agree within the stated tolerances; the all-GPU chain is then
+compared with the all-oracle chain.  Shrunk versions of the five BASELINE.json configs: several tiles, ragged lists,
+masks, multiple views, SH degree 0 and 3.
+
+Tolerances (BASELINE.json north_star): tile lists / sorted order / ranges bit-exact; colour and alpha 1e-4 absolute;
+gradients 1e-3 relative (measured against the largest magnitude of each output array, reading A25)."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+import oracle as orc
+from helpers import ocfg, oracle_mask, small_scene
+
+pytestmark = pytest.mark.gpu
+
+MARGIN = 2e-3      # pixels whose nearest alpha/T decision is closer than this (relative) may legitimately flip in fp32
+
+
+def _gpu():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2606_29794_b200 import binding as B, rasterizer as R
+    return B, R
+
+
+def dev(a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    if dtype is not None:
+        t = t.view(dtype) if t.element_size() == torch.empty(0, dtype=dtype).element_size() else t.to(dtype)
+    return t.cuda().contiguous()
+
+
+def u64(t): return t.cpu().numpy().view(np.uint64)
+def u32(t): return t.cpu().numpy().view(np.uint32)
+
+
+# shrunk configs: (cfg_id, n_gauss, order, extra)
+CASES = [
+    pytest.param(1, 1000, 6, {}, id="cfg1-tiny-full"),
+    pytest.param(2, 12000, 7, {}, id="cfg2-panorama-sh3"),
+    pytest.param(3, 12000, 7, {}, id="cfg3-fisheye-cap-mask"),
+    pytest.param(4, 3000, 7, {}, id="cfg4-large-outliers"),
+    pytest.param(5, 8000, 8, {"n_views": 2}, id="cfg5-frustum-2views"),
+    pytest.param(4, 30000, 5, {}, id="cfg4-dense-long-lists-early-exit"),     # lists up to ~1500 entries (6 batches), 40 % of pixels saturate
+]
+
+
+class Case:
+    """Oracle results for one shrunk config, computed once per test session."""
+    _cache = {}
+
+    def __init__(self, cfg_id, P, order, extra):
+        self.scene = small_scene(cfg_id, P, order, **extra)
+        self.ocfg = ocfg(self.scene)
+        self.bits, self.act, self.slot = oracle_mask(self.ocfg, self.scene)
+        self.fw = orc.forward_chain(self.ocfg, self.scene, self.slot, self.act, self.bits)
+        assert self.fw["qinfo"]["min_margin"] > 1e-12, "margin certificate failed: change the seed"
+
+    @classmethod
+    def get(cls, cfg_id, P, order, extra):
+        key = (cfg_id, P, order, tuple(sorted(extra.items())))
+        if key not in cls._cache:
+            cls._cache[key] = Case(cfg_id, P, order, extra)
+        return cls._cache[key]
+
+    def gpu_mask(self, B):
+        if self.bits is None:
+            return B.Mask.full()
+        return B.Mask(dev(self.act.view(np.int32)), int(self.act.shape[0]), dev(self.slot), dev(self.bits.view(np.int32)))
+
+    def gpu_proj(self, B):
+        p = self.fw["proj"]
+        return B.Proj(dev(p.dir), dev(p.lonlat), dev(p.rho), dev(p.conic_opac), dev(p.rs), dev(p.rgb), dev(p.flags))
+
+
+def _cfg(R, scene, **kw):
+    return R.config_of(scene, **kw)
+
+
+# ------------------------------------------------------------------------------------------- HEALPix
+def test_pixel_centers_match_oracle():
+    B, _ = _gpu()
+    for order in range(0, 9):
+        n = 12 << (2 * order)
+        got = B.uts_pixel_centers(order, 0, n).cpu().numpy()
+        _, _, want = orc.centers(order, which=2)
+        assert np.abs(got - want).max() < 5e-15
+    # a slice at the maximum supported order
+    first = (12 << 26) - 1000
+    got = B.uts_pixel_centers(13, first, 1000).cpu().numpy()
+    _, _, want = orc.centers(13, which=2, first=first, n=1000)
+    assert np.abs(got - want).max() < 5e-15
+
+
+def test_mask_builder_matches_oracle_mask():
+    B, R = _gpu()
+    for cfg_id, order in ((3, 7), (5, 8)):
+        scene = small_scene(cfg_id, 10, order)
+        oc = ocfg(scene)
+        bits, act, slot = oracle_mask(oc, scene)
+        m = B.uts_build_mask(_cfg(R, scene), scene["mask"]["kind"], scene["mask"]["params"])
+        gb = u32(m.pixel_mask_bits)
+        # the predicate is evaluated in double on both sides; allow a handful of boundary pixels to differ
+        diff = np.unpackbits((gb ^ bits).view(np.uint8)).sum()
+        assert diff <= 4
+        if diff == 0:
+            assert m.n_active == act.shape[0]
+            assert np.array_equal(u32(m.active_tiles), act)
+            assert np.array_equal(m.slot_of_tile.cpu().numpy(), slot)
+
+
+# ------------------------------------------------------------------------------------------- F1
+@pytest.mark.parametrize("cfg_id,P,order,extra", CASES)
+def test_preprocess(cfg_id, P, order, extra):
+    B, R = _gpu()
+    c = Case.get(cfg_id, P, order, extra)
+    cfg = _cfg(R, c.scene)
+    g, views = R.scene_to_device(c.scene)
+    out = B.Proj.empty(cfg)
+    B.uts_preprocess(cfg, g, views, out)
+    want = c.fw["proj"]
+    assert np.array_equal(out.flags.cpu().numpy(), want.flags)
+    for name, rtol in (("dir", 0), ("rho", 0), ("rs", 0), ("lonlat", 1e-6), ("conic_opac", 1e-6), ("rgb", 1e-5)):
+        a = getattr(out, name).cpu().numpy().astype(np.float64); b = getattr(want, name).astype(np.float64)
+        if rtol == 0:
+            # geometry is computed in double and rounded once: identical fp32 bits except where the double results straddle a
+            # rounding boundary (allow 1 ulp on < 0.01 % of the values)
+            neq = a != b
+            assert neq.mean() < 1e-4, (name, neq.mean())
+            assert np.all(np.abs(a - b)[neq] <= np.abs(b[neq]) * 1.3e-7), name
+        else:
+            assert np.allclose(a, b, rtol=rtol, atol=rtol), (name, np.abs(a - b).max())
+
+
+def test_preprocess_culls_and_degree_variants():
+    B, R = _gpu()
+    for deg in (0, 1, 2, 3):
+        scene = small_scene(2, 500, 6, sh_degree=deg)
+        scene["means"][:5] *= 1e-3            # rho <= r_near  -> culled
+        scene["means"][5] = np.nan            # non-finite     -> culled
+        scene["scales"][6] = 0.0              # with dilation still positive definite -> kept
+        oc = ocfg(scene)
+        want = orc.preprocess(oc, scene["means"], scene["scales"], scene["quats"], scene["opac"], scene["sh"], scene["W"], scene["b"])
+        cfg = _cfg(R, scene)
+        g, views = R.scene_to_device(scene)
+        out = B.Proj.empty(cfg)
+        B.uts_preprocess(cfg, g, views, out)
+        assert np.array_equal(out.flags.cpu().numpy(), want.flags)
+        assert (want.flags[0, :6] & 1).all()
+        assert np.allclose(out.rgb.cpu().numpy(), want.rgb, atol=1e-5)
+        assert np.allclose(out.conic_opac.cpu().numpy(), want.conic_opac, rtol=1e-6, atol=1e-6)
+
+
+# ------------------------------------------------------------------------------------------- F2
+@pytest.mark.parametrize("cfg_id,P,order,extra", CASES)
+def test_tile_query_bit_exact(cfg_id, P, order, extra):
+    B, R = _gpu()
+    c = Case.get(cfg_id, P, order, extra)
+    cfg = _cfg(R, c.scene)
+    proj, mask = c.gpu_proj(B), c.gpu_mask(B)
+    n_want = int(c.fw["keys"].shape[0])
+    offsets = torch.empty(cfg.n_views * cfg.n_gauss + 1, dtype=torch.int64, device="cuda")
+    scratch = torch.empty(B.uts_tile_query_scratch_bytes(cfg) // 8 + 32, dtype=torch.int64, device="cuda")
+    # count-only call
+    n = B.uts_tile_query(cfg, proj, mask, offsets, None, None, 0, scratch)
+    assert n == n_want
+    assert np.array_equal(u64(offsets), c.fw["offsets"])
+    # capacity too small -> error carrying the needed size
+    keys = torch.empty(max(n, 1), dtype=torch.int64, device="cuda"); vals = torch.empty(max(n, 1), dtype=torch.int32, device="cuda")
+    if n > 1:
+        with pytest.raises(B.UtsError) as ei:
+            B.uts_tile_query(cfg, proj, mask, offsets, keys, vals, n - 1, scratch)
+        assert ei.value.status == B.UTS_ERR_CAPACITY and ei.value.needed == n
+    n = B.uts_tile_query(cfg, proj, mask, offsets, keys, vals, n, scratch)
+    assert np.array_equal(u64(keys)[:n], c.fw["keys"])
+    assert np.array_equal(u32(vals)[:n], c.fw["vals"])
+
+
+@pytest.mark.parametrize("refine", [0, 1, 3, 4])
+def test_tile_query_other_refinements(refine):
+    B, R = _gpu()
+    scene = small_scene(4, 800, 6)
+    oc = ocfg(scene, query_refine_log2=refine)
+    pr = orc.preprocess(oc, scene["means"], scene["scales"], scene["quats"], scene["opac"], scene["sh"], scene["W"], scene["b"])
+    off, keys, vals, info = orc.tile_query(oc, pr)
+    assert info["min_margin"] > 1e-12
+    cfg = _cfg(R, scene, query_refine_log2=refine)
+    proj = B.Proj(dev(pr.dir), dev(pr.lonlat), dev(pr.rho), dev(pr.conic_opac), dev(pr.rs), dev(pr.rgb), dev(pr.flags))
+    r = R.Rasterizer(cfg, pair_capacity=16)       # forces the capacity-retry path
+    r.proj = proj
+    n = r.tile_query()
+    assert n == keys.shape[0]
+    assert np.array_equal(u64(r.offsets), off)
+    assert np.array_equal(u64(r.keys)[:n], keys) and np.array_equal(u32(r.vals)[:n], vals)
+
+
+def test_tile_query_whole_sphere_and_empty():
+    B, R = _gpu()
+    scene = small_scene(1, 4, 6)
+    scene["scales"][0] = 50.0                      # r_s clamps to pi: every tile (reading A24)
+    scene["means"][1] *= 1e-4                      # culled: zero tiles
+    oc = ocfg(scene)
+    pr = orc.preprocess(oc, scene["means"], scene["scales"], scene["quats"], scene["opac"], scene["sh"], scene["W"], scene["b"])
+    off, keys, vals, _ = orc.tile_query(oc, pr)
+    assert off[1] - off[0] == oc.n_tiles and off[2] == off[1]
+    cfg = _cfg(R, scene)
+    r = R.Rasterizer(cfg)
+    r.proj = B.Proj(dev(pr.dir), dev(pr.lonlat), dev(pr.rho), dev(pr.conic_opac), dev(pr.rs), dev(pr.rgb), dev(pr.flags))
+    n = r.tile_query()
+    assert np.array_equal(u64(r.offsets), off) and np.array_equal(u64(r.keys)[:n], keys) and np.array_equal(u32(r.vals)[:n], vals)
+    # P = 0
+    cfg0 = B.Config(order=6, n_gauss=0)
+    r0 = R.Rasterizer(cfg0)
+    assert r0.tile_query() == 0
+
+
+# ------------------------------------------------------------------------------------------- F3 / F4
+@pytest.mark.parametrize("cfg_id,P,order,extra", CASES)
+def test_sort_and_ranges_bit_exact(cfg_id, P, order, extra):
+    B, R = _gpu()
+    c = Case.get(cfg_id, P, order, extra)
+    cfg = _cfg(R, c.scene)
+    n = int(c.fw["keys"].shape[0])
+    keys = dev(c.fw["keys"].view(np.int64)); vals = dev(c.fw["vals"].view(np.int32))
+    kt = torch.empty_like(keys); vt = torch.empty_like(vals)
+    scratch = torch.empty(B.uts_sort_scratch_bytes(n) // 8 + 32, dtype=torch.int64, device="cuda")
+    B.uts_sort(cfg, n, keys, vals, kt, vt, scratch)
+    assert np.array_equal(u64(keys), c.fw["skeys"])
+    assert np.array_equal(u32(vals), c.fw["svals"])           # ties broken by Gaussian id (stability)
+    ranges = torch.empty(cfg.n_views * cfg.n_tiles, 2, dtype=torch.int64, device="cuda")
+    B.uts_tile_ranges(cfg, n, keys, ranges)
+    assert np.array_equal(u64(ranges), c.fw["ranges"])
+
+
+@pytest.mark.parametrize("n", [0, 1, 2, 255, 3071, 3072, 3073, 50_000, 1_000_003])
+def test_sort_sizes_and_ties(n):
+    """Ragged sizes around the 3072-pair block and heavy ties: values record the input position, so stability is visible."""
+    B, R = _gpu()
+    cfg = B.Config(order=10, n_gauss=1, n_views=4)           # 18 tile bits -> 7 passes
+    rng = np.random.default_rng(n)
+    tile = rng.integers(0, 4 * cfg.n_tiles, n, dtype=np.uint64)
+    depth = rng.integers(0, 7, n, dtype=np.uint64) * np.uint64(0x01010101) if n % 2 else rng.integers(0, 1 << 32, n, dtype=np.uint64)
+    keys_h = (tile << np.uint64(32)) | depth
+    vals_h = np.arange(n, dtype=np.uint32)
+    wk, wv = orc.sort_pairs(keys_h, vals_h)
+    keys = dev(keys_h.view(np.int64)) if n else torch.empty(0, dtype=torch.int64, device="cuda")
+    vals = dev(vals_h.view(np.int32)) if n else torch.empty(0, dtype=torch.int32, device="cuda")
+    kt = torch.empty_like(keys); vt = torch.empty_like(vals)
+    scratch = torch.empty(B.uts_sort_scratch_bytes(max(n, 1)) // 8 + 32, dtype=torch.int64, device="cuda")
+    B.uts_sort(cfg, n, keys, vals, kt, vt, scratch)
+    assert np.array_equal(u64(keys), wk) and np.array_equal(u32(vals), wv)
+    ranges = torch.empty(cfg.n_views * cfg.n_tiles, 2, dtype=torch.int64, device="cuda")
+    B.uts_tile_ranges(cfg, n, keys, ranges)
+    assert np.array_equal(u64(ranges), orc.tile_ranges(orc.Config(order=10, n_gauss=1, n_views=4), wk))
+
+
+# ------------------------------------------------------------------------------------------- F5 / F6
+def _render_gpu(B, R, c, cfg):
+    mask = c.gpu_mask(B)
+    r = R.Rasterizer(cfg, mask)
+    r.proj = c.gpu_proj(B)
+    r.ranges = dev(c.fw["ranges"].view(np.int64))
+    r.vals = dev(c.fw["svals"].view(np.int32))
+    r.render_fwd()
+    return r
+
+
+def _compare_image(c, color, alpha, n_last):
+    want_c, want_a, want_n, margin = c.fw["color"], c.fw["alpha"], c.fw["n_last"], c.fw["margin"]
+    safe = margin > MARGIN
+    assert safe.mean() > 0.9
+    dc = np.abs(color.astype(np.float64) - want_c).max(axis=-1)
+    da = np.abs(alpha.astype(np.float64) - want_a)
+    assert dc[safe].max() <= 1e-4, dc[safe].max()
+    assert da[safe].max() <= 1e-4, da[safe].max()
+    assert np.array_equal(n_last[safe], want_n[safe])
+    # a flipped borderline decision changes a pixel by at most about alpha_min (or the clamp step)
+    assert dc.max() < 2e-2 and da.max() < 2e-2
+
+
+@pytest.mark.parametrize("cfg_id,P,order,extra", CASES)
+def test_render_fwd(cfg_id, P, order, extra):
+    B, R = _gpu()
+    c = Case.get(cfg_id, P, order, extra)
+    r = _render_gpu(B, R, c, _cfg(R, c.scene))
+    color, alpha = r.color.cpu().numpy(), r.alpha.cpu().numpy()
+    _compare_image(c, color, alpha, u32(r.n_last))
+    assert np.allclose(r.trans.cpu().numpy() + alpha, 1.0, atol=1e-6)
+    if c.bits is not None:       # masked-out pixels of active tiles are exactly zero
+        ppt = c.ocfg.ppt
+        pix = (c.act.astype(np.int64)[:, None] * ppt + np.arange(ppt)[None, :]).reshape(-1)
+        on = ((c.bits[pix >> 5] >> (pix & 31).astype(np.uint32)) & 1).astype(bool)
+        assert (color[:, ~on] == 0).all() and (alpha[:, ~on] == 0).all()
+
+
+def test_render_fwd_background_and_no_thresholds():
+    """bg != 0; alpha rules disabled (alpha_min 0, alpha_max 1, eps 0): no decision can flip, every pixel must agree."""
+    B, R = _gpu()
+    scene = small_scene(1, 1000, 6)
+    kw = dict(alpha_min=0.0, alpha_max=1.0, t_eps=0.0, bg=(0.25, 0.5, 0.75))
+    oc = ocfg(scene, **kw)
+    fw = orc.forward_chain(oc, scene)
+    cfg = _cfg(R, scene, **kw)
+    r = R.Rasterizer(cfg)
+    p = fw["proj"]
+    r.proj = B.Proj(dev(p.dir), dev(p.lonlat), dev(p.rho), dev(p.conic_opac), dev(p.rs), dev(p.rgb), dev(p.flags))
+    r.ranges = dev(fw["ranges"].view(np.int64)); r.vals = dev(fw["svals"].view(np.int32))
+    r.render_fwd()
+    assert np.abs(r.color.cpu().numpy() - fw["color"]).max() <= 1e-4
+    assert np.abs(r.alpha.cpu().numpy() - fw["alpha"]).max() <= 1e-4
+
+
+# ------------------------------------------------------------------------------------------- B1 / B2
+def _rel_err(got, want):
+    scale = max(np.abs(want).max(), 1e-30)
+    return np.abs(got.astype(np.float64) - want).max() / scale
+
+
+def _zero_unsafe(c, gcol, galpha=None):
+    """A pixel whose forward decisions sit within MARGIN of a threshold may legitimately take the other branch in fp32, which
+    changes its gradient contributions by a finite step; such pixels get zero upstream gradient on BOTH sides, so the
+    comparison below measures arithmetic, not branch flips.  (The thresholds-off test further down covers every pixel.)"""
+    unsafe = ~(c.fw["margin"] > MARGIN)
+    gcol = gcol.copy(); gcol[unsafe] = 0
+    if galpha is not None:
+        galpha = galpha.copy(); galpha[unsafe] = 0
+    return gcol, galpha
+
+
+@pytest.mark.parametrize("cfg_id,P,order,extra", CASES)
+def test_backward(cfg_id, P, order, extra):
+    B, R = _gpu()
+    c = Case.get(cfg_id, P, order, extra)
+    cfg = _cfg(R, c.scene)
+    r = _render_gpu(B, R, c, cfg)
+    V, npx = r.color.shape[0], r.color.shape[1]
+    from paper_2606_29794_b200 import scenes
+    gcol, galpha = _zero_unsafe(c, *scenes.upstream_grad(V, npx, seed=cfg_id, with_alpha=True))
+    # oracle backward on the oracle's own forward state
+    w_rgb, w_conic, w_mu2, w_opac = orc.render_bwd(c.ocfg, c.fw["proj"], c.fw["ranges"], c.fw["svals"], c.fw["n_last"], gcol, galpha,
+                                                   c.act, c.bits)
+    r.render_bwd(dev(gcol), dev(galpha))
+    G = r.grads
+    for name, want in (("rgb", w_rgb), ("conic", w_conic), ("mu2", w_mu2), ("opac", w_opac)):
+        e = _rel_err(G[name].cpu().numpy(), want)
+        assert e <= 1e-3, (name, e)
+    # B2 on the oracle's B1 output (stage-wise)
+    s = c.scene
+    w_means, w_scales, w_quats, w_sh = orc.preprocess_bwd(c.ocfg, s["means"], s["scales"], s["quats"], s["sh"], s["W"], s["b"],
+                                                          w_rgb, w_conic, w_mu2)
+    g, views = R.scene_to_device(s)
+    G["rgb"].copy_(dev(w_rgb.astype(np.float32))); G["conic"].copy_(dev(w_conic.astype(np.float32))); G["mu2"].copy_(dev(w_mu2.astype(np.float32)))
+    r.preprocess_bwd(g, views)
+    for name, want in (("means", w_means), ("scales", w_scales), ("quats", w_quats), ("sh", w_sh)):
+        e = _rel_err(G[name].cpu().numpy(), want)
+        assert e <= 1e-3, (name, e)
+
+
+@pytest.mark.parametrize("cfg_id,P,order", [(1, 1000, 6), (2, 12000, 7), (4, 30000, 5)])
+def test_backward_thresholds_off_every_pixel(cfg_id, P, order):
+    """alpha_min 0, alpha_max 1, eps 0: no decision exists, so every pixel takes part and the whole chain (forward on the GPU,
+    backward on the GPU) must match the oracle's within 1e-3 on every gradient array."""
+    B, R = _gpu()
+    scene = small_scene(cfg_id, P, order)
+    kw = dict(alpha_min=0.0, alpha_max=1.0, t_eps=0.0, bg=(0.1, 0.2, 0.3))
+    oc = ocfg(scene, **kw)
+    fw = orc.forward_chain(oc, scene)
+    cfg = _cfg(R, scene, **kw)
+    g, views = R.scene_to_device(scene)
+    r = R.Rasterizer(cfg)
+    r.forward(g, views)
+    assert np.array_equal(u64(r.keys)[: r.n_pairs], fw["skeys"])
+    assert np.abs(r.color.cpu().numpy() - fw["color"]).max() <= 1e-4
+    from paper_2606_29794_b200 import scenes
+    gcol, galpha = scenes.upstream_grad(1, r.color.shape[1], seed=7, with_alpha=True)
+    w_rgb, w_conic, w_mu2, w_opac = orc.render_bwd(oc, fw["proj"], fw["ranges"], fw["svals"], fw["n_last"], gcol, galpha)
+    w_means, w_scales, w_quats, w_sh = orc.preprocess_bwd(oc, scene["means"], scene["scales"], scene["quats"], scene["sh"], scene["W"],
+                                                          scene["b"], w_rgb, w_conic, w_mu2)
+    r.render_bwd(dev(gcol), dev(galpha))
+    r.preprocess_bwd(g, views)
+    G = r.grads
+    for name, want in (("rgb", w_rgb), ("conic", w_conic), ("mu2", w_mu2), ("opac", w_opac), ("means", w_means), ("scales", w_scales),
+                       ("quats", w_quats), ("sh", w_sh)):
+        e = _rel_err(G[name].cpu().numpy(), want)
+        assert e <= 1e-3, (name, e)
+
+
+# ------------------------------------------------------------------------------------------- whole chain
+@pytest.mark.parametrize("cfg_id,P,order,extra", CASES)
+def test_end_to_end_chain(cfg_id, P, order, extra):
+    """All-GPU chain against the all-oracle chain: pair lists, sorted order and ranges bit-exact (the GPU preprocess
+    rounds double results to fp32 once, as the oracle does), image within 1e-4, parameter gradients within 1e-3."""
+    B, R = _gpu()
+    c = Case.get(cfg_id, P, order, extra)
+    cfg = _cfg(R, c.scene)
+    if c.scene["mask"] is not None:
+        mask = B.uts_build_mask(cfg, c.scene["mask"]["kind"], c.scene["mask"]["params"])
+        if not np.array_equal(u32(mask.pixel_mask_bits), c.bits):
+            mask = c.gpu_mask(B)           # a boundary pixel differs: use the oracle's mask (the mask is an input of the path)
+    else:
+        mask = B.Mask.full()
+    g, views = R.scene_to_device(c.scene)
+    r = R.Rasterizer(cfg, mask)
+    r.forward(g, views)
+    n = r.n_pairs
+    # fp32 records straddling a rounding boundary could flip a borderline tile; require exact equality and report if not
+    assert n == c.fw["skeys"].shape[0]
+    assert np.array_equal(u64(r.keys)[:n], c.fw["skeys"])
+    assert np.array_equal(u32(r.vals)[:n], c.fw["svals"])
+    assert np.array_equal(u64(r.ranges), c.fw["ranges"])
+    _compare_image(c, r.color.cpu().numpy(), r.alpha.cpu().numpy(), u32(r.n_last))
+    from paper_2606_29794_b200 import scenes
+    V, npx = r.color.shape[0], r.color.shape[1]
+    gcol, _ = _zero_unsafe(c, scenes.upstream_grad(V, npx, seed=100 + cfg_id))
+    s = c.scene
+    w_rgb, w_conic, w_mu2, w_opac = orc.render_bwd(c.ocfg, c.fw["proj"], c.fw["ranges"], c.fw["svals"], c.fw["n_last"], gcol, None, c.act, c.bits)
+    w_means, w_scales, w_quats, w_sh = orc.preprocess_bwd(c.ocfg, s["means"], s["scales"], s["quats"], s["sh"], s["W"], s["b"], w_rgb, w_conic, w_mu2)
+    G = r.backward(g, views, dev(gcol))
+    for name, want in (("means", w_means), ("scales", w_scales), ("quats", w_quats), ("opac", w_opac), ("sh", w_sh)):
+        e = _rel_err(G[name].cpu().numpy(), want)
+        assert e <= 1e-3, (name, e)
+
+
+def test_host_call_matches_device_chain():
+    """uts_host_forward_backward (host buffers, copies inside) returns what the stage calls return."""
+    B, R = _gpu()
+    scene = small_scene(2, 5000, 7)
+    cfg = _cfg(R, scene)
+    g, views = R.scene_to_device(scene)
+    r = R.Rasterizer(cfg)
+    r.forward(g, views)
+    from paper_2606_29794_b200 import scenes
+    gcol = scenes.upstream_grad(1, r.color.shape[1], seed=5)
+    G = r.backward(g, views, dev(gcol))
+    h = {k: torch.from_numpy(scene[k]).contiguous() for k in ("means", "scales", "quats", "opac", "sh", "W", "b")}
+    P, M = cfg.n_gauss, cfg.n_sh
+    out = dict(color=torch.empty(1, r.color.shape[1], 3), alpha=torch.empty(1, r.color.shape[1]), dL_dmeans=torch.empty(P, 3),
+               dL_dscales=torch.empty(P, 3), dL_dquats=torch.empty(P, 4), dL_dopac=torch.empty(P), dL_dsh=torch.empty(P, M, 3))
+    cap = r.n_pairs + 10
+    ws = torch.empty(B.uts_host_workspace_bytes(cfg, -1, cap) // 8 + 64, dtype=torch.int64, device="cuda")
+    with pytest.raises(B.UtsError):
+        B.uts_host_forward_backward(cfg, h, B.Mask.full(), torch.from_numpy(gcol), out, 7, ws)      # capacity too small
+    n = B.uts_host_forward_backward(cfg, h, B.Mask.full(), torch.from_numpy(gcol), out, cap, ws)
+    assert n == r.n_pairs
+    assert torch.equal(out["color"], r.color.cpu()) and torch.equal(out["alpha"], r.alpha.cpu())
+    for name in ("means", "scales", "quats", "opac", "sh"):
+        a, b = out["dL_d" + name].numpy(), G[name].cpu().numpy()
+        assert np.abs(a - b).max() <= 1e-4 * max(np.abs(b).max(), 1e-30)      # atomics: summation order differs run to run
+
+
+def test_invalid_arguments_are_reported():
+    B, R = _gpu()
+    bad = B.Config(order=3, n_gauss=10)              # order < tile_log2
+    with pytest.raises(B.UtsError) as ei:
+        B.uts_preprocess(bad, B.Gaussians(*[torch.zeros(40, device="cuda")] * 5), B.Views(torch.zeros(9, device="cuda"), torch.zeros(3, device="cuda")),
+                         B.Proj.empty(B.Config(order=6, n_gauss=10)))
+    assert ei.value.status == B.UTS_ERR_INVALID_ARG
+    with pytest.raises(B.UtsError) as ei:
+        B.uts_sort(B.Config(order=6, n_gauss=1, tile_log2=3), 4, *[torch.zeros(8, dtype=torch.int64, device="cuda"), torch.zeros(8, dtype=torch.int32, device="cuda")] * 2,
+                   torch.zeros(4096, dtype=torch.int64, device="cuda"))
+    assert ei.value.status == B.UTS_ERR_UNSUPPORTED
+    with pytest.raises(RuntimeError):
+        B.uts_tile_ranges(B.Config(order=6, n_gauss=1), 1, torch.zeros(1, dtype=torch.int64), torch.zeros(4, dtype=torch.int64, device="cuda"))

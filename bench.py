@@ -1,0 +1,341 @@
+#!/usr/bin/env python
+"""bench.py — HEALPix forward+backward rasterisation throughput on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (preprocess -> tile query -> sort -> ranges -> blend forward -> blend
+backward -> preprocess backward) over one seeded synthetic scene.  Default workload: BASELINE.json config 4
+("large_sphere": Nside 1024, 12.58 M px, 2 M Gaussians, SH degree 3), the configuration the metric is quoted on.
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2606_29794_b200 import scenes  # noqa: E402  (input generator: no method arithmetic)
+
+METRIC = "healpix_px_per_s_fwd_bwd"
+UNIT = "px/s"
+STAGES = ["preprocess", "tile_query", "sort", "tile_ranges", "render_fwd", "render_bwd", "preprocess_bwd"]
+# FP32 operations one evaluated (Gaussian, pixel) pair costs in the blend kernels (counted from the
+# arithmetic of Eq.6 + SphericalOffset as implemented, FMA = 2): forward 46, backward 118.
+FLOP_FWD, FLOP_BWD = 46, 118
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self._stop_evt = index, [], threading.Event()
+
+    def run(self):
+        while not self._stop_evt.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([c.strip() for c in out.split(",")])
+            except Exception:
+                pass
+            self._stop_evt.wait(0.1)
+
+    def stop(self):
+        self._stop_evt.set(); self.join(timeout=6)
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 7 for i in range(4) if r[3 + i].lower().startswith("active")})
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None, reasons=reasons, samples=len(sm))
+
+
+# ----------------------------------------------------------------------------------------------- reference arm
+def oracle_sample(cfg_id, seed=0, n_pre=100_000, n_query=10_000, n_tiles_sample=24):
+    """The oracle, as it stands, on a BOUNDED sample of the workload; returns (estimated whole-frame seconds, description).
+
+    per-Gaussian stages (preprocess, preprocess backward) : first n_pre Gaussians, scaled by P/n_pre
+    tile query + sort + ranges                           : first n_query Gaussians on every tile, scaled by P/n_query
+    blend forward + backward                             : n_tiles_sample random tiles with their complete lists (all P
+                                                           Gaussians pre-filtered by a conservative angular test, the oracle's
+                                                           own query decides), scaled by active tiles / sampled tiles
+    """
+    import oracle as orc
+    sc = scenes.make_scene(cfg_id, seed=seed)
+    P, V = sc["n_gauss"], sc["n_views"]
+    oc = orc.Config(order=sc["order"], n_gauss=P, n_views=V, sh_degree=sc["sh_degree"])
+    bits = act = slot = None
+    if sc["mask"] is not None:
+        bits = orc.mask_bits(oc.order, sc["mask"]["kind"], sc["mask"]["params"]); act, slot = orc.mask_tiles(oc, bits)
+    n_active = oc.n_tiles if act is None else int(act.shape[0])
+    n_pre, n_query = min(n_pre, P), min(n_query, P)
+    sub = lambda n: {k: (sc[k][:n] if k in ("means", "scales", "quats", "opac", "sh") else sc[k]) for k in sc}
+
+    # (1) per-Gaussian stages
+    s1 = sub(n_pre); c1 = orc.Config(order=oc.order, n_gauss=n_pre, n_views=V, sh_degree=oc.sh_degree)
+    t = time.perf_counter()
+    pr1 = orc.preprocess(c1, s1["means"], s1["scales"], s1["quats"], s1["opac"], s1["sh"], s1["W"], s1["b"])
+    z3 = np.zeros((V, n_pre, 3)); z2 = np.zeros((V, n_pre, 2))
+    orc.preprocess_bwd(c1, s1["means"], s1["scales"], s1["quats"], s1["sh"], s1["W"], s1["b"], z3 + 1.0, z3 + 1.0, z2 + 1.0)
+    t_pre = (time.perf_counter() - t) * (P / n_pre)
+
+    # (2) query + sort + ranges
+    s2 = sub(n_query); c2 = orc.Config(order=oc.order, n_gauss=n_query, n_views=V, sh_degree=oc.sh_degree)
+    pr2 = orc.preprocess(c2, s2["means"], s2["scales"], s2["quats"], s2["opac"], s2["sh"], s2["W"], s2["b"])
+    t = time.perf_counter()
+    _, keys, vals, _ = orc.tile_query(c2, pr2, slot)
+    sk, sv = orc.sort_pairs(keys, vals)
+    orc.tile_ranges(c2, sk)
+    t_qs = (time.perf_counter() - t) * (P / n_query)
+    pairs_est = keys.shape[0] * (P / n_query)
+
+    # (3) blend on sampled tiles with complete lists
+    pr = orc.preprocess(oc, sc["means"], sc["scales"], sc["quats"], sc["opac"], sc["sh"], sc["W"], sc["b"])
+    rng = np.random.default_rng(seed + 17)
+    pool = np.arange(oc.n_tiles) if act is None else act.astype(np.int64)
+    pick = np.sort(rng.choice(pool, min(n_tiles_sample, pool.shape[0]), replace=False))
+    sact = pick.astype(np.uint32)
+    sslot = np.full(oc.n_tiles, -1, np.int32); sslot[pick] = np.arange(pick.shape[0], dtype=np.int32)
+    _, _, tc = orc.centers(oc.tile_order, which=2)                           # tile centre directions
+    reach = pr.rs[..., None].astype(np.float64) + orc.rho_max_closed(oc.tile_order + oc.query_refine_log2) + orc.rho_max_closed(oc.tile_order) + 1e-6
+    cand = np.zeros(P, bool)
+    for v in range(V):
+        d = pr.dir[v].astype(np.float64) @ tc[pick].T                         # [P, n_sample]
+        cand |= (np.arccos(np.clip(d, -1, 1)) <= reach[v]).any(axis=1)
+    cand_ids = np.flatnonzero(cand).astype(np.int32)
+    _, keys, vals, _ = orc.tile_query(oc, pr, sslot, gauss_subset=cand_ids)
+    sk, sv = orc.sort_pairs(keys, vals)
+    rg = orc.tile_ranges(oc, sk)
+    npx = pick.shape[0] * oc.ppt
+    gcol = scenes.upstream_grad(V, npx, seed=seed)
+    t = time.perf_counter()
+    col, al, nl, _, ctr = orc.render_fwd(oc, pr, rg, sv, sact, bits)
+    t_f = time.perf_counter() - t
+    t = time.perf_counter()
+    orc.render_bwd(oc, pr, rg, sv, nl, gcol, None, sact, bits)
+    t_b = time.perf_counter() - t
+    scale = n_active / pick.shape[0]
+    total = t_pre + t_qs + (t_f + t_b) * scale
+    desc = (f"oracle (single thread, fp64) on a bounded sample of config {cfg_id}: preprocess+preprocess_bwd on {n_pre} of {P} Gaussians "
+            f"(x{P / n_pre:.0f}), query+sort+ranges on {n_query} Gaussians (x{P / n_query:.0f}, ~{pairs_est:.3g} pairs), blend fwd+bwd on "
+            f"{pick.shape[0]} of {n_active} tiles with complete lists ({sk.shape[0]} pairs, {ctr['evaluated']} evaluations; x{scale:.0f}); "
+            f"extrapolated whole-frame time {total:.1f} s = pre {t_pre:.1f} + query/sort {t_qs:.1f} + blend {(t_f + t_b) * scale:.1f}")
+    return total, desc, dict(n_pix=V * n_active * oc.ppt)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    sc_meta = scenes.CONFIGS[args.config]
+    times = []
+    desc = ""
+    for i in range(args.warmup + args.steps):
+        t, desc, meta = oracle_sample(args.config, seed=0, n_pre=50_000, n_query=5_000, n_tiles_sample=12)
+        if i >= args.warmup:
+            times.append(t)
+    t = float(np.mean(times))
+    val = meta["n_pix"] / t
+    line = dict(metric=METRIC, value=val, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup, ms_per_step=t * 1e3,
+                higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic", impl="reference",
+                config=dict(workload=f"config{args.config}:{sc_meta['name']}", order=sc_meta["order"], n_gauss=sc_meta["n_gauss"],
+                            sh_degree=sc_meta["sh_degree"], n_views=sc_meta["n_views"]),
+                cpu_baseline=dict(value=val, unit=UNIT, cores=1, kind="oracle", sample=desc),
+                e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(line))
+
+
+# ----------------------------------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_29794_b200 import binding as B, rasterizer as R
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    peaks = _peaks()
+
+    # replicas only: every rank renders its own scene of the same recipe; no data-path collective
+    scene = scenes.make_scene(args.config, seed=rank)
+    cfg = R.config_of(scene)
+    mask = B.Mask.full() if scene["mask"] is None else B.uts_build_mask(cfg, scene["mask"]["kind"], scene["mask"]["params"])
+    g, views = R.scene_to_device(scene)
+    r = R.Rasterizer(cfg, mask)
+    V, S = cfg.n_views, r.S
+    npx = S * cfg.ppt
+    gcol = torch.from_numpy(scenes.upstream_grad(V, npx, seed=rank)).cuda()
+    n_pix_active = int(V * cfg.n_pix) if scene["mask"] is None else int(V * sum(bin(int(w) & 0xffffffff).count("1") for w in mask.pixel_mask_bits.cpu().numpy().tolist()))
+
+    stream = torch.cuda.current_stream()
+
+    def step(events=None):
+        def mark(i):
+            if events is not None:
+                events[i].record(stream)
+        mark(0); r.preprocess(g, views)
+        mark(1); r.tile_query()
+        mark(2); r.sort()
+        mark(3); r.tile_ranges()
+        mark(4); r.render_fwd()
+        mark(5); r.render_bwd(gcol)
+        mark(6); r.preprocess_bwd(g, views)
+        mark(7)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local); sampler.start()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(8)] for _ in range(args.steps)]
+    t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    t0.record(stream)
+    for k in range(args.steps):
+        step(ev[k])
+    t1.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    total_ms = t0.elapsed_time(t1)
+    ms_step = total_ms / args.steps
+    stage_ms = {STAGES[i]: float(np.mean([ev[k][i].elapsed_time(ev[k][i + 1]) for k in range(args.steps)])) for i in range(7)}
+    ms_fwd = sum(stage_ms[s] for s in STAGES[:5])
+
+    # work counters from the forward outputs (measurement plumbing): entries each pixel evaluated
+    lens = (r.ranges[:, 1] - r.ranges[:, 0])
+    tiles = torch.arange(cfg.n_tiles, device="cuda") if mask.active_tiles is None else mask.active_tiles.long()
+    ev_f = ev_b = 0
+    for v in range(V):
+        L = lens[v * cfg.n_tiles + tiles].repeat_interleave(cfg.ppt)
+        nl = r.n_last[v].long()
+        sat = r.trans[v] < cfg.t_eps
+        ev_f += int(torch.where(sat, nl, L).sum().item())
+        ev_b += int(nl.sum().item())
+
+    # end to end through the C ABI with HOST buffers (H2D + D2H inside the timed region)
+    h = {k: torch.from_numpy(scene[k]).contiguous().pin_memory() for k in ("means", "scales", "quats", "opac", "sh", "W", "b")}
+    hg = gcol.cpu().pin_memory()
+    P, M = cfg.n_gauss, cfg.n_sh
+    pin = lambda *s: torch.empty(*s, dtype=torch.float32).pin_memory()
+    out = dict(color=pin(V, npx, 3), alpha=pin(V, npx), dL_dmeans=pin(P, 3), dL_dscales=pin(P, 3), dL_dquats=pin(P, 4), dL_dopac=pin(P),
+               dL_dsh=pin(P, M, 3))
+    cap = r.n_pairs + 1024
+    n_pairs = r.n_pairs
+    ws_bytes = B.uts_host_workspace_bytes(cfg, mask.n_active, cap)
+    keep = dict(stage_proj=None)
+    del r
+    torch.cuda.empty_cache()
+    ws = torch.empty(ws_bytes // 8 + 64, dtype=torch.int64, device="cuda")
+    h2d = sum(t.numel() * 4 for t in h.values()) + hg.numel() * 4
+    d2h = sum(t.numel() * 4 for t in out.values())
+    e2e_steps = max(1, min(args.steps, 3))
+    B.uts_host_forward_backward(cfg, h, mask, hg, out, cap, ws)           # warm-up
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    tt = time.perf_counter()
+    for _ in range(e2e_steps):
+        B.uts_host_forward_backward(cfg, h, mask, hg, out, cap, ws)       # synchronises the stream itself
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - tt) * 1e3 / e2e_steps
+
+    times = torch.tensor([ms_step, e2e_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+    ms_step_max, e2e_ms_max = float(times[0]), float(times[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    value = world * n_pix_active / (ms_step_max * 1e-3)
+    # dominant kernel and its roofline
+    dom = max(stage_ms, key=stage_ms.get)
+    fp32_peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12       # TFLOP/s at the maximum SM clock
+    if dom in ("render_fwd", "render_bwd"):
+        flop = ev_f * FLOP_FWD if dom == "render_fwd" else ev_b * FLOP_BWD
+        ach = flop / (stage_ms[dom] * 1e-3) / 1e12
+        roof = dict(kernel=dom, bound="alu", achieved=ach, peak=fp32_peak, unit="TFLOP/s", frac=ach / fp32_peak, traffic=None,
+                    peak_source="derived: 148 SM x 128 FP32 lanes x 2 x sm_max_mhz")
+    else:
+        per_pair = {"sort": 32.0 * (4 + 2), "tile_query": 12.0, "tile_ranges": 8.0}.get(dom)
+        byts = per_pair * n_pairs if per_pair else P * V * (44 + 12 * M + 57)
+        ach = byts / (stage_ms[dom] * 1e-3) / 1e9
+        roof = dict(kernel=dom, bound="hbm", achieved=ach, peak=peaks["hbm_gbs"], unit="GB/s", frac=ach / peaks["hbm_gbs"], traffic=None,
+                    peak_source=peaks["source"])
+    per_kernel = {}
+    for s_, ms in stage_ms.items():
+        if s_ == "render_fwd":
+            per_kernel[s_] = dict(ms=ms, tflops=ev_f * FLOP_FWD / (ms * 1e-3) / 1e12, frac_fp32_peak=ev_f * FLOP_FWD / (ms * 1e-3) / 1e12 / fp32_peak)
+        elif s_ == "render_bwd":
+            per_kernel[s_] = dict(ms=ms, tflops=ev_b * FLOP_BWD / (ms * 1e-3) / 1e12, frac_fp32_peak=ev_b * FLOP_BWD / (ms * 1e-3) / 1e12 / fp32_peak)
+        else:
+            byts = {"preprocess": P * V * (44 + 12 * M + 57), "preprocess_bwd": P * (44 + 12 * M + V * 33 + 40 + 12 * M),
+                    "tile_query": P * V * 2 * 21 + 8 * P * V + 12 * n_pairs, "sort": 32.0 * n_pairs * (4 + ((max(1, (V * cfg.n_tiles - 1)).bit_length() + 7) // 8)),
+                    "tile_ranges": 8.0 * n_pairs + 16 * V * cfg.n_tiles}[s_]
+            per_kernel[s_] = dict(ms=ms, gbs=byts / (ms * 1e-3) / 1e9, frac_hbm_peak=byts / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
+
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup, ms_per_step=ms_step_max,
+                higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
+                config=dict(workload=f"config{args.config}:{scene['name']}", order=cfg.order, nside=1 << cfg.order, n_pix=n_pix_active,
+                            n_gauss=P, sh_degree=cfg.sh_degree, n_views=V, n_pairs=n_pairs, parallelism=f"replicas{world}",
+                            l2="inputs larger than L2 (Gaussians 472 MB, pairs GBs); no flush needed"),
+                ms_forward=ms_fwd, ms_forward_backward=ms_step, stage_ms=stage_ms, per_kernel=per_kernel,
+                evaluated_pairs=dict(forward=ev_f, backward=ev_b),
+                roofline=roof, clocks=clocks,
+                e2e=dict(value=world * n_pix_active / (e2e_ms_max * 1e-3), unit=UNIT, ms_per_step=e2e_ms_max, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h),
+                gpu_launches=0)
+    # launches of our kernels per step: 1 preprocess + (1 count + 3 scan + 1 emit) + passes*(1 + 3 + 1) (+1 copy) + 1 ranges + 1 fwd + 1 bwd + 1 pre-bwd
+    passes = 4 + ((max(1, (V * cfg.n_tiles - 1)).bit_length() + 7) // 8)
+    line["gpu_launches"] = args.steps * (1 + 5 + passes * 5 + (passes % 2) + 1 + 1 + 1 + 1)
+    if not args.no_cpu_baseline:
+        t, desc, meta = oracle_sample(args.config, seed=0)
+        line["cpu_baseline"] = dict(value=meta["n_pix"] / t, unit=UNIT, cores=1, kind="oracle", sample=desc)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config id 1..5 (default 4 = the metric's workload)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

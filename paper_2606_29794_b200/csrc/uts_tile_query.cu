@@ -3,133 +3,375 @@
 //
 // Tile set of one projected Gaussian (direction u, radius r_s):
 //     T = { q >> 2(k_q - k_t) : q an order-k_q pixel,  u . centre(q) >= cos R },   R = min(pi, r_s + rho_max(k_q)),
-// intersected with the active tiles of the mask.  The predicate is evaluated in double precision.
+// intersected with the active tiles of the mask.  The defining predicate is evaluated in double precision.
 //
-// Differences from the paper's kernel (written for sm_89):
-//   * The paper's DFS keeps an explicit O(log Nside) stack per thread.  Here the traversal is
-//     STACKLESS: a NESTED index IS its own path (child c of p is 4p+c), so "next node in depth-first order" is
+// Differences from the paper's kernel (written for sm_89), see DESIGN.md "Kernels/F2":
+//   * STACKLESS traversal.  The paper's DFS keeps an O(log Nside) stack per thread.  A NESTED index
+//     IS its own path (child c of p is 4p+c), so "next node in depth-first order" is
 //     `while ((p & 3) == 3) p >>= 2, --o;  ++p` — two registers, no local memory.
-//   * Zone tests compare the dot product with per-level cosine thresholds cos(R +- rho_max(o)) obtained from one
-//     sincos(R) and a constant table of cos/sin rho_max(o) — no inverse trigonometry per node.
-//   * count -> exclusive scan -> emit, so the pair arrays are written once, densely, in (view, Gaussian, tile) order;
-//     depth-first order over NESTED indices is ascending tile order, so no per-Gaussian sort is needed.
+//   * Zone tests (Alg.2's Classify) run in single precision on CHORD lengths |u - c| against 2 sin((R +- rho_o)/2), with a
+//     margin far above the fp32 error, and only prune / accept whole subtrees; the leaf test falls back to the double
+//     precision dot product whenever it is within the margin, so the emitted set is exactly T.
+//   * Two work shapes.  Small discs: one thread per Gaussian walks the tree.  Large discs (tens of thousands of tiles;
+//     config 4's outliers own most of the pairs): one thread BLOCK per Gaussian classifies every order-o_s node in
+//     parallel, walks the boundary subtrees from a shared work list, and records tiles in a shared-memory BITMAP over all
+//     tiles.  The bitmap makes the result independent of visiting order, removes duplicates for free, and turns emission
+//     into a rank query, so pairs come out in ascending tile order with fully coalesced stores.
+//   * count -> exclusive scan -> emit: the pair arrays are written once, densely, in (view, Gaussian, tile) order.
 #include "uts_internal.cuh"
 #include "uts_scan.cuh"
 
 namespace uts {
 
+constexpr float kDelta = 4e-6f;         // fp32 chord margin (chord error of the fp32 centres is below 1e-6)
+constexpr int kLargeThreads = 256;
+
 struct QueryParams {
   int kt, kq, P, V;
+  int os;                               // split order of the block-per-Gaussian path
+  int n_words;                          // bitmap words = n_tile / 32 (0: block path disabled)
   int64_t n_tile;
   double rho_q;                         // rho_max(k_q)
-  double cos_rho[kMaxOrder + 1], sin_rho[kMaxOrder + 1];
+  float r_large;                        // discs with R above this go to the block path
+  float rho[kMaxOrder + 1], sin_hrho[kMaxOrder + 1], cos_hrho[kMaxOrder + 1];   // rho_max(o), sin/cos(rho_max(o)/2)
 };
 
-constexpr double kSlack = 1e-12;        // zone decisions are conservative by this much; the leaf test alone defines T
+// Per-Gaussian query state.
+struct Disc {
+  double u[3]; double cosR;
+  float uf[3]; float Rf, sh, ch;        // sin(R/2), cos(R/2)
+  bool all;                             // R >= pi: every tile (reading A24)
+};
 
+__device__ __forceinline__ bool load_disc(const QueryParams& qp, const float* __restrict__ dir, const float* __restrict__ rs,
+                                          int64_t k, Disc& D) {
+  D.u[0] = (double)__ldg(dir + 3 * k); D.u[1] = (double)__ldg(dir + 3 * k + 1); D.u[2] = (double)__ldg(dir + 3 * k + 2);
+  const double nrm = sqrt(D.u[0] * D.u[0] + D.u[1] * D.u[1] + D.u[2] * D.u[2]);
+  D.u[0] /= nrm; D.u[1] /= nrm; D.u[2] /= nrm;
+  const double R = fmin(kPi, (double)__ldg(rs + k) + qp.rho_q);
+  D.all = R >= kPi;
+  D.cosR = cos(R);
+  double s, c;
+  sincos(0.5 * R, &s, &c);
+  D.uf[0] = (float)D.u[0]; D.uf[1] = (float)D.u[1]; D.uf[2] = (float)D.u[2];
+  D.Rf = (float)R; D.sh = (float)s; D.ch = (float)c;
+  return true;
+}
+
+enum Zone { kOutside = 0, kInside = 1, kPartial = 2 };
+
+// Alg.2's Classify for node (o,p): kOutside = no descendant centre can be within R, kInside = all are.
+__device__ __forceinline__ Zone classify(const QueryParams& qp, const Disc& D, int o, uint64_t p, float& chord) {
+  float cx, cy, cz;
+  pix_center_cam_f32(o, p, cx, cy, cz);
+  const float dx = D.uf[0] - cx, dy = D.uf[1] - cy, dz = D.uf[2] - cz;
+  chord = sqrtf(dx * dx + dy * dy + dz * dz);
+  const float a = D.sh * qp.cos_hrho[o], b = D.ch * qp.sin_hrho[o];
+  const float rho = qp.rho[o];
+  if (D.Rf + rho < 3.1415f && chord > 2.0f * (a + b) + kDelta) return kOutside;
+  if (D.Rf - rho > 1e-4f && chord < 2.0f * (a - b) - kDelta) return kInside;
+  return kPartial;
+}
+
+// The defining predicate at a leaf (order k_q).
+__device__ __forceinline__ bool leaf_inside(const QueryParams& qp, const Disc& D, uint64_t p, float chord) {
+  const float t = 2.0f * D.sh;
+  if (chord < t - kDelta) return true;
+  if (chord > t + kDelta) return false;
+  double cx, cy, cz;
+  pix_center_cam(qp.kq, p, cx, cy, cz);
+  return D.u[0] * cx + D.u[1] * cy + D.u[2] * cz >= D.cosR;
+}
+
+// Depth-first walk of the subtrees rooted at the order-ro nodes rp0..rp1 (inclusive), one node per step().
+// Sink: add(tile), add_range(t0,t1), has(tile).  The climb after a finished subtree is a count of trailing 11 bit pairs,
+// so a step has no data-dependent loop in its control path.  Callers drive step() from a WARP-SYNCHRONOUS loop
+// (`while (__any_sync(full, running))`): every lane walks its own tree, and the vote makes the lanes reconverge at every
+// node.  (Left to the compiler, the walk loop's reconvergence point was the loop exit: 2 of 32 lanes active, measured.)
+struct Walker {
+  int o, ro;
+  uint64_t p, rp1;
+  __device__ __forceinline__ void start(int ro_, uint64_t rp0, uint64_t rp1_) { o = ro = ro_; p = rp0; rp1 = rp1_; }
+  // returns true when the walk is finished
+  template <class Sink>
+  __device__ __forceinline__ bool step(const QueryParams& qp, const Disc& D, Sink& sink) {
+    const int kt = qp.kt, kq = qp.kq;
+    float chord;
+    const Zone z = classify(qp, D, o, p, chord);
+    bool descend = false;
+    if (z != kOutside) {
+      if (o <= kt) {
+        if (z == kInside) { const int sh = 2 * (kt - o); sink.add_range((int64_t)(p << sh), (int64_t)((p + 1) << sh)); }
+        else descend = true;
+      } else {
+        const int64_t tile = (int64_t)(p >> (2 * (o - kt)));
+        if (!sink.has(tile)) {
+          if (z == kInside && o < kq) sink.add(tile);
+          else descend = true;
+        }
+      }
+      if (descend && o == kq) {
+        if (leaf_inside(qp, D, p, chord)) sink.add((int64_t)(p >> (2 * (kq - kt))));
+        descend = false;
+      }
+    }
+    bool finished = false;
+    if (descend) { p <<= 2; ++o; }
+    else {
+      const int ones = __ffsll((long long)~p) - 1;              // trailing one bits of p
+      const int up = min(ones >> 1, o - ro);                    // finished last children to climb over
+      p >>= 2 * up; o -= up;
+      if (o == ro && p == rp1) finished = true; else ++p;
+    }
+    return finished;
+  }
+};
+
+// ------------------------------------------------------------------------------------- thread-per-Gaussian path
 template <bool EMIT>
-struct Sink {
+struct ThreadSink {
   uint64_t* keys; uint32_t* vals; uint64_t base; uint64_t key_hi_base; uint32_t depth_bits; uint32_t gid;
   const int32_t* slot_of_tile;
   uint32_t count;
   int64_t last_tile;
+  __device__ __forceinline__ bool has(int64_t tile) const { return tile == last_tile; }
   __device__ __forceinline__ void add(int64_t tile) {
     if (tile == last_tile) return;
+    last_tile = tile;
     if (slot_of_tile && __ldg(slot_of_tile + tile) < 0) return;
     if (EMIT) {
       keys[base + count] = ((key_hi_base + (uint64_t)tile) << 32) | depth_bits;   // Alg.1 l.12: ((t, rho), i)
       vals[base + count] = gid;
     }
     ++count;
-    last_tile = tile;
   }
+  __device__ __forceinline__ void add_range(int64_t t0, int64_t t1) { for (int64_t t = t0; t < t1; ++t) add(t); }
 };
 
-// Depth-first walk over the NESTED quadtree from the 12 base pixels down to order k_q.
-template <bool EMIT>
-__device__ __forceinline__ void walk(const QueryParams& qp, const double u[3], double R, Sink<EMIT>& sink) {
-  const int kt = qp.kt, kq = qp.kq;
-  if (R >= kPi) {                       // reading A24: the disc is the whole sphere
-    for (int64_t t = 0; t < qp.n_tile; ++t) sink.add(t);
-    return;
-  }
-  double sR, cR;
-  sincos(R, &sR, &cR);
-  int o = 0;
-  uint64_t p = 0;
-  while (true) {
-    double cx, cy, cz;
-    pix_center_cam(o, p, cx, cy, cz);
-    const double dot = u[0] * cx + u[1] * cy + u[2] * cz;
-    const double cr = qp.cos_rho[o], sr = qp.sin_rho[o];
-    // cos(R + rho_o) is a valid "outside" threshold only while R + rho_o < pi, cos(R - rho_o) a valid "inside" one only
-    // while R - rho_o >= 0; encoded by the host as sin/cos of rho_o and checked here through the sign of sin(R +- rho_o).
-    const double cos_sum = cR * cr - sR * sr, sin_sum = sR * cr + cR * sr;     // R + rho_o in (0, 2pi)
-    const double cos_dif = cR * cr + sR * sr, sin_dif = sR * cr - cR * sr;     // R - rho_o in (-pi/2, pi)
-    const bool outside = (sin_sum > 0.0) && (dot < cos_sum - kSlack);
-    const bool inside = (sin_dif >= 0.0) && (dot >= cos_dif + kSlack);
-    bool descend = false;
-    if (!outside) {
-      if (o <= kt) {
-        if (inside) {
-          const int sh = 2 * (kt - o);
-          const int64_t t0 = (int64_t)(p << sh), t1 = (int64_t)((p + 1) << sh);
-          for (int64_t t = t0; t < t1; ++t) sink.add(t);
-        } else descend = true;
-      } else {
-        const int64_t tile = (int64_t)(p >> (2 * (o - kt)));
-        if (tile != sink.last_tile) {
-          if (inside && o < kq) sink.add(tile);
-          else descend = true;
-        }
-      }
-      if (descend && o == kq) {          // leaf: the defining predicate
-        if (dot >= cR) sink.add((int64_t)(p >> (2 * (kq - kt))));
-        descend = false;
-      }
+// Work classes.  A thread-per-Gaussian walk is only efficient when the 32 lanes of a warp have similar amounts of work
+// (measured: with Gaussians in input order 1.7 of 32 lanes were active on config 4).  So the count pass first buckets the
+// Gaussians by disc radius (4 buckets per octave of R, largest first) into a permutation; thread t then walks perm[t].
+constexpr int kBuckets = 64;
+
+__device__ __forceinline__ int radius_bucket(float R32) {      // larger discs -> smaller bucket index
+  const int e = (int)(__float_as_uint(R32) >> 21);               // exponent and two mantissa bits; R32 in (0, pi]
+  const int top = (int)(__float_as_uint(4.0f) >> 21);
+  return min(kBuckets - 1, max(0, top - e));
+}
+
+// which = 0: histogram of buckets (+ culled counts, + block-path list); which = 1: scatter into perm.
+template <int WHICH>
+__global__ void __launch_bounds__(256)
+classify_kernel(QueryParams qp, const float* __restrict__ rs, const uint8_t* __restrict__ flags, uint32_t* __restrict__ counts,
+                uint32_t* __restrict__ large_list, uint32_t* __restrict__ n_large, uint32_t* __restrict__ hist /*[64] counts, then cursors*/,
+                uint32_t* __restrict__ perm) {
+  __shared__ uint32_t s_hist[kBuckets];
+  if (threadIdx.x < kBuckets) s_hist[threadIdx.x] = 0;
+  __syncthreads();
+  const int64_t n = (int64_t)qp.P * qp.V;
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int b = -1;
+  if (k < n) {
+    if (__ldg(flags + k) & 1) { if (WHICH == 0) counts[k] = 0; }
+    else {
+      const float R32 = fminf(3.14159274f, __ldg(rs + k) + (float)qp.rho_q);
+      if (qp.n_words > 0 && R32 > qp.r_large) { if (WHICH == 0) large_list[atomicAdd(n_large, 1u)] = (uint32_t)k; }
+      else b = radius_bucket(R32);
     }
-    if (descend) { p <<= 2; ++o; continue; }
-    while (o > 0 && (p & 3) == 3) { p >>= 2; --o; }
-    ++p;
-    if (o == 0 && p == 12) break;
+  }
+  uint32_t local = 0;
+  if (b >= 0) local = atomicAdd(&s_hist[b], 1u);
+  __syncthreads();
+  if (WHICH == 0) {
+    if (threadIdx.x < kBuckets && s_hist[threadIdx.x]) atomicAdd(hist + threadIdx.x, s_hist[threadIdx.x]);
+  } else {
+    __shared__ uint32_t s_base[kBuckets];
+    if (threadIdx.x < kBuckets) s_base[threadIdx.x] = s_hist[threadIdx.x] ? atomicAdd(hist + threadIdx.x, s_hist[threadIdx.x]) : 0u;
+    __syncthreads();
+    if (b >= 0) perm[s_base[b] + local] = (uint32_t)k;
+  }
+}
+
+// hist[64] counts -> exclusive start offsets (in place); n_small = total
+__global__ void bucket_scan_kernel(uint32_t* __restrict__ hist, uint32_t* __restrict__ n_small) {
+  if (threadIdx.x == 0) {
+    uint32_t run = 0;
+    for (int b = 0; b < kBuckets; ++b) { const uint32_t c = hist[b]; hist[b] = run; run += c; }
+    *n_small = run;
   }
 }
 
 template <bool EMIT>
 __global__ void __launch_bounds__(128)
-tile_query_kernel(QueryParams qp, const float* __restrict__ dir, const float* __restrict__ rho, const float* __restrict__ rs,
-                  const uint8_t* __restrict__ flags, const int32_t* __restrict__ slot_of_tile, uint32_t* __restrict__ counts,
-                  const uint64_t* __restrict__ offsets, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
-  const int64_t n = (int64_t)qp.P * qp.V;
-  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= n) return;
-  if (__ldg(flags + k) & 1) { if (!EMIT) counts[k] = 0; return; }
-  if (EMIT && offsets[k + 1] == offsets[k]) return;
-  const int v = (int)(k / qp.P);
-  const uint32_t i = (uint32_t)(k - (int64_t)v * qp.P);
-  double u[3] = {(double)__ldg(dir + 3 * k), (double)__ldg(dir + 3 * k + 1), (double)__ldg(dir + 3 * k + 2)};
-  const double nrm = sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
-  u[0] /= nrm; u[1] /= nrm; u[2] /= nrm;
-  const double R = fmin(kPi, (double)__ldg(rs + k) + qp.rho_q);
-  Sink<EMIT> sink;
-  sink.keys = keys; sink.vals = vals; sink.base = EMIT ? offsets[k] : 0;
-  sink.key_hi_base = (uint64_t)v * (uint64_t)qp.n_tile;
-  sink.depth_bits = __float_as_uint(__ldg(rho + k));                         // reading A10
-  sink.gid = i; sink.slot_of_tile = slot_of_tile; sink.count = 0; sink.last_tile = -1;
-  walk<EMIT>(qp, u, R, sink);
-  if (!EMIT) counts[k] = sink.count;
+tile_query_small_kernel(QueryParams qp, const float* __restrict__ dir, const float* __restrict__ rho, const float* __restrict__ rs,
+                        const int32_t* __restrict__ slot_of_tile, const uint32_t* __restrict__ perm, const uint32_t* __restrict__ n_small,
+                        uint32_t* __restrict__ counts, const uint64_t* __restrict__ offsets, uint64_t* __restrict__ keys,
+                        uint32_t* __restrict__ vals) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  bool running = t < (int64_t)*n_small;
+  const int64_t k = running ? (int64_t)perm[t] : 0;
+  if (EMIT && running && offsets[k + 1] == offsets[k]) running = false;
+  Disc D;
+  ThreadSink<EMIT> sink;
+  sink.count = 0; sink.last_tile = -1; sink.slot_of_tile = slot_of_tile; sink.keys = keys; sink.vals = vals;
+  sink.base = 0; sink.key_hi_base = 0; sink.depth_bits = 0; sink.gid = 0;
+  const bool valid = running;
+  if (running) {
+    load_disc(qp, dir, rs, k, D);
+    const int v = (int)(k / qp.P);
+    sink.base = EMIT ? offsets[k] : 0;
+    sink.key_hi_base = (uint64_t)v * (uint64_t)qp.n_tile;
+    sink.depth_bits = __float_as_uint(__ldg(rho + k));                       // reading A10
+    sink.gid = (uint32_t)(k - (int64_t)v * qp.P);
+    if (D.all) { sink.add_range(0, qp.n_tile); running = false; }
+  }
+  Walker w;
+  w.start(0, 0, 11);
+  while (__any_sync(0xffffffffu, running)) {
+    if (running) running = !w.step(qp, D, sink);
+  }
+  if (!EMIT && valid) counts[k] = sink.count;
+}
+
+// -------------------------------------------------------------------------------------- block-per-Gaussian path
+struct BitmapSink {
+  uint32_t* bits;
+  __device__ __forceinline__ bool has(int64_t tile) const { return (bits[tile >> 5] >> (tile & 31)) & 1u; }
+  __device__ __forceinline__ void add(int64_t tile) { atomicOr(bits + (tile >> 5), 1u << (tile & 31)); }
+  __device__ __forceinline__ void add_range(int64_t t0, int64_t t1) {       // [t0,t1) is an aligned block of 4^j tiles
+    if (t1 - t0 >= 32) { for (int64_t w = t0 >> 5; w < (t1 >> 5); ++w) bits[w] = 0xffffffffu; }
+    else atomicOr(bits + (t0 >> 5), (uint32_t)((((uint64_t)1 << (t1 - t0)) - 1) << (t0 & 31)));
+  }
+};
+
+__device__ __forceinline__ uint32_t block_sum_u32(uint32_t x, uint32_t* s_w /*[8]*/, uint32_t& before) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  uint32_t incl = x;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += y; }
+  __syncthreads();
+  if (lane == 31) s_w[wid] = incl;
+  __syncthreads();
+  uint32_t b = 0, total = 0;
+#pragma unroll
+  for (int w = 0; w < kLargeThreads / 32; ++w) { const uint32_t s = s_w[w]; if (w < wid) b += s; total += s; }
+  before = b + incl - x;
+  return total;
+}
+
+// active_words[w]: bit t set <=> tile 32w+t is active (built once per call from slot_of_tile)
+__global__ void active_words_kernel(const int32_t* __restrict__ slot_of_tile, int n_words, uint32_t* __restrict__ active_words) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= n_words) return;
+  uint32_t m = 0;
+  for (int t = 0; t < 32; ++t) if (__ldg(slot_of_tile + 32 * (int64_t)w + t) >= 0) m |= 1u << t;
+  active_words[w] = m;
+}
+
+template <bool EMIT>
+__global__ void __launch_bounds__(kLargeThreads)
+tile_query_large_kernel(QueryParams qp, const float* __restrict__ dir, const float* __restrict__ rho, const float* __restrict__ rs,
+                        const uint32_t* __restrict__ active_words, const uint32_t* __restrict__ large_list,
+                        const uint32_t* __restrict__ n_large, uint32_t* __restrict__ counts, const uint64_t* __restrict__ offsets,
+                        uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+  extern __shared__ uint32_t smem[];
+  uint32_t* bits = smem;                         // [n_words]
+  uint32_t* pref = smem + qp.n_words;            // [n_words]  exclusive popcount prefix (emit only)
+  uint32_t* work = smem + 2 * qp.n_words;        // [12 * 4^os] partial nodes at the split order
+  __shared__ Disc s_disc;
+  __shared__ uint32_t s_count, s_next, s_w[kLargeThreads / 32];
+  const int n_split = 12 << (2 * qp.os);
+  const uint32_t nl = *n_large;
+  for (uint32_t li = blockIdx.x; li < nl; li += gridDim.x) {
+    const int64_t k = (int64_t)large_list[li];
+    __syncthreads();
+    if (threadIdx.x == 0) { load_disc(qp, dir, rs, k, s_disc); s_count = 0; s_next = 0; }
+    for (int w = threadIdx.x; w < qp.n_words; w += kLargeThreads) bits[w] = 0u;
+    __syncthreads();
+    const Disc D = s_disc;
+    BitmapSink sink{bits};
+    if (D.all) {
+      for (int w = threadIdx.x; w < qp.n_words; w += kLargeThreads) bits[w] = 0xffffffffu;
+    } else {
+      for (int node = threadIdx.x; node < n_split; node += kLargeThreads) {
+        float chord;
+        const Zone z = classify(qp, D, qp.os, (uint64_t)node, chord);
+        if (z == kInside) { const int sh = 2 * (qp.kt - qp.os); sink.add_range((int64_t)node << sh, (int64_t)(node + 1) << sh); }
+        else if (z == kPartial) work[atomicAdd(&s_count, 1u)] = (uint32_t)node;
+      }
+      __syncthreads();
+      const uint32_t nw = s_count;
+      Walker w;
+      bool active = false, exhausted = false;
+      while (true) {                                  // every lane does one node per iteration and refills itself when idle
+        if (!active && !exhausted) {
+          const uint32_t i = atomicAdd(&s_next, 1u);
+          if (i < nw) { w.start(qp.os, (uint64_t)work[i], (uint64_t)work[i]); active = true; }
+          else exhausted = true;
+        }
+        if (!__any_sync(0xffffffffu, active)) break;
+        if (active) active = !w.step(qp, D, sink);
+      }
+    }
+    __syncthreads();
+    // mask, then count / prefix: each thread owns a contiguous chunk of words
+    const int chunk = (qp.n_words + kLargeThreads - 1) / kLargeThreads;
+    const int w0 = min(qp.n_words, (int)threadIdx.x * chunk), w1 = min(qp.n_words, w0 + chunk);
+    uint32_t mine = 0;
+    for (int w = w0; w < w1; ++w) {
+      uint32_t b = bits[w];
+      if (active_words) { b &= __ldg(active_words + w); bits[w] = b; }
+      mine += __popc(b);
+    }
+    uint32_t before;
+    const uint32_t total = block_sum_u32(mine, s_w, before);
+    if (!EMIT) { if (threadIdx.x == 0) counts[k] = total; continue; }
+    for (int w = w0; w < w1; ++w) { pref[w] = before; before += __popc(bits[w]); }
+    __syncthreads();
+    const int v = (int)(k / qp.P);
+    const uint32_t gid = (uint32_t)(k - (int64_t)v * qp.P);
+    const uint64_t base = offsets[k], hi = (uint64_t)v * (uint64_t)qp.n_tile;
+    const uint32_t depth = __float_as_uint(__ldg(rho + k));
+    for (uint32_t r = threadIdx.x; r < total; r += kLargeThreads) {
+      int lo = 0, hi_w = qp.n_words - 1;                       // largest w with pref[w] <= r
+      while (lo < hi_w) { const int mid = (lo + hi_w + 1) >> 1; if (pref[mid] <= r) lo = mid; else hi_w = mid - 1; }
+      const uint32_t bit = __fns(bits[lo], 0, (int)(r - pref[lo]) + 1);
+      keys[base + r] = ((hi + (uint64_t)lo * 32 + bit) << 32) | depth;
+      vals[base + r] = gid;
+    }
+  }
 }
 
 }  // namespace uts
 
 using namespace uts;
 
+namespace {
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+constexpr size_t kMaxLargeSmem = 200 * 1024;
+
+struct QueryLayout { size_t counts, list, perm, nlarge, active, scan, total; };
+QueryLayout query_layout(const uts_config* cfg) {
+  const size_t n = (size_t)cfg->n_gauss * cfg->n_views;
+  const size_t n_tile = (size_t)12 << (2 * (cfg->order - cfg->tile_log2));
+  QueryLayout L;
+  size_t off = 0;
+  L.counts = off; off += align256(n * 4);
+  L.list = off;   off += align256(n * 4);
+  L.perm = off;   off += align256(n * 4);
+  L.nlarge = off; off += 512;      // n_large, n_small, 64 bucket counters
+  L.active = off; off += align256((n_tile / 32 + 1) * 4);
+  L.scan = off;   off += scan_scratch_bytes((int64_t)n);
+  L.total = off + 256;
+  return L;
+}
+}  // namespace
+
 extern "C" {
 
 size_t uts_tile_query_scratch_bytes(const uts_config* cfg) {
   if (check_config(cfg) != UTS_OK) return 0;
-  const int64_t n = (int64_t)cfg->n_gauss * cfg->n_views;
-  return (size_t)(((n * 4 + 255) / 256) * 256) + scan_scratch_bytes(n);
+  return query_layout(cfg).total;
 }
 
 int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, uint64_t* offsets, uint64_t* keys, uint32_t* vals,
@@ -150,24 +392,74 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, uint64_t* 
   if (!in.dir || !in.rho || !in.rs || !in.flags || !scratch) return UTS_ERR_INVALID_ARG;
   if (keys && !vals) return UTS_ERR_INVALID_ARG;
   if (scratch_bytes < uts_tile_query_scratch_bytes(cfg) || ((uintptr_t)scratch & 255)) return UTS_ERR_INVALID_ARG;
+
   QueryParams qp;
   qp.kt = d.kt; qp.kq = d.kq; qp.P = d.P; qp.V = d.V; qp.n_tile = d.n_tile;
   const double* rm = rho_max_table_host();
   qp.rho_q = rm[d.kq];
-  for (int o = 0; o <= kMaxOrder; ++o) { qp.cos_rho[o] = cos(rm[o]); qp.sin_rho[o] = sin(rm[o]); }
-  uint32_t* counts = reinterpret_cast<uint32_t*>(scratch);
-  uint64_t* block_sums = reinterpret_cast<uint64_t*>(reinterpret_cast<char*>(scratch) + ((n * 4 + 255) / 256) * 256);
+  for (int o = 0; o <= kMaxOrder; ++o) { qp.rho[o] = (float)rm[o]; qp.sin_hrho[o] = (float)sin(0.5 * rm[o]); qp.cos_hrho[o] = (float)cos(0.5 * rm[o]); }
+  qp.os = d.kt < 4 ? d.kt : 4;
+  const size_t n_split = (size_t)12 << (2 * qp.os);
+  const size_t large_smem = (2 * (size_t)(d.n_tile / 32) + n_split) * 4;
+  const bool use_large = d.kt >= 2 && large_smem <= kMaxLargeSmem;
+  qp.n_words = use_large ? (int)(d.n_tile / 32) : 0;
+  qp.r_large = (float)(64.0 / sqrt((double)d.n_tile));      // ~1024 tiles: pi R^2 / (4 pi / n_tile)
+
+  const QueryLayout L = query_layout(cfg);
+  char* sp = reinterpret_cast<char*>(scratch);
+  uint32_t* counts = reinterpret_cast<uint32_t*>(sp + L.counts);
+  uint32_t* list = reinterpret_cast<uint32_t*>(sp + L.list);
+  uint32_t* n_large = reinterpret_cast<uint32_t*>(sp + L.nlarge);
+  uint32_t* n_small = n_large + 1;
+  uint32_t* hist = n_large + 32;
+  uint32_t* perm = reinterpret_cast<uint32_t*>(sp + L.perm);
+  uint32_t* active = reinterpret_cast<uint32_t*>(sp + L.active);
+  uint64_t* block_sums = reinterpret_cast<uint64_t*>(sp + L.scan);
+  const uint32_t* active_arg = nullptr;
   const unsigned qgrid = (unsigned)((n + 127) / 128);
-  tile_query_kernel<false><<<qgrid, 128, 0, s>>>(qp, in.dir, in.rho, in.rs, in.flags, mask.slot_of_tile, counts, nullptr, nullptr, nullptr);
+  const unsigned lgrid = (unsigned)(sm_count() * 4);
+  if (use_large) {
+    static bool attr_set = false;
+    if (!attr_set) {
+      UTS_CUDA(cudaFuncSetAttribute(tile_query_large_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxLargeSmem));
+      UTS_CUDA(cudaFuncSetAttribute(tile_query_large_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxLargeSmem));
+      attr_set = true;
+    }
+    if (mask.slot_of_tile) {
+      active_words_kernel<<<(qp.n_words + 255) / 256, 256, 0, s>>>(mask.slot_of_tile, qp.n_words, active);
+      UTS_LAUNCH_CHECK();
+      active_arg = active;
+    }
+  }
+  UTS_CUDA(cudaMemsetAsync(n_large, 0, 512, s));
+  const unsigned cgrid = (unsigned)((n + 255) / 256);
+  classify_kernel<0><<<cgrid, 256, 0, s>>>(qp, in.rs, in.flags, counts, list, n_large, hist, perm);
   UTS_LAUNCH_CHECK();
+  bucket_scan_kernel<<<1, 32, 0, s>>>(hist, n_small);
+  UTS_LAUNCH_CHECK();
+  classify_kernel<1><<<cgrid, 256, 0, s>>>(qp, in.rs, in.flags, counts, list, n_large, hist, perm);
+  UTS_LAUNCH_CHECK();
+  tile_query_small_kernel<false><<<qgrid, 128, 0, s>>>(qp, in.dir, in.rho, in.rs, mask.slot_of_tile, perm, n_small, counts, nullptr, nullptr,
+                                                       nullptr);
+  UTS_LAUNCH_CHECK();
+  if (use_large) {
+    tile_query_large_kernel<false><<<lgrid, kLargeThreads, large_smem, s>>>(qp, in.dir, in.rho, in.rs, active_arg, list, n_large, counts,
+                                                                            nullptr, nullptr, nullptr);
+    UTS_LAUNCH_CHECK();
+  }
   if ((st = exclusive_scan_u32(counts, n, offsets, block_sums, s))) return st;
   UTS_CUDA(cudaMemcpyAsync(h_n_pairs, offsets + n, sizeof(uint64_t), cudaMemcpyDeviceToHost, s));
   UTS_CUDA(cudaStreamSynchronize(s));
   if (!keys) return UTS_OK;
   if (*h_n_pairs > capacity) return UTS_ERR_CAPACITY;
   if (*h_n_pairs == 0) return UTS_OK;
-  tile_query_kernel<true><<<qgrid, 128, 0, s>>>(qp, in.dir, in.rho, in.rs, in.flags, mask.slot_of_tile, nullptr, offsets, keys, vals);
+  tile_query_small_kernel<true><<<qgrid, 128, 0, s>>>(qp, in.dir, in.rho, in.rs, mask.slot_of_tile, perm, n_small, nullptr, offsets, keys, vals);
   UTS_LAUNCH_CHECK();
+  if (use_large) {
+    tile_query_large_kernel<true><<<lgrid, kLargeThreads, large_smem, s>>>(qp, in.dir, in.rho, in.rs, active_arg, list, n_large, nullptr,
+                                                                           offsets, keys, vals);
+    UTS_LAUNCH_CHECK();
+  }
   return UTS_OK;
 }
 

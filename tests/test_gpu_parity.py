@@ -197,6 +197,29 @@ def test_tile_query_other_refinements(refine):
     assert np.array_equal(u64(r.keys)[:n], keys) and np.array_equal(u32(r.vals)[:n], vals)
 
 
+@pytest.mark.parametrize("cfg_id,order,refine", [(4, 9, 2), (3, 9, 2), (4, 8, 1), (5, 10, 2)])
+def test_tile_query_block_path_large_discs(cfg_id, order, refine):
+    """Discs of thousands of tiles take the block-per-Gaussian bitmap path (R > 64/sqrt(N_tile)); with and without a mask."""
+    B, R = _gpu()
+    scene = small_scene(cfg_id, 300, order, n_views=1)
+    scene["scales"][::2] *= 30.0                   # every other Gaussian becomes a very large disc
+    scene["scales"][7] = 80.0                      # r_s = pi inside the block path
+    oc = ocfg(scene, query_refine_log2=refine)
+    bits, act, slot = oracle_mask(oc, scene)
+    pr = orc.preprocess(oc, scene["means"], scene["scales"], scene["quats"], scene["opac"], scene["sh"], scene["W"], scene["b"])
+    assert (pr.rs[0] + orc.rho_max_closed(oc.tile_order + refine) > 64.0 / np.sqrt(oc.n_tiles)).sum() > 8
+    off, keys, vals, info = orc.tile_query(oc, pr, slot)
+    assert info["min_margin"] > 1e-12
+    cfg = _cfg(R, scene, query_refine_log2=refine)
+    mask = B.Mask.full() if bits is None else B.Mask(dev(act.view(np.int32)), int(act.shape[0]), dev(slot), dev(bits.view(np.int32)))
+    r = R.Rasterizer(cfg, mask)
+    r.proj = B.Proj(dev(pr.dir), dev(pr.lonlat), dev(pr.rho), dev(pr.conic_opac), dev(pr.rs), dev(pr.rgb), dev(pr.flags))
+    n = r.tile_query()
+    assert n == keys.shape[0]
+    assert np.array_equal(u64(r.offsets), off)
+    assert np.array_equal(u64(r.keys)[:n], keys) and np.array_equal(u32(r.vals)[:n], vals)
+
+
 def test_tile_query_whole_sphere_and_empty():
     B, R = _gpu()
     scene = small_scene(1, 4, 6)

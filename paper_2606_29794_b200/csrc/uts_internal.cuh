@@ -109,28 +109,37 @@ __device__ __forceinline__ void pix_center_cam(int o, uint64_t p, double& vx, do
   vx = g.sth * s; vy = g.z; vz = g.sth * c;
 }
 
-// Single-precision pixel centre (absolute error below 1e-6 on every component): used only to pre-classify quadtree nodes
-// with a safety margin; every decision that defines an output is re-taken in double when it falls inside the margin.
-__device__ __forceinline__ void pix_center_cam_f32(int o, uint64_t p, float& vx, float& vy, float& vz) {
+// Single-precision pixel centre (absolute error about 1e-6 per component): used only to pre-classify quadtree nodes with a
+// safety margin; every decision that defines an output is re-taken in double when it falls inside the margin.
+// A NESTED index at order <= 13 fits 32 bits (12 * 4^13 < 2^32).
+__host__ __device__ __forceinline__ uint32_t squeeze_even_bits32(uint32_t v) {
+  v &= 0x55555555u;
+  v = (v | (v >> 1)) & 0x33333333u;
+  v = (v | (v >> 2)) & 0x0f0f0f0fu;
+  v = (v | (v >> 4)) & 0x00ff00ffu;
+  v = (v | (v >> 8)) & 0x0000ffffu;
+  return v;
+}
+
+__device__ __forceinline__ void pix_center_cam_f32(int o, uint32_t p, float& vx, float& vy, float& vz) {
   const int N = 1 << o;
   const int f = (int)(p >> (2 * o));
-  const uint64_t m = p & (((uint64_t)1 << (2 * o)) - 1);
-  const int x = (int)squeeze_even_bits(m), y = (int)squeeze_even_bits(m >> 1);
+  const uint32_t m = p & ((1u << (2 * o)) - 1u);
+  const int x = (int)squeeze_even_bits32(m), y = (int)squeeze_even_bits32(m >> 1);
   const int r = f >> 2, c = f & 3;
   const int i = (r + 1) * N - (x + y - (N - 1));
   const int h = x - y;
-  const float fN = (float)N;
-  const float inv3N2 = 1.0f / (3.0f * fN * fN);
-  float z, sth;
-  int n;
-  if (i < N) { n = i; const float w = (float)n * (float)n * inv3N2; z = 1.0f - w; sth = sqrtf(w * (2.0f - w)); }
-  else if (i > 3 * N) { n = 4 * N - i; const float w = (float)n * (float)n * inv3N2; z = w - 1.0f; sth = sqrtf(w * (2.0f - w)); }
-  else { n = N; z = (float)(2 * (2 * N - i)) / (3.0f * fN); sth = sqrtf((1.0f - z) * (1.0f + z)); }
-  // longitude in quarter turns, reduced to (-4, 4] before scaling so that sincosf sees |lam| <= pi
-  float q = (float)(2 * c + 1 - (r & 1)) + (float)h / (float)n;
+  const float invN = __int_as_float((127 - o) << 23);          // 2^-o, exact
+  const float inv3N2 = 0.333333343f * invN * invN;
+  float z, sth, q;
+  if (i < N) { const float fn = (float)i; const float w = fn * fn * inv3N2; z = 1.0f - w; sth = sqrtf(w * (2.0f - w)); q = __fdividef((float)h, fn); }
+  else if (i > 3 * N) { const float fn = (float)(4 * N - i); const float w = fn * fn * inv3N2; z = w - 1.0f; sth = sqrtf(w * (2.0f - w)); q = __fdividef((float)h, fn); }
+  else { z = (float)(2 * (2 * N - i)) * (0.333333343f * invN); sth = sqrtf((1.0f - z) * (1.0f + z)); q = (float)h * invN; }
+  // longitude in quarter turns, reduced to (-4, 4] so that the fast sincos sees |lam| <= pi (absolute error < 5e-7 there)
+  q += (float)(2 * c + 1 - (r & 1));
   if (q > 4.0f) q -= 8.0f;
   float s, cs;
-  sincosf(q * 0.78539816339744831f, &s, &cs);
+  __sincosf(q * 0.78539816339744831f, &s, &cs);
   vx = sth * s; vy = z; vz = sth * cs;
 }
 

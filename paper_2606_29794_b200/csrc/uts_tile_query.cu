@@ -20,6 +20,7 @@
 //   * count -> exclusive scan -> emit: the pair arrays are written once, densely, in (view, Gaussian, tile) order.
 #include "uts_internal.cuh"
 #include "uts_scan.cuh"
+#include <cstdlib>
 
 namespace uts {
 
@@ -30,6 +31,7 @@ struct QueryParams {
   int kt, kq, P, V;
   int os;                               // split order of the block-per-Gaussian path
   int n_words;                          // bitmap words = n_tile / 32 (0: block path disabled)
+  int wl_cap;                           // capacity of each of the two block work lists
   int64_t n_tile;
   double rho_q;                         // rho_max(k_q)
   float r_large;                        // discs with R above this go to the block path
@@ -61,7 +63,7 @@ __device__ __forceinline__ bool load_disc(const QueryParams& qp, const float* __
 enum Zone { kOutside = 0, kInside = 1, kPartial = 2 };
 
 // Alg.2's Classify for node (o,p): kOutside = no descendant centre can be within R, kInside = all are.
-__device__ __forceinline__ Zone classify(const QueryParams& qp, const Disc& D, int o, uint64_t p, float& chord) {
+__device__ __forceinline__ Zone classify(const QueryParams& qp, const Disc& D, int o, uint32_t p, float& chord) {
   float cx, cy, cz;
   pix_center_cam_f32(o, p, cx, cy, cz);
   const float dx = D.uf[0] - cx, dy = D.uf[1] - cy, dz = D.uf[2] - cz;
@@ -74,12 +76,12 @@ __device__ __forceinline__ Zone classify(const QueryParams& qp, const Disc& D, i
 }
 
 // The defining predicate at a leaf (order k_q).
-__device__ __forceinline__ bool leaf_inside(const QueryParams& qp, const Disc& D, uint64_t p, float chord) {
+__device__ __forceinline__ bool leaf_inside(const QueryParams& qp, const Disc& D, uint32_t p, float chord) {
   const float t = 2.0f * D.sh;
   if (chord < t - kDelta) return true;
   if (chord > t + kDelta) return false;
   double cx, cy, cz;
-  pix_center_cam(qp.kq, p, cx, cy, cz);
+  pix_center_cam(qp.kq, (uint64_t)p, cx, cy, cz);
   return D.u[0] * cx + D.u[1] * cy + D.u[2] * cz >= D.cosR;
 }
 
@@ -90,8 +92,8 @@ __device__ __forceinline__ bool leaf_inside(const QueryParams& qp, const Disc& D
 // node.  (Left to the compiler, the walk loop's reconvergence point was the loop exit: 2 of 32 lanes active, measured.)
 struct Walker {
   int o, ro;
-  uint64_t p, rp1;
-  __device__ __forceinline__ void start(int ro_, uint64_t rp0, uint64_t rp1_) { o = ro = ro_; p = rp0; rp1 = rp1_; }
+  uint32_t p, rp1;               // a NESTED index at order <= 13 fits 32 bits
+  __device__ __forceinline__ void start(int ro_, uint32_t rp0, uint32_t rp1_) { o = ro = ro_; p = rp0; rp1 = rp1_; }
   // returns true when the walk is finished
   template <class Sink>
   __device__ __forceinline__ bool step(const QueryParams& qp, const Disc& D, Sink& sink) {
@@ -101,7 +103,7 @@ struct Walker {
     bool descend = false;
     if (z != kOutside) {
       if (o <= kt) {
-        if (z == kInside) { const int sh = 2 * (kt - o); sink.add_range((int64_t)(p << sh), (int64_t)((p + 1) << sh)); }
+        if (z == kInside) { const int sh = 2 * (kt - o); sink.add_range((int64_t)p << sh, (int64_t)(p + 1) << sh); }
         else descend = true;
       } else {
         const int64_t tile = (int64_t)(p >> (2 * (o - kt)));
@@ -118,7 +120,7 @@ struct Walker {
     bool finished = false;
     if (descend) { p <<= 2; ++o; }
     else {
-      const int ones = __ffsll((long long)~p) - 1;              // trailing one bits of p
+      const int ones = __ffs((int)~p) - 1;              // trailing one bits of p
       const int up = min(ones >> 1, o - ro);                    // finished last children to climb over
       p >>= 2 * up; o -= up;
       if (o == ro && p == rp1) finished = true; else ++p;
@@ -202,12 +204,12 @@ __global__ void bucket_scan_kernel(uint32_t* __restrict__ hist, uint32_t* __rest
 }
 
 template <bool EMIT>
-__global__ void __launch_bounds__(128)
-tile_query_small_kernel(QueryParams qp, const float* __restrict__ dir, const float* __restrict__ rho, const float* __restrict__ rs,
+__device__ __forceinline__ void
+small_body(int64_t block, const QueryParams& qp, const float* __restrict__ dir, const float* __restrict__ rho, const float* __restrict__ rs,
                         const int32_t* __restrict__ slot_of_tile, const uint32_t* __restrict__ perm, const uint32_t* __restrict__ n_small,
                         uint32_t* __restrict__ counts, const uint64_t* __restrict__ offsets, uint64_t* __restrict__ keys,
                         uint32_t* __restrict__ vals) {
-  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t t = block * blockDim.x + threadIdx.x;
   bool running = t < (int64_t)*n_small;
   const int64_t k = running ? (int64_t)perm[t] : 0;
   if (EMIT && running && offsets[k + 1] == offsets[k]) running = false;
@@ -269,20 +271,20 @@ __global__ void active_words_kernel(const int32_t* __restrict__ slot_of_tile, in
 }
 
 template <bool EMIT>
-__global__ void __launch_bounds__(kLargeThreads)
-tile_query_large_kernel(QueryParams qp, const float* __restrict__ dir, const float* __restrict__ rho, const float* __restrict__ rs,
+__device__ __forceinline__ void
+large_body(int n_blocks, const QueryParams& qp, const float* __restrict__ dir, const float* __restrict__ rho, const float* __restrict__ rs,
                         const uint32_t* __restrict__ active_words, const uint32_t* __restrict__ large_list,
                         const uint32_t* __restrict__ n_large, uint32_t* __restrict__ counts, const uint64_t* __restrict__ offsets,
                         uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
   extern __shared__ uint32_t smem[];
   uint32_t* bits = smem;                         // [n_words]
   uint32_t* pref = smem + qp.n_words;            // [n_words]  exclusive popcount prefix (emit only)
-  uint32_t* work = smem + 2 * qp.n_words;        // [12 * 4^os] partial nodes at the split order
+  uint32_t* work = smem + 2 * qp.n_words;        // [2][wl_cap] boundary nodes, ping-pong
   __shared__ Disc s_disc;
   __shared__ uint32_t s_count, s_next, s_w[kLargeThreads / 32];
   const int n_split = 12 << (2 * qp.os);
   const uint32_t nl = *n_large;
-  for (uint32_t li = blockIdx.x; li < nl; li += gridDim.x) {
+  for (uint32_t li = blockIdx.x; li < nl; li += (uint32_t)n_blocks) {
     const int64_t k = (int64_t)large_list[li];
     __syncthreads();
     if (threadIdx.x == 0) { load_disc(qp, dir, rs, k, s_disc); s_count = 0; s_next = 0; }
@@ -295,18 +297,37 @@ tile_query_large_kernel(QueryParams qp, const float* __restrict__ dir, const flo
     } else {
       for (int node = threadIdx.x; node < n_split; node += kLargeThreads) {
         float chord;
-        const Zone z = classify(qp, D, qp.os, (uint64_t)node, chord);
+        const Zone z = classify(qp, D, qp.os, (uint32_t)node, chord);
         if (z == kInside) { const int sh = 2 * (qp.kt - qp.os); sink.add_range((int64_t)node << sh, (int64_t)(node + 1) << sh); }
         else if (z == kPartial) work[atomicAdd(&s_count, 1u)] = (uint32_t)node;
       }
       __syncthreads();
-      const uint32_t nw = s_count;
+      // breadth-first refinement of the boundary nodes down to tile order while the next level fits the work list: turns a
+      // few large subtrees into many small ones, so that all 256 lanes have walks of a few nodes each
+      uint32_t* cur = work; uint32_t* nxt = work + qp.wl_cap;
+      int level = qp.os;
+      uint32_t nw = s_count;
+      while (level < qp.kt && 4u * nw <= (uint32_t)qp.wl_cap && nw > 0) {
+        __syncthreads();
+        if (threadIdx.x == 0) s_count = 0;
+        __syncthreads();
+        for (uint32_t i = threadIdx.x; i < 4u * nw; i += kLargeThreads) {
+          const uint32_t child = 4u * cur[i >> 2] + (i & 3u);
+          float chord;
+          const Zone z = classify(qp, D, level + 1, child, chord);
+          if (z == kInside) { const int sh = 2 * (qp.kt - level - 1); sink.add_range((int64_t)child << sh, (int64_t)(child + 1) << sh); }
+          else if (z == kPartial) nxt[atomicAdd(&s_count, 1u)] = child;
+        }
+        __syncthreads();
+        nw = s_count; ++level;
+        uint32_t* t = cur; cur = nxt; nxt = t;
+      }
       Walker w;
       bool active = false, exhausted = false;
       while (true) {                                  // every lane does one node per iteration and refills itself when idle
         if (!active && !exhausted) {
           const uint32_t i = atomicAdd(&s_next, 1u);
-          if (i < nw) { w.start(qp.os, (uint64_t)work[i], (uint64_t)work[i]); active = true; }
+          if (i < nw) { w.start(level, cur[i], cur[i]); active = true; }
           else exhausted = true;
         }
         if (!__any_sync(0xffffffffu, active)) break;
@@ -340,6 +361,21 @@ tile_query_large_kernel(QueryParams qp, const float* __restrict__ dir, const flo
       vals[base + r] = gid;
     }
   }
+}
+
+// One launch for both work shapes: the first n_large_blocks blocks run the block-per-Gaussian path (long, few), the others
+// the thread-per-Gaussian path, so the two overlap instead of running back to back.
+template <bool EMIT>
+__global__ void __launch_bounds__(kLargeThreads)
+tile_query_kernel(QueryParams qp, int n_large_blocks, const float* __restrict__ dir, const float* __restrict__ rho,
+                  const float* __restrict__ rs, const int32_t* __restrict__ slot_of_tile, const uint32_t* __restrict__ active_words,
+                  const uint32_t* __restrict__ perm, const uint32_t* __restrict__ n_small, const uint32_t* __restrict__ large_list,
+                  const uint32_t* __restrict__ n_large, uint32_t* __restrict__ counts, const uint64_t* __restrict__ offsets,
+                  uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+  if ((int)blockIdx.x < n_large_blocks)
+    large_body<EMIT>(n_large_blocks, qp, dir, rho, rs, active_words, large_list, n_large, counts, offsets, keys, vals);
+  else
+    small_body<EMIT>((int64_t)blockIdx.x - n_large_blocks, qp, dir, rho, rs, slot_of_tile, perm, n_small, counts, offsets, keys, vals);
 }
 
 }  // namespace uts
@@ -400,10 +436,12 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, uint64_t* 
   for (int o = 0; o <= kMaxOrder; ++o) { qp.rho[o] = (float)rm[o]; qp.sin_hrho[o] = (float)sin(0.5 * rm[o]); qp.cos_hrho[o] = (float)cos(0.5 * rm[o]); }
   qp.os = d.kt < 4 ? d.kt : 4;
   const size_t n_split = (size_t)12 << (2 * qp.os);
-  const size_t large_smem = (2 * (size_t)(d.n_tile / 32) + n_split) * 4;
+  qp.wl_cap = (int)(n_split > 4096 ? n_split : 4096);
+  const size_t large_smem = (2 * (size_t)(d.n_tile / 32) + 2 * (size_t)qp.wl_cap) * 4;
   const bool use_large = d.kt >= 2 && large_smem <= kMaxLargeSmem;
   qp.n_words = use_large ? (int)(d.n_tile / 32) : 0;
-  qp.r_large = (float)(64.0 / sqrt((double)d.n_tile));      // ~1024 tiles: pi R^2 / (4 pi / n_tile)
+  const char* e1__ = getenv("UTS_RLARGE"); const char* e2__ = getenv("UTS_LGRID");
+  qp.r_large = (float)((e1__ ? atof(e1__) : 36.0) / sqrt((double)d.n_tile));      // ~320 tiles (pi R^2 / (4 pi / n_tile)); measured crossover on config 4
 
   const QueryLayout L = query_layout(cfg);
   char* sp = reinterpret_cast<char*>(scratch);
@@ -416,13 +454,14 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, uint64_t* 
   uint32_t* active = reinterpret_cast<uint32_t*>(sp + L.active);
   uint64_t* block_sums = reinterpret_cast<uint64_t*>(sp + L.scan);
   const uint32_t* active_arg = nullptr;
-  const unsigned qgrid = (unsigned)((n + 127) / 128);
-  const unsigned lgrid = (unsigned)(sm_count() * 4);
+  const unsigned qgrid = (unsigned)((n + kLargeThreads - 1) / kLargeThreads);
+  const int lgrid = use_large ? sm_count() * (e2__ ? atoi(e2__) : 2) : 0;
+  const size_t dyn_smem = use_large ? large_smem : 0;
   if (use_large) {
     static bool attr_set = false;
     if (!attr_set) {
-      UTS_CUDA(cudaFuncSetAttribute(tile_query_large_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxLargeSmem));
-      UTS_CUDA(cudaFuncSetAttribute(tile_query_large_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxLargeSmem));
+      UTS_CUDA(cudaFuncSetAttribute(tile_query_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxLargeSmem));
+      UTS_CUDA(cudaFuncSetAttribute(tile_query_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxLargeSmem));
       attr_set = true;
     }
     if (mask.slot_of_tile) {
@@ -439,27 +478,18 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, uint64_t* 
   UTS_LAUNCH_CHECK();
   classify_kernel<1><<<cgrid, 256, 0, s>>>(qp, in.rs, in.flags, counts, list, n_large, hist, perm);
   UTS_LAUNCH_CHECK();
-  tile_query_small_kernel<false><<<qgrid, 128, 0, s>>>(qp, in.dir, in.rho, in.rs, mask.slot_of_tile, perm, n_small, counts, nullptr, nullptr,
-                                                       nullptr);
+  tile_query_kernel<false><<<qgrid + lgrid, kLargeThreads, dyn_smem, s>>>(qp, lgrid, in.dir, in.rho, in.rs, mask.slot_of_tile, active_arg, perm,
+                                                                         n_small, list, n_large, counts, nullptr, nullptr, nullptr);
   UTS_LAUNCH_CHECK();
-  if (use_large) {
-    tile_query_large_kernel<false><<<lgrid, kLargeThreads, large_smem, s>>>(qp, in.dir, in.rho, in.rs, active_arg, list, n_large, counts,
-                                                                            nullptr, nullptr, nullptr);
-    UTS_LAUNCH_CHECK();
-  }
   if ((st = exclusive_scan_u32(counts, n, offsets, block_sums, s))) return st;
   UTS_CUDA(cudaMemcpyAsync(h_n_pairs, offsets + n, sizeof(uint64_t), cudaMemcpyDeviceToHost, s));
   UTS_CUDA(cudaStreamSynchronize(s));
   if (!keys) return UTS_OK;
   if (*h_n_pairs > capacity) return UTS_ERR_CAPACITY;
   if (*h_n_pairs == 0) return UTS_OK;
-  tile_query_small_kernel<true><<<qgrid, 128, 0, s>>>(qp, in.dir, in.rho, in.rs, mask.slot_of_tile, perm, n_small, nullptr, offsets, keys, vals);
+  tile_query_kernel<true><<<qgrid + lgrid, kLargeThreads, dyn_smem, s>>>(qp, lgrid, in.dir, in.rho, in.rs, mask.slot_of_tile, active_arg, perm,
+                                                                        n_small, list, n_large, nullptr, offsets, keys, vals);
   UTS_LAUNCH_CHECK();
-  if (use_large) {
-    tile_query_large_kernel<true><<<lgrid, kLargeThreads, large_smem, s>>>(qp, in.dir, in.rho, in.rs, active_arg, list, n_large, nullptr,
-                                                                           offsets, keys, vals);
-    UTS_LAUNCH_CHECK();
-  }
   return UTS_OK;
 }
 

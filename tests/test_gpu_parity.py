@@ -199,7 +199,7 @@ def test_tile_query_other_refinements(refine):
 
 @pytest.mark.parametrize("cfg_id,order,refine", [(4, 9, 2), (3, 9, 2), (4, 8, 1), (5, 10, 2)])
 def test_tile_query_block_path_large_discs(cfg_id, order, refine):
-    """Discs of thousands of tiles take the block-per-Gaussian bitmap path (R > 64/sqrt(N_tile)); with and without a mask."""
+    """Discs of thousands of tiles take the block-per-Gaussian bitmap path (R > 36/sqrt(N_tile)); with and without a mask."""
     B, R = _gpu()
     scene = small_scene(cfg_id, 300, order, n_views=1)
     scene["scales"][::2] *= 30.0                   # every other Gaussian becomes a very large disc
@@ -207,7 +207,7 @@ def test_tile_query_block_path_large_discs(cfg_id, order, refine):
     oc = ocfg(scene, query_refine_log2=refine)
     bits, act, slot = oracle_mask(oc, scene)
     pr = orc.preprocess(oc, scene["means"], scene["scales"], scene["quats"], scene["opac"], scene["sh"], scene["W"], scene["b"])
-    assert (pr.rs[0] + orc.rho_max_closed(oc.tile_order + refine) > 64.0 / np.sqrt(oc.n_tiles)).sum() > 8
+    assert (pr.rs[0] + orc.rho_max_closed(oc.tile_order + refine) > 36.0 / np.sqrt(oc.n_tiles)).sum() > 8
     off, keys, vals, info = orc.tile_query(oc, pr, slot)
     assert info["min_margin"] > 1e-12
     cfg = _cfg(R, scene, query_refine_log2=refine)

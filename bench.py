@@ -27,7 +27,7 @@ from paper_2606_29794_b200 import scenes  # noqa: E402  (input generator: no met
 
 METRIC = "healpix_px_per_s_fwd_bwd"
 UNIT = "px/s"
-STAGES = ["preprocess", "tile_query", "sort", "tile_ranges", "render_fwd", "render_bwd", "preprocess_bwd"]
+STAGES = ["preprocess", "depth_order", "tile_query", "sort", "tile_ranges", "render_fwd", "render_bwd", "preprocess_bwd"]
 # FP32 operations one evaluated (Gaussian, pixel) pair costs in the blend kernels (counted from the
 # arithmetic of Eq.6 + SphericalOffset as implemented, FMA = 2): forward 46, backward 118.
 FLOP_FWD, FLOP_BWD = 46, 118
@@ -199,13 +199,14 @@ def run_ours(args):
             if events is not None:
                 events[i].record(stream)
         mark(0); r.preprocess(g, views)
-        mark(1); r.tile_query()
-        mark(2); r.sort()
-        mark(3); r.tile_ranges()
-        mark(4); r.render_fwd()
-        mark(5); r.render_bwd(gcol)
-        mark(6); r.preprocess_bwd(g, views)
-        mark(7)
+        mark(1); r.depth_order()
+        mark(2); r.tile_query()
+        mark(3); r.sort()
+        mark(4); r.tile_ranges()
+        mark(5); r.render_fwd()
+        mark(6); r.render_bwd(gcol)
+        mark(7); r.preprocess_bwd(g, views)
+        mark(8)
 
     for _ in range(args.warmup):
         step()
@@ -213,7 +214,7 @@ def run_ours(args):
     if world > 1:
         dist.barrier()
     sampler = ClockSampler(local); sampler.start()
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(8)] for _ in range(args.steps)]
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(9)] for _ in range(args.steps)]
     t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
     t0.record(stream)
@@ -224,8 +225,8 @@ def run_ours(args):
     clocks = sampler.stop()
     total_ms = t0.elapsed_time(t1)
     ms_step = total_ms / args.steps
-    stage_ms = {STAGES[i]: float(np.mean([ev[k][i].elapsed_time(ev[k][i + 1]) for k in range(args.steps)])) for i in range(7)}
-    ms_fwd = sum(stage_ms[s] for s in STAGES[:5])
+    stage_ms = {STAGES[i]: float(np.mean([ev[k][i].elapsed_time(ev[k][i + 1]) for k in range(args.steps)])) for i in range(8)}
+    ms_fwd = sum(stage_ms[s] for s in STAGES[:6])
 
     # work counters from the forward outputs (measurement plumbing): entries each pixel evaluated
     lens = (r.ranges[:, 1] - r.ranges[:, 0])
@@ -284,7 +285,7 @@ def run_ours(args):
         roof = dict(kernel=dom, bound="alu", achieved=ach, peak=fp32_peak, unit="TFLOP/s", frac=ach / fp32_peak, traffic=None,
                     peak_source="derived: 148 SM x 128 FP32 lanes x 2 x sm_max_mhz")
     else:
-        per_pair = {"sort": 32.0 * (4 + 2), "tile_query": 12.0, "tile_ranges": 8.0}.get(dom)
+        per_pair = {"sort": 32.0 * ((max(1, (V * cfg.n_tiles - 1)).bit_length() + 7) // 8), "tile_query": 12.0, "tile_ranges": 8.0}.get(dom)
         byts = per_pair * n_pairs if per_pair else P * V * (44 + 12 * M + 57)
         ach = byts / (stage_ms[dom] * 1e-3) / 1e9
         roof = dict(kernel=dom, bound="hbm", achieved=ach, peak=peaks["hbm_gbs"], unit="GB/s", frac=ach / peaks["hbm_gbs"], traffic=None,
@@ -297,7 +298,7 @@ def run_ours(args):
             per_kernel[s_] = dict(ms=ms, tflops=ev_b * FLOP_BWD / (ms * 1e-3) / 1e12, frac_fp32_peak=ev_b * FLOP_BWD / (ms * 1e-3) / 1e12 / fp32_peak)
         else:
             byts = {"preprocess": P * V * (44 + 12 * M + 57), "preprocess_bwd": P * (44 + 12 * M + V * 33 + 40 + 12 * M),
-                    "tile_query": P * V * 2 * 21 + 8 * P * V + 12 * n_pairs, "sort": 32.0 * n_pairs * (4 + ((max(1, (V * cfg.n_tiles - 1)).bit_length() + 7) // 8)),
+                    "depth_order": P * V * (4 + 5 * 32 + 16), "tile_query": P * V * 2 * 21 + 8 * P * V + 12 * n_pairs, "sort": 32.0 * n_pairs * ((max(1, (V * cfg.n_tiles - 1)).bit_length() + 7) // 8),
                     "tile_ranges": 8.0 * n_pairs + 16 * V * cfg.n_tiles}[s_]
             per_kernel[s_] = dict(ms=ms, gbs=byts / (ms * 1e-3) / 1e9, frac_hbm_peak=byts / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
 
@@ -312,8 +313,11 @@ def run_ours(args):
                 e2e=dict(value=world * n_pix_active / (e2e_ms_max * 1e-3), unit=UNIT, ms_per_step=e2e_ms_max, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h),
                 gpu_launches=0)
     # launches of our kernels per step: 1 preprocess + (1 count + 3 scan + 1 emit) + passes*(1 + 3 + 1) (+1 copy) + 1 ranges + 1 fwd + 1 bwd + 1 pre-bwd
-    passes = 4 + ((max(1, (V * cfg.n_tiles - 1)).bit_length() + 7) // 8)
-    line["gpu_launches"] = args.steps * (1 + 5 + passes * 5 + (passes % 2) + 1 + 1 + 1 + 1)
+    passes = (max(1, (V * cfg.n_tiles - 1)).bit_length() + 7) // 8          # pair sort: (view,tile) bytes only
+    dpass = 4 + ((max(1, V - 1).bit_length() + 7) // 8 if V > 1 else 0)     # depth order of the Gaussians
+    # preprocess 1; depth order 1 + 5/pass (+copy) + 1; query 3 classify + 1 count + 3 scan + 1 emit; sort 5/pass (+copy);
+    # ranges 1; blend fwd 1; blend bwd 1; preprocess bwd 1
+    line["gpu_launches"] = args.steps * (1 + (2 + dpass * 5 + dpass % 2) + 8 + (passes * 5 + passes % 2) + 4)
     if not args.no_cpu_baseline:
         t, desc, meta = oracle_sample(args.config, seed=0)
         line["cpu_baseline"] = dict(value=meta["n_pix"] / t, unit=UNIT, cores=1, kind="oracle", sample=desc)

@@ -3,6 +3,7 @@
  * One entry point per stage of UniTriSplat's Alg.1 and of its backward:
  *
  *   uts_preprocess      Alg.1 l.2-8   (Eq.1-2): projection to the unit sphere, Sigma_arc, conic, r_s, colour
+ *   uts_depth_order     (optional) radial-depth order of the Gaussians, lets the sort skip its depth passes
  *   uts_tile_query      Alg.1 l.9-14  (Alg.2): NESTED tile query, emits ((tile,rho),i) pairs
  *   uts_sort            Alg.1 l.15: stable radix sort of the pairs by (tile, radial depth)
  *   uts_tile_ranges     Alg.1 l.16: per-tile [start,end)
@@ -99,24 +100,34 @@ typedef struct {
  * (rho <= r_near, non-finite input, det(Sigma_arc) <= 0) are written as zeros with flags bit0 set. */
 int uts_preprocess(const uts_config* cfg, uts_gaussians g, uts_views views, uts_proj out, void* stream);
 
+/* Optional, Alg.1 l.15 moved ahead of the query: emit_rank[v*P+i] = position of (v,i) in the
+ * stable order by (view, float_bits(rho), i).  Passing it to uts_tile_query makes the pairs come out already ordered by radial
+ * depth, so that uts_sort(depth_presorted = 1) only has to run its (view,tile) passes; the sorted result is bit-identical.
+ * scratch: uts_depth_order_scratch_bytes(cfg) bytes, 256-byte aligned. */
+int uts_depth_order(const uts_config* cfg, const float* rho /*[V,P]*/, uint32_t* emit_rank /*[V*P]*/, void* scratch,
+                    size_t scratch_bytes, void* stream);
+size_t uts_depth_order_scratch_bytes(const uts_config* cfg);
+
 /* Alg.1 l.9-14 with Alg.2 (reading A6).  The tile set of (v,i) is
  *     { q >> 2(k_q-k_t) : q an order-k_q NESTED pixel with  u . centre(q) >= cos(min(pi, r_s + rho_max(k_q))) } ∩ active tiles,
- * evaluated in double precision.  Pairs are written in (view, Gaussian, tile) ascending order:
+ * evaluated in double precision.  Pairs are written Gaussian by Gaussian, tiles ascending inside a Gaussian:
  *     keys[j] = ((v*N_tile + tile) << 32) | float_bits(rho[v,i]),   vals[j] = i.
- * offsets[V*P+1] (exclusive scan of the per-(v,i) counts) is always written.  The call synchronises `stream`
- * and writes the pair count to *h_n_pairs (host).  keys == NULL: count only.  If the count exceeds `capacity`
- * nothing is emitted and UTS_ERR_CAPACITY is returned (*h_n_pairs holds the needed capacity).
+ * emit_rank == NULL: Gaussians in (view, Gaussian id) order (slot of (v,i) = v*P+i).  Otherwise slot = emit_rank[v*P+i]
+ * (a permutation of 0..V*P-1, e.g. from uts_depth_order).  offsets[V*P+1] (exclusive scan of the per-slot counts) is always
+ * written.  The call synchronises `stream` and writes the pair count to *h_n_pairs (host).  keys == NULL: count only.
+ * If the count exceeds `capacity` nothing is emitted and UTS_ERR_CAPACITY is returned (*h_n_pairs = needed capacity).
  * scratch: uts_tile_query_scratch_bytes(cfg) bytes, 256-byte aligned. */
-int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, uint64_t* offsets, uint64_t* keys,
-                   uint32_t* vals, uint64_t capacity, uint64_t* h_n_pairs, void* scratch, size_t scratch_bytes,
-                   void* stream);
+int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint32_t* emit_rank, uint64_t* offsets,
+                   uint64_t* keys, uint32_t* vals, uint64_t capacity, uint64_t* h_n_pairs, void* scratch,
+                   size_t scratch_bytes, void* stream);
 size_t uts_tile_query_scratch_bytes(const uts_config* cfg);
 
-/* Alg.1 l.15.  Stable ascending LSD radix sort on the 64-bit key (ties keep emission order = ascending
- * Gaussian id, reading A9).  Result is left in keys/vals; keys_tmp/vals_tmp are ping-pong buffers of the same
- * size.  scratch: uts_sort_scratch_bytes(n_pairs) bytes, 256-byte aligned. */
+/* Alg.1 l.15.  Stable ascending LSD radix sort on the 64-bit key (ties keep emission order; with emission in Gaussian-id
+ * or depth order that is ascending Gaussian id, reading A9).  depth_presorted != 0: the pairs were emitted through
+ * uts_depth_order's emit_rank, only the (view,tile) bytes are sorted.  Result is left in keys/vals; keys_tmp/vals_tmp are
+ * ping-pong buffers of the same size.  scratch: uts_sort_scratch_bytes(n_pairs) bytes, 256-byte aligned. */
 int uts_sort(const uts_config* cfg, uint64_t n_pairs, uint64_t* keys, uint32_t* vals, uint64_t* keys_tmp,
-             uint32_t* vals_tmp, void* scratch, size_t scratch_bytes, void* stream);
+             uint32_t* vals_tmp, int depth_presorted, void* scratch, size_t scratch_bytes, void* stream);
 size_t uts_sort_scratch_bytes(uint64_t n_pairs);
 
 /* Alg.1 l.16.  ranges[(v*N_tile + tile)*2 + {0,1}] = [start,end) in the sorted arrays; empty tiles get (0,0). */

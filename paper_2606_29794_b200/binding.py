@@ -19,7 +19,7 @@ UTS_OK, UTS_ERR_INVALID_ARG, UTS_ERR_CAPACITY, UTS_ERR_CUDA, UTS_ERR_UNSUPPORTED
 
 # every symbol include/uts.h declares
 SYMBOLS = [
-    "uts_preprocess", "uts_tile_query", "uts_tile_query_scratch_bytes", "uts_sort", "uts_sort_scratch_bytes",
+    "uts_preprocess", "uts_depth_order", "uts_depth_order_scratch_bytes", "uts_tile_query", "uts_tile_query_scratch_bytes", "uts_sort", "uts_sort_scratch_bytes",
     "uts_tile_ranges", "uts_render_fwd", "uts_render_bwd", "uts_preprocess_bwd", "uts_build_mask", "uts_pixel_centers",
     "uts_rho_max_table", "uts_host_workspace_bytes", "uts_host_forward_backward", "uts_last_cuda_error", "uts_strerror",
     "uts_version",
@@ -99,7 +99,7 @@ def lib():
         L = C.CDLL(LIB_PATH)
         L.uts_strerror.restype = C.c_char_p
         L.uts_version.restype = C.c_char_p
-        for n in ("uts_tile_query_scratch_bytes", "uts_sort_scratch_bytes", "uts_host_workspace_bytes"):
+        for n in ("uts_depth_order_scratch_bytes", "uts_tile_query_scratch_bytes", "uts_sort_scratch_bytes", "uts_host_workspace_bytes"):
             getattr(L, n).restype = C.c_size_t
         L.uts_sort_scratch_bytes.argtypes = [C.c_uint64]
         L.uts_host_workspace_bytes.argtypes = [C.POINTER(CConfig), C.c_int, C.c_uint64]
@@ -187,11 +187,22 @@ def uts_tile_query_scratch_bytes(cfg: Config) -> int:
     return int(lib().uts_tile_query_scratch_bytes(C.byref(c)))
 
 
-def uts_tile_query(cfg: Config, proj: Proj, mask: Mask, offsets, keys, vals, capacity: int, scratch, stream=None) -> int:
+def uts_depth_order_scratch_bytes(cfg: Config) -> int:
+    c = cfg.c()
+    return int(lib().uts_depth_order_scratch_bytes(C.byref(c)))
+
+
+def uts_depth_order(cfg: Config, rho, emit_rank, scratch, stream=None):
+    c = cfg.c()
+    _check(lib().uts_depth_order(C.byref(c), _ptr(rho, torch.float32), _ptr(emit_rank, torch.int32), _ptr(scratch),
+                                 C.c_size_t(scratch.numel() * scratch.element_size()), _stream(stream)), "uts_depth_order")
+
+
+def uts_tile_query(cfg: Config, proj: Proj, mask: Mask, offsets, keys, vals, capacity: int, scratch, emit_rank=None, stream=None) -> int:
     """Returns the pair count.  keys=None: count only.  Raises UtsError(UTS_ERR_CAPACITY) with .needed set."""
     c = cfg.c()
     n = C.c_uint64(0)
-    st = lib().uts_tile_query(C.byref(c), proj.c(), mask.c(), _ptr(offsets, torch.int64), _ptr(keys, torch.int64), _ptr(vals, torch.int32),
+    st = lib().uts_tile_query(C.byref(c), proj.c(), mask.c(), _ptr(emit_rank, torch.int32), _ptr(offsets, torch.int64), _ptr(keys, torch.int64), _ptr(vals, torch.int32),
                               C.c_uint64(capacity), C.byref(n), _ptr(scratch), C.c_size_t(scratch.numel() * scratch.element_size()),
                               _stream(stream))
     if st == UTS_ERR_CAPACITY:
@@ -204,11 +215,11 @@ def uts_sort_scratch_bytes(n_pairs: int) -> int:
     return int(lib().uts_sort_scratch_bytes(C.c_uint64(n_pairs)))
 
 
-def uts_sort(cfg: Config, n_pairs: int, keys, vals, keys_tmp, vals_tmp, scratch, stream=None):
+def uts_sort(cfg: Config, n_pairs: int, keys, vals, keys_tmp, vals_tmp, scratch, depth_presorted=False, stream=None):
     c = cfg.c()
     _check(lib().uts_sort(C.byref(c), C.c_uint64(n_pairs), _ptr(keys, torch.int64), _ptr(vals, torch.int32), _ptr(keys_tmp, torch.int64),
-                          _ptr(vals_tmp, torch.int32), _ptr(scratch), C.c_size_t(scratch.numel() * scratch.element_size()),
-                          _stream(stream)), "uts_sort")
+                          _ptr(vals_tmp, torch.int32), C.c_int(1 if depth_presorted else 0), _ptr(scratch),
+                          C.c_size_t(scratch.numel() * scratch.element_size()), _stream(stream)), "uts_sort")
 
 
 def uts_tile_ranges(cfg: Config, n_pairs: int, keys, ranges, stream=None):

@@ -20,8 +20,9 @@ struct HostLayout {
   uts_proj proj;
   uint64_t *offsets, *keys, *keys_tmp, *ranges;
   uint32_t *vals, *vals_tmp, *n_last;
-  void *tq_scratch, *sort_scratch;
-  size_t tq_bytes, sort_bytes;
+  void *tq_scratch, *sort_scratch, *do_scratch;
+  size_t tq_bytes, sort_bytes, do_bytes;
+  uint32_t* emit_rank;
   float *color, *alpha, *trans, *g_color;
   float *g_rgb, *g_conic, *g_mu2, *g_opac, *g_means, *g_scales, *g_quats, *g_sh;
   size_t total;
@@ -40,6 +41,8 @@ static HostLayout layout(const uts_config* cfg, int64_t n_slot, uint64_t cap, ch
   L.proj.flags = B.take<uint8_t>(VP);
   L.offsets = B.take<uint64_t>(VP + 1);
   L.tq_bytes = uts_tile_query_scratch_bytes(cfg); L.tq_scratch = B.take<char>(L.tq_bytes);
+  L.do_bytes = uts_depth_order_scratch_bytes(cfg); L.do_scratch = B.take<char>(L.do_bytes);
+  L.emit_rank = B.take<uint32_t>(VP);
   L.keys = B.take<uint64_t>(cap); L.keys_tmp = B.take<uint64_t>(cap);
   L.vals = B.take<uint32_t>(cap); L.vals_tmp = B.take<uint32_t>(cap);
   L.sort_bytes = uts_sort_scratch_bytes(cap); L.sort_scratch = B.take<char>(L.sort_bytes);
@@ -96,10 +99,11 @@ int uts_host_forward_backward(const uts_config* cfg, const float* h_means, const
   uts_gaussians g{L.means, L.scales, L.quats, L.opac, L.sh};
   uts_views vw{L.W, L.b};
   if ((st = uts_preprocess(cfg, g, vw, L.proj, stream))) return st;
-  if ((st = uts_tile_query(cfg, L.proj, mask, L.offsets, L.keys, L.vals, pair_capacity, h_n_pairs, L.tq_scratch, L.tq_bytes, stream)))
+  if ((st = uts_depth_order(cfg, L.proj.rho, L.emit_rank, L.do_scratch, L.do_bytes, stream))) return st;
+  if ((st = uts_tile_query(cfg, L.proj, mask, L.emit_rank, L.offsets, L.keys, L.vals, pair_capacity, h_n_pairs, L.tq_scratch, L.tq_bytes, stream)))
     return st;
   const uint64_t n = *h_n_pairs;
-  if ((st = uts_sort(cfg, n, L.keys, L.vals, L.keys_tmp, L.vals_tmp, L.sort_scratch, L.sort_bytes, stream))) return st;
+  if ((st = uts_sort(cfg, n, L.keys, L.vals, L.keys_tmp, L.vals_tmp, 1, L.sort_scratch, L.sort_bytes, stream))) return st;
   if ((st = uts_tile_ranges(cfg, n, L.keys, L.ranges, stream))) return st;
   if ((st = uts_render_fwd(cfg, L.proj, mask, L.ranges, L.vals, L.color, L.alpha, L.trans, L.n_last, stream))) return st;
   UTS_CUDA(cudaMemcpyAsync(h_color, L.color, 3 * npx * f, cudaMemcpyDeviceToHost, s));

@@ -170,28 +170,25 @@ size_t uts_sort_scratch_bytes(uint64_t n_pairs) {
   return (size_t)(((m * 4 + 255) / 256) * 256 + ((m + 1) * 8 + 255) / 256 * 256) + scan_scratch_bytes((int64_t)m);
 }
 
-int uts_sort(const uts_config* cfg, uint64_t n_pairs, uint64_t* keys, uint32_t* vals, uint64_t* keys_tmp, uint32_t* vals_tmp,
-             void* scratch, size_t scratch_bytes, void* stream) {
-  int st = check_config(cfg);
-  if (st) return st;
-  if (n_pairs == 0) return UTS_OK;
-  if (!keys || !vals || !keys_tmp || !vals_tmp || !scratch) return UTS_ERR_INVALID_ARG;
-  if (scratch_bytes < uts_sort_scratch_bytes(n_pairs) || ((uintptr_t)scratch & 255)) return UTS_ERR_INVALID_ARG;
-  if (n_pairs > ((uint64_t)1 << 40)) return UTS_ERR_UNSUPPORTED;
-  cudaStream_t s = (cudaStream_t)stream;
+}  // extern "C"
+
+namespace uts {
+// LSD passes over key bytes [first_byte, first_byte + n_bytes); result left in keys/vals.
+static int radix_sort_bytes(uint64_t n_pairs, uint64_t* keys, uint32_t* vals, uint64_t* keys_tmp, uint32_t* vals_tmp, void* scratch,
+                            int first_byte, int n_bytes, cudaStream_t s) {
   const uint32_t nb = (uint32_t)((n_pairs + kSortTile - 1) / kSortTile);
   const uint64_t m = (uint64_t)nb * kRadix;
   char* sp = reinterpret_cast<char*>(scratch);
   uint32_t* counts = reinterpret_cast<uint32_t*>(sp);            sp += ((m * 4 + 255) / 256) * 256;
   uint64_t* offs = reinterpret_cast<uint64_t*>(sp);              sp += (((m + 1) * 8 + 255) / 256) * 256;
   uint64_t* block_sums = reinterpret_cast<uint64_t*>(sp);
-  const int n_pass = 4 + (tile_bits_of(cfg) + 7) / 8;
   uint64_t* kin = keys; uint32_t* vin = vals; uint64_t* kout = keys_tmp; uint32_t* vout = vals_tmp;
-  for (int pass = 0; pass < n_pass; ++pass) {
-    const int shift = 8 * pass;
+  for (int pass = 0; pass < n_bytes; ++pass) {
+    const int shift = 8 * (first_byte + pass);
     sort_upsweep<<<nb, kSortThreads, 0, s>>>(kin, n_pairs, shift, nb, counts);
     UTS_LAUNCH_CHECK();
-    if ((st = exclusive_scan_u32(counts, (int64_t)m, offs, block_sums, s))) return st;
+    int st = exclusive_scan_u32(counts, (int64_t)m, offs, block_sums, s);
+    if (st) return st;
     sort_downsweep<<<nb, kSortThreads, 0, s>>>(kin, vin, kout, vout, n_pairs, shift, nb, offs);
     UTS_LAUNCH_CHECK();
     uint64_t* tk = kin; kin = kout; kout = tk;
@@ -201,6 +198,65 @@ int uts_sort(const uts_config* cfg, uint64_t n_pairs, uint64_t* keys, uint32_t* 
     copy_pairs<<<sm_count() * 8, 256, 0, s>>>(kin, vin, keys, vals, n_pairs);
     UTS_LAUNCH_CHECK();
   }
+  return UTS_OK;
+}
+
+// keys[k] = (view << 32) | float_bits(rho[k]),  vals[k] = k
+__global__ void depth_keys_kernel(const float* __restrict__ rho, int64_t n, int P, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  keys[k] = ((uint64_t)(k / P) << 32) | (uint64_t)__float_as_uint(__ldg(rho + k));
+  vals[k] = (uint32_t)k;
+}
+__global__ void invert_kernel(const uint32_t* __restrict__ order, int64_t n, uint32_t* __restrict__ rank) {
+  const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j < n) rank[order[j]] = (uint32_t)j;
+}
+}  // namespace uts
+
+extern "C" {
+
+int uts_sort(const uts_config* cfg, uint64_t n_pairs, uint64_t* keys, uint32_t* vals, uint64_t* keys_tmp, uint32_t* vals_tmp,
+             int depth_presorted, void* scratch, size_t scratch_bytes, void* stream) {
+  int st = check_config(cfg);
+  if (st) return st;
+  if (n_pairs == 0) return UTS_OK;
+  if (!keys || !vals || !keys_tmp || !vals_tmp || !scratch) return UTS_ERR_INVALID_ARG;
+  if (scratch_bytes < uts_sort_scratch_bytes(n_pairs) || ((uintptr_t)scratch & 255)) return UTS_ERR_INVALID_ARG;
+  if (n_pairs > ((uint64_t)1 << 40)) return UTS_ERR_UNSUPPORTED;
+  const int tile_bytes = (tile_bits_of(cfg) + 7) / 8;
+  // stable LSD: when the pairs already arrive in (view, depth, id) order only the (view, tile) bytes need sorting
+  return depth_presorted ? radix_sort_bytes(n_pairs, keys, vals, keys_tmp, vals_tmp, scratch, 4, tile_bytes, (cudaStream_t)stream)
+                         : radix_sort_bytes(n_pairs, keys, vals, keys_tmp, vals_tmp, scratch, 0, 4 + tile_bytes, (cudaStream_t)stream);
+}
+
+size_t uts_depth_order_scratch_bytes(const uts_config* cfg) {
+  if (check_config(cfg) != UTS_OK) return 0;
+  const uint64_t n = (uint64_t)cfg->n_gauss * cfg->n_views;
+  return (size_t)(2 * ((n * 8 + 255) / 256 * 256) + 2 * ((n * 4 + 255) / 256 * 256)) + uts_sort_scratch_bytes(n) + 256;
+}
+
+int uts_depth_order(const uts_config* cfg, const float* rho, uint32_t* emit_rank, void* scratch, size_t scratch_bytes, void* stream) {
+  int st = check_config(cfg);
+  if (st) return st;
+  const int64_t n = (int64_t)cfg->n_gauss * cfg->n_views;
+  if (n == 0) return UTS_OK;
+  if (!rho || !emit_rank || !scratch) return UTS_ERR_INVALID_ARG;
+  if (scratch_bytes < uts_depth_order_scratch_bytes(cfg) || ((uintptr_t)scratch & 255)) return UTS_ERR_INVALID_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  char* sp = reinterpret_cast<char*>(scratch);
+  const size_t kb = ((size_t)n * 8 + 255) / 256 * 256, vb = ((size_t)n * 4 + 255) / 256 * 256;
+  uint64_t* keys = reinterpret_cast<uint64_t*>(sp); sp += kb;
+  uint64_t* keys_tmp = reinterpret_cast<uint64_t*>(sp); sp += kb;
+  uint32_t* vals = reinterpret_cast<uint32_t*>(sp); sp += vb;
+  uint32_t* vals_tmp = reinterpret_cast<uint32_t*>(sp); sp += vb;
+  depth_keys_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(rho, n, cfg->n_gauss, keys, vals);
+  UTS_LAUNCH_CHECK();
+  int view_bits = 0;
+  while ((1 << view_bits) < cfg->n_views) ++view_bits;
+  if ((st = radix_sort_bytes((uint64_t)n, keys, vals, keys_tmp, vals_tmp, sp, 0, 4 + (view_bits + 7) / 8, s))) return st;
+  invert_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(vals, n, emit_rank);
+  UTS_LAUNCH_CHECK();
   return UTS_OK;
 }
 

@@ -166,7 +166,7 @@ template <int WHICH>
 __global__ void __launch_bounds__(256)
 classify_kernel(QueryParams qp, const float* __restrict__ rs, const uint8_t* __restrict__ flags, uint32_t* __restrict__ counts,
                 uint32_t* __restrict__ large_list, uint32_t* __restrict__ n_large, uint32_t* __restrict__ hist /*[64] counts, then cursors*/,
-                uint32_t* __restrict__ perm) {
+                uint32_t* __restrict__ perm, const uint32_t* __restrict__ emit_rank) {
   __shared__ uint32_t s_hist[kBuckets];
   if (threadIdx.x < kBuckets) s_hist[threadIdx.x] = 0;
   __syncthreads();
@@ -174,7 +174,7 @@ classify_kernel(QueryParams qp, const float* __restrict__ rs, const uint8_t* __r
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   int b = -1;
   if (k < n) {
-    if (__ldg(flags + k) & 1) { if (WHICH == 0) counts[k] = 0; }
+    if (__ldg(flags + k) & 1) { if (WHICH == 0) counts[emit_rank ? emit_rank[k] : k] = 0; }
     else {
       const float R32 = fminf(3.14159274f, __ldg(rs + k) + (float)qp.rho_q);
       if (qp.n_words > 0 && R32 > qp.r_large) { if (WHICH == 0) large_list[atomicAdd(n_large, 1u)] = (uint32_t)k; }
@@ -207,12 +207,14 @@ template <bool EMIT>
 __device__ __forceinline__ void
 small_body(int64_t block, const QueryParams& qp, const float* __restrict__ dir, const float* __restrict__ rho, const float* __restrict__ rs,
                         const int32_t* __restrict__ slot_of_tile, const uint32_t* __restrict__ perm, const uint32_t* __restrict__ n_small,
+           const uint32_t* __restrict__ emit_rank,
                         uint32_t* __restrict__ counts, const uint64_t* __restrict__ offsets, uint64_t* __restrict__ keys,
                         uint32_t* __restrict__ vals) {
   const int64_t t = block * blockDim.x + threadIdx.x;
   bool running = t < (int64_t)*n_small;
   const int64_t k = running ? (int64_t)perm[t] : 0;
-  if (EMIT && running && offsets[k + 1] == offsets[k]) running = false;
+  const int64_t slot = emit_rank ? (int64_t)emit_rank[k] : k;     // position of this Gaussian in the emission order
+  if (EMIT && running && offsets[slot + 1] == offsets[slot]) running = false;
   Disc D;
   ThreadSink<EMIT> sink;
   sink.count = 0; sink.last_tile = -1; sink.slot_of_tile = slot_of_tile; sink.keys = keys; sink.vals = vals;
@@ -221,7 +223,7 @@ small_body(int64_t block, const QueryParams& qp, const float* __restrict__ dir, 
   if (running) {
     load_disc(qp, dir, rs, k, D);
     const int v = (int)(k / qp.P);
-    sink.base = EMIT ? offsets[k] : 0;
+    sink.base = EMIT ? offsets[slot] : 0;
     sink.key_hi_base = (uint64_t)v * (uint64_t)qp.n_tile;
     sink.depth_bits = __float_as_uint(__ldg(rho + k));                       // reading A10
     sink.gid = (uint32_t)(k - (int64_t)v * qp.P);
@@ -232,7 +234,7 @@ small_body(int64_t block, const QueryParams& qp, const float* __restrict__ dir, 
   while (__any_sync(0xffffffffu, running)) {
     if (running) running = !w.step(qp, D, sink);
   }
-  if (!EMIT && valid) counts[k] = sink.count;
+  if (!EMIT && valid) counts[slot] = sink.count;
 }
 
 // -------------------------------------------------------------------------------------- block-per-Gaussian path
@@ -273,7 +275,7 @@ __global__ void active_words_kernel(const int32_t* __restrict__ slot_of_tile, in
 template <bool EMIT>
 __device__ __forceinline__ void
 large_body(int n_blocks, const QueryParams& qp, const float* __restrict__ dir, const float* __restrict__ rho, const float* __restrict__ rs,
-                        const uint32_t* __restrict__ active_words, const uint32_t* __restrict__ large_list,
+                        const uint32_t* __restrict__ active_words, const uint32_t* __restrict__ emit_rank, const uint32_t* __restrict__ large_list,
                         const uint32_t* __restrict__ n_large, uint32_t* __restrict__ counts, const uint64_t* __restrict__ offsets,
                         uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
   extern __shared__ uint32_t smem[];
@@ -346,12 +348,13 @@ large_body(int n_blocks, const QueryParams& qp, const float* __restrict__ dir, c
     }
     uint32_t before;
     const uint32_t total = block_sum_u32(mine, s_w, before);
-    if (!EMIT) { if (threadIdx.x == 0) counts[k] = total; continue; }
+    const int64_t slot = emit_rank ? (int64_t)emit_rank[k] : k;
+    if (!EMIT) { if (threadIdx.x == 0) counts[slot] = total; continue; }
     for (int w = w0; w < w1; ++w) { pref[w] = before; before += __popc(bits[w]); }
     __syncthreads();
     const int v = (int)(k / qp.P);
     const uint32_t gid = (uint32_t)(k - (int64_t)v * qp.P);
-    const uint64_t base = offsets[k], hi = (uint64_t)v * (uint64_t)qp.n_tile;
+    const uint64_t base = offsets[slot], hi = (uint64_t)v * (uint64_t)qp.n_tile;
     const uint32_t depth = __float_as_uint(__ldg(rho + k));
     for (uint32_t r = threadIdx.x; r < total; r += kLargeThreads) {
       int lo = 0, hi_w = qp.n_words - 1;                       // largest w with pref[w] <= r
@@ -370,12 +373,12 @@ __global__ void __launch_bounds__(kLargeThreads)
 tile_query_kernel(QueryParams qp, int n_large_blocks, const float* __restrict__ dir, const float* __restrict__ rho,
                   const float* __restrict__ rs, const int32_t* __restrict__ slot_of_tile, const uint32_t* __restrict__ active_words,
                   const uint32_t* __restrict__ perm, const uint32_t* __restrict__ n_small, const uint32_t* __restrict__ large_list,
-                  const uint32_t* __restrict__ n_large, uint32_t* __restrict__ counts, const uint64_t* __restrict__ offsets,
-                  uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+                  const uint32_t* __restrict__ n_large, const uint32_t* __restrict__ emit_rank, uint32_t* __restrict__ counts,
+                  const uint64_t* __restrict__ offsets, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
   if ((int)blockIdx.x < n_large_blocks)
-    large_body<EMIT>(n_large_blocks, qp, dir, rho, rs, active_words, large_list, n_large, counts, offsets, keys, vals);
+    large_body<EMIT>(n_large_blocks, qp, dir, rho, rs, active_words, emit_rank, large_list, n_large, counts, offsets, keys, vals);
   else
-    small_body<EMIT>((int64_t)blockIdx.x - n_large_blocks, qp, dir, rho, rs, slot_of_tile, perm, n_small, counts, offsets, keys, vals);
+    small_body<EMIT>((int64_t)blockIdx.x - n_large_blocks, qp, dir, rho, rs, slot_of_tile, perm, n_small, emit_rank, counts, offsets, keys, vals);
 }
 
 }  // namespace uts
@@ -410,8 +413,8 @@ size_t uts_tile_query_scratch_bytes(const uts_config* cfg) {
   return query_layout(cfg).total;
 }
 
-int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, uint64_t* offsets, uint64_t* keys, uint32_t* vals,
-                   uint64_t capacity, uint64_t* h_n_pairs, void* scratch, size_t scratch_bytes, void* stream) {
+int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint32_t* emit_rank, uint64_t* offsets, uint64_t* keys,
+                   uint32_t* vals, uint64_t capacity, uint64_t* h_n_pairs, void* scratch, size_t scratch_bytes, void* stream) {
   int st = check_config(cfg);
   if (st) return st;
   if ((st = check_mask(cfg, mask))) return st;
@@ -472,14 +475,14 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, uint64_t* 
   }
   UTS_CUDA(cudaMemsetAsync(n_large, 0, 512, s));
   const unsigned cgrid = (unsigned)((n + 255) / 256);
-  classify_kernel<0><<<cgrid, 256, 0, s>>>(qp, in.rs, in.flags, counts, list, n_large, hist, perm);
+  classify_kernel<0><<<cgrid, 256, 0, s>>>(qp, in.rs, in.flags, counts, list, n_large, hist, perm, emit_rank);
   UTS_LAUNCH_CHECK();
   bucket_scan_kernel<<<1, 32, 0, s>>>(hist, n_small);
   UTS_LAUNCH_CHECK();
-  classify_kernel<1><<<cgrid, 256, 0, s>>>(qp, in.rs, in.flags, counts, list, n_large, hist, perm);
+  classify_kernel<1><<<cgrid, 256, 0, s>>>(qp, in.rs, in.flags, counts, list, n_large, hist, perm, emit_rank);
   UTS_LAUNCH_CHECK();
   tile_query_kernel<false><<<qgrid + lgrid, kLargeThreads, dyn_smem, s>>>(qp, lgrid, in.dir, in.rho, in.rs, mask.slot_of_tile, active_arg, perm,
-                                                                         n_small, list, n_large, counts, nullptr, nullptr, nullptr);
+                                                                         n_small, list, n_large, emit_rank, counts, nullptr, nullptr, nullptr);
   UTS_LAUNCH_CHECK();
   if ((st = exclusive_scan_u32(counts, n, offsets, block_sums, s))) return st;
   UTS_CUDA(cudaMemcpyAsync(h_n_pairs, offsets + n, sizeof(uint64_t), cudaMemcpyDeviceToHost, s));
@@ -488,7 +491,7 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, uint64_t* 
   if (*h_n_pairs > capacity) return UTS_ERR_CAPACITY;
   if (*h_n_pairs == 0) return UTS_OK;
   tile_query_kernel<true><<<qgrid + lgrid, kLargeThreads, dyn_smem, s>>>(qp, lgrid, in.dir, in.rho, in.rs, mask.slot_of_tile, active_arg, perm,
-                                                                        n_small, list, n_large, nullptr, offsets, keys, vals);
+                                                                        n_small, list, n_large, emit_rank, nullptr, offsets, keys, vals);
   UTS_LAUNCH_CHECK();
   return UTS_OK;
 }

@@ -17,7 +17,7 @@ class Rasterizer:
     """Holds every buffer of one configuration.  forward() / backward() enqueue on torch's current stream; the only host
     synchronisation is the pair count returned by uts_tile_query."""
 
-    def __init__(self, cfg: B.Config, mask: B.Mask | None = None, device="cuda", pair_capacity: int = 0):
+    def __init__(self, cfg: B.Config, mask: B.Mask | None = None, device="cuda", pair_capacity: int = 0, depth_presort: bool = True):
         B.lib()
         if not torch.cuda.is_available():
             raise RuntimeError("uts: a CUDA device is required (no CPU fallback)")
@@ -28,6 +28,10 @@ class Rasterizer:
         self.proj = B.Proj.empty(cfg, device)
         self.offsets = _i64(V * P + 1, device)
         self.tq_scratch = _bytes(B.uts_tile_query_scratch_bytes(cfg), device)
+        # depth_presort: order the Gaussians by radial depth first so that the pair sort only runs its (view,tile) passes
+        self.depth_presort = depth_presort
+        self.emit_rank = _i32(max(V * P, 1), device) if depth_presort else None
+        self.do_scratch = _bytes(B.uts_depth_order_scratch_bytes(cfg), device) if depth_presort else None
         self.ranges = _i64(V * cfg.n_tiles * 2, device).view(V * cfg.n_tiles, 2)
         self.color = _f32(V, npx, 3, dev=device); self.alpha = _f32(V, npx, dev=device)
         self.trans = _f32(V, npx, dev=device); self.n_last = _i32(V * npx, device).view(V, npx)
@@ -47,17 +51,24 @@ class Rasterizer:
     # ---- stages (each is one ABI call) -------------------------------------------------------------
     def preprocess(self, g, views): B.uts_preprocess(self.cfg, g, views, self.proj)
 
+    def depth_order(self):
+        if self.depth_presort:
+            B.uts_depth_order(self.cfg, self.proj.rho, self.emit_rank, self.do_scratch)
+
     def tile_query(self):
         try:
-            self.n_pairs = B.uts_tile_query(self.cfg, self.proj, self.mask, self.offsets, self.keys, self.vals, self.capacity, self.tq_scratch)
+            self.n_pairs = B.uts_tile_query(self.cfg, self.proj, self.mask, self.offsets, self.keys, self.vals, self.capacity, self.tq_scratch,
+                                            self.emit_rank)
         except B.UtsError as e:
             if e.status != B.UTS_ERR_CAPACITY:
                 raise
             self._alloc_pairs(int(e.needed * 1.05) + 1024)
-            self.n_pairs = B.uts_tile_query(self.cfg, self.proj, self.mask, self.offsets, self.keys, self.vals, self.capacity, self.tq_scratch)
+            self.n_pairs = B.uts_tile_query(self.cfg, self.proj, self.mask, self.offsets, self.keys, self.vals, self.capacity, self.tq_scratch,
+                                            self.emit_rank)
         return self.n_pairs
 
-    def sort(self): B.uts_sort(self.cfg, self.n_pairs, self.keys, self.vals, self.keys_tmp, self.vals_tmp, self.sort_scratch)
+    def sort(self):
+        B.uts_sort(self.cfg, self.n_pairs, self.keys, self.vals, self.keys_tmp, self.vals_tmp, self.sort_scratch, self.depth_presort)
     def tile_ranges(self): B.uts_tile_ranges(self.cfg, self.n_pairs, self.keys, self.ranges)
 
     def render_fwd(self):
@@ -82,6 +93,7 @@ class Rasterizer:
     # ---- whole path --------------------------------------------------------------------------------
     def forward(self, g, views):
         self.preprocess(g, views)
+        self.depth_order()
         self.tile_query()
         self.sort()
         self.tile_ranges()

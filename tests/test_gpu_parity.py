@@ -189,7 +189,7 @@ def test_tile_query_other_refinements(refine):
     assert info["min_margin"] > 1e-12
     cfg = _cfg(R, scene, query_refine_log2=refine)
     proj = B.Proj(dev(pr.dir), dev(pr.lonlat), dev(pr.rho), dev(pr.conic_opac), dev(pr.rs), dev(pr.rgb), dev(pr.flags))
-    r = R.Rasterizer(cfg, pair_capacity=16)       # forces the capacity-retry path
+    r = R.Rasterizer(cfg, pair_capacity=16, depth_presort=False)       # forces the capacity-retry path
     r.proj = proj
     n = r.tile_query()
     assert n == keys.shape[0]
@@ -212,7 +212,7 @@ def test_tile_query_block_path_large_discs(cfg_id, order, refine):
     assert info["min_margin"] > 1e-12
     cfg = _cfg(R, scene, query_refine_log2=refine)
     mask = B.Mask.full() if bits is None else B.Mask(dev(act.view(np.int32)), int(act.shape[0]), dev(slot), dev(bits.view(np.int32)))
-    r = R.Rasterizer(cfg, mask)
+    r = R.Rasterizer(cfg, mask, depth_presort=False)
     r.proj = B.Proj(dev(pr.dir), dev(pr.lonlat), dev(pr.rho), dev(pr.conic_opac), dev(pr.rs), dev(pr.rgb), dev(pr.flags))
     n = r.tile_query()
     assert n == keys.shape[0]
@@ -230,13 +230,13 @@ def test_tile_query_whole_sphere_and_empty():
     off, keys, vals, _ = orc.tile_query(oc, pr)
     assert off[1] - off[0] == oc.n_tiles and off[2] == off[1]
     cfg = _cfg(R, scene)
-    r = R.Rasterizer(cfg)
+    r = R.Rasterizer(cfg, depth_presort=False)
     r.proj = B.Proj(dev(pr.dir), dev(pr.lonlat), dev(pr.rho), dev(pr.conic_opac), dev(pr.rs), dev(pr.rgb), dev(pr.flags))
     n = r.tile_query()
     assert np.array_equal(u64(r.offsets), off) and np.array_equal(u64(r.keys)[:n], keys) and np.array_equal(u32(r.vals)[:n], vals)
     # P = 0
     cfg0 = B.Config(order=6, n_gauss=0)
-    r0 = R.Rasterizer(cfg0)
+    r0 = R.Rasterizer(cfg0, depth_presort=False)
     assert r0.tile_query() == 0
 
 
@@ -412,8 +412,9 @@ def test_backward_thresholds_off_every_pixel(cfg_id, P, order):
 
 
 # ------------------------------------------------------------------------------------------- whole chain
+@pytest.mark.parametrize("presort", [True, False], ids=["depth-presorted", "plain-sort"])
 @pytest.mark.parametrize("cfg_id,P,order,extra", CASES)
-def test_end_to_end_chain(cfg_id, P, order, extra):
+def test_end_to_end_chain(cfg_id, P, order, extra, presort):
     """All-GPU chain against the all-oracle chain: pair lists, sorted order and ranges bit-exact (the GPU preprocess
     rounds double results to fp32 once, as the oracle does), image within 1e-4, parameter gradients within 1e-3."""
     B, R = _gpu()
@@ -426,7 +427,7 @@ def test_end_to_end_chain(cfg_id, P, order, extra):
     else:
         mask = B.Mask.full()
     g, views = R.scene_to_device(c.scene)
-    r = R.Rasterizer(cfg, mask)
+    r = R.Rasterizer(cfg, mask, depth_presort=presort)
     r.forward(g, views)
     n = r.n_pairs
     # fp32 records straddling a rounding boundary could flip a borderline tile; require exact equality and report if not

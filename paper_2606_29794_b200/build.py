@@ -15,6 +15,9 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libuts.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
+# The tile query's fp32 arithmetic is a conservative pre-filter with a 4e-6 margin (every defining decision is re-taken in
+# double inside the margin), so approximate fp32 sqrt / division are safe there; double precision code is unaffected.
+PER_FILE_FLAGS = {"uts_tile_query.cu": ["--use_fast_math"]}
 
 
 def sources():
@@ -43,7 +46,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     for src in sources():
         obj = os.path.join(objdir, os.path.basename(src)[:-3] + ".o")
         objs.append(obj)
-        procs.append((src, subprocess.Popen([NVCC, "-c", src, "-o", obj] + flags, stdout=subprocess.PIPE, stderr=subprocess.STDOUT)))
+        extra = PER_FILE_FLAGS.get(os.path.basename(src), [])
+        procs.append((src, subprocess.Popen([NVCC, "-c", src, "-o", obj] + flags + extra, stdout=subprocess.PIPE, stderr=subprocess.STDOUT)))
     failed = False
     for src, p in procs:
         out = p.communicate()[0].decode()

@@ -11,8 +11,8 @@
 // is the haversine distance + bearing decomposition of PAPER.md:112 in vector form.  Because e.u = n.u = 0,
 // a = e.(w-u) and b = n.(w-u): the difference w-u = (c_tile - u) + (w - c_tile) is formed in double precision once per
 // (tile, Gaussian) and once per pixel, then everything per (pixel, Gaussian) is fp32 FMAs on small, exactly known
-// differences.  k = d_gc/sin d_gc = asin(s)/s is a degree-5 polynomial in s^2 for s < 0.3 (error < 1e-8) and
-// atan2f otherwise.  power*log2(e) = k^2 (qa a^2 + qb a b + qc b^2) with the conic pre-scaled at staging; alpha uses ex2.
+// differences.  k = d_gc/sin d_gc = P(c) rsqrt(1+c) with a degree-7 polynomial P for c = cos d_gc >= 0 (atan2f beyond
+// 90 degrees).  power*log2(e) = k^2 (qa a^2 + qb a b + qc b^2) with the conic pre-scaled at staging; alpha uses ex2.
 #include "uts_internal.cuh"
 
 namespace uts {
@@ -24,7 +24,6 @@ struct RenderParams {
 };
 
 constexpr float kLog2e = 1.4426950408889634f;
-constexpr float kPolyT = 0.09f;                       // fast path for s^2 < 0.09 (s < 0.3, 17.5 degrees) and c > 0
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
@@ -32,16 +31,21 @@ __device__ __forceinline__ float ex2_approx(float x) {
   return y;
 }
 
-// d_gc / sin(d_gc) from t = sin^2 and c = cos
+// k = d_gc / sin(d_gc).  For cos(d_gc) = c >= 0:  acos(c) = sqrt(1-c) P(c) with P analytic on [0,1], so
+// k = acos(c) / sqrt((1-c)(1+c)) = P(c) rsqrt(1+c): no cancellation (1-c never formed), no branch, one MUFU.
+// P is a degree-7 Chebyshev fit of acos(c)/sqrt(1-c) on [0,1] (own fit; max relative error of k in fp32: 1.7e-7).
+// Beyond 90 degrees (c < 0; only the far tail of very large Gaussians) fall back to atan2f on sin = sqrt(t).
 __device__ __forceinline__ float arc_over_sin(float t, float c) {
-  if (c > 0.f && t < kPolyT) {
-    float k = 0.02237215909f;                         // asin(s)/s = sum_n (2n)! / (4^n (n!)^2 (2n+1)) s^(2n)
-    k = fmaf(k, t, 0.03038194444f);
-    k = fmaf(k, t, 0.04464285714f);
-    k = fmaf(k, t, 0.075f);
-    k = fmaf(k, t, 0.16666666667f);
-    k = fmaf(k, t, 1.0f);
-    return k;
+  if (c >= 0.f) {
+    float p = -0.00115729403f;
+    p = fmaf(p, c, 0.00628544204f);
+    p = fmaf(p, c, -0.016528869f);
+    p = fmaf(p, c, 0.0304812621f);
+    p = fmaf(p, c, -0.0500148833f);
+    p = fmaf(p, c, 0.0889478773f);
+    p = fmaf(p, c, -0.214596227f);
+    p = fmaf(p, c, 1.57079625f);
+    return p * rsqrtf(1.0f + c);
   }
   if (!(t > 0.f)) return 1.0f;
   const float s = sqrtf(t);
@@ -259,7 +263,7 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
       if (!__any_sync(0xffffffffu, used)) continue;
       float d_r = 0.f, d_g = 0.f, d_b = 0.f, d_A = 0.f, d_B = 0.f, d_C = 0.f, d_o = 0.f, d_om = 0.f, d_ph = 0.f;
       if (used) {
-        const float inv1a = 1.f / (1.f - a);
+        const float inv1a = __frcp_rn(1.f - a);
         const float Tb = T * inv1a;                    // transmittance before this entry
         const float w = Tb * a;
         d_r = w * gr; d_g = w * gg; d_b = w * gb;
@@ -278,10 +282,11 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
           if (ev.t > 0.f) {
             const float den = ev.t + ev.c * ev.c;
             const float gk = gdx * ev.a + gdy * ev.b;
-            const float kp = (ev.c / den - ev.k) / ev.t;
+            const float iden = __frcp_rn(den);
+            const float kp = __fdividef(ev.c * iden - ev.k, ev.t);
             g_a = fmaf(gk * kp, ev.a, ev.k * gdx);
             g_b = fmaf(gk * kp, ev.b, ev.k * gdy);
-            g_c = -gk / den;
+            g_c = -gk * iden;
           }
           // a = e.w, b = n.w, c = u.w with de/dom = -hh, dn/dom = -sin(phi) e, du/dom = cos(phi) e, dn/dphi = -u, du/dphi = n,
           // and hh.w = cos(phi) c - sin(phi) b
@@ -290,16 +295,41 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
           d_ph = g_c * ev.b - g_b * ev.c;
         }
       }
-      d_r = warp_sum(d_r); d_g = warp_sum(d_g); d_b = warp_sum(d_b);
-      d_A = warp_sum(d_A); d_B = warp_sum(d_B); d_C = warp_sum(d_C);
-      d_o = warp_sum(d_o); d_om = warp_sum(d_om); d_ph = warp_sum(d_ph);
-      if (lane == 0) {
+      // 9 sums over the warp.  Eight of them go through a transposing butterfly: at each of the first three steps a lane
+      // keeps half of its values and hands the other half to its partner, so 4+2+1 shuffles leave every lane with ONE value
+      // summed over 8 lanes, and two more steps finish it: 9 shuffles instead of 40.  Lane 4*j ends up owning value j.
+      float v0 = d_r, v1 = d_g, v2 = d_b, v3 = d_A, v4 = d_B, v5 = d_C, v6 = d_om, v7 = d_ph;
+      {
+        const bool hi = lane & 16;
+        const float s0 = hi ? v0 : v4, s1 = hi ? v1 : v5, s2 = hi ? v2 : v6, s3 = hi ? v3 : v7;
+        const float k0 = hi ? v4 : v0, k1 = hi ? v5 : v1, k2 = hi ? v6 : v2, k3 = hi ? v7 : v3;
+        v0 = k0 + __shfl_xor_sync(0xffffffffu, s0, 16); v1 = k1 + __shfl_xor_sync(0xffffffffu, s1, 16);
+        v2 = k2 + __shfl_xor_sync(0xffffffffu, s2, 16); v3 = k3 + __shfl_xor_sync(0xffffffffu, s3, 16);
+      }
+      {
+        const bool hi = lane & 8;
+        const float s0 = hi ? v0 : v2, s1 = hi ? v1 : v3;
+        const float k0 = hi ? v2 : v0, k1 = hi ? v3 : v1;
+        v0 = k0 + __shfl_xor_sync(0xffffffffu, s0, 8); v1 = k1 + __shfl_xor_sync(0xffffffffu, s1, 8);
+      }
+      {
+        const bool hi = lane & 4;
+        const float s0 = hi ? v0 : v1, k0 = hi ? v1 : v0;
+        v0 = k0 + __shfl_xor_sync(0xffffffffu, s0, 4);
+      }
+      v0 += __shfl_xor_sync(0xffffffffu, v0, 2);
+      v0 += __shfl_xor_sync(0xffffffffu, v0, 1);
+      d_o = warp_sum(d_o);
+      {
+        // value index owned by this lane: bit4 -> +4, bit3 -> +2, bit2 -> +1  (0 r, 1 g, 2 b, 3 A, 4 B, 5 C, 6 omega, 7 phi)
+        const int vi = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
         const uint32_t id = S.id[jj];
         const size_t gi = gbase + id;
-        atomicAdd(dL_drgb + 3 * gi, d_r); atomicAdd(dL_drgb + 3 * gi + 1, d_g); atomicAdd(dL_drgb + 3 * gi + 2, d_b);
-        atomicAdd(dL_dconic + 3 * gi, d_A); atomicAdd(dL_dconic + 3 * gi + 1, d_B); atomicAdd(dL_dconic + 3 * gi + 2, d_C);
-        atomicAdd(dL_dmu2 + 2 * gi, d_om); atomicAdd(dL_dmu2 + 2 * gi + 1, d_ph);
-        atomicAdd(dL_dopac + id, d_o);
+        if ((lane & 3) == 0) {
+          float* dst = vi < 3 ? dL_drgb + 3 * gi + vi : vi < 6 ? dL_dconic + 3 * gi + (vi - 3) : dL_dmu2 + 2 * gi + (vi - 6);
+          atomicAdd(dst, v0);
+        }
+        if (lane == 1) atomicAdd(dL_dopac + id, d_o);
       }
     }
   }

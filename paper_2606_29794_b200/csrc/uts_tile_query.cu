@@ -26,6 +26,8 @@ namespace uts {
 
 constexpr float kDelta = 4e-6f;         // fp32 chord margin (chord error of the fp32 centres is below 1e-6)
 constexpr int kLargeThreads = 256;
+constexpr size_t kMaxLargeSmem = 200 * 1024;
+constexpr int kTileCacheK = 16;         // tiles of a small disc remembered by the count pass (64 B per Gaussian)
 
 struct QueryParams {
   int kt, kq, P, V;
@@ -35,6 +37,9 @@ struct QueryParams {
   int64_t n_tile;
   double rho_q;                         // rho_max(k_q)
   float r_large;                        // discs with R above this go to the block path
+  uint32_t* tile_cache;                 // [V*P][kTileCacheK] tiles found by the count pass (thread path), reused by the emit pass
+  uint32_t* bitmap_cache;               // [bitmap_cache_cap][n_words] bitmaps of the count pass (block path)
+  uint32_t bitmap_cache_cap;
   float rho[kMaxOrder + 1], sin_hrho[kMaxOrder + 1], cos_hrho[kMaxOrder + 1];   // rho_max(o), sin/cos(rho_max(o)/2)
 };
 
@@ -134,6 +139,7 @@ template <bool EMIT>
 struct ThreadSink {
   uint64_t* keys; uint32_t* vals; uint64_t base; uint64_t key_hi_base; uint32_t depth_bits; uint32_t gid;
   const int32_t* slot_of_tile;
+  uint32_t* cache;                       // count pass: this Gaussian's kTileCacheK-entry slot
   uint32_t count;
   int64_t last_tile;
   __device__ __forceinline__ bool has(int64_t tile) const { return tile == last_tile; }
@@ -144,7 +150,7 @@ struct ThreadSink {
     if (EMIT) {
       keys[base + count] = ((key_hi_base + (uint64_t)tile) << 32) | depth_bits;   // Alg.1 l.12: ((t, rho), i)
       vals[base + count] = gid;
-    }
+    } else if (count < (uint32_t)kTileCacheK) cache[count] = (uint32_t)tile;
     ++count;
   }
   __device__ __forceinline__ void add_range(int64_t t0, int64_t t1) { for (int64_t t = t0; t < t1; ++t) add(t); }
@@ -214,9 +220,21 @@ small_body(int64_t block, const QueryParams& qp, const float* __restrict__ dir, 
   bool running = t < (int64_t)*n_small;
   const int64_t k = running ? (int64_t)perm[t] : 0;
   const int64_t slot = emit_rank ? (int64_t)emit_rank[k] : k;     // position of this Gaussian in the emission order
-  if (EMIT && running && offsets[slot + 1] == offsets[slot]) running = false;
+  if (EMIT && running) {
+    // the count pass left the tiles of discs with at most kTileCacheK tiles in tile_cache: emit them without walking
+    const uint64_t b0 = offsets[slot], cnt = offsets[slot + 1] - b0;
+    if (cnt <= (uint64_t)kTileCacheK) {
+      const int v = (int)(k / qp.P);
+      const uint64_t hi = (uint64_t)v * (uint64_t)qp.n_tile;
+      const uint32_t depth = __float_as_uint(__ldg(rho + k)), gid = (uint32_t)(k - (int64_t)v * qp.P);
+      const uint32_t* c = qp.tile_cache + (size_t)k * kTileCacheK;
+      for (uint32_t j = 0; j < (uint32_t)cnt; ++j) { keys[b0 + j] = ((hi + c[j]) << 32) | depth; vals[b0 + j] = gid; }
+      running = false;
+    }
+  }
   Disc D;
   ThreadSink<EMIT> sink;
+  sink.cache = qp.tile_cache + (size_t)k * kTileCacheK;
   sink.count = 0; sink.last_tile = -1; sink.slot_of_tile = slot_of_tile; sink.keys = keys; sink.vals = vals;
   sink.base = 0; sink.key_hi_base = 0; sink.depth_bits = 0; sink.gid = 0;
   const bool valid = running;
@@ -288,13 +306,17 @@ large_body(int n_blocks, const QueryParams& qp, const float* __restrict__ dir, c
   const uint32_t nl = *n_large;
   for (uint32_t li = blockIdx.x; li < nl; li += (uint32_t)n_blocks) {
     const int64_t k = (int64_t)large_list[li];
+    const bool cached = li < qp.bitmap_cache_cap;                 // the count pass kept this disc's (masked) bitmap
+    uint32_t* cache_row = qp.bitmap_cache + (size_t)li * qp.n_words;
     __syncthreads();
-    if (threadIdx.x == 0) { load_disc(qp, dir, rs, k, s_disc); s_count = 0; s_next = 0; }
-    for (int w = threadIdx.x; w < qp.n_words; w += kLargeThreads) bits[w] = 0u;
+    if (threadIdx.x == 0) { if (!(EMIT && cached)) load_disc(qp, dir, rs, k, s_disc); s_count = 0; s_next = 0; }
+    for (int w = threadIdx.x; w < qp.n_words; w += kLargeThreads) bits[w] = (EMIT && cached) ? cache_row[w] : 0u;
     __syncthreads();
     const Disc D = s_disc;
     BitmapSink sink{bits};
-    if (D.all) {
+    if (EMIT && cached) {
+      // nothing to walk
+    } else if (D.all) {
       for (int w = threadIdx.x; w < qp.n_words; w += kLargeThreads) bits[w] = 0xffffffffu;
     } else {
       for (int node = threadIdx.x; node < n_split; node += kLargeThreads) {
@@ -343,7 +365,8 @@ large_body(int n_blocks, const QueryParams& qp, const float* __restrict__ dir, c
     uint32_t mine = 0;
     for (int w = w0; w < w1; ++w) {
       uint32_t b = bits[w];
-      if (active_words) { b &= __ldg(active_words + w); bits[w] = b; }
+      if (active_words && !(EMIT && cached)) { b &= __ldg(active_words + w); bits[w] = b; }
+      if (!EMIT && cached) cache_row[w] = b;
       mine += __popc(b);
     }
     uint32_t before;
@@ -387,9 +410,8 @@ using namespace uts;
 
 namespace {
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
-constexpr size_t kMaxLargeSmem = 200 * 1024;
 
-struct QueryLayout { size_t counts, list, perm, nlarge, active, scan, total; };
+struct QueryLayout { size_t counts, list, perm, nlarge, active, scan, tcache, bcache, total; uint32_t bcache_cap; };
 QueryLayout query_layout(const uts_config* cfg) {
   const size_t n = (size_t)cfg->n_gauss * cfg->n_views;
   const size_t n_tile = (size_t)12 << (2 * (cfg->order - cfg->tile_log2));
@@ -401,6 +423,14 @@ QueryLayout query_layout(const uts_config* cfg) {
   L.nlarge = off; off += 512;      // n_large, n_small, 64 bucket counters
   L.active = off; off += align256((n_tile / 32 + 1) * 4);
   L.scan = off;   off += scan_scratch_bytes((int64_t)n);
+  L.tcache = off; off += align256(n * kTileCacheK * 4);
+  // bitmap cache of the block path: as many discs as fit 384 MB (config 4: 65 536 bitmaps of 6 KB)
+  const size_t row = (n_tile / 32) * 4;
+  size_t cap = row ? (size_t)(384u << 20) / row : 0;
+  if (cap > n) cap = n;
+  if (n_tile < 192 || row * 2 + 4096 * 8 > kMaxLargeSmem) cap = 0;
+  L.bcache_cap = (uint32_t)cap;
+  L.bcache = off; off += align256(cap * row);
   L.total = off + 256;
   return L;
 }
@@ -456,6 +486,9 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   uint32_t* perm = reinterpret_cast<uint32_t*>(sp + L.perm);
   uint32_t* active = reinterpret_cast<uint32_t*>(sp + L.active);
   uint64_t* block_sums = reinterpret_cast<uint64_t*>(sp + L.scan);
+  qp.tile_cache = reinterpret_cast<uint32_t*>(sp + L.tcache);
+  qp.bitmap_cache = reinterpret_cast<uint32_t*>(sp + L.bcache);
+  qp.bitmap_cache_cap = L.bcache_cap;
   const uint32_t* active_arg = nullptr;
   const unsigned qgrid = (unsigned)((n + kLargeThreads - 1) / kLargeThreads);
   const int lgrid = use_large ? sm_count() * (e2__ ? atoi(e2__) : 2) : 0;

@@ -21,3 +21,27 @@ def oracle_mask(cfg, scene):
 
 def small_scene(cfg_id, n_gauss, order, seed=0, **kw):
     return scenes.make_scene(cfg_id, seed=seed, n_gauss=n_gauss, order=order, **kw)
+
+
+def oracle_on_tiles(oc, scene, pick, bits=None):
+    """Oracle forward state restricted to the tiles `pick` (sorted tile ids) but with their COMPLETE lists: every Gaussian is
+    preprocessed, a conservative angular pre-filter (plain numpy on the oracle's own records) selects the Gaussians that can
+    reach a picked tile, and the oracle's own tile query decides.  Returns dict(proj, sact, skeys, svals, ranges, color, alpha,
+    n_last, margin)."""
+    pr = orc.preprocess(oc, scene["means"], scene["scales"], scene["quats"], scene["opac"], scene["sh"], scene["W"], scene["b"])
+    P, V = oc.n_gauss, oc.n_views
+    pick = np.asarray(pick, np.int64)
+    sact = pick.astype(np.uint32)
+    sslot = np.full(oc.n_tiles, -1, np.int32); sslot[pick] = np.arange(pick.shape[0], dtype=np.int32)
+    _, _, tc = orc.centers(oc.tile_order, which=2)
+    reach = pr.rs.astype(np.float64) + orc.rho_max_closed(oc.tile_order + oc.query_refine_log2) + orc.rho_max_closed(oc.tile_order) + 1e-6
+    cand = np.zeros(P, bool)
+    for v in range(V):
+        d = pr.dir[v].astype(np.float64) @ tc[pick].T
+        cand |= (np.arccos(np.clip(d, -1, 1)) <= reach[v][:, None]).any(axis=1)
+    cand_ids = np.flatnonzero(cand).astype(np.int32)
+    _, keys, vals, info = orc.tile_query(oc, pr, sslot, gauss_subset=cand_ids)
+    sk, sv = orc.sort_pairs(keys, vals)
+    rg = orc.tile_ranges(oc, sk)
+    col, al, nl, margin, ctr = orc.render_fwd(oc, pr, rg, sv, sact, bits)
+    return dict(proj=pr, sact=sact, skeys=sk, svals=sv, ranges=rg, color=col, alpha=al, n_last=nl, margin=margin, qinfo=info, counters=ctr)

@@ -169,11 +169,9 @@ def run_reference(args):
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_2606_29794_b200 import binding as B, rasterizer as R
+    from paper_2606_29794_b200 import binding as B, rasterizer as R, replicas
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world, rank, local = replicas.world()
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
     torch.cuda.set_device(local)
@@ -182,7 +180,7 @@ def run_ours(args):
     peaks = _peaks()
 
     # replicas only: every rank renders its own scene of the same recipe; no data-path collective
-    scene = scenes.make_scene(args.config, seed=rank)
+    scene = scenes.make_scene(args.config, seed=replicas.rank_seed(rank))
     cfg = R.config_of(scene)
     mask = B.Mask.full() if scene["mask"] is None else B.uts_build_mask(cfg, scene["mask"]["kind"], scene["mask"]["params"])
     g, views = R.scene_to_device(scene)
@@ -266,16 +264,13 @@ def run_ours(args):
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - tt) * 1e3 / e2e_steps
 
-    times = torch.tensor([ms_step, e2e_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-    ms_step_max, e2e_ms_max = float(times[0]), float(times[1])
+    ms_step_max, e2e_ms_max = replicas.max_over_ranks([ms_step, e2e_ms], device="cuda")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    value = world * n_pix_active / (ms_step_max * 1e-3)
+    value = replicas.aggregate_throughput(n_pix_active, ms_step_max, world)
     # dominant kernel and its roofline
     dom = max(stage_ms, key=stage_ms.get)
     fp32_peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12       # TFLOP/s at the maximum SM clock
@@ -310,7 +305,7 @@ def run_ours(args):
                 ms_forward=ms_fwd, ms_forward_backward=ms_step, stage_ms=stage_ms, per_kernel=per_kernel,
                 evaluated_pairs=dict(forward=ev_f, backward=ev_b),
                 roofline=roof, clocks=clocks,
-                e2e=dict(value=world * n_pix_active / (e2e_ms_max * 1e-3), unit=UNIT, ms_per_step=e2e_ms_max, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h),
+                e2e=dict(value=replicas.aggregate_throughput(n_pix_active, e2e_ms_max, world), unit=UNIT, ms_per_step=e2e_ms_max, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h),
                 gpu_launches=0)
     # launches of our kernels per step: 1 preprocess + (1 count + 3 scan + 1 emit) + passes*(1 + 3 + 1) (+1 copy) + 1 ranges + 1 fwd + 1 bwd + 1 pre-bwd
     passes = (max(1, (V * cfg.n_tiles - 1)).bit_length() + 7) // 8          # pair sort: (view,tile) bytes only

@@ -71,76 +71,83 @@ class ClockSampler(threading.Thread):
 
 
 # ----------------------------------------------------------------------------------------------- reference arm
-def oracle_sample(cfg_id, seed=0, n_pre=100_000, n_query=10_000, n_tiles_sample=24):
-    """The oracle, as it stands, on a BOUNDED sample of the workload; returns (estimated whole-frame seconds, description).
+class OracleSample:
+    """The oracle, as it stands, on a BOUNDED sample of the workload.  Set-up (scene, full preprocess, choice of the sampled
+    tiles and their candidate Gaussians) happens once, untimed; step() times the oracle stages and extrapolates per stage:
 
     per-Gaussian stages (preprocess, preprocess backward) : first n_pre Gaussians, scaled by P/n_pre
     tile query + sort + ranges                           : first n_query Gaussians on every tile, scaled by P/n_query
-    blend forward + backward                             : n_tiles_sample random tiles with their complete lists (all P
+    blend forward + backward                             : n_tiles_sample random tiles with their COMPLETE lists (all P
                                                            Gaussians pre-filtered by a conservative angular test, the oracle's
                                                            own query decides), scaled by active tiles / sampled tiles
     """
-    import oracle as orc
-    sc = scenes.make_scene(cfg_id, seed=seed)
-    P, V = sc["n_gauss"], sc["n_views"]
-    oc = orc.Config(order=sc["order"], n_gauss=P, n_views=V, sh_degree=sc["sh_degree"])
-    bits = act = slot = None
-    if sc["mask"] is not None:
-        bits = orc.mask_bits(oc.order, sc["mask"]["kind"], sc["mask"]["params"]); act, slot = orc.mask_tiles(oc, bits)
-    n_active = oc.n_tiles if act is None else int(act.shape[0])
-    n_pre, n_query = min(n_pre, P), min(n_query, P)
-    sub = lambda n: {k: (sc[k][:n] if k in ("means", "scales", "quats", "opac", "sh") else sc[k]) for k in sc}
 
-    # (1) per-Gaussian stages
-    s1 = sub(n_pre); c1 = orc.Config(order=oc.order, n_gauss=n_pre, n_views=V, sh_degree=oc.sh_degree)
-    t = time.perf_counter()
-    pr1 = orc.preprocess(c1, s1["means"], s1["scales"], s1["quats"], s1["opac"], s1["sh"], s1["W"], s1["b"])
-    z3 = np.zeros((V, n_pre, 3)); z2 = np.zeros((V, n_pre, 2))
-    orc.preprocess_bwd(c1, s1["means"], s1["scales"], s1["quats"], s1["sh"], s1["W"], s1["b"], z3 + 1.0, z3 + 1.0, z2 + 1.0)
-    t_pre = (time.perf_counter() - t) * (P / n_pre)
+    def __init__(self, cfg_id, seed=0, n_pre=100_000, n_query=10_000, n_tiles_sample=24):
+        import oracle as orc
+        self.orc, self.cfg_id = orc, cfg_id
+        sc = self.sc = scenes.make_scene(cfg_id, seed=seed)
+        P, V = sc["n_gauss"], sc["n_views"]
+        oc = self.oc = orc.Config(order=sc["order"], n_gauss=P, n_views=V, sh_degree=sc["sh_degree"])
+        self.bits = self.act = self.slot = None
+        if sc["mask"] is not None:
+            self.bits = orc.mask_bits(oc.order, sc["mask"]["kind"], sc["mask"]["params"]); self.act, self.slot = orc.mask_tiles(oc, self.bits)
+        self.n_active = oc.n_tiles if self.act is None else int(self.act.shape[0])
+        self.n_pre, self.n_query = min(n_pre, P), min(n_query, P)
+        self.n_pix = V * self.n_active * oc.ppt
+        pr = self.pr = orc.preprocess(oc, sc["means"], sc["scales"], sc["quats"], sc["opac"], sc["sh"], sc["W"], sc["b"])
+        rng = np.random.default_rng(seed + 17)
+        pool = np.arange(oc.n_tiles) if self.act is None else self.act.astype(np.int64)
+        pick = self.pick = np.sort(rng.choice(pool, min(n_tiles_sample, pool.shape[0]), replace=False))
+        self.sact = pick.astype(np.uint32)
+        self.sslot = np.full(oc.n_tiles, -1, np.int32); self.sslot[pick] = np.arange(pick.shape[0], dtype=np.int32)
+        _, _, tc = orc.centers(oc.tile_order, which=2)
+        reach = pr.rs.astype(np.float64) + orc.rho_max_closed(oc.tile_order + oc.query_refine_log2) + orc.rho_max_closed(oc.tile_order) + 1e-6
+        cand = np.zeros(P, bool)
+        for v in range(V):
+            d = pr.dir[v].astype(np.float64) @ tc[pick].T
+            cand |= (np.arccos(np.clip(d, -1, 1)) <= reach[v][:, None]).any(axis=1)
+        self.cand_ids = np.flatnonzero(cand).astype(np.int32)
+        self.gcol = scenes.upstream_grad(V, pick.shape[0] * oc.ppt, seed=seed)
+        _, keys, vals, _ = orc.tile_query(oc, pr, self.sslot, gauss_subset=self.cand_ids)          # complete lists of the sampled tiles
+        self.sk, self.sv = orc.sort_pairs(keys, vals)
+        self.rg = orc.tile_ranges(oc, self.sk)
 
-    # (2) query + sort + ranges
-    s2 = sub(n_query); c2 = orc.Config(order=oc.order, n_gauss=n_query, n_views=V, sh_degree=oc.sh_degree)
-    pr2 = orc.preprocess(c2, s2["means"], s2["scales"], s2["quats"], s2["opac"], s2["sh"], s2["W"], s2["b"])
-    t = time.perf_counter()
-    _, keys, vals, _ = orc.tile_query(c2, pr2, slot)
-    sk, sv = orc.sort_pairs(keys, vals)
-    orc.tile_ranges(c2, sk)
-    t_qs = (time.perf_counter() - t) * (P / n_query)
-    pairs_est = keys.shape[0] * (P / n_query)
+    def _sub(self, n):
+        sc = self.sc
+        return {k: (sc[k][:n] if k in ("means", "scales", "quats", "opac", "sh") else sc[k]) for k in sc}
 
-    # (3) blend on sampled tiles with complete lists
-    pr = orc.preprocess(oc, sc["means"], sc["scales"], sc["quats"], sc["opac"], sc["sh"], sc["W"], sc["b"])
-    rng = np.random.default_rng(seed + 17)
-    pool = np.arange(oc.n_tiles) if act is None else act.astype(np.int64)
-    pick = np.sort(rng.choice(pool, min(n_tiles_sample, pool.shape[0]), replace=False))
-    sact = pick.astype(np.uint32)
-    sslot = np.full(oc.n_tiles, -1, np.int32); sslot[pick] = np.arange(pick.shape[0], dtype=np.int32)
-    _, _, tc = orc.centers(oc.tile_order, which=2)                           # tile centre directions
-    reach = pr.rs[..., None].astype(np.float64) + orc.rho_max_closed(oc.tile_order + oc.query_refine_log2) + orc.rho_max_closed(oc.tile_order) + 1e-6
-    cand = np.zeros(P, bool)
-    for v in range(V):
-        d = pr.dir[v].astype(np.float64) @ tc[pick].T                         # [P, n_sample]
-        cand |= (np.arccos(np.clip(d, -1, 1)) <= reach[v]).any(axis=1)
-    cand_ids = np.flatnonzero(cand).astype(np.int32)
-    _, keys, vals, _ = orc.tile_query(oc, pr, sslot, gauss_subset=cand_ids)
-    sk, sv = orc.sort_pairs(keys, vals)
-    rg = orc.tile_ranges(oc, sk)
-    npx = pick.shape[0] * oc.ppt
-    gcol = scenes.upstream_grad(V, npx, seed=seed)
-    t = time.perf_counter()
-    col, al, nl, _, ctr = orc.render_fwd(oc, pr, rg, sv, sact, bits)
-    t_f = time.perf_counter() - t
-    t = time.perf_counter()
-    orc.render_bwd(oc, pr, rg, sv, nl, gcol, None, sact, bits)
-    t_b = time.perf_counter() - t
-    scale = n_active / pick.shape[0]
-    total = t_pre + t_qs + (t_f + t_b) * scale
-    desc = (f"oracle (single thread, fp64) on a bounded sample of config {cfg_id}: preprocess+preprocess_bwd on {n_pre} of {P} Gaussians "
-            f"(x{P / n_pre:.0f}), query+sort+ranges on {n_query} Gaussians (x{P / n_query:.0f}, ~{pairs_est:.3g} pairs), blend fwd+bwd on "
-            f"{pick.shape[0]} of {n_active} tiles with complete lists ({sk.shape[0]} pairs, {ctr['evaluated']} evaluations; x{scale:.0f}); "
-            f"extrapolated whole-frame time {total:.1f} s = pre {t_pre:.1f} + query/sort {t_qs:.1f} + blend {(t_f + t_b) * scale:.1f}")
-    return total, desc, dict(n_pix=V * n_active * oc.ppt)
+    def step(self):
+        orc, oc, sc = self.orc, self.oc, self.sc
+        P, V = oc.n_gauss, oc.n_views
+        s1 = self._sub(self.n_pre); c1 = orc.Config(order=oc.order, n_gauss=self.n_pre, n_views=V, sh_degree=oc.sh_degree)
+        z3 = np.ones((V, self.n_pre, 3)); z2 = np.ones((V, self.n_pre, 2))
+        t = time.perf_counter()
+        orc.preprocess(c1, s1["means"], s1["scales"], s1["quats"], s1["opac"], s1["sh"], s1["W"], s1["b"])
+        orc.preprocess_bwd(c1, s1["means"], s1["scales"], s1["quats"], s1["sh"], s1["W"], s1["b"], z3, z3, z2)
+        t_pre = (time.perf_counter() - t) * (P / self.n_pre)
+
+        s2 = self._sub(self.n_query); c2 = orc.Config(order=oc.order, n_gauss=self.n_query, n_views=V, sh_degree=oc.sh_degree)
+        pr2 = orc.preprocess(c2, s2["means"], s2["scales"], s2["quats"], s2["opac"], s2["sh"], s2["W"], s2["b"])
+        t = time.perf_counter()
+        _, keys, vals, _ = orc.tile_query(c2, pr2, self.slot)
+        sk, sv = orc.sort_pairs(keys, vals)
+        orc.tile_ranges(c2, sk)
+        t_qs = (time.perf_counter() - t) * (P / self.n_query)
+        pairs_est = keys.shape[0] * (P / self.n_query)
+
+        sk, sv, rg = self.sk, self.sv, self.rg
+        t = time.perf_counter()
+        col, al, nl, _, ctr = orc.render_fwd(oc, self.pr, rg, sv, self.sact, self.bits)
+        orc.render_bwd(oc, self.pr, rg, sv, nl, self.gcol, None, self.sact, self.bits)
+        t_blend = time.perf_counter() - t
+        scale = self.n_active / self.pick.shape[0]
+        total = t_pre + t_qs + t_blend * scale
+        desc = (f"oracle (single thread, fp64) on a bounded sample of config {self.cfg_id}: preprocess+preprocess_bwd on {self.n_pre} of {P} "
+                f"Gaussians (x{P / self.n_pre:.0f}), query+sort+ranges on {self.n_query} Gaussians (x{P / self.n_query:.0f}, ~{pairs_est:.3g} pairs), "
+                f"blend fwd+bwd on {self.pick.shape[0]} of {self.n_active} tiles with complete lists ({sk.shape[0]} pairs, {ctr['evaluated']} "
+                f"evaluations; x{scale:.0f}); extrapolated whole-frame time {total:.1f} s = pre {t_pre:.1f} + query/sort {t_qs:.1f} + "
+                f"blend {t_blend * scale:.1f}; measured CPU time of the sample {t_pre * self.n_pre / P + t_qs * self.n_query / P + t_blend:.1f} s")
+        return total, desc
 
 
 def run_reference(args):
@@ -150,12 +157,13 @@ def run_reference(args):
     sc_meta = scenes.CONFIGS[args.config]
     times = []
     desc = ""
+    smp = OracleSample(args.config, seed=0, n_pre=200_000, n_query=20_000, n_tiles_sample=48)
     for i in range(args.warmup + args.steps):
-        t, desc, meta = oracle_sample(args.config, seed=0, n_pre=50_000, n_query=5_000, n_tiles_sample=12)
+        t, desc = smp.step()
         if i >= args.warmup:
             times.append(t)
     t = float(np.mean(times))
-    val = meta["n_pix"] / t
+    val = smp.n_pix / t
     line = dict(metric=METRIC, value=val, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup, ms_per_step=t * 1e3,
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic", impl="reference",
                 config=dict(workload=f"config{args.config}:{sc_meta['name']}", order=sc_meta["order"], n_gauss=sc_meta["n_gauss"],
@@ -314,8 +322,9 @@ def run_ours(args):
     # ranges 1; blend fwd 1; blend bwd 1; preprocess bwd 1
     line["gpu_launches"] = args.steps * (1 + (2 + dpass * 5 + dpass % 2) + 8 + (passes * 5 + passes % 2) + 4)
     if not args.no_cpu_baseline:
-        t, desc, meta = oracle_sample(args.config, seed=0)
-        line["cpu_baseline"] = dict(value=meta["n_pix"] / t, unit=UNIT, cores=1, kind="oracle", sample=desc)
+        smp = OracleSample(args.config, seed=0, n_pre=400_000, n_query=40_000, n_tiles_sample=96)
+        t, desc = smp.step()
+        line["cpu_baseline"] = dict(value=smp.n_pix / t, unit=UNIT, cores=1, kind="oracle", sample=desc)
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -90,6 +90,55 @@ __device__ __forceinline__ bool leaf_inside(const QueryParams& qp, const Disc& D
   return D.u[0] * cx + D.u[1] * cy + D.u[2] * cz >= D.cosR;
 }
 
+__device__ __forceinline__ uint32_t spread_bits16(uint32_t v) {          // 16 bits -> even bit positions
+  v &= 0xffffu;
+  v = (v | (v << 8)) & 0x00ff00ffu;
+  v = (v | (v << 4)) & 0x0f0f0f0fu;
+  v = (v | (v << 2)) & 0x33333333u;
+  v = (v | (v << 1)) & 0x55555555u;
+  return v;
+}
+
+// A tile that the zone tests leave undecided: does any of its 4^(k_q-k_t) query pixels satisfy the defining predicate?
+// Straight-line loop over the leaves with the face / tile decode shared (about 25 instructions per leaf, early exit), instead
+// of walking two more quadtree levels node by node (measured: the leaf levels were most of the walk).
+__device__ __forceinline__ bool any_leaf_inside(const QueryParams& qp, const Disc& D, uint32_t tile) {
+  const int kt = qp.kt, kq = qp.kq, ref = kq - kt, m = 1 << ref;
+  const int f = (int)(tile >> (2 * kt));
+  const uint32_t mt = tile & ((1u << (2 * kt)) - 1u);
+  const int x0 = (int)squeeze_even_bits32(mt) << ref, y0 = (int)squeeze_even_bits32(mt >> 1) << ref;
+  const int N = 1 << kq, r = f >> 2, c = f & 3;
+  const int base_i = (r + 2) * N - 1;                                     // ring = base_i - (x + y)
+  const float Fc = (float)(2 * c + 1 - (r & 1));
+  const float invN = __int_as_float((127 - kq) << 23);
+  const float inv3N2 = 0.333333343f * invN * invN;
+  const float T = 2.0f * D.sh;
+  for (int dy = 0; dy < m; ++dy) {
+    for (int dx = 0; dx < m; ++dx) {
+      const int x = x0 + dx, y = y0 + dy;
+      const int i = base_i - (x + y), h = x - y;
+      float z, sth, q;
+      if (i < N) { const float fn = (float)i; const float w = fn * fn * inv3N2; z = 1.0f - w; sth = sqrtf(w * (2.0f - w)); q = __fdividef((float)h, fn); }
+      else if (i > 3 * N) { const float fn = (float)(4 * N - i); const float w = fn * fn * inv3N2; z = w - 1.0f; sth = sqrtf(w * (2.0f - w)); q = __fdividef((float)h, fn); }
+      else { z = (float)(2 * (2 * N - i)) * (0.333333343f * invN); sth = sqrtf((1.0f - z) * (1.0f + z)); q = (float)h * invN; }
+      q += Fc;
+      if (q > 4.0f) q -= 8.0f;
+      float sn, cs;
+      __sincosf(q * 0.78539816339744831f, &sn, &cs);
+      const float ex = D.uf[0] - sth * sn, ey = D.uf[1] - z, ez = D.uf[2] - sth * cs;
+      const float chord = sqrtf(ex * ex + ey * ey + ez * ez);
+      if (chord < T - kDelta) return true;
+      if (chord <= T + kDelta) {                                          // inside the fp32 margin: the exact predicate decides
+        const uint32_t p = ((uint32_t)f << (2 * kq)) | spread_bits16((uint32_t)x) | (spread_bits16((uint32_t)y) << 1);
+        double cx, cy, cz;
+        pix_center_cam(kq, (uint64_t)p, cx, cy, cz);
+        if (D.u[0] * cx + D.u[1] * cy + D.u[2] * cz >= D.cosR) return true;
+      }
+    }
+  }
+  return false;
+}
+
 // Depth-first walk of the subtrees rooted at the order-ro nodes rp0..rp1 (inclusive), one node per step().
 // Sink: add(tile), add_range(t0,t1), has(tile).  The climb after a finished subtree is a count of trailing 11 bit pairs,
 // so a step has no data-dependent loop in its control path.  Callers drive step() from a WARP-SYNCHRONOUS loop
@@ -100,7 +149,9 @@ struct Walker {
   uint32_t p, rp1;               // a NESTED index at order <= 13 fits 32 bits
   __device__ __forceinline__ void start(int ro_, uint32_t rp0, uint32_t rp1_) { o = ro = ro_; p = rp0; rp1 = rp1_; }
   // returns true when the walk is finished
-  template <class Sink>
+  // LEAF_LOOP: undecided tiles are settled by any_leaf_inside (pays off in the block path, where idle lanes refill
+  // themselves; in the thread-per-Gaussian path the long inner loop costs more in divergence than it saves: measured)
+  template <bool LEAF_LOOP, class Sink>
   __device__ __forceinline__ bool step(const QueryParams& qp, const Disc& D, Sink& sink) {
     const int kt = qp.kt, kq = qp.kq;
     float chord;
@@ -109,6 +160,7 @@ struct Walker {
     if (z != kOutside) {
       if (o <= kt) {
         if (z == kInside) { const int sh = 2 * (kt - o); sink.add_range((int64_t)p << sh, (int64_t)(p + 1) << sh); }
+        else if (LEAF_LOOP && o == kt && kq > kt) { if (any_leaf_inside(qp, D, p)) sink.add((int64_t)p); }      // undecided tile: test its leaves
         else descend = true;
       } else {
         const int64_t tile = (int64_t)(p >> (2 * (o - kt)));
@@ -250,7 +302,7 @@ small_body(int64_t block, const QueryParams& qp, const float* __restrict__ dir, 
   Walker w;
   w.start(0, 0, 11);
   while (__any_sync(0xffffffffu, running)) {
-    if (running) running = !w.step(qp, D, sink);
+    if (running) running = !w.step<false>(qp, D, sink);
   }
   if (!EMIT && valid) counts[slot] = sink.count;
 }
@@ -355,7 +407,7 @@ large_body(int n_blocks, const QueryParams& qp, const float* __restrict__ dir, c
           else exhausted = true;
         }
         if (!__any_sync(0xffffffffu, active)) break;
-        if (active) active = !w.step(qp, D, sink);
+        if (active) active = !w.step<true>(qp, D, sink);
       }
     }
     __syncthreads();

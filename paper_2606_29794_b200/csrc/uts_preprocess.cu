@@ -135,7 +135,7 @@ __device__ __forceinline__ void geometry(const ViewConst& vc, const double mu[3]
   if (!(g.det > 0) || !isfinite(g.det)) g.culled = true;                   // reading A23
 }
 
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, 6)
 preprocess_fwd_kernel(uts_config cfg, const float* __restrict__ means, const float* __restrict__ scales,
                       const float* __restrict__ quats, const float* __restrict__ opac, const float* __restrict__ sh,
                       const float* __restrict__ Wv, const float* __restrict__ bv, uts_proj out, double h) {
@@ -224,7 +224,7 @@ preprocess_fwd_kernel(uts_config cfg, const float* __restrict__ means, const flo
 //   e = e(omega), n = n(omega,phi), u = u(omega,phi):  de/domega = -hh, dn/domega = -sin(phi) e, dn/dphi = -u,
 //   with hh = cos(phi) u - sin(phi) n the horizontal unit vector;  d omega/dt = e / rxz,  d phi/dt = n / rho,  d rho/dt = u.
 // The three paths of PAPER.md:91-96 (mu' path, J path, S_phi path) are this single chain written in the (e,n,u) frame.
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, 4)
 preprocess_bwd_kernel(uts_config cfg, const float* __restrict__ means, const float* __restrict__ scales,
                       const float* __restrict__ quats, const float* __restrict__ sh, const float* __restrict__ Wv,
                       const float* __restrict__ bv, const uint8_t* __restrict__ flags, const float* __restrict__ dL_drgb,
@@ -260,11 +260,32 @@ preprocess_bwd_kernel(uts_config cfg, const float* __restrict__ means, const flo
     float Y[16];
     sh_basis_eval<float>(deg, dx, dy, dz, Y);
     float cmix[16];                                      // sum_ch g_ch sh[m,ch]
-    for (int m = 0; m < M; ++m) {
-      const float c0 = __ldg(shp + 3 * m), c1 = __ldg(shp + 3 * m + 1), c2 = __ldg(shp + 3 * m + 2);
-      cmix[m] = gr[0] * c0 + gr[1] * c1 + gr[2] * c2;
-      if (first) { gsh[3 * m] = Y[m] * gr[0]; gsh[3 * m + 1] = Y[m] * gr[1]; gsh[3 * m + 2] = Y[m] * gr[2]; }
-      else { gsh[3 * m] += Y[m] * gr[0]; gsh[3 * m + 1] += Y[m] * gr[1]; gsh[3 * m + 2] += Y[m] * gr[2]; }
+    if (M == 16) {                                       // degree 3: 48 floats = 12 aligned float4 in and out
+#pragma unroll
+      for (int m = 0; m < 16; ++m) cmix[m] = 0.f;
+      const float4* s4 = reinterpret_cast<const float4*>(shp);
+      float4* g4 = reinterpret_cast<float4*>(gsh);
+#pragma unroll
+      for (int j = 0; j < 12; ++j) {
+        const float4 c4 = __ldg(s4 + j);
+        const float cc[4] = {c4.x, c4.y, c4.z, c4.w};
+        float o4[4];
+#pragma unroll
+        for (int l = 0; l < 4; ++l) {
+          const int idx = 4 * j + l;                       // = 3 m + ch, compile-time after unrolling
+          cmix[idx / 3] += gr[idx % 3] * cc[l];
+          o4[l] = Y[idx / 3] * gr[idx % 3];
+        }
+        if (first) g4[j] = make_float4(o4[0], o4[1], o4[2], o4[3]);
+        else { float4 p4 = g4[j]; g4[j] = make_float4(p4.x + o4[0], p4.y + o4[1], p4.z + o4[2], p4.w + o4[3]); }
+      }
+    } else {
+      for (int m = 0; m < M; ++m) {
+        const float c0 = __ldg(shp + 3 * m), c1 = __ldg(shp + 3 * m + 1), c2 = __ldg(shp + 3 * m + 2);
+        cmix[m] = gr[0] * c0 + gr[1] * c1 + gr[2] * c2;
+        if (first) { gsh[3 * m] = Y[m] * gr[0]; gsh[3 * m + 1] = Y[m] * gr[1]; gsh[3 * m + 2] = Y[m] * gr[2]; }
+        else { gsh[3 * m] += Y[m] * gr[0]; gsh[3 * m + 1] += Y[m] * gr[1]; gsh[3 * m + 2] += Y[m] * gr[2]; }
+      }
     }
     float gvx, gvy, gvz;
     sh_dir_grad(deg, dx, dy, dz, cmix, gvx, gvy, gvz);

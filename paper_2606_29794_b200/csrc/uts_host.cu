@@ -94,7 +94,21 @@ int uts_host_forward_backward(const uts_config* cfg, const float* h_means, const
   UTS_CUDA(cudaMemcpyAsync(L.sh, h_sh, 3 * M * P * f, cudaMemcpyHostToDevice, s));
   UTS_CUDA(cudaMemcpyAsync(L.W, h_W, 9 * V * f, cudaMemcpyHostToDevice, s));
   UTS_CUDA(cudaMemcpyAsync(L.b, h_b, 3 * V * f, cudaMemcpyHostToDevice, s));
-  if (bwd) UTS_CUDA(cudaMemcpyAsync(L.g_color, h_dL_dcolor, 3 * npx * f, cudaMemcpyHostToDevice, s));
+  // A second, library-private stream carries the copies that are not on the critical path: the upstream gradient goes up while
+  // the forward runs, the image comes down while the backward runs (effective with pinned host buffers).
+  cudaStream_t s2 = nullptr;
+  cudaEvent_t ev_up = nullptr, ev_fwd = nullptr, ev_start = nullptr;
+  UTS_CUDA(cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking));
+  UTS_CUDA(cudaEventCreateWithFlags(&ev_up, cudaEventDisableTiming));
+  UTS_CUDA(cudaEventCreateWithFlags(&ev_fwd, cudaEventDisableTiming));
+  UTS_CUDA(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
+  struct Cleanup { cudaStream_t s2; cudaEvent_t a, b, c; ~Cleanup() { cudaStreamSynchronize(s2); cudaEventDestroy(a); cudaEventDestroy(b); cudaEventDestroy(c); cudaStreamDestroy(s2); } } cleanup{s2, ev_up, ev_fwd, ev_start};
+  UTS_CUDA(cudaEventRecord(ev_start, s));                 // s2 must not run ahead of work already queued on the caller's stream
+  UTS_CUDA(cudaStreamWaitEvent(s2, ev_start, 0));
+  if (bwd) {
+    UTS_CUDA(cudaMemcpyAsync(L.g_color, h_dL_dcolor, 3 * npx * f, cudaMemcpyHostToDevice, s2));
+    UTS_CUDA(cudaEventRecord(ev_up, s2));
+  }
 
   uts_gaussians g{L.means, L.scales, L.quats, L.opac, L.sh};
   uts_views vw{L.W, L.b};
@@ -106,9 +120,12 @@ int uts_host_forward_backward(const uts_config* cfg, const float* h_means, const
   if ((st = uts_sort(cfg, n, L.keys, L.vals, L.keys_tmp, L.vals_tmp, 1, L.sort_scratch, L.sort_bytes, stream))) return st;
   if ((st = uts_tile_ranges(cfg, n, L.keys, L.ranges, stream))) return st;
   if ((st = uts_render_fwd(cfg, L.proj, mask, L.ranges, L.vals, L.color, L.alpha, L.trans, L.n_last, stream))) return st;
-  UTS_CUDA(cudaMemcpyAsync(h_color, L.color, 3 * npx * f, cudaMemcpyDeviceToHost, s));
-  if (h_alpha) UTS_CUDA(cudaMemcpyAsync(h_alpha, L.alpha, npx * f, cudaMemcpyDeviceToHost, s));
+  UTS_CUDA(cudaEventRecord(ev_fwd, s));
+  UTS_CUDA(cudaStreamWaitEvent(s2, ev_fwd, 0));
+  UTS_CUDA(cudaMemcpyAsync(h_color, L.color, 3 * npx * f, cudaMemcpyDeviceToHost, s2));
+  if (h_alpha) UTS_CUDA(cudaMemcpyAsync(h_alpha, L.alpha, npx * f, cudaMemcpyDeviceToHost, s2));
   if (bwd) {
+    UTS_CUDA(cudaStreamWaitEvent(s, ev_up, 0));
     if ((st = uts_render_bwd(cfg, L.proj, mask, L.ranges, L.vals, L.trans, L.n_last, L.g_color, nullptr, L.g_rgb, L.g_conic,
                              L.g_mu2, L.g_opac, stream)))
       return st;
@@ -120,6 +137,7 @@ int uts_host_forward_backward(const uts_config* cfg, const float* h_means, const
     UTS_CUDA(cudaMemcpyAsync(h_dL_dopac, L.g_opac, P * f, cudaMemcpyDeviceToHost, s));
     UTS_CUDA(cudaMemcpyAsync(h_dL_dsh, L.g_sh, 3 * M * P * f, cudaMemcpyDeviceToHost, s));
   }
+  UTS_CUDA(cudaStreamSynchronize(s2));
   UTS_CUDA(cudaStreamSynchronize(s));
   return UTS_OK;
 }

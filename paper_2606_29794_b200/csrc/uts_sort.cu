@@ -16,7 +16,13 @@
 namespace uts {
 
 constexpr int kSortThreads = 256;
-constexpr int kSortItems = 12;
+#ifndef UTS_SORT_ITEMS
+#define UTS_SORT_ITEMS 12
+#endif
+#ifndef UTS_SORT_MINB
+#define UTS_SORT_MINB 3
+#endif
+constexpr int kSortItems = UTS_SORT_ITEMS;
 constexpr int kSortTile = kSortThreads * kSortItems;     // 3072 pairs per block (47 KB of static shared memory)
 constexpr int kSortWarps = kSortThreads / 32;
 constexpr int kRadix = 256;
@@ -45,14 +51,15 @@ sort_upsweep(const uint64_t* __restrict__ keys, uint64_t n, int shift, uint32_t 
   }
 }
 
-__global__ void __launch_bounds__(kSortThreads, 3)
+__global__ void __launch_bounds__(kSortThreads, UTS_SORT_MINB)
 sort_downsweep(const uint64_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in, uint64_t* __restrict__ keys_out,
                uint32_t* __restrict__ vals_out, uint64_t n, int shift, uint32_t nb, const uint64_t* __restrict__ offsets) {
   __shared__ uint32_t whist[kSortWarps][kRadix];      // per-warp digit counts, then per-warp exclusive bases
   __shared__ uint32_t dstart[kRadix];                 // start of each digit's run inside the block
   __shared__ uint64_t gbase[kRadix];                  // global start of this block's run of each digit
-  __shared__ uint64_t skeys[kSortTile];
-  __shared__ uint32_t svals[kSortTile];
+  extern __shared__ uint64_t sort_dyn[];
+  uint64_t* skeys = sort_dyn;                                            // [kSortTile]
+  uint32_t* svals = reinterpret_cast<uint32_t*>(sort_dyn + kSortTile);   // [kSortTile]
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const uint32_t lt_mask = (1u << lane) - 1u;
   for (int i = threadIdx.x; i < kSortWarps * kRadix; i += kSortThreads) (&whist[0][0])[i] = 0;
@@ -181,13 +188,14 @@ static int radix_sort_bytes(uint64_t n_pairs, uint64_t* keys, uint32_t* vals, ui
   uint64_t* offs = reinterpret_cast<uint64_t*>(sp);              sp += (((m + 1) * 8 + 255) / 256) * 256;
   uint64_t* block_sums = reinterpret_cast<uint64_t*>(sp);
   uint64_t* kin = keys; uint32_t* vin = vals; uint64_t* kout = keys_tmp; uint32_t* vout = vals_tmp;
+  UTS_CUDA(cudaFuncSetAttribute(sort_downsweep, cudaFuncAttributeMaxDynamicSharedMemorySize, kSortTile * 12));
   for (int pass = 0; pass < n_bytes; ++pass) {
     const int shift = 8 * (first_byte + pass);
     sort_upsweep<<<nb, kSortThreads, 0, s>>>(kin, n_pairs, shift, nb, counts);
     UTS_LAUNCH_CHECK();
     int st = exclusive_scan_u32(counts, (int64_t)m, offs, block_sums, s);
     if (st) return st;
-    sort_downsweep<<<nb, kSortThreads, 0, s>>>(kin, vin, kout, vout, n_pairs, shift, nb, offs);
+    sort_downsweep<<<nb, kSortThreads, kSortTile * 12, s>>>(kin, vin, kout, vout, n_pairs, shift, nb, offs);
     UTS_LAUNCH_CHECK();
     uint64_t* tk = kin; kin = kout; kout = tk;
     uint32_t* tv = vin; vin = vout; vout = tv;

@@ -4,7 +4,8 @@
  *
  *   uts_preprocess      Alg.1 l.2-8   (Eq.1-2): projection to the unit sphere, Sigma_arc, conic, r_s, colour
  *   uts_depth_order     (optional) radial-depth order of the Gaussians, lets the sort skip its depth passes
- *   uts_tile_query      Alg.1 l.9-14  (Alg.2): NESTED tile query, emits ((tile,rho),i) pairs
+ *   uts_tile_query      Alg.1 l.9-14  (Alg.2; Alg.3 PAPER.md:635-684 with query_mode = RING): tile query, emits
+ *                       ((tile,rho),i) pairs
  *   uts_sort            Alg.1 l.15: stable radix sort of the pairs by (tile, radial depth)
  *   uts_tile_ranges     Alg.1 l.16: per-tile [start,end)
  *   uts_render_fwd      Alg.1 l.17-30 (Eq.6) + FoV mask
@@ -57,7 +58,12 @@ typedef struct {
   float alpha_max;         /* alpha = min(alpha_max, o*exp(power)); gradient zero when clamped     reading A7 */
   float t_eps;             /* stop after the update when T < t_eps                                 Alg.1 l.27 PAPER.md:578 */
   float bg[3];             /* out = C + T*bg                                                       reading A8 */
+  int   query_mode;        /* UTS_QUERY_NESTED (0): Alg.2's set, centres within r_s + PixRad(k_q)  PAPER.md:599-620, reading A6
+                              UTS_QUERY_RING   (1): Alg.3's set, centres within r_s (the paper's default "R", non-conservative)
+                                                                                                   PAPER.md:104-108, 635-684 */
 } uts_config;
+
+enum { UTS_QUERY_NESTED = 0, UTS_QUERY_RING = 1 };
 
 /* Gaussian set G = {mu, s, q, o, c} (Alg.1 Require), SoA. */
 typedef struct {

@@ -35,7 +35,8 @@ def build(force: bool = False) -> str:
 class _Cfg(C.Structure):
     _fields_ = [("order", C.c_int), ("tile_log2", C.c_int), ("query_refine_log2", C.c_int), ("sh_degree", C.c_int),
                 ("n_gauss", C.c_int), ("n_views", C.c_int), ("r_near", C.c_float), ("cov_dilation_px2", C.c_float),
-                ("alpha_min", C.c_float), ("alpha_max", C.c_float), ("t_eps", C.c_float), ("bg", C.c_float * 3)]
+                ("alpha_min", C.c_float), ("alpha_max", C.c_float), ("t_eps", C.c_float), ("bg", C.c_float * 3),
+                ("query_mode", C.c_int)]
 
 
 @dataclass
@@ -52,6 +53,7 @@ class Config:
     alpha_max: float = 0.99
     t_eps: float = 1e-4
     bg: tuple = (0.0, 0.0, 0.0)
+    query_mode: int = 0          # 0 NESTED descent (Alg.2), 1 RING scan (Alg.3)
 
     @property
     def n_pix(self): return 12 << (2 * self.order)
@@ -66,7 +68,8 @@ class Config:
 
     def c(self) -> _Cfg:
         return _Cfg(self.order, self.tile_log2, self.query_refine_log2, self.sh_degree, self.n_gauss, self.n_views,
-                    self.r_near, self.cov_dilation_px2, self.alpha_min, self.alpha_max, self.t_eps, (C.c_float * 3)(*self.bg))
+                    self.r_near, self.cov_dilation_px2, self.alpha_min, self.alpha_max, self.t_eps, (C.c_float * 3)(*self.bg),
+                    self.query_mode)
 
 
 _lib = None

@@ -132,6 +132,19 @@ int64_t ring_npix_in_ring(int order, int64_t i) {
   return 4 * std::min(i, std::min(n, 4 * n - i));
 }
 
+// RingInfo of Alg.3, from the ring form D2: ring i holds npix = 4*n_r pixels at longitudes
+// lam0 + j * 2pi/npix, j = 0..npix-1, lam0 = (1 - (kshift+1)/2) * pi / (2 n_r).
+RingInfo ring_info(int order, int64_t i) {
+  int64_t n = (int64_t)1 << order, npix = 12 * n * n, ncap = 2 * n * (n - 1);
+  int64_t nr; int kshift; int64_t first;
+  if (i < n) { nr = i; kshift = 0; first = 2 * i * (i - 1); }
+  else if (i > 3 * n) { nr = 4 * n - i; kshift = 0; first = npix - 2 * nr * (nr + 1); }
+  else { nr = n; kshift = (int)((i - n) & 1); first = ncap + (i - n) * 4 * n; }
+  ZPhi c = ring_coords_to_zphi(order, i, nr, 1, kshift);
+  RingInfo r; r.z = c.z; r.npix = 4 * nr; r.lam0 = c.lam; r.first = first;
+  return r;
+}
+
 static int64_t isqrt64(int64_t v) {
   int64_t r = (int64_t)std::sqrt((double)v);
   while (r * r > v) --r;

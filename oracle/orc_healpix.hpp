@@ -34,6 +34,10 @@ int64_t nest2ring(int order, int64_t p);
 ZPhi    ring_center(int order, int64_t r);           // textbook pix2ang in RING order
 int64_t ring2nest(int order, int64_t r);             // = ang2pix_nest(ring_center(r))
 int64_t ring_npix_in_ring(int order, int64_t i);     // ring i in [1,4Nside-1] has 4*min(i,Nside,4Nside-i) pixels
+// RingInfo(i_r) of Alg.3 l.7: z of the ring, its pixel count, the longitude of its first pixel, and the
+// RING index of that first pixel (so that Ring2Nest(i_r, j) = ring2nest(first + j)).
+struct RingInfo { double z; int64_t npix; double lam0; int64_t first; };
+RingInfo ring_info(int order, int64_t i);
 // sphere -> pixel (inverse of D1)
 int64_t ang2pix_nest(int order, double z, double lam);
 

@@ -232,12 +232,71 @@ struct Descent {
 };
 }  // namespace
 
+// Alg.3 QUERYDISCRING (§10.2; Eq.5), step by step at the query
+// resolution N_side^q = 2^k_q, results mapped back to tile resolution.  Line numbers are Alg.3's.
+// Readings: A17 (z-bounds from l.2-3, not the garbled prose), A18 (l.19-20 = ceil / floor: the pixels whose centres lie in
+// the longitude interval), epsilon of l.9 = 1e-12 (unstated).  Output sorted ascending, each tile once (the ABI's order).
+static void query_disc_ring(const Config& cfg, const double u[3], double rs, const int32_t* slot, std::vector<uint32_t>& out,
+                            QueryStats& st) {
+  const int kt = tile_order(cfg), kq = query_order(cfg);
+  const int64_t N = (int64_t)1 << kq;                                         // l.1
+  const double omega = std::atan2(u[0], u[2]);                                // disc centre (omega, phi), Eq.1
+  const double phi = std::atan2(u[1], std::sqrt(u[0] * u[0] + u[2] * u[2]));
+  const double zc = std::sin(phi);                                            // l.1
+  const double phimin = std::max(-kPi / 2, phi - rs), phimax = std::min(kPi / 2, phi + rs);   // l.2
+  const double zmin = std::sin(phimin), zmax = std::sin(phimax);              // l.3
+  const double cosrs = std::cos(rs);
+  // l.4 ZToRingRange: the rings whose z lies in [zmin, zmax] (z decreases with the ring number)
+  static std::map<int, std::vector<double>> ring_z_cache;                     // z of every ring of an order, computed once
+  std::vector<double>& ring_z = ring_z_cache[kq];
+  if (ring_z.empty()) { ring_z.assign(4 * N, 2.0); for (int64_t i = 1; i <= 4 * N - 1; ++i) ring_z[i] = ring_info(kq, i).z; }
+  int64_t ir_min = 4 * N, ir_max = 0;
+  for (int64_t i = 1; i <= 4 * N - 1; ++i)
+    if (ring_z[i] >= zmin && ring_z[i] <= zmax) { ir_min = std::min(ir_min, i); ir_max = std::max(ir_max, i); }
+  std::vector<uint32_t> found;
+  auto add = [&](const RingInfo& ri, int64_t j) {                             // Ring2Nest(i_r, j), then the ancestor tile
+    int64_t p = ring2nest(kq, ri.first + j);
+    int64_t tile = p >> (2 * (kq - kt));
+    if (slot && slot[tile] < 0) return;
+    found.push_back((uint32_t)tile);
+  };
+  auto margin = [&](const RingInfo& ri, int64_t j) {                          // instrumentation only: distance of a centre to the disc edge
+    j = ((j % ri.npix) + ri.npix) % ri.npix;
+    double c[3]; to_cam_vec(ring_center(kq, ri.first + j), c);
+    st.min_margin = std::min(st.min_margin, std::fabs(u[0] * c[0] + u[1] * c[1] + u[2] * c[2] - cosrs));
+  };
+  for (int64_t ir = ir_min; ir <= ir_max; ++ir) {                             // l.5
+    const RingInfo ri = ring_info(kq, ir);                                    // l.7 (z_r, n_r, omega_0)
+    st.node_tests++;
+    const double delta = std::sqrt(std::max(0.0, 1 - zc * zc)) * std::sqrt(std::max(0.0, 1 - ri.z * ri.z));   // l.8
+    if (delta < 1e-12) {                                                      // l.9 disc centre or ring at a pole
+      if (zc * ri.z >= cosrs) for (int64_t j = 0; j < ri.npix; ++j) add(ri, j);   // l.10-11
+      continue;                                                               // l.13
+    }
+    const double cw = (cosrs - zc * ri.z) / delta;                            // l.15, Eq.5
+    if (cw <= -1) { for (int64_t j = 0; j < ri.npix; ++j) add(ri, j); }       // l.16-17 full ring
+    else if (cw < 1) {                                                        // l.18
+      const double dw = std::acos(std::min(1.0, std::max(-1.0, cw)));
+      const double a = (omega - dw - ri.lam0) * (double)ri.npix / (2 * kPi);  // l.19
+      const double b = (omega + dw - ri.lam0) * (double)ri.npix / (2 * kPi);  // l.20
+      const int64_t ipmin = (int64_t)std::ceil(a), ipmax = (int64_t)std::floor(b);
+      margin(ri, ipmin); margin(ri, ipmin - 1); margin(ri, ipmax); margin(ri, ipmax + 1);
+      if (ipmax - ipmin + 1 >= ri.npix) { for (int64_t j = 0; j < ri.npix; ++j) add(ri, j); }
+      else for (int64_t ip = ipmin; ip <= ipmax; ++ip) add(ri, ((ip % ri.npix) + ri.npix) % ri.npix);   // l.21-22
+    }
+  }
+  std::sort(found.begin(), found.end());
+  found.erase(std::unique(found.begin(), found.end()), found.end());
+  out = found;                                                                // l.26
+}
+
 void tile_query_one(const Config& cfg, const double dir_in[3], double rs, const int32_t* slot_of_tile, bool brute,
                     std::vector<uint32_t>& tiles_out, QueryStats& st) {
   int kt = tile_order(cfg), kq = query_order(cfg);
   double nrm = std::sqrt(dir_in[0] * dir_in[0] + dir_in[1] * dir_in[1] + dir_in[2] * dir_in[2]);
   double u[3] = {dir_in[0] / nrm, dir_in[1] / nrm, dir_in[2] / nrm};
-  double R = std::min(kPi, rs + rho_max_cached(kq));
+  // NESTED (Alg.2, reading A6): centres within r_s + PixRad(k_q).  RING (Alg.3): centres within r_s itself.
+  double R = cfg.query_mode == 1 ? std::min(kPi, rs) : std::min(kPi, rs + rho_max_cached(kq));
   double cosR = std::cos(R);
   tiles_out.clear();
   if (brute) {
@@ -256,6 +315,7 @@ void tile_query_one(const Config& cfg, const double dir_in[3], double rs, const 
     }
     return;
   }
+  if (cfg.query_mode == 1) { query_disc_ring(cfg, u, R, slot_of_tile, tiles_out, st); return; }
   Descent D{&cfg, u, R, cosR, kt, kq, slot_of_tile, &tiles_out, &st};
   for (int64_t f = 0; f < 12; ++f) D.visit(f, 0);
 }

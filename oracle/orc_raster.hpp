@@ -9,6 +9,8 @@
 //   preprocess      : isotropic closed form, literal Eq.2 == tangent-basis form, J == finite differences of Eq.1,
 //                     degree-0 colour, SH orthonormality by quadrature on the HEALPix grid
 //   tile query      : brute force every-Gaussian x every-order-k_q-pixel == descent; superset property; r_s>=pi
+//   RING tile query : Alg.3 == brute force "order-k_q centres within r_s" (every Gaussian x every pixel); subset of the
+//                     NESTED set; z-range / full-ring / pole branches exercised by discs over the poles
 //   sort / ranges   : permutation + order properties
 //   blend forward   : single isotropic Gaussian closed form (independent haversine), two-Gaussian closed form,
 //                     permutation invariance, 4-fold rotation symmetry
@@ -31,6 +33,7 @@ struct Config {                 // oracle's own definition (same meaning as the 
   float cov_dilation_px2;       // h = value * Omega_pix added to diag(Sigma_arc)     reading A3
   float alpha_min, alpha_max, t_eps;   //                                             reading A7
   float bg[3];                  //                                                    reading A8
+  int   query_mode;             // 0: NESTED descent, Alg.2 (reading A6); 1: RING scan, Alg.3 (readings A17, A18)
 };
 
 inline int  tile_order(const Config& c) { return c.order - c.tile_log2; }            // k_t, Table 6
@@ -71,6 +74,8 @@ void sh_basis_grad(int degree, const double d[3], double* dY /*[16][3]*/);
 struct QueryStats { double min_margin; int64_t node_tests; };
 
 // Tile set of one Gaussian.  brute=true: literal loop over every order-k_q pixel.
+// cfg.query_mode 0: the NESTED set (centres within r_s + rho_max(k_q), reading A6) by a safe descent;
+// cfg.query_mode 1: Alg.3 QueryDiscRing step by step (centres within r_s).
 void tile_query_one(const Config& cfg, const double dir[3], double rs, const int32_t* slot_of_tile /*may be null*/,
                     bool brute, std::vector<uint32_t>& tiles_out, QueryStats& st);
 

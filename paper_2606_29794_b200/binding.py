@@ -37,7 +37,8 @@ class UtsError(RuntimeError):
 class CConfig(C.Structure):
     _fields_ = [("order", C.c_int), ("tile_log2", C.c_int), ("query_refine_log2", C.c_int), ("sh_degree", C.c_int),
                 ("n_gauss", C.c_int), ("n_views", C.c_int), ("r_near", C.c_float), ("cov_dilation_px2", C.c_float),
-                ("alpha_min", C.c_float), ("alpha_max", C.c_float), ("t_eps", C.c_float), ("bg", C.c_float * 3)]
+                ("alpha_min", C.c_float), ("alpha_max", C.c_float), ("t_eps", C.c_float), ("bg", C.c_float * 3),
+                ("query_mode", C.c_int)]
 
 
 class CGaussians(C.Structure):
@@ -71,6 +72,7 @@ class Config:
     alpha_max: float = 0.99
     t_eps: float = 1e-4
     bg: tuple = (0.0, 0.0, 0.0)
+    query_mode: int = 0          # UTS_QUERY_NESTED (Alg.2) / 1 = UTS_QUERY_RING (Alg.3)
 
     @property
     def n_pix(self): return 12 << (2 * self.order)
@@ -83,7 +85,8 @@ class Config:
 
     def c(self) -> CConfig:
         return CConfig(self.order, self.tile_log2, self.query_refine_log2, self.sh_degree, self.n_gauss, self.n_views,
-                       self.r_near, self.cov_dilation_px2, self.alpha_min, self.alpha_max, self.t_eps, (C.c_float * 3)(*self.bg))
+                       self.r_near, self.cov_dilation_px2, self.alpha_min, self.alpha_max, self.t_eps, (C.c_float * 3)(*self.bg),
+                       self.query_mode)
 
 
 _lib = None

@@ -24,6 +24,7 @@ int check_config(const uts_config* c) {
   if (c->order < c->tile_log2 || c->order > kMaxOrder) return UTS_ERR_INVALID_ARG;
   if (c->query_refine_log2 < 0 || c->query_refine_log2 > c->tile_log2) return UTS_ERR_INVALID_ARG;
   if (c->sh_degree < 0 || c->sh_degree > 3) return UTS_ERR_INVALID_ARG;
+  if (c->query_mode != UTS_QUERY_NESTED && c->query_mode != UTS_QUERY_RING) return UTS_ERR_INVALID_ARG;
   if (c->n_gauss < 0 || c->n_views < 1) return UTS_ERR_INVALID_ARG;
   if ((int64_t)c->n_gauss * c->n_views > (int64_t)0x7fffffff) return UTS_ERR_UNSUPPORTED;
   if ((((int64_t)12 << (2 * (c->order - c->tile_log2))) * c->n_views) > (int64_t)0xffffffffll) return UTS_ERR_UNSUPPORTED;

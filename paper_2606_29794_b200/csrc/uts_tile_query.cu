@@ -35,7 +35,7 @@ struct QueryParams {
   int n_words;                          // bitmap words = n_tile / 32 (0: block path disabled)
   int wl_cap;                           // capacity of each of the two block work lists
   int64_t n_tile;
-  double rho_q;                         // rho_max(k_q)
+  double rho_q;                         // rho_max(k_q) (NESTED set) or 0 (RING set): R = min(pi, r_s + rho_q)
   float r_large;                        // discs with R above this go to the block path
   uint32_t* tile_cache;                 // [V*P][kTileCacheK] tiles found by the count pass (thread path), reused by the emit pass
   uint32_t* bitmap_cache;               // [bitmap_cache_cap][n_words] bitmaps of the count pass (block path)
@@ -517,7 +517,7 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   QueryParams qp;
   qp.kt = d.kt; qp.kq = d.kq; qp.P = d.P; qp.V = d.V; qp.n_tile = d.n_tile;
   const double* rm = rho_max_table_host();
-  qp.rho_q = rm[d.kq];
+  qp.rho_q = cfg->query_mode == UTS_QUERY_RING ? 0.0 : rm[d.kq];      // Alg.3's set has no PixRad margin
   for (int o = 0; o <= kMaxOrder; ++o) { qp.rho[o] = (float)rm[o]; qp.sin_hrho[o] = (float)sin(0.5 * rm[o]); qp.cos_hrho[o] = (float)cos(0.5 * rm[o]); }
   qp.os = d.kt < 4 ? d.kt : 4;
   const size_t n_split = (size_t)12 << (2 * qp.os);

@@ -52,18 +52,18 @@ class Case:
     """Oracle results for one shrunk config, computed once per test session."""
     _cache = {}
 
-    def __init__(self, cfg_id, P, order, extra):
+    def __init__(self, cfg_id, P, order, extra, query_mode=0):
         self.scene = small_scene(cfg_id, P, order, **extra)
-        self.ocfg = ocfg(self.scene)
+        self.ocfg = ocfg(self.scene, query_mode=query_mode)
         self.bits, self.act, self.slot = oracle_mask(self.ocfg, self.scene)
         self.fw = orc.forward_chain(self.ocfg, self.scene, self.slot, self.act, self.bits)
         assert self.fw["qinfo"]["min_margin"] > 1e-12, "margin certificate failed: change the seed"
 
     @classmethod
-    def get(cls, cfg_id, P, order, extra):
-        key = (cfg_id, P, order, tuple(sorted(extra.items())))
+    def get(cls, cfg_id, P, order, extra, query_mode=0):
+        key = (cfg_id, P, order, tuple(sorted(extra.items())), query_mode)
         if key not in cls._cache:
-            cls._cache[key] = Case(cfg_id, P, order, extra)
+            cls._cache[key] = Case(cfg_id, P, order, extra, query_mode)
         return cls._cache[key]
 
     def gpu_mask(self, B):
@@ -238,6 +238,64 @@ def test_tile_query_whole_sphere_and_empty():
     cfg0 = B.Config(order=6, n_gauss=0)
     r0 = R.Rasterizer(cfg0, depth_presort=False)
     assert r0.tile_query() == 0
+
+
+# ------------------------------------------------------------------------------------------- F2, RING mode (NEXT-1)
+@pytest.mark.parametrize("cfg_id,P,order,refine,big", [
+    (1, 1000, 6, 2, False), (2, 12000, 7, 2, False), (4, 3000, 7, 2, False), (3, 12000, 7, 2, False), (5, 8000, 8, 2, False),
+    (4, 800, 6, 0, False), (4, 800, 6, 1, False), (4, 800, 6, 4, False), (4, 300, 9, 2, True), (3, 300, 9, 2, True), (5, 300, 10, 2, True)])
+def test_tile_query_ring_mode_bit_exact(cfg_id, P, order, refine, big):
+    """query_mode = UTS_QUERY_RING: the CUDA path against the oracle's Alg.3 step by step.  Small discs,
+    masks, refinements x1..x16, and (big) discs of thousands of tiles incl. r_s = pi and discs over the poles."""
+    B, R = _gpu()
+    scene = small_scene(cfg_id, P, order, n_views=1)
+    if big:
+        scene["scales"][::2] *= 30.0
+        scene["scales"][7] = 80.0
+        scene["means"][9] = np.array([0.01, 3.0, 0.02]); scene["means"][11] = np.array([0.02, -2.0, 0.01])   # discs over the poles
+    oc = ocfg(scene, query_refine_log2=refine, query_mode=1)
+    bits, act, slot = oracle_mask(oc, scene)
+    pr = orc.preprocess(oc, scene["means"], scene["scales"], scene["quats"], scene["opac"], scene["sh"], scene["W"], scene["b"])
+    off, keys, vals, info = orc.tile_query(oc, pr, slot)
+    assert info["min_margin"] > 1e-12
+    cfg = _cfg(R, scene, query_refine_log2=refine, query_mode=1)
+    mask = B.Mask.full() if bits is None else B.Mask(dev(act.view(np.int32)), int(act.shape[0]), dev(slot), dev(bits.view(np.int32)))
+    r = R.Rasterizer(cfg, mask, depth_presort=False)
+    r.proj = B.Proj(dev(pr.dir), dev(pr.lonlat), dev(pr.rho), dev(pr.conic_opac), dev(pr.rs), dev(pr.rgb), dev(pr.flags))
+    n = r.tile_query()
+    assert n == keys.shape[0]
+    assert np.array_equal(u64(r.offsets), off)
+    assert np.array_equal(u64(r.keys)[:n], keys) and np.array_equal(u32(r.vals)[:n], vals)
+    # and it is not the NESTED set
+    ocn = ocfg(scene, query_refine_log2=refine)
+    assert orc.tile_query(ocn, pr, slot)[1].shape[0] > n
+
+
+@pytest.mark.parametrize("cfg_id,P,order,extra", [CASES[1], CASES[2]])
+def test_end_to_end_chain_ring_mode(cfg_id, P, order, extra):
+    """All-GPU chain in RING mode against the all-oracle chain in RING mode: lists bit-exact, image 1e-4, gradients 1e-3."""
+    B, R = _gpu()
+    c = Case.get(cfg_id, P, order, extra, query_mode=1)
+    cfg = _cfg(R, c.scene, query_mode=1)
+    mask = c.gpu_mask(B)
+    g, views = R.scene_to_device(c.scene)
+    r = R.Rasterizer(cfg, mask)
+    r.forward(g, views)
+    n = r.n_pairs
+    assert n == c.fw["skeys"].shape[0]
+    assert np.array_equal(u64(r.keys)[:n], c.fw["skeys"]) and np.array_equal(u32(r.vals)[:n], c.fw["svals"])
+    assert np.array_equal(u64(r.ranges), c.fw["ranges"])
+    _compare_image(c, r.color.cpu().numpy(), r.alpha.cpu().numpy(), u32(r.n_last))
+    from paper_2606_29794_b200 import scenes
+    V, npx = r.color.shape[0], r.color.shape[1]
+    gcol, _ = _zero_unsafe(c, scenes.upstream_grad(V, npx, seed=200 + cfg_id))
+    s = c.scene
+    w_rgb, w_conic, w_mu2, w_opac = orc.render_bwd(c.ocfg, c.fw["proj"], c.fw["ranges"], c.fw["svals"], c.fw["n_last"], gcol, None, c.act, c.bits)
+    w_means, w_scales, w_quats, w_sh = orc.preprocess_bwd(c.ocfg, s["means"], s["scales"], s["quats"], s["sh"], s["W"], s["b"], w_rgb, w_conic, w_mu2)
+    G = r.backward(g, views, dev(gcol))
+    for name, want in (("means", w_means), ("scales", w_scales), ("quats", w_quats), ("opac", w_opac), ("sh", w_sh)):
+        e = _rel_err(G[name].cpu().numpy(), want)
+        assert e <= 1e-3, (name, e)
 
 
 # ------------------------------------------------------------------------------------------- F3 / F4

@@ -188,6 +188,61 @@ def test_tile_query_respects_mask_and_views():
     assert np.all(tid[int(off[cfg.n_gauss]):] >= cfg.n_tiles) and np.all(tid[:int(off[cfg.n_gauss])] < cfg.n_tiles)
 
 
+# ------------------------------------------------------------------ O2', RING scan (Alg.3; NEXT-1)
+@pytest.mark.parametrize("cfg_id,P,order,refine", [(1, 1000, 6, 2), (2, 400, 8, 2), (4, 300, 7, 2), (4, 200, 6, 1), (1, 200, 5, 0), (4, 150, 6, 3)])
+def test_ring_scan_equals_bruteforce_centres_within_rs(cfg_id, P, order, refine):
+    """Alg.3 step by step == the plain definition it computes: tiles owning an order-k_q pixel whose CENTRE is within r_s
+    (no PixRad margin), by a literal loop over every Gaussian x every order-k_q pixel."""
+    sc = small_scene(cfg_id, P, order)
+    cfg = ocfg(sc, query_refine_log2=refine, query_mode=1)
+    pr = orc.preprocess(cfg, sc["means"], sc["scales"], sc["quats"], sc["opac"], sc["sh"], sc["W"], sc["b"])
+    o1, k1, v1, i1 = orc.tile_query(cfg, pr, brute=True)
+    o2, k2, v2, i2 = orc.tile_query(cfg, pr, brute=False)
+    assert i1["min_margin"] > 1e-12
+    assert np.array_equal(o1, o2) and np.array_equal(k1, k2) and np.array_equal(v1, v2)
+    # the brute-force set re-derived here in numpy from the oracle's pixel centres (independent of orc.tile_query)
+    _, _, vq = orc.centers(cfg.tile_order + refine, 2)
+    tiles = (k2 >> np.uint64(32)).astype(np.int64)
+    for i in range(0, cfg.n_gauss, 7):
+        u = pr.dir[0, i].astype(np.float64); u /= np.linalg.norm(u)
+        inside = np.flatnonzero(vq @ u >= math.cos(min(math.pi, float(pr.rs[0, i]))))
+        assert sorted(set((inside >> (2 * refine)).tolist())) == tiles[int(o2[i]):int(o2[i + 1])].tolist()
+    # non-conservative: a subset of the NESTED set (PAPER.md:108 "at the expense of quality"), strictly smaller on these scenes
+    cfgn = ocfg(sc, query_refine_log2=refine)
+    on, kn, vn, _ = orc.tile_query(cfgn, pr)
+    assert set(zip(k2.tolist(), v2.tolist())) <= set(zip(kn.tolist(), vn.tolist())) and k2.shape[0] < kn.shape[0]
+
+
+def test_ring_scan_poles_full_rings_and_whole_sphere():
+    """Branches of Alg.3: disc over a pole (l.2 clamp, l.16 full rings), centre exactly at a pole (l.9), r_s = pi."""
+    sc = small_scene(1, 6, 6)
+    cfg = ocfg(sc, query_mode=1)
+    pr = orc.preprocess(cfg, sc["means"], sc["scales"], sc["quats"], sc["opac"], sc["sh"], sc["W"], sc["b"])
+    d = np.array([[0.02, 1, 0.01], [0.0, 1.0, 0.0], [0.3, -1, 0.2], [0, -1, 0], [1, 0.05, 0], [0.1, 0.2, -1]], np.float64)
+    d /= np.linalg.norm(d, axis=1, keepdims=True)
+    pr.dir[0] = d.astype(np.float32)
+    pr.rs[0] = np.array([0.3, 0.21, 0.9, 0.08, math.pi, 2.5], np.float32)
+    o1, k1, v1, i1 = orc.tile_query(cfg, pr, brute=True)
+    o2, k2, v2, i2 = orc.tile_query(cfg, pr, brute=False)
+    assert i1["min_margin"] > 1e-12
+    assert np.array_equal(o1, o2) and np.array_equal(k1, k2) and np.array_equal(v1, v2)
+    assert int(o2[5] - o2[4]) == cfg.n_tiles                 # r_s = pi: every tile
+    assert int(o2[2] - o2[1]) > 0 and int(o2[4] - o2[3]) > 0  # discs centred exactly on the poles are found
+
+
+def test_ring_scan_respects_mask():
+    sc = small_scene(5, 300, 7, n_views=2)
+    cfg = ocfg(sc, query_mode=1)
+    bits = orc.mask_bits(cfg.order, sc["mask"]["kind"], sc["mask"]["params"])
+    act, slot = orc.mask_tiles(cfg, bits)
+    pr = orc.preprocess(cfg, sc["means"], sc["scales"], sc["quats"], sc["opac"], sc["sh"], sc["W"], sc["b"])
+    off, keys, vals, _ = orc.tile_query(cfg, pr, slot_of_tile=slot)
+    offf, keysf, valsf, _ = orc.tile_query(cfg, pr)
+    tf = (keysf >> np.uint64(32)).astype(np.int64)
+    keep = slot[tf % cfg.n_tiles] >= 0
+    assert np.array_equal(keysf[keep], keys) and np.array_equal(valsf[keep], vals)
+
+
 # ------------------------------------------------------------------ O3 / O4
 def test_sort_and_ranges_properties():
     sc = small_scene(2, 3000, 7)

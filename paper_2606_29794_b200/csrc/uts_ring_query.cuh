@@ -24,7 +24,10 @@ constexpr float kRingDelta = 4e-6f;       // fp32 chord margin, as in the descen
 constexpr int kRingFull = 1 << 28;        // |first|, |last| of a ring that lies entirely inside the disc
 
 struct RingDisc {
-  double u[3], cosR, lq;                  // unit direction; cos R; longitude in eighth-ring units: g_c = lq * n_r, lq in [0,8)
+  float dir[3];                           // the record's direction as stored (fp32); normalised in double where a decision needs it
+  double R;                               // min(pi, r_s + rho_q)
+  float lq;                               // longitude in eighth-ring units: g_c = lq * n_r, lq in [0,8)
+  float dq;                               // the disc's longitude half-extent in the same units (4 = everywhere)
   float zc, sc, T2, T2lo, T2hi;           // z and sin(colatitude) of u; chord thresholds T^2, (T -+ delta)^2, T = 2 sin(R/2)
   int i_lo, i_hi;                         // rings that can hold an in-disc centre (superset)
   bool all;                               // R >= pi: every tile (reading A24)
@@ -33,37 +36,59 @@ struct RingDisc {
 __host__ __device__ __forceinline__ int ring_n(int N, int i) { return min(i, min(N, 4 * N - i)); }
 __host__ __device__ __forceinline__ int ring_parity(int N, int i) { return (i < N || i > 3 * N) ? 1 : ((N + 1 + i) & 1); }
 
-// real-valued ring coordinate of colatitude theta (ring i sits at coordinate i)
-__host__ __device__ __forceinline__ double ring_coord(int N, double theta) {
-  const double z = cos(theta);
-  if (z >= 2.0 / 3.0) return (double)N * 2.449489742783178 * sin(0.5 * theta);
-  if (z <= -2.0 / 3.0) return 4.0 * N - (double)N * 2.449489742783178 * cos(0.5 * theta);
-  return (double)N * (2.0 - 1.5 * z);
+// sin(t) for |t| <= pi/2 + 0.05 with relative error 1e-7 (own fit of sin(t)/t in t^2); independent of --use_fast_math
+__host__ __device__ __forceinline__ float sin_poly(float t) {
+  const float x = t * t;
+  return t * (0.99999999416f + x * (-0.16666655522f + x * (0.00833299300f + x * (-0.000198048254f + x * 2.5956970e-06f))));
 }
 
-__host__ __device__ __forceinline__ void make_ring_disc(int kq, const double u[3], double R, RingDisc& D) {
+// real-valued ring coordinate of colatitude theta (ring i sits at coordinate i); fp32, good to a small fraction of a ring
+__host__ __device__ __forceinline__ float ring_coord(int N, float theta) {
+  const float z = cosf(theta);
+  if (z >= 0.6666667f) return (float)N * 2.4494897f * sinf(0.5f * theta);
+  if (z <= -0.6666667f) return 4.0f * (float)N - (float)N * 2.4494897f * cosf(0.5f * theta);
+  return (float)N * (2.0f - 1.5f * z);
+}
+
+// dir: the projected record's unit direction (fp32); lon, lat: its (omega, phi) of Eq.1 (fp32, from the same record).
+// The fp32 quantities only steer estimates and margin-guarded tests; the defining predicate uses dir and R in double.
+__host__ __device__ __forceinline__ void make_ring_disc(int kq, const float dir[3], float lon, float lat, double R, RingDisc& D) {
   const int N = 1 << kq;
-  D.u[0] = u[0]; D.u[1] = u[1]; D.u[2] = u[2];
+  D.dir[0] = dir[0]; D.dir[1] = dir[1]; D.dir[2] = dir[2];
+  D.R = R;
   D.all = R >= kPi;
-  D.cosR = cos(R);
-  const double T = 2.0 * sin(0.5 * R);
-  D.T2 = (float)(T * T);
-  D.T2lo = T > (double)kRingDelta ? (float)((T - kRingDelta) * (T - kRingDelta)) : -1.0f;
-  D.T2hi = (float)((T + kRingDelta) * (T + kRingDelta));
-  const double scd = sqrt(u[0] * u[0] + u[2] * u[2]);
-  D.zc = (float)u[1]; D.sc = (float)scd;
-  double lq = atan2(u[0], u[2]) * (4.0 / kPi);
-  if (lq < 0) lq += 8.0;
-  if (lq >= 8.0) lq = 0.0;
+  const float Rf = (float)R;
+  const float T = 2.0f * sin_poly(0.5f * Rf);
+  D.T2 = T * T;
+  D.T2lo = T > kRingDelta ? (T - kRingDelta) * (T - kRingDelta) : -1.0f;
+  D.T2hi = (T + kRingDelta) * (T + kRingDelta);
+  D.zc = dir[1]; D.sc = sqrtf(dir[0] * dir[0] + dir[2] * dir[2]);
+  float lq = lon * 1.2732395447351628f;
+  if (lq < 0.0f) lq += 8.0f;
+  if (!(lq < 8.0f)) lq = 0.0f;
   D.lq = lq;
-  const double th = atan2(scd, u[1]);
-  const double t0 = fmax(0.0, th - R - 1e-6), t1 = fmin(kPi, th + R + 1e-6);
-  D.i_lo = max(1, (int)ceil(ring_coord(N, t0)) - 1);
-  D.i_hi = min(4 * N - 1, (int)floor(ring_coord(N, t1)) + 1);
+  const float th = 1.5707963267948966f - lat;
+  const float t0 = th - Rf - 4e-6f, t1 = th + Rf + 4e-6f;
+  D.i_lo = max(1, (int)ceilf(ring_coord(N, fmaxf(0.0f, t0))) - 1);
+  D.i_hi = min(4 * N - 1, (int)floorf(ring_coord(N, fminf(3.14159265f, t1))) + 1);
+  // longitude extent: a disc that holds no pole stays within asin(sin R / sin theta_c) of its centre's meridian
+  if (t0 <= 1e-5f || t1 >= 3.14158f || !(D.sc > 0.0f)) D.dq = 4.0f;
+  else D.dq = asinf(fminf(1.0f, sinf(Rf) / D.sc)) * 1.2732395447351628f + 1e-3f;
+}
+
+// can face f hold a tile of the disc?  (its pixels lie within one eighth-ring unit of F2 on every ring)
+__host__ __device__ __forceinline__ bool face_in_extent(const RingDisc& D, int f) {
+  const int F2 = 2 * (f & 3) + 1 - ((f >> 2) & 1);
+  float d = fabsf(D.lq - (float)F2);
+  if (d > 4.0f) d = 8.0f - d;
+  return d <= 1.0f + D.dq;
 }
 
 // the defining predicate for the pixel at position g of ring i, in double
 __host__ __device__ __forceinline__ bool ring_pixel_inside_exact(const RingDisc& D, int N, int i, int g) {
+  double u[3] = {(double)D.dir[0], (double)D.dir[1], (double)D.dir[2]};
+  const double nrm = sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
+  u[0] /= nrm; u[1] /= nrm; u[2] /= nrm;
   double z, sth;
   int n;
   const double inv3N2 = 1.0 / (3.0 * (double)N * (double)N);
@@ -73,7 +98,7 @@ __host__ __device__ __forceinline__ bool ring_pixel_inside_exact(const RingDisc&
   const double lam = (kPi / 4) * ((double)g / (double)n);
   double sn, cs;
   sincos(lam, &sn, &cs);
-  return D.u[0] * (sth * sn) + D.u[1] * z + D.u[2] * (sth * cs) >= D.cosR;
+  return u[0] * (sth * sn) + u[1] * z + u[2] * (sth * cs) >= cos(D.R);
 }
 
 // Phase 1.  In-disc pixel positions of ring i: the integers g = first, first+2, ..., last (not reduced mod 8 n_r;
@@ -91,15 +116,14 @@ __host__ __device__ __forceinline__ void ring_interval(const RingDisc& D, int N,
   const float A = dz * dz + ds * ds, B = 4.0f * s * D.sc;      // chord^2(g) = A + B sin^2((lam_g - lam_c)/2) >= A
   if (A > D.T2hi) return;
   const int par = ring_parity(N, i);
-  const double gc = D.lq * (double)n;
+  const double gc = (double)D.lq * (double)n;                              // exact product: g_c reaches 8 * 8192
   const int g0 = 2 * (int)floor(0.5 * (gc - (double)par) + 0.5) + par;     // pixel position nearest to g_c
   const float frac = (float)(gc - (double)g0);                             // in [-1, 1]
   const float k = 0.39269908169872414f / (float)n;                         // (pi/8) / n_r: half the longitude step per unit g
   auto inside = [&](int g) -> bool {
     float t = fabsf((float)(g - g0) - frac) * k;
     if (t > 1.5707963267948966f) t = 3.14159265358979f - t;
-    const float x = t * t;
-    const float sn = t * (0.99999999f + x * (-0.16666655f + x * (0.0083329930f + x * (-0.00019804825f + x * 2.5956970e-06f))));
+    const float sn = sin_poly(t);
     const float c2 = A + B * sn * sn;
     if (c2 < D.T2lo) return true;
     if (c2 > D.T2hi) return false;
@@ -151,8 +175,16 @@ __host__ __device__ __forceinline__ unsigned long long tile_row_mask(const RingD
     tab(i, first, last);
     if (last < first) continue;
     const int n = ring_n(N, i), a = F2 * n, w = min(d, 2 * m - 2 - d);
-    // the run of this tile on ring i is [a + mH - w, a + mH + w]; it must meet [first, last] + 8 n k for some k
-    for (int k = -1; k <= 1; ++k) {
+    // the run of this tile on ring i is [a + mH - w, a + mH + w]; it must meet [first, last] + 8 n k for some k.  The copy
+    // whose middle is nearest to the face (|mid + 8 n k - a| <= 4 n) is the only one that can reach the face's pixels
+    // (|g - a| < n) unless the interval is wider than 6 n; then its two neighbours are tried as well.
+    int k0 = 0, kw = 0;
+    if (first != -kRingFull) {
+      const int mid = (first + last) >> 1;
+      k0 = a - mid > 4 * n ? 1 : (mid - a > 4 * n ? -1 : 0);
+      kw = last - first >= 6 * n ? 1 : 0;
+    }
+    for (int k = k0 - kw; k <= k0 + kw; ++k) {
       const int P = first + 8 * n * k - a - w, Q = last + 8 * n * k - a + w;     // P <= m H <= Q
       const int Hlo = (P + m - 1) >> ref, Hhi = Q >> ref;
       const int jlo = max(jbase, (Hlo + Hm + 1) >> 1), jhi = min(jtop, (Hhi + Hm) >> 1);
@@ -160,7 +192,6 @@ __host__ __device__ __forceinline__ unsigned long long tile_row_mask(const RingD
         const int cnt = jhi - jlo + 1;
         mask |= (cnt >= 64 ? ~0ull : ((1ull << cnt) - 1ull)) << (jlo - jbase);
       }
-      if (first == -kRingFull) break;
     }
   }
   return mask;

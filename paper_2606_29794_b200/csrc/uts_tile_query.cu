@@ -20,7 +20,9 @@
 //   * count -> exclusive scan -> emit: the pair arrays are written once, densely, in (view, Gaussian, tile) order.
 #include "uts_internal.cuh"
 #include "uts_scan.cuh"
+#include "uts_ring_query.cuh"
 #include <cstdlib>
+#include <cstring>
 
 namespace uts {
 
@@ -41,6 +43,10 @@ struct QueryParams {
   uint32_t* bitmap_cache;               // [bitmap_cache_cap][n_words] bitmaps of the count pass (block path)
   uint32_t bitmap_cache_cap;
   float rho[kMaxOrder + 1], sin_hrho[kMaxOrder + 1], cos_hrho[kMaxOrder + 1];   // rho_max(o), sin/cos(rho_max(o)/2)
+  // ring-interval path (uts_ring_query.cuh): discs are split by radius bucket into block / warp / thread work
+  int b_block, b_warp;                  // buckets <= b_block: one block per disc; <= b_warp: one warp; others: one thread
+  int rc_thread, rc_warp, rc_block;     // ring-table capacities of the three shapes
+  const uint32_t* active_tiles; int n_active;   // mask's ascending active-tile list (whole-sphere discs), or null
 };
 
 // Per-Gaussian query state.
@@ -253,11 +259,16 @@ classify_kernel(QueryParams qp, const float* __restrict__ rs, const uint8_t* __r
 }
 
 // hist[64] counts -> exclusive start offsets (in place); n_small = total
-__global__ void bucket_scan_kernel(uint32_t* __restrict__ hist, uint32_t* __restrict__ n_small) {
+// n_small[1], n_small[2]: ends of the block-per-disc and warp-per-disc parts of perm (ring-interval path)
+__global__ void bucket_scan_kernel(uint32_t* __restrict__ hist, uint32_t* __restrict__ n_small, int b_block, int b_warp) {
   if (threadIdx.x == 0) {
-    uint32_t run = 0;
-    for (int b = 0; b < kBuckets; ++b) { const uint32_t c = hist[b]; hist[b] = run; run += c; }
-    *n_small = run;
+    uint32_t run = 0, e_block = 0, e_warp = 0;
+    for (int b = 0; b < kBuckets; ++b) {
+      const uint32_t c = hist[b]; hist[b] = run; run += c;
+      if (b <= b_block) e_block = run;
+      if (b <= b_warp) e_warp = run;
+    }
+    n_small[0] = run; n_small[1] = e_block; n_small[2] = e_warp;
   }
 }
 
@@ -456,12 +467,270 @@ tile_query_kernel(QueryParams qp, int n_large_blocks, const float* __restrict__ 
     small_body<EMIT>((int64_t)blockIdx.x - n_large_blocks, qp, dir, rho, rs, slot_of_tile, perm, n_small, emit_rank, counts, offsets, keys, vals);
 }
 
+// ================================================================================== ring-interval path
+// (uts_ring_query.cuh)  Two work shapes over the radius-bucketed permutation `perm` (largest discs first):
+//   perm[0, e_block)         one thread block per disc (ring table: every ring of the order);
+//   perm[e_block, e_warp)    batches of kBatchB discs of up to rc_warp rings   } one block per batch; the rings of all discs of the
+//   perm[e_warp, n_small)    batches of kBatchA discs of up to rc_thread rings } batch, then their tile rows, are FLATTENED over the
+//                                                                                block's lanes, so that no lane waits for a longer disc.
+// Phase 1 fills the ring tables in shared memory, phase 2 walks the (face, tile diagonal) rows, a lane per row.  A row's tiles
+// are placed with a shared-memory cursor per disc, so the pairs of one Gaussian are contiguous but their order inside the
+// segment is not fixed; the sort's result does not depend on it (a Gaussian's tiles are distinct: no two of its keys tie).
+
+struct GroupTab {
+  const int2* base; int i_lo;
+  __device__ __forceinline__ void operator()(int i, int& f, int& l) const { const int2 v = base[i - i_lo]; f = v.x; l = v.y; }
+};
+
+__device__ __forceinline__ void load_ring_disc(const QueryParams& qp, const float* __restrict__ dir, const float* __restrict__ lonlat,
+                                               const float* __restrict__ rs, int64_t k, RingDisc& D) {
+  const float d[3] = {__ldg(dir + 3 * k), __ldg(dir + 3 * k + 1), __ldg(dir + 3 * k + 2)};
+  make_ring_disc(qp.kq, d, __ldg(lonlat + 2 * k), __ldg(lonlat + 2 * k + 1), fmin(kPi, (double)__ldg(rs + k) + qp.rho_q), D);
+}
+
+// Tiles of one 64-candidate chunk of a row.  Returns how many are active; with VISIT, fn(tile) is called for each.
+// X = (S - Hm)/2 + j, Y = (S + Hm)/2 - j: the interleaved bits are stepped along the row, not recomputed.
+template <bool VISIT, class Fn>
+__device__ __forceinline__ uint32_t visit_row_chunk(int kt, int f, int S, int jbase, unsigned long long mask, const int32_t* __restrict__ slot_of_tile, Fn&& fn) {
+  if (!VISIT && !slot_of_tile) return (uint32_t)__popcll(mask);
+  const int Nt = 1 << kt, Hm = min(S, 2 * Nt - 2 - S);
+  const uint32_t fbase = (uint32_t)f << (2 * kt);
+  const int j0 = __ffsll((long long)mask) - 1, j1 = 63 - __clzll((long long)mask);
+  uint32_t sX = spread_bits16_hd((uint32_t)(((S - Hm) >> 1) + jbase + j0));
+  uint32_t sY = spread_bits16_hd((uint32_t)(((S + Hm) >> 1) - jbase - j0)) << 1;
+  uint32_t cnt = 0;
+  for (int j = j0; j <= j1; ++j) {
+    if ((mask >> j) & 1ull) {
+      const uint32_t tile = fbase | sX | sY;
+      if (!slot_of_tile || __ldg(slot_of_tile + tile) >= 0) { if (VISIT) fn(tile); ++cnt; }
+    }
+    sX = ((sX | 0xAAAAAAAAu) + 1u) & 0x55555555u;
+    sY = (sY - 2u) & 0xAAAAAAAAu;
+  }
+  return cnt;
+}
+
+// rows of a disc: face f owns rows [pre[f], pre[f+1]) of the flat enumeration, S = S_lo(f) + (row - pre[f])
+__device__ __forceinline__ int disc_face_rows(const QueryParams& qp, const RingDisc& D, uint16_t* pre /*[13]*/) {
+  int run = 0;
+  for (int f = 0; f < 12; ++f) {
+    pre[f] = (uint16_t)run;
+    if (!face_in_extent(D, f)) continue;
+    int S_lo, S_hi;
+    face_row_range(D, qp.kq, qp.kt, f, S_lo, S_hi);
+    if (S_hi >= S_lo) run += S_hi - S_lo + 1;
+  }
+  pre[12] = (uint16_t)run;
+  return run;
+}
+
+// ---------------------------------------------------------------------------------------------- batch of small discs
+struct BatchRec {
+  RingDisc D;
+  uint64_t hi, base;          // key high part of the view; first pair of the Gaussian (emit)
+  uint32_t depth, gid, slot, k;
+  uint32_t cached;            // emit: the count pass left the tiles in tile_cache
+};
+
+template <int G, bool EMIT>
+__global__ void __launch_bounds__(kLargeThreads)
+ring_query_batch_kernel(QueryParams qp, int which /*0: rc_warp class, 1: rc_thread class*/, const float* __restrict__ dir, const float* __restrict__ lonlat,
+                        const float* __restrict__ rho, const float* __restrict__ rs, const int32_t* __restrict__ slot_of_tile,
+                        const uint32_t* __restrict__ perm, const uint32_t* __restrict__ n_small, const uint32_t* __restrict__ emit_rank,
+                        uint32_t* __restrict__ counts, const uint64_t* __restrict__ offsets, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ uint32_t s_w[kLargeThreads / 32];
+  __shared__ int ring_off[G + 1], row_off[G + 1];
+  __shared__ uint32_t cursor[G];
+  __shared__ uint16_t rowpre[G][13];
+  BatchRec* rec = reinterpret_cast<BatchRec*>(smem_raw);
+  int2* tab = reinterpret_cast<int2*>(smem_raw + sizeof(BatchRec) * G);
+  const int rc = which == 0 ? qp.rc_warp : qp.rc_thread;
+  const uint32_t begin = which == 0 ? n_small[1] : n_small[2], end = which == 0 ? n_small[2] : n_small[0];
+  const int N = 1 << qp.kq, tid = threadIdx.x;
+  for (uint32_t b0 = begin + blockIdx.x * G; b0 < end; b0 += gridDim.x * G) {
+    const int ng = min((uint32_t)G, end - b0);
+    __syncthreads();                                   // the previous batch is done with shared memory
+    // ---- records
+    uint32_t my_rings = 0;
+    if (tid < ng) {
+      BatchRec& r = rec[tid];
+      const int64_t k = (int64_t)perm[b0 + tid];
+      const int64_t slot = emit_rank ? (int64_t)emit_rank[k] : k;
+      const int v = (int)(k / qp.P);
+      r.k = (uint32_t)k; r.slot = (uint32_t)slot;
+      r.hi = (uint64_t)v * (uint64_t)qp.n_tile;
+      r.depth = __float_as_uint(__ldg(rho + k)); r.gid = (uint32_t)(k - (int64_t)v * qp.P);           // reading A10
+      r.cached = 0; r.base = 0;
+      cursor[tid] = 0;
+      bool skip = false;
+      if (EMIT) {
+        r.base = offsets[slot];
+        const uint64_t cnt = offsets[slot + 1] - r.base;
+        if (cnt == 0) skip = true;
+        else if (cnt <= (uint64_t)kTileCacheK) { r.cached = (uint32_t)cnt; skip = true; }
+      }
+      load_ring_disc(qp, dir, lonlat, rs, k, r.D);
+      if (r.D.all) skip = true;                        // handled after the row loop
+      r.D.i_hi = min(r.D.i_hi, r.D.i_lo + rc - 1);
+      if (skip) r.D.i_hi = r.D.i_lo - 1;
+      my_rings = (uint32_t)(r.D.i_hi - r.D.i_lo + 1);
+    }
+    uint32_t before;
+    const uint32_t n_rings = block_sum_u32(my_rings, s_w, before);
+    if (tid < ng) ring_off[tid] = (int)before;
+    if (tid == 0) ring_off[ng] = (int)n_rings;
+    __syncthreads();
+    // ---- phase 1, flattened over (disc, ring)
+    for (uint32_t it = tid; it < n_rings; it += kLargeThreads) {
+      int lo = 0, hi = ng;                             // largest g with ring_off[g] <= it
+      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if ((uint32_t)ring_off[mid] <= it) lo = mid; else hi = mid; }
+      const RingDisc& D = rec[lo].D;
+      int2 fl;
+      ring_interval(D, N, D.i_lo + (int)(it - (uint32_t)ring_off[lo]), fl.x, fl.y);
+      tab[it] = fl;
+    }
+    // ---- rows of every disc
+    uint32_t my_rows = 0;
+    if (tid < ng && rec[tid].D.i_hi >= rec[tid].D.i_lo) my_rows = (uint32_t)disc_face_rows(qp, rec[tid].D, rowpre[tid]);
+    const uint32_t n_rows = block_sum_u32(my_rows, s_w, before);
+    if (tid < ng) row_off[tid] = (int)before;
+    if (tid == 0) row_off[ng] = (int)n_rows;
+    __syncthreads();
+    // ---- phase 2, flattened over (disc, row)
+    for (uint32_t it = tid; it < n_rows; it += kLargeThreads) {
+      int lo = 0, hi = ng;
+      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if ((uint32_t)row_off[mid] <= it) lo = mid; else hi = mid; }
+      const BatchRec& r = rec[lo];
+      const int row = (int)(it - (uint32_t)row_off[lo]);
+      int f = 0;
+      while (f < 11 && (int)rowpre[lo][f + 1] <= row) ++f;
+      int S_lo, S_hi;
+      face_row_range(r.D, qp.kq, qp.kt, f, S_lo, S_hi);
+      const int S = S_lo + row - (int)rowpre[lo][f], Hm = min(S, (2 << qp.kt) - 2 - S);
+      const GroupTab T{tab + ring_off[lo], r.D.i_lo};
+      for (int jbase = 0; jbase <= Hm; jbase += 64) {
+        const unsigned long long mask = tile_row_mask(r.D, qp.kq, qp.kt, f, S, jbase, T);
+        if (!mask) continue;
+        if (EMIT) {
+          const uint32_t c = visit_row_chunk<false>(qp.kt, f, S, jbase, mask, slot_of_tile, [](uint32_t) {});
+          uint64_t pos = r.base + atomicAdd(&cursor[lo], c);
+          visit_row_chunk<true>(qp.kt, f, S, jbase, mask, slot_of_tile, [&](uint32_t tile) {
+            keys[pos] = ((r.hi + tile) << 32) | r.depth; vals[pos] = r.gid; ++pos;            // Alg.1 l.12: ((t, rho), i)
+          });
+        } else {
+          const uint32_t c = visit_row_chunk<false>(qp.kt, f, S, jbase, mask, slot_of_tile, [](uint32_t) {});
+          uint32_t pos = atomicAdd(&cursor[lo], c);
+          if (pos < (uint32_t)kTileCacheK) {           // remember the first tiles: the emit pass replays discs of <= kTileCacheK tiles
+            uint32_t* cache = qp.tile_cache + (size_t)r.k * kTileCacheK;
+            visit_row_chunk<true>(qp.kt, f, S, jbase, mask, slot_of_tile, [&](uint32_t tile) { if (pos < (uint32_t)kTileCacheK) cache[pos] = tile; ++pos; });
+          }
+        }
+      }
+    }
+    __syncthreads();
+    // ---- results, cached discs, whole-sphere discs
+    if (tid < ng) {
+      const BatchRec& r = rec[tid];
+      if (r.D.all) {
+        const uint32_t total = qp.active_tiles ? (uint32_t)qp.n_active : (uint32_t)qp.n_tile;
+        if (!EMIT) counts[r.slot] = total;
+        else if (!r.cached && offsets[r.slot + 1] != r.base)
+          for (uint32_t j = 0; j < total; ++j) { const uint32_t tile = qp.active_tiles ? __ldg(qp.active_tiles + j) : j; keys[r.base + j] = ((r.hi + tile) << 32) | r.depth; vals[r.base + j] = r.gid; }
+        if (!EMIT && total <= (uint32_t)kTileCacheK) {
+          uint32_t* cache = qp.tile_cache + (size_t)r.k * kTileCacheK;
+          for (uint32_t j = 0; j < total; ++j) cache[j] = qp.active_tiles ? __ldg(qp.active_tiles + j) : j;
+        }
+      } else if (!EMIT) counts[r.slot] = cursor[tid];
+      if (EMIT && r.cached) {
+        const uint32_t* cache = qp.tile_cache + (size_t)r.k * kTileCacheK;
+        for (uint32_t j = 0; j < r.cached; ++j) { keys[r.base + j] = ((r.hi + cache[j]) << 32) | r.depth; vals[r.base + j] = r.gid; }
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------- one block per large disc
+template <bool EMIT>
+__global__ void __launch_bounds__(kLargeThreads)
+ring_query_block_kernel(QueryParams qp, const float* __restrict__ dir, const float* __restrict__ lonlat, const float* __restrict__ rho,
+                        const float* __restrict__ rs, const int32_t* __restrict__ slot_of_tile, const uint32_t* __restrict__ perm,
+                        const uint32_t* __restrict__ n_small, const uint32_t* __restrict__ emit_rank, uint32_t* __restrict__ counts,
+                        const uint64_t* __restrict__ offsets, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+  extern __shared__ int2 ring_tab[];                 // [rc_block]
+  __shared__ RingDisc s_disc;
+  __shared__ uint16_t s_pre[13];
+  __shared__ int s_Slo[12];
+  __shared__ uint32_t s_cursor;
+  const uint32_t end = n_small[1];
+  const int N = 1 << qp.kq, tid = threadIdx.x;
+  for (uint32_t idx = blockIdx.x; idx < end; idx += gridDim.x) {
+    const int64_t k = (int64_t)perm[idx];
+    const int64_t slot = emit_rank ? (int64_t)emit_rank[k] : k;
+    uint64_t b0 = 0;
+    if (EMIT) { b0 = offsets[slot]; if (offsets[slot + 1] == b0) continue; }
+    const int v = (int)(k / qp.P);
+    const uint64_t hi = (uint64_t)v * (uint64_t)qp.n_tile;
+    const uint32_t depth = __float_as_uint(__ldg(rho + k)), gid = (uint32_t)(k - (int64_t)v * qp.P);
+    __syncthreads();                                   // the previous disc is done with shared memory
+    if (tid == 0) {
+      load_ring_disc(qp, dir, lonlat, rs, k, s_disc);
+      s_disc.i_hi = min(s_disc.i_hi, s_disc.i_lo + qp.rc_block - 1);
+      disc_face_rows(qp, s_disc, s_pre);
+      for (int f = 0; f < 12; ++f) { int S_lo, S_hi; face_row_range(s_disc, qp.kq, qp.kt, f, S_lo, S_hi); s_Slo[f] = S_lo; }
+      s_cursor = 0;
+    }
+    __syncthreads();
+    const RingDisc& D = s_disc;
+    if (D.all) {                                       // reading A24: every active tile
+      const uint32_t total = qp.active_tiles ? (uint32_t)qp.n_active : (uint32_t)qp.n_tile;
+      if (!EMIT) { if (tid == 0) counts[slot] = total; }
+      else for (uint32_t j = tid; j < total; j += kLargeThreads) {
+        const uint32_t tile = qp.active_tiles ? __ldg(qp.active_tiles + j) : j;
+        keys[b0 + j] = ((hi + tile) << 32) | depth; vals[b0 + j] = gid;
+      }
+      continue;
+    }
+    for (int e = tid; e <= D.i_hi - D.i_lo; e += kLargeThreads) { int2 fl; ring_interval(D, N, D.i_lo + e, fl.x, fl.y); ring_tab[e] = fl; }
+    __syncthreads();
+    const GroupTab T{ring_tab, D.i_lo};
+    const int n_rows = (int)s_pre[12];
+    for (int row = tid; row < n_rows; row += kLargeThreads) {
+      int f = 0;
+      while (f < 11 && (int)s_pre[f + 1] <= row) ++f;
+      const int S = s_Slo[f] + row - (int)s_pre[f], Hm = min(S, (2 << qp.kt) - 2 - S);
+      for (int jbase = 0; jbase <= Hm; jbase += 64) {
+        const unsigned long long mask = tile_row_mask(D, qp.kq, qp.kt, f, S, jbase, T);
+        if (!mask) continue;
+        const uint32_t c = visit_row_chunk<false>(qp.kt, f, S, jbase, mask, slot_of_tile, [](uint32_t) {});
+        const uint32_t at = atomicAdd(&s_cursor, c);
+        if (EMIT) {
+          uint64_t pos = b0 + at;
+          visit_row_chunk<true>(qp.kt, f, S, jbase, mask, slot_of_tile, [&](uint32_t tile) {
+            keys[pos] = ((hi + tile) << 32) | depth; vals[pos] = gid; ++pos;                  // Alg.1 l.12: ((t, rho), i)
+          });
+        }
+      }
+    }
+    __syncthreads();
+    if (!EMIT && tid == 0) counts[slot] = s_cursor;
+  }
+}
+
 }  // namespace uts
 
 using namespace uts;
 
 namespace {
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+int radius_bucket_host(float R32) {                    // host replica of radius_bucket()
+  uint32_t u, t; const float four = 4.0f;
+  memcpy(&u, &R32, 4); memcpy(&t, &four, 4);
+  const int b = (int)(t >> 21) - (int)(u >> 21);
+  return b < 0 ? 0 : (b > kBuckets - 1 ? kBuckets - 1 : b);
+}
+constexpr int kRingThreadRings = 24, kRingWarpRings = 128, kRingBlockRingsMax = 24575;   // ring-table capacities (8 B per ring)
 
 struct QueryLayout { size_t counts, list, perm, nlarge, active, scan, tcache, bcache, total; uint32_t bcache_cap; };
 QueryLayout query_layout(const uts_config* cfg) {
@@ -510,7 +779,7 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
     *h_n_pairs = 0;
     return UTS_OK;
   }
-  if (!in.dir || !in.rho || !in.rs || !in.flags || !scratch) return UTS_ERR_INVALID_ARG;
+  if (!in.dir || !in.lonlat || !in.rho || !in.rs || !in.flags || !scratch) return UTS_ERR_INVALID_ARG;
   if (keys && !vals) return UTS_ERR_INVALID_ARG;
   if (scratch_bytes < uts_tile_query_scratch_bytes(cfg) || ((uintptr_t)scratch & 255)) return UTS_ERR_INVALID_ARG;
 
@@ -519,11 +788,22 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   const double* rm = rho_max_table_host();
   qp.rho_q = cfg->query_mode == UTS_QUERY_RING ? 0.0 : rm[d.kq];      // Alg.3's set has no PixRad margin
   for (int o = 0; o <= kMaxOrder; ++o) { qp.rho[o] = (float)rm[o]; qp.sin_hrho[o] = (float)sin(0.5 * rm[o]); qp.cos_hrho[o] = (float)cos(0.5 * rm[o]); }
+  // Implementation choice: the ring-interval path (uts_ring_query.cuh) whenever a block's ring table fits shared memory
+  // (k_q <= 12); the quadtree descent below otherwise, or when UTS_QUERY_IMPL=tree asks for it (A/B measurements).
+  const char* impl_env = getenv("UTS_QUERY_IMPL");
+  const int Nq = 1 << d.kq;
+  const bool ring_impl = 4 * Nq - 1 <= kRingBlockRingsMax && !(impl_env && strcmp(impl_env, "tree") == 0);
+  qp.rc_thread = kRingThreadRings; qp.rc_warp = 4 * Nq - 1 < kRingWarpRings ? 4 * Nq - 1 : kRingWarpRings; qp.rc_block = 4 * Nq - 1;
+  // a disc of radius R reaches at most 3 R N + 4 rings (ring spacing >= 2/(3N) in colatitude, +-1 ring of padding at each end)
+  qp.b_warp = radius_bucket_host((float)((qp.rc_thread - 6) / (3.0 * Nq)));
+  qp.b_block = radius_bucket_host((float)((qp.rc_warp - 6) / (3.0 * Nq)));
+  if (qp.b_block > qp.b_warp) qp.b_block = qp.b_warp;
+  qp.active_tiles = mask.active_tiles; qp.n_active = mask.active_tiles ? mask.n_active : -1;
   qp.os = d.kt < 4 ? d.kt : 4;
   const size_t n_split = (size_t)12 << (2 * qp.os);
   qp.wl_cap = (int)(n_split > 4096 ? n_split : 4096);
   const size_t large_smem = (2 * (size_t)(d.n_tile / 32) + 2 * (size_t)qp.wl_cap) * 4;
-  const bool use_large = d.kt >= 2 && large_smem <= kMaxLargeSmem;
+  const bool use_large = !ring_impl && d.kt >= 2 && large_smem <= kMaxLargeSmem;
   qp.n_words = use_large ? (int)(d.n_tile / 32) : 0;
   const char* e1__ = getenv("UTS_RLARGE"); const char* e2__ = getenv("UTS_LGRID");
   qp.r_large = (float)((e1__ ? atof(e1__) : 36.0) / sqrt((double)d.n_tile));      // ~320 tiles (pi R^2 / (4 pi / n_tile)); measured crossover on config 4
@@ -562,19 +842,57 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   const unsigned cgrid = (unsigned)((n + 255) / 256);
   classify_kernel<0><<<cgrid, 256, 0, s>>>(qp, in.rs, in.flags, counts, list, n_large, hist, perm, emit_rank);
   UTS_LAUNCH_CHECK();
-  bucket_scan_kernel<<<1, 32, 0, s>>>(hist, n_small);
+  bucket_scan_kernel<<<1, 32, 0, s>>>(hist, n_small, qp.b_block, qp.b_warp);
   UTS_LAUNCH_CHECK();
   classify_kernel<1><<<cgrid, 256, 0, s>>>(qp, in.rs, in.flags, counts, list, n_large, hist, perm, emit_rank);
   UTS_LAUNCH_CHECK();
-  tile_query_kernel<false><<<qgrid + lgrid, kLargeThreads, dyn_smem, s>>>(qp, lgrid, in.dir, in.rho, in.rs, mask.slot_of_tile, active_arg, perm,
-                                                                         n_small, list, n_large, emit_rank, counts, nullptr, nullptr, nullptr);
-  UTS_LAUNCH_CHECK();
+  constexpr int kBatchA = 128, kBatchB = 32;          // discs per batch: rc_thread class, rc_warp class
+  const size_t smem_a = sizeof(BatchRec) * kBatchA + (size_t)kBatchA * qp.rc_thread * sizeof(int2),
+               smem_b = sizeof(BatchRec) * kBatchB + (size_t)kBatchB * qp.rc_warp * sizeof(int2), smem_block = (size_t)qp.rc_block * sizeof(int2);
+  const unsigned agrid = (unsigned)sm_count() * 8u, wgrid = (unsigned)sm_count() * 8u, bgrid = (unsigned)sm_count() * 4u;
+  if (ring_impl) {
+    static bool ring_attr_set = false;
+    if (!ring_attr_set) {
+      UTS_CUDA(cudaFuncSetAttribute(ring_query_block_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kRingBlockRingsMax * 8 + 8));
+      UTS_CUDA(cudaFuncSetAttribute(ring_query_block_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kRingBlockRingsMax * 8 + 8));
+      UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchA, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+      UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchA, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+      UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+      UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+      ring_attr_set = true;
+    }
+    ring_query_block_kernel<false><<<bgrid, kLargeThreads, smem_block, s>>>(qp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small, emit_rank,
+                                                                          counts, nullptr, nullptr, nullptr);
+    UTS_LAUNCH_CHECK();
+    ring_query_batch_kernel<kBatchB, false><<<wgrid, kLargeThreads, smem_b, s>>>(qp, 0, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
+                                                                               emit_rank, counts, nullptr, nullptr, nullptr);
+    UTS_LAUNCH_CHECK();
+    ring_query_batch_kernel<kBatchA, false><<<agrid, kLargeThreads, smem_a, s>>>(qp, 1, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
+                                                                               emit_rank, counts, nullptr, nullptr, nullptr);
+    UTS_LAUNCH_CHECK();
+  } else {
+    tile_query_kernel<false><<<qgrid + lgrid, kLargeThreads, dyn_smem, s>>>(qp, lgrid, in.dir, in.rho, in.rs, mask.slot_of_tile, active_arg, perm,
+                                                                           n_small, list, n_large, emit_rank, counts, nullptr, nullptr, nullptr);
+    UTS_LAUNCH_CHECK();
+  }
   if ((st = exclusive_scan_u32(counts, n, offsets, block_sums, s))) return st;
   UTS_CUDA(cudaMemcpyAsync(h_n_pairs, offsets + n, sizeof(uint64_t), cudaMemcpyDeviceToHost, s));
   UTS_CUDA(cudaStreamSynchronize(s));
   if (!keys) return UTS_OK;
   if (*h_n_pairs > capacity) return UTS_ERR_CAPACITY;
   if (*h_n_pairs == 0) return UTS_OK;
+  if (ring_impl) {
+    ring_query_block_kernel<true><<<bgrid, kLargeThreads, smem_block, s>>>(qp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small, emit_rank,
+                                                                         nullptr, offsets, keys, vals);
+    UTS_LAUNCH_CHECK();
+    ring_query_batch_kernel<kBatchB, true><<<wgrid, kLargeThreads, smem_b, s>>>(qp, 0, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
+                                                                              emit_rank, nullptr, offsets, keys, vals);
+    UTS_LAUNCH_CHECK();
+    ring_query_batch_kernel<kBatchA, true><<<agrid, kLargeThreads, smem_a, s>>>(qp, 1, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
+                                                                              emit_rank, nullptr, offsets, keys, vals);
+    UTS_LAUNCH_CHECK();
+    return UTS_OK;
+  }
   tile_query_kernel<true><<<qgrid + lgrid, kLargeThreads, dyn_smem, s>>>(qp, lgrid, in.dir, in.rho, in.rs, mask.slot_of_tile, active_arg, perm,
                                                                         n_small, list, n_large, emit_rank, nullptr, offsets, keys, vals);
   UTS_LAUNCH_CHECK();

@@ -19,6 +19,17 @@ def oracle_mask(cfg, scene):
     return bits, act, slot
 
 
+def canon_pairs(offsets, keys, vals):
+    """Pairs before the sort: the pairs of one (view, Gaussian) are contiguous (offsets[i]..offsets[i+1]) and its tiles are
+    distinct, but their order inside the segment is the library's choice (include/uts.h, uts_tile_query).  Returns (keys, vals)
+    with every segment sorted by key, the form in which two implementations are compared bit for bit."""
+    off = np.asarray(offsets).astype(np.int64)
+    n = int(off[-1])
+    seg = np.repeat(np.arange(off.shape[0] - 1), np.diff(off))
+    order = np.lexsort((np.asarray(keys)[:n], seg))
+    return np.asarray(keys)[:n][order], np.asarray(vals)[:n][order]
+
+
 def small_scene(cfg_id, n_gauss, order, seed=0, **kw):
     return scenes.make_scene(cfg_id, seed=seed, n_gauss=n_gauss, order=order, **kw)
 

@@ -7,9 +7,9 @@
 
 using namespace uts;
 
-extern "C" int ring_query_host(int kt, int kq, const double* u, double R, uint32_t* out, int cap, int* n_rings) {
+extern "C" int ring_query_host(int kt, int kq, const float* dir, float lon, float lat, double R, uint32_t* out, int cap, int* n_rings) {
   RingDisc D;
-  make_ring_disc(kq, u, R, D);
+  make_ring_disc(kq, dir, lon, lat, R, D);
   const int N = 1 << kq, Nt = 1 << kt;
   std::vector<uint32_t> tiles;
   if (D.all) {
@@ -23,6 +23,7 @@ extern "C" int ring_query_host(int kt, int kq, const double* u, double R, uint32
       __host__ __device__ void operator()(int i, int& f, int& l) const { f = first[i - i_lo]; l = last[i - i_lo]; }
     } tab{first.data(), last.data(), D.i_lo};
     for (int f = 0; f < 12; ++f) {
+      if (!face_in_extent(D, f)) continue;
       int S_lo, S_hi;
       face_row_range(D, kq, kt, f, S_lo, S_hi);
       for (int S = S_lo; S <= S_hi; ++S) {

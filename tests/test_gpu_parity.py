@@ -12,7 +12,7 @@ import pytest
 torch = pytest.importorskip("torch")
 
 import oracle as orc
-from helpers import ocfg, oracle_mask, small_scene
+from helpers import canon_pairs, ocfg, oracle_mask, small_scene
 
 pytestmark = pytest.mark.gpu
 
@@ -175,8 +175,9 @@ def test_tile_query_bit_exact(cfg_id, P, order, extra):
             B.uts_tile_query(cfg, proj, mask, offsets, keys, vals, n - 1, scratch)
         assert ei.value.status == B.UTS_ERR_CAPACITY and ei.value.needed == n
     n = B.uts_tile_query(cfg, proj, mask, offsets, keys, vals, n, scratch)
-    assert np.array_equal(u64(keys)[:n], c.fw["keys"])
-    assert np.array_equal(u32(vals)[:n], c.fw["vals"])
+    gk, gv = canon_pairs(u64(offsets), u64(keys), u32(vals))
+    assert np.array_equal(gk, c.fw["keys"])
+    assert np.array_equal(gv, c.fw["vals"])
 
 
 @pytest.mark.parametrize("refine", [0, 1, 3, 4])
@@ -194,7 +195,8 @@ def test_tile_query_other_refinements(refine):
     n = r.tile_query()
     assert n == keys.shape[0]
     assert np.array_equal(u64(r.offsets), off)
-    assert np.array_equal(u64(r.keys)[:n], keys) and np.array_equal(u32(r.vals)[:n], vals)
+    gk, gv = canon_pairs(u64(r.offsets), u64(r.keys), u32(r.vals))
+    assert np.array_equal(gk, keys) and np.array_equal(gv, vals)
 
 
 @pytest.mark.parametrize("cfg_id,order,refine", [(4, 9, 2), (3, 9, 2), (4, 8, 1), (5, 10, 2)])
@@ -217,7 +219,8 @@ def test_tile_query_block_path_large_discs(cfg_id, order, refine):
     n = r.tile_query()
     assert n == keys.shape[0]
     assert np.array_equal(u64(r.offsets), off)
-    assert np.array_equal(u64(r.keys)[:n], keys) and np.array_equal(u32(r.vals)[:n], vals)
+    gk, gv = canon_pairs(u64(r.offsets), u64(r.keys), u32(r.vals))
+    assert np.array_equal(gk, keys) and np.array_equal(gv, vals)
 
 
 def test_tile_query_whole_sphere_and_empty():
@@ -233,7 +236,8 @@ def test_tile_query_whole_sphere_and_empty():
     r = R.Rasterizer(cfg, depth_presort=False)
     r.proj = B.Proj(dev(pr.dir), dev(pr.lonlat), dev(pr.rho), dev(pr.conic_opac), dev(pr.rs), dev(pr.rgb), dev(pr.flags))
     n = r.tile_query()
-    assert np.array_equal(u64(r.offsets), off) and np.array_equal(u64(r.keys)[:n], keys) and np.array_equal(u32(r.vals)[:n], vals)
+    gk, gv = canon_pairs(u64(r.offsets), u64(r.keys), u32(r.vals))
+    assert np.array_equal(u64(r.offsets), off) and np.array_equal(gk, keys) and np.array_equal(gv, vals)
     # P = 0
     cfg0 = B.Config(order=6, n_gauss=0)
     r0 = R.Rasterizer(cfg0, depth_presort=False)
@@ -265,7 +269,8 @@ def test_tile_query_ring_mode_bit_exact(cfg_id, P, order, refine, big):
     n = r.tile_query()
     assert n == keys.shape[0]
     assert np.array_equal(u64(r.offsets), off)
-    assert np.array_equal(u64(r.keys)[:n], keys) and np.array_equal(u32(r.vals)[:n], vals)
+    gk, gv = canon_pairs(u64(r.offsets), u64(r.keys), u32(r.vals))
+    assert np.array_equal(gk, keys) and np.array_equal(gv, vals)
     # and it is not the NESTED set
     ocn = ocfg(scene, query_refine_log2=refine)
     assert orc.tile_query(ocn, pr, slot)[1].shape[0] > n

@@ -41,9 +41,10 @@ def _host_sets(L, oc, pr, mode):
     for i in range(oc.n_gauss):
         if pr.flags[0, i] & 1:
             out.append(np.zeros(0, np.uint32)); continue
-        u = pr.dir[0, i].astype(np.float64); u = u / math.sqrt(float(u @ u))
+        d = np.ascontiguousarray(pr.dir[0, i], np.float32)
         R = min(math.pi, float(pr.rs[0, i]) + rho_q)
-        n = L.ring_query_host(kt, kq, u.ctypes.data_as(C.c_void_p), C.c_double(R), buf.ctypes.data_as(C.c_void_p), buf.shape[0], C.byref(nr))
+        n = L.ring_query_host(kt, kq, d.ctypes.data_as(C.c_void_p), C.c_float(pr.lonlat[0, i, 0]), C.c_float(pr.lonlat[0, i, 1]), C.c_double(R),
+                              buf.ctypes.data_as(C.c_void_p), buf.shape[0], C.byref(nr))
         out.append(buf[:n].copy())
     return out
 
@@ -81,6 +82,8 @@ def test_ring_interval_query_poles_large_and_whole_sphere(hostlib, order, refine
         d[8:24, 1] = np.where(np.arange(16) % 2 == 0, 1, -1) * (1.0 + 4.0 * rng.random(16))        # near the poles
         d /= np.linalg.norm(d, axis=1, keepdims=True)
         pr.dir[0] = d.astype(np.float32)
+        pr.lonlat[0, :, 0] = np.arctan2(d[:, 0], d[:, 2]).astype(np.float32)            # Eq.1 PAPER.md:72 for the hand-made directions
+        pr.lonlat[0, :, 1] = np.arctan2(d[:, 1], np.hypot(d[:, 0], d[:, 2])).astype(np.float32)
         rs = np.exp(rng.uniform(math.log(0.003), math.log(3.2), 64))
         rs[:8] = [0.3, 0.21, 0.9, 0.08, math.pi, 2.5, 0.4, 1.6]
         pr.rs[0] = np.minimum(rs, math.pi).astype(np.float32)

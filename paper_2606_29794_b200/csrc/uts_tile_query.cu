@@ -47,6 +47,9 @@ struct QueryParams {
   int b_block, b_warp;                  // buckets <= b_block: one block per disc; <= b_warp: one warp; others: one thread
   int rc_thread, rc_warp, rc_block;     // ring-table capacities of the three shapes
   const uint32_t* active_tiles; int n_active;   // mask's ascending active-tile list (whole-sphere discs), or null
+  // row-mask cache of the block-per-disc shape: the count pass stores every (row, chunk) mask of a disc at
+  // mask_cache[mask_base[k] ...], the emit pass replays them (no ring phase); a disc that does not fit is recomputed
+  unsigned long long* mask_cache; uint32_t mask_cache_cap; uint32_t* mask_cursor; uint32_t* mask_base;
 };
 
 // Per-Gaussian query state.
@@ -510,6 +513,29 @@ __device__ __forceinline__ uint32_t visit_row_chunk(int kt, int f, int S, int jb
   return cnt;
 }
 
+// the chunk's mask restricted to active tiles
+__device__ __forceinline__ unsigned long long filter_row_chunk(int kt, int f, int S, int jbase, unsigned long long mask, const int32_t* __restrict__ slot_of_tile) {
+  if (!slot_of_tile || !mask) return mask;
+  unsigned long long out = 0;
+  int j = __ffsll((long long)mask) - 1;
+  visit_row_chunk<true>(kt, f, S, jbase, mask, nullptr, [&](uint32_t tile) {
+    while (!((mask >> j) & 1ull)) ++j;
+    if (__ldg(slot_of_tile + tile) >= 0) out |= 1ull << j;
+    ++j;
+  });
+  return out;
+}
+
+// position of the r-th (0-based) set bit of mask
+__device__ __forceinline__ int nth_set_bit(unsigned long long mask, int r) {
+  const int j0 = __ffsll((long long)mask) - 1;
+  const unsigned long long run = mask >> j0;
+  if ((run & (run + 1ull)) == 0ull) return j0 + r;                      // one contiguous run (the usual case)
+  const uint32_t lo = (uint32_t)mask, hi = (uint32_t)(mask >> 32);
+  const int nlo = __popc(lo);
+  return r < nlo ? (int)__fns(lo, 0, r + 1) : 32 + (int)__fns(hi, 0, r - nlo + 1);
+}
+
 // rows of a disc: face f owns rows [pre[f], pre[f+1]) of the flat enumeration, S = S_lo(f) + (row - pre[f])
 __device__ __forceinline__ int disc_face_rows(const QueryParams& qp, const RingDisc& D, uint16_t* pre /*[13]*/) {
   int run = 0;
@@ -533,7 +559,7 @@ struct BatchRec {
 };
 
 template <int G, bool EMIT>
-__global__ void __launch_bounds__(kLargeThreads)
+__global__ void __launch_bounds__(kLargeThreads, 4)
 ring_query_batch_kernel(QueryParams qp, int which /*0: rc_warp class, 1: rc_thread class*/, const float* __restrict__ dir, const float* __restrict__ lonlat,
                         const float* __restrict__ rho, const float* __restrict__ rs, const int32_t* __restrict__ slot_of_tile,
                         const uint32_t* __restrict__ perm, const uint32_t* __restrict__ n_small, const uint32_t* __restrict__ emit_rank,
@@ -652,7 +678,7 @@ ring_query_batch_kernel(QueryParams qp, int which /*0: rc_warp class, 1: rc_thre
 
 // ---------------------------------------------------------------------------------------------- one block per large disc
 template <bool EMIT>
-__global__ void __launch_bounds__(kLargeThreads)
+__global__ void __launch_bounds__(kLargeThreads, 4)
 ring_query_block_kernel(QueryParams qp, const float* __restrict__ dir, const float* __restrict__ lonlat, const float* __restrict__ rho,
                         const float* __restrict__ rs, const int32_t* __restrict__ slot_of_tile, const uint32_t* __restrict__ perm,
                         const uint32_t* __restrict__ n_small, const uint32_t* __restrict__ emit_rank, uint32_t* __restrict__ counts,
@@ -661,7 +687,9 @@ ring_query_block_kernel(QueryParams qp, const float* __restrict__ dir, const flo
   __shared__ RingDisc s_disc;
   __shared__ uint16_t s_pre[13];
   __shared__ int s_Slo[12];
-  __shared__ uint32_t s_cursor;
+  __shared__ uint32_t s_cursor, s_mbase;
+  __shared__ unsigned long long s_em_mask[kLargeThreads / 32][32];
+  __shared__ uint32_t s_em_pre[kLargeThreads / 32][33], s_em_row[kLargeThreads / 32][32];
   const uint32_t end = n_small[1];
   const int N = 1 << qp.kq, tid = threadIdx.x;
   for (uint32_t idx = blockIdx.x; idx < end; idx += gridDim.x) {
@@ -679,6 +707,13 @@ ring_query_block_kernel(QueryParams qp, const float* __restrict__ dir, const flo
       disc_face_rows(qp, s_disc, s_pre);
       for (int f = 0; f < 12; ++f) { int S_lo, S_hi; face_row_range(s_disc, qp.kq, qp.kt, f, S_lo, S_hi); s_Slo[f] = S_lo; }
       s_cursor = 0;
+      const uint32_t n_it = (uint32_t)s_pre[12] * (uint32_t)(((1 << qp.kt) + 63) >> 6);
+      if (s_disc.all) s_mbase = 0xffffffffu;
+      else if (!EMIT) {                                // claim room for this disc's row masks
+        uint32_t at = atomicAdd(qp.mask_cursor, n_it);
+        if (at > qp.mask_cache_cap || n_it > qp.mask_cache_cap - at) at = 0xffffffffu;
+        qp.mask_base[k] = at; s_mbase = at;
+      } else s_mbase = qp.mask_base[k];
     }
     __syncthreads();
     const RingDisc& D = s_disc;
@@ -691,24 +726,75 @@ ring_query_block_kernel(QueryParams qp, const float* __restrict__ dir, const flo
       }
       continue;
     }
-    for (int e = tid; e <= D.i_hi - D.i_lo; e += kLargeThreads) { int2 fl; ring_interval(D, N, D.i_lo + e, fl.x, fl.y); ring_tab[e] = fl; }
-    __syncthreads();
+    const bool cached = s_mbase != 0xffffffffu;
+    unsigned long long* mcache = qp.mask_cache + (cached ? (size_t)s_mbase : 0);
+    if (!(EMIT && cached)) {                           // phase 1 (the emit pass skips it when the masks were kept)
+      for (int e = tid; e <= D.i_hi - D.i_lo; e += kLargeThreads) { int2 fl; ring_interval(D, N, D.i_lo + e, fl.x, fl.y); ring_tab[e] = fl; }
+      __syncthreads();
+    }
     const GroupTab T{ring_tab, D.i_lo};
     const int n_rows = (int)s_pre[12];
-    for (int row = tid; row < n_rows; row += kLargeThreads) {
-      int f = 0;
+    const int n_chunks = ((1 << qp.kt) + 63) >> 6;                         // chunks per row (a row has at most 2^kt tiles)
+    const int n_items = n_rows * n_chunks;
+    // the active-tile mask of item = (row, 64-candidate chunk)
+    auto item_mask = [&](int item, int& f, int& S, int& jbase) -> unsigned long long {
+      const int row = item / n_chunks;
+      jbase = (item - row * n_chunks) << 6;
+      f = 0;
       while (f < 11 && (int)s_pre[f + 1] <= row) ++f;
-      const int S = s_Slo[f] + row - (int)s_pre[f], Hm = min(S, (2 << qp.kt) - 2 - S);
-      for (int jbase = 0; jbase <= Hm; jbase += 64) {
-        const unsigned long long mask = tile_row_mask(D, qp.kq, qp.kt, f, S, jbase, T);
-        if (!mask) continue;
-        const uint32_t c = visit_row_chunk<false>(qp.kt, f, S, jbase, mask, slot_of_tile, [](uint32_t) {});
-        const uint32_t at = atomicAdd(&s_cursor, c);
-        if (EMIT) {
-          uint64_t pos = b0 + at;
-          visit_row_chunk<true>(qp.kt, f, S, jbase, mask, slot_of_tile, [&](uint32_t tile) {
-            keys[pos] = ((hi + tile) << 32) | depth; vals[pos] = gid; ++pos;                  // Alg.1 l.12: ((t, rho), i)
-          });
+      S = s_Slo[f] + row - (int)s_pre[f];
+      if (EMIT && cached) return mcache[item];
+      if (jbase > min(S, (2 << qp.kt) - 2 - S)) return 0ull;
+      return filter_row_chunk(qp.kt, f, S, jbase, tile_row_mask(D, qp.kq, qp.kt, f, S, jbase, T), slot_of_tile);
+    };
+    if (!EMIT) {
+      uint32_t mine = 0;
+      for (int item = tid; item < n_items; item += kLargeThreads) {
+        int f, S, jbase;
+        const unsigned long long mask = item_mask(item, f, S, jbase);
+        if (cached) mcache[item] = mask;
+        mine += (uint32_t)__popcll(mask);
+      }
+      if (mine) atomicAdd(&s_cursor, mine);
+    } else {
+      // Each lane settles one (row, chunk); the warp then writes the tiles of its 32 chunks as ONE contiguous run of pairs
+      // (lane p takes the p-th tile of the run), so the stores are coalesced.
+      const int lane = tid & 31, wid = tid >> 5;
+      const int n_rounds = (n_items + kLargeThreads - 1) / kLargeThreads;
+      for (int round = 0; round < n_rounds; ++round) {
+        const int item = round * kLargeThreads + tid;
+        unsigned long long mask = 0;
+        int f = 0, S = 0, jbase = 0;
+        if (item < n_items) mask = item_mask(item, f, S, jbase);
+        const uint32_t c = (uint32_t)__popcll(mask);
+        uint32_t incl = c;
+#pragma unroll
+        for (int dd = 1; dd < 32; dd <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, incl, dd); if (lane >= dd) incl += y; }
+        const uint32_t wtotal = __shfl_sync(0xffffffffu, incl, 31);
+        if (wtotal == 0) continue;
+        uint32_t wbase = 0;
+        if (lane == 0) wbase = atomicAdd(&s_cursor, wtotal);
+        wbase = __shfl_sync(0xffffffffu, wbase, 0);
+        __syncwarp();
+        {
+          const int Hm = min(S, (2 << qp.kt) - 2 - S);
+          s_em_mask[wid][lane] = mask;
+          s_em_pre[wid][lane] = incl - c;
+          if (lane == 31) s_em_pre[wid][32] = wtotal;
+          s_em_row[wid][lane] = ((uint32_t)f << 24) | ((uint32_t)(((S - Hm) >> 1) + jbase) << 12) | (uint32_t)(((S + Hm) >> 1) - jbase);   // f, X0, Y0
+        }
+        __syncwarp();
+        int lo = 0, hi2 = 32;                                              // owner of pair `lane`: last chunk whose exclusive prefix is <= it
+        while (hi2 - lo > 1) { const int mid = (lo + hi2) >> 1; if (s_em_pre[wid][mid] <= (uint32_t)lane) lo = mid; else hi2 = mid; }
+        for (uint32_t pp = lane; pp < wtotal; pp += 32) {
+          while (s_em_pre[wid][lo + 1] <= pp) ++lo;                        // owners are monotone in pp; skips empty chunks
+          const unsigned long long mk = s_em_mask[wid][lo];
+          const uint32_t rw = s_em_row[wid][lo];
+          const int j = nth_set_bit(mk, (int)(pp - s_em_pre[wid][lo]));
+          const uint32_t tile = ((rw >> 24) << (2 * qp.kt)) | spread_bits16_hd(((rw >> 12) & 0xfffu) + (uint32_t)j) |
+                                (spread_bits16_hd((rw & 0xfffu) - (uint32_t)j) << 1);
+          keys[b0 + wbase + pp] = ((hi + tile) << 32) | depth;            // Alg.1 l.12: ((t, rho), i)
+          vals[b0 + wbase + pp] = gid;
         }
       }
     }
@@ -732,7 +818,7 @@ int radius_bucket_host(float R32) {                    // host replica of radius
 }
 constexpr int kRingThreadRings = 24, kRingWarpRings = 128, kRingBlockRingsMax = 24575;   // ring-table capacities (8 B per ring)
 
-struct QueryLayout { size_t counts, list, perm, nlarge, active, scan, tcache, bcache, total; uint32_t bcache_cap; };
+struct QueryLayout { size_t counts, list, perm, nlarge, active, scan, tcache, bcache, bcache_bytes, total; uint32_t bcache_cap; };
 QueryLayout query_layout(const uts_config* cfg) {
   const size_t n = (size_t)cfg->n_gauss * cfg->n_views;
   const size_t n_tile = (size_t)12 << (2 * (cfg->order - cfg->tile_log2));
@@ -751,7 +837,12 @@ QueryLayout query_layout(const uts_config* cfg) {
   if (cap > n) cap = n;
   if (n_tile < 192 || row * 2 + 4096 * 8 > kMaxLargeSmem) cap = 0;
   L.bcache_cap = (uint32_t)cap;
-  L.bcache = off; off += align256(cap * row);
+  // at least 64 B per (view, Gaussian), at most 384 MB: the ring path keeps its row masks here
+  size_t bytes = cap * row;
+  const size_t want = n * 64 < (size_t)(384u << 20) ? n * 64 : (size_t)(384u << 20);
+  if (bytes < want) bytes = want;
+  L.bcache_bytes = bytes;
+  L.bcache = off; off += align256(bytes);
   L.total = off + 256;
   return L;
 }
@@ -799,6 +890,8 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   qp.b_block = radius_bucket_host((float)((qp.rc_warp - 6) / (3.0 * Nq)));
   if (qp.b_block > qp.b_warp) qp.b_block = qp.b_warp;
   qp.active_tiles = mask.active_tiles; qp.n_active = mask.active_tiles ? mask.n_active : -1;
+  // the ring path reuses two scratch regions of the descent: the bitmap cache holds the row masks, `list` their bases
+  qp.mask_cache = nullptr; qp.mask_cache_cap = 0; qp.mask_cursor = nullptr; qp.mask_base = nullptr;
   qp.os = d.kt < 4 ? d.kt : 4;
   const size_t n_split = (size_t)12 << (2 * qp.os);
   qp.wl_cap = (int)(n_split > 4096 ? n_split : 4096);
@@ -821,6 +914,10 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   qp.tile_cache = reinterpret_cast<uint32_t*>(sp + L.tcache);
   qp.bitmap_cache = reinterpret_cast<uint32_t*>(sp + L.bcache);
   qp.bitmap_cache_cap = L.bcache_cap;
+  qp.mask_cache = reinterpret_cast<unsigned long long*>(sp + L.bcache);
+  qp.mask_cache_cap = (uint32_t)(L.bcache_bytes / 8);
+  qp.mask_cursor = n_large + 8;                                              // zeroed with the header below
+  qp.mask_base = list;
   const uint32_t* active_arg = nullptr;
   const unsigned qgrid = (unsigned)((n + kLargeThreads - 1) / kLargeThreads);
   const int lgrid = use_large ? sm_count() * (e2__ ? atoi(e2__) : 2) : 0;
@@ -849,7 +946,7 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   constexpr int kBatchA = 128, kBatchB = 32;          // discs per batch: rc_thread class, rc_warp class
   const size_t smem_a = sizeof(BatchRec) * kBatchA + (size_t)kBatchA * qp.rc_thread * sizeof(int2),
                smem_b = sizeof(BatchRec) * kBatchB + (size_t)kBatchB * qp.rc_warp * sizeof(int2), smem_block = (size_t)qp.rc_block * sizeof(int2);
-  const unsigned agrid = (unsigned)sm_count() * 8u, wgrid = (unsigned)sm_count() * 8u, bgrid = (unsigned)sm_count() * 4u;
+  unsigned agrid = 0, wgrid = 0, bgrid = 0, agrid_e = 0, wgrid_e = 0, bgrid_e = 0;     // persistent grids: exactly the resident blocks
   if (ring_impl) {
     static bool ring_attr_set = false;
     if (!ring_attr_set) {
@@ -860,6 +957,19 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
       UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
       UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
       ring_attr_set = true;
+    }
+    {
+      int occ[6] = {1, 1, 1, 1, 1, 1};
+      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[0], ring_query_block_kernel<false>, kLargeThreads, smem_block));
+      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[1], ring_query_block_kernel<true>, kLargeThreads, smem_block));
+      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[2], ring_query_batch_kernel<kBatchB, false>, kLargeThreads, smem_b));
+      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[3], ring_query_batch_kernel<kBatchB, true>, kLargeThreads, smem_b));
+      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[4], ring_query_batch_kernel<kBatchA, false>, kLargeThreads, smem_a));
+      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[5], ring_query_batch_kernel<kBatchA, true>, kLargeThreads, smem_a));
+      const unsigned sms = (unsigned)sm_count();
+      bgrid = sms * (unsigned)(occ[0] > 0 ? occ[0] : 1); bgrid_e = sms * (unsigned)(occ[1] > 0 ? occ[1] : 1);
+      wgrid = sms * (unsigned)(occ[2] > 0 ? occ[2] : 1); wgrid_e = sms * (unsigned)(occ[3] > 0 ? occ[3] : 1);
+      agrid = sms * (unsigned)(occ[4] > 0 ? occ[4] : 1); agrid_e = sms * (unsigned)(occ[5] > 0 ? occ[5] : 1);
     }
     ring_query_block_kernel<false><<<bgrid, kLargeThreads, smem_block, s>>>(qp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small, emit_rank,
                                                                           counts, nullptr, nullptr, nullptr);
@@ -882,13 +992,13 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   if (*h_n_pairs > capacity) return UTS_ERR_CAPACITY;
   if (*h_n_pairs == 0) return UTS_OK;
   if (ring_impl) {
-    ring_query_block_kernel<true><<<bgrid, kLargeThreads, smem_block, s>>>(qp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small, emit_rank,
+    ring_query_block_kernel<true><<<bgrid_e, kLargeThreads, smem_block, s>>>(qp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small, emit_rank,
                                                                          nullptr, offsets, keys, vals);
     UTS_LAUNCH_CHECK();
-    ring_query_batch_kernel<kBatchB, true><<<wgrid, kLargeThreads, smem_b, s>>>(qp, 0, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
+    ring_query_batch_kernel<kBatchB, true><<<wgrid_e, kLargeThreads, smem_b, s>>>(qp, 0, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
                                                                               emit_rank, nullptr, offsets, keys, vals);
     UTS_LAUNCH_CHECK();
-    ring_query_batch_kernel<kBatchA, true><<<agrid, kLargeThreads, smem_a, s>>>(qp, 1, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
+    ring_query_batch_kernel<kBatchA, true><<<agrid_e, kLargeThreads, smem_a, s>>>(qp, 1, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
                                                                               emit_rank, nullptr, offsets, keys, vals);
     UTS_LAUNCH_CHECK();
     return UTS_OK;

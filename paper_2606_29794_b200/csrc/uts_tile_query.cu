@@ -556,6 +556,8 @@ struct BatchRec {
   uint64_t hi, base;          // key high part of the view; first pair of the Gaussian (emit)
   uint32_t depth, gid, slot, k;
   uint32_t cached;            // emit: the count pass left the tiles in tile_cache
+  uint32_t mbase;             // first row mask of this disc in mask_cache, or 0xffffffff
+  uint32_t skip;              // no rows to walk (no tiles, replayed from tile_cache, or a whole-sphere disc)
 };
 
 template <int G, bool EMIT>
@@ -568,6 +570,7 @@ ring_query_batch_kernel(QueryParams qp, int which /*0: rc_warp class, 1: rc_thre
   __shared__ uint32_t s_w[kLargeThreads / 32];
   __shared__ int ring_off[G + 1], row_off[G + 1];
   __shared__ uint32_t cursor[G];
+  __shared__ uint32_t s_bbase;
   __shared__ uint16_t rowpre[G][13];
   BatchRec* rec = reinterpret_cast<BatchRec*>(smem_raw);
   int2* tab = reinterpret_cast<int2*>(smem_raw + sizeof(BatchRec) * G);
@@ -599,8 +602,9 @@ ring_query_batch_kernel(QueryParams qp, int which /*0: rc_warp class, 1: rc_thre
       load_ring_disc(qp, dir, lonlat, rs, k, r.D);
       if (r.D.all) skip = true;                        // handled after the row loop
       r.D.i_hi = min(r.D.i_hi, r.D.i_lo + rc - 1);
-      if (skip) r.D.i_hi = r.D.i_lo - 1;
-      my_rings = (uint32_t)(r.D.i_hi - r.D.i_lo + 1);
+      r.skip = skip ? 1u : 0u;
+      r.mbase = (EMIT && !skip) ? qp.mask_base[k] : 0xffffffffu;          // emit: the count pass kept this disc's row masks
+      if (!skip && r.mbase == 0xffffffffu) my_rings = (uint32_t)(r.D.i_hi - r.D.i_lo + 1);
     }
     uint32_t before;
     const uint32_t n_rings = block_sum_u32(my_rings, s_w, before);
@@ -618,10 +622,24 @@ ring_query_batch_kernel(QueryParams qp, int which /*0: rc_warp class, 1: rc_thre
     }
     // ---- rows of every disc
     uint32_t my_rows = 0;
-    if (tid < ng && rec[tid].D.i_hi >= rec[tid].D.i_lo) my_rows = (uint32_t)disc_face_rows(qp, rec[tid].D, rowpre[tid]);
+    if (tid < ng && !rec[tid].skip) my_rows = (uint32_t)disc_face_rows(qp, rec[tid].D, rowpre[tid]);
     const uint32_t n_rows = block_sum_u32(my_rows, s_w, before);
+    const int n_chunks = ((1 << qp.kt) + 63) >> 6;     // 64-candidate chunks per row
     if (tid < ng) row_off[tid] = (int)before;
-    if (tid == 0) row_off[ng] = (int)n_rows;
+    if (tid == 0) {
+      row_off[ng] = (int)n_rows;
+      if (!EMIT) {                                     // claim room for the batch's row masks
+        const uint32_t n_it = n_rows * (uint32_t)n_chunks;
+        uint32_t at = atomicAdd(qp.mask_cursor, n_it);
+        if (at > qp.mask_cache_cap || n_it > qp.mask_cache_cap - at) at = 0xffffffffu;
+        s_bbase = at;
+      }
+    }
+    __syncthreads();
+    if (!EMIT && tid < ng && !rec[tid].skip) {
+      rec[tid].mbase = s_bbase == 0xffffffffu ? 0xffffffffu : s_bbase + (uint32_t)row_off[tid] * (uint32_t)n_chunks;
+      qp.mask_base[rec[tid].k] = rec[tid].mbase;
+    }
     __syncthreads();
     // ---- phase 2, flattened over (disc, row)
     for (uint32_t it = tid; it < n_rows; it += kLargeThreads) {
@@ -636,20 +654,25 @@ ring_query_batch_kernel(QueryParams qp, int which /*0: rc_warp class, 1: rc_thre
       const int S = S_lo + row - (int)rowpre[lo][f], Hm = min(S, (2 << qp.kt) - 2 - S);
       const GroupTab T{tab + ring_off[lo], r.D.i_lo};
       for (int jbase = 0; jbase <= Hm; jbase += 64) {
-        const unsigned long long mask = tile_row_mask(r.D, qp.kq, qp.kt, f, S, jbase, T);
+        const size_t mi = (size_t)r.mbase + (size_t)row * n_chunks + (size_t)(jbase >> 6);
+        unsigned long long mask;
+        if (EMIT && r.mbase != 0xffffffffu) mask = qp.mask_cache[mi];
+        else {
+          mask = filter_row_chunk(qp.kt, f, S, jbase, tile_row_mask(r.D, qp.kq, qp.kt, f, S, jbase, T), slot_of_tile);
+          if (!EMIT && r.mbase != 0xffffffffu) qp.mask_cache[mi] = mask;
+        }
         if (!mask) continue;
+        const uint32_t c = (uint32_t)__popcll(mask);
         if (EMIT) {
-          const uint32_t c = visit_row_chunk<false>(qp.kt, f, S, jbase, mask, slot_of_tile, [](uint32_t) {});
           uint64_t pos = r.base + atomicAdd(&cursor[lo], c);
-          visit_row_chunk<true>(qp.kt, f, S, jbase, mask, slot_of_tile, [&](uint32_t tile) {
+          visit_row_chunk<true>(qp.kt, f, S, jbase, mask, nullptr, [&](uint32_t tile) {
             keys[pos] = ((r.hi + tile) << 32) | r.depth; vals[pos] = r.gid; ++pos;            // Alg.1 l.12: ((t, rho), i)
           });
         } else {
-          const uint32_t c = visit_row_chunk<false>(qp.kt, f, S, jbase, mask, slot_of_tile, [](uint32_t) {});
           uint32_t pos = atomicAdd(&cursor[lo], c);
           if (pos < (uint32_t)kTileCacheK) {           // remember the first tiles: the emit pass replays discs of <= kTileCacheK tiles
             uint32_t* cache = qp.tile_cache + (size_t)r.k * kTileCacheK;
-            visit_row_chunk<true>(qp.kt, f, S, jbase, mask, slot_of_tile, [&](uint32_t tile) { if (pos < (uint32_t)kTileCacheK) cache[pos] = tile; ++pos; });
+            visit_row_chunk<true>(qp.kt, f, S, jbase, mask, nullptr, [&](uint32_t tile) { if (pos < (uint32_t)kTileCacheK) cache[pos] = tile; ++pos; });
           }
         }
       }

@@ -301,7 +301,7 @@ def run_ours(args):
             per_kernel[s_] = dict(ms=ms, tflops=ev_b * FLOP_BWD / (ms * 1e-3) / 1e12, frac_fp32_peak=ev_b * FLOP_BWD / (ms * 1e-3) / 1e12 / fp32_peak)
         else:
             byts = {"preprocess": P * V * (44 + 12 * M + 57), "preprocess_bwd": P * (44 + 12 * M + V * 33 + 40 + 12 * M),
-                    "depth_order": P * V * (4 + 5 * 32 + 16), "tile_query": P * V * 2 * 21 + 8 * P * V + 12 * n_pairs, "sort": 32.0 * n_pairs * ((max(1, (V * cfg.n_tiles - 1)).bit_length() + 7) // 8),
+                    "depth_order": P * V * (4 + 5 * 32 + 16), "tile_query": P * V * 2 * 29 + 8 * P * V + 12 * n_pairs, "sort": 32.0 * n_pairs * ((max(1, (V * cfg.n_tiles - 1)).bit_length() + 7) // 8),
                     "tile_ranges": 8.0 * n_pairs + 16 * V * cfg.n_tiles}[s_]
             per_kernel[s_] = dict(ms=ms, gbs=byts / (ms * 1e-3) / 1e9, frac_hbm_peak=byts / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
 
@@ -318,9 +318,9 @@ def run_ours(args):
     # launches of our kernels per step: 1 preprocess + (1 count + 3 scan + 1 emit) + passes*(1 + 3 + 1) (+1 copy) + 1 ranges + 1 fwd + 1 bwd + 1 pre-bwd
     passes = (max(1, (V * cfg.n_tiles - 1)).bit_length() + 7) // 8          # pair sort: (view,tile) bytes only
     dpass = 4 + ((max(1, V - 1).bit_length() + 7) // 8 if V > 1 else 0)     # depth order of the Gaussians
-    # preprocess 1; depth order 1 + 5/pass (+copy) + 1; query 3 classify + 1 count + 3 scan + 1 emit; sort 5/pass (+copy);
+    # preprocess 1; depth order 1 + 5/pass (+copy) + 1; query 3 classify + 3 count + 3 scan + 3 emit; sort 5/pass (+copy);
     # ranges 1; blend fwd 1; blend bwd 1; preprocess bwd 1
-    line["gpu_launches"] = args.steps * (1 + (2 + dpass * 5 + dpass % 2) + 8 + (passes * 5 + passes % 2) + 4)
+    line["gpu_launches"] = args.steps * (1 + (2 + dpass * 5 + dpass % 2) + 12 + (passes * 5 + passes % 2) + 4)
     if not args.no_cpu_baseline:
         smp = OracleSample(args.config, seed=0, n_pre=400_000, n_query=40_000, n_tiles_sample=96)
         t, desc = smp.step()

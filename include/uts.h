@@ -114,9 +114,13 @@ int uts_depth_order(const uts_config* cfg, const float* rho /*[V,P]*/, uint32_t*
                     size_t scratch_bytes, void* stream);
 size_t uts_depth_order_scratch_bytes(const uts_config* cfg);
 
-/* Alg.1 l.9-14 with Alg.2 (reading A6).  The tile set of (v,i) is
- *     { q >> 2(k_q-k_t) : q an order-k_q NESTED pixel with  u . centre(q) >= cos(min(pi, r_s + rho_max(k_q))) } ∩ active tiles,
- * evaluated in double precision.  Pairs are written Gaussian by Gaussian, tiles ascending inside a Gaussian:
+/* Alg.1 l.9-14 with Alg.2 (reading A6) or, with cfg->query_mode = UTS_QUERY_RING, Alg.3.  The tile set of (v,i) is
+ *     { q >> 2(k_q-k_t) : q an order-k_q NESTED pixel with  u . centre(q) >= cos R } ∩ active tiles,
+ *     R = min(pi, r_s + rho_max(k_q)) (NESTED set)  or  min(pi, r_s) (RING set),
+ * the predicate evaluated in double precision wherever single precision cannot decide it.  Reads in.dir, in.lonlat, in.rho,
+ * in.rs, in.flags.  Pairs are written Gaussian by Gaussian; the pairs of one (v,i) are contiguous (offsets) and its tiles are
+ * distinct, but their ORDER INSIDE THAT SEGMENT IS UNSPECIFIED (no two keys of a segment tie, so uts_sort's result does not
+ * depend on it):
  *     keys[j] = ((v*N_tile + tile) << 32) | float_bits(rho[v,i]),   vals[j] = i.
  * emit_rank == NULL: Gaussians in (view, Gaussian id) order (slot of (v,i) = v*P+i).  Otherwise slot = emit_rank[v*P+i]
  * (a permutation of 0..V*P-1, e.g. from uts_depth_order).  offsets[V*P+1] (exclusive scan of the per-slot counts) is always

@@ -839,6 +839,24 @@ int radius_bucket_host(float R32) {                    // host replica of radius
   const int b = (int)(t >> 21) - (int)(u >> 21);
   return b < 0 ? 0 : (b > kBuckets - 1 ? kBuckets - 1 : b);
 }
+// The three shapes of the ring path are independent: they run side by side on two library-private streams that are forked from
+// and joined back to the caller's stream with events, so the caller still sees one ordered stream.
+struct ForkJoin {
+  cudaStream_t aux[2] = {nullptr, nullptr};
+  cudaEvent_t fork = nullptr, join[2] = {nullptr, nullptr};
+  bool ok = false;
+  bool init() {
+    if (ok) return true;
+    for (int i = 0; i < 2; ++i) {
+      if (cudaStreamCreateWithFlags(&aux[i], cudaStreamNonBlocking) != cudaSuccess) return false;
+      if (cudaEventCreateWithFlags(&join[i], cudaEventDisableTiming) != cudaSuccess) return false;
+    }
+    if (cudaEventCreateWithFlags(&fork, cudaEventDisableTiming) != cudaSuccess) return false;
+    ok = true;
+    return true;
+  }
+};
+ForkJoin g_fj;
 constexpr int kRingThreadRings = 24, kRingWarpRings = 128, kRingBlockRingsMax = 24575;   // ring-table capacities (8 B per ring)
 
 struct QueryLayout { size_t counts, list, perm, nlarge, active, scan, tcache, bcache, bcache_bytes, total; uint32_t bcache_cap; };
@@ -994,15 +1012,20 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
       wgrid = sms * (unsigned)(occ[2] > 0 ? occ[2] : 1); wgrid_e = sms * (unsigned)(occ[3] > 0 ? occ[3] : 1);
       agrid = sms * (unsigned)(occ[4] > 0 ? occ[4] : 1); agrid_e = sms * (unsigned)(occ[5] > 0 ? occ[5] : 1);
     }
+    if (!g_fj.init()) { set_last_cuda_error(cudaGetLastError()); return UTS_ERR_CUDA; }
+    UTS_CUDA(cudaEventRecord(g_fj.fork, s));
+    UTS_CUDA(cudaStreamWaitEvent(g_fj.aux[0], g_fj.fork, 0));
+    UTS_CUDA(cudaStreamWaitEvent(g_fj.aux[1], g_fj.fork, 0));
     ring_query_block_kernel<false><<<bgrid, kLargeThreads, smem_block, s>>>(qp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small, emit_rank,
                                                                           counts, nullptr, nullptr, nullptr);
     UTS_LAUNCH_CHECK();
-    ring_query_batch_kernel<kBatchB, false><<<wgrid, kLargeThreads, smem_b, s>>>(qp, 0, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
+    ring_query_batch_kernel<kBatchB, false><<<wgrid, kLargeThreads, smem_b, g_fj.aux[0]>>>(qp, 0, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
                                                                                emit_rank, counts, nullptr, nullptr, nullptr);
     UTS_LAUNCH_CHECK();
-    ring_query_batch_kernel<kBatchA, false><<<agrid, kLargeThreads, smem_a, s>>>(qp, 1, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
+    ring_query_batch_kernel<kBatchA, false><<<agrid, kLargeThreads, smem_a, g_fj.aux[1]>>>(qp, 1, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
                                                                                emit_rank, counts, nullptr, nullptr, nullptr);
     UTS_LAUNCH_CHECK();
+    for (int i = 0; i < 2; ++i) { UTS_CUDA(cudaEventRecord(g_fj.join[i], g_fj.aux[i])); UTS_CUDA(cudaStreamWaitEvent(s, g_fj.join[i], 0)); }
   } else {
     tile_query_kernel<false><<<qgrid + lgrid, kLargeThreads, dyn_smem, s>>>(qp, lgrid, in.dir, in.rho, in.rs, mask.slot_of_tile, active_arg, perm,
                                                                            n_small, list, n_large, emit_rank, counts, nullptr, nullptr, nullptr);
@@ -1015,15 +1038,19 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   if (*h_n_pairs > capacity) return UTS_ERR_CAPACITY;
   if (*h_n_pairs == 0) return UTS_OK;
   if (ring_impl) {
+    UTS_CUDA(cudaEventRecord(g_fj.fork, s));
+    UTS_CUDA(cudaStreamWaitEvent(g_fj.aux[0], g_fj.fork, 0));
+    UTS_CUDA(cudaStreamWaitEvent(g_fj.aux[1], g_fj.fork, 0));
     ring_query_block_kernel<true><<<bgrid_e, kLargeThreads, smem_block, s>>>(qp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small, emit_rank,
                                                                          nullptr, offsets, keys, vals);
     UTS_LAUNCH_CHECK();
-    ring_query_batch_kernel<kBatchB, true><<<wgrid_e, kLargeThreads, smem_b, s>>>(qp, 0, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
+    ring_query_batch_kernel<kBatchB, true><<<wgrid_e, kLargeThreads, smem_b, g_fj.aux[0]>>>(qp, 0, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
                                                                               emit_rank, nullptr, offsets, keys, vals);
     UTS_LAUNCH_CHECK();
-    ring_query_batch_kernel<kBatchA, true><<<agrid_e, kLargeThreads, smem_a, s>>>(qp, 1, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
+    ring_query_batch_kernel<kBatchA, true><<<agrid_e, kLargeThreads, smem_a, g_fj.aux[1]>>>(qp, 1, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
                                                                               emit_rank, nullptr, offsets, keys, vals);
     UTS_LAUNCH_CHECK();
+    for (int i = 0; i < 2; ++i) { UTS_CUDA(cudaEventRecord(g_fj.join[i], g_fj.aux[i])); UTS_CUDA(cudaStreamWaitEvent(s, g_fj.join[i], 0)); }
     return UTS_OK;
   }
   tile_query_kernel<true><<<qgrid + lgrid, kLargeThreads, dyn_smem, s>>>(qp, lgrid, in.dir, in.rho, in.rs, mask.slot_of_tile, active_arg, perm,

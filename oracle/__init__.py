@@ -16,8 +16,8 @@ from dataclasses import dataclass, field
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SRCS = ["orc_healpix.cpp", "orc_raster.cpp", "orc_capi.cpp"]
-_HDRS = ["orc_healpix.hpp", "orc_raster.hpp"]
+_SRCS = ["orc_healpix.cpp", "orc_raster.cpp", "orc_resample.cpp", "orc_capi.cpp"]
+_HDRS = ["orc_healpix.hpp", "orc_raster.hpp", "orc_resample.hpp"]
 _LIB = os.path.join(_HERE, "liboracle.so")
 
 
@@ -170,6 +170,66 @@ def mask_tiles(cfg: Config, bits):
     slot = np.full(cfg.n_tiles, -1, np.int32)
     slot[act] = np.arange(act.shape[0], dtype=np.int32)
     return act, slot
+
+
+# ------------------------------------------------------------------ image synthesis (orc_resample.hpp)
+CAMERA_MODELS = {"pinhole": 0, "fisheye": 1, "equirect": 2}
+
+
+@dataclass
+class Camera:
+    """model 'pinhole' (p0, p1 = FoV_x, FoV_y in radians), 'fisheye' (p0, p1 = w_x, w_y of Eq.12), 'equirect'."""
+    model: str
+    width: int
+    height: int
+    p0: float = 0.0
+    p1: float = 0.0
+
+    def args(self):
+        return (C.c_int(CAMERA_MODELS[self.model]), C.c_int(self.width), C.c_int(self.height), C.c_double(self.p0), C.c_double(self.p1))
+
+
+def cam_pixel_dir(cam: Camera, u, v):
+    d = np.zeros(3)
+    ok = lib().orc_cam_pixel_dir(*cam.args(), C.c_double(u), C.c_double(v), _p(d))
+    return d, bool(ok)
+
+
+def cam_project(cam: Camera, d):
+    uv = np.zeros(2)
+    dd = _f64(d)
+    ok = lib().orc_cam_project(*cam.args(), _p(dd), _p(uv))
+    return uv, bool(ok)
+
+
+def interp_weights(order, theta, lam):
+    pix = np.zeros(8, np.int64); w = np.zeros(8)
+    n = lib().orc_interp_weights(C.c_int(order), C.c_double(theta), C.c_double(lam), _p(pix), _p(w))
+    return pix[:n], w[:n]
+
+
+def resample_fwd(order, cam: Camera, image, slot_of_tile=None, pixel_mask_bits=None):
+    """image [n_slot*256, C] fp32 (slot layout) -> out [H, W, C] float64, valid [H, W] uint8."""
+    img = _f32(image); ch = img.shape[-1]
+    out = np.zeros((cam.height, cam.width, ch)); valid = np.zeros((cam.height, cam.width), np.uint8)
+    sl, mb = _i32(slot_of_tile), _u32(pixel_mask_bits)
+    lib().orc_resample_fwd(C.c_int(order), *cam.args(), _p(sl), _p(mb), _p(img), C.c_int(ch), _p(out), _p(valid))
+    return out, valid
+
+
+def resample_bwd(order, cam: Camera, dL_dout, n_slot, slot_of_tile=None, pixel_mask_bits=None):
+    g = _f64(dL_dout); ch = g.shape[-1]
+    out = np.zeros((n_slot * 256, ch))
+    sl, mb = _i32(slot_of_tile), _u32(pixel_mask_bits)
+    lib().orc_resample_bwd(C.c_int(order), *cam.args(), _p(sl), _p(mb), C.c_int64(n_slot), _p(g), C.c_int(ch), _p(out))
+    return out
+
+
+def camera_mask_bits(order, cam: Camera):
+    n = 12 << (2 * order)
+    bits = np.zeros((n + 31) // 32, np.uint32)
+    lib().orc_camera_mask(C.c_int(order), *cam.args(), _p(bits))
+    return bits
 
 
 # ------------------------------------------------------------------ stages (fp32 ABI arrays)

@@ -4,6 +4,7 @@
 // The *_f64 functions run preprocess -> blend without any fp32 rounding, for finite-difference pins.
 #include "orc_healpix.hpp"
 #include "orc_raster.hpp"
+#include "orc_resample.hpp"
 #include <cmath>
 #include <cstring>
 #include <vector>
@@ -83,6 +84,31 @@ void orc_mask(int order, int kind, const double* prm, uint32_t* bits /*N_pix/32 
     }
     if (on) bits[p >> 5] |= 1u << (p & 31);
   }
+}
+
+// ---------------------------------------------------------------- image synthesis (orc_resample.hpp; Eq.7, Eq.9, Eq.11-15)
+int orc_cam_pixel_dir(int model, int W, int H, double p0, double p1, double u, double v, double* d) {
+  Camera c{model, W, H, p0, p1};
+  return cam_pixel_dir(c, u, v, d) ? 1 : 0;
+}
+int orc_cam_project(int model, int W, int H, double p0, double p1, const double* d, double* uv) {
+  Camera c{model, W, H, p0, p1};
+  return cam_project(c, d, uv[0], uv[1]) ? 1 : 0;
+}
+int orc_interp_weights(int order, double theta, double lam, int64_t* pix, double* w) { return interp_weights(order, theta, lam, pix, w); }
+void orc_resample_fwd(int order, int model, int W, int H, double p0, double p1, const int32_t* slot_of_tile, const uint32_t* bits,
+                      const float* image, int channels, double* out, uint8_t* valid) {
+  Camera c{model, W, H, p0, p1};
+  resample_fwd(order, c, slot_of_tile, bits, image, channels, out, valid);
+}
+void orc_resample_bwd(int order, int model, int W, int H, double p0, double p1, const int32_t* slot_of_tile, const uint32_t* bits,
+                      int64_t n_slot, const double* dL_dout, int channels, double* dL_dimage) {
+  Camera c{model, W, H, p0, p1};
+  resample_bwd(order, c, slot_of_tile, bits, n_slot, dL_dout, channels, dL_dimage);
+}
+void orc_camera_mask(int order, int model, int W, int H, double p0, double p1, uint32_t* bits) {
+  Camera c{model, W, H, p0, p1};
+  camera_mask(order, c, bits);
 }
 
 // ---------------------------------------------------------------- O1 preprocess, fp32 ABI

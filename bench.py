@@ -104,8 +104,10 @@ class OracleSample:
         reach = pr.rs.astype(np.float64) + orc.rho_max_closed(oc.tile_order + oc.query_refine_log2) + orc.rho_max_closed(oc.tile_order) + 1e-6
         cand = np.zeros(P, bool)
         for v in range(V):
-            d = pr.dir[v].astype(np.float64) @ tc[pick].T
-            cand |= (np.arccos(np.clip(d, -1, 1)) <= reach[v][:, None]).any(axis=1)
+            for g0 in range(0, P, 262144):                 # chunked: the (Gaussian x sampled tile) table stays small
+                g1 = min(P, g0 + 262144)
+                d = pr.dir[v][g0:g1].astype(np.float64) @ tc[pick].T
+                cand[g0:g1] |= (np.arccos(np.clip(d, -1, 1)) <= reach[v][g0:g1, None]).any(axis=1)
         self.cand_ids = np.flatnonzero(cand).astype(np.int32)
         self.gcol = scenes.upstream_grad(V, pick.shape[0] * oc.ppt, seed=seed)
         _, keys, vals, _ = orc.tile_query(oc, pr, self.sslot, gauss_subset=self.cand_ids)          # complete lists of the sampled tiles
@@ -279,19 +281,28 @@ def run_ours(args):
         return
 
     value = replicas.aggregate_throughput(n_pix_active, ms_step_max, world)
+    # DRAM bytes per launch of each kernel from the committed ncu --set full capture of this workload (profiles/), or None
+    traffic = {}
+    tp = os.path.join(ROOT, "profiles", "r01_traffic.csv")
+    if os.path.exists(tp):
+        with open(tp) as f:
+            for ln in f.read().splitlines()[1:]:
+                w_, st_, by_ = ln.split(",")
+                if w_ == f"config{args.config}":
+                    traffic[st_] = int(by_)
     # dominant kernel and its roofline
     dom = max(stage_ms, key=stage_ms.get)
     fp32_peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12       # TFLOP/s at the maximum SM clock
     if dom in ("render_fwd", "render_bwd"):
         flop = ev_f * FLOP_FWD if dom == "render_fwd" else ev_b * FLOP_BWD
         ach = flop / (stage_ms[dom] * 1e-3) / 1e12
-        roof = dict(kernel=dom, bound="alu", achieved=ach, peak=fp32_peak, unit="TFLOP/s", frac=ach / fp32_peak, traffic=None,
+        roof = dict(kernel=dom, bound="alu", achieved=ach, peak=fp32_peak, unit="TFLOP/s", frac=ach / fp32_peak, traffic=traffic.get(dom),
                     peak_source="derived: 148 SM x 128 FP32 lanes x 2 x sm_max_mhz")
     else:
         per_pair = {"sort": 32.0 * ((max(1, (V * cfg.n_tiles - 1)).bit_length() + 7) // 8), "tile_query": 12.0, "tile_ranges": 8.0}.get(dom)
         byts = per_pair * n_pairs if per_pair else P * V * (44 + 12 * M + 57)
         ach = byts / (stage_ms[dom] * 1e-3) / 1e9
-        roof = dict(kernel=dom, bound="hbm", achieved=ach, peak=peaks["hbm_gbs"], unit="GB/s", frac=ach / peaks["hbm_gbs"], traffic=None,
+        roof = dict(kernel=dom, bound="hbm", achieved=ach, peak=peaks["hbm_gbs"], unit="GB/s", frac=ach / peaks["hbm_gbs"], traffic=traffic.get(dom),
                     peak_source=peaks["source"])
     per_kernel = {}
     for s_, ms in stage_ms.items():
@@ -322,7 +333,7 @@ def run_ours(args):
     # ranges 1; blend fwd 1; blend bwd 1; preprocess bwd 1
     line["gpu_launches"] = args.steps * (1 + (2 + dpass * 5 + dpass % 2) + 12 + (passes * 5 + passes % 2) + 4)
     if not args.no_cpu_baseline:
-        smp = OracleSample(args.config, seed=0, n_pre=400_000, n_query=40_000, n_tiles_sample=96)
+        smp = OracleSample(args.config, seed=0, n_pre=1_000_000, n_query=120_000, n_tiles_sample=384)   # about 10 s of oracle time on config 4
         t, desc = smp.step()
         line["cpu_baseline"] = dict(value=smp.n_pix / t, unit=UNIT, cores=1, kind="oracle", sample=desc)
     print(json.dumps(line))

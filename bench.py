@@ -247,6 +247,33 @@ def run_ours(args):
         ev_f += int(torch.where(sat, nl, L).sum().item())
         ev_b += int(nl.sum().item())
 
+    # next step after the hot path (not part of the step): Interp_H of Eq.7 to the camera image and its adjoint,
+    # timed on view 0's HEALPix image.  Camera: the paper's case for this grid where there is no mask (6080 x 3040 panorama ->
+    # Nside 1024, Table 5), else a 1920 x 1080 pinhole of 60 x 45 degrees (config 5's frustum).
+    extras = {}
+    try:
+        cam = B.Camera("equirect", 6080, 3040) if mask.active_tiles is None else B.Camera("pinhole", 1920, 1080, np.radians(60.0), np.radians(45.0))
+        img = r.color[0].contiguous()
+        o_img = torch.empty(cam.height, cam.width, 3, dtype=torch.float32, device="cuda")
+        g_img = torch.randn(cam.height, cam.width, 3, device="cuda")
+        gi = torch.empty_like(img)
+        tms = []
+        for fn in (lambda: B.uts_resample_fwd(cfg, cam, mask, img, o_img, None), lambda: B.uts_resample_bwd(cfg, cam, mask, g_img, gi)):
+            for _ in range(3):
+                fn()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(5):
+                fn()
+            e1.record(); torch.cuda.synchronize()
+            tms.append(e0.elapsed_time(e1) / 5)
+        byts = cam.width * cam.height * 12 + img.numel() * 4
+        extras["resample"] = dict(camera=f"{cam.model} {cam.width}x{cam.height}", fwd_ms=tms[0], bwd_ms=tms[1], fwd_gbs=byts / (tms[0] * 1e-3) / 1e9,
+                                  bwd_gbs=(byts + img.numel() * 4) / (tms[1] * 1e-3) / 1e9, bytes_model="12 B per image pixel + 12 B per HEALPix pixel (+ its zero-fill in the adjoint)")
+        del o_img, g_img, gi, img
+    except Exception as e:      # measurement plumbing only; never hides a failure of the step itself
+        extras["resample"] = dict(error=str(e))
+
     # end to end through the C ABI with HOST buffers (H2D + D2H inside the timed region)
     h = {k: torch.from_numpy(scene[k]).contiguous().pin_memory() for k in ("means", "scales", "quats", "opac", "sh", "W", "b")}
     hg = gcol.cpu().pin_memory()
@@ -323,7 +350,7 @@ def run_ours(args):
                             l2="inputs larger than L2 (Gaussians 472 MB, pairs GBs); no flush needed"),
                 ms_forward=ms_fwd, ms_forward_backward=ms_step, stage_ms=stage_ms, per_kernel=per_kernel,
                 evaluated_pairs=dict(forward=ev_f, backward=ev_b),
-                roofline=roof, clocks=clocks,
+                roofline=roof, clocks=clocks, extras=extras,
                 e2e=dict(value=replicas.aggregate_throughput(n_pix_active, e2e_ms_max, world), unit=UNIT, ms_per_step=e2e_ms_max, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h),
                 gpu_launches=0)
     # launches of our kernels per step: 1 preprocess + (1 count + 3 scan + 1 emit) + passes*(1 + 3 + 1) (+1 copy) + 1 ranges + 1 fwd + 1 bwd + 1 pre-bwd

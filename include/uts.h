@@ -176,6 +176,30 @@ int uts_preprocess_bwd(const uts_config* cfg, uts_gaussians g, uts_views views, 
 int uts_build_mask(const uts_config* cfg, int kind, const double* h_params, uint32_t* pixel_mask_bits,
                    int32_t* slot_of_tile, uint32_t* active_tiles, int* h_n_active, void* stream);
 
+/* ------------------------------------------------------------------- image synthesis */
+
+/* Camera models of PAPER.md:477-515.  Principal point (W/2, H/2).  UTS_CAM_PINHOLE: p0, p1 = FoV_x, FoV_y in radians,
+ * f_x = W / (2 tan(FoV_x / 2)) (Eq.11).  UTS_CAM_FISHEYE: anisotropic equidistant, p0, p1 = w_x, w_y = FoV / 180 deg,
+ * f_x = W / pi, f_y = H / pi, valid domain = the ellipse of Eq.14-15 (Eq.12-13).  UTS_CAM_EQUIRECT: omega = 2 pi u / W - pi,
+ * phi = pi/2 - pi v / H.  The camera frame is the one of uts_views (t = W mu + b): +z forward, polar axis +y. */
+enum { UTS_CAM_PINHOLE = 0, UTS_CAM_FISHEYE = 1, UTS_CAM_EQUIRECT = 2 };
+typedef struct { int model; int width, height; double p0, p1; } uts_camera;
+
+/* I_C(u,v) = Interp_H(I_H, P_C(u,v)) for (u,v) in D_C (Eq.7).  image [S*256, channels] fp32 in the slot layout
+ * of uts_render_fwd (one view); out [H, W, channels] row-major, 0 outside D_C; valid [H, W] = 1 inside D_C (may be NULL).
+ * Interp_H is the HEALPix ring-bilinear interpolation (reading A26); samples with M_C = 0 are dropped and the weights
+ * renormalised (A27); pixel (i,j) is sampled at (i + 1/2, j + 1/2) (A28).  1 <= channels <= 16. */
+int uts_resample_fwd(const uts_config* cfg, uts_camera cam, uts_mask mask, const float* image, int channels, float* out,
+                     uint8_t* valid, void* stream);
+/* Adjoint of uts_resample_fwd: dL_dimage [S*256, channels] is zeroed by the call, then accumulated with atomics
+ * (summation order is not deterministic).  dL_dout [H, W, channels]. */
+int uts_resample_bwd(const uts_config* cfg, uts_camera cam, uts_mask mask, const float* dL_dout, int channels, float* dL_dimage,
+                     void* stream);
+/* M_C(q) = 1[Pi_C^{-1}(s_q) in D_C] (Eq.9) from the camera intrinsics; outputs as uts_build_mask.
+ * Synchronises `stream` and writes n_active to *h_n_active. */
+int uts_build_camera_mask(const uts_config* cfg, uts_camera cam, uint32_t* pixel_mask_bits, int32_t* slot_of_tile,
+                          uint32_t* active_tiles, int* h_n_active, void* stream);
+
 /* NESTED pixel centres as camera-frame unit vectors, double [n,3], pixels first..first+n-1 at `order`
  * (exposes the library's HEALPix indexing for tests). */
 int uts_pixel_centers(int order, uint64_t first, uint64_t n, double* out_xyz, void* stream);

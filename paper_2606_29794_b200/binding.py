@@ -21,7 +21,7 @@ UTS_OK, UTS_ERR_INVALID_ARG, UTS_ERR_CAPACITY, UTS_ERR_CUDA, UTS_ERR_UNSUPPORTED
 SYMBOLS = [
     "uts_preprocess", "uts_depth_order", "uts_depth_order_scratch_bytes", "uts_tile_query", "uts_tile_query_scratch_bytes", "uts_sort", "uts_sort_scratch_bytes",
     "uts_tile_ranges", "uts_render_fwd", "uts_render_bwd", "uts_preprocess_bwd", "uts_build_mask", "uts_pixel_centers",
-    "uts_rho_max_table", "uts_host_workspace_bytes", "uts_host_forward_backward", "uts_last_cuda_error", "uts_strerror",
+    "uts_rho_max_table", "uts_resample_fwd", "uts_resample_bwd", "uts_build_camera_mask", "uts_host_workspace_bytes", "uts_host_forward_backward", "uts_last_cuda_error", "uts_strerror",
     "uts_version",
 ]
 
@@ -51,6 +51,10 @@ class CViews(C.Structure):
 
 class CProj(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in ("dir", "lonlat", "rho", "conic_opac", "rs", "rgb", "flags")]
+
+
+class CCamera(C.Structure):
+    _fields_ = [("model", C.c_int), ("width", C.c_int), ("height", C.c_int), ("p0", C.c_double), ("p1", C.c_double)]
 
 
 class CMask(C.Structure):
@@ -266,6 +270,50 @@ def uts_build_mask(cfg: Config, kind: str, params, device="cuda", stream=None) -
     n = C.c_int(0)
     _check(lib().uts_build_mask(C.byref(c), C.c_int(0 if kind == "cap" else 1), prm, _ptr(bits), _ptr(slot), _ptr(act), C.byref(n),
                                 _stream(stream)), "uts_build_mask")
+    return Mask(act[: n.value].contiguous(), int(n.value), slot, bits)
+
+
+CAMERA_MODELS = {"pinhole": 0, "fisheye": 1, "equirect": 2}
+
+
+@dataclass
+class Camera:
+    """PAPER.md:477-515.  'pinhole': p0, p1 = FoV_x, FoV_y (radians); 'fisheye': p0, p1 = w_x, w_y (Eq.12); 'equirect'."""
+    model: str
+    width: int
+    height: int
+    p0: float = 0.0
+    p1: float = 0.0
+
+    def c(self): return CCamera(CAMERA_MODELS[self.model], self.width, self.height, float(self.p0), float(self.p1))
+
+
+def uts_resample_fwd(cfg: Config, cam: Camera, mask: Mask, image, out, valid=None, stream=None):
+    """image [S*256, C] -> out [H, W, C] (Eq.7); valid [H, W] uint8 or None."""
+    c = cfg.c()
+    ch = int(image.shape[-1])
+    assert image.shape[0] == mask.n_slots(cfg) * 256 and tuple(out.shape) == (cam.height, cam.width, ch)
+    _check(lib().uts_resample_fwd(C.byref(c), cam.c(), mask.c(), _ptr(image, torch.float32), C.c_int(ch), _ptr(out, torch.float32),
+                                  _ptr(valid, torch.uint8), _stream(stream)), "uts_resample_fwd")
+
+
+def uts_resample_bwd(cfg: Config, cam: Camera, mask: Mask, dL_dout, dL_dimage, stream=None):
+    c = cfg.c()
+    ch = int(dL_dout.shape[-1])
+    assert dL_dimage.shape[0] == mask.n_slots(cfg) * 256 and int(dL_dimage.shape[-1]) == ch
+    _check(lib().uts_resample_bwd(C.byref(c), cam.c(), mask.c(), _ptr(dL_dout, torch.float32), C.c_int(ch), _ptr(dL_dimage, torch.float32),
+                                  _stream(stream)), "uts_resample_bwd")
+
+
+def uts_build_camera_mask(cfg: Config, cam: Camera, device="cuda", stream=None) -> Mask:
+    """M_C of Eq.9 from the camera intrinsics."""
+    c = cfg.c()
+    bits = torch.empty(cfg.n_pix // 32, dtype=torch.int32, device=device)
+    slot = torch.empty(cfg.n_tiles, dtype=torch.int32, device=device)
+    act = torch.empty(cfg.n_tiles, dtype=torch.int32, device=device)
+    n = C.c_int(0)
+    _check(lib().uts_build_camera_mask(C.byref(c), cam.c(), _ptr(bits), _ptr(slot), _ptr(act), C.byref(n), _stream(stream)),
+           "uts_build_camera_mask")
     return Mask(act[: n.value].contiguous(), int(n.value), slot, bits)
 
 

@@ -131,6 +131,18 @@ __global__ void mask_tiles_kernel(const uint32_t* __restrict__ bits, int64_t n_t
   if (threadIdx.x == 0) *n_active_out = base;
 }
 
+// active-tile list and slot table of a pixel bitmap (shared by uts_build_mask and uts_build_camera_mask); synchronises s
+int build_mask_tiles(const Dims& d, uint32_t* pixel_mask_bits, int32_t* slot_of_tile, uint32_t* active_tiles, int* h_n_active, cudaStream_t s) {
+  int* d_count = nullptr;   // 4 library-private bytes, freed below; this call is not on the per-frame path
+  UTS_CUDA(cudaMallocAsync((void**)&d_count, sizeof(int), s));
+  mask_tiles_kernel<<<1, 1024, 0, s>>>(pixel_mask_bits, d.n_tile, slot_of_tile, active_tiles, d_count);
+  UTS_LAUNCH_CHECK();
+  UTS_CUDA(cudaMemcpyAsync(h_n_active, d_count, sizeof(int), cudaMemcpyDeviceToHost, s));
+  UTS_CUDA(cudaFreeAsync(d_count, s));
+  UTS_CUDA(cudaStreamSynchronize(s));
+  return UTS_OK;
+}
+
 }  // namespace uts
 
 using namespace uts;
@@ -183,14 +195,7 @@ int uts_build_mask(const uts_config* cfg, int kind, const double* h_params, uint
   const uint64_t n_words = (uint64_t)d.n_pix / 32;
   mask_bits_kernel<<<(unsigned)((n_words + 255) / 256), 256, 0, s>>>(d.k, mp, pixel_mask_bits, n_words);
   UTS_LAUNCH_CHECK();
-  int* d_count = nullptr;   // 4 library-private bytes, freed below; this call is not on the per-frame path
-  UTS_CUDA(cudaMallocAsync((void**)&d_count, sizeof(int), s));
-  mask_tiles_kernel<<<1, 1024, 0, s>>>(pixel_mask_bits, d.n_tile, slot_of_tile, active_tiles, d_count);
-  UTS_LAUNCH_CHECK();
-  UTS_CUDA(cudaMemcpyAsync(h_n_active, d_count, sizeof(int), cudaMemcpyDeviceToHost, s));
-  UTS_CUDA(cudaFreeAsync(d_count, s));
-  UTS_CUDA(cudaStreamSynchronize(s));
-  return UTS_OK;
+  return build_mask_tiles(d, pixel_mask_bits, slot_of_tile, active_tiles, h_n_active, s);
 }
 
 }  // extern "C"

@@ -16,7 +16,7 @@ from dataclasses import dataclass, field
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SRCS = ["orc_healpix.cpp", "orc_raster.cpp", "orc_resample.cpp", "orc_capi.cpp"]
+_SRCS = ["orc_healpix.cpp", "orc_raster.cpp", "orc_resample.cpp", "orc_depth.cpp", "orc_capi.cpp"]
 _HDRS = ["orc_healpix.hpp", "orc_raster.hpp", "orc_resample.hpp"]
 _LIB = os.path.join(_HERE, "liboracle.so")
 
@@ -230,6 +230,35 @@ def camera_mask_bits(order, cam: Camera):
     bits = np.zeros((n + 31) // 32, np.uint32)
     lib().orc_camera_mask(C.c_int(order), *cam.args(), _p(bits))
     return bits
+
+
+# ------------------------------------------------------------------ inverse radial depth, r_s,max (orc_depth.cpp)
+def inv_depth_channel(rho, flags=None):
+    """rho [V,P] fp32 -> per-Gaussian channel [V,P,3] = (1/rho, 0, 0), to be blended in place of the colour (reading A29)."""
+    r = _f32(rho); V, P = r.shape
+    fl = None if flags is None else np.ascontiguousarray(flags, dtype=np.uint8)
+    out = np.zeros((V, P, 3), np.float32)
+    lib().orc_inv_depth_channel(C.c_int(V), C.c_int(P), _p(r), _p(fl), _p(out))
+    return out
+
+
+def inv_depth_bwd(means, W, b, dL_dinv, flags=None):
+    """dL/dmeans [P,3] of sum_v,i dL_dinv[v,i] / ||W_v mu_i + b_v||."""
+    m, Wf, bf, g = _f32(means), _f32(W), _f32(b), _f64(dL_dinv)
+    V, P = g.shape
+    fl = None if flags is None else np.ascontiguousarray(flags, dtype=np.uint8)
+    out = np.zeros((P, 3))
+    lib().orc_inv_depth_bwd(C.c_int(V), C.c_int(P), _p(m), _p(Wf), _p(bf), _p(fl), _p(g), _p(out))
+    return out
+
+
+def rs_max_update(rs, flags, rs_max):
+    """r_s,max <- max(r_s,max, r_s) for visible Gaussians; returns the updated copy."""
+    r = _f32(rs); V, P = r.shape
+    fl = None if flags is None else np.ascontiguousarray(flags, dtype=np.uint8)
+    out = _f32(rs_max).copy()
+    lib().orc_rs_max_update(C.c_int(V), C.c_int(P), _p(r), _p(fl), _p(out))
+    return out
 
 
 # ------------------------------------------------------------------ stages (fp32 ABI arrays)

@@ -200,6 +200,21 @@ int uts_resample_bwd(const uts_config* cfg, uts_camera cam, uts_mask mask, const
 int uts_build_camera_mask(const uts_config* cfg, uts_camera cam, uint32_t* pixel_mask_bits, int32_t* slot_of_tile,
                           uint32_t* active_tiles, int* h_n_active, void* stream);
 
+/* ------------------------------------------------- inverse radial depth, r_s,max */
+
+/* Per-Gaussian channel of the inverse radial depth image (reading A29: D = Eq.6 with c_i = 1 / r_i):
+ * chan [V,P,3] = (1 / rho, 0, 0), culled Gaussians 0.  Use it as `uts_proj.rgb` of uts_render_fwd (bg = 0): color[...,0] is the
+ * depth image; uts_render_bwd on the same record with dL_dcolor = (dL/dD, 0, 0) returns dL/d(1/r_i) in dL_drgb[...,0] and the
+ * depth loss's share of dL_dconic / dL_dmu2 / dL_dopac. */
+int uts_inv_depth_channel(const uts_config* cfg, const float* rho, const uint8_t* flags, float* chan, void* stream);
+/* d(1/r)/dt = -t / r^3 carried to the means: dL_dmeans [P,3] (+)= sum_v W_v^T (-t / r^3) dL_dchan[v,i,0].
+ * accumulate != 0 adds to dL_dmeans (after uts_preprocess_bwd), 0 overwrites. */
+int uts_inv_depth_bwd(const uts_config* cfg, const float* means, uts_views views, const uint8_t* flags, const float* dL_dchan,
+                      int accumulate, float* dL_dmeans, void* stream);
+/* Radian-space density control buffer: rs_max[i] <- max(rs_max[i], rs[v,i]) over the views in which Gaussian i
+ * is visible (not culled by uts_preprocess).  rs, flags: uts_preprocess's records; rs_max [P], caller-initialised. */
+int uts_rs_max_update(const uts_config* cfg, const float* rs, const uint8_t* flags, float* rs_max, void* stream);
+
 /* NESTED pixel centres as camera-frame unit vectors, double [n,3], pixels first..first+n-1 at `order`
  * (exposes the library's HEALPix indexing for tests). */
 int uts_pixel_centers(int order, uint64_t first, uint64_t n, double* out_xyz, void* stream);

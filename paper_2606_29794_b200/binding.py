@@ -21,7 +21,8 @@ UTS_OK, UTS_ERR_INVALID_ARG, UTS_ERR_CAPACITY, UTS_ERR_CUDA, UTS_ERR_UNSUPPORTED
 SYMBOLS = [
     "uts_preprocess", "uts_depth_order", "uts_depth_order_scratch_bytes", "uts_tile_query", "uts_tile_query_scratch_bytes", "uts_sort", "uts_sort_scratch_bytes",
     "uts_tile_ranges", "uts_render_fwd", "uts_render_bwd", "uts_preprocess_bwd", "uts_build_mask", "uts_pixel_centers",
-    "uts_rho_max_table", "uts_resample_fwd", "uts_resample_bwd", "uts_build_camera_mask", "uts_host_workspace_bytes", "uts_host_forward_backward", "uts_last_cuda_error", "uts_strerror",
+    "uts_rho_max_table", "uts_resample_fwd", "uts_resample_bwd", "uts_build_camera_mask", "uts_inv_depth_channel", "uts_inv_depth_bwd", "uts_rs_max_update",
+    "uts_host_workspace_bytes", "uts_host_forward_backward", "uts_last_cuda_error", "uts_strerror",
     "uts_version",
 ]
 
@@ -271,6 +272,24 @@ def uts_build_mask(cfg: Config, kind: str, params, device="cuda", stream=None) -
     _check(lib().uts_build_mask(C.byref(c), C.c_int(0 if kind == "cap" else 1), prm, _ptr(bits), _ptr(slot), _ptr(act), C.byref(n),
                                 _stream(stream)), "uts_build_mask")
     return Mask(act[: n.value].contiguous(), int(n.value), slot, bits)
+
+
+def uts_inv_depth_channel(cfg: Config, rho, flags, chan, stream=None):
+    c = cfg.c()
+    _check(lib().uts_inv_depth_channel(C.byref(c), _ptr(rho, torch.float32), _ptr(flags, torch.uint8), _ptr(chan, torch.float32), _stream(stream)),
+           "uts_inv_depth_channel")
+
+
+def uts_inv_depth_bwd(cfg: Config, means, views: Views, flags, dL_dchan, dL_dmeans, accumulate=True, stream=None):
+    c = cfg.c()
+    _check(lib().uts_inv_depth_bwd(C.byref(c), _ptr(means, torch.float32), views.c(), _ptr(flags, torch.uint8), _ptr(dL_dchan, torch.float32),
+                                   C.c_int(1 if accumulate else 0), _ptr(dL_dmeans, torch.float32), _stream(stream)), "uts_inv_depth_bwd")
+
+
+def uts_rs_max_update(cfg: Config, rs, flags, rs_max, stream=None):
+    c = cfg.c()
+    _check(lib().uts_rs_max_update(C.byref(c), _ptr(rs, torch.float32), _ptr(flags, torch.uint8), _ptr(rs_max, torch.float32), _stream(stream)),
+           "uts_rs_max_update")
 
 
 CAMERA_MODELS = {"pinhole": 0, "fisheye": 1, "equirect": 2}

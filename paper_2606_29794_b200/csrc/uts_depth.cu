@@ -1,0 +1,96 @@
+// uts_depth.cu — inverse radial depth channel and the r_s,max buffer.
+//   "For depth supervision, we use inverse radial depth r^-1, whose gradient is d r^-1/dt = -t / r^3"
+//   "r_s,max <- max(r_s,max, r_s) whenever the Gaussian is visible"
+// Reading A29: the depth image is Eq.6 with the colour c_i replaced by r_i^-1.  The blend kernels take the per-Gaussian value to
+// composite from `uts_proj.rgb`, so the depth image is uts_render_fwd on a record whose rgb is the channel (r^-1, 0, 0) built
+// here, and uts_render_bwd on the same record returns dL/d(r_i^-1) in dL_drgb[..., 0] together with the alpha-path terms of the
+// depth loss (dL_dconic, dL_dmu2, dL_dopac), which add to those of the colour loss.  uts_inv_depth_bwd then carries dL/d(r^-1)
+// to the means.  Streaming kernels, one thread per (view, Gaussian) or per Gaussian.
+#include "uts_internal.cuh"
+
+namespace uts {
+
+__global__ void inv_depth_channel_kernel(int64_t n, const float* __restrict__ rho, const uint8_t* __restrict__ flags, float* __restrict__ chan) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  const bool culled = (__ldg(flags + k) & 1) != 0;
+  chan[3 * k] = culled ? 0.f : __fdiv_rn(1.0f, __ldg(rho + k));
+  chan[3 * k + 1] = 0.f; chan[3 * k + 2] = 0.f;
+}
+
+// one thread per Gaussian, views summed in registers; double like the geometry chain of the preprocess
+__global__ void inv_depth_bwd_kernel(int P, int V, const float* __restrict__ means, const float* __restrict__ Wv, const float* __restrict__ bv,
+                                     const uint8_t* __restrict__ flags, const float* __restrict__ dL_dchan, int accumulate,
+                                     float* __restrict__ dL_dmeans) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= P) return;
+  const double mx = __ldg(means + 3 * i), my = __ldg(means + 3 * i + 1), mz = __ldg(means + 3 * i + 2);
+  double gx = 0.0, gy = 0.0, gz = 0.0;
+  for (int v = 0; v < V; ++v) {
+    const int64_t k = (int64_t)v * P + i;
+    if (__ldg(flags + k) & 1) continue;
+    const float* W = Wv + 9 * v; const float* b = bv + 3 * v;
+    const double tx = (double)W[0] * mx + (double)W[1] * my + (double)W[2] * mz + (double)b[0];
+    const double ty = (double)W[3] * mx + (double)W[4] * my + (double)W[5] * mz + (double)b[1];
+    const double tz = (double)W[6] * mx + (double)W[7] * my + (double)W[8] * mz + (double)b[2];
+    const double r2 = tx * tx + ty * ty + tz * tz;
+    const double s = -(double)__ldg(dL_dchan + 3 * k) / (r2 * sqrt(r2));      // dL/d(r^-1) * (-1/r^3)
+    gx += s * ((double)W[0] * tx + (double)W[3] * ty + (double)W[6] * tz);    // W^T (s t)
+    gy += s * ((double)W[1] * tx + (double)W[4] * ty + (double)W[7] * tz);
+    gz += s * ((double)W[2] * tx + (double)W[5] * ty + (double)W[8] * tz);
+  }
+  if (accumulate) { dL_dmeans[3 * i] += (float)gx; dL_dmeans[3 * i + 1] += (float)gy; dL_dmeans[3 * i + 2] += (float)gz; }
+  else { dL_dmeans[3 * i] = (float)gx; dL_dmeans[3 * i + 1] = (float)gy; dL_dmeans[3 * i + 2] = (float)gz; }
+}
+
+__global__ void rs_max_kernel(int P, int V, const float* __restrict__ rs, const uint8_t* __restrict__ flags, float* __restrict__ rs_max) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= P) return;
+  float m = rs_max[i];
+  for (int v = 0; v < V; ++v) {
+    const int64_t k = (int64_t)v * P + i;
+    if (!(__ldg(flags + k) & 1)) m = fmaxf(m, __ldg(rs + k));
+  }
+  rs_max[i] = m;
+}
+
+}  // namespace uts
+
+using namespace uts;
+
+extern "C" {
+
+int uts_inv_depth_channel(const uts_config* cfg, const float* rho, const uint8_t* flags, float* chan, void* stream) {
+  int st = check_config(cfg);
+  if (st) return st;
+  const int64_t n = (int64_t)cfg->n_gauss * cfg->n_views;
+  if (n == 0) return UTS_OK;
+  if (!rho || !flags || !chan) return UTS_ERR_INVALID_ARG;
+  inv_depth_channel_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(n, rho, flags, chan);
+  UTS_LAUNCH_CHECK();
+  return UTS_OK;
+}
+
+int uts_inv_depth_bwd(const uts_config* cfg, const float* means, uts_views views, const uint8_t* flags, const float* dL_dchan,
+                      int accumulate, float* dL_dmeans, void* stream) {
+  int st = check_config(cfg);
+  if (st) return st;
+  if (cfg->n_gauss == 0) return UTS_OK;
+  if (!means || !views.W || !views.b || !flags || !dL_dchan || !dL_dmeans) return UTS_ERR_INVALID_ARG;
+  inv_depth_bwd_kernel<<<(unsigned)((cfg->n_gauss + 255) / 256), 256, 0, (cudaStream_t)stream>>>(cfg->n_gauss, cfg->n_views, means, views.W, views.b,
+                                                                                               flags, dL_dchan, accumulate, dL_dmeans);
+  UTS_LAUNCH_CHECK();
+  return UTS_OK;
+}
+
+int uts_rs_max_update(const uts_config* cfg, const float* rs, const uint8_t* flags, float* rs_max, void* stream) {
+  int st = check_config(cfg);
+  if (st) return st;
+  if (cfg->n_gauss == 0) return UTS_OK;
+  if (!rs || !flags || !rs_max) return UTS_ERR_INVALID_ARG;
+  rs_max_kernel<<<(unsigned)((cfg->n_gauss + 255) / 256), 256, 0, (cudaStream_t)stream>>>(cfg->n_gauss, cfg->n_views, rs, flags, rs_max);
+  UTS_LAUNCH_CHECK();
+  return UTS_OK;
+}
+
+}  // extern "C"

@@ -27,7 +27,9 @@ from paper_2606_29794_b200 import scenes  # noqa: E402  (input generator: no met
 
 METRIC = "healpix_px_per_s_fwd_bwd"
 UNIT = "px/s"
-STAGES = ["preprocess", "depth_order", "tile_query", "sort", "tile_ranges", "render_fwd", "render_bwd", "preprocess_bwd"]
+# default: Alg.1 l.9-16 through uts_tile_lists (one call); --lists staged times uts_tile_query / uts_sort / uts_tile_ranges one by one
+STAGES_FUSED = ["preprocess", "depth_order", "tile_lists", "render_fwd", "render_bwd", "preprocess_bwd"]
+STAGES_STAGED = ["preprocess", "depth_order", "tile_query", "sort", "tile_ranges", "render_fwd", "render_bwd", "preprocess_bwd"]
 # FP32 operations one evaluated (Gaussian, pixel) pair costs in the blend kernels (counted from the
 # arithmetic of Eq.6 + SphericalOffset as implemented, FMA = 2): forward 46, backward 118.
 FLOP_FWD, FLOP_BWD = 46, 118
@@ -194,7 +196,10 @@ def run_ours(args):
     cfg = R.config_of(scene)
     mask = B.Mask.full() if scene["mask"] is None else B.uts_build_mask(cfg, scene["mask"]["kind"], scene["mask"]["params"])
     g, views = R.scene_to_device(scene)
-    r = R.Rasterizer(cfg, mask)
+    fused = args.lists == "fused"
+    STAGES = STAGES_FUSED if fused else STAGES_STAGED
+    NS = len(STAGES)
+    r = R.Rasterizer(cfg, mask, fused_lists=fused)
     V, S = cfg.n_views, r.S
     npx = S * cfg.ppt
     gcol = torch.from_numpy(scenes.upstream_grad(V, npx, seed=rank)).cuda()
@@ -208,13 +213,18 @@ def run_ours(args):
                 events[i].record(stream)
         mark(0); r.preprocess(g, views)
         mark(1); r.depth_order()
-        mark(2); r.tile_query()
-        mark(3); r.sort()
-        mark(4); r.tile_ranges()
-        mark(5); r.render_fwd()
-        mark(6); r.render_bwd(gcol)
-        mark(7); r.preprocess_bwd(g, views)
-        mark(8)
+        if fused:
+            mark(2); r.tile_lists()
+            i = 3
+        else:
+            mark(2); r.tile_query()
+            mark(3); r.sort()
+            mark(4); r.tile_ranges()
+            i = 5
+        mark(i); r.render_fwd()
+        mark(i + 1); r.render_bwd(gcol)
+        mark(i + 2); r.preprocess_bwd(g, views)
+        mark(i + 3)
 
     for _ in range(args.warmup):
         step()
@@ -222,19 +232,21 @@ def run_ours(args):
     if world > 1:
         dist.barrier()
     sampler = ClockSampler(local); sampler.start()
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(9)] for _ in range(args.steps)]
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(NS + 1)] for _ in range(args.steps)]
     t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
+    launches0 = B.uts_launch_count()
     t0.record(stream)
     for k in range(args.steps):
         step(ev[k])
     t1.record(stream)
     torch.cuda.synchronize()
+    launches = B.uts_launch_count() - launches0          # counted by the library itself, one tick per kernel launch
     clocks = sampler.stop()
     total_ms = t0.elapsed_time(t1)
     ms_step = total_ms / args.steps
-    stage_ms = {STAGES[i]: float(np.mean([ev[k][i].elapsed_time(ev[k][i + 1]) for k in range(args.steps)])) for i in range(8)}
-    ms_fwd = sum(stage_ms[s] for s in STAGES[:6])
+    stage_ms = {STAGES[i]: float(np.mean([ev[k][i].elapsed_time(ev[k][i + 1]) for k in range(args.steps)])) for i in range(NS)}
+    ms_fwd = sum(stage_ms[s] for s in STAGES[:NS - 2])
 
     # work counters from the forward outputs (measurement plumbing): entries each pixel evaluated
     lens = (r.ranges[:, 1] - r.ranges[:, 0])
@@ -318,7 +330,8 @@ def run_ours(args):
                 if w_ == f"config{args.config}":
                     traffic[st_] = int(by_)
     # dominant kernel and its roofline
-    dom = max(stage_ms, key=stage_ms.get)
+    # (uts_tile_lists is a call of about 25 kernels, the longest of them shorter than the forward blend: not a candidate)
+    dom = max((k_ for k_ in stage_ms if k_ != "tile_lists"), key=stage_ms.get)
     fp32_peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12       # TFLOP/s at the maximum SM clock
     if dom in ("render_fwd", "render_bwd"):
         flop = ev_f * FLOP_FWD if dom == "render_fwd" else ev_b * FLOP_BWD
@@ -339,26 +352,23 @@ def run_ours(args):
             per_kernel[s_] = dict(ms=ms, tflops=ev_b * FLOP_BWD / (ms * 1e-3) / 1e12, frac_fp32_peak=ev_b * FLOP_BWD / (ms * 1e-3) / 1e12 / fp32_peak)
         else:
             byts = {"preprocess": P * V * (44 + 12 * M + 57), "preprocess_bwd": P * (44 + 12 * M + V * 33 + 40 + 12 * M),
-                    "depth_order": P * V * (4 + 5 * 32 + 16), "tile_query": P * V * 2 * 29 + 8 * P * V + 12 * n_pairs, "sort": 32.0 * n_pairs * ((max(1, (V * cfg.n_tiles - 1)).bit_length() + 7) // 8),
+                    "depth_order": P * V * (4 + 5 * 32 + 16), "tile_query": P * V * 2 * 29 + 8 * P * V + 12 * n_pairs,
+                    "tile_lists": P * V * 2 * 29 + 12 * n_pairs + 16 * V * cfg.n_tiles,      # floor: every sorted pair written once
+                    "sort": 32.0 * n_pairs * ((max(1, (V * cfg.n_tiles - 1)).bit_length() + 7) // 8),
                     "tile_ranges": 8.0 * n_pairs + 16 * V * cfg.n_tiles}[s_]
             per_kernel[s_] = dict(ms=ms, gbs=byts / (ms * 1e-3) / 1e9, frac_hbm_peak=byts / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
 
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup, ms_per_step=ms_step_max,
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
                 config=dict(workload=f"config{args.config}:{scene['name']}", order=cfg.order, nside=1 << cfg.order, n_pix=n_pix_active,
-                            n_gauss=P, sh_degree=cfg.sh_degree, n_views=V, n_pairs=n_pairs, parallelism=f"replicas{world}",
+                            n_gauss=P, sh_degree=cfg.sh_degree, n_views=V, n_pairs=n_pairs, parallelism=f"replicas{world}", lists=args.lists,
                             l2="inputs larger than L2 (Gaussians 472 MB, pairs GBs); no flush needed"),
                 ms_forward=ms_fwd, ms_forward_backward=ms_step, stage_ms=stage_ms, per_kernel=per_kernel,
                 evaluated_pairs=dict(forward=ev_f, backward=ev_b),
                 roofline=roof, clocks=clocks, extras=extras,
                 e2e=dict(value=replicas.aggregate_throughput(n_pix_active, e2e_ms_max, world), unit=UNIT, ms_per_step=e2e_ms_max, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h),
                 gpu_launches=0)
-    # launches of our kernels per step: 1 preprocess + (1 count + 3 scan + 1 emit) + passes*(1 + 3 + 1) (+1 copy) + 1 ranges + 1 fwd + 1 bwd + 1 pre-bwd
-    passes = (max(1, (V * cfg.n_tiles - 1)).bit_length() + 7) // 8          # pair sort: (view,tile) bytes only
-    dpass = 4 + ((max(1, V - 1).bit_length() + 7) // 8 if V > 1 else 0)     # depth order of the Gaussians
-    # preprocess 1; depth order 1 + 5/pass (+copy) + 1; query 3 classify + 3 count + 3 scan + 3 emit; sort 5/pass (+copy);
-    # ranges 1; blend fwd 1; blend bwd 1; preprocess bwd 1
-    line["gpu_launches"] = args.steps * (1 + (2 + dpass * 5 + dpass % 2) + 12 + (passes * 5 + passes % 2) + 4)
+    line["gpu_launches"] = int(launches)                 # uts_launch_count() over the timed region
     if not args.no_cpu_baseline:
         smp = OracleSample(args.config, seed=0, n_pre=1_000_000, n_query=120_000, n_tiles_sample=384)   # about 10 s of oracle time on config 4
         t, desc = smp.step()
@@ -376,6 +386,8 @@ def main():
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config id 1..5 (default 4 = the metric's workload)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--lists", default="fused", choices=["fused", "staged"],
+                    help="Alg.1 l.9-16 as one uts_tile_lists call (default) or as uts_tile_query + uts_sort + uts_tile_ranges")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

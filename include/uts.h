@@ -130,6 +130,22 @@ size_t uts_depth_order_scratch_bytes(const uts_config* cfg);
 int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint32_t* emit_rank, uint64_t* offsets,
                    uint64_t* keys, uint32_t* vals, uint64_t capacity, uint64_t* h_n_pairs, void* scratch,
                    size_t scratch_bytes, void* stream);
+
+/* F2 + F3 + F4 in one call (Alg.1 l.9-16): the sorted pair arrays and the tile ranges, bit-identical to
+ *     uts_tile_query(emit_rank) -> uts_sort(depth_presorted = 1) -> uts_tile_ranges,
+ * without sending every pair through the sort.  Discs that cover many tiles (a radius class chosen so that one bitmap row over the
+ * tiles is cheaper than the disc's pairs through the radix sort) are recorded as rows of a (disc x tile) bit matrix in depth
+ * order; the matrix is transposed and every (view, tile) reads its list of large discs off its own bit vector, already grouped
+ * by tile and ordered by depth.  Only the remaining discs' pairs are emitted and radix-sorted; a per-tile merge of the two
+ * depth-ordered lists writes keys / vals.
+ * emit_rank: uts_depth_order's output (required).  keys, vals, keys_tmp, vals_tmp: `capacity` entries each; ranges [V*N_tile][2].
+ * The call synchronises `stream` once (pair counts) and writes the pair count to *h_n_pairs; if it exceeds `capacity` nothing is
+ * emitted and UTS_ERR_CAPACITY is returned.  scratch: uts_tile_lists_scratch_bytes(cfg) bytes, sort_scratch:
+ * uts_sort_scratch_bytes(capacity) bytes, both 256-byte aligned. */
+size_t uts_tile_lists_scratch_bytes(const uts_config* cfg);
+int uts_tile_lists(const uts_config* cfg, uts_proj in, uts_mask mask, const uint32_t* emit_rank, uint64_t* keys, uint32_t* vals,
+                   uint64_t* keys_tmp, uint32_t* vals_tmp, uint64_t capacity, uint64_t* ranges, uint64_t* h_n_pairs, void* scratch,
+                   size_t scratch_bytes, void* sort_scratch, size_t sort_scratch_bytes, void* stream);
 size_t uts_tile_query_scratch_bytes(const uts_config* cfg);
 
 /* Alg.1 l.15.  Stable ascending LSD radix sort on the 64-bit key (ties keep emission order; with emission in Gaussian-id
@@ -240,6 +256,9 @@ int uts_host_forward_backward(const uts_config* cfg, const float* h_means, const
                               void* stream);
 
 int         uts_last_cuda_error(void);
+/* Kernel launches this library has enqueued since it was loaded (all streams, all calls; memsets and copies not counted).
+ * bench.py reports the difference over its timed region as "gpu_launches". */
+uint64_t    uts_launch_count(void);
 const char* uts_strerror(int status);
 const char* uts_version(void);
 

@@ -19,10 +19,10 @@ UTS_OK, UTS_ERR_INVALID_ARG, UTS_ERR_CAPACITY, UTS_ERR_CUDA, UTS_ERR_UNSUPPORTED
 
 # every symbol include/uts.h declares
 SYMBOLS = [
-    "uts_preprocess", "uts_depth_order", "uts_depth_order_scratch_bytes", "uts_tile_query", "uts_tile_query_scratch_bytes", "uts_sort", "uts_sort_scratch_bytes",
+    "uts_preprocess", "uts_depth_order", "uts_depth_order_scratch_bytes", "uts_tile_query", "uts_tile_query_scratch_bytes", "uts_tile_lists", "uts_tile_lists_scratch_bytes", "uts_sort", "uts_sort_scratch_bytes",
     "uts_tile_ranges", "uts_render_fwd", "uts_render_bwd", "uts_preprocess_bwd", "uts_build_mask", "uts_pixel_centers",
     "uts_rho_max_table", "uts_resample_fwd", "uts_resample_bwd", "uts_build_camera_mask", "uts_inv_depth_channel", "uts_inv_depth_bwd", "uts_rs_max_update",
-    "uts_host_workspace_bytes", "uts_host_forward_backward", "uts_last_cuda_error", "uts_strerror",
+    "uts_host_workspace_bytes", "uts_host_forward_backward", "uts_last_cuda_error", "uts_launch_count", "uts_strerror",
     "uts_version",
 ]
 
@@ -216,6 +216,34 @@ def uts_tile_query(cfg: Config, proj: Proj, mask: Mask, offsets, keys, vals, cap
     if st == UTS_ERR_CAPACITY:
         e = UtsError(st, "uts_tile_query"); e.needed = int(n.value); raise e
     _check(st, "uts_tile_query")
+    return int(n.value)
+
+
+def uts_launch_count() -> int:
+    """Kernel launches enqueued by libuts.so since it was loaded."""
+    lib().uts_launch_count.restype = C.c_uint64
+    return int(lib().uts_launch_count())
+
+
+def uts_tile_lists_scratch_bytes(cfg: Config) -> int:
+    c = cfg.c()
+    lib().uts_tile_lists_scratch_bytes.restype = C.c_size_t
+    return int(lib().uts_tile_lists_scratch_bytes(C.byref(c)))
+
+
+def uts_tile_lists(cfg: Config, proj: Proj, mask: Mask, emit_rank, keys, vals, keys_tmp, vals_tmp, capacity: int, ranges, scratch, sort_scratch,
+                   stream=None) -> int:
+    """Sorted pairs + tile ranges in one call (see include/uts.h).  Returns the pair count; raises UtsError (status
+    UTS_ERR_CAPACITY, .needed = required capacity) when the buffers are too small."""
+    c = cfg.c()
+    n = C.c_uint64(0)
+    st = lib().uts_tile_lists(C.byref(c), proj.c(), mask.c(), _ptr(emit_rank), _ptr(keys), _ptr(vals), _ptr(keys_tmp), _ptr(vals_tmp),
+                              C.c_uint64(capacity), _ptr(ranges), C.byref(n), _ptr(scratch), C.c_size_t(scratch.numel() * scratch.element_size()),
+                              _ptr(sort_scratch), C.c_size_t(sort_scratch.numel() * sort_scratch.element_size()), _stream(stream))
+    if st == UTS_ERR_CAPACITY:
+        e = UtsError(st, "uts_tile_lists"); e.needed = int(n.value)
+        raise e
+    _check(st, "uts_tile_lists")
     return int(n.value)
 
 

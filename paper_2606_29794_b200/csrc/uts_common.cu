@@ -7,6 +7,8 @@ namespace uts {
 
 static std::atomic<int> g_last_cuda_error{0};
 void set_last_cuda_error(cudaError_t e) { g_last_cuda_error.store((int)e); }
+static std::atomic<unsigned long long> g_launches{0};
+void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
 
 int sm_count() {
   static int n = 0;
@@ -150,6 +152,7 @@ using namespace uts;
 extern "C" {
 
 int uts_last_cuda_error(void) { return g_last_cuda_error.load(); }
+uint64_t uts_launch_count(void) { return (uint64_t)g_launches.load(); }
 
 const char* uts_strerror(int s) {
   switch (s) {

@@ -40,7 +40,7 @@ static HostLayout layout(const uts_config* cfg, int64_t n_slot, uint64_t cap, ch
   L.proj.conic_opac = B.take<float>(4 * VP); L.proj.rs = B.take<float>(VP); L.proj.rgb = B.take<float>(3 * VP);
   L.proj.flags = B.take<uint8_t>(VP);
   L.offsets = B.take<uint64_t>(VP + 1);
-  L.tq_bytes = uts_tile_query_scratch_bytes(cfg); L.tq_scratch = B.take<char>(L.tq_bytes);
+  L.tq_bytes = uts_tile_lists_scratch_bytes(cfg); L.tq_scratch = B.take<char>(L.tq_bytes);
   L.do_bytes = uts_depth_order_scratch_bytes(cfg); L.do_scratch = B.take<char>(L.do_bytes);
   L.emit_rank = B.take<uint32_t>(VP);
   L.keys = B.take<uint64_t>(cap); L.keys_tmp = B.take<uint64_t>(cap);
@@ -114,11 +114,10 @@ int uts_host_forward_backward(const uts_config* cfg, const float* h_means, const
   uts_views vw{L.W, L.b};
   if ((st = uts_preprocess(cfg, g, vw, L.proj, stream))) return st;
   if ((st = uts_depth_order(cfg, L.proj.rho, L.emit_rank, L.do_scratch, L.do_bytes, stream))) return st;
-  if ((st = uts_tile_query(cfg, L.proj, mask, L.emit_rank, L.offsets, L.keys, L.vals, pair_capacity, h_n_pairs, L.tq_scratch, L.tq_bytes, stream)))
+  // Alg.1 l.9-16 in one call: sorted pairs + tile ranges (large discs through the bit matrix, the rest through emit + radix sort)
+  if ((st = uts_tile_lists(cfg, L.proj, mask, L.emit_rank, L.keys, L.vals, L.keys_tmp, L.vals_tmp, pair_capacity, L.ranges, h_n_pairs,
+                           L.tq_scratch, L.tq_bytes, L.sort_scratch, L.sort_bytes, stream)))
     return st;
-  const uint64_t n = *h_n_pairs;
-  if ((st = uts_sort(cfg, n, L.keys, L.vals, L.keys_tmp, L.vals_tmp, 1, L.sort_scratch, L.sort_bytes, stream))) return st;
-  if ((st = uts_tile_ranges(cfg, n, L.keys, L.ranges, stream))) return st;
   if ((st = uts_render_fwd(cfg, L.proj, mask, L.ranges, L.vals, L.color, L.alpha, L.trans, L.n_last, stream))) return st;
   UTS_CUDA(cudaEventRecord(ev_fwd, s));
   UTS_CUDA(cudaStreamWaitEvent(s2, ev_fwd, 0));

@@ -21,7 +21,8 @@ void set_last_cuda_error(cudaError_t e);
     cudaError_t e__ = (call);                                               \
     if (e__ != cudaSuccess) { ::uts::set_last_cuda_error(e__); return UTS_ERR_CUDA; } \
   } while (0)
-#define UTS_LAUNCH_CHECK() UTS_CUDA(cudaGetLastError())
+void count_launch();                     // uts_launch_count(): one tick per kernel launch of this library
+#define UTS_LAUNCH_CHECK() do { ::uts::count_launch(); UTS_CUDA(cudaGetLastError()); } while (0)
 
 int check_config(const uts_config* c);   // UTS_OK / UTS_ERR_INVALID_ARG / UTS_ERR_UNSUPPORTED
 int check_mask(const uts_config* c, const uts_mask& m);

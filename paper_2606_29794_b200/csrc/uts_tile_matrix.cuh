@@ -1,0 +1,342 @@
+// uts_tile_matrix.cuh — tile-major emission of the LARGE discs for uts_tile_lists (F2 + F3 + F4 in one call).
+//
+// Alg.1 l.9-16 emits ((tile, rho), i) pairs per Gaussian, sorts all of them and cuts the tile ranges.  On the
+// paper's kind of scene most pairs belong to a few large discs (config 4: 4 % of the Gaussians own 90 % of the 267 M pairs), and
+// for those the per-Gaussian view is the wrong way round: a disc that covers thousands of tiles is better described by ONE bit per
+// tile.  So the large discs (radius class chosen so that a bitmap row is cheaper than the disc's pairs through the radix sort) are
+// taken out of the pair stream:
+//   count     each large disc's tile set is written as a bitmap row of a (disc x tile) bit matrix, rows in (view, depth, id) order
+//   transpose 32 x 32 bit blocks -> one bit VECTOR over the large discs per (view, tile)
+//   emit      a warp per (view, tile) walks its bit vector: set bit r = disc r belongs to this tile's list.  The list comes out
+//             already grouped by tile and ordered by depth — no sort — with coalesced writes.
+// Only the small discs' pairs go through emit + radix sort; a per-tile merge of the two depth-ordered lists gives the final
+// arrays, bit-identical to uts_tile_query + uts_sort + uts_tile_ranges (tests compare both against the oracle).
+// Included by uts_tile_query.cu after its ring-query helpers.
+#pragma once
+
+namespace uts {
+
+struct MatView { uint32_t row_start, n_rows, W, pad; unsigned long long mt_base; };   // W: words of a tile's bit vector (multiple of 8)
+
+struct MatParams {
+  uint32_t* M;                     // [cap_rows][n_words] disc-major bitmaps
+  uint32_t* MT;                    // view v: [n_tile][W_v] at views[v].mt_base
+  unsigned long long* row_key;     // [cap_rows] (depth bits << 32) | Gaussian id
+  const uint64_t* row_of_rank;     // [V*P + 1] exclusive scan of the large-disc flags in (view, depth, id) order
+  MatView* views;                  // [V]
+  uint32_t* large_count;           // [V * n_tile] large discs per (view, tile)
+  unsigned long long* n_L;         // total number of matrix pairs
+  int n_words;                     // n_tile / 32
+};
+
+// after the call: x[b] bit i == x_in[i] bit b
+__device__ __forceinline__ void transpose32(uint32_t (&x)[32]) {
+#pragma unroll
+  for (int s = 0; s < 5; ++s) {
+    const int j = 16 >> s;
+    const uint32_t m = j == 16 ? 0x0000ffffu : j == 8 ? 0x00ff00ffu : j == 4 ? 0x0f0f0f0fu : j == 2 ? 0x33333333u : 0x55555555u;
+#pragma unroll
+    for (int k = 0; k < 32; ++k) {
+      if ((k & j) == 0) {
+        const uint32_t t = ((x[k] >> j) ^ x[k + j]) & m;
+        x[k] ^= (t << j); x[k + j] ^= t;
+      }
+    }
+  }
+}
+
+// flag_by_rank[emit_rank[k]] = 1 for the large discs perm[0 .. n_mat)
+__global__ void mat_flag_kernel(const uint32_t* __restrict__ perm, const uint32_t* __restrict__ n_small, const uint32_t* __restrict__ emit_rank,
+                                uint32_t* __restrict__ flag_by_rank) {
+  const uint32_t n_mat = n_small[3];
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_mat; i += gridDim.x * blockDim.x) flag_by_rank[emit_rank[perm[i]]] = 1u;
+}
+
+// per view: its rows, the width of its bit vectors and where they start
+__global__ void mat_view_tab_kernel(MatParams mp, int P, int V, int64_t n_tile) {
+  if (threadIdx.x || blockIdx.x) return;
+  unsigned long long base = 0;
+  for (int v = 0; v < V; ++v) {
+    MatView mv;
+    mv.row_start = (uint32_t)mp.row_of_rank[(int64_t)v * P];
+    mv.n_rows = (uint32_t)mp.row_of_rank[(int64_t)(v + 1) * P] - mv.row_start;
+    mv.W = ((mv.n_rows + 255u) >> 8) << 3;
+    mv.pad = 0; mv.mt_base = base;
+    base += (unsigned long long)n_tile * mv.W;
+    mp.views[v] = mv;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------- count: bitmap rows
+__global__ void __launch_bounds__(kLargeThreads, 4)
+matrix_count_kernel(QueryParams qp, MatParams mp, const float* __restrict__ dir, const float* __restrict__ lonlat, const float* __restrict__ rho,
+                    const float* __restrict__ rs, const int32_t* __restrict__ slot_of_tile, const uint32_t* __restrict__ active_words,
+                    const uint32_t* __restrict__ perm, const uint32_t* __restrict__ n_small, const uint32_t* __restrict__ emit_rank,
+                    uint32_t* __restrict__ counts) {
+  extern __shared__ int2 ring_tab[];                 // [rc_block], then the bitmap [n_words]
+  uint32_t* bitmap = reinterpret_cast<uint32_t*>(ring_tab + qp.rc_block);
+  __shared__ RingDisc s_disc;
+  __shared__ uint16_t s_pre[13];
+  __shared__ int s_Slo[12];
+  __shared__ uint32_t s_total;
+  const uint32_t end = n_small[3];
+  const int N = 1 << qp.kq, tid = threadIdx.x;
+  for (uint32_t idx = blockIdx.x; idx < end; idx += gridDim.x) {
+    const int64_t k = (int64_t)perm[idx];
+    const int64_t slot = (int64_t)emit_rank[k];
+    const uint32_t row = (uint32_t)mp.row_of_rank[slot];
+    const int v = (int)(k / qp.P);
+    __syncthreads();                                   // the previous disc is done with shared memory
+    for (int w = tid; w < mp.n_words; w += kLargeThreads) bitmap[w] = 0u;
+    if (tid < 32) {                                    // set-up by the first warp: lane 0 the disc, lanes 0..11 one face each
+      if (tid == 0) {
+        load_ring_disc(qp, dir, lonlat, rs, k, s_disc);
+        s_disc.i_hi = min(s_disc.i_hi, s_disc.i_lo + qp.rc_block - 1);
+        s_total = 0;
+      }
+      __syncwarp();
+      int nrows = 0, S_lo = 0, S_hi = -1;
+      if (tid < 12 && face_in_extent(s_disc, tid)) { face_row_range(s_disc, qp.kq, qp.kt, tid, S_lo, S_hi); if (S_hi >= S_lo) nrows = S_hi - S_lo + 1; }
+      int incl = nrows;
+#pragma unroll
+      for (int dd = 1; dd < 16; dd <<= 1) { const int y = __shfl_up_sync(0xffffffffu, incl, dd); if (tid >= dd) incl += y; }
+      if (tid < 12) { s_pre[tid] = (uint16_t)(incl - nrows); int a, b; face_row_range(s_disc, qp.kq, qp.kt, tid, a, b); s_Slo[tid] = a; }
+      if (tid == 11) s_pre[12] = (uint16_t)incl;
+    }
+    __syncthreads();
+    const RingDisc& D = s_disc;
+    if (D.all) {                                       // reading A24: every active tile
+      for (int w = tid; w < mp.n_words; w += kLargeThreads) bitmap[w] = active_words ? __ldg(active_words + w) : 0xffffffffu;
+      if (tid == 0) s_total = qp.active_tiles ? (uint32_t)qp.n_active : (uint32_t)qp.n_tile;
+    } else {
+      for (int e = tid; e <= D.i_hi - D.i_lo; e += kLargeThreads) { int2 fl; ring_interval(D, N, D.i_lo + e, fl.x, fl.y); ring_tab[e] = fl; }
+      __syncthreads();
+      const GroupTab T{ring_tab, D.i_lo};
+      const int n_rows = (int)s_pre[12];
+      const int n_chunks = ((1 << qp.kt) + 63) >> 6;
+      const int n_items = n_rows * n_chunks;
+      uint32_t mine = 0;
+      for (int item = tid; item < n_items; item += kLargeThreads) {
+        const int rowi = item / n_chunks, jbase = (item - rowi * n_chunks) << 6;
+        int f = 0;
+        while (f < 11 && (int)s_pre[f + 1] <= rowi) ++f;
+        const int S = s_Slo[f] + rowi - (int)s_pre[f];
+        if (jbase > min(S, (2 << qp.kt) - 2 - S)) continue;
+        const unsigned long long mask = filter_row_chunk(qp.kt, f, S, jbase, tile_row_mask(D, qp.kq, qp.kt, f, S, jbase, T), slot_of_tile);
+        if (!mask) continue;
+        mine += (uint32_t)__popcll(mask);
+        visit_row_chunk<true>(qp.kt, f, S, jbase, mask, nullptr, [&](uint32_t tile) { atomicOr(&bitmap[tile >> 5], 1u << (tile & 31)); });
+      }
+      if (mine) atomicAdd(&s_total, mine);
+    }
+    __syncthreads();
+    uint32_t* dst = mp.M + (size_t)row * mp.n_words;
+    for (int w = tid; w < mp.n_words; w += kLargeThreads) dst[w] = bitmap[w];
+    if (tid == 0) {
+      counts[slot] = 0;                                // this disc emits no pairs of its own
+      const uint32_t gid = (uint32_t)(k - (int64_t)v * qp.P);
+      mp.row_key[row] = ((unsigned long long)__float_as_uint(__ldg(rho + k)) << 32) | gid;        // reading A10
+      atomicAdd(mp.n_L, (unsigned long long)s_total);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------- transpose
+// block = 256 local rows of one view x 32 word columns (1024 tiles); warp w transposes rows [32 w, 32 w + 32) in registers
+__global__ void __launch_bounds__(256)
+matrix_transpose_kernel(MatParams mp, int V, int64_t n_tile) {
+  __shared__ uint32_t sT[8][32 * 33];
+  // which view does row block blockIdx.y belong to?
+  int v = 0; uint32_t rb = blockIdx.y;
+  for (; v < V; ++v) { const uint32_t nb = (mp.views[v].n_rows + 255u) >> 8; if (rb < nb) break; rb -= nb; }
+  if (v == V) return;
+  const MatView mv = mp.views[v];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int c = blockIdx.x * 32 + lane;                        // word column
+  uint32_t x[32];
+  const uint32_t r0 = rb * 256u + (uint32_t)wid * 32u;         // local row of x[0]
+#pragma unroll
+  for (int i = 0; i < 32; ++i) {
+    const uint32_t lr = r0 + (uint32_t)i;
+    x[i] = (lr < mv.n_rows && c < mp.n_words) ? __ldg(mp.M + (size_t)(mv.row_start + lr) * mp.n_words + c) : 0u;
+  }
+  transpose32(x);                                              // x[b] = bits of tile 32 c + b over the 32 rows
+#pragma unroll
+  for (int b = 0; b < 32; ++b) sT[wid][lane * 33 + b] = x[b];
+  __syncthreads();
+  uint32_t* out = mp.MT + mv.mt_base;
+  for (int q = 0; q < 4; ++q) {
+    const int tl = threadIdx.x + 256 * q;                      // tile inside the slab
+    const int cc = tl >> 5, b = tl & 31;
+    const int64_t tile = ((int64_t)blockIdx.x * 32 + cc) * 32 + b;
+    if (tile >= n_tile) continue;
+    uint4 lo, hi;
+    lo.x = sT[0][cc * 33 + b]; lo.y = sT[1][cc * 33 + b]; lo.z = sT[2][cc * 33 + b]; lo.w = sT[3][cc * 33 + b];
+    hi.x = sT[4][cc * 33 + b]; hi.y = sT[5][cc * 33 + b]; hi.z = sT[6][cc * 33 + b]; hi.w = sT[7][cc * 33 + b];
+    uint4* dst = reinterpret_cast<uint4*>(out + (size_t)tile * mv.W + (size_t)rb * 8);
+    dst[0] = lo; dst[1] = hi;
+  }
+}
+
+// large_count[(v, tile)] = popcount of the tile's bit vector; one warp per (view, tile)
+__global__ void __launch_bounds__(256)
+matrix_popcount_kernel(MatParams mp, int V, int64_t n_tile) {
+  const int lane = threadIdx.x & 31;
+  const int64_t n = (int64_t)V * n_tile;
+  for (int64_t vt = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5); vt < n; vt += (int64_t)gridDim.x * 8) {
+    const int v = (int)(vt / n_tile);
+    const MatView mv = mp.views[v];
+    const uint32_t* bv = mp.MT + mv.mt_base + (size_t)(vt - (int64_t)v * n_tile) * mv.W;
+    uint32_t c = 0;
+    for (uint32_t w = lane; w < mv.W; w += 32) c += (uint32_t)__popc(__ldg(bv + w));
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xffffffffu, c, d);
+    if (lane == 0) mp.large_count[vt] = c;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------- emit + merge
+__device__ __forceinline__ bool pair_less(uint64_t ka, uint32_t va, uint64_t kb, uint32_t vb) { return ka < kb || (ka == kb && va < vb); }
+
+// number of entries of the sorted buffer (bk, bv)[0, n) that are less than (k, v)
+__device__ __forceinline__ uint32_t buf_lower_bound(const unsigned long long* bk, const uint32_t* bv, uint32_t n, unsigned long long k, uint32_t v) {
+  uint32_t lo = 0, hi = n;
+  while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (pair_less(bk[mid], bv[mid], k, v)) lo = mid + 1; else hi = mid; }
+  return lo;
+}
+
+// One warp per (view, tile) writes the tile's FINAL list at keys / vals[start[vt] ...): a streaming merge of two depth-ordered
+// streams held in shared memory 128 entries at a time —
+//   A: the large discs of the tile, generated from its bit vector (set bit r = matrix row r; key from row_key[r]),
+//   B: the tile's small-disc pairs, already radix-sorted (keysS / valsS[s_ranges[vt] ...)).
+// Each round refills both buffers, emits everything up to the smaller of the two "last buffered" entries of streams that still
+// continue (so nothing that could precede an emitted entry is still unread), ranks every emitted entry by a binary search in the
+// other buffer (the two streams never tie: different Gaussians) and stores it straight at its final position — consecutive lanes
+// hit nearly consecutive addresses — then shifts the unconsumed entries to the front.  One buffer is fully consumed per round.
+#ifndef UTS_MB
+#define UTS_MB 256
+#endif
+#ifndef UTS_MB_MINB
+#define UTS_MB_MINB 4
+#endif
+constexpr int kMB = UTS_MB;
+__global__ void __launch_bounds__(256, UTS_MB_MINB)
+matrix_emit_merge_kernel(MatParams mp, int V, int64_t n_tile, const uint64_t* __restrict__ start, const uint64_t* __restrict__ s_ranges,
+                         const uint64_t* __restrict__ keysS, const uint32_t* __restrict__ valsS, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+  __shared__ unsigned long long sAk[8][kMB], sBk[8][kMB];
+  __shared__ uint32_t sAv[8][kMB], sBv[8][kMB];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  unsigned long long* Ak = sAk[wid]; unsigned long long* Bk = sBk[wid];
+  uint32_t* Av = sAv[wid]; uint32_t* Bv = sBv[wid];
+  const int64_t n = (int64_t)V * n_tile;
+  for (int64_t vt = (int64_t)blockIdx.x * 8 + wid; vt < n; vt += (int64_t)gridDim.x * 8) {
+    uint64_t o = start[vt];
+    if (start[vt + 1] == o) continue;
+    uint64_t b_pos = s_ranges[2 * vt];
+    const uint64_t b_end = s_ranges[2 * vt + 1];
+    const int v = (int)(vt / n_tile);
+    const MatView mv = mp.views[v];
+    const uint32_t* bvec = mp.MT + mv.mt_base + (size_t)(vt - (int64_t)v * n_tile) * mv.W;
+    const unsigned long long hi = (unsigned long long)vt << 32;
+    uint32_t w_next = 0, w_cur = 0, x = 0;               // A stream: next chunk, current chunk, this lane's unread bits of it
+    bool a_done = mv.W == 0 || mp.large_count[vt] == 0;
+    uint32_t x_pref = (!a_done && (uint32_t)lane < mv.W) ? __ldg(bvec + lane) : 0u;     // the next chunk's word, fetched one chunk ahead
+    uint32_t fillA = 0, fillB = 0;
+    __syncwarp();
+    for (;;) {
+      // ---- refill A from the bit vector
+      const uint32_t fillA0 = fillA;
+      while (fillA < (uint32_t)kMB && !a_done) {
+        if (!__any_sync(0xffffffffu, x != 0u)) {
+          if (w_next >= mv.W) { a_done = true; break; }
+          w_cur = w_next; w_next += 32;
+          x = x_pref;
+          x_pref = (w_next + lane < mv.W) ? __ldg(bvec + w_next + lane) : 0u;
+          if (!__any_sync(0xffffffffu, x != 0u)) continue;
+        }
+        const uint32_t c = (uint32_t)__popc(x);
+        uint32_t incl = c;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += y; }
+        const uint32_t tot = __shfl_sync(0xffffffffu, incl, 31);
+        const uint32_t room = (uint32_t)kMB - fillA;
+        uint32_t r = incl - c;
+        const uint32_t row0 = (w_cur + lane) * 32;
+        while (x && r < room) {                            // phase 1: matrix rows of the set bits (no memory access)
+          const int b = __ffs((int)x) - 1; x &= x - 1;
+          Av[fillA + r] = row0 + (uint32_t)b; ++r;
+        }
+        fillA += tot < room ? tot : room;
+      }
+      __syncwarp();
+      // phase 2: the rows' (depth, id) in one batch of independent loads
+      {
+        const unsigned long long* rk = mp.row_key + mv.row_start;
+#pragma unroll
+        for (int q = 0; q < kMB / 32; ++q) {
+          const uint32_t i = fillA0 + lane + 32 * q;
+          if (i < fillA) { const unsigned long long k2 = __ldg(rk + Av[i]); Ak[i] = hi | (k2 >> 32); Av[i] = (uint32_t)k2; }
+        }
+      }
+      // ---- refill B from the sorted small pairs
+      if (fillB < (uint32_t)kMB && b_pos < b_end) {
+        const uint32_t take = (uint32_t)(((uint64_t)kMB - fillB) < (b_end - b_pos) ? ((uint64_t)kMB - fillB) : (b_end - b_pos));
+        for (uint32_t j = lane; j < take; j += 32) { Bk[fillB + j] = keysS[b_pos + j]; Bv[fillB + j] = valsS[b_pos + j]; }
+        b_pos += take; fillB += take;
+      }
+      __syncwarp();
+      if (fillA == 0 && fillB == 0) break;
+      const bool b_done = b_pos == b_end;
+      uint32_t na = fillA, nb = fillB;
+      if (fillA && fillB && !(a_done && b_done)) {
+        const bool lastA_smaller = pair_less(Ak[fillA - 1], Av[fillA - 1], Bk[fillB - 1], Bv[fillB - 1]);
+        const bool bound_is_A = !a_done && (b_done || lastA_smaller);
+        if (bound_is_A) nb = buf_lower_bound(Bk, Bv, fillB, Ak[fillA - 1], Av[fillA - 1]);
+        else na = buf_lower_bound(Ak, Av, fillA, Bk[fillB - 1], Bv[fillB - 1]);
+      } else if (fillA && !fillB && !b_done) { na = 0; }      // cannot happen: B is refilled whenever it has entries left
+      // ---- rank and store
+      for (uint32_t i = lane; i < na; i += 32) {
+        const unsigned long long kk = Ak[i]; const uint32_t vv = Av[i];
+        const uint64_t pos = o + i + buf_lower_bound(Bk, Bv, nb, kk, vv);
+        keys[pos] = kk; vals[pos] = vv;
+      }
+      for (uint32_t j = lane; j < nb; j += 32) {
+        const unsigned long long kk = Bk[j]; const uint32_t vv = Bv[j];
+        const uint64_t pos = o + j + buf_lower_bound(Ak, Av, na, kk, vv);
+        keys[pos] = kk; vals[pos] = vv;
+      }
+      o += na + nb;
+      // ---- shift the unconsumed entries to the front
+      unsigned long long tk[kMB / 32]; uint32_t tv[kMB / 32];
+#pragma unroll
+      for (int q = 0; q < kMB / 32; ++q) { const uint32_t i = na + lane + 32 * q; if (i < fillA) { tk[q] = Ak[i]; tv[q] = Av[i]; } }
+      __syncwarp();
+#pragma unroll
+      for (int q = 0; q < kMB / 32; ++q) { const uint32_t i = na + lane + 32 * q; if (i < fillA) { Ak[i - na] = tk[q]; Av[i - na] = tv[q]; } }
+      fillA -= na;
+#pragma unroll
+      for (int q = 0; q < kMB / 32; ++q) { const uint32_t i = nb + lane + 32 * q; if (i < fillB) { tk[q] = Bk[i]; tv[q] = Bv[i]; } }
+      __syncwarp();
+#pragma unroll
+      for (int q = 0; q < kMB / 32; ++q) { const uint32_t i = nb + lane + 32 * q; if (i < fillB) { Bk[i - nb] = tk[q]; Bv[i - nb] = tv[q]; } }
+      fillB -= nb;
+      __syncwarp();
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------- totals, ranges
+// total[vt] = large discs + small pairs of (view, tile)
+__global__ void mat_totals_kernel(int64_t n, const uint32_t* __restrict__ large_count, const uint64_t* __restrict__ s_ranges, uint32_t* __restrict__ total) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) total[i] = large_count[i] + (uint32_t)(s_ranges[2 * i + 1] - s_ranges[2 * i]);
+}
+// ranges[vt] = [start, end) of the final arrays, (0,0) for an empty tile (as uts_tile_ranges)
+__global__ void mat_ranges_kernel(int64_t n, const uint64_t* __restrict__ start, uint64_t* __restrict__ ranges) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint64_t a = start[i], b = start[i + 1];
+  ranges[2 * i] = a == b ? 0 : a; ranges[2 * i + 1] = a == b ? 0 : b;
+}
+
+}  // namespace uts

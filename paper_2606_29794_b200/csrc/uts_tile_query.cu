@@ -263,15 +263,25 @@ classify_kernel(QueryParams qp, const float* __restrict__ rs, const uint8_t* __r
 
 // hist[64] counts -> exclusive start offsets (in place); n_small = total
 // n_small[1], n_small[2]: ends of the block-per-disc and warp-per-disc parts of perm (ring-interval path)
-__global__ void bucket_scan_kernel(uint32_t* __restrict__ hist, uint32_t* __restrict__ n_small, int b_block, int b_warp) {
+// n_small[3]: end of the matrix class (uts_tile_lists): whole buckets <= b_mat while they fit cap_rows rows; 0 when b_mat < 0 or
+// when the pairs those discs own (estimated from the bucket radii) would not pay for the per-(view, tile) bookkeeping of the
+// matrix path (about 256 B per (view, tile) against about 90 B per pair saved)
+__global__ void bucket_scan_kernel(uint32_t* __restrict__ hist, uint32_t* __restrict__ n_small, int b_block, int b_warp, int b_mat, uint32_t cap_rows,
+                                   double n_tile, double nvt) {
   if (threadIdx.x == 0) {
-    uint32_t run = 0, e_block = 0, e_warp = 0;
+    uint32_t run = 0, e_block = 0, e_warp = 0, e_mat = 0;
+    double est_pairs = 0.0, est_at_mat = 0.0;
+    const int top = (int)(__float_as_uint(4.0f) >> 21);
     for (int b = 0; b < kBuckets; ++b) {
       const uint32_t c = hist[b]; hist[b] = run; run += c;
+      const float r_lo = fminf(3.14159274f, __uint_as_float((uint32_t)(top - b) << 21));     // smallest radius of bucket b
+      est_pairs += (double)c * fmin(n_tile, 0.5 * n_tile * (1.0 - cos((double)r_lo)));
       if (b <= b_block) e_block = run;
       if (b <= b_warp) e_warp = run;
+      if (b <= b_mat && run <= cap_rows) { e_mat = run; est_at_mat = est_pairs; }
     }
-    n_small[0] = run; n_small[1] = e_block; n_small[2] = e_warp;
+    if (est_at_mat * 90.0 < nvt * 256.0) e_mat = 0;
+    n_small[0] = run; n_small[1] = e_block; n_small[2] = e_warp; n_small[3] = e_mat;
   }
 }
 
@@ -715,7 +725,7 @@ ring_query_block_kernel(QueryParams qp, const float* __restrict__ dir, const flo
   __shared__ uint32_t s_em_pre[kLargeThreads / 32][33], s_em_row[kLargeThreads / 32][32];
   const uint32_t end = n_small[1];
   const int N = 1 << qp.kq, tid = threadIdx.x;
-  for (uint32_t idx = blockIdx.x; idx < end; idx += gridDim.x) {
+  for (uint32_t idx = n_small[3] + blockIdx.x; idx < end; idx += gridDim.x) {        // discs before n_small[3] are uts_tile_lists' matrix rows
     const int64_t k = (int64_t)perm[idx];
     const int64_t slot = emit_rank ? (int64_t)emit_rank[k] : k;
     uint64_t b0 = 0;
@@ -828,6 +838,8 @@ ring_query_block_kernel(QueryParams qp, const float* __restrict__ dir, const flo
 
 }  // namespace uts
 
+#include "uts_tile_matrix.cuh"
+
 using namespace uts;
 
 namespace {
@@ -887,6 +899,228 @@ QueryLayout query_layout(const uts_config* cfg) {
   L.total = off + 256;
   return L;
 }
+// Scratch of the matrix path (uts_tile_lists), appended after the query's own scratch.
+struct MatLayout { size_t flag, rank_scan, scan, M, MT, row_key, views, large, loff, total, start, sranges, offsets, misc, total_bytes; uint32_t cap_rows; size_t mt_words; };
+MatLayout mat_layout(const uts_config* cfg, size_t base) {
+  const size_t n = (size_t)cfg->n_gauss * cfg->n_views;
+  const size_t n_tile = (size_t)12 << (2 * (cfg->order - cfg->tile_log2));
+  const size_t nvt = n_tile * (size_t)cfg->n_views;
+  const size_t n_words = n_tile / 32;
+  MatLayout L;
+  size_t cap = n_words ? ((size_t)1 << 30) / (n_words * 4) : 0;         // bitmap rows that fit 1 GB
+  if (cap > n) cap = n;
+  if (cap > 0xfffffff0u) cap = 0xfffffff0u;
+  L.cap_rows = (uint32_t)cap;
+  L.mt_words = n_tile * (((cap + 255) / 256 + (size_t)cfg->n_views) * 8);  // sum over views of n_tile * W_v
+  size_t off = base;
+  L.flag = off;      off += align256(n * 4);
+  L.rank_scan = off; off += align256((n + 1) * 8);
+  L.scan = off;      off += scan_scratch_bytes((int64_t)(n > nvt ? n : nvt));
+  L.M = off;         off += align256(cap * n_words * 4);
+  L.MT = off;        off += align256(L.mt_words * 4);
+  L.row_key = off;   off += align256((cap + 1024) * 8);
+  L.views = off;     off += align256((size_t)cfg->n_views * sizeof(MatView));
+  L.large = off;     off += align256(nvt * 4);
+  L.loff = off;      off += align256((nvt + 1) * 8);
+  L.total = off;     off += align256(nvt * 4);
+  L.start = off;     off += align256((nvt + 1) * 8);
+  L.sranges = off;   off += align256(nvt * 16);
+  L.offsets = off;   off += align256((n + 1) * 8);
+  L.misc = off;      off += 256;
+  L.total_bytes = off + 256;
+  return L;
+}
+
+// One tile query on the ring-interval path (or the quadtree descent): host-side parameters, then count() and emit().
+struct QueryRun {
+  const uts_config* cfg; uts_proj in; uts_mask mask; const uint32_t* emit_rank; cudaStream_t s;
+  Dims d; int64_t n;
+  QueryParams qp;
+  bool ring_impl, use_large;
+  uint32_t *counts, *list, *n_large, *n_small, *hist, *perm, *active;
+  uint64_t* block_sums;
+  const uint32_t* active_arg;
+  unsigned qgrid; int lgrid; size_t dyn_smem;
+  size_t smem_a, smem_b, smem_block;
+  unsigned agrid, wgrid, bgrid, agrid_e, wgrid_e, bgrid_e;
+  static constexpr int kBatchA = 128, kBatchB = 32;          // discs per batch: rc_thread class, rc_warp class
+  int b_mat; uint32_t cap_rows;                              // matrix class of uts_tile_lists (b_mat < 0: none)
+
+  int setup(const uts_config* cfg_, uts_proj in_, uts_mask mask_, const uint32_t* emit_rank_, void* scratch, cudaStream_t s_) {
+    cfg = cfg_; in = in_; mask = mask_; emit_rank = emit_rank_; s = s_;
+    d = dims_of(cfg, &mask);
+    n = (int64_t)d.P * d.V;
+    b_mat = -1; cap_rows = 0;
+    qp.kt = d.kt; qp.kq = d.kq; qp.P = d.P; qp.V = d.V; qp.n_tile = d.n_tile;
+    const double* rm = rho_max_table_host();
+    qp.rho_q = cfg->query_mode == UTS_QUERY_RING ? 0.0 : rm[d.kq];      // Alg.3's set has no PixRad margin
+    for (int o = 0; o <= kMaxOrder; ++o) { qp.rho[o] = (float)rm[o]; qp.sin_hrho[o] = (float)sin(0.5 * rm[o]); qp.cos_hrho[o] = (float)cos(0.5 * rm[o]); }
+    // Implementation choice: the ring-interval path (uts_ring_query.cuh) whenever a block's ring table fits shared memory
+    // (k_q <= 12); the quadtree descent below otherwise, or when UTS_QUERY_IMPL=tree asks for it (A/B measurements).
+    const char* impl_env = getenv("UTS_QUERY_IMPL");
+    const int Nq = 1 << d.kq;
+    ring_impl = 4 * Nq - 1 <= kRingBlockRingsMax && !(impl_env && strcmp(impl_env, "tree") == 0);
+    qp.rc_thread = kRingThreadRings; qp.rc_warp = 4 * Nq - 1 < kRingWarpRings ? 4 * Nq - 1 : kRingWarpRings; qp.rc_block = 4 * Nq - 1;
+    // a disc of radius R reaches at most 3 R N + 4 rings (ring spacing >= 2/(3N) in colatitude, +-1 ring of padding at each end)
+    qp.b_warp = radius_bucket_host((float)((qp.rc_thread - 6) / (3.0 * Nq)));
+    qp.b_block = radius_bucket_host((float)((qp.rc_warp - 6) / (3.0 * Nq)));
+    if (qp.b_block > qp.b_warp) qp.b_block = qp.b_warp;
+    qp.active_tiles = mask.active_tiles; qp.n_active = mask.active_tiles ? mask.n_active : -1;
+    qp.os = d.kt < 4 ? d.kt : 4;
+    const size_t n_split = (size_t)12 << (2 * qp.os);
+    qp.wl_cap = (int)(n_split > 4096 ? n_split : 4096);
+    const size_t large_smem = (2 * (size_t)(d.n_tile / 32) + 2 * (size_t)qp.wl_cap) * 4;
+    use_large = !ring_impl && d.kt >= 2 && large_smem <= kMaxLargeSmem;
+    qp.n_words = use_large ? (int)(d.n_tile / 32) : 0;
+    const char* e1__ = getenv("UTS_RLARGE"); const char* e2__ = getenv("UTS_LGRID");
+    qp.r_large = (float)((e1__ ? atof(e1__) : 36.0) / sqrt((double)d.n_tile));      // ~320 tiles (pi R^2 / (4 pi / n_tile)); measured crossover on config 4
+
+    const QueryLayout L = query_layout(cfg);
+    char* sp = reinterpret_cast<char*>(scratch);
+    counts = reinterpret_cast<uint32_t*>(sp + L.counts);
+    list = reinterpret_cast<uint32_t*>(sp + L.list);
+    n_large = reinterpret_cast<uint32_t*>(sp + L.nlarge);
+    n_small = n_large + 1;
+    hist = n_large + 32;
+    perm = reinterpret_cast<uint32_t*>(sp + L.perm);
+    active = reinterpret_cast<uint32_t*>(sp + L.active);
+    block_sums = reinterpret_cast<uint64_t*>(sp + L.scan);
+    qp.tile_cache = reinterpret_cast<uint32_t*>(sp + L.tcache);
+    qp.bitmap_cache = reinterpret_cast<uint32_t*>(sp + L.bcache);
+    qp.bitmap_cache_cap = L.bcache_cap;
+    // the ring path reuses two scratch regions of the descent: the bitmap cache holds the row masks, `list` their bases
+    qp.mask_cache = reinterpret_cast<unsigned long long*>(sp + L.bcache);
+    qp.mask_cache_cap = (uint32_t)(L.bcache_bytes / 8);
+    qp.mask_cursor = n_large + 8;                                              // zeroed with the header in count()
+    qp.mask_base = list;
+    active_arg = nullptr;
+    qgrid = (unsigned)((n + kLargeThreads - 1) / kLargeThreads);
+    lgrid = use_large ? sm_count() * (e2__ ? atoi(e2__) : 2) : 0;
+    dyn_smem = use_large ? large_smem : 0;
+    smem_a = sizeof(BatchRec) * kBatchA + (size_t)kBatchA * qp.rc_thread * sizeof(int2);
+    smem_b = sizeof(BatchRec) * kBatchB + (size_t)kBatchB * qp.rc_warp * sizeof(int2);
+    smem_block = (size_t)qp.rc_block * sizeof(int2);
+    agrid = wgrid = bgrid = agrid_e = wgrid_e = bgrid_e = 0;     // persistent grids: exactly the resident blocks
+    if (use_large) {
+      static bool attr_set = false;
+      if (!attr_set) {
+        UTS_CUDA(cudaFuncSetAttribute(tile_query_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxLargeSmem));
+        UTS_CUDA(cudaFuncSetAttribute(tile_query_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxLargeSmem));
+        attr_set = true;
+      }
+    }
+    if (ring_impl) {
+      static bool ring_attr_set = false;
+      if (!ring_attr_set) {
+        UTS_CUDA(cudaFuncSetAttribute(ring_query_block_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kRingBlockRingsMax * 8 + 8));
+        UTS_CUDA(cudaFuncSetAttribute(ring_query_block_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kRingBlockRingsMax * 8 + 8));
+        UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchA, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+        UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchA, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+        UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+        UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+        UTS_CUDA(cudaFuncSetAttribute(matrix_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024));
+        ring_attr_set = true;
+      }
+      int occ[6] = {1, 1, 1, 1, 1, 1};
+      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[0], ring_query_block_kernel<false>, kLargeThreads, smem_block));
+      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[1], ring_query_block_kernel<true>, kLargeThreads, smem_block));
+      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[2], ring_query_batch_kernel<kBatchB, false>, kLargeThreads, smem_b));
+      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[3], ring_query_batch_kernel<kBatchB, true>, kLargeThreads, smem_b));
+      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[4], ring_query_batch_kernel<kBatchA, false>, kLargeThreads, smem_a));
+      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[5], ring_query_batch_kernel<kBatchA, true>, kLargeThreads, smem_a));
+      const unsigned sms = (unsigned)sm_count();
+      bgrid = sms * (unsigned)(occ[0] > 0 ? occ[0] : 1); bgrid_e = sms * (unsigned)(occ[1] > 0 ? occ[1] : 1);
+      wgrid = sms * (unsigned)(occ[2] > 0 ? occ[2] : 1); wgrid_e = sms * (unsigned)(occ[3] > 0 ? occ[3] : 1);
+      agrid = sms * (unsigned)(occ[4] > 0 ? occ[4] : 1); agrid_e = sms * (unsigned)(occ[5] > 0 ? occ[5] : 1);
+      if (!g_fj.init()) { set_last_cuda_error(cudaGetLastError()); return UTS_ERR_CUDA; }
+    }
+    return UTS_OK;
+  }
+
+  // classification + count pass + exclusive scan of the per-slot counts into offsets[n + 1].  mp != nullptr: the discs of the
+  // matrix class write bitmap rows instead (and count 0).  Enqueues only.
+  int count(uint64_t* offsets, MatParams* mp, uint32_t* flag_by_rank, uint64_t* rank_scan, uint64_t* rank_scan_sums) {
+    if (use_large && mask.slot_of_tile) {
+      active_words_kernel<<<(qp.n_words + 255) / 256, 256, 0, s>>>(mask.slot_of_tile, qp.n_words, active);
+      UTS_LAUNCH_CHECK();
+      active_arg = active;
+    }
+    UTS_CUDA(cudaMemsetAsync(n_large, 0, 512, s));
+    const unsigned cgrid = (unsigned)((n + 255) / 256);
+    classify_kernel<0><<<cgrid, 256, 0, s>>>(qp, in.rs, in.flags, counts, list, n_large, hist, perm, emit_rank);
+    UTS_LAUNCH_CHECK();
+    bucket_scan_kernel<<<1, 32, 0, s>>>(hist, n_small, qp.b_block, qp.b_warp, mp ? b_mat : -1, cap_rows, (double)d.n_tile, (double)d.n_tile * d.V);
+    UTS_LAUNCH_CHECK();
+    classify_kernel<1><<<cgrid, 256, 0, s>>>(qp, in.rs, in.flags, counts, list, n_large, hist, perm, emit_rank);
+    UTS_LAUNCH_CHECK();
+    if (ring_impl) {
+      if (mp) {                                       // rows of the bit matrix: rank order of the matrix-class discs
+        UTS_CUDA(cudaMemsetAsync(flag_by_rank, 0, (size_t)n * 4, s));
+        UTS_CUDA(cudaMemsetAsync(mp->n_L, 0, 8, s));
+        mat_flag_kernel<<<sm_count() * 4, 256, 0, s>>>(perm, n_small, emit_rank, flag_by_rank);
+        UTS_LAUNCH_CHECK();
+        int st = exclusive_scan_u32(flag_by_rank, n, rank_scan, rank_scan_sums, s);
+        if (st) return st;
+        mat_view_tab_kernel<<<1, 32, 0, s>>>(*mp, d.P, d.V, d.n_tile);
+        UTS_LAUNCH_CHECK();
+        if (mask.slot_of_tile) {
+          active_words_kernel<<<(mp->n_words + 255) / 256, 256, 0, s>>>(mask.slot_of_tile, mp->n_words, active);
+          UTS_LAUNCH_CHECK();
+        }
+      }
+      UTS_CUDA(cudaEventRecord(g_fj.fork, s));
+      UTS_CUDA(cudaStreamWaitEvent(g_fj.aux[0], g_fj.fork, 0));
+      UTS_CUDA(cudaStreamWaitEvent(g_fj.aux[1], g_fj.fork, 0));
+      ring_query_block_kernel<false><<<bgrid, kLargeThreads, smem_block, s>>>(qp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small, emit_rank,
+                                                                            counts, nullptr, nullptr, nullptr);
+      UTS_LAUNCH_CHECK();
+      if (mp) {
+        const size_t smem_m = smem_block + (size_t)mp->n_words * 4;
+        int occ = 1;
+        UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, matrix_count_kernel, kLargeThreads, smem_m));
+        matrix_count_kernel<<<(unsigned)sm_count() * (unsigned)(occ > 0 ? occ : 1), kLargeThreads, smem_m, s>>>(
+            qp, *mp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, mask.slot_of_tile ? active : nullptr, perm, n_small, emit_rank, counts);
+        UTS_LAUNCH_CHECK();
+      }
+      ring_query_batch_kernel<kBatchB, false><<<wgrid, kLargeThreads, smem_b, g_fj.aux[0]>>>(qp, 0, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
+                                                                                 emit_rank, counts, nullptr, nullptr, nullptr);
+      UTS_LAUNCH_CHECK();
+      ring_query_batch_kernel<kBatchA, false><<<agrid, kLargeThreads, smem_a, g_fj.aux[1]>>>(qp, 1, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
+                                                                                 emit_rank, counts, nullptr, nullptr, nullptr);
+      UTS_LAUNCH_CHECK();
+      for (int i = 0; i < 2; ++i) { UTS_CUDA(cudaEventRecord(g_fj.join[i], g_fj.aux[i])); UTS_CUDA(cudaStreamWaitEvent(s, g_fj.join[i], 0)); }
+    } else {
+      tile_query_kernel<false><<<qgrid + lgrid, kLargeThreads, dyn_smem, s>>>(qp, lgrid, in.dir, in.rho, in.rs, mask.slot_of_tile, active_arg, perm,
+                                                                             n_small, list, n_large, emit_rank, counts, nullptr, nullptr, nullptr);
+      UTS_LAUNCH_CHECK();
+    }
+    return exclusive_scan_u32(counts, n, offsets, block_sums, s);
+  }
+
+  // emit pass: the pairs of every slot at keys/vals[offsets[slot] ...).  Enqueues only.
+  int emit(const uint64_t* offsets, uint64_t* keys, uint32_t* vals) {
+    if (ring_impl) {
+      UTS_CUDA(cudaEventRecord(g_fj.fork, s));
+      UTS_CUDA(cudaStreamWaitEvent(g_fj.aux[0], g_fj.fork, 0));
+      UTS_CUDA(cudaStreamWaitEvent(g_fj.aux[1], g_fj.fork, 0));
+      ring_query_block_kernel<true><<<bgrid_e, kLargeThreads, smem_block, s>>>(qp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small, emit_rank,
+                                                                           nullptr, offsets, keys, vals);
+      UTS_LAUNCH_CHECK();
+      ring_query_batch_kernel<kBatchB, true><<<wgrid_e, kLargeThreads, smem_b, g_fj.aux[0]>>>(qp, 0, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
+                                                                                emit_rank, nullptr, offsets, keys, vals);
+      UTS_LAUNCH_CHECK();
+      ring_query_batch_kernel<kBatchA, true><<<agrid_e, kLargeThreads, smem_a, g_fj.aux[1]>>>(qp, 1, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
+                                                                                emit_rank, nullptr, offsets, keys, vals);
+      UTS_LAUNCH_CHECK();
+      for (int i = 0; i < 2; ++i) { UTS_CUDA(cudaEventRecord(g_fj.join[i], g_fj.aux[i])); UTS_CUDA(cudaStreamWaitEvent(s, g_fj.join[i], 0)); }
+      return UTS_OK;
+    }
+    tile_query_kernel<true><<<qgrid + lgrid, kLargeThreads, dyn_smem, s>>>(qp, lgrid, in.dir, in.rho, in.rs, mask.slot_of_tile, active_arg, perm,
+                                                                          n_small, list, n_large, emit_rank, nullptr, offsets, keys, vals);
+    UTS_LAUNCH_CHECK();
+    return UTS_OK;
+  }
+};
 }  // namespace
 
 extern "C" {
@@ -903,8 +1137,7 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   if ((st = check_mask(cfg, mask))) return st;
   if (!offsets || !h_n_pairs) return UTS_ERR_INVALID_ARG;
   cudaStream_t s = (cudaStream_t)stream;
-  Dims d = dims_of(cfg, &mask);
-  const int64_t n = (int64_t)d.P * d.V;
+  const int64_t n = (int64_t)cfg->n_gauss * cfg->n_views;
   if (n == 0) {                         // empty Gaussian set: no pairs, nothing else is read
     UTS_CUDA(cudaMemsetAsync(offsets, 0, sizeof(uint64_t), s));
     UTS_CUDA(cudaStreamSynchronize(s));
@@ -914,147 +1147,114 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   if (!in.dir || !in.lonlat || !in.rho || !in.rs || !in.flags || !scratch) return UTS_ERR_INVALID_ARG;
   if (keys && !vals) return UTS_ERR_INVALID_ARG;
   if (scratch_bytes < uts_tile_query_scratch_bytes(cfg) || ((uintptr_t)scratch & 255)) return UTS_ERR_INVALID_ARG;
-
-  QueryParams qp;
-  qp.kt = d.kt; qp.kq = d.kq; qp.P = d.P; qp.V = d.V; qp.n_tile = d.n_tile;
-  const double* rm = rho_max_table_host();
-  qp.rho_q = cfg->query_mode == UTS_QUERY_RING ? 0.0 : rm[d.kq];      // Alg.3's set has no PixRad margin
-  for (int o = 0; o <= kMaxOrder; ++o) { qp.rho[o] = (float)rm[o]; qp.sin_hrho[o] = (float)sin(0.5 * rm[o]); qp.cos_hrho[o] = (float)cos(0.5 * rm[o]); }
-  // Implementation choice: the ring-interval path (uts_ring_query.cuh) whenever a block's ring table fits shared memory
-  // (k_q <= 12); the quadtree descent below otherwise, or when UTS_QUERY_IMPL=tree asks for it (A/B measurements).
-  const char* impl_env = getenv("UTS_QUERY_IMPL");
-  const int Nq = 1 << d.kq;
-  const bool ring_impl = 4 * Nq - 1 <= kRingBlockRingsMax && !(impl_env && strcmp(impl_env, "tree") == 0);
-  qp.rc_thread = kRingThreadRings; qp.rc_warp = 4 * Nq - 1 < kRingWarpRings ? 4 * Nq - 1 : kRingWarpRings; qp.rc_block = 4 * Nq - 1;
-  // a disc of radius R reaches at most 3 R N + 4 rings (ring spacing >= 2/(3N) in colatitude, +-1 ring of padding at each end)
-  qp.b_warp = radius_bucket_host((float)((qp.rc_thread - 6) / (3.0 * Nq)));
-  qp.b_block = radius_bucket_host((float)((qp.rc_warp - 6) / (3.0 * Nq)));
-  if (qp.b_block > qp.b_warp) qp.b_block = qp.b_warp;
-  qp.active_tiles = mask.active_tiles; qp.n_active = mask.active_tiles ? mask.n_active : -1;
-  // the ring path reuses two scratch regions of the descent: the bitmap cache holds the row masks, `list` their bases
-  qp.mask_cache = nullptr; qp.mask_cache_cap = 0; qp.mask_cursor = nullptr; qp.mask_base = nullptr;
-  qp.os = d.kt < 4 ? d.kt : 4;
-  const size_t n_split = (size_t)12 << (2 * qp.os);
-  qp.wl_cap = (int)(n_split > 4096 ? n_split : 4096);
-  const size_t large_smem = (2 * (size_t)(d.n_tile / 32) + 2 * (size_t)qp.wl_cap) * 4;
-  const bool use_large = !ring_impl && d.kt >= 2 && large_smem <= kMaxLargeSmem;
-  qp.n_words = use_large ? (int)(d.n_tile / 32) : 0;
-  const char* e1__ = getenv("UTS_RLARGE"); const char* e2__ = getenv("UTS_LGRID");
-  qp.r_large = (float)((e1__ ? atof(e1__) : 36.0) / sqrt((double)d.n_tile));      // ~320 tiles (pi R^2 / (4 pi / n_tile)); measured crossover on config 4
-
-  const QueryLayout L = query_layout(cfg);
-  char* sp = reinterpret_cast<char*>(scratch);
-  uint32_t* counts = reinterpret_cast<uint32_t*>(sp + L.counts);
-  uint32_t* list = reinterpret_cast<uint32_t*>(sp + L.list);
-  uint32_t* n_large = reinterpret_cast<uint32_t*>(sp + L.nlarge);
-  uint32_t* n_small = n_large + 1;
-  uint32_t* hist = n_large + 32;
-  uint32_t* perm = reinterpret_cast<uint32_t*>(sp + L.perm);
-  uint32_t* active = reinterpret_cast<uint32_t*>(sp + L.active);
-  uint64_t* block_sums = reinterpret_cast<uint64_t*>(sp + L.scan);
-  qp.tile_cache = reinterpret_cast<uint32_t*>(sp + L.tcache);
-  qp.bitmap_cache = reinterpret_cast<uint32_t*>(sp + L.bcache);
-  qp.bitmap_cache_cap = L.bcache_cap;
-  qp.mask_cache = reinterpret_cast<unsigned long long*>(sp + L.bcache);
-  qp.mask_cache_cap = (uint32_t)(L.bcache_bytes / 8);
-  qp.mask_cursor = n_large + 8;                                              // zeroed with the header below
-  qp.mask_base = list;
-  const uint32_t* active_arg = nullptr;
-  const unsigned qgrid = (unsigned)((n + kLargeThreads - 1) / kLargeThreads);
-  const int lgrid = use_large ? sm_count() * (e2__ ? atoi(e2__) : 2) : 0;
-  const size_t dyn_smem = use_large ? large_smem : 0;
-  if (use_large) {
-    static bool attr_set = false;
-    if (!attr_set) {
-      UTS_CUDA(cudaFuncSetAttribute(tile_query_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxLargeSmem));
-      UTS_CUDA(cudaFuncSetAttribute(tile_query_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxLargeSmem));
-      attr_set = true;
-    }
-    if (mask.slot_of_tile) {
-      active_words_kernel<<<(qp.n_words + 255) / 256, 256, 0, s>>>(mask.slot_of_tile, qp.n_words, active);
-      UTS_LAUNCH_CHECK();
-      active_arg = active;
-    }
-  }
-  UTS_CUDA(cudaMemsetAsync(n_large, 0, 512, s));
-  const unsigned cgrid = (unsigned)((n + 255) / 256);
-  classify_kernel<0><<<cgrid, 256, 0, s>>>(qp, in.rs, in.flags, counts, list, n_large, hist, perm, emit_rank);
-  UTS_LAUNCH_CHECK();
-  bucket_scan_kernel<<<1, 32, 0, s>>>(hist, n_small, qp.b_block, qp.b_warp);
-  UTS_LAUNCH_CHECK();
-  classify_kernel<1><<<cgrid, 256, 0, s>>>(qp, in.rs, in.flags, counts, list, n_large, hist, perm, emit_rank);
-  UTS_LAUNCH_CHECK();
-  constexpr int kBatchA = 128, kBatchB = 32;          // discs per batch: rc_thread class, rc_warp class
-  const size_t smem_a = sizeof(BatchRec) * kBatchA + (size_t)kBatchA * qp.rc_thread * sizeof(int2),
-               smem_b = sizeof(BatchRec) * kBatchB + (size_t)kBatchB * qp.rc_warp * sizeof(int2), smem_block = (size_t)qp.rc_block * sizeof(int2);
-  unsigned agrid = 0, wgrid = 0, bgrid = 0, agrid_e = 0, wgrid_e = 0, bgrid_e = 0;     // persistent grids: exactly the resident blocks
-  if (ring_impl) {
-    static bool ring_attr_set = false;
-    if (!ring_attr_set) {
-      UTS_CUDA(cudaFuncSetAttribute(ring_query_block_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kRingBlockRingsMax * 8 + 8));
-      UTS_CUDA(cudaFuncSetAttribute(ring_query_block_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kRingBlockRingsMax * 8 + 8));
-      UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchA, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
-      UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchA, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
-      UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
-      UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
-      ring_attr_set = true;
-    }
-    {
-      int occ[6] = {1, 1, 1, 1, 1, 1};
-      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[0], ring_query_block_kernel<false>, kLargeThreads, smem_block));
-      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[1], ring_query_block_kernel<true>, kLargeThreads, smem_block));
-      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[2], ring_query_batch_kernel<kBatchB, false>, kLargeThreads, smem_b));
-      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[3], ring_query_batch_kernel<kBatchB, true>, kLargeThreads, smem_b));
-      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[4], ring_query_batch_kernel<kBatchA, false>, kLargeThreads, smem_a));
-      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[5], ring_query_batch_kernel<kBatchA, true>, kLargeThreads, smem_a));
-      const unsigned sms = (unsigned)sm_count();
-      bgrid = sms * (unsigned)(occ[0] > 0 ? occ[0] : 1); bgrid_e = sms * (unsigned)(occ[1] > 0 ? occ[1] : 1);
-      wgrid = sms * (unsigned)(occ[2] > 0 ? occ[2] : 1); wgrid_e = sms * (unsigned)(occ[3] > 0 ? occ[3] : 1);
-      agrid = sms * (unsigned)(occ[4] > 0 ? occ[4] : 1); agrid_e = sms * (unsigned)(occ[5] > 0 ? occ[5] : 1);
-    }
-    if (!g_fj.init()) { set_last_cuda_error(cudaGetLastError()); return UTS_ERR_CUDA; }
-    UTS_CUDA(cudaEventRecord(g_fj.fork, s));
-    UTS_CUDA(cudaStreamWaitEvent(g_fj.aux[0], g_fj.fork, 0));
-    UTS_CUDA(cudaStreamWaitEvent(g_fj.aux[1], g_fj.fork, 0));
-    ring_query_block_kernel<false><<<bgrid, kLargeThreads, smem_block, s>>>(qp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small, emit_rank,
-                                                                          counts, nullptr, nullptr, nullptr);
-    UTS_LAUNCH_CHECK();
-    ring_query_batch_kernel<kBatchB, false><<<wgrid, kLargeThreads, smem_b, g_fj.aux[0]>>>(qp, 0, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
-                                                                               emit_rank, counts, nullptr, nullptr, nullptr);
-    UTS_LAUNCH_CHECK();
-    ring_query_batch_kernel<kBatchA, false><<<agrid, kLargeThreads, smem_a, g_fj.aux[1]>>>(qp, 1, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
-                                                                               emit_rank, counts, nullptr, nullptr, nullptr);
-    UTS_LAUNCH_CHECK();
-    for (int i = 0; i < 2; ++i) { UTS_CUDA(cudaEventRecord(g_fj.join[i], g_fj.aux[i])); UTS_CUDA(cudaStreamWaitEvent(s, g_fj.join[i], 0)); }
-  } else {
-    tile_query_kernel<false><<<qgrid + lgrid, kLargeThreads, dyn_smem, s>>>(qp, lgrid, in.dir, in.rho, in.rs, mask.slot_of_tile, active_arg, perm,
-                                                                           n_small, list, n_large, emit_rank, counts, nullptr, nullptr, nullptr);
-    UTS_LAUNCH_CHECK();
-  }
-  if ((st = exclusive_scan_u32(counts, n, offsets, block_sums, s))) return st;
+  QueryRun q;
+  if ((st = q.setup(cfg, in, mask, emit_rank, scratch, s))) return st;
+  if ((st = q.count(offsets, nullptr, nullptr, nullptr, nullptr))) return st;
   UTS_CUDA(cudaMemcpyAsync(h_n_pairs, offsets + n, sizeof(uint64_t), cudaMemcpyDeviceToHost, s));
   UTS_CUDA(cudaStreamSynchronize(s));
   if (!keys) return UTS_OK;
   if (*h_n_pairs > capacity) return UTS_ERR_CAPACITY;
   if (*h_n_pairs == 0) return UTS_OK;
-  if (ring_impl) {
-    UTS_CUDA(cudaEventRecord(g_fj.fork, s));
-    UTS_CUDA(cudaStreamWaitEvent(g_fj.aux[0], g_fj.fork, 0));
-    UTS_CUDA(cudaStreamWaitEvent(g_fj.aux[1], g_fj.fork, 0));
-    ring_query_block_kernel<true><<<bgrid_e, kLargeThreads, smem_block, s>>>(qp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small, emit_rank,
-                                                                         nullptr, offsets, keys, vals);
-    UTS_LAUNCH_CHECK();
-    ring_query_batch_kernel<kBatchB, true><<<wgrid_e, kLargeThreads, smem_b, g_fj.aux[0]>>>(qp, 0, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
-                                                                              emit_rank, nullptr, offsets, keys, vals);
-    UTS_LAUNCH_CHECK();
-    ring_query_batch_kernel<kBatchA, true><<<agrid_e, kLargeThreads, smem_a, g_fj.aux[1]>>>(qp, 1, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
-                                                                              emit_rank, nullptr, offsets, keys, vals);
-    UTS_LAUNCH_CHECK();
-    for (int i = 0; i < 2; ++i) { UTS_CUDA(cudaEventRecord(g_fj.join[i], g_fj.aux[i])); UTS_CUDA(cudaStreamWaitEvent(s, g_fj.join[i], 0)); }
+  return q.emit(offsets, keys, vals);
+}
+
+size_t uts_tile_lists_scratch_bytes(const uts_config* cfg) {
+  if (check_config(cfg) != UTS_OK) return 0;
+  return mat_layout(cfg, query_layout(cfg).total).total_bytes;
+}
+
+int uts_tile_lists(const uts_config* cfg, uts_proj in, uts_mask mask, const uint32_t* emit_rank, uint64_t* keys, uint32_t* vals,
+                   uint64_t* keys_tmp, uint32_t* vals_tmp, uint64_t capacity, uint64_t* ranges, uint64_t* h_n_pairs, void* scratch,
+                   size_t scratch_bytes, void* sort_scratch, size_t sort_scratch_bytes, void* stream) {
+  int st = check_config(cfg);
+  if (st) return st;
+  if ((st = check_mask(cfg, mask))) return st;
+  if (!ranges || !h_n_pairs || !emit_rank) return UTS_ERR_INVALID_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  const Dims d = dims_of(cfg, &mask);
+  const int64_t n = (int64_t)d.P * d.V, nvt = (int64_t)d.V * d.n_tile;
+  if (n == 0) {
+    UTS_CUDA(cudaMemsetAsync(ranges, 0, (size_t)nvt * 16, s));
+    UTS_CUDA(cudaStreamSynchronize(s));
+    *h_n_pairs = 0;
     return UTS_OK;
   }
-  tile_query_kernel<true><<<qgrid + lgrid, kLargeThreads, dyn_smem, s>>>(qp, lgrid, in.dir, in.rho, in.rs, mask.slot_of_tile, active_arg, perm,
-                                                                        n_small, list, n_large, emit_rank, nullptr, offsets, keys, vals);
+  if (!in.dir || !in.lonlat || !in.rho || !in.rs || !in.flags || !scratch || !sort_scratch) return UTS_ERR_INVALID_ARG;
+  if (!keys || !vals || !keys_tmp || !vals_tmp) return UTS_ERR_INVALID_ARG;
+  if (scratch_bytes < uts_tile_lists_scratch_bytes(cfg) || ((uintptr_t)scratch & 255) || ((uintptr_t)sort_scratch & 255)) return UTS_ERR_INVALID_ARG;
+  const QueryLayout QL = query_layout(cfg);
+  const MatLayout ML = mat_layout(cfg, QL.total);
+  char* sp = reinterpret_cast<char*>(scratch);
+  uint64_t* offsets = reinterpret_cast<uint64_t*>(sp + ML.offsets);
+  QueryRun q;
+  if ((st = q.setup(cfg, in, mask, emit_rank, scratch, s))) return st;
+  MatParams mp;
+  mp.M = reinterpret_cast<uint32_t*>(sp + ML.M); mp.MT = reinterpret_cast<uint32_t*>(sp + ML.MT);
+  mp.row_key = reinterpret_cast<unsigned long long*>(sp + ML.row_key);
+  mp.row_of_rank = reinterpret_cast<const uint64_t*>(sp + ML.rank_scan);
+  mp.views = reinterpret_cast<MatView*>(sp + ML.views);
+  mp.large_count = reinterpret_cast<uint32_t*>(sp + ML.large);
+  mp.n_L = reinterpret_cast<unsigned long long*>(sp + ML.misc);
+  mp.n_words = (int)(d.n_tile / 32);
+  // Matrix class: ring-interval path, tile bitmaps that fit a block's shared memory next to the ring table, and discs large enough
+  // that a bitmap row (about 5 passes over n_tile / 8 bytes) is cheaper than the disc's pairs through emit + radix sort + ranges
+  // (about 90 B per pair): tiles >= n_tile / 144.
+  const size_t smem_m = q.smem_block + (size_t)mp.n_words * 4;
+  const bool mat_ok = q.ring_impl && d.kt >= 2 && smem_m <= 220 * 1024 && ML.cap_rows > 0 && !getenv("UTS_NO_MATRIX");
+  if (mat_ok) {
+    const char* e = getenv("UTS_MAT_TILES");
+    const double tiles_min = e ? atof(e) : fmax(48.0, (double)d.n_tile / 144.0);
+    const double cosR = 1.0 - 2.0 * tiles_min / (double)d.n_tile;           // cap of tiles_min tiles: n_tile (1 - cos R) / 2
+    q.b_mat = cosR <= -1.0 ? -1 : radius_bucket_host((float)acos(cosR));
+    if (q.b_mat > q.qp.b_block) q.b_mat = q.qp.b_block;                     // only discs of the block-per-disc class
+    q.cap_rows = ML.cap_rows;
+  }
+  uint32_t* flag_by_rank = reinterpret_cast<uint32_t*>(sp + ML.flag);
+  uint64_t* scan_sums = reinterpret_cast<uint64_t*>(sp + ML.scan);
+  if ((st = q.count(offsets, mat_ok ? &mp : nullptr, flag_by_rank, reinterpret_cast<uint64_t*>(sp + ML.rank_scan), scan_sums))) return st;
+  // host needs: small pairs, matrix pairs, matrix rows
+  uint64_t h3[3] = {0, 0, 0};
+  UTS_CUDA(cudaMemcpyAsync(&h3[0], offsets + n, 8, cudaMemcpyDeviceToHost, s));
+  if (mat_ok) {
+    UTS_CUDA(cudaMemcpyAsync(&h3[1], mp.n_L, 8, cudaMemcpyDeviceToHost, s));
+    UTS_CUDA(cudaMemcpyAsync(&h3[2], mp.row_of_rank + n, 8, cudaMemcpyDeviceToHost, s));
+  }
+  UTS_CUDA(cudaStreamSynchronize(s));
+  const uint64_t n_S = h3[0], n_L = h3[1], n_mat = h3[2];
+  *h_n_pairs = n_S + n_L;
+  if (*h_n_pairs > capacity) return UTS_ERR_CAPACITY;
+  if (sort_scratch_bytes < uts_sort_scratch_bytes(n_S)) return UTS_ERR_INVALID_ARG;
+  if (n_L == 0) {                                     // no large discs: the plain sequence
+    if (n_S) {
+      if ((st = q.emit(offsets, keys, vals))) return st;
+      if ((st = uts_sort(cfg, n_S, keys, vals, keys_tmp, vals_tmp, 1, sort_scratch, sort_scratch_bytes, stream))) return st;
+    }
+    return uts_tile_ranges(cfg, n_S, keys, ranges, stream);
+  }
+  // ---- large discs: transpose the bit matrix, count per (view, tile)
+  {
+    dim3 grid((unsigned)((mp.n_words + 31) / 32), (unsigned)(n_mat / 256 + (uint64_t)d.V + 1));
+    matrix_transpose_kernel<<<grid, 256, 0, s>>>(mp, d.V, d.n_tile);
+    UTS_LAUNCH_CHECK();
+    matrix_popcount_kernel<<<(unsigned)sm_count() * 8, 256, 0, s>>>(mp, d.V, d.n_tile);
+    UTS_LAUNCH_CHECK();
+  }
+  // ---- small discs: emit at keys_tmp / vals_tmp, sort there (ping-pong through keys / vals, free until the merge), their ranges
+  uint64_t* s_ranges = reinterpret_cast<uint64_t*>(sp + ML.sranges);
+  if (n_S) {
+    if ((st = q.emit(offsets, keys_tmp, vals_tmp))) return st;
+    if ((st = uts_sort(cfg, n_S, keys_tmp, vals_tmp, keys, vals, 1, sort_scratch, sort_scratch_bytes, stream))) return st;
+  }
+  if ((st = uts_tile_ranges(cfg, n_S, keys_tmp, s_ranges, stream))) return st;
+  // ---- final ranges, then one warp per (view, tile) merges its large discs (bit vector) with its small pairs into keys / vals
+  uint32_t* total = reinterpret_cast<uint32_t*>(sp + ML.total);
+  uint64_t* start = reinterpret_cast<uint64_t*>(sp + ML.start);
+  mat_totals_kernel<<<(unsigned)((nvt + 255) / 256), 256, 0, s>>>(nvt, mp.large_count, s_ranges, total);
+  UTS_LAUNCH_CHECK();
+  if ((st = exclusive_scan_u32(total, nvt, start, scan_sums, s))) return st;
+  mat_ranges_kernel<<<(unsigned)((nvt + 255) / 256), 256, 0, s>>>(nvt, start, ranges);
+  UTS_LAUNCH_CHECK();
+  matrix_emit_merge_kernel<<<(unsigned)sm_count() * 8, 256, 0, s>>>(mp, d.V, d.n_tile, start, s_ranges, keys_tmp, vals_tmp, keys, vals);
   UTS_LAUNCH_CHECK();
   return UTS_OK;
 }

@@ -17,7 +17,8 @@ class Rasterizer:
     """Holds every buffer of one configuration.  forward() / backward() enqueue on torch's current stream; the only host
     synchronisation is the pair count returned by uts_tile_query."""
 
-    def __init__(self, cfg: B.Config, mask: B.Mask | None = None, device="cuda", pair_capacity: int = 0, depth_presort: bool = True):
+    def __init__(self, cfg: B.Config, mask: B.Mask | None = None, device="cuda", pair_capacity: int = 0, depth_presort: bool = True,
+                 fused_lists: bool = True):
         B.lib()
         if not torch.cuda.is_available():
             raise RuntimeError("uts: a CUDA device is required (no CPU fallback)")
@@ -27,7 +28,9 @@ class Rasterizer:
         npx = self.S * cfg.ppt
         self.proj = B.Proj.empty(cfg, device)
         self.offsets = _i64(V * P + 1, device)
-        self.tq_scratch = _bytes(B.uts_tile_query_scratch_bytes(cfg), device)
+        # fused_lists: uts_tile_lists (query + sort + ranges in one call, large discs emitted tile-major) instead of the three calls
+        self.fused_lists = bool(fused_lists) and depth_presort
+        self.tq_scratch = _bytes(B.uts_tile_lists_scratch_bytes(cfg) if self.fused_lists else B.uts_tile_query_scratch_bytes(cfg), device)
         # depth_presort: order the Gaussians by radial depth first so that the pair sort only runs its (view,tile) passes
         self.depth_presort = depth_presort
         self.emit_rank = _i32(max(V * P, 1), device) if depth_presort else None
@@ -67,6 +70,19 @@ class Rasterizer:
                                             self.emit_rank)
         return self.n_pairs
 
+    def tile_lists(self):
+        """uts_tile_lists: sorted keys / vals and ranges in one call (needs the depth order)."""
+        args = lambda: (self.cfg, self.proj, self.mask, self.emit_rank, self.keys, self.vals, self.keys_tmp, self.vals_tmp, self.capacity, self.ranges,
+                        self.tq_scratch, self.sort_scratch)
+        try:
+            self.n_pairs = B.uts_tile_lists(*args())
+        except B.UtsError as e:
+            if e.status != B.UTS_ERR_CAPACITY:
+                raise
+            self._alloc_pairs(int(e.needed * 1.05) + 1024)
+            self.n_pairs = B.uts_tile_lists(*args())
+        return self.n_pairs
+
     def sort(self):
         B.uts_sort(self.cfg, self.n_pairs, self.keys, self.vals, self.keys_tmp, self.vals_tmp, self.sort_scratch, self.depth_presort)
     def tile_ranges(self): B.uts_tile_ranges(self.cfg, self.n_pairs, self.keys, self.ranges)
@@ -94,9 +110,12 @@ class Rasterizer:
     def forward(self, g, views):
         self.preprocess(g, views)
         self.depth_order()
-        self.tile_query()
-        self.sort()
-        self.tile_ranges()
+        if self.fused_lists:
+            self.tile_lists()
+        else:
+            self.tile_query()
+            self.sort()
+            self.tile_ranges()
         self.render_fwd()
         return self.color, self.alpha
 

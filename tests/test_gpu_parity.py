@@ -551,3 +551,51 @@ def test_invalid_arguments_are_reported():
     assert ei.value.status == B.UTS_ERR_UNSUPPORTED
     with pytest.raises(RuntimeError):
         B.uts_tile_ranges(B.Config(order=6, n_gauss=1), 1, torch.zeros(1, dtype=torch.int64), torch.zeros(4, dtype=torch.int64, device="cuda"))
+
+
+# ------------------------------------------------------------------------------------------- F2 + F3 + F4 fused
+@pytest.mark.parametrize("mat_tiles", [None, "3", "40"], ids=["default-threshold", "matrix-from-3-tiles", "matrix-from-40-tiles"])
+@pytest.mark.parametrize("cfg_id,P,order,extra", CASES + [pytest.param(4, 3000, 8, {"n_views": 3}, id="cfg4-3views-order8"),
+                                                          pytest.param(3, 4000, 6, {}, id="cfg3-cap-mask-order6")])
+def test_tile_lists_bit_exact(cfg_id, P, order, extra, mat_tiles, monkeypatch):
+    """uts_tile_lists (large discs through the bit matrix, small discs through emit + sort, per-tile merge) against the oracle's
+    sorted pairs and ranges, bit for bit; the matrix threshold is moved so that few, most or nearly all discs take the matrix."""
+    B, R = _gpu()
+    if mat_tiles is None:
+        monkeypatch.delenv("UTS_MAT_TILES", raising=False)
+    else:
+        monkeypatch.setenv("UTS_MAT_TILES", mat_tiles)
+    c = Case.get(cfg_id, P, order, extra)
+    cfg = _cfg(R, c.scene)
+    r = R.Rasterizer(cfg, c.gpu_mask(B), fused_lists=True, pair_capacity=16)          # tiny capacity: exercises UTS_ERR_CAPACITY + regrow
+    r.proj = c.gpu_proj(B)
+    r.depth_order()
+    n = r.tile_lists()
+    assert n == c.fw["skeys"].shape[0]
+    assert np.array_equal(u64(r.keys)[:n], c.fw["skeys"])
+    assert np.array_equal(u32(r.vals)[:n], c.fw["svals"])
+    assert np.array_equal(u64(r.ranges), c.fw["ranges"])
+
+
+def test_tile_lists_whole_sphere_discs_and_empty(monkeypatch):
+    """Whole-sphere discs (reading A24) as matrix rows, with and without a mask; culled Gaussians; P = 0."""
+    B, R = _gpu()
+    monkeypatch.setenv("UTS_MAT_TILES", "8")
+    scene = small_scene(3, 600, 6)
+    scene["scales"][:40] *= 400.0                                     # r_s = pi
+    scene["means"][40:60] *= 1e-3                                     # inside r_near: culled
+    oc = ocfg(scene)
+    bits, act, slot = oracle_mask(oc, scene)
+    fw = orc.forward_chain(oc, scene, slot, act, bits)
+    assert (fw["proj"].rs >= 3.14159).sum() >= 15 and (fw["proj"].flags & 1).sum() >= 20
+    cfg = _cfg(R, scene)
+    mask = B.Mask(dev(act.view(np.int32)), int(act.shape[0]), dev(slot), dev(bits.view(np.int32)))
+    g, views = R.scene_to_device(scene)
+    r = R.Rasterizer(cfg, mask, fused_lists=True)
+    r.preprocess(g, views); r.depth_order()
+    n = r.tile_lists()
+    assert n == fw["skeys"].shape[0] and np.array_equal(u64(r.keys)[:n], fw["skeys"]) and np.array_equal(u32(r.vals)[:n], fw["svals"])
+    assert np.array_equal(u64(r.ranges), fw["ranges"])
+    cfg0 = B.Config(order=6, n_gauss=0)
+    r0 = R.Rasterizer(cfg0, fused_lists=True)
+    assert r0.tile_lists() == 0 and int(r0.ranges.abs().sum()) == 0

@@ -31,25 +31,53 @@ __device__ __forceinline__ float ex2_approx(float x) {
   return y;
 }
 
+// Bare MUFU forms (no denormal / range fix-up code around them: the arguments here are never denormal or huge).
+__device__ __forceinline__ float rsqrt_approx(float x) {
+  float y;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float rcp_approx(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+// Broadcast reads of the staged entries with the shared-window address kept in a register by the caller.
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ float2 lds64(uint32_t addr) {
+  float2 v;
+  asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+  return v;
+}
+
 // k = d_gc / sin(d_gc).  For cos(d_gc) = c >= 0:  acos(c) = sqrt(1-c) P(c) with P analytic on [0,1], so
-// k = acos(c) / sqrt((1-c)(1+c)) = P(c) rsqrt(1+c): no cancellation (1-c never formed), no branch, one MUFU.
+// k = acos(c) / sqrt((1-c)(1+c)) = P(c) rsqrt(1+c): no cancellation (1-c never formed), one MUFU.
 // P is a degree-7 Chebyshev fit of acos(c)/sqrt(1-c) on [0,1] (own fit; max relative error of k in fp32: 1.7e-7).
-// Beyond 90 degrees (c < 0; only the far tail of very large Gaussians) fall back to atan2f on sin = sqrt(t).
+// Beyond 90 degrees (c < 0; only the far tail of very large Gaussians): acos(c) = pi - acos(|c|) and
+// sqrt(1-|c|) = sin / sqrt(1+|c|), so k = (pi - sin P(|c|) rsqrt(1+|c|)) / sin with sin = sqrt(t): still no cancellation.
+// That branch is out of line so that the common path stays straight.
+__device__ __forceinline__ float acos_poly(float c) {
+  float p = -0.00115729403f;
+  p = fmaf(p, c, 0.00628544204f);
+  p = fmaf(p, c, -0.016528869f);
+  p = fmaf(p, c, 0.0304812621f);
+  p = fmaf(p, c, -0.0500148833f);
+  p = fmaf(p, c, 0.0889478773f);
+  p = fmaf(p, c, -0.214596227f);
+  return fmaf(p, c, 1.57079625f);
+}
+__device__ __noinline__ float arc_over_sin_far(float t, float c) {
+  if (!(t > 0.f)) return 1.0f;                      // antipode: never reached by a finite conic (alpha underflows first)
+  const float is = rsqrt_approx(t), s = t * is, ac = -c;
+  return (3.14159274f - s * acos_poly(ac) * rsqrt_approx(1.0f + ac)) * is;
+}
 __device__ __forceinline__ float arc_over_sin(float t, float c) {
-  if (c >= 0.f) {
-    float p = -0.00115729403f;
-    p = fmaf(p, c, 0.00628544204f);
-    p = fmaf(p, c, -0.016528869f);
-    p = fmaf(p, c, 0.0304812621f);
-    p = fmaf(p, c, -0.0500148833f);
-    p = fmaf(p, c, 0.0889478773f);
-    p = fmaf(p, c, -0.214596227f);
-    p = fmaf(p, c, 1.57079625f);
-    return p * rsqrtf(1.0f + c);
-  }
-  if (!(t > 0.f)) return 1.0f;
-  const float s = sqrtf(t);
-  return atan2f(s, c) / s;
+  if (c >= 0.f) return acos_poly(c) * rsqrt_approx(1.0f + c);
+  return arc_over_sin_far(t, c);
 }
 
 // What one (tile, Gaussian) list entry contributes to every pixel of the tile, staged once per entry.
@@ -104,7 +132,7 @@ __device__ __forceinline__ void eval_entry(const float4 f0, const float4 f1, con
   ev.c = fmaf(f2.y, px, fmaf(f2.z, py, fmaf(f2.w, pz, f0.z)));
   ev.t = fmaf(ev.a, ev.a, ev.b * ev.b);
   ev.k = arc_over_sin(ev.t, ev.c);
-  const float q = fmaf(f3.x * ev.a, ev.a, fmaf(f3.y * ev.a, ev.b, f3.z * ev.b * ev.b));
+  const float q = fmaf(ev.a, fmaf(f3.x, ev.a, f3.y * ev.b), f3.z * ev.b * ev.b);     // qa a^2 + qb a b + qc b^2
   ev.p2 = q * ev.k * ev.k;
 }
 
@@ -145,6 +173,7 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
   uint32_t n_last = 0;
   bool done = !ps.on;
   const uint64_t len = ps.end - ps.start;
+  const uint32_t sS = (uint32_t)__cvta_generic_to_shared(&S);
   for (uint64_t b0 = 0; b0 < len; b0 += kTilePix) {
     if (__syncthreads_and(done)) break;               // every pixel of the tile saturated (or masked)
     const uint64_t j = b0 + threadIdx.x;
@@ -155,23 +184,33 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
                   __ldg(reinterpret_cast<const float4*>(conic_opac) + gi), __ldg(rgb + 3 * gi), __ldg(rgb + 3 * gi + 1),
                   __ldg(rgb + 3 * gi + 2), E);
       put_entry(S, threadIdx.x, E);
+    } else if (j < len + 3) {
+      // null entries pad the list to a multiple of 4: a = 1, qa = 1 give power > 0, which Alg.1 l.23 skips whatever the thresholds
+      S.f0[threadIdx.x] = make_float4(1.f, 0.f, 0.f, 0.f); S.f1[threadIdx.x] = make_float4(0.f, 0.f, 0.f, 0.f);
+      S.f2[threadIdx.x] = make_float4(0.f, 0.f, 0.f, 0.f); S.f3[threadIdx.x] = make_float4(1.f, 0.f, 0.f, 0.f);
     }
     __syncthreads();
     const int nb = (int)((len - b0) < (uint64_t)kTilePix ? (len - b0) : (uint64_t)kTilePix);
-    for (int jj = 0; jj < nb; ++jj) {
+    // four entries per warp vote: the vote only ends the walk early, every skip / clamp decision is per lane
+    for (int j4 = 0; j4 < nb; j4 += 4) {
       if (__all_sync(0xffffffffu, done)) break;       // warp vote: the whole 8x4 patch is saturated
-      const float4 f0 = S.f0[jj], f1 = S.f1[jj], f2 = S.f2[jj], f3 = S.f3[jj];
-      Eval ev;
-      eval_entry(f0, f1, f2, f3, ps.px, ps.py, ps.pz, ev);
-      if (done || ev.p2 > 0.f) continue;              // Alg.1 l.23: power > 0 skipped (reading A7)
-      const float a = fminf(rp.amax, f0.w * ex2_approx(ev.p2));
-      if (a < rp.amin) continue;
-      const float2 f4 = S.f4[jj];
-      const float w = T * a;                          // Eq.6: c_i alpha_i prod_{j<i} (1 - alpha_j)
-      Cr = fmaf(w, f3.w, Cr); Cg = fmaf(w, f4.x, Cg); Cb = fmaf(w, f4.y, Cb);
-      T = T * (1.f - a);
-      n_last = (uint32_t)(b0 + jj) + 1u;
-      if (T < rp.teps) done = true;                   // Alg.1 l.27: test after the update
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int jj = j4 + u;
+        const uint32_t sa = sS + (uint32_t)jj * 16u;
+        const float4 f0 = lds128(sa), f1 = lds128(sa + 0x1000u), f2 = lds128(sa + 0x2000u), f3 = lds128(sa + 0x3000u);
+        Eval ev;
+        eval_entry(f0, f1, f2, f3, ps.px, ps.py, ps.pz, ev);
+        if (done || ev.p2 > 0.f) continue;            // Alg.1 l.23: power > 0 skipped (reading A7)
+        const float a = fminf(rp.amax, f0.w * ex2_approx(ev.p2));
+        if (a < rp.amin) continue;
+        const float2 f4 = lds64(sS + 0x4000u + (uint32_t)jj * 8u);
+        const float w = T * a;                        // Eq.6: c_i alpha_i prod_{j<i} (1 - alpha_j)
+        Cr = fmaf(w, f3.w, Cr); Cg = fmaf(w, f4.x, Cg); Cb = fmaf(w, f4.y, Cb);
+        T = T * (1.f - a);
+        n_last = (uint32_t)(b0 + jj) + 1u;
+        if (T < rp.teps) done = true;                 // Alg.1 l.27: test after the update
+      }
     }
   }
   if (ps.on) {
@@ -227,6 +266,13 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
   for (int w = 0; w < kTilePix / 32; ++w) max_nl = max(max_nl, s_max[w]);
   if (max_nl == 0) return;
 
+  // the gradient word this lane owns after the butterfly below (lanes 4j: value j), as base pointer + stride per Gaussian:
+  // bit4 -> +4, bit3 -> +2, bit2 -> +1  (0 r, 1 g, 2 b, 3 A, 4 B, 5 C, 6 omega, 7 phi)
+  const int vi = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
+  float* const lane_dst = (vi < 3 ? dL_drgb + vi : vi < 6 ? dL_dconic + (vi - 3) : dL_dmu2 + (vi - 6)) + (size_t)(vi < 6 ? 3 : 2) * gbase;
+  const uint32_t lane_stride = vi < 6 ? 3u : 2u;
+  const uint32_t sS = (uint32_t)__cvta_generic_to_shared(&S);
+
   float T = Tfin;                                      // transmittance after the entry being visited
   float Sr = Tfin * rp.bg[0], Sg = Tfin * rp.bg[1], Sb = Tfin * rp.bg[2];                // colour accumulated behind it
   const int n_batch = (int)((max_nl + kTilePix - 1) / kTilePix);
@@ -254,7 +300,8 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
       const uint32_t jl = b0 + (uint32_t)jj;
       const bool reach = jl < nl;                      // this pixel's forward pass got this far
       if (!__any_sync(0xffffffffu, reach)) continue;
-      const float4 f0 = S.f0[jj], f1 = S.f1[jj], f2 = S.f2[jj], f3 = S.f3[jj], f5 = S.f5[jj];
+      const uint32_t sa = sS + (uint32_t)jj * 16u;
+      const float4 f0 = lds128(sa), f1 = lds128(sa + 0x1000u), f2 = lds128(sa + 0x2000u), f3 = lds128(sa + 0x3000u), f5 = lds128(sa + 0x4000u);
       Eval ev;
       eval_entry(f0, f1, f2, f3, ps.px, ps.py, ps.pz, ev);
       float e2 = 0.f, raw = 0.f, a = 0.f;
@@ -263,7 +310,7 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
       if (!__any_sync(0xffffffffu, used)) continue;
       float d_r = 0.f, d_g = 0.f, d_b = 0.f, d_A = 0.f, d_B = 0.f, d_C = 0.f, d_o = 0.f, d_om = 0.f, d_ph = 0.f;
       if (used) {
-        const float inv1a = __frcp_rn(1.f - a);
+        const float inv1a = rcp_approx(1.f - a);
         const float Tb = T * inv1a;                    // transmittance before this entry
         const float w = Tb * a;
         d_r = w * gr; d_g = w * gg; d_b = w * gb;
@@ -282,8 +329,8 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
           if (ev.t > 0.f) {
             const float den = ev.t + ev.c * ev.c;
             const float gk = gdx * ev.a + gdy * ev.b;
-            const float iden = __frcp_rn(den);
-            const float kp = __fdividef(ev.c * iden - ev.k, ev.t);
+            const float iden = rcp_approx(den);
+            const float kp = (ev.c * iden - ev.k) * rcp_approx(ev.t);
             g_a = fmaf(gk * kp, ev.a, ev.k * gdx);
             g_b = fmaf(gk * kp, ev.b, ev.k * gdy);
             g_c = -gk * iden;
@@ -321,14 +368,8 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
       v0 += __shfl_xor_sync(0xffffffffu, v0, 1);
       d_o = warp_sum(d_o);
       {
-        // value index owned by this lane: bit4 -> +4, bit3 -> +2, bit2 -> +1  (0 r, 1 g, 2 b, 3 A, 4 B, 5 C, 6 omega, 7 phi)
-        const int vi = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
         const uint32_t id = S.id[jj];
-        const size_t gi = gbase + id;
-        if ((lane & 3) == 0) {
-          float* dst = vi < 3 ? dL_drgb + 3 * gi + vi : vi < 6 ? dL_dconic + 3 * gi + (vi - 3) : dL_dmu2 + 2 * gi + (vi - 6);
-          atomicAdd(dst, v0);
-        }
+        if ((lane & 3) == 0) atomicAdd(lane_dst + (size_t)id * lane_stride, v0);
         if (lane == 1) atomicAdd(dL_dopac + id, d_o);
       }
     }

@@ -48,6 +48,9 @@ __device__ __forceinline__ float4 lds128(uint32_t addr) {
   asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
   return v;
 }
+__device__ __forceinline__ void red_add_global(float* p, float v) {       // p is a global address (cudaMalloc'ed gradient buffer)
+  asm volatile("red.global.add.f32 [%0], %1;" :: "l"(p), "f"(v) : "memory");
+}
 __device__ __forceinline__ float2 lds64(uint32_t addr) {
   float2 v;
   asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
@@ -269,8 +272,11 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
   // the gradient word this lane owns after the butterfly below (lanes 4j: value j), as base pointer + stride per Gaussian:
   // bit4 -> +4, bit3 -> +2, bit2 -> +1  (0 r, 1 g, 2 b, 3 A, 4 B, 5 C, 6 omega, 7 phi)
   const int vi = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
-  float* const lane_dst = (vi < 3 ? dL_drgb + vi : vi < 6 ? dL_dconic + (vi - 3) : dL_dmu2 + (vi - 6)) + (size_t)(vi < 6 ? 3 : 2) * gbase;
-  const uint32_t lane_stride = vi < 6 ? 3u : 2u;
+  float* lane_dst = (vi < 3 ? dL_drgb + vi : vi < 6 ? dL_dconic + (vi - 3) : dL_dmu2 + (vi - 6)) + (size_t)(vi < 6 ? 3 : 2) * gbase;
+  uint32_t lane_stride = vi < 6 ? 3u : 2u;
+  if (lane == 1) { lane_dst = dL_dopac; lane_stride = 1u; }                    // lane 1 owns the opacity sum (summed over views)
+  const bool lane_owns = (lane & 3) == 0 || lane == 1;
+  asm volatile("" : "+l"(lane_dst));                   // keep the per-view base folded into the pointer (one IMAD.WIDE per atomic)
   const uint32_t sS = (uint32_t)__cvta_generic_to_shared(&S);
 
   float T = Tfin;                                      // transmittance after the entry being visited
@@ -369,8 +375,7 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
       d_o = warp_sum(d_o);
       {
         const uint32_t id = S.id[jj];
-        if ((lane & 3) == 0) atomicAdd(lane_dst + (size_t)id * lane_stride, v0);
-        if (lane == 1) atomicAdd(dL_dopac + id, d_o);
+        if (lane_owns) red_add_global(lane_dst + (size_t)id * lane_stride, lane == 1 ? d_o : v0);
       }
     }
   }

@@ -16,8 +16,8 @@ from dataclasses import dataclass, field
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SRCS = ["orc_healpix.cpp", "orc_raster.cpp", "orc_resample.cpp", "orc_depth.cpp", "orc_capi.cpp"]
-_HDRS = ["orc_healpix.hpp", "orc_raster.hpp", "orc_resample.hpp"]
+_SRCS = ["orc_healpix.cpp", "orc_raster.cpp", "orc_resample.cpp", "orc_depth.cpp", "orc_hssim.cpp", "orc_capi.cpp"]
+_HDRS = ["orc_healpix.hpp", "orc_raster.hpp", "orc_resample.hpp", "orc_hssim.hpp"]
 _LIB = os.path.join(_HERE, "liboracle.so")
 
 
@@ -259,6 +259,33 @@ def rs_max_update(rs, flags, rs_max):
     out = _f32(rs_max).copy()
     lib().orc_rs_max_update(C.c_int(V), C.c_int(P), _p(r), _p(fl), _p(out))
     return out
+
+
+# ------------------------------------------------------------------ L1 + HEALPix-SSIM loss (orc_hssim.cpp, NEXT-3)
+def hssim_neighbor(order, p, dx, dy):
+    """(pixel at offset (dx,dy) in p's face frame or -1, quarter turns of the axes)  — reading A30."""
+    lib().orc_hssim_neighbor.restype = C.c_int64
+    rot = C.c_int(0)
+    q = lib().orc_hssim_neighbor(C.c_int(order), C.c_int64(int(p)), C.c_int(dx), C.c_int(dy), C.byref(rot))
+    return int(q), int(rot.value)
+
+
+def hssim_weight(face, dx, dy, sigma=1.5):
+    lib().orc_hssim_weight.restype = C.c_double
+    return float(lib().orc_hssim_weight(C.c_int(face), C.c_int(dx), C.c_int(dy), C.c_double(sigma)))
+
+
+def hssim_loss(order, X, G, slot_of_tile=None, bits=None, lam=0.2, sigma=1.5, grad=True):
+    """X, G [n_slot*256, 3] fp32 (slot layout).  Returns dict(loss, l1, hssim, h_map [n_slot*256], grad [n_slot*256, 3] or None)."""
+    Xf, Gf = _f32(X), _f32(G)
+    n_store = Xf.shape[0]
+    st = None if slot_of_tile is None else np.ascontiguousarray(slot_of_tile, dtype=np.int32)
+    bt = None if bits is None else np.ascontiguousarray(bits, dtype=np.uint32)
+    h = np.zeros(n_store); g = np.zeros((n_store, 3)) if grad else None
+    out = np.zeros(3)
+    lib().orc_hssim_loss(C.c_int(order), _p(st), _p(bt), C.c_int64(n_store // 256), _p(Xf), _p(Gf), C.c_double(lam), C.c_double(sigma),
+                         _p(h), _p(g), _p(out))
+    return dict(loss=float(out[0]), l1=float(out[1]), hssim=float(out[2]), h_map=h, grad=g)
 
 
 # ------------------------------------------------------------------ stages (fp32 ABI arrays)

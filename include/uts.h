@@ -11,6 +11,7 @@
  *   uts_render_fwd      Alg.1 l.17-30 (Eq.6) + FoV mask
  *   uts_render_bwd      backward of Eq.6
  *   uts_preprocess_bwd  Eq.3-4: to means, scales, rotations, SH
+ *   uts_hssim_loss      L1 + HEALPix-SSIM loss and dL/dI (Eq.10): produces uts_render_bwd's upstream gradient
  *
  * Conventions
  *   - extern "C"; every call returns an int status (UTS_OK = 0).  Nothing throws, aborts, allocates or frees
@@ -230,6 +231,23 @@ int uts_inv_depth_bwd(const uts_config* cfg, const float* means, uts_views views
 /* Radian-space density control buffer: rs_max[i] <- max(rs_max[i], rs[v,i]) over the views in which Gaussian i
  * is visible (not culled by uts_preprocess).  rs, flags: uts_preprocess's records; rs_max [P], caller-initialised. */
 int uts_rs_max_update(const uts_config* cfg, const float* rs, const uint8_t* flags, float* rs_max, void* stream);
+
+/* ------------------------------------------------------- L1 + HEALPix-SSIM loss */
+
+/* L = (1 - lambda) L1^H + lambda (1 - HSSIM), HSSIM = sum_q M(q) h_q / sum_q M(q) (Eq.10), and its
+ * gradient with respect to the rendered image, in one pass.  X (rendered) and G (ground truth): [S*256, 3] fp32 in the slot layout
+ * of uts_render_fwd, one view.  h_q is the SSIM index (C1 = 0.01^2, C2 = 0.03^2, mean over the 3 channels) of the 11 x 11 window
+ * around q in the (x,y) grid of q's base face, continued across face edges into the neighbouring faces ("cross-face padding",
+ * PAPER.md:143; reading A30); taps that do not exist (the quadrant beyond a vertex shared by 3 faces) or have
+ * M_C = 0 are dropped and the remaining weights renormalised (A32).  Weights: Gaussian of width `sigma` pixels, isotropic on the
+ * equatorial faces 4..7, stretched pi/4 : 4/pi along the pixel diagonals on the polar faces (reading A31).
+ * Outputs: loss3 [3] DEVICE doubles (L, L1^H, HSSIM); h_map [S*256] h_q, 0 where M_C = 0 (may be NULL); dL_dX [S*256, 3] (may be
+ * NULL: forward only), zeroed by the call and accumulated with atomics (summation order is not deterministic).
+ * L1^H = sum_q M(q) sum_ch |X - G| / (3 sum_q M(q)) (A34); lambda in [0,1] (0.2 in 3DGS, A35); sigma > 0 (1.5, A31).
+ * scratch: uts_hssim_scratch_bytes(cfg) bytes, 8-byte aligned.  Asynchronous on `stream`. */
+size_t uts_hssim_scratch_bytes(const uts_config* cfg);
+int uts_hssim_loss(const uts_config* cfg, uts_mask mask, const float* X, const float* G, float lambda, float sigma, float* h_map,
+                   float* dL_dX, double* loss3, void* scratch, size_t scratch_bytes, void* stream);
 
 /* NESTED pixel centres as camera-frame unit vectors, double [n,3], pixels first..first+n-1 at `order`
  * (exposes the library's HEALPix indexing for tests). */

@@ -21,7 +21,7 @@ UTS_OK, UTS_ERR_INVALID_ARG, UTS_ERR_CAPACITY, UTS_ERR_CUDA, UTS_ERR_UNSUPPORTED
 SYMBOLS = [
     "uts_preprocess", "uts_depth_order", "uts_depth_order_scratch_bytes", "uts_tile_query", "uts_tile_query_scratch_bytes", "uts_tile_lists", "uts_tile_lists_scratch_bytes", "uts_sort", "uts_sort_scratch_bytes",
     "uts_tile_ranges", "uts_render_fwd", "uts_render_bwd", "uts_preprocess_bwd", "uts_build_mask", "uts_pixel_centers",
-    "uts_rho_max_table", "uts_resample_fwd", "uts_resample_bwd", "uts_build_camera_mask", "uts_inv_depth_channel", "uts_inv_depth_bwd", "uts_rs_max_update",
+    "uts_rho_max_table", "uts_resample_fwd", "uts_resample_bwd", "uts_build_camera_mask", "uts_inv_depth_channel", "uts_inv_depth_bwd", "uts_rs_max_update", "uts_hssim_loss", "uts_hssim_scratch_bytes",
     "uts_host_workspace_bytes", "uts_host_forward_backward", "uts_last_cuda_error", "uts_launch_count", "uts_strerror",
     "uts_version",
 ]
@@ -107,7 +107,7 @@ def lib():
         L = C.CDLL(LIB_PATH)
         L.uts_strerror.restype = C.c_char_p
         L.uts_version.restype = C.c_char_p
-        for n in ("uts_depth_order_scratch_bytes", "uts_tile_query_scratch_bytes", "uts_sort_scratch_bytes", "uts_host_workspace_bytes"):
+        for n in ("uts_hssim_scratch_bytes", "uts_depth_order_scratch_bytes", "uts_tile_query_scratch_bytes", "uts_sort_scratch_bytes", "uts_host_workspace_bytes"):
             getattr(L, n).restype = C.c_size_t
         L.uts_sort_scratch_bytes.argtypes = [C.c_uint64]
         L.uts_host_workspace_bytes.argtypes = [C.POINTER(CConfig), C.c_int, C.c_uint64]
@@ -362,6 +362,23 @@ def uts_build_camera_mask(cfg: Config, cam: Camera, device="cuda", stream=None) 
     _check(lib().uts_build_camera_mask(C.byref(c), cam.c(), _ptr(bits), _ptr(slot), _ptr(act), C.byref(n), _stream(stream)),
            "uts_build_camera_mask")
     return Mask(act[: n.value].contiguous(), int(n.value), slot, bits)
+
+
+def uts_hssim_scratch_bytes(cfg: Config) -> int:
+    c = cfg.c()
+    return int(lib().uts_hssim_scratch_bytes(C.byref(c)))
+
+
+def uts_hssim_loss(cfg: Config, mask: Mask, X, G, loss3, scratch, h_map=None, dL_dX=None, lam=0.2, sigma=1.5, stream=None):
+    """L = (1 - lam) L1^H + lam (1 - HSSIM) and dL/dX (PAPER.md:135-143, Eq.10).  X, G [S*256, 3]; loss3 [3] float64 (device)."""
+    c = cfg.c()
+    n = mask.n_slots(cfg) * 256
+    assert tuple(X.shape) == (n, 3) and tuple(G.shape) == (n, 3) and loss3.numel() == 3
+    assert h_map is None or h_map.numel() == n
+    assert dL_dX is None or tuple(dL_dX.shape) == (n, 3)
+    _check(lib().uts_hssim_loss(C.byref(c), mask.c(), _ptr(X, torch.float32), _ptr(G, torch.float32), C.c_float(lam), C.c_float(sigma),
+                                _ptr(h_map, torch.float32), _ptr(dL_dX, torch.float32), _ptr(loss3, torch.float64), _ptr(scratch),
+                                C.c_size_t(scratch.numel() * scratch.element_size()), _stream(stream)), "uts_hssim_loss")
 
 
 def uts_pixel_centers(order: int, first: int, n: int, device="cuda", stream=None):

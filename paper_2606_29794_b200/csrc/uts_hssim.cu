@@ -1,0 +1,310 @@
+// uts_hssim.cu — training loss on the HEALPix grid, forward and backward in one pass.
+//   "L = (1 - lambda) L1^H + lambda L_HSSIM"
+//   "the NESTED (x,y,f) parameterization approximates a local 2D grid ... some corner pixels have only 7 neighbors;
+//    we detect such cases and renormalize kernel weights accordingly ... isotropic for the equatorial zone ...
+//    anisotropic for polar zones"
+//   "shared memory with cross-face padding ... cached derivatives"
+//   HSSIM = sum_q M(q) h_q / sum_q M(q)                                                                   Eq.10
+// Readings A30-A35: 11 x 11 window in the face grid of the centre pixel, continued into the neighbouring faces,
+// taps that do not exist (3-face vertices, M_C = 0) dropped and the weights renormalised, zone of the centre pixel's face,
+// SSIM constants 0.01^2 / 0.03^2, h_q = channel mean.
+//
+// B200 design.  One block per 16 x 16 tile (the rasteriser's slot), 256 threads.  The block stages the 26 x 26 patch of the
+// tile's own face frame — tile plus a 5-pixel apron, the apron resolved through the face-adjacency rules below — in shared
+// memory as (x, g) pairs per channel plus a validity plane.  Every thread then walks the 121 taps of its pixel once for the five
+// window sums per channel (taken about the centre pixel's own value: variances do not lose digits to e11 - m1^2), forms the SSIM
+// index and its derivatives with respect to (m1, s11, s12), and — this is the "transposed convolution" — walks the taps a second
+// time scattering weight * (K0 + K1 (x - m1) + K2 (g - m2)) into a shared gradient patch with shared-memory reductions.  The
+// patch is flushed to dL_dX with one red.global per cell and channel.  The upstream gradient of a loss is 1, so forward and
+// backward share the staged patch and X, G are read from HBM once.  The path is bound by fp32 ALU and shared-memory issue, not
+// by HBM: 121 taps x 3 channels x (9 ALU ops + 1 LDS.64) per pixel forward, 121 x 3 x (5 ALU + LDS.64 + RED.shared) backward,
+// against 24 B of compulsory traffic per pixel.
+#include "uts_internal.cuh"
+
+namespace uts {
+
+constexpr int kHR = 5;                       // window radius (A30)
+constexpr int kHW = 2 * kHR + 1;             // 11
+constexpr int kHTaps = kHW * kHW;            // 121
+constexpr int kHP = 16 + 2 * kHR;            // 26: patch side
+constexpr int kHCells = kHP * kHP;           // 676
+
+struct HssimWeights { float w[2][kHTaps]; }; // [0] equatorial faces, [1] polar faces; tap t = (dy + R) * 11 + (dx + R)
+
+// ---------------------------------------------------------------------------------------------- face adjacency
+// Faces f = 4 r + c: r = 0 north (touching the pole), 1 equatorial, 2 south.  In-face axes: +x points north-east, +y north-west.
+// A cell (X, Y) outside [0, N)^2 of face f lies in another face.  Eight directions o = (ox, oy), ox, oy in {-1, 0, +1}:
+//   - where the neighbour across that edge / vertex has the same axis orientation the step is a translation by N
+//     (every edge of an equatorial face; the two lower edges of a north face; the two upper edges of a south face; the lower
+//     vertex of a north face and the upper vertex of a south face, where 4 faces meet);
+//   - the two upper edges of a north face are meridians glued to the next / previous north face: the coordinate along the edge
+//     becomes the other face's coordinate along ITS glued edge, the depth beyond the edge becomes depth below that edge — a
+//     quarter turn; beyond both (over the pole) two quarter turns.  Mirror image for the lower edges of a south face;
+//   - the left / right vertex of a polar face and the upper / lower vertex of an equatorial face are shared by 3 faces only:
+//     the diagonal quadrant there does not exist.
+// One table entry per (r, oy + 1, ox + 1): kind 0 none, 1 translate, 2..4 quarter turn +1 / two / -1; dr, dc: face row, column step.
+struct FaceStep { int8_t kind, row, dcol; };
+__device__ __constant__ FaceStep kFaceStep[3][3][3] = {
+    // north faces                 ox = -1            ox = 0            ox = +1
+    {/* oy = -1 */ {{1, 2, 0}, {1, 1, 1}, {0, 0, 0}},
+     /* oy =  0 */ {{1, 1, 0}, {1, 0, 0}, {2, 0, 1}},
+     /* oy = +1 */ {{0, 0, 0}, {4, 0, 3}, {3, 0, 2}}},
+    // equatorial faces
+    {/* oy = -1 */ {{0, 0, 0}, {1, 2, 0}, {1, 1, 1}},
+     /* oy =  0 */ {{1, 2, 3}, {1, 1, 0}, {1, 0, 0}},
+     /* oy = +1 */ {{1, 1, 3}, {1, 0, 3}, {0, 0, 0}}},
+    // south faces
+    {/* oy = -1 */ {{3, 2, 2}, {4, 2, 1}, {0, 0, 0}},
+     /* oy =  0 */ {{2, 2, 3}, {1, 2, 0}, {1, 1, 1}},
+     /* oy = +1 */ {{0, 0, 0}, {1, 1, 0}, {1, 0, 0}}},
+};
+
+__device__ __forceinline__ uint32_t spread16(uint32_t v) {          // 16 bits -> even bit positions
+  v = (v | (v << 8)) & 0x00ff00ffu;
+  v = (v | (v << 4)) & 0x0f0f0f0fu;
+  v = (v | (v << 2)) & 0x33333333u;
+  v = (v | (v << 1)) & 0x55555555u;
+  return v;
+}
+
+// NESTED pixel of cell (X, Y) in the extended frame of face f at order k (N = 2^k, -N <= X, Y < 2N), or -1.
+__device__ __forceinline__ int64_t cell_to_pixel(int k, int f, int X, int Y) {
+  const int N = 1 << k;
+  const int ox = X < 0 ? -1 : (X >= N ? 1 : 0), oy = Y < 0 ? -1 : (Y >= N ? 1 : 0);
+  const FaceStep s = kFaceStep[f >> 2][oy + 1][ox + 1];
+  if (s.kind == 0) return -1;
+  const int pole = (f >> 2) == 0 ? 2 * N - 1 : -1;      // north: the glued edges are x = N, y = N; south: x = -1, y = -1
+  int x, y;
+  switch (s.kind) {
+    case 1: x = X - ox * N; y = Y - oy * N; break;       // translation
+    case 2: x = Y; y = pole - X; break;                  // quarter turn: along-edge y -> x, depth beyond x-edge -> depth in y
+    case 4: x = pole - Y; y = X; break;                  // quarter turn the other way
+    default: x = pole - X; y = pole - Y; break;          // over the pole
+  }
+  const int g = 4 * s.row + ((f + s.dcol) & 3);
+  return ((int64_t)g << (2 * k)) | spread16((uint32_t)x) | (spread16((uint32_t)y) << 1);
+}
+
+// storage index (slot layout) of pixel p, or -1 when masked out
+__device__ __forceinline__ int64_t store_index(int64_t p, const int32_t* __restrict__ slot_of_tile, const uint32_t* __restrict__ bits) {
+  if (p < 0) return -1;
+  if (bits && !((__ldg(bits + (p >> 5)) >> (p & 31)) & 1u)) return -1;
+  const int64_t tile = p >> 8;
+  const int64_t slot = slot_of_tile ? (int64_t)__ldg(slot_of_tile + tile) : tile;
+  return slot < 0 ? -1 : slot * 256 + (p & 255);
+}
+
+// ------------------------------------------------------------------------------------------------- count
+// acc[2] = number of valid pixels (Eq.10's denominator): one warp per slot, 8 mask words each.
+__global__ void hssim_count_kernel(int64_t n_slot, const uint32_t* __restrict__ active_tiles, const uint32_t* __restrict__ bits, double* acc) {
+  const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 3;   // 8 lanes per slot
+  const int j = threadIdx.x & 7;
+  int c = 0;
+  if (w < n_slot) {
+    const int64_t tile = active_tiles ? (int64_t)__ldg(active_tiles + w) : w;
+    c = __popc(__ldg(bits + tile * 8 + j));
+  }
+  for (int o = 16; o; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+  if ((threadIdx.x & 31) == 0 && c) atomicAdd(acc + 2, (double)c);
+}
+
+// -------------------------------------------------------------------------------------------------- main
+template <bool GRAD>
+__global__ void __launch_bounds__(256, 3)
+hssim_kernel(int k, int64_t n_pix_full, const uint32_t* __restrict__ active_tiles, const int32_t* __restrict__ slot_of_tile,
+             const uint32_t* __restrict__ bits, const float* __restrict__ X, const float* __restrict__ G, float lambda,
+             const __grid_constant__ HssimWeights wts, float* __restrict__ h_map, float* __restrict__ dL_dX, double* acc) {
+  __shared__ float2 s_xg[3][kHCells];        // (x, g) per channel
+  __shared__ float s_val[kHCells];           // 1 valid, 0 missing
+  __shared__ int s_idx[kHCells];             // storage index (pixels, < 2^31) or -1
+  __shared__ float s_w[kHTaps];
+  __shared__ float s_grad[GRAD ? 3 * kHCells : 1];
+  __shared__ float s_red[2][8];
+
+  const int tid = threadIdx.x;
+  const int64_t slot = blockIdx.x;
+  const int64_t tile = active_tiles ? (int64_t)__ldg(active_tiles + slot) : slot;
+  const int kt = k - kTileLog2;
+  const int f = (int)(tile >> (2 * kt));
+  const uint32_t tm = (uint32_t)(tile & (((int64_t)1 << (2 * kt)) - 1));
+  const int x0 = (int)squeeze_even_bits32(tm) << kTileLog2, y0 = (int)squeeze_even_bits32(tm >> 1) << kTileLog2;
+  const bool polar = (f >> 2) != 1;
+
+  if (tid < kHTaps) s_w[tid] = wts.w[polar ? 1 : 0][tid];
+  for (int c = tid; c < kHCells; c += 256) {
+    const int cy = c / kHP, cx = c - cy * kHP;
+    const int64_t p = cell_to_pixel(k, f, x0 - kHR + cx, y0 - kHR + cy);
+    const int64_t i = store_index(p, slot_of_tile, bits);
+    s_idx[c] = (int)i;
+    s_val[c] = i >= 0 ? 1.f : 0.f;
+    float x[3] = {0.f, 0.f, 0.f}, g[3] = {0.f, 0.f, 0.f};
+    if (i >= 0) {
+#pragma unroll
+      for (int ch = 0; ch < 3; ++ch) { x[ch] = __ldg(X + 3 * i + ch); g[ch] = __ldg(G + 3 * i + ch); }
+    }
+#pragma unroll
+    for (int ch = 0; ch < 3; ++ch) s_xg[ch][c] = make_float2(x[ch], g[ch]);
+    if (GRAD) { s_grad[3 * c] = 0.f; s_grad[3 * c + 1] = 0.f; s_grad[3 * c + 2] = 0.f; }
+  }
+  __syncthreads();
+
+  // thread -> pixel (lx, ly) row-major in the tile: a half warp reads 16 consecutive float2 of one patch row (no bank conflicts)
+  const int lx = tid & 15, ly = tid >> 4;
+  const int cc = (ly + kHR) * kHP + lx + kHR;                 // centre cell
+  const bool live = s_idx[cc] >= 0;
+  const double n_valid = bits ? acc[2] : (double)n_pix_full;
+  const float inv_n = (float)(1.0 / n_valid);
+  float hq = 0.f, l1 = 0.f;
+  if (live) {
+    float xq[3], gq[3];
+#pragma unroll
+    for (int ch = 0; ch < 3; ++ch) { const float2 v = s_xg[ch][cc]; xq[ch] = v.x; gq[ch] = v.y; }
+    float wsum = 0.f;
+    float S1[3] = {0, 0, 0}, S2[3] = {0, 0, 0}, S11[3] = {0, 0, 0}, S22[3] = {0, 0, 0}, S12[3] = {0, 0, 0};
+    const int base = ly * kHP + lx;
+    for (int ty = 0; ty < kHW; ++ty) {
+#pragma unroll
+      for (int tx = 0; tx < kHW; ++tx) {
+        const int c = base + ty * kHP + tx;
+        const float wv = s_w[ty * kHW + tx] * s_val[c];
+        wsum += wv;
+#pragma unroll
+        for (int ch = 0; ch < 3; ++ch) {
+          const float2 v = s_xg[ch][c];
+          const float dx = v.x - xq[ch], dg = v.y - gq[ch];
+          const float a = wv * dx, b = wv * dg;
+          S1[ch] += a; S2[ch] += b;
+          S11[ch] = fmaf(a, dx, S11[ch]); S22[ch] = fmaf(b, dg, S22[ch]); S12[ch] = fmaf(a, dg, S12[ch]);
+        }
+      }
+    }
+    const float inv_w = 1.0f / wsum;                          // the centre tap is valid: wsum >= w(0,0) = 1
+    const float C1 = 1e-4f, C2 = 9e-4f;                       // A33
+    float K0[3], K1[3], K2[3], m1[3], m2[3];
+#pragma unroll
+    for (int ch = 0; ch < 3; ++ch) {
+      const float u1 = S1[ch] * inv_w, u2 = S2[ch] * inv_w;   // means about the centre value
+      const float s11 = S11[ch] * inv_w - u1 * u1, s22 = S22[ch] * inv_w - u2 * u2, s12 = S12[ch] * inv_w - u1 * u2;
+      m1[ch] = xq[ch] + u1; m2[ch] = gq[ch] + u2;
+      const float a1 = 2.f * m1[ch] * m2[ch] + C1, a2 = 2.f * s12 + C2;
+      const float b1 = m1[ch] * m1[ch] + m2[ch] * m2[ch] + C1, b2 = s11 + s22 + C2;
+      const float ib1 = 1.0f / b1, ib2 = 1.0f / b2;
+      const float ssim = a1 * a2 * ib1 * ib2;
+      hq += ssim;
+      // d ssim / d(m1 | s11 | s12) with s11 = e11 - m1^2, s12 = e12 - m1 m2 held as independent variables:
+      //   d/dm1 = 2 m2 a2 / (b1 b2) - 2 m1 ssim / b1,  d/ds11 = -ssim / b2,  d/ds12 = 2 a1 / (b1 b2);
+      // a tap value x enters m1 with weight w, s11 with 2 w (x - m1), s12 with w (g - m2).
+      K0[ch] = 2.f * (m2[ch] * a2 * ib1 * ib2 - m1[ch] * ssim * ib1);
+      K1[ch] = -2.f * ssim * ib2;
+      K2[ch] = 2.f * a1 * ib1 * ib2;
+      const float d = xq[ch] - gq[ch];
+      l1 += fabsf(d);
+      if (GRAD) atomicAdd(&s_grad[3 * cc + ch], (1.f - lambda) * inv_n * (1.f / 3.f) * (d > 0.f ? 1.f : (d < 0.f ? -1.f : 0.f)));
+    }
+    hq *= (1.f / 3.f);
+    if (GRAD) {
+      const float scale = -lambda * inv_n * (1.f / 3.f) * inv_w;
+      for (int ty = 0; ty < kHW; ++ty) {
+#pragma unroll
+        for (int tx = 0; tx < kHW; ++tx) {
+          const int c = base + ty * kHP + tx;
+          const float wn = s_w[ty * kHW + tx] * s_val[c] * scale;
+#pragma unroll
+          for (int ch = 0; ch < 3; ++ch) {
+            const float2 v = s_xg[ch][c];
+            const float t = fmaf(K1[ch], v.x - m1[ch], fmaf(K2[ch], v.y - m2[ch], K0[ch]));
+            atomicAdd(&s_grad[3 * c + ch], wn * t);
+          }
+        }
+      }
+    }
+  }
+  if (h_map) {
+    // storage position of (lx, ly) inside the slot: Morton interleave
+    const uint32_t m = spread16((uint32_t)lx) | (spread16((uint32_t)ly) << 1);
+    h_map[slot * 256 + m] = hq;
+  }
+  // block sums of h and |X - G| -> two double atomics per block
+  float a = hq, b = l1;
+  for (int o = 16; o; o >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, o); b += __shfl_xor_sync(0xffffffffu, b, o); }
+  if ((tid & 31) == 0) { s_red[0][tid >> 5] = a; s_red[1][tid >> 5] = b; }
+  __syncthreads();                                            // also orders the s_grad reductions before the flush
+  if (tid < 2) {
+    double s = 0.0;
+    for (int w = 0; w < 8; ++w) s += (double)s_red[tid][w];
+    if (s != 0.0) atomicAdd(acc + tid, s);
+  }
+  if (GRAD) {
+    for (int c = tid; c < kHCells; c += 256) {
+      const int i = s_idx[c];
+      if (i < 0) continue;
+      float* o = dL_dX + 3 * (int64_t)i;
+#pragma unroll
+      for (int ch = 0; ch < 3; ++ch) {
+        const float v = s_grad[3 * c + ch];
+        if (v != 0.f) atomicAdd(o + ch, v);
+      }
+    }
+  }
+}
+
+// loss3 = (L, L1^H, mean h) from acc = (sum h, sum |X - G|, n_valid)
+__global__ void hssim_finish_kernel(const double* acc, double n_pix_full, int has_bits, double lambda, double* loss3) {
+  const double n = has_bits ? acc[2] : n_pix_full;
+  if (n <= 0.0) { loss3[0] = loss3[1] = loss3[2] = 0.0; return; }
+  const double h = acc[0] / n, l1 = acc[1] / (3.0 * n);
+  loss3[0] = (1.0 - lambda) * l1 + lambda * (1.0 - h); loss3[1] = l1; loss3[2] = h;
+}
+
+}  // namespace uts
+
+using namespace uts;
+
+extern "C" {
+
+size_t uts_hssim_scratch_bytes(const uts_config*) { return 256; }
+
+int uts_hssim_loss(const uts_config* cfg, uts_mask mask, const float* X, const float* G, float lambda, float sigma, float* h_map,
+                   float* dL_dX, double* loss3, void* scratch, size_t scratch_bytes, void* stream) {
+  int st = check_config(cfg);
+  if (st) return st;
+  st = check_mask(cfg, mask);
+  if (st) return st;
+  if (!loss3 || !scratch || scratch_bytes < 256 || ((uintptr_t)scratch & 7) || !(sigma > 0.f) || !(lambda >= 0.f && lambda <= 1.f))
+    return UTS_ERR_INVALID_ARG;
+  const Dims d = dims_of(cfg, &mask);
+  cudaStream_t s = (cudaStream_t)stream;
+  double* acc = (double*)scratch;
+  UTS_CUDA(cudaMemsetAsync(acc, 0, 3 * sizeof(double), s));
+  const bool has_bits = mask.pixel_mask_bits != nullptr;
+  if (d.n_slot > 0) {
+    if (!X || !G) return UTS_ERR_INVALID_ARG;
+    if (dL_dX) UTS_CUDA(cudaMemsetAsync(dL_dX, 0, (size_t)d.n_slot * 256 * 3 * sizeof(float), s));
+    if (has_bits) {
+      hssim_count_kernel<<<(unsigned)((d.n_slot * 8 + 255) / 256), 256, 0, s>>>(d.n_slot, mask.active_tiles, mask.pixel_mask_bits, acc);
+      UTS_LAUNCH_CHECK();
+    }
+    // tap weights (A31), double on the host, rounded once
+    HssimWeights w;
+    const double sg = (double)sigma, a = kPi / 4.0, b = 4.0 / kPi;
+    for (int dy = -kHR; dy <= kHR; ++dy)
+      for (int dx = -kHR; dx <= kHR; ++dx) {
+        const int t = (dy + kHR) * kHW + (dx + kHR);
+        const double ew = (double)(dx - dy), ns = (double)(dx + dy);     // east-west and north-south diagonals of the pixel
+        w.w[0][t] = (float)exp(-(double)(dx * dx + dy * dy) / (2.0 * sg * sg));
+        w.w[1][t] = (float)exp(-(a * ew * ew + b * ns * ns) / (4.0 * sg * sg));
+      }
+    if (dL_dX)
+      hssim_kernel<true><<<(unsigned)d.n_slot, 256, 0, s>>>(d.k, d.n_pix, mask.active_tiles, mask.slot_of_tile, mask.pixel_mask_bits, X, G, lambda, w,
+                                                            h_map, dL_dX, acc);
+    else
+      hssim_kernel<false><<<(unsigned)d.n_slot, 256, 0, s>>>(d.k, d.n_pix, mask.active_tiles, mask.slot_of_tile, mask.pixel_mask_bits, X, G, lambda, w,
+                                                             h_map, dL_dX, acc);
+    UTS_LAUNCH_CHECK();
+  }
+  hssim_finish_kernel<<<1, 1, 0, s>>>(acc, (double)d.n_pix, has_bits ? 1 : 0, (double)lambda, loss3);
+  UTS_LAUNCH_CHECK();
+  return UTS_OK;
+}
+
+}  // extern "C"

@@ -286,6 +286,32 @@ def run_ours(args):
     except Exception as e:      # measurement plumbing only; never hides a failure of the step itself
         extras["resample"] = dict(error=str(e))
 
+    # the step before the backward hot path (not part of the step): L1 + HEALPix-SSIM loss and dL/dI on view 0's
+    # image against a seeded target (the image plus N(0, 0.05) noise, clipped)
+    try:
+        img = r.color[0].contiguous()
+        tgt = (img + 0.05 * torch.randn(img.shape, device="cuda", generator=torch.Generator(device="cuda").manual_seed(7))).clamp_(0, 1)
+        loss3 = torch.empty(3, dtype=torch.float64, device="cuda")
+        g_l = torch.empty_like(img)
+        sc_l = torch.empty(B.uts_hssim_scratch_bytes(cfg), dtype=torch.uint8, device="cuda")
+        tms = []
+        for fn in (lambda: B.uts_hssim_loss(cfg, mask, img, tgt, loss3, sc_l, dL_dX=g_l), lambda: B.uts_hssim_loss(cfg, mask, img, tgt, loss3, sc_l)):
+            for _ in range(3):
+                fn()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(5):
+                fn()
+            e1.record(); torch.cuda.synchronize()
+            tms.append(e0.elapsed_time(e1) / 5)
+        npx_l = img.shape[0]
+        extras["hssim_loss"] = dict(loss=float(loss3[0]), l1=float(loss3[1]), hssim=float(loss3[2]), fwd_bwd_ms=tms[0], fwd_ms=tms[1],
+                                    gtap_per_s=npx_l * 121 * 3 / (tms[0] * 1e-3) / 1e9,
+                                    work_model="121 taps x 3 channels per pixel, forward sums + gradient scatter; 36 B compulsory traffic per pixel")
+        del img, tgt, g_l
+    except Exception as e:      # measurement plumbing only
+        extras["hssim_loss"] = dict(error=str(e))
+
     # end to end through the C ABI with HOST buffers (H2D + D2H inside the timed region)
     h = {k: torch.from_numpy(scene[k]).contiguous().pin_memory() for k in ("means", "scales", "quats", "opac", "sh", "W", "b")}
     hg = gcol.cpu().pin_memory()

@@ -9,16 +9,19 @@
 // taps that do not exist (3-face vertices, M_C = 0) dropped and the weights renormalised, zone of the centre pixel's face,
 // SSIM constants 0.01^2 / 0.03^2, h_q = channel mean.
 //
-// B200 design.  One block per 16 x 16 tile (the rasteriser's slot), 256 threads.  The block stages the 26 x 26 patch of the
+// B200 design.  One block of 64 threads per 16 x 16 tile (the rasteriser's slot).  The block stages the 26 x 26 patch of the
 // tile's own face frame — tile plus a 5-pixel apron, the apron resolved through the face-adjacency rules below — in shared
-// memory as (x, g) pairs per channel plus a validity plane.  Every thread then walks the 121 taps of its pixel once for the five
-// window sums per channel (taken about the centre pixel's own value: variances do not lose digits to e11 - m1^2), forms the SSIM
-// index and its derivatives with respect to (m1, s11, s12), and — this is the "transposed convolution" — walks the taps a second
-// time scattering weight * (K0 + K1 (x - m1) + K2 (g - m2)) into a shared gradient patch with shared-memory reductions.  The
-// patch is flushed to dL_dX with one red.global per cell and channel.  The upstream gradient of a loss is 1, so forward and
-// backward share the staged patch and X, G are read from HBM once.  The path is bound by fp32 ALU and shared-memory issue, not
-// by HBM: 121 taps x 3 channels x (9 ALU ops + 1 LDS.64) per pixel forward, 121 x 3 x (5 ALU + LDS.64 + RED.shared) backward,
-// against 24 B of compulsory traffic per pixel.
+// memory as (x, g) pairs per channel plus a validity plane.  Every thread owns four pixels of one tile column: a patch cell read
+// once from shared memory serves up to four windows, which is what keeps the kernel on the FP32 pipe rather than on the
+// shared-memory pipe (the first version, one pixel per thread, ran at 99 % of the L1/shared wavefront rate).  The thread walks
+// the 11 x 14 cells under its four windows once for the five window sums per pixel and channel (taken about a reference value
+// next to the pixel: variances do not lose digits to e11 - m1^2), forms the SSIM index and its derivatives with respect to
+// (m1, s11, s12), and — this is the "transposed convolution" with "cached derivatives" — walks the cells a second time adding
+// weight * (c0 + K1 dx + K2 dg), summed over its four pixels in registers, into a gradient patch private to its warp (plain
+// read-add-write between __syncwarp()s: float atomics on shared memory are compare-and-swap loops on sm_100).  The two warps'
+// patches are summed and flushed to dL_dX with one red.global per cell and channel.  The upstream gradient of a loss is 1, so
+// forward and backward share the staged patch and X, G are read from HBM once.  The path is bound by fp32 ALU: about 24 FP32
+// instructions per tap and pixel forward and 10 backward, against 36 B of compulsory traffic per pixel.
 #include "uts_internal.cuh"
 
 namespace uts {
@@ -109,17 +112,29 @@ __global__ void hssim_count_kernel(int64_t n_slot, const uint32_t* __restrict__ 
 }
 
 // -------------------------------------------------------------------------------------------------- main
+// 64 threads per tile: thread (lx, strip) owns the four pixels (lx, 4 strip + j), j = 0..3, of one tile column.  A patch cell
+// loaded once serves up to four of the thread's windows (14 patch rows instead of 44 per window column), which takes the kernel
+// off the shared-memory pipe.  Sums are taken about the value of the thread's second pixel.
+constexpr int kHT = 64;                      // threads per block
+constexpr int kHJ = 4;                       // pixels per thread (rows)
+constexpr int kHRows = kHJ + 2 * kHR;        // 14 patch rows per thread
+constexpr int kHS = 28;                      // patch row stride: 4 rows apart = 16 banks apart (the two half warps never collide)
+constexpr int kHCellsS = kHP * kHS;
+constexpr int kGR = 8 + 2 * kHR;             // 18 rows of a warp's private gradient patch (8 tile rows + apron)
+
+template <int V> struct Int { static constexpr int value = V; };
+
 template <bool GRAD>
-__global__ void __launch_bounds__(256, 3)
+__global__ void __launch_bounds__(kHT, 6)
 hssim_kernel(int k, int64_t n_pix_full, const uint32_t* __restrict__ active_tiles, const int32_t* __restrict__ slot_of_tile,
              const uint32_t* __restrict__ bits, const float* __restrict__ X, const float* __restrict__ G, float lambda,
              const __grid_constant__ HssimWeights wts, float* __restrict__ h_map, float* __restrict__ dL_dX, double* acc) {
-  __shared__ float2 s_xg[3][kHCells];        // (x, g) per channel
-  __shared__ float s_val[kHCells];           // 1 valid, 0 missing
-  __shared__ int s_idx[kHCells];             // storage index (pixels, < 2^31) or -1
+  __shared__ float2 s_xg[3][kHCellsS];       // (x, g) per channel
+  __shared__ float s_val[kHCellsS];          // 1 valid, 0 missing
+  __shared__ int s_idx[kHCellsS];            // storage index (pixels, < 2^31) or -1
   __shared__ float s_w[kHTaps];
-  __shared__ float s_grad[GRAD ? 3 * kHCells : 1];
-  __shared__ float s_red[2][8];
+  __shared__ float s_grad[GRAD ? 2 * 3 * kGR * kHS : 1];   // [warp][channel][row][col]: no two warps share a cell
+  __shared__ float s_red[2][2];
 
   const int tid = threadIdx.x;
   const int64_t slot = blockIdx.x;
@@ -130,118 +145,188 @@ hssim_kernel(int k, int64_t n_pix_full, const uint32_t* __restrict__ active_tile
   const int x0 = (int)squeeze_even_bits32(tm) << kTileLog2, y0 = (int)squeeze_even_bits32(tm >> 1) << kTileLog2;
   const bool polar = (f >> 2) != 1;
 
-  if (tid < kHTaps) s_w[tid] = wts.w[polar ? 1 : 0][tid];
-  for (int c = tid; c < kHCells; c += 256) {
+  for (int t = tid; t < kHTaps; t += kHT) s_w[t] = wts.w[polar ? 1 : 0][t];
+  for (int c = tid; c < kHCells; c += kHT) {
     const int cy = c / kHP, cx = c - cy * kHP;
+    const int cell = cy * kHS + cx;
     const int64_t p = cell_to_pixel(k, f, x0 - kHR + cx, y0 - kHR + cy);
     const int64_t i = store_index(p, slot_of_tile, bits);
-    s_idx[c] = (int)i;
-    s_val[c] = i >= 0 ? 1.f : 0.f;
+    s_idx[cell] = (int)i;
+    s_val[cell] = i >= 0 ? 1.f : 0.f;
     float x[3] = {0.f, 0.f, 0.f}, g[3] = {0.f, 0.f, 0.f};
     if (i >= 0) {
 #pragma unroll
       for (int ch = 0; ch < 3; ++ch) { x[ch] = __ldg(X + 3 * i + ch); g[ch] = __ldg(G + 3 * i + ch); }
     }
 #pragma unroll
-    for (int ch = 0; ch < 3; ++ch) s_xg[ch][c] = make_float2(x[ch], g[ch]);
-    if (GRAD) { s_grad[3 * c] = 0.f; s_grad[3 * c + 1] = 0.f; s_grad[3 * c + 2] = 0.f; }
+    for (int ch = 0; ch < 3; ++ch) s_xg[ch][cell] = make_float2(x[ch], g[ch]);
   }
+  if (GRAD) for (int c = tid; c < 2 * 3 * kGR * kHS; c += kHT) s_grad[c] = 0.f;
   __syncthreads();
 
-  // thread -> pixel (lx, ly) row-major in the tile: a half warp reads 16 consecutive float2 of one patch row (no bank conflicts)
-  const int lx = tid & 15, ly = tid >> 4;
-  const int cc = (ly + kHR) * kHP + lx + kHR;                 // centre cell
-  const bool live = s_idx[cc] >= 0;
+  const int lx = tid & 15, r0 = (tid >> 4) * kHJ;             // tile rows r0 .. r0+3; half warp = one strip of 16 x 4 pixels
+  const int base = r0 * kHS + lx;                             // patch cell of tap (0,0) of pixel j = 0
+  float xr[3], gr[3];
+  {
+    // reference value of the sums: the thread's second pixel, or its first visible one (a masked cell holds 0, which would
+    // leave the sums uncentred)
+    int cref = (r0 + 1 + kHR) * kHS + lx + kHR;
+    if (s_idx[cref] < 0) {
+#pragma unroll
+      for (int j = kHJ - 1; j >= 0; --j) { const int cj = (r0 + j + kHR) * kHS + lx + kHR; if (s_idx[cj] >= 0) cref = cj; }
+    }
+#pragma unroll
+    for (int ch = 0; ch < 3; ++ch) { const float2 v = s_xg[ch][cref]; xr[ch] = v.x; gr[ch] = v.y; }
+  }
   const double n_valid = bits ? acc[2] : (double)n_pix_full;
   const float inv_n = (float)(1.0 / n_valid);
-  float hq = 0.f, l1 = 0.f;
-  if (live) {
-    float xq[3], gq[3];
+
+  float wsum[kHJ], S1[kHJ][3], S2[kHJ][3], S11[kHJ][3], S22[kHJ][3], S12[kHJ][3];
 #pragma unroll
-    for (int ch = 0; ch < 3; ++ch) { const float2 v = s_xg[ch][cc]; xq[ch] = v.x; gq[ch] = v.y; }
-    float wsum = 0.f;
-    float S1[3] = {0, 0, 0}, S2[3] = {0, 0, 0}, S11[3] = {0, 0, 0}, S22[3] = {0, 0, 0}, S12[3] = {0, 0, 0};
-    const int base = ly * kHP + lx;
-    for (int ty = 0; ty < kHW; ++ty) {
+  for (int j = 0; j < kHJ; ++j) {
+    wsum[j] = 0.f;
 #pragma unroll
-      for (int tx = 0; tx < kHW; ++tx) {
-        const int c = base + ty * kHP + tx;
-        const float wv = s_w[ty * kHW + tx] * s_val[c];
-        wsum += wv;
+    for (int ch = 0; ch < 3; ++ch) S1[j][ch] = S2[j][ch] = S11[j][ch] = S22[j][ch] = S12[j][ch] = 0.f;
+  }
+  // One patch cell under the windows of pixels J0..J1 (compile-time range): wp points at the weight of pixel j = 0 for this cell,
+  // pixel j's weight sits j window rows before it.
+  auto fwd_cell = [&](int c, const float* wp, auto j0, auto j1) {
+    const float val = s_val[c];
+    float dx[3], dg[3];
 #pragma unroll
-        for (int ch = 0; ch < 3; ++ch) {
-          const float2 v = s_xg[ch][c];
-          const float dx = v.x - xq[ch], dg = v.y - gq[ch];
-          const float a = wv * dx, b = wv * dg;
-          S1[ch] += a; S2[ch] += b;
-          S11[ch] = fmaf(a, dx, S11[ch]); S22[ch] = fmaf(b, dg, S22[ch]); S12[ch] = fmaf(a, dg, S12[ch]);
-        }
+    for (int ch = 0; ch < 3; ++ch) { const float2 v = s_xg[ch][c]; dx[ch] = v.x - xr[ch]; dg[ch] = v.y - gr[ch]; }
+#pragma unroll
+    for (int j = decltype(j0)::value; j <= decltype(j1)::value; ++j) {
+      const float wv = wp[-j * kHW] * val;
+      wsum[j] += wv;
+#pragma unroll
+      for (int ch = 0; ch < 3; ++ch) {
+        const float a = wv * dx[ch], b = wv * dg[ch];
+        S1[j][ch] += a; S2[j][ch] += b;
+        S11[j][ch] = fmaf(a, dx[ch], S11[j][ch]); S22[j][ch] = fmaf(b, dg[ch], S22[j][ch]); S12[j][ch] = fmaf(a, dg[ch], S12[j][ch]);
       }
     }
-    const float inv_w = 1.0f / wsum;                          // the centre tap is valid: wsum >= w(0,0) = 1
-    const float C1 = 1e-4f, C2 = 9e-4f;                       // A33
-    float K0[3], K1[3], K2[3], m1[3], m2[3];
+  };
+  // Patch rows 0..2 and 11..13 lie under fewer than four of the thread's windows (unrolled); rows 3..10 under all four: a real
+  // loop, so that the body stays inside the instruction cache (fully unrolled, 14 rows x 4 pixels, it stalled on fetch).
+  using I0 = Int<0>; using I1 = Int<1>; using I2 = Int<2>; using I3 = Int<3>;
+#pragma unroll 1
+  for (int tx = 0; tx < kHW; ++tx) {
+    const int c = base + tx;
+    const float* wp = s_w + tx;
+    fwd_cell(c, wp, I0(), I0());
+    fwd_cell(c + kHS, wp + kHW, I0(), I1());
+    fwd_cell(c + 2 * kHS, wp + 2 * kHW, I0(), I2());
+#pragma unroll 2
+    for (int rho = 3; rho < kHW; ++rho) fwd_cell(c + rho * kHS, wp + rho * kHW, I0(), I3());
+    fwd_cell(c + 11 * kHS, wp + 11 * kHW, I1(), I3());
+    fwd_cell(c + 12 * kHS, wp + 12 * kHW, I2(), I3());
+    fwd_cell(c + 13 * kHS, wp + 13 * kHW, I3(), I3());
+  }
+
+  // SSIM index and, for the gradient, its derivatives folded into three coefficients per pixel and channel:
+  //   d ssim / d(m1 | s11 | s12) with s11 = e11 - m1^2, s12 = e12 - m1 m2 held as independent variables:
+  //     d/dm1 = 2 m2 a2 / (b1 b2) - 2 m1 ssim / b1,  d/ds11 = -ssim / b2,  d/ds12 = 2 a1 / (b1 b2);
+  //   a tap value x enters m1 with weight w, s11 with 2 w (x - m1), s12 with w (g - m2), so the tap's share of dL/dx is
+  //     w [K0 + K1 (x - m1) + K2 (g - m2)] = w [c0 + K1 dx + K2 dg],  dx = x - x_ref,  c0 = K0 - K1 u1 - K2 u2.
+  const float C1 = 1e-4f, C2 = 9e-4f;                         // A33
+  float hsum = 0.f, l1 = 0.f;
+  float c0[kHJ][3], k1[kHJ][3], k2[kHJ][3], gl1[kHJ][3];
+#pragma unroll
+  for (int j = 0; j < kHJ; ++j) {
+    const int cc = base + (j + kHR) * kHS + kHR;              // centre cell of pixel j
+    const bool live = s_idx[cc] >= 0;
+    const float inv_w = live ? 1.0f / wsum[j] : 0.f;          // the centre tap is valid: wsum >= w(0,0) = 1
+    const float sc = -lambda * inv_n * (1.f / 3.f) * inv_w;
+    float hq = 0.f;
 #pragma unroll
     for (int ch = 0; ch < 3; ++ch) {
-      const float u1 = S1[ch] * inv_w, u2 = S2[ch] * inv_w;   // means about the centre value
-      const float s11 = S11[ch] * inv_w - u1 * u1, s22 = S22[ch] * inv_w - u2 * u2, s12 = S12[ch] * inv_w - u1 * u2;
-      m1[ch] = xq[ch] + u1; m2[ch] = gq[ch] + u2;
-      const float a1 = 2.f * m1[ch] * m2[ch] + C1, a2 = 2.f * s12 + C2;
-      const float b1 = m1[ch] * m1[ch] + m2[ch] * m2[ch] + C1, b2 = s11 + s22 + C2;
+      const float u1 = S1[j][ch] * inv_w, u2 = S2[j][ch] * inv_w;   // means about the reference value
+      const float s11 = S11[j][ch] * inv_w - u1 * u1, s22 = S22[j][ch] * inv_w - u2 * u2, s12 = S12[j][ch] * inv_w - u1 * u2;
+      const float m1 = xr[ch] + u1, m2 = gr[ch] + u2;
+      const float a1 = 2.f * m1 * m2 + C1, a2 = 2.f * s12 + C2;
+      const float b1 = m1 * m1 + m2 * m2 + C1, b2 = s11 + s22 + C2;
       const float ib1 = 1.0f / b1, ib2 = 1.0f / b2;
       const float ssim = a1 * a2 * ib1 * ib2;
       hq += ssim;
-      // d ssim / d(m1 | s11 | s12) with s11 = e11 - m1^2, s12 = e12 - m1 m2 held as independent variables:
-      //   d/dm1 = 2 m2 a2 / (b1 b2) - 2 m1 ssim / b1,  d/ds11 = -ssim / b2,  d/ds12 = 2 a1 / (b1 b2);
-      // a tap value x enters m1 with weight w, s11 with 2 w (x - m1), s12 with w (g - m2).
-      K0[ch] = 2.f * (m2[ch] * a2 * ib1 * ib2 - m1[ch] * ssim * ib1);
-      K1[ch] = -2.f * ssim * ib2;
-      K2[ch] = 2.f * a1 * ib1 * ib2;
-      const float d = xq[ch] - gq[ch];
-      l1 += fabsf(d);
-      if (GRAD) atomicAdd(&s_grad[3 * cc + ch], (1.f - lambda) * inv_n * (1.f / 3.f) * (d > 0.f ? 1.f : (d < 0.f ? -1.f : 0.f)));
+      const float K0 = 2.f * (m2 * a2 * ib1 * ib2 - m1 * ssim * ib1), K1 = -2.f * ssim * ib2, K2 = 2.f * a1 * ib1 * ib2;
+      c0[j][ch] = sc * (K0 - K1 * u1 - K2 * u2); k1[j][ch] = sc * K1; k2[j][ch] = sc * K2;
+      const float2 v = s_xg[ch][cc];
+      const float d = v.x - v.y;
+      l1 += live ? fabsf(d) : 0.f;
+      gl1[j][ch] = live ? (1.f - lambda) * inv_n * (1.f / 3.f) * (d > 0.f ? 1.f : (d < 0.f ? -1.f : 0.f)) : 0.f;
     }
-    hq *= (1.f / 3.f);
-    if (GRAD) {
-      const float scale = -lambda * inv_n * (1.f / 3.f) * inv_w;
-      for (int ty = 0; ty < kHW; ++ty) {
+    hq = live ? hq * (1.f / 3.f) : 0.f;
+    hsum += hq;
+    if (h_map) h_map[slot * 256 + (spread16((uint32_t)lx) | (spread16((uint32_t)(r0 + j)) << 1))] = hq;   // Morton position in the slot
+  }
+
+  if (GRAD) {
+    // transposed window: every tap scatters into the warp's private patch.  Within one group of four patch rows the 32 lanes
+    // touch 32 different cells (the other half warp works 4 rows further down), so plain read-add-write is safe between the
+    // __syncwarp()s (after rows 2, 6, 10, 13); sums over the thread's own four pixels are taken in registers first.
+    float* gw = s_grad + (tid >> 5) * (3 * kGR * kHS) + (((tid >> 4) & 1) * kHJ) * kHS + lx;
+    auto bwd_cell = [&](int c, const float* wp, float* gp, auto j0, auto j1) {
+      const float val = s_val[c];
+      float dx[3], dg[3], ac[3] = {0.f, 0.f, 0.f};
 #pragma unroll
-        for (int tx = 0; tx < kHW; ++tx) {
-          const int c = base + ty * kHP + tx;
-          const float wn = s_w[ty * kHW + tx] * s_val[c] * scale;
+      for (int ch = 0; ch < 3; ++ch) { const float2 v = s_xg[ch][c]; dx[ch] = v.x - xr[ch]; dg[ch] = v.y - gr[ch]; }
 #pragma unroll
-          for (int ch = 0; ch < 3; ++ch) {
-            const float2 v = s_xg[ch][c];
-            const float t = fmaf(K1[ch], v.x - m1[ch], fmaf(K2[ch], v.y - m2[ch], K0[ch]));
-            atomicAdd(&s_grad[3 * c + ch], wn * t);
-          }
-        }
+      for (int j = decltype(j0)::value; j <= decltype(j1)::value; ++j) {
+        const float wv = wp[-j * kHW] * val;
+#pragma unroll
+        for (int ch = 0; ch < 3; ++ch) ac[ch] = fmaf(wv, fmaf(k1[j][ch], dx[ch], fmaf(k2[j][ch], dg[ch], c0[j][ch])), ac[ch]);
       }
+#pragma unroll
+      for (int ch = 0; ch < 3; ++ch) gp[ch * (kGR * kHS)] += ac[ch];
+    };
+#pragma unroll 1
+    for (int tx = 0; tx < kHW; ++tx) {
+      const int c = base + tx;
+      const float* wp = s_w + tx;
+      float* gp = gw + tx;
+      bwd_cell(c, wp, gp, I0(), I0());
+      bwd_cell(c + kHS, wp + kHW, gp + kHS, I0(), I1());
+      bwd_cell(c + 2 * kHS, wp + 2 * kHW, gp + 2 * kHS, I0(), I2());
+      __syncwarp();
+#pragma unroll 1
+      for (int rho = 3; rho < kHW; rho += 4) {                // rows 3..6, 7..10
+#pragma unroll
+        for (int d = 0; d < 4; ++d) bwd_cell(c + (rho + d) * kHS, wp + (rho + d) * kHW, gp + (rho + d) * kHS, I0(), I3());
+        __syncwarp();
+      }
+      bwd_cell(c + 11 * kHS, wp + 11 * kHW, gp + 11 * kHS, I1(), I3());
+      bwd_cell(c + 12 * kHS, wp + 12 * kHW, gp + 12 * kHS, I2(), I3());
+      bwd_cell(c + 13 * kHS, wp + 13 * kHW, gp + 13 * kHS, I3(), I3());
+      __syncwarp();
     }
+    // L1 term at the thread's own pixels
+#pragma unroll
+    for (int j = 0; j < kHJ; ++j)
+#pragma unroll
+      for (int ch = 0; ch < 3; ++ch) gw[ch * (kGR * kHS) + (j + kHR) * kHS + kHR] += gl1[j][ch];
   }
-  if (h_map) {
-    // storage position of (lx, ly) inside the slot: Morton interleave
-    const uint32_t m = spread16((uint32_t)lx) | (spread16((uint32_t)ly) << 1);
-    h_map[slot * 256 + m] = hq;
-  }
+
   // block sums of h and |X - G| -> two double atomics per block
-  float a = hq, b = l1;
+  float a = hsum, b = l1;
   for (int o = 16; o; o >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, o); b += __shfl_xor_sync(0xffffffffu, b, o); }
   if ((tid & 31) == 0) { s_red[0][tid >> 5] = a; s_red[1][tid >> 5] = b; }
-  __syncthreads();                                            // also orders the s_grad reductions before the flush
+  __syncthreads();                                            // also: both warps' gradient patches are complete
   if (tid < 2) {
-    double s = 0.0;
-    for (int w = 0; w < 8; ++w) s += (double)s_red[tid][w];
+    const double s = (double)s_red[tid][0] + (double)s_red[tid][1];
     if (s != 0.0) atomicAdd(acc + tid, s);
   }
   if (GRAD) {
-    for (int c = tid; c < kHCells; c += 256) {
-      const int i = s_idx[c];
+    for (int c = tid; c < kHCells; c += kHT) {
+      const int cy = c / kHP, cx = c - cy * kHP;
+      const int i = s_idx[cy * kHS + cx];
       if (i < 0) continue;
       float* o = dL_dX + 3 * (int64_t)i;
 #pragma unroll
       for (int ch = 0; ch < 3; ++ch) {
-        const float v = s_grad[3 * c + ch];
+        float v = 0.f;
+        if (cy < kGR) v += s_grad[(ch * kGR + cy) * kHS + cx];                          // warp 0: patch rows 0..17
+        if (cy >= 8) v += s_grad[((3 + ch) * kGR + (cy - 8)) * kHS + cx];               // warp 1: patch rows 8..25
         if (v != 0.f) atomicAdd(o + ch, v);
       }
     }
@@ -295,10 +380,10 @@ int uts_hssim_loss(const uts_config* cfg, uts_mask mask, const float* X, const f
         w.w[1][t] = (float)exp(-(a * ew * ew + b * ns * ns) / (4.0 * sg * sg));
       }
     if (dL_dX)
-      hssim_kernel<true><<<(unsigned)d.n_slot, 256, 0, s>>>(d.k, d.n_pix, mask.active_tiles, mask.slot_of_tile, mask.pixel_mask_bits, X, G, lambda, w,
+      hssim_kernel<true><<<(unsigned)d.n_slot, kHT, 0, s>>>(d.k, d.n_pix, mask.active_tiles, mask.slot_of_tile, mask.pixel_mask_bits, X, G, lambda, w,
                                                             h_map, dL_dX, acc);
     else
-      hssim_kernel<false><<<(unsigned)d.n_slot, 256, 0, s>>>(d.k, d.n_pix, mask.active_tiles, mask.slot_of_tile, mask.pixel_mask_bits, X, G, lambda, w,
+      hssim_kernel<false><<<(unsigned)d.n_slot, kHT, 0, s>>>(d.k, d.n_pix, mask.active_tiles, mask.slot_of_tile, mask.pixel_mask_bits, X, G, lambda, w,
                                                              h_map, dL_dX, acc);
     UTS_LAUNCH_CHECK();
   }

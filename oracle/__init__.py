@@ -275,16 +275,18 @@ def hssim_weight(face, dx, dy, sigma=1.5):
     return float(lib().orc_hssim_weight(C.c_int(face), C.c_int(dx), C.c_int(dy), C.c_double(sigma)))
 
 
-def hssim_loss(order, X, G, slot_of_tile=None, bits=None, lam=0.2, sigma=1.5, grad=True):
-    """X, G [n_slot*256, 3] fp32 (slot layout).  Returns dict(loss, l1, hssim, h_map [n_slot*256], grad [n_slot*256, 3] or None)."""
+def hssim_loss(order, X, G, slot_of_tile=None, bits=None, lam=0.2, sigma=1.5, grad=True, q_list=None):
+    """X, G [n_slot*256, 3] fp32 (slot layout).  Returns dict(loss, l1, hssim, h_map [n_slot*256], grad [n_slot*256, 3] or None).
+    q_list: evaluate only these centre pixels (NESTED ids) — h_map, sums and grad then hold their terms only."""
     Xf, Gf = _f32(X), _f32(G)
     n_store = Xf.shape[0]
     st = None if slot_of_tile is None else np.ascontiguousarray(slot_of_tile, dtype=np.int32)
     bt = None if bits is None else np.ascontiguousarray(bits, dtype=np.uint32)
     h = np.zeros(n_store); g = np.zeros((n_store, 3)) if grad else None
     out = np.zeros(3)
+    ql = None if q_list is None else np.ascontiguousarray(q_list, dtype=np.int64)
     lib().orc_hssim_loss(C.c_int(order), _p(st), _p(bt), C.c_int64(n_store // 256), _p(Xf), _p(Gf), C.c_double(lam), C.c_double(sigma),
-                         _p(h), _p(g), _p(out))
+                         _p(h), _p(g), _p(out), _p(ql), C.c_int64(0 if ql is None else ql.shape[0]))
     return dict(loss=float(out[0]), l1=float(out[1]), hssim=float(out[2]), h_map=h, grad=g)
 
 

@@ -369,8 +369,8 @@ double orc_e2e_f64(const Config* cfg, const double* means, const double* scales,
 int64_t orc_hssim_neighbor(int order, int64_t p, int dx, int dy, int* rot) { return hssim_neighbor(order, p, dx, dy, rot); }
 double orc_hssim_weight(int face, int dx, int dy, double sigma) { return hssim_weight(face, dx, dy, sigma); }
 void orc_hssim_loss(int order, const int32_t* slot_of_tile, const uint32_t* bits, int64_t n_slot, const float* X, const float* G,
-                    double lambda, double sigma, double* h_map, double* dL_dX, double* out3) {
-  const HssimOut o = hssim_loss(order, slot_of_tile, bits, n_slot, X, G, lambda, sigma, h_map, dL_dX);
+                    double lambda, double sigma, double* h_map, double* dL_dX, double* out3, const int64_t* q_list, int64_t n_q) {
+  const HssimOut o = hssim_loss(order, slot_of_tile, bits, n_slot, X, G, lambda, sigma, h_map, dL_dX, q_list, n_q);
   out3[0] = o.loss; out3[1] = o.l1; out3[2] = o.hssim;
 }
 }  // extern "C"

@@ -78,7 +78,7 @@ struct Image {
 }  // namespace
 
 HssimOut hssim_loss(int order, const int32_t* slot_of_tile, const uint32_t* pixel_mask_bits, int64_t n_slot, const float* X,
-                    const float* G, double lambda, double sigma, double* h_map, double* dL_dX) {
+                    const float* G, double lambda, double sigma, double* h_map, double* dL_dX, const int64_t* q_list, int64_t n_q) {
   const int R = kHssimR, Wn = 2 * R + 1, CH = 3;
   const double C1 = 0.01 * 0.01, C2 = 0.03 * 0.03;       // A33
   const int64_t npix = npix_of_order(order);
@@ -95,7 +95,11 @@ HssimOut hssim_loss(int order, const int32_t* slot_of_tile, const uint32_t* pixe
   double sum_h = 0.0, sum_l1 = 0.0;
   std::vector<int64_t> tap(Wn * Wn);
   std::vector<double> wt(Wn * Wn);
-  for (int64_t q = 0; q < npix; ++q) {
+  // q_list (test sampling at sizes where the whole sphere is too slow): only the listed centre pixels are evaluated, against
+  // the whole image and with Eq.10's denominator of the whole image; the sums and the gradient then hold their terms only.
+  const int64_t n_centres = q_list ? n_q : npix;
+  for (int64_t qi = 0; qi < n_centres; ++qi) {
+    const int64_t q = q_list ? q_list[qi] : qi;
     const int64_t iq = im.index(q);
     if (iq < 0) continue;
     const int face = (int)(q >> (2 * order));

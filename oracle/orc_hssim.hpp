@@ -44,7 +44,10 @@ struct HssimOut { double loss, l1, hssim; };     // L, L1^H, mean h (so L_HSSIM 
 
 // X, G: [n_slot*256][3] fp32 in the rasteriser's slot layout (slot_of_tile NULL: slot = tile; bits NULL: all pixels valid).
 // h_map (may be NULL): [n_slot*256] per-pixel h_q (0 where masked out).  dL_dX (may be NULL): [n_slot*256][3] gradient of L.
+// q_list (may be NULL = every pixel): centre pixels q to evaluate; with a list, h_map / the sums / dL_dX hold the listed centres'
+// terms only (Eq.10's denominator stays the whole image's), which lets a test check sampled outputs of a full-size image.
 HssimOut hssim_loss(int order, const int32_t* slot_of_tile, const uint32_t* pixel_mask_bits, int64_t n_slot, const float* X,
-                    const float* G, double lambda, double sigma, double* h_map, double* dL_dX);
+                    const float* G, double lambda, double sigma, double* h_map, double* dL_dX, const int64_t* q_list = nullptr,
+                    int64_t n_q = 0);
 
 }  // namespace orc

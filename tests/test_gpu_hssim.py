@@ -182,3 +182,70 @@ def test_chain_render_loss_backward():
     grads = r.backward(g_dev, views, g.view(1, n, 3))
     torch.cuda.synchronize()
     assert all(bool(torch.isfinite(v).all()) for v in grads.values()) and float(grads["means"].abs().max()) > 0
+
+
+def _sample_pixels(order, rng, n_random):
+    """Pixels where the window meets every kind of face boundary — the four corners of every face (both poles, the eight 3-face
+    vertices, the 4-face vertices), edge midpoints — plus random ones."""
+    N = 1 << order
+    def nest(f, x, y):
+        p = 0
+        for b in range(order):
+            p |= ((x >> b) & 1) << (2 * b) | ((y >> b) & 1) << (2 * b + 1)
+        return (f << (2 * order)) | p
+    pts = []
+    for f in range(12):
+        for (x, y) in [(0, 0), (N - 1, 0), (0, N - 1), (N - 1, N - 1), (N // 2, 0), (0, N // 2), (N - 1, N // 2), (N // 2, N - 1), (3, N - 2), (N - 4, 2)]:
+            pts.append(nest(f, x, y))
+    pts += list(rng.integers(0, 12 << (2 * order), size=n_random))
+    return np.unique(np.array(pts, np.int64))
+
+
+@pytest.mark.parametrize("masked", [False, True], ids=["config4-full-sphere", "fisheye-mask"])
+def test_full_size_sampled_against_oracle(masked):
+    """BASELINE.json's image size (order 10, Nside 1024: 12.6 M pixels), the launch bench.py times under extras.hssim_loss.  The
+    oracle evaluates a sample: the centres P (face corners, edges, random) and every pixel of their windows, Q; h is compared on all
+    of Q, the gradient on P (every centre whose window holds a pixel of P is in Q, by the window's symmetry, pinned in
+    tests/test_oracle_hssim.py).  Whole-image properties: HSSIM = mean of the kernel's own h_map, L1^H = the plain mean of |X - G|."""
+    B = _gpu()
+    order = 10
+    cfg = B.Config(order=order, n_gauss=1)
+    oc = orc.Config(order=order, n_gauss=1, n_views=1, sh_degree=0)
+    rng = np.random.default_rng(21 + masked)
+    if masked:
+        spec = ("fisheye", 2048, 2048, 200.0 / 180.0, 200.0 / 180.0)
+        mask = B.uts_build_camera_mask(cfg, B.Camera(*spec))
+        bits = orc.camera_mask_bits(order, orc.Camera(*spec))
+        act, slot = orc.mask_tiles(oc, bits)
+        n = act.shape[0] * 256
+    else:
+        mask, bits, slot, n = B.Mask.full(), None, None, 12 << (2 * order)
+    X, G = _images(order, n, 5, "natural")
+    P = _sample_pixels(order, rng, 150)
+    Q = set()
+    for p in P:
+        for dy in range(-5, 6):
+            for dx in range(-5, 6):
+                q, _ = orc.hssim_neighbor(order, int(p), dx, dy)
+                if q >= 0:
+                    Q.add(q)
+    Q = np.array(sorted(Q), np.int64)
+    want = orc.hssim_loss(order, X, G, slot_of_tile=slot, bits=bits, q_list=Q)
+    l3, h, g = _run(B, cfg, mask, X, G)
+
+    def store(p):
+        if bits is not None and not (bits[p >> 5] >> (p & 31)) & 1:
+            return -1
+        s = p >> 8 if slot is None else slot[p >> 8]
+        return -1 if s < 0 else s * 256 + (p & 255)
+    iQ = np.array([store(int(q)) for q in Q]); iQ = iQ[iQ >= 0]
+    iP = np.array([store(int(p)) for p in P]); iP = iP[iP >= 0]
+    assert iQ.size > 5000 and iP.size > (60 if masked else 250)
+    assert np.abs(h[iQ] - want["h_map"][iQ]).max() <= TOL_H
+    scale = np.abs(want["grad"][iP]).max()
+    assert np.abs(g[iP] - want["grad"][iP]).max() <= TOL_G * scale
+    n_valid = n if bits is None else int(sum(bin(int(w)).count("1") for w in bits))
+    assert abs(l3[2] - h.astype(np.float64).sum() / n_valid) <= TOL_L
+    if bits is None:
+        assert abs(l3[1] - np.abs(X.astype(np.float64) - G).mean()) <= TOL_L
+    assert abs(l3[0] - (0.8 * l3[1] + 0.2 * (1 - l3[2]))) <= 1e-8              # lambda is an fp32 argument of the ABI

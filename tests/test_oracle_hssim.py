@@ -206,3 +206,28 @@ def test_gradient_against_central_differences(masked):
         fd = (orc.hssim_loss(order, Xp, G, bits=bits, grad=False)["loss"] - orc.hssim_loss(order, Xm, G, bits=bits, grad=False)["loss"]) / (2 * eps)
         worst = max(worst, abs(fd - o["grad"][p, ch]) / abs(fd))
     assert worst < 2e-4, worst
+
+
+def test_sampled_centres_equal_the_full_evaluation():
+    """hssim_loss(q_list=...) (used by the full-size GPU test) evaluates exactly the listed centres of the full evaluation: its
+    h_map equals the full one there and is 0 elsewhere, and with every pixel listed (in any order) loss and gradient are the full ones."""
+    order = 4
+    n = 12 << (2 * order)
+    rng = np.random.default_rng(11)
+    X = rng.uniform(size=(n, 3)).astype(np.float32); G = rng.uniform(size=(n, 3)).astype(np.float32)
+    bits = orc.mask_bits(order, "cap", [0.0, 1.0, 0.0, 1.2])
+    oc = orc.Config(order=order, n_gauss=1, n_views=1, sh_degree=0)
+    act, slot = orc.mask_tiles(oc, bits)
+    Xs, Gs = X[: act.shape[0] * 256], G[: act.shape[0] * 256]
+    full = orc.hssim_loss(order, Xs, Gs, slot_of_tile=slot, bits=bits)
+    pick = rng.choice(n, size=300, replace=False)
+    part = orc.hssim_loss(order, Xs, Gs, slot_of_tile=slot, bits=bits, q_list=pick)
+    idx = np.array([slot[p >> 8] * 256 + (p & 255) if (slot[p >> 8] >= 0 and (bits[p >> 5] >> (p & 31)) & 1) else -1 for p in pick])
+    live = idx[idx >= 0]
+    assert live.size > 50
+    assert np.array_equal(part["h_map"][live], full["h_map"][live])
+    rest = np.ones(Xs.shape[0], bool); rest[live] = False
+    assert not part["h_map"][rest].any()
+    everything = orc.hssim_loss(order, Xs, Gs, slot_of_tile=slot, bits=bits, q_list=rng.permutation(n))
+    assert abs(everything["loss"] - full["loss"]) < 1e-14
+    assert np.allclose(everything["grad"], full["grad"], rtol=1e-12, atol=1e-15)      # summation order differs

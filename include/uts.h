@@ -106,6 +106,12 @@ typedef struct {
 /* Alg.1 l.2-8.  For each view v and Gaussian i fills every array of `out` at index v*P+i.  Culled records
  * (rho <= r_near, non-finite input, det(Sigma_arc) <= 0) are written as zeros with flags bit0 set. */
 int uts_preprocess(const uts_config* cfg, uts_gaussians g, uts_views views, uts_proj out, void* stream);
+/* uts_preprocess in two calls, for callers that get the SH coefficients later than the geometry (the host call uploads them while the
+ * tile lists are built): uts_preprocess_geometry writes every array of `out` except rgb and needs no g.sh (flags: bit0 only);
+ * uts_preprocess_color then writes rgb and the clamp bits of flags from g.means, g.sh and the views (it reads flags bit0).
+ * geometry followed by color leaves `out` bit-identical to uts_preprocess. */
+int uts_preprocess_geometry(const uts_config* cfg, uts_gaussians g, uts_views views, uts_proj out, void* stream);
+int uts_preprocess_color(const uts_config* cfg, uts_gaussians g, uts_views views, uts_proj out, void* stream);
 
 /* Optional, Alg.1 l.15 moved ahead of the query: emit_rank[v*P+i] = position of (v,i) in the
  * stable order by (view, float_bits(rho), i).  Passing it to uts_tile_query makes the pairs come out already ordered by radial

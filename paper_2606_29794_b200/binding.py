@@ -19,7 +19,7 @@ UTS_OK, UTS_ERR_INVALID_ARG, UTS_ERR_CAPACITY, UTS_ERR_CUDA, UTS_ERR_UNSUPPORTED
 
 # every symbol include/uts.h declares
 SYMBOLS = [
-    "uts_preprocess", "uts_depth_order", "uts_depth_order_scratch_bytes", "uts_tile_query", "uts_tile_query_scratch_bytes", "uts_tile_lists", "uts_tile_lists_scratch_bytes", "uts_sort", "uts_sort_scratch_bytes",
+    "uts_preprocess", "uts_preprocess_geometry", "uts_preprocess_color", "uts_depth_order", "uts_depth_order_scratch_bytes", "uts_tile_query", "uts_tile_query_scratch_bytes", "uts_tile_lists", "uts_tile_lists_scratch_bytes", "uts_sort", "uts_sort_scratch_bytes",
     "uts_tile_ranges", "uts_render_fwd", "uts_render_bwd", "uts_preprocess_bwd", "uts_build_mask", "uts_pixel_centers",
     "uts_rho_max_table", "uts_resample_fwd", "uts_resample_bwd", "uts_build_camera_mask", "uts_inv_depth_channel", "uts_inv_depth_bwd", "uts_rs_max_update", "uts_hssim_loss", "uts_hssim_scratch_bytes",
     "uts_host_workspace_bytes", "uts_host_forward_backward", "uts_last_cuda_error", "uts_launch_count", "uts_strerror",
@@ -188,6 +188,16 @@ class Mask:
 def uts_preprocess(cfg: Config, g: Gaussians, views: Views, out: Proj, stream=None):
     c = cfg.c()
     _check(lib().uts_preprocess(C.byref(c), g.c(), views.c(), out.c(), _stream(stream)), "uts_preprocess")
+
+
+def uts_preprocess_geometry(cfg: Config, g: Gaussians, views: Views, out: Proj, stream=None):
+    c = cfg.c()
+    _check(lib().uts_preprocess_geometry(C.byref(c), g.c(), views.c(), out.c(), _stream(stream)), "uts_preprocess_geometry")
+
+
+def uts_preprocess_color(cfg: Config, g: Gaussians, views: Views, out: Proj, stream=None):
+    c = cfg.c()
+    _check(lib().uts_preprocess_color(C.byref(c), g.c(), views.c(), out.c(), _stream(stream)), "uts_preprocess_color")
 
 
 def uts_tile_query_scratch_bytes(cfg: Config) -> int:

@@ -91,20 +91,24 @@ int uts_host_forward_backward(const uts_config* cfg, const float* h_means, const
   UTS_CUDA(cudaMemcpyAsync(L.scales, h_scales, 3 * P * f, cudaMemcpyHostToDevice, s));
   UTS_CUDA(cudaMemcpyAsync(L.quats, h_quats, 4 * P * f, cudaMemcpyHostToDevice, s));
   UTS_CUDA(cudaMemcpyAsync(L.opac, h_opac, P * f, cudaMemcpyHostToDevice, s));
-  UTS_CUDA(cudaMemcpyAsync(L.sh, h_sh, 3 * M * P * f, cudaMemcpyHostToDevice, s));
   UTS_CUDA(cudaMemcpyAsync(L.W, h_W, 9 * V * f, cudaMemcpyHostToDevice, s));
   UTS_CUDA(cudaMemcpyAsync(L.b, h_b, 3 * V * f, cudaMemcpyHostToDevice, s));
-  // A second, library-private stream carries the copies that are not on the critical path: the upstream gradient goes up while
-  // the forward runs, the image comes down while the backward runs (effective with pinned host buffers).
+  // A second, library-private stream carries the copies that are not on the critical path: the SH coefficients (4/5 of the
+  // Gaussian bytes at degree 3) and the upstream gradient go up while the geometry is projected and the tile lists are built —
+  // only the colour pass, just before the blend, needs the SH — and the image comes down while the backward runs (effective
+  // with pinned host buffers).
   cudaStream_t s2 = nullptr;
-  cudaEvent_t ev_up = nullptr, ev_fwd = nullptr, ev_start = nullptr;
+  cudaEvent_t ev_up = nullptr, ev_fwd = nullptr, ev_start = nullptr, ev_sh = nullptr;
   UTS_CUDA(cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking));
   UTS_CUDA(cudaEventCreateWithFlags(&ev_up, cudaEventDisableTiming));
   UTS_CUDA(cudaEventCreateWithFlags(&ev_fwd, cudaEventDisableTiming));
   UTS_CUDA(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
-  struct Cleanup { cudaStream_t s2; cudaEvent_t a, b, c; ~Cleanup() { cudaStreamSynchronize(s2); cudaEventDestroy(a); cudaEventDestroy(b); cudaEventDestroy(c); cudaStreamDestroy(s2); } } cleanup{s2, ev_up, ev_fwd, ev_start};
+  UTS_CUDA(cudaEventCreateWithFlags(&ev_sh, cudaEventDisableTiming));
+  struct Cleanup { cudaStream_t s2; cudaEvent_t a, b, c, d; ~Cleanup() { cudaStreamSynchronize(s2); cudaEventDestroy(a); cudaEventDestroy(b); cudaEventDestroy(c); cudaEventDestroy(d); cudaStreamDestroy(s2); } } cleanup{s2, ev_up, ev_fwd, ev_start, ev_sh};
   UTS_CUDA(cudaEventRecord(ev_start, s));                 // s2 must not run ahead of work already queued on the caller's stream
   UTS_CUDA(cudaStreamWaitEvent(s2, ev_start, 0));
+  UTS_CUDA(cudaMemcpyAsync(L.sh, h_sh, 3 * M * P * f, cudaMemcpyHostToDevice, s2));
+  UTS_CUDA(cudaEventRecord(ev_sh, s2));
   if (bwd) {
     UTS_CUDA(cudaMemcpyAsync(L.g_color, h_dL_dcolor, 3 * npx * f, cudaMemcpyHostToDevice, s2));
     UTS_CUDA(cudaEventRecord(ev_up, s2));
@@ -112,12 +116,14 @@ int uts_host_forward_backward(const uts_config* cfg, const float* h_means, const
 
   uts_gaussians g{L.means, L.scales, L.quats, L.opac, L.sh};
   uts_views vw{L.W, L.b};
-  if ((st = uts_preprocess(cfg, g, vw, L.proj, stream))) return st;
+  if ((st = uts_preprocess_geometry(cfg, g, vw, L.proj, stream))) return st;
   if ((st = uts_depth_order(cfg, L.proj.rho, L.emit_rank, L.do_scratch, L.do_bytes, stream))) return st;
   // Alg.1 l.9-16 in one call: sorted pairs + tile ranges (large discs through the bit matrix, the rest through emit + radix sort)
   if ((st = uts_tile_lists(cfg, L.proj, mask, L.emit_rank, L.keys, L.vals, L.keys_tmp, L.vals_tmp, pair_capacity, L.ranges, h_n_pairs,
                            L.tq_scratch, L.tq_bytes, L.sort_scratch, L.sort_bytes, stream)))
     return st;
+  UTS_CUDA(cudaStreamWaitEvent(s, ev_sh, 0));
+  if ((st = uts_preprocess_color(cfg, g, vw, L.proj, stream))) return st;
   if ((st = uts_render_fwd(cfg, L.proj, mask, L.ranges, L.vals, L.color, L.alpha, L.trans, L.n_last, stream))) return st;
   UTS_CUDA(cudaEventRecord(ev_fwd, s));
   UTS_CUDA(cudaStreamWaitEvent(s2, ev_fwd, 0));

@@ -135,6 +135,9 @@ __device__ __forceinline__ void geometry(const ViewConst& vc, const double mu[3]
   if (!(g.det > 0) || !isfinite(g.det)) g.culled = true;                   // reading A23
 }
 
+// PARTS: 1 = geometry records only (everything but rgb; needs no SH), 2 = colour only (rgb and the clamp bits of flags, on records
+// whose geometry part has run), 3 = both in one pass (uts_preprocess).  1 then 2 writes exactly what 3 writes.
+template <int PARTS>
 __global__ void __launch_bounds__(128, 6)
 preprocess_fwd_kernel(uts_config cfg, const float* __restrict__ means, const float* __restrict__ scales,
                       const float* __restrict__ quats, const float* __restrict__ opac, const float* __restrict__ sh,
@@ -145,28 +148,48 @@ preprocess_fwd_kernel(uts_config cfg, const float* __restrict__ means, const flo
   if (i >= P) return;
   ViewConst vc; load_view(Wv, bv, v, vc);
   const double mu[3] = {(double)__ldg(means + 3 * i), (double)__ldg(means + 3 * i + 1), (double)__ldg(means + 3 * i + 2)};
-  const double s[3] = {(double)__ldg(scales + 3 * i), (double)__ldg(scales + 3 * i + 1), (double)__ldg(scales + 3 * i + 2)};
-  const float4 qf = __ldg(reinterpret_cast<const float4*>(quats) + i);
-  const double q[4] = {(double)qf.x, (double)qf.y, (double)qf.z, (double)qf.w};
-  const float o = __ldg(opac + i);
-  Geo g;
-  geometry(vc, mu, s, q, (double)cfg.r_near, h, g);
-  if (!isfinite(o)) g.culled = true;
+  double s[3] = {0, 0, 0}, q[4] = {0, 0, 0, 0};
+  float o = 0.f;
+  if (PARTS & 1) {
+    s[0] = (double)__ldg(scales + 3 * i); s[1] = (double)__ldg(scales + 3 * i + 1); s[2] = (double)__ldg(scales + 3 * i + 2);
+    const float4 qf = __ldg(reinterpret_cast<const float4*>(quats) + i);
+    q[0] = (double)qf.x; q[1] = (double)qf.y; q[2] = (double)qf.z; q[3] = (double)qf.w;
+    o = __ldg(opac + i);
+  }
   const size_t k = (size_t)v * P + i;
+  Geo g;
+  if (PARTS & 1) {
+    geometry(vc, mu, s, q, (double)cfg.r_near, h, g);
+    if (!isfinite(o)) g.culled = true;
+  } else {
+    g.culled = (out.flags[k] & 1) != 0;
+  }
   if (g.culled) {
-    out.dir[3 * k] = out.dir[3 * k + 1] = out.dir[3 * k + 2] = 0.f;
-    out.lonlat[2 * k] = out.lonlat[2 * k + 1] = 0.f;
-    out.rho[k] = 0.f; out.rs[k] = 0.f;
-    reinterpret_cast<float4*>(out.conic_opac)[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-    out.rgb[3 * k] = out.rgb[3 * k + 1] = out.rgb[3 * k + 2] = 0.f;
-    out.flags[k] = 1;
+    if (PARTS & 1) {
+      out.dir[3 * k] = out.dir[3 * k + 1] = out.dir[3 * k + 2] = 0.f;
+      out.lonlat[2 * k] = out.lonlat[2 * k + 1] = 0.f;
+      out.rho[k] = 0.f; out.rs[k] = 0.f;
+      reinterpret_cast<float4*>(out.conic_opac)[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+      out.flags[k] = 1;
+    }
+    if (PARTS & 2) out.rgb[3 * k] = out.rgb[3 * k + 1] = out.rgb[3 * k + 2] = 0.f;
     return;
   }
-  // l.7: r_s = 3 sqrt(lambda_max), clamped to pi (reading A4)
-  const double hd = 0.5 * (g.a - g.c);
-  const double lmax = 0.5 * (g.a + g.c) + sqrt(fmax(0.0, hd * hd + g.b * g.b));
-  const double rs = fmin(kPi, 3.0 * sqrt(lmax));
-  const double idet = 1.0 / g.det;
+  if (PARTS & 1) {
+    // l.7: r_s = 3 sqrt(lambda_max), clamped to pi (reading A4)
+    const double hd = 0.5 * (g.a - g.c);
+    const double lmax = 0.5 * (g.a + g.c) + sqrt(fmax(0.0, hd * hd + g.b * g.b));
+    const double rs = fmin(kPi, 3.0 * sqrt(lmax));
+    const double idet = 1.0 / g.det;
+    out.dir[3 * k] = (float)g.u[0]; out.dir[3 * k + 1] = (float)g.u[1]; out.dir[3 * k + 2] = (float)g.u[2];
+    out.lonlat[2 * k] = (float)atan2(g.t[0], g.t[2]);                         // Eq.1
+    out.lonlat[2 * k + 1] = (float)atan2(g.t[1], g.rxz);
+    out.rho[k] = (float)g.rho;
+    out.rs[k] = (float)rs;
+    reinterpret_cast<float4*>(out.conic_opac)[k] =
+        make_float4((float)(g.c * idet), (float)(-g.b * idet), (float)(g.a * idet), o);   // Sigma_arc^{-1}
+    if (!(PARTS & 2)) { out.flags[k] = 0; return; }
+  }
   // colour (reading A13): direction from the camera centre to mu in world space
   double vd[3] = {mu[0] - vc.cam[0], mu[1] - vc.cam[1], mu[2] - vc.cam[2]};
   const double vl = sqrt(vd[0] * vd[0] + vd[1] * vd[1] + vd[2] * vd[2]);
@@ -205,15 +228,8 @@ preprocess_fwd_kernel(uts_config cfg, const float* __restrict__ means, const flo
 #pragma unroll
   for (int ch = 0; ch < 3; ++ch) if (acc[ch] < 0.f) { acc[ch] = 0.f; fl |= (uint8_t)(2u << ch); }
 
-  out.dir[3 * k] = (float)g.u[0]; out.dir[3 * k + 1] = (float)g.u[1]; out.dir[3 * k + 2] = (float)g.u[2];
-  out.lonlat[2 * k] = (float)atan2(g.t[0], g.t[2]);                         // Eq.1
-  out.lonlat[2 * k + 1] = (float)atan2(g.t[1], g.rxz);
-  out.rho[k] = (float)g.rho;
-  out.rs[k] = (float)rs;
-  reinterpret_cast<float4*>(out.conic_opac)[k] =
-      make_float4((float)(g.c * idet), (float)(-g.b * idet), (float)(g.a * idet), o);   // Sigma_arc^{-1}
   out.rgb[3 * k] = acc[0]; out.rgb[3 * k + 1] = acc[1]; out.rgb[3 * k + 2] = acc[2];
-  out.flags[k] = fl;
+  out.flags[k] = fl;                     // (a record that reaches this line is not culled: bit0 = 0)
 }
 
 // ------------------------------------------------------------------------------------------- backward
@@ -376,7 +392,31 @@ int uts_preprocess(const uts_config* cfg, uts_gaussians g, uts_views views, uts_
   if (cfg->n_gauss == 0) return UTS_OK;
   const double h = (double)cfg->cov_dilation_px2 * 4.0 * kPi / (double)((int64_t)12 << (2 * cfg->order));
   dim3 grid((cfg->n_gauss + 127) / 128, cfg->n_views);
-  preprocess_fwd_kernel<<<grid, 128, 0, (cudaStream_t)stream>>>(*cfg, g.means, g.scales, g.quats, g.opac, g.sh, views.W, views.b, out, h);
+  preprocess_fwd_kernel<3><<<grid, 128, 0, (cudaStream_t)stream>>>(*cfg, g.means, g.scales, g.quats, g.opac, g.sh, views.W, views.b, out, h);
+  UTS_LAUNCH_CHECK();
+  return UTS_OK;
+}
+
+int uts_preprocess_geometry(const uts_config* cfg, uts_gaussians g, uts_views views, uts_proj out, void* stream) {
+  int st = check_config(cfg);
+  if (st) return st;
+  if (!g.means || !g.scales || !g.quats || !g.opac || !views.W || !views.b) return UTS_ERR_INVALID_ARG;
+  if (!out.dir || !out.lonlat || !out.rho || !out.conic_opac || !out.rs || !out.flags) return UTS_ERR_INVALID_ARG;
+  if (cfg->n_gauss == 0) return UTS_OK;
+  const double h = (double)cfg->cov_dilation_px2 * 4.0 * kPi / (double)((int64_t)12 << (2 * cfg->order));
+  dim3 grid((cfg->n_gauss + 127) / 128, cfg->n_views);
+  preprocess_fwd_kernel<1><<<grid, 128, 0, (cudaStream_t)stream>>>(*cfg, g.means, g.scales, g.quats, g.opac, nullptr, views.W, views.b, out, h);
+  UTS_LAUNCH_CHECK();
+  return UTS_OK;
+}
+
+int uts_preprocess_color(const uts_config* cfg, uts_gaussians g, uts_views views, uts_proj out, void* stream) {
+  int st = check_config(cfg);
+  if (st) return st;
+  if (!g.means || !g.sh || !views.W || !views.b || !out.rgb || !out.flags) return UTS_ERR_INVALID_ARG;
+  if (cfg->n_gauss == 0) return UTS_OK;
+  dim3 grid((cfg->n_gauss + 127) / 128, cfg->n_views);
+  preprocess_fwd_kernel<2><<<grid, 128, 0, (cudaStream_t)stream>>>(*cfg, g.means, nullptr, nullptr, nullptr, g.sh, views.W, views.b, out, 0.0);
   UTS_LAUNCH_CHECK();
   return UTS_OK;
 }

@@ -154,6 +154,31 @@ def test_preprocess_culls_and_degree_variants():
         assert np.allclose(out.conic_opac.cpu().numpy(), want.conic_opac, rtol=1e-6, atol=1e-6)
 
 
+def test_preprocess_in_two_calls_is_bit_identical():
+    """uts_preprocess_geometry (no SH needed) followed by uts_preprocess_color leaves the records bit-identical to uts_preprocess
+    (the host call uploads the SH while the tile lists are built); checked with culled, clamped and multi-view records."""
+    B, R = _gpu()
+    for deg, V in ((0, 1), (3, 1), (2, 3)):
+        scene = small_scene(5, 4000, 6, sh_degree=deg, n_views=V)
+        scene["means"][:5] *= 1e-3; scene["means"][5] = np.nan
+        scene["sh"][7:400] -= 0.6                                   # pushes colours below 0: clamp bits
+        cfg = _cfg(R, scene)
+        g, views = R.scene_to_device(scene)
+        one = B.Proj.empty(cfg); two = B.Proj.empty(cfg)
+        for t in (two.dir, two.lonlat, two.rho, two.conic_opac, two.rs, two.rgb):
+            t.fill_(-3.0)
+        two.flags.fill_(255)
+        B.uts_preprocess(cfg, g, views, one)
+        no_sh = B.Gaussians(g.means, g.scales, g.quats, g.opac, None)
+        B.uts_preprocess_geometry(cfg, no_sh, views, two)
+        assert int((two.flags > 1).sum()) == 0
+        B.uts_preprocess_color(cfg, B.Gaussians(g.means, None, None, None, g.sh), views, two)
+        torch.cuda.synchronize()
+        assert int((one.flags & 1).sum()) >= 6 * V and int((one.flags > 1).sum()) > 0
+        for name in ("dir", "lonlat", "rho", "conic_opac", "rs", "rgb", "flags"):
+            assert torch.equal(getattr(one, name), getattr(two, name)), name
+
+
 # ------------------------------------------------------------------------------------------- F2
 @pytest.mark.parametrize("cfg_id,P,order,extra", CASES)
 def test_tile_query_bit_exact(cfg_id, P, order, extra):

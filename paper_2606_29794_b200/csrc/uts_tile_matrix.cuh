@@ -196,23 +196,27 @@ matrix_popcount_kernel(MatParams mp, int V, int64_t n_tile) {
 }
 
 // ---------------------------------------------------------------------------------------------- emit + merge
-__device__ __forceinline__ bool pair_less(uint64_t ka, uint32_t va, uint64_t kb, uint32_t vb) { return ka < kb || (ka == kb && va < vb); }
-
-// number of entries of the sorted buffer (bk, bv)[0, n) that are less than (k, v)
-__device__ __forceinline__ uint32_t buf_lower_bound(const unsigned long long* bk, const uint32_t* bv, uint32_t n, unsigned long long k, uint32_t v) {
+// Inside one (view, tile) list every key has the same high word, so an entry is ordered by (depth bits, Gaussian id) alone: the
+// merge buffers hold that pair packed in one 64-bit word, (depth << 32) | id — the form row_key already has — and one unsigned
+// compare orders two entries.
+// number of entries of the sorted buffer b[0, n) that are less than x
+__device__ __forceinline__ uint32_t buf_lower_bound(const unsigned long long* b, uint32_t n, unsigned long long x) {
   uint32_t lo = 0, hi = n;
-  while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (pair_less(bk[mid], bv[mid], k, v)) lo = mid + 1; else hi = mid; }
+  while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (b[mid] < x) lo = mid + 1; else hi = mid; }
   return lo;
 }
 
 // One warp per (view, tile) writes the tile's FINAL list at keys / vals[start[vt] ...): a streaming merge of two depth-ordered
-// streams held in shared memory 128 entries at a time —
-//   A: the large discs of the tile, generated from its bit vector (set bit r = matrix row r; key from row_key[r]),
+// streams held in shared memory 256 entries at a time —
+//   A: the large discs of the tile, generated from its bit vector (set bit r = matrix row r; entry = row_key[r]),
 //   B: the tile's small-disc pairs, already radix-sorted (keysS / valsS[s_ranges[vt] ...)).
 // Each round refills both buffers, emits everything up to the smaller of the two "last buffered" entries of streams that still
-// continue (so nothing that could precede an emitted entry is still unread), ranks every emitted entry by a binary search in the
-// other buffer (the two streams never tie: different Gaussians) and stores it straight at its final position — consecutive lanes
-// hit nearly consecutive addresses — then shifts the unconsumed entries to the front.  One buffer is fully consumed per round.
+// continue (so nothing that could precede an emitted entry is still unread) and stores every emitted entry straight at its final
+// position, own index + rank in the other buffer (the two streams never tie: different Gaussians) — consecutive lanes hit nearly
+// consecutive addresses.  Ranks: the B entries (the minority) by binary search in A; the A entries from those — B[j] precedes A[i]
+// iff rank_A(B[j]) <= i, so a histogram of the B ranks over the A positions, prefix-summed by the warp, is every A entry's rank at
+// once (a binary search per A entry was half of this kernel's instructions).  Then the unconsumed entries shift to the front;
+// one buffer is fully consumed per round.
 #ifndef UTS_MB
 #define UTS_MB 256
 #endif
@@ -220,14 +224,15 @@ __device__ __forceinline__ uint32_t buf_lower_bound(const unsigned long long* bk
 #define UTS_MB_MINB 4
 #endif
 constexpr int kMB = UTS_MB;
+static_assert(kMB == 256, "the rank scan below gives every lane 8 consecutive A positions");
 __global__ void __launch_bounds__(256, UTS_MB_MINB)
 matrix_emit_merge_kernel(MatParams mp, int V, int64_t n_tile, const uint64_t* __restrict__ start, const uint64_t* __restrict__ s_ranges,
                          const uint64_t* __restrict__ keysS, const uint32_t* __restrict__ valsS, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
-  __shared__ unsigned long long sAk[8][kMB], sBk[8][kMB];
-  __shared__ uint32_t sAv[8][kMB], sBv[8][kMB];
+  __shared__ unsigned long long sA[8][kMB], sB[8][kMB];
+  __shared__ __align__(16) uint32_t sH[8][kMB];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  unsigned long long* Ak = sAk[wid]; unsigned long long* Bk = sBk[wid];
-  uint32_t* Av = sAv[wid]; uint32_t* Bv = sBv[wid];
+  unsigned long long* A = sA[wid]; unsigned long long* Bq = sB[wid];
+  uint32_t* H = sH[wid];
   const int64_t n = (int64_t)V * n_tile;
   for (int64_t vt = (int64_t)blockIdx.x * 8 + wid; vt < n; vt += (int64_t)gridDim.x * 8) {
     uint64_t o = start[vt];
@@ -264,7 +269,7 @@ matrix_emit_merge_kernel(MatParams mp, int V, int64_t n_tile, const uint64_t* __
         const uint32_t row0 = (w_cur + lane) * 32;
         while (x && r < room) {                            // phase 1: matrix rows of the set bits (no memory access)
           const int b = __ffs((int)x) - 1; x &= x - 1;
-          Av[fillA + r] = row0 + (uint32_t)b; ++r;
+          A[fillA + r] = row0 + (uint32_t)b; ++r;
         }
         fillA += tot < room ? tot : room;
       }
@@ -275,13 +280,13 @@ matrix_emit_merge_kernel(MatParams mp, int V, int64_t n_tile, const uint64_t* __
 #pragma unroll
         for (int q = 0; q < kMB / 32; ++q) {
           const uint32_t i = fillA0 + lane + 32 * q;
-          if (i < fillA) { const unsigned long long k2 = __ldg(rk + Av[i]); Ak[i] = hi | (k2 >> 32); Av[i] = (uint32_t)k2; }
+          if (i < fillA) A[i] = __ldg(rk + (uint32_t)A[i]);
         }
       }
       // ---- refill B from the sorted small pairs
       if (fillB < (uint32_t)kMB && b_pos < b_end) {
         const uint32_t take = (uint32_t)(((uint64_t)kMB - fillB) < (b_end - b_pos) ? ((uint64_t)kMB - fillB) : (b_end - b_pos));
-        for (uint32_t j = lane; j < take; j += 32) { Bk[fillB + j] = keysS[b_pos + j]; Bv[fillB + j] = valsS[b_pos + j]; }
+        for (uint32_t j = lane; j < take; j += 32) Bq[fillB + j] = (keysS[b_pos + j] << 32) | valsS[b_pos + j];
         b_pos += take; fillB += take;
       }
       __syncwarp();
@@ -289,36 +294,60 @@ matrix_emit_merge_kernel(MatParams mp, int V, int64_t n_tile, const uint64_t* __
       const bool b_done = b_pos == b_end;
       uint32_t na = fillA, nb = fillB;
       if (fillA && fillB && !(a_done && b_done)) {
-        const bool lastA_smaller = pair_less(Ak[fillA - 1], Av[fillA - 1], Bk[fillB - 1], Bv[fillB - 1]);
+        const bool lastA_smaller = A[fillA - 1] < Bq[fillB - 1];
         const bool bound_is_A = !a_done && (b_done || lastA_smaller);
-        if (bound_is_A) nb = buf_lower_bound(Bk, Bv, fillB, Ak[fillA - 1], Av[fillA - 1]);
-        else na = buf_lower_bound(Ak, Av, fillA, Bk[fillB - 1], Bv[fillB - 1]);
+        if (bound_is_A) nb = buf_lower_bound(Bq, fillB, A[fillA - 1]);
+        else na = buf_lower_bound(A, fillA, Bq[fillB - 1]);
       } else if (fillA && !fillB && !b_done) { na = 0; }      // cannot happen: B is refilled whenever it has entries left
       // ---- rank and store
-      for (uint32_t i = lane; i < na; i += 32) {
-        const unsigned long long kk = Ak[i]; const uint32_t vv = Av[i];
-        const uint64_t pos = o + i + buf_lower_bound(Bk, Bv, nb, kk, vv);
-        keys[pos] = kk; vals[pos] = vv;
-      }
-      for (uint32_t j = lane; j < nb; j += 32) {
-        const unsigned long long kk = Bk[j]; const uint32_t vv = Bv[j];
-        const uint64_t pos = o + j + buf_lower_bound(Ak, Av, na, kk, vv);
-        keys[pos] = kk; vals[pos] = vv;
+      if (nb == 0) {
+        for (uint32_t i = lane; i < na; i += 32) { const unsigned long long p = A[i]; keys[o + i] = hi | (p >> 32); vals[o + i] = (uint32_t)p; }
+      } else {
+        if (na) {
+#pragma unroll
+          for (int q = 0; q < kMB / 32; ++q) H[lane + 32 * q] = 0u;
+          __syncwarp();
+        }
+        for (uint32_t j = lane; j < nb; j += 32) {
+          const unsigned long long p = Bq[j];
+          const uint32_t rb = buf_lower_bound(A, na, p);
+          if (rb < na) atomicAdd(&H[rb], 1u);              // B[j] precedes A[rb], A[rb+1], ...
+          const uint64_t pos = o + j + rb;
+          keys[pos] = hi | (p >> 32); vals[pos] = (uint32_t)p;
+        }
+        if (na) {
+          __syncwarp();
+          // inclusive prefix sum of H over the A positions: lane l owns positions 8l .. 8l+7
+          uint4 h0 = reinterpret_cast<uint4*>(H)[2 * lane], h1 = reinterpret_cast<uint4*>(H)[2 * lane + 1];
+          h0.y += h0.x; h0.z += h0.y; h0.w += h0.z; h1.x += h0.w; h1.y += h1.x; h1.z += h1.y; h1.w += h1.z;
+          uint32_t incl = h1.w;
+#pragma unroll
+          for (int d = 1; d < 32; d <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += y; }
+          const uint32_t ex = incl - h1.w;
+          h0.x += ex; h0.y += ex; h0.z += ex; h0.w += ex; h1.x += ex; h1.y += ex; h1.z += ex; h1.w += ex;
+          reinterpret_cast<uint4*>(H)[2 * lane] = h0; reinterpret_cast<uint4*>(H)[2 * lane + 1] = h1;
+          __syncwarp();
+          for (uint32_t i = lane; i < na; i += 32) {
+            const unsigned long long p = A[i];
+            const uint64_t pos = o + i + H[i];
+            keys[pos] = hi | (p >> 32); vals[pos] = (uint32_t)p;
+          }
+        }
       }
       o += na + nb;
       // ---- shift the unconsumed entries to the front
-      unsigned long long tk[kMB / 32]; uint32_t tv[kMB / 32];
+      unsigned long long tk[kMB / 32];
 #pragma unroll
-      for (int q = 0; q < kMB / 32; ++q) { const uint32_t i = na + lane + 32 * q; if (i < fillA) { tk[q] = Ak[i]; tv[q] = Av[i]; } }
+      for (int q = 0; q < kMB / 32; ++q) { const uint32_t i = na + lane + 32 * q; if (i < fillA) tk[q] = A[i]; }
       __syncwarp();
 #pragma unroll
-      for (int q = 0; q < kMB / 32; ++q) { const uint32_t i = na + lane + 32 * q; if (i < fillA) { Ak[i - na] = tk[q]; Av[i - na] = tv[q]; } }
+      for (int q = 0; q < kMB / 32; ++q) { const uint32_t i = na + lane + 32 * q; if (i < fillA) A[i - na] = tk[q]; }
       fillA -= na;
 #pragma unroll
-      for (int q = 0; q < kMB / 32; ++q) { const uint32_t i = nb + lane + 32 * q; if (i < fillB) { tk[q] = Bk[i]; tv[q] = Bv[i]; } }
+      for (int q = 0; q < kMB / 32; ++q) { const uint32_t i = nb + lane + 32 * q; if (i < fillB) tk[q] = Bq[i]; }
       __syncwarp();
 #pragma unroll
-      for (int q = 0; q < kMB / 32; ++q) { const uint32_t i = nb + lane + 32 * q; if (i < fillB) { Bk[i - nb] = tk[q]; Bv[i - nb] = tv[q]; } }
+      for (int q = 0; q < kMB / 32; ++q) { const uint32_t i = nb + lane + 32 * q; if (i < fillB) Bq[i - nb] = tk[q]; }
       fillB -= nb;
       __syncwarp();
     }

@@ -68,7 +68,16 @@ __global__ void mat_view_tab_kernel(MatParams mp, int P, int V, int64_t n_tile) 
 }
 
 // ---------------------------------------------------------------------------------------------- count: bitmap rows
-__global__ void __launch_bounds__(kLargeThreads, 4)
+// One block per large disc at a time.  A disc costs a chain of dependent phases (load, ring table, rows, row copy) with block-wide
+// barriers between them, so what matters is how many discs an SM has in flight: blocks of kMatThreads threads.
+#ifndef UTS_MAT_THREADS
+#define UTS_MAT_THREADS 64
+#endif
+#ifndef UTS_MAT_MINB
+#define UTS_MAT_MINB 16
+#endif
+constexpr int kMatThreads = UTS_MAT_THREADS;
+__global__ void __launch_bounds__(kMatThreads, UTS_MAT_MINB)
 matrix_count_kernel(QueryParams qp, MatParams mp, const float* __restrict__ dir, const float* __restrict__ lonlat, const float* __restrict__ rho,
                     const float* __restrict__ rs, const int32_t* __restrict__ slot_of_tile, const uint32_t* __restrict__ active_words,
                     const uint32_t* __restrict__ perm, const uint32_t* __restrict__ n_small, const uint32_t* __restrict__ emit_rank,
@@ -87,7 +96,7 @@ matrix_count_kernel(QueryParams qp, MatParams mp, const float* __restrict__ dir,
     const uint32_t row = (uint32_t)mp.row_of_rank[slot];
     const int v = (int)(k / qp.P);
     __syncthreads();                                   // the previous disc is done with shared memory
-    for (int w = tid; w < mp.n_words; w += kLargeThreads) bitmap[w] = 0u;
+    for (int w = tid; w < mp.n_words; w += kMatThreads) bitmap[w] = 0u;
     if (tid < 32) {                                    // set-up by the first warp: lane 0 the disc, lanes 0..11 one face each
       if (tid == 0) {
         load_ring_disc(qp, dir, lonlat, rs, k, s_disc);
@@ -106,17 +115,17 @@ matrix_count_kernel(QueryParams qp, MatParams mp, const float* __restrict__ dir,
     __syncthreads();
     const RingDisc& D = s_disc;
     if (D.all) {                                       // reading A24: every active tile
-      for (int w = tid; w < mp.n_words; w += kLargeThreads) bitmap[w] = active_words ? __ldg(active_words + w) : 0xffffffffu;
+      for (int w = tid; w < mp.n_words; w += kMatThreads) bitmap[w] = active_words ? __ldg(active_words + w) : 0xffffffffu;
       if (tid == 0) s_total = qp.active_tiles ? (uint32_t)qp.n_active : (uint32_t)qp.n_tile;
     } else {
-      for (int e = tid; e <= D.i_hi - D.i_lo; e += kLargeThreads) { int2 fl; ring_interval(D, N, D.i_lo + e, fl.x, fl.y); ring_tab[e] = fl; }
+      for (int e = tid; e <= D.i_hi - D.i_lo; e += kMatThreads) { int2 fl; ring_interval(D, N, D.i_lo + e, fl.x, fl.y); ring_tab[e] = fl; }
       __syncthreads();
       const GroupTab T{ring_tab, D.i_lo};
       const int n_rows = (int)s_pre[12];
       const int n_chunks = ((1 << qp.kt) + 63) >> 6;
       const int n_items = n_rows * n_chunks;
       uint32_t mine = 0;
-      for (int item = tid; item < n_items; item += kLargeThreads) {
+      for (int item = tid; item < n_items; item += kMatThreads) {
         const int rowi = item / n_chunks, jbase = (item - rowi * n_chunks) << 6;
         int f = 0;
         while (f < 11 && (int)s_pre[f + 1] <= rowi) ++f;
@@ -131,7 +140,7 @@ matrix_count_kernel(QueryParams qp, MatParams mp, const float* __restrict__ dir,
     }
     __syncthreads();
     uint32_t* dst = mp.M + (size_t)row * mp.n_words;
-    for (int w = tid; w < mp.n_words; w += kLargeThreads) dst[w] = bitmap[w];
+    for (int w = tid; w < mp.n_words; w += kMatThreads) dst[w] = bitmap[w];
     if (tid == 0) {
       counts[slot] = 0;                                // this disc emits no pairs of its own
       const uint32_t gid = (uint32_t)(k - (int64_t)v * qp.P);

@@ -1077,8 +1077,8 @@ struct QueryRun {
       if (mp) {
         const size_t smem_m = smem_block + (size_t)mp->n_words * 4;
         int occ = 1;
-        UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, matrix_count_kernel, kLargeThreads, smem_m));
-        matrix_count_kernel<<<(unsigned)sm_count() * (unsigned)(occ > 0 ? occ : 1), kLargeThreads, smem_m, s>>>(
+        UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, matrix_count_kernel, kMatThreads, smem_m));
+        matrix_count_kernel<<<(unsigned)sm_count() * (unsigned)(occ > 0 ? occ : 1), kMatThreads, smem_m, s>>>(
             qp, *mp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, mask.slot_of_tile ? active : nullptr, perm, n_small, emit_rank, counts);
         UTS_LAUNCH_CHECK();
       }

@@ -199,7 +199,7 @@ def run_ours(args):
     fused = args.lists == "fused"
     STAGES = STAGES_FUSED if fused else STAGES_STAGED
     NS = len(STAGES)
-    r = R.Rasterizer(cfg, mask, fused_lists=fused)
+    r = R.Rasterizer(cfg, mask, fused_lists=fused, marks=(args.marks == "on"))
     V, S = cfg.n_views, r.S
     npx = S * cfg.ppt
     gcol = torch.from_numpy(scenes.upstream_grad(V, npx, seed=rank)).cuda()
@@ -414,6 +414,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--lists", default="fused", choices=["fused", "staged"],
                     help="Alg.1 l.9-16 as one uts_tile_lists call (default) or as uts_tile_query + uts_sort + uts_tile_ranges")
+    ap.add_argument("--marks", default="on", choices=["on", "off"],
+                    help="blend through uts_render_fwd_marked / uts_render_bwd_marked (default) or the plain pair")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -184,6 +184,21 @@ int uts_render_bwd(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
                    const float* trans, const uint32_t* n_last, const float* dL_dcolor, const float* dL_dalpha,
                    float* dL_drgb, float* dL_dconic, float* dL_dmu2, float* dL_dopac, void* stream);
 
+/* The blend pair with MARKS: uts_render_fwd_marked also records, per warp of a tile's thread block (8 warps of 32 pixels) and list
+ * entry, whether any of the warp's pixels blended the entry; uts_render_bwd_marked visits only the marked (warp, entry) pairs.
+ * Outputs are those of uts_render_fwd / uts_render_bwd (same decisions per pixel: the image is bit-identical, the gradients are the
+ * same sums in a possibly different order).  marks: uts_render_marks_bytes(cfg, pair_capacity) bytes, 4-byte aligned, written by
+ * the forward, read by the backward.  It need not be cleared: the forward writes every word that describes an entry one of the warp's
+ * pixels reached, and stale bits beyond cost the backward one vote each, never a wrong sum with the same cfg / ranges / pair_capacity (>= the number of pairs in vals). */
+size_t uts_render_marks_bytes(const uts_config* cfg, uint64_t pair_capacity);
+int uts_render_fwd_marked(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
+                          uint64_t pair_capacity, float* color, float* alpha, float* trans, uint32_t* n_last, uint32_t* marks,
+                          size_t marks_bytes, void* stream);
+int uts_render_bwd_marked(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
+                          uint64_t pair_capacity, const float* trans, const uint32_t* n_last, const uint32_t* marks,
+                          const float* dL_dcolor, const float* dL_dalpha, float* dL_drgb, float* dL_dconic, float* dL_dmu2,
+                          float* dL_dopac, void* stream);
+
 /* Eq.3-4 and the rest of the chain: every output is overwritten with the sum over views.
  * dL_dmeans [P,3], dL_dscales [P,3], dL_dquats [P,4] (gradient of the R(q) polynomial), dL_dsh [P,M,3]. */
 int uts_preprocess_bwd(const uts_config* cfg, uts_gaussians g, uts_views views, const uint8_t* flags,

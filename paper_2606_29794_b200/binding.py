@@ -20,7 +20,7 @@ UTS_OK, UTS_ERR_INVALID_ARG, UTS_ERR_CAPACITY, UTS_ERR_CUDA, UTS_ERR_UNSUPPORTED
 # every symbol include/uts.h declares
 SYMBOLS = [
     "uts_preprocess", "uts_preprocess_geometry", "uts_preprocess_color", "uts_depth_order", "uts_depth_order_scratch_bytes", "uts_tile_query", "uts_tile_query_scratch_bytes", "uts_tile_lists", "uts_tile_lists_scratch_bytes", "uts_sort", "uts_sort_scratch_bytes",
-    "uts_tile_ranges", "uts_render_fwd", "uts_render_bwd", "uts_preprocess_bwd", "uts_build_mask", "uts_pixel_centers",
+    "uts_tile_ranges", "uts_render_fwd", "uts_render_bwd", "uts_render_marks_bytes", "uts_render_fwd_marked", "uts_render_bwd_marked", "uts_preprocess_bwd", "uts_build_mask", "uts_pixel_centers",
     "uts_rho_max_table", "uts_resample_fwd", "uts_resample_bwd", "uts_build_camera_mask", "uts_inv_depth_channel", "uts_inv_depth_bwd", "uts_rs_max_update", "uts_hssim_loss", "uts_hssim_scratch_bytes",
     "uts_host_workspace_bytes", "uts_host_forward_backward", "uts_last_cuda_error", "uts_launch_count", "uts_strerror",
     "uts_version",
@@ -107,7 +107,7 @@ def lib():
         L = C.CDLL(LIB_PATH)
         L.uts_strerror.restype = C.c_char_p
         L.uts_version.restype = C.c_char_p
-        for n in ("uts_hssim_scratch_bytes", "uts_depth_order_scratch_bytes", "uts_tile_query_scratch_bytes", "uts_sort_scratch_bytes", "uts_host_workspace_bytes"):
+        for n in ("uts_render_marks_bytes", "uts_hssim_scratch_bytes", "uts_depth_order_scratch_bytes", "uts_tile_query_scratch_bytes", "uts_sort_scratch_bytes", "uts_host_workspace_bytes"):
             getattr(L, n).restype = C.c_size_t
         L.uts_sort_scratch_bytes.argtypes = [C.c_uint64]
         L.uts_host_workspace_bytes.argtypes = [C.POINTER(CConfig), C.c_int, C.c_uint64]
@@ -288,6 +288,27 @@ def uts_render_bwd(cfg: Config, proj: Proj, mask: Mask, ranges, vals, trans, n_l
                                 _ptr(trans, torch.float32), _ptr(n_last, torch.int32), _ptr(dL_dcolor, torch.float32),
                                 _ptr(dL_dalpha, torch.float32), _ptr(dL_drgb, torch.float32), _ptr(dL_dconic, torch.float32),
                                 _ptr(dL_dmu2, torch.float32), _ptr(dL_dopac, torch.float32), _stream(stream)), "uts_render_bwd")
+
+
+def uts_render_marks_bytes(cfg: Config, pair_capacity: int) -> int:
+    c = cfg.c()
+    return int(lib().uts_render_marks_bytes(C.byref(c), C.c_uint64(pair_capacity)))
+
+
+def uts_render_fwd_marked(cfg: Config, proj: Proj, mask: Mask, ranges, vals, pair_capacity: int, color, alpha, trans, n_last, marks, stream=None):
+    c = cfg.c()
+    _check(lib().uts_render_fwd_marked(C.byref(c), proj.c(), mask.c(), _ptr(ranges), _ptr(vals), C.c_uint64(pair_capacity), _ptr(color, torch.float32),
+                                       _ptr(alpha, torch.float32), _ptr(trans, torch.float32), _ptr(n_last), _ptr(marks),
+                                       C.c_size_t(marks.numel() * marks.element_size()), _stream(stream)), "uts_render_fwd_marked")
+
+
+def uts_render_bwd_marked(cfg: Config, proj: Proj, mask: Mask, ranges, vals, pair_capacity: int, trans, n_last, marks, dL_dcolor, dL_dalpha,
+                          dL_drgb, dL_dconic, dL_dmu2, dL_dopac, stream=None):
+    c = cfg.c()
+    _check(lib().uts_render_bwd_marked(C.byref(c), proj.c(), mask.c(), _ptr(ranges), _ptr(vals), C.c_uint64(pair_capacity), _ptr(trans, torch.float32),
+                                       _ptr(n_last), _ptr(marks), _ptr(dL_dcolor, torch.float32), _ptr(dL_dalpha, torch.float32),
+                                       _ptr(dL_drgb, torch.float32), _ptr(dL_dconic, torch.float32), _ptr(dL_dmu2, torch.float32),
+                                       _ptr(dL_dopac, torch.float32), _stream(stream)), "uts_render_bwd_marked")
 
 
 def uts_preprocess_bwd(cfg: Config, g: Gaussians, views: Views, flags, dL_drgb, dL_dconic, dL_dmu2, dL_dmeans, dL_dscales,

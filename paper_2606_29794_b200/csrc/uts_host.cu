@@ -19,7 +19,8 @@ struct HostLayout {
   float *means, *scales, *quats, *opac, *sh, *W, *b;
   uts_proj proj;
   uint64_t *offsets, *keys, *keys_tmp, *ranges;
-  uint32_t *vals, *vals_tmp, *n_last;
+  uint32_t *vals, *vals_tmp, *n_last, *marks;
+  size_t marks_bytes;
   void *tq_scratch, *sort_scratch, *do_scratch;
   size_t tq_bytes, sort_bytes, do_bytes;
   uint32_t* emit_rank;
@@ -49,6 +50,7 @@ static HostLayout layout(const uts_config* cfg, int64_t n_slot, uint64_t cap, ch
   L.ranges = B.take<uint64_t>(2 * ids);
   L.color = B.take<float>(3 * npx); L.alpha = B.take<float>(npx); L.trans = B.take<float>(npx); L.n_last = B.take<uint32_t>(npx);
   L.g_color = B.take<float>(3 * npx);
+  L.marks_bytes = uts_render_marks_bytes(cfg, cap); L.marks = B.take<uint32_t>(L.marks_bytes / 4);
   L.g_rgb = B.take<float>(3 * VP); L.g_conic = B.take<float>(3 * VP); L.g_mu2 = B.take<float>(2 * VP); L.g_opac = B.take<float>(P);
   L.g_means = B.take<float>(3 * P); L.g_scales = B.take<float>(3 * P); L.g_quats = B.take<float>(4 * P); L.g_sh = B.take<float>(3 * M * P);
   L.total = B.off + 256;
@@ -124,15 +126,17 @@ int uts_host_forward_backward(const uts_config* cfg, const float* h_means, const
     return st;
   UTS_CUDA(cudaStreamWaitEvent(s, ev_sh, 0));
   if ((st = uts_preprocess_color(cfg, g, vw, L.proj, stream))) return st;
-  if ((st = uts_render_fwd(cfg, L.proj, mask, L.ranges, L.vals, L.color, L.alpha, L.trans, L.n_last, stream))) return st;
+  if ((st = uts_render_fwd_marked(cfg, L.proj, mask, L.ranges, L.vals, pair_capacity, L.color, L.alpha, L.trans, L.n_last, L.marks, L.marks_bytes,
+                                  stream)))
+    return st;
   UTS_CUDA(cudaEventRecord(ev_fwd, s));
   UTS_CUDA(cudaStreamWaitEvent(s2, ev_fwd, 0));
   UTS_CUDA(cudaMemcpyAsync(h_color, L.color, 3 * npx * f, cudaMemcpyDeviceToHost, s2));
   if (h_alpha) UTS_CUDA(cudaMemcpyAsync(h_alpha, L.alpha, npx * f, cudaMemcpyDeviceToHost, s2));
   if (bwd) {
     UTS_CUDA(cudaStreamWaitEvent(s, ev_up, 0));
-    if ((st = uts_render_bwd(cfg, L.proj, mask, L.ranges, L.vals, L.trans, L.n_last, L.g_color, nullptr, L.g_rgb, L.g_conic,
-                             L.g_mu2, L.g_opac, stream)))
+    if ((st = uts_render_bwd_marked(cfg, L.proj, mask, L.ranges, L.vals, pair_capacity, L.trans, L.n_last, L.marks, L.g_color, nullptr, L.g_rgb,
+                                    L.g_conic, L.g_mu2, L.g_opac, stream)))
       return st;
     if ((st = uts_preprocess_bwd(cfg, g, vw, L.proj.flags, L.g_rgb, L.g_conic, L.g_mu2, L.g_means, L.g_scales, L.g_quats, L.g_sh, stream)))
       return st;

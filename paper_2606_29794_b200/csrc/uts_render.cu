@@ -140,7 +140,7 @@ __device__ __forceinline__ void eval_entry(const float4 f0, const float4 f1, con
 }
 
 // Pixel and tile set-up common to both kernels.
-struct PixelSetup { float px, py, pz; bool on; size_t out; uint64_t start, end; int v; };
+struct PixelSetup { float px, py, pz; bool on; size_t out; uint64_t start, end; int v; int64_t tile; };
 
 __device__ __forceinline__ void setup_pixel(const RenderParams& rp, const uint32_t* __restrict__ active_tiles,
                                             const uint32_t* __restrict__ mask_bits, const uint64_t* __restrict__ ranges,
@@ -149,6 +149,7 @@ __device__ __forceinline__ void setup_pixel(const RenderParams& rp, const uint32
   ps.v = (int)(blockIdx.x / rp.n_slot);
   const int64_t tile = active_tiles ? (int64_t)__ldg(active_tiles + slot) : slot;
   const uint64_t p = (uint64_t)tile * kTilePix + threadIdx.x;
+  ps.tile = tile;
   ps.on = mask_bits ? ((__ldg(mask_bits + (p >> 5)) >> (p & 31)) & 1u) != 0 : true;
   ps.out = ((size_t)ps.v * rp.n_slot + slot) * kTilePix + threadIdx.x;
   const uint64_t rix = 2 * ((uint64_t)ps.v * rp.n_tile + tile);
@@ -160,11 +161,22 @@ __device__ __forceinline__ void setup_pixel(const RenderParams& rp, const uint32
   ps.px = (float)(wx - s_tf->cx); ps.py = (float)(wy - s_tf->cy); ps.pz = (float)(wz - s_tf->cz);
 }
 
+// Marks (uts_render_fwd_marked / uts_render_bwd_marked): one bit per (warp of the tile's block, list entry), set by the forward
+// when at least one of the warp's 32 pixels blended the entry.  Plane w (of 8) holds warp w's bits; the bits of (view, tile) vt
+// start at word (start_vt >> 5) + vt of the plane, entry j of the list at bit j of that run — runs of different tiles never share a
+// word.  The backward walks only the set bits: on the paper's kind of scene half of the (warp, entry) visits re-evaluate alpha just
+// to find that no pixel of the warp took the entry.
+__device__ __forceinline__ uint64_t mark_base(const RenderParams& rp, const PixelSetup& ps, int64_t tile) {
+  return (ps.start >> 5) + (uint64_t)ps.v * (uint64_t)rp.n_tile + (uint64_t)tile;
+}
+
+template <bool MARK>
 __global__ void __launch_bounds__(kTilePix)
 render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* __restrict__ conic_opac, const float* __restrict__ rgb,
                   const uint32_t* __restrict__ active_tiles, const uint32_t* __restrict__ mask_bits,
                   const uint64_t* __restrict__ ranges, const uint32_t* __restrict__ vals, float* __restrict__ color,
-                  float* __restrict__ alpha_out, float* __restrict__ trans_out, uint32_t* __restrict__ n_last_out) {
+                  float* __restrict__ alpha_out, float* __restrict__ trans_out, uint32_t* __restrict__ n_last_out,
+                  uint32_t* __restrict__ marks, uint64_t plane_words) {
   __shared__ SEntry S;
   __shared__ TileFrame s_tf;
   PixelSetup ps;
@@ -177,6 +189,8 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
   bool done = !ps.on;
   const uint64_t len = ps.end - ps.start;
   const uint32_t sS = (uint32_t)__cvta_generic_to_shared(&S);
+  uint32_t* mark_w = nullptr;                         // this warp's run of mark words for the tile
+  if (MARK) mark_w = marks + (uint64_t)(threadIdx.x >> 5) * plane_words + mark_base(rp, ps, ps.tile);
   for (uint64_t b0 = 0; b0 < len; b0 += kTilePix) {
     if (__syncthreads_and(done)) break;               // every pixel of the tile saturated (or masked)
     const uint64_t j = b0 + threadIdx.x;
@@ -195,7 +209,9 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
     __syncthreads();
     const int nb = (int)((len - b0) < (uint64_t)kTilePix ? (len - b0) : (uint64_t)kTilePix);
     // four entries per warp vote: the vote only ends the walk early, every skip / clamp decision is per lane
-    for (int j4 = 0; j4 < nb; j4 += 4) {
+    uint32_t mw = 0;                                  // marks of the current group of 32 entries
+    int j4 = 0;
+    for (; j4 < nb; j4 += 4) {
       if (__all_sync(0xffffffffu, done)) break;       // warp vote: the whole 8x4 patch is saturated
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
@@ -207,6 +223,7 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
         if (done || ev.p2 > 0.f) continue;            // Alg.1 l.23: power > 0 skipped (reading A7)
         const float a = fminf(rp.amax, f0.w * ex2_approx(ev.p2));
         if (a < rp.amin) continue;
+        if (MARK) mw |= 1u << (jj & 31);              // this lane blended the entry; the warp ORs the lanes' words per group
         const float2 f4 = lds64(sS + 0x4000u + (uint32_t)jj * 8u);
         const float w = T * a;                        // Eq.6: c_i alpha_i prod_{j<i} (1 - alpha_j)
         Cr = fmaf(w, f3.w, Cr); Cg = fmaf(w, f4.x, Cg); Cb = fmaf(w, f4.y, Cb);
@@ -214,6 +231,16 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
         n_last = (uint32_t)(b0 + jj) + 1u;
         if (T < rp.teps) done = true;                 // Alg.1 l.27: test after the update
       }
+      if (MARK && ((j4 + 4) & 31) == 0) {             // a group of 32 entries is complete
+        const uint32_t gw = __reduce_or_sync(0xffffffffu, mw);
+        if ((threadIdx.x & 31) == 0) mark_w[(b0 + (uint64_t)j4) >> 5] = gw;       // written even when 0: the buffer is not cleared
+        mw = 0;
+      }
+    }
+    // partial group: the walk ended inside it, at j4 (all lanes leave the loop together, with the same j4)
+    if (MARK && (j4 & 31) != 0) {
+      const uint32_t gw = __reduce_or_sync(0xffffffffu, mw);
+      if ((threadIdx.x & 31) == 0) mark_w[(b0 + (uint64_t)(j4 - 1)) >> 5] = gw;
     }
   }
   if (ps.on) {
@@ -238,12 +265,14 @@ struct SEntryBwd {
   uint32_t id[kTilePix];
 };
 
+template <bool MARK>
 __global__ void __launch_bounds__(kTilePix)
 render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* __restrict__ conic_opac, const float* __restrict__ rgb,
                   const uint32_t* __restrict__ active_tiles, const uint32_t* __restrict__ mask_bits,
                   const uint64_t* __restrict__ ranges, const uint32_t* __restrict__ vals, const float* __restrict__ trans,
                   const uint32_t* __restrict__ n_last_in, const float* __restrict__ dL_dcolor, const float* __restrict__ dL_dalpha,
-                  float* __restrict__ dL_drgb, float* __restrict__ dL_dconic, float* __restrict__ dL_dmu2, float* __restrict__ dL_dopac) {
+                  float* __restrict__ dL_drgb, float* __restrict__ dL_dconic, float* __restrict__ dL_dmu2, float* __restrict__ dL_dopac,
+                  const uint32_t* __restrict__ marks, uint64_t plane_words) {
   __shared__ SEntryBwd S;
   __shared__ TileFrame s_tf;
   __shared__ uint32_t s_max[kTilePix / 32];
@@ -282,8 +311,15 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
   float T = Tfin;                                      // transmittance after the entry being visited
   float Sr = Tfin * rp.bg[0], Sg = Tfin * rp.bg[1], Sb = Tfin * rp.bg[2];                // colour accumulated behind it
   const int n_batch = (int)((max_nl + kTilePix - 1) / kTilePix);
+  const uint32_t* mark_w = nullptr;                    // this warp's run of mark words for the tile (see render_fwd_kernel)
+  if (MARK) mark_w = marks + (uint64_t)wid * plane_words + mark_base(rp, ps, ps.tile);
   for (int bi = n_batch - 1; bi >= 0; --bi) {
     const uint32_t b0 = (uint32_t)bi * kTilePix;
+    // lane g < 8: the marks of entries b0 + 32 g .. + 31.  The forward wrote this warp's words up to the last entry any of its
+    // pixels blended; words beyond that hold whatever the buffer held (it is never cleared) — a set bit there only costs the
+    // visit's first vote, because no pixel of the warp reaches such an entry.
+    uint32_t myw = 0u;
+    if (MARK && lane < 8) myw = __ldg(mark_w + (size_t)bi * 8 + lane);
     __syncthreads();
     const uint32_t j = b0 + threadIdx.x;
     if (j < max_nl) {
@@ -302,10 +338,10 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
     }
     __syncthreads();
     const int nb = (int)min((uint32_t)kTilePix, max_nl - b0);
-    for (int jj = nb - 1; jj >= 0; --jj) {
+    auto visit = [&](const int jj) {
       const uint32_t jl = b0 + (uint32_t)jj;
       const bool reach = jl < nl;                      // this pixel's forward pass got this far
-      if (!__any_sync(0xffffffffu, reach)) continue;
+      if (!__any_sync(0xffffffffu, reach)) return;
       const uint32_t sa = sS + (uint32_t)jj * 16u;
       const float4 f0 = lds128(sa), f1 = lds128(sa + 0x1000u), f2 = lds128(sa + 0x2000u), f3 = lds128(sa + 0x3000u), f5 = lds128(sa + 0x4000u);
       Eval ev;
@@ -313,7 +349,7 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
       float e2 = 0.f, raw = 0.f, a = 0.f;
       bool used = reach && !(ev.p2 > 0.f);
       if (used) { e2 = ex2_approx(ev.p2); raw = f0.w * e2; a = fminf(rp.amax, raw); used = !(a < rp.amin); }
-      if (!__any_sync(0xffffffffu, used)) continue;
+      if (!__any_sync(0xffffffffu, used)) return;
       float d_r = 0.f, d_g = 0.f, d_b = 0.f, d_A = 0.f, d_B = 0.f, d_C = 0.f, d_o = 0.f, d_om = 0.f, d_ph = 0.f;
       if (used) {
         const float inv1a = rcp_approx(1.f - a);
@@ -377,6 +413,19 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
         const uint32_t id = S.id[jj];
         if (lane_owns) red_add_global(lane_dst + (size_t)id * lane_stride, lane == 1 ? d_o : v0);
       }
+    };
+    if (MARK) {
+      for (int grp = (nb - 1) >> 5; grp >= 0; --grp) {
+        uint32_t wb = __shfl_sync(0xffffffffu, myw, grp);
+        if (nb - 32 * grp < 32) wb &= (1u << (nb - 32 * grp)) - 1u;   // entries >= nb: beyond the tile's largest n_last
+        while (wb) {                                                  // back to front over the marked entries
+          const int bit = 31 - __clz((int)wb);
+          wb &= ~(1u << bit);
+          visit(32 * grp + bit);
+        }
+      }
+    } else {
+      for (int jj = nb - 1; jj >= 0; --jj) visit(jj);
     }
   }
 }
@@ -395,8 +444,18 @@ using namespace uts;
 
 extern "C" {
 
-int uts_render_fwd(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
-                   float* color, float* alpha, float* trans, uint32_t* n_last, void* stream) {
+static uint64_t mark_plane_words(const uts_config* cfg, uint64_t pair_capacity) {
+  const uint64_t n_vt = (uint64_t)cfg->n_views * ((uint64_t)12 << (2 * (cfg->order - cfg->tile_log2)));
+  return (pair_capacity >> 5) + n_vt + 16;            // runs start at (start >> 5) + vt; a batch read takes 8 words
+}
+
+size_t uts_render_marks_bytes(const uts_config* cfg, uint64_t pair_capacity) {
+  if (check_config(cfg) != UTS_OK) return 0;
+  return (size_t)mark_plane_words(cfg, pair_capacity) * 8 * sizeof(uint32_t);
+}
+
+static int render_fwd_impl(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
+                           float* color, float* alpha, float* trans, uint32_t* n_last, uint32_t* marks, uint64_t plane_words, void* stream) {
   int st = check_config(cfg);
   if (st) return st;
   if ((st = check_mask(cfg, mask))) return st;
@@ -405,15 +464,34 @@ int uts_render_fwd(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   if (d.n_slot == 0) return UTS_OK;
   if (d.n_slot * d.V > 0x7fffffffll) return UTS_ERR_UNSUPPORTED;
   RenderParams rp = make_params(cfg, d);
-  render_fwd_kernel<<<(unsigned)(d.n_slot * d.V), kTilePix, 0, (cudaStream_t)stream>>>(
-      rp, in.dir, in.conic_opac, in.rgb, mask.active_tiles, mask.pixel_mask_bits, ranges, vals, color, alpha, trans, n_last);
+  if (marks)
+    render_fwd_kernel<true><<<(unsigned)(d.n_slot * d.V), kTilePix, 0, (cudaStream_t)stream>>>(
+        rp, in.dir, in.conic_opac, in.rgb, mask.active_tiles, mask.pixel_mask_bits, ranges, vals, color, alpha, trans, n_last, marks, plane_words);
+  else
+    render_fwd_kernel<false><<<(unsigned)(d.n_slot * d.V), kTilePix, 0, (cudaStream_t)stream>>>(
+        rp, in.dir, in.conic_opac, in.rgb, mask.active_tiles, mask.pixel_mask_bits, ranges, vals, color, alpha, trans, n_last, nullptr, 0);
   UTS_LAUNCH_CHECK();
   return UTS_OK;
 }
 
-int uts_render_bwd(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
-                   const float* trans, const uint32_t* n_last, const float* dL_dcolor, const float* dL_dalpha,
-                   float* dL_drgb, float* dL_dconic, float* dL_dmu2, float* dL_dopac, void* stream) {
+int uts_render_fwd(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
+                   float* color, float* alpha, float* trans, uint32_t* n_last, void* stream) {
+  return render_fwd_impl(cfg, in, mask, ranges, vals, color, alpha, trans, n_last, nullptr, 0, stream);
+}
+
+int uts_render_fwd_marked(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
+                          uint64_t pair_capacity, float* color, float* alpha, float* trans, uint32_t* n_last, uint32_t* marks,
+                          size_t marks_bytes, void* stream) {
+  if (!marks || check_config(cfg) != UTS_OK) return UTS_ERR_INVALID_ARG;
+  const uint64_t pw = mark_plane_words(cfg, pair_capacity);
+  if (marks_bytes < (size_t)pw * 8 * sizeof(uint32_t)) return UTS_ERR_CAPACITY;
+  return render_fwd_impl(cfg, in, mask, ranges, vals, color, alpha, trans, n_last, marks, pw, stream);
+}
+
+static int render_bwd_impl(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
+                           const float* trans, const uint32_t* n_last, const float* dL_dcolor, const float* dL_dalpha,
+                           float* dL_drgb, float* dL_dconic, float* dL_dmu2, float* dL_dopac, const uint32_t* marks, uint64_t plane_words,
+                           void* stream) {
   int st = check_config(cfg);
   if (st) return st;
   if ((st = check_mask(cfg, mask))) return st;
@@ -429,11 +507,32 @@ int uts_render_bwd(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   if (d.n_slot == 0 || d.P == 0) return UTS_OK;
   if (d.n_slot * d.V > 0x7fffffffll) return UTS_ERR_UNSUPPORTED;
   RenderParams rp = make_params(cfg, d);
-  render_bwd_kernel<<<(unsigned)(d.n_slot * d.V), kTilePix, 0, (cudaStream_t)stream>>>(
-      rp, in.dir, in.conic_opac, in.rgb, mask.active_tiles, mask.pixel_mask_bits, ranges, vals, trans, n_last, dL_dcolor,
-      dL_dalpha, dL_drgb, dL_dconic, dL_dmu2, dL_dopac);
+  if (marks)
+    render_bwd_kernel<true><<<(unsigned)(d.n_slot * d.V), kTilePix, 0, (cudaStream_t)stream>>>(
+        rp, in.dir, in.conic_opac, in.rgb, mask.active_tiles, mask.pixel_mask_bits, ranges, vals, trans, n_last, dL_dcolor,
+        dL_dalpha, dL_drgb, dL_dconic, dL_dmu2, dL_dopac, marks, plane_words);
+  else
+    render_bwd_kernel<false><<<(unsigned)(d.n_slot * d.V), kTilePix, 0, (cudaStream_t)stream>>>(
+        rp, in.dir, in.conic_opac, in.rgb, mask.active_tiles, mask.pixel_mask_bits, ranges, vals, trans, n_last, dL_dcolor,
+        dL_dalpha, dL_drgb, dL_dconic, dL_dmu2, dL_dopac, nullptr, 0);
   UTS_LAUNCH_CHECK();
   return UTS_OK;
+}
+
+int uts_render_bwd(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
+                   const float* trans, const uint32_t* n_last, const float* dL_dcolor, const float* dL_dalpha,
+                   float* dL_drgb, float* dL_dconic, float* dL_dmu2, float* dL_dopac, void* stream) {
+  return render_bwd_impl(cfg, in, mask, ranges, vals, trans, n_last, dL_dcolor, dL_dalpha, dL_drgb, dL_dconic, dL_dmu2, dL_dopac, nullptr, 0,
+                         stream);
+}
+
+int uts_render_bwd_marked(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
+                          uint64_t pair_capacity, const float* trans, const uint32_t* n_last, const uint32_t* marks,
+                          const float* dL_dcolor, const float* dL_dalpha, float* dL_drgb, float* dL_dconic, float* dL_dmu2,
+                          float* dL_dopac, void* stream) {
+  if (!marks || check_config(cfg) != UTS_OK) return UTS_ERR_INVALID_ARG;
+  return render_bwd_impl(cfg, in, mask, ranges, vals, trans, n_last, dL_dcolor, dL_dalpha, dL_drgb, dL_dconic, dL_dmu2, dL_dopac, marks,
+                         mark_plane_words(cfg, pair_capacity), stream);
 }
 
 }  // extern "C"

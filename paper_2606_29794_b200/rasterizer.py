@@ -18,7 +18,7 @@ class Rasterizer:
     synchronisation is the pair count returned by uts_tile_query."""
 
     def __init__(self, cfg: B.Config, mask: B.Mask | None = None, device="cuda", pair_capacity: int = 0, depth_presort: bool = True,
-                 fused_lists: bool = True):
+                 fused_lists: bool = True, marks: bool = True):
         B.lib()
         if not torch.cuda.is_available():
             raise RuntimeError("uts: a CUDA device is required (no CPU fallback)")
@@ -38,6 +38,9 @@ class Rasterizer:
         self.ranges = _i64(V * cfg.n_tiles * 2, device).view(V * cfg.n_tiles, 2)
         self.color = _f32(V, npx, 3, dev=device); self.alpha = _f32(V, npx, dev=device)
         self.trans = _f32(V, npx, dev=device); self.n_last = _i32(V * npx, device).view(V, npx)
+        # marks: the forward blend records which (warp, entry) pairs blended anything, the backward visits only those
+        self.use_marks = bool(marks)
+        self.marks = None
         self.capacity = 0
         self.n_pairs = 0
         self._alloc_pairs(max(int(pair_capacity), 1024))
@@ -50,6 +53,7 @@ class Rasterizer:
         self.keys, self.keys_tmp = _i64(cap, d), _i64(cap, d)
         self.vals, self.vals_tmp = _i32(cap, d), _i32(cap, d)
         self.sort_scratch = _bytes(B.uts_sort_scratch_bytes(cap), d)
+        self.marks = torch.zeros(B.uts_render_marks_bytes(self.cfg, cap) // 4, dtype=torch.int32, device=d) if self.use_marks else None
 
     # ---- stages (each is one ABI call) -------------------------------------------------------------
     def preprocess(self, g, views): B.uts_preprocess(self.cfg, g, views, self.proj)
@@ -88,7 +92,11 @@ class Rasterizer:
     def tile_ranges(self): B.uts_tile_ranges(self.cfg, self.n_pairs, self.keys, self.ranges)
 
     def render_fwd(self):
-        B.uts_render_fwd(self.cfg, self.proj, self.mask, self.ranges, self.vals, self.color, self.alpha, self.trans, self.n_last)
+        if self.use_marks:
+            B.uts_render_fwd_marked(self.cfg, self.proj, self.mask, self.ranges, self.vals, self.capacity, self.color, self.alpha, self.trans,
+                                    self.n_last, self.marks)
+        else:
+            B.uts_render_fwd(self.cfg, self.proj, self.mask, self.ranges, self.vals, self.color, self.alpha, self.trans, self.n_last)
 
     def _alloc_grads(self):
         if self.grads is None:
@@ -99,8 +107,12 @@ class Rasterizer:
 
     def render_bwd(self, dL_dcolor, dL_dalpha=None):
         G = self._alloc_grads()
-        B.uts_render_bwd(self.cfg, self.proj, self.mask, self.ranges, self.vals, self.trans, self.n_last, dL_dcolor, dL_dalpha,
-                         G["rgb"], G["conic"], G["mu2"], G["opac"])
+        if self.use_marks:
+            B.uts_render_bwd_marked(self.cfg, self.proj, self.mask, self.ranges, self.vals, self.capacity, self.trans, self.n_last, self.marks,
+                                    dL_dcolor, dL_dalpha, G["rgb"], G["conic"], G["mu2"], G["opac"])
+        else:
+            B.uts_render_bwd(self.cfg, self.proj, self.mask, self.ranges, self.vals, self.trans, self.n_last, dL_dcolor, dL_dalpha,
+                             G["rgb"], G["conic"], G["mu2"], G["opac"])
 
     def preprocess_bwd(self, g, views):
         G = self._alloc_grads()

@@ -48,7 +48,7 @@ def test_depth_image_and_gradients(cfg_id, P, order, extra):
     pd = dataclasses.replace(pr, rgb=want_chan)
     D, _, n_last, margin, _ = orc.render_fwd(oc, pd, fw["ranges"], fw["svals"], act, bits)
     mask = B.Mask.full() if bits is None else B.Mask(dev(act.view(np.int32)), int(act.shape[0]), dev(slot), dev(bits.view(np.int32)))
-    r = R.Rasterizer(cfg, mask)
+    r = R.Rasterizer(cfg, mask, pair_capacity=int(fw["svals"].shape[0]))
     r.proj = B.Proj(dev(pr.dir), dev(pr.lonlat), dev(pr.rho), dev(pr.conic_opac), dev(pr.rs), dev(want_chan), dev(pr.flags))
     r.ranges = dev(fw["ranges"].view(np.int64)); r.vals = dev(fw["svals"].view(np.int32))
     r.render_fwd()

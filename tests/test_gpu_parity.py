@@ -371,7 +371,7 @@ def test_sort_sizes_and_ties(n):
 # ------------------------------------------------------------------------------------------- F5 / F6
 def _render_gpu(B, R, c, cfg):
     mask = c.gpu_mask(B)
-    r = R.Rasterizer(cfg, mask)
+    r = R.Rasterizer(cfg, mask, pair_capacity=int(c.fw["svals"].shape[0]))      # the marks are sized by the capacity
     r.proj = c.gpu_proj(B)
     r.ranges = dev(c.fw["ranges"].view(np.int64))
     r.vals = dev(c.fw["svals"].view(np.int32))
@@ -415,7 +415,7 @@ def test_render_fwd_background_and_no_thresholds():
     oc = ocfg(scene, **kw)
     fw = orc.forward_chain(oc, scene)
     cfg = _cfg(R, scene, **kw)
-    r = R.Rasterizer(cfg)
+    r = R.Rasterizer(cfg, pair_capacity=int(fw["svals"].shape[0]))
     p = fw["proj"]
     r.proj = B.Proj(dev(p.dir), dev(p.lonlat), dev(p.rho), dev(p.conic_opac), dev(p.rs), dev(p.rgb), dev(p.flags))
     r.ranges = dev(fw["ranges"].view(np.int64)); r.vals = dev(fw["svals"].view(np.int32))
@@ -624,3 +624,29 @@ def test_tile_lists_whole_sphere_discs_and_empty(monkeypatch):
     cfg0 = B.Config(order=6, n_gauss=0)
     r0 = R.Rasterizer(cfg0, fused_lists=True)
     assert r0.tile_lists() == 0 and int(r0.ranges.abs().sum()) == 0
+
+
+@pytest.mark.parametrize("cfg_id,P,order", [(1, 3000, 6), (3, 20000, 7), (4, 20000, 7), (5, 8000, 8)])
+def test_marked_blend_equals_plain_blend(cfg_id, P, order):
+    """uts_render_fwd_marked / uts_render_bwd_marked (the backward visits only the (warp, entry) pairs the forward marked) against
+    uts_render_fwd / uts_render_bwd on the same lists: image, alpha, trans, n_last bit-identical; gradients the same sums (the set
+    of visited entries per pixel is unchanged, only whole-warp no-ops are skipped), compared at 2e-4 of the largest entry (fp32 atomics:
+    two runs of the same kernel differ by a few 1e-5 where large terms cancel)."""
+    B, R = _gpu()
+    scene = small_scene(cfg_id, P, order)
+    cfg = _cfg(R, scene)
+    g, views = R.scene_to_device(scene)
+    mask = B.uts_build_mask(cfg, scene["mask"]["kind"], scene["mask"]["params"]) if scene["mask"] is not None else B.Mask.full()
+    rm = R.Rasterizer(cfg, mask, marks=True); rp = R.Rasterizer(cfg, mask, marks=False)
+    rm.marks.fill_(-1)                                   # the forward must write every word the backward reads
+    cm, am = rm.forward(g, views); cp, ap = rp.forward(g, views)
+    assert rm.n_pairs == rp.n_pairs > 0
+    for a, b in ((cm, cp), (am, ap), (rm.trans, rp.trans), (rm.n_last, rp.n_last)):
+        assert torch.equal(a, b)
+    gen = torch.Generator(device="cuda").manual_seed(3)
+    gcol = torch.randn(cm.shape, device="cuda", generator=gen)
+    gal = torch.randn(am.shape, device="cuda", generator=gen)
+    Gm = rm.backward(g, views, gcol, gal); Gp = rp.backward(g, views, gcol, gal)
+    for k in Gm:
+        a, b = Gm[k], Gp[k]
+        assert float((a - b).abs().max()) <= 2e-4 * float(b.abs().max()) + 1e-12, k

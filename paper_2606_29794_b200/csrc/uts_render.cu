@@ -208,39 +208,38 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
     }
     __syncthreads();
     const int nb = (int)((len - b0) < (uint64_t)kTilePix ? (len - b0) : (uint64_t)kTilePix);
-    // four entries per warp vote: the vote only ends the walk early, every skip / clamp decision is per lane
-    uint32_t mw = 0;                                  // marks of the current group of 32 entries
-    int j4 = 0;
-    for (; j4 < nb; j4 += 4) {
-      if (__all_sync(0xffffffffu, done)) break;       // warp vote: the whole 8x4 patch is saturated
+    // four entries per warp vote: the vote only ends the walk early, every skip / clamp decision is per lane.  The batch is walked
+    // in groups of 32 entries, one mark word each.
+    bool left = false;
+    for (int g0 = 0; g0 < nb && !left; g0 += 32) {
+      uint32_t mw = 0;                                // this lane's marks of the group
+      const int ge = min(nb, g0 + 32);
+      for (int j4 = g0; j4 < ge; j4 += 4) {
+        if (__all_sync(0xffffffffu, done)) { left = true; break; }     // warp vote: the whole 8x4 patch is saturated
+        const uint32_t bit4 = 1u << (j4 - g0);
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const int jj = j4 + u;
-        const uint32_t sa = sS + (uint32_t)jj * 16u;
-        const float4 f0 = lds128(sa), f1 = lds128(sa + 0x1000u), f2 = lds128(sa + 0x2000u), f3 = lds128(sa + 0x3000u);
-        Eval ev;
-        eval_entry(f0, f1, f2, f3, ps.px, ps.py, ps.pz, ev);
-        if (done || ev.p2 > 0.f) continue;            // Alg.1 l.23: power > 0 skipped (reading A7)
-        const float a = fminf(rp.amax, f0.w * ex2_approx(ev.p2));
-        if (a < rp.amin) continue;
-        if (MARK) mw |= 1u << (jj & 31);              // this lane blended the entry; the warp ORs the lanes' words per group
-        const float2 f4 = lds64(sS + 0x4000u + (uint32_t)jj * 8u);
-        const float w = T * a;                        // Eq.6: c_i alpha_i prod_{j<i} (1 - alpha_j)
-        Cr = fmaf(w, f3.w, Cr); Cg = fmaf(w, f4.x, Cg); Cb = fmaf(w, f4.y, Cb);
-        T = T * (1.f - a);
-        n_last = (uint32_t)(b0 + jj) + 1u;
-        if (T < rp.teps) done = true;                 // Alg.1 l.27: test after the update
+        for (int u = 0; u < 4; ++u) {
+          const int jj = j4 + u;
+          const uint32_t sa = sS + (uint32_t)jj * 16u;
+          const float4 f0 = lds128(sa), f1 = lds128(sa + 0x1000u), f2 = lds128(sa + 0x2000u), f3 = lds128(sa + 0x3000u);
+          Eval ev;
+          eval_entry(f0, f1, f2, f3, ps.px, ps.py, ps.pz, ev);
+          if (done || ev.p2 > 0.f) continue;          // Alg.1 l.23: power > 0 skipped (reading A7)
+          const float a = fminf(rp.amax, f0.w * ex2_approx(ev.p2));
+          if (a < rp.amin) continue;
+          if (MARK) mw |= bit4 << u;                  // this lane blended the entry
+          const float2 f4 = lds64(sS + 0x4000u + (uint32_t)jj * 8u);
+          const float w = T * a;                      // Eq.6: c_i alpha_i prod_{j<i} (1 - alpha_j)
+          Cr = fmaf(w, f3.w, Cr); Cg = fmaf(w, f4.x, Cg); Cb = fmaf(w, f4.y, Cb);
+          T = T * (1.f - a);
+          n_last = (uint32_t)(b0 + jj) + 1u;
+          if (T < rp.teps) done = true;               // Alg.1 l.27: test after the update
+        }
       }
-      if (MARK && ((j4 + 4) & 31) == 0) {             // a group of 32 entries is complete
+      if (MARK) {                                     // the warp's word of the group (written even when 0: the buffer is not cleared)
         const uint32_t gw = __reduce_or_sync(0xffffffffu, mw);
-        if ((threadIdx.x & 31) == 0) mark_w[(b0 + (uint64_t)j4) >> 5] = gw;       // written even when 0: the buffer is not cleared
-        mw = 0;
+        if ((threadIdx.x & 31) == 0) mark_w[(b0 + (uint64_t)g0) >> 5] = gw;
       }
-    }
-    // partial group: the walk ended inside it, at j4 (all lanes leave the loop together, with the same j4)
-    if (MARK && (j4 & 31) != 0) {
-      const uint32_t gw = __reduce_or_sync(0xffffffffu, mw);
-      if ((threadIdx.x & 31) == 0) mark_w[(b0 + (uint64_t)(j4 - 1)) >> 5] = gw;
     }
   }
   if (ps.on) {

@@ -10,6 +10,8 @@
  *   uts_tile_ranges     Alg.1 l.16: per-tile [start,end)
  *   uts_render_fwd      Alg.1 l.17-30 (Eq.6) + FoV mask
  *   uts_render_bwd      backward of Eq.6
+ *   uts_render_fwd_marked / uts_render_bwd_marked   the same pair; the forward records which (warp, entry) pairs blended anything and
+ *                       the backward visits only those (same image, same gradient sums)
  *   uts_preprocess_bwd  Eq.3-4: to means, scales, rotations, SH
  *   uts_hssim_loss      L1 + HEALPix-SSIM loss and dL/dI (Eq.10): produces uts_render_bwd's upstream gradient
  *

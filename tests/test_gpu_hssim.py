@@ -249,3 +249,47 @@ def test_full_size_sampled_against_oracle(masked):
     if bits is None:
         assert abs(l3[1] - np.abs(X.astype(np.float64) - G).mean()) <= TOL_L
     assert abs(l3[0] - (0.8 * l3[1] + 0.2 * (1 - l3[2]))) <= 1e-8              # lambda is an fp32 argument of the ABI
+
+
+def test_max_order_flat_images():
+    """Order 13 (Nside 8192, 8.05e8 pixels: the largest grid uts_config accepts; 3 * n_store exceeds 2^31, so every storage index
+    has to be 64-bit).  Flat X = a, G = b: h = (2ab + C1) / (a^2 + b^2 + C1) at every pixel for any window, L1^H = |a - b|, and
+    dL/dX = (1 - lambda) sign(a - b) / (3 N) + the SSIM term, whose window weights sum to 1: the same value at every pixel."""
+    B = _gpu()
+    if torch.cuda.mem_get_info()[0] < 40e9:
+        pytest.skip("needs 40 GB of free device memory")
+    order = 13
+    cfg = B.Config(order=order, n_gauss=1)
+    n = 12 << (2 * order)
+    a, b, lam = 0.25, 0.75, 0.2
+    X = torch.full((n, 3), a, dtype=torch.float32, device="cuda"); G = torch.full((n, 3), b, dtype=torch.float32, device="cuda")
+    h = torch.empty(n, dtype=torch.float32, device="cuda"); g = torch.empty(n, 3, dtype=torch.float32, device="cuda")
+    loss3 = torch.empty(3, dtype=torch.float64, device="cuda")
+    scratch = torch.empty(B.uts_hssim_scratch_bytes(cfg), dtype=torch.uint8, device="cuda")
+    B.uts_hssim_loss(cfg, B.Mask.full(), X, G, loss3, scratch, h_map=h, dL_dX=g, lam=lam)
+    torch.cuda.synchronize()
+    want = (2 * a * b + 1e-4) / (a * a + b * b + 1e-4)
+    assert float((h - want).abs().max()) <= 1e-6
+    l3 = loss3.cpu().numpy()
+    assert abs(l3[1] - abs(a - b)) <= 1e-7 and abs(l3[2] - want) <= 1e-6
+    # d ssim / dx for flat windows: only the mean path is left, (2 b b1 - 2 a a1) / b1^2 with a1 = 2ab + C1, b1 = a^2 + b^2 + C1
+    a1, b1 = 2 * a * b + 1e-4, a * a + b * b + 1e-4
+    dssim = (2 * b * b1 - 2 * a * a1) / (b1 * b1)
+    gw = ((1 - lam) * (-1.0) - lam * dssim) / (3.0 * n)
+    # "the same value" holds where every window that contains the pixel uses one kernel and is complete: face interiors (across a
+    # face edge the zone's kernel changes, at 3-face vertices taps are missing, and the normalised weights a pixel receives no longer
+    # sum to 1).  Checked on pixels at least 8 from the face edges, tile corners and tile edges included; everywhere else bounded.
+    rng = np.random.default_rng(13)
+    N = 1 << order
+    xs = np.concatenate([rng.integers(8, N - 8, 1500), 16 * rng.integers(1, N // 16 - 1, 500), 16 * rng.integers(1, N // 16 - 1, 500) - 1])
+    ys = np.concatenate([rng.integers(8, N - 8, 1500), 16 * rng.integers(1, N // 16 - 1, 500) - 1, rng.integers(8, N - 8, 500)])
+    fs = rng.integers(0, 12, xs.shape[0])
+    p = np.zeros(xs.shape[0], np.int64)
+    for bit in range(order):
+        p |= ((xs >> bit) & 1) << (2 * bit) | ((ys >> bit) & 1) << (2 * bit + 1)
+    p |= fs.astype(np.int64) << (2 * order)
+    gs = g[torch.from_numpy(p).cuda()]
+    assert float((gs / gw - 1.0).abs().max()) <= 2e-4
+    assert float((g / gw - 1.0).abs().max()) <= 0.15
+    del X, G, h, g
+    torch.cuda.empty_cache()

@@ -96,7 +96,12 @@ matrix_count_kernel(QueryParams qp, MatParams mp, const float* __restrict__ dir,
     const uint32_t row = (uint32_t)mp.row_of_rank[slot];
     const int v = (int)(k / qp.P);
     __syncthreads();                                   // the previous disc is done with shared memory
-    for (int w = tid; w < mp.n_words; w += kMatThreads) bitmap[w] = 0u;
+    if ((mp.n_words & 1) == 0) {                       // 8-byte stores (the bitmap follows an int2 array: 8-byte aligned)
+      uint2* b2 = reinterpret_cast<uint2*>(bitmap);
+      for (int w = tid; w < (mp.n_words >> 1); w += kMatThreads) b2[w] = make_uint2(0u, 0u);
+    } else {
+      for (int w = tid; w < mp.n_words; w += kMatThreads) bitmap[w] = 0u;
+    }
     if (tid < 32) {                                    // set-up by the first warp: lane 0 the disc, lanes 0..11 one face each
       if (tid == 0) {
         load_ring_disc(qp, dir, lonlat, rs, k, s_disc);
@@ -140,7 +145,13 @@ matrix_count_kernel(QueryParams qp, MatParams mp, const float* __restrict__ dir,
     }
     __syncthreads();
     uint32_t* dst = mp.M + (size_t)row * mp.n_words;
-    for (int w = tid; w < mp.n_words; w += kMatThreads) dst[w] = bitmap[w];
+    if ((mp.n_words & 1) == 0) {                       // rows of M are 8-byte aligned when n_words is even
+      uint2* d2 = reinterpret_cast<uint2*>(dst);
+      const uint2* b2 = reinterpret_cast<const uint2*>(bitmap);
+      for (int w = tid; w < (mp.n_words >> 1); w += kMatThreads) d2[w] = b2[w];
+    } else {
+      for (int w = tid; w < mp.n_words; w += kMatThreads) dst[w] = bitmap[w];
+    }
     if (tid == 0) {
       counts[slot] = 0;                                // this disc emits no pairs of its own
       const uint32_t gid = (uint32_t)(k - (int64_t)v * qp.P);

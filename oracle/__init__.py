@@ -9,6 +9,7 @@ CUDA path imports nothing from here.
 from __future__ import annotations
 
 import ctypes as C
+import math
 import os
 import subprocess
 from dataclasses import dataclass, field
@@ -259,6 +260,14 @@ def rs_max_update(rs, flags, rs_max):
     out = _f32(rs_max).copy()
     lib().orc_rs_max_update(C.c_int(V), C.c_int(P), _p(r), _p(fl), _p(out))
     return out
+
+
+# ------------------------------------------------------------------ resolution hierarchy (Table 6)
+def select_order(width, height, omega_in):
+    """Table 6: continuous target N*_side = sqrt(4 pi W H / (12 Omega_in)); returns (N*_side, k = round(log2 N*), k_L = floor, k_H = ceil)."""
+    n_star = math.sqrt(4.0 * math.pi * width * height / (12.0 * omega_in))
+    l2 = math.log2(n_star)
+    return n_star, int(round(l2)), int(math.floor(l2)), int(math.ceil(l2))
 
 
 # ------------------------------------------------------------------ L1 + HEALPix-SSIM loss (orc_hssim.cpp, NEXT-3)

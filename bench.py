@@ -371,16 +371,16 @@ def run_ours(args):
     dom = max((k_ for k_ in stage_ms if k_ != "tile_lists"), key=stage_ms.get)
     fp32_peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12       # TFLOP/s at the maximum SM clock
     if dom in ("render_fwd", "render_bwd"):
-        # backward with marks: only the visited (warp, entry) pairs are evaluated, 32 pixels each; without: every entry before n_last
-        ev_b_eff = ev_b_visited if ev_b_visited is not None else ev_b
-        flop = ev_f * FLOP_FWD if dom == "render_fwd" else ev_b_eff * FLOP_BWD
+        # units as SURVEY 8(d) defines them: E_fwd / E_bwd = the pairs Alg.1's loop evaluates, every entry before n_last for every pixel
+        flop = ev_f * FLOP_FWD if dom == "render_fwd" else ev_b * FLOP_BWD
         ach = flop / (stage_ms[dom] * 1e-3) / 1e12
         roof = dict(kernel=dom, bound="alu", achieved=ach, peak=fp32_peak, unit="TFLOP/s", frac=ach / fp32_peak, traffic=traffic.get(dom),
                     peak_source="derived: 148 SM x 128 FP32 lanes x 2 x sm_max_mhz")
         if dom == "render_bwd" and ev_b_visited is not None:
-            a1 = ev_b * FLOP_BWD / (stage_ms[dom] * 1e-3) / 1e12
-            roof["note"] = ("units = 32 pixel evaluations per (warp, entry) pair the marked backward visits; counted as before the marks (every entry "
-                            f"before n_last for every pixel, Alg.1's own loop) achieved = {a1:.1f} TFLOP/s, frac = {a1 / fp32_peak:.3f}")
+            a1 = ev_b_visited * FLOP_BWD / (stage_ms[dom] * 1e-3) / 1e12
+            roof["note"] = ("units = E_bwd of SURVEY 8(d): every entry before n_last for every pixel (Alg.1's loop).  The marked backward skips the (warp, "
+                            "entry) visits in which no pixel of the warp blended the entry; counting only the 32 pixel evaluations of each visit it "
+                            f"does make: achieved = {a1:.1f} TFLOP/s, frac = {a1 / fp32_peak:.3f}")
     else:
         per_pair = {"sort": 32.0 * ((max(1, (V * cfg.n_tiles - 1)).bit_length() + 7) // 8), "tile_query": 12.0, "tile_ranges": 8.0}.get(dom)
         byts = per_pair * n_pairs if per_pair else P * V * (44 + 12 * M + 57)
@@ -392,8 +392,9 @@ def run_ours(args):
         if s_ == "render_fwd":
             per_kernel[s_] = dict(ms=ms, tflops=ev_f * FLOP_FWD / (ms * 1e-3) / 1e12, frac_fp32_peak=ev_f * FLOP_FWD / (ms * 1e-3) / 1e12 / fp32_peak)
         elif s_ == "render_bwd":
-            eb_ = ev_b_visited if ev_b_visited is not None else ev_b
-            per_kernel[s_] = dict(ms=ms, tflops=eb_ * FLOP_BWD / (ms * 1e-3) / 1e12, frac_fp32_peak=eb_ * FLOP_BWD / (ms * 1e-3) / 1e12 / fp32_peak)
+            per_kernel[s_] = dict(ms=ms, tflops=ev_b * FLOP_BWD / (ms * 1e-3) / 1e12, frac_fp32_peak=ev_b * FLOP_BWD / (ms * 1e-3) / 1e12 / fp32_peak)
+            if ev_b_visited is not None:
+                per_kernel[s_]["tflops_visited_only"] = ev_b_visited * FLOP_BWD / (ms * 1e-3) / 1e12
         else:
             byts = {"preprocess": P * V * (44 + 12 * M + 57), "preprocess_bwd": P * (44 + 12 * M + V * 33 + 40 + 12 * M),
                     "depth_order": P * V * (4 + 5 * 32 + 16), "tile_query": P * V * 2 * 29 + 8 * P * V + 12 * n_pairs,

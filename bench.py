@@ -274,6 +274,7 @@ def run_ours(args):
     # timed on view 0's HEALPix image.  Camera: the paper's case for this grid where there is no mask (6080 x 3040 panorama ->
     # Nside 1024, Table 5), else a 1920 x 1080 pinhole of 60 x 45 degrees (config 5's frustum).
     extras = {}
+    r._color_full = r.color.clone()          # the full lists' image, for the bit-identity check of the depth-prefix leg below
     try:
         cam = B.Camera("equirect", 6080, 3040) if mask.active_tiles is None else B.Camera("pinhole", 1920, 1080, np.radians(60.0), np.radians(45.0))
         img = r.color[0].contiguous()
@@ -322,6 +323,36 @@ def run_ours(args):
         del img, tgt, g_l
     except Exception as e:      # measurement plumbing only
         extras["hssim_loss"] = dict(error=str(e))
+
+    # occlusion-bounded lists (not the step: Alg.1 builds the full lists): lists from the nearest `keep`
+    # Gaussians, verified every time by uts_count_unsaturated — when no visible pixel is left open, image and gradients are exactly
+    # the full lists' ones.  keep is found by doubling from P/256; the timed steps include the check.
+    try:
+        if fused:
+            Pn = cfg.n_gauss
+            keep, n_open = max(Pn // 256, 1), 1
+            while True:
+                _, _, n_open = r.forward_depth_prefix(g, views, keep)
+                if n_open == 0 or keep >= Pn:
+                    break
+                keep = min(Pn, keep * 2)
+            if n_open == 0:
+                same = bool(torch.equal(r.color, color_full)) if (color_full := getattr(r, "_color_full", None)) is not None else None
+                for _ in range(2):
+                    r.forward_depth_prefix(g, views, keep); r.backward(g, views, gcol)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                for _ in range(5):
+                    r.forward_depth_prefix(g, views, keep); r.backward(g, views, gcol)
+                e1.record(); torch.cuda.synchronize()
+                extras["depth_prefix"] = dict(keep=keep, n_gauss=Pn, n_pairs=int(r.n_pairs), ms_per_step=e0.elapsed_time(e1) / 5,
+                                              image_bit_identical_to_full_lists=same,
+                                              note="lists from the nearest `keep` Gaussians per view; every step checks that no visible pixel is left open")
+            else:
+                extras["depth_prefix"] = dict(keep=keep, open_pixels=int(n_open), note="not every pixel saturates on this workload: the full lists are needed")
+            r.forward(g, views)          # leave the rasteriser in the state of the full path for what follows
+    except Exception as e:      # measurement plumbing only
+        extras["depth_prefix"] = dict(error=str(e))
 
     # end to end through the C ABI with HOST buffers (H2D + D2H inside the timed region)
     h = {k: torch.from_numpy(scene[k]).contiguous().pin_memory() for k in ("means", "scales", "quats", "opac", "sh", "W", "b")}

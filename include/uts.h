@@ -272,6 +272,20 @@ size_t uts_hssim_scratch_bytes(const uts_config* cfg);
 int uts_hssim_loss(const uts_config* cfg, uts_mask mask, const float* X, const float* G, float lambda, float sigma, float* h_map,
                    float* dL_dX, double* loss3, void* scratch, size_t scratch_bytes, void* stream);
 
+/* ----------------------------------------------- occlusion-bounded lists: helpers */
+
+/* A pixel stops reading its tile's list once T < t_eps, so when every visible pixel saturates inside the lists of the `keep` nearest
+ * Gaussians of its view, the image and the gradients do not depend on the other Gaussians at all.  These two calls let a caller use
+ * that, exactly: build the tile lists from a depth prefix, blend, and check; if a pixel is still open, repeat with a larger prefix (or
+ * all Gaussians).  The tile lists of a prefix are the first entries of Alg.1's full lists (same order), so n_last, marks, image and
+ * gradients are those of the full lists; only keys / vals / ranges are shorter.
+ * uts_depth_prefix_flags: flags_out[v,i] = flags[v,i] | 1 when (v,i) is not among the `keep` first of view v in uts_depth_order's order
+ * (emit_rank); pass a uts_proj with flags_out to uts_tile_lists / uts_tile_query (only they read it as "culled"; uts_preprocess_bwd keeps
+ * the original flags).  uts_count_unsaturated: *h_count = number of visible pixels (M_C = 1) with trans >= cfg->t_eps; trans is
+ * uts_render_fwd's output; scratch: 8 bytes, 8-byte aligned; synchronises `stream`. */
+int uts_depth_prefix_flags(const uts_config* cfg, const uint8_t* flags, const uint32_t* emit_rank, uint32_t keep, uint8_t* flags_out, void* stream);
+int uts_count_unsaturated(const uts_config* cfg, uts_mask mask, const float* trans, uint64_t* h_count, void* scratch, void* stream);
+
 /* NESTED pixel centres as camera-frame unit vectors, double [n,3], pixels first..first+n-1 at `order`
  * (exposes the library's HEALPix indexing for tests). */
 int uts_pixel_centers(int order, uint64_t first, uint64_t n, double* out_xyz, void* stream);

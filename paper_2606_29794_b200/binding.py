@@ -21,7 +21,7 @@ UTS_OK, UTS_ERR_INVALID_ARG, UTS_ERR_CAPACITY, UTS_ERR_CUDA, UTS_ERR_UNSUPPORTED
 SYMBOLS = [
     "uts_preprocess", "uts_preprocess_geometry", "uts_preprocess_color", "uts_depth_order", "uts_depth_order_scratch_bytes", "uts_tile_query", "uts_tile_query_scratch_bytes", "uts_tile_lists", "uts_tile_lists_scratch_bytes", "uts_sort", "uts_sort_scratch_bytes",
     "uts_tile_ranges", "uts_render_fwd", "uts_render_bwd", "uts_render_marks_bytes", "uts_render_fwd_marked", "uts_render_bwd_marked", "uts_preprocess_bwd", "uts_build_mask", "uts_pixel_centers",
-    "uts_rho_max_table", "uts_resample_fwd", "uts_resample_bwd", "uts_build_camera_mask", "uts_inv_depth_channel", "uts_inv_depth_bwd", "uts_rs_max_update", "uts_hssim_loss", "uts_hssim_scratch_bytes",
+    "uts_rho_max_table", "uts_resample_fwd", "uts_resample_bwd", "uts_build_camera_mask", "uts_inv_depth_channel", "uts_inv_depth_bwd", "uts_rs_max_update", "uts_depth_prefix_flags", "uts_count_unsaturated", "uts_hssim_loss", "uts_hssim_scratch_bytes",
     "uts_host_workspace_bytes", "uts_host_forward_backward", "uts_last_cuda_error", "uts_launch_count", "uts_strerror",
     "uts_version",
 ]
@@ -393,6 +393,20 @@ def uts_build_camera_mask(cfg: Config, cam: Camera, device="cuda", stream=None) 
     _check(lib().uts_build_camera_mask(C.byref(c), cam.c(), _ptr(bits), _ptr(slot), _ptr(act), C.byref(n), _stream(stream)),
            "uts_build_camera_mask")
     return Mask(act[: n.value].contiguous(), int(n.value), slot, bits)
+
+
+def uts_depth_prefix_flags(cfg: Config, flags, emit_rank, keep: int, flags_out, stream=None):
+    c = cfg.c()
+    _check(lib().uts_depth_prefix_flags(C.byref(c), _ptr(flags, torch.uint8), _ptr(emit_rank), C.c_uint32(keep), _ptr(flags_out, torch.uint8),
+                                        _stream(stream)), "uts_depth_prefix_flags")
+
+
+def uts_count_unsaturated(cfg: Config, mask: Mask, trans, scratch, stream=None) -> int:
+    c = cfg.c()
+    n = C.c_uint64(0)
+    _check(lib().uts_count_unsaturated(C.byref(c), mask.c(), _ptr(trans, torch.float32), C.byref(n), _ptr(scratch), _stream(stream)),
+           "uts_count_unsaturated")
+    return int(n.value)
 
 
 def uts_hssim_scratch_bytes(cfg: Config) -> int:

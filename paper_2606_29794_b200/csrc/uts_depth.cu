@@ -54,6 +54,31 @@ __global__ void rs_max_kernel(int P, int V, const float* __restrict__ rs, const 
   rs_max[i] = m;
 }
 
+// ---- occlusion-bounded lists: helpers, the orchestration is the caller's
+__global__ void depth_prefix_flags_kernel(int P, int64_t n, const uint8_t* __restrict__ flags, const uint32_t* __restrict__ emit_rank, uint32_t keep,
+                                          uint8_t* __restrict__ out) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  const uint32_t v = (uint32_t)(k / P);
+  const uint32_t rank_in_view = __ldg(emit_rank + k) - v * (uint32_t)P;       // emit_rank orders by (view, depth, id)
+  out[k] = (uint8_t)(__ldg(flags + k) | (rank_in_view >= keep ? 1u : 0u));
+}
+
+__global__ void count_unsaturated_kernel(int64_t n, int64_t n_slot, const uint32_t* __restrict__ active_tiles, const uint32_t* __restrict__ bits,
+                                         const float* __restrict__ trans, float t_eps, unsigned long long* __restrict__ count) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  bool open = false;
+  if (idx < n) {
+    const int64_t slot = (idx >> 8) % n_slot;
+    const int64_t tile = active_tiles ? (int64_t)__ldg(active_tiles + slot) : slot;
+    const int64_t p = tile * 256 + (idx & 255);
+    const bool on = bits ? ((__ldg(bits + (p >> 5)) >> (p & 31)) & 1u) != 0 : true;
+    open = on && !(__ldg(trans + idx) < t_eps);
+  }
+  const unsigned m = __ballot_sync(0xffffffffu, open);
+  if ((threadIdx.x & 31) == 0 && m) atomicAdd(count, (unsigned long long)__popc(m));
+}
+
 }  // namespace uts
 
 using namespace uts;
@@ -90,6 +115,37 @@ int uts_rs_max_update(const uts_config* cfg, const float* rs, const uint8_t* fla
   if (!rs || !flags || !rs_max) return UTS_ERR_INVALID_ARG;
   rs_max_kernel<<<(unsigned)((cfg->n_gauss + 255) / 256), 256, 0, (cudaStream_t)stream>>>(cfg->n_gauss, cfg->n_views, rs, flags, rs_max);
   UTS_LAUNCH_CHECK();
+  return UTS_OK;
+}
+
+int uts_depth_prefix_flags(const uts_config* cfg, const uint8_t* flags, const uint32_t* emit_rank, uint32_t keep, uint8_t* flags_out, void* stream) {
+  int st = check_config(cfg);
+  if (st) return st;
+  const int64_t n = (int64_t)cfg->n_gauss * cfg->n_views;
+  if (n == 0) return UTS_OK;
+  if (!flags || !emit_rank || !flags_out) return UTS_ERR_INVALID_ARG;
+  depth_prefix_flags_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(cfg->n_gauss, n, flags, emit_rank, keep, flags_out);
+  UTS_LAUNCH_CHECK();
+  return UTS_OK;
+}
+
+int uts_count_unsaturated(const uts_config* cfg, uts_mask mask, const float* trans, uint64_t* h_count, void* scratch, void* stream) {
+  int st = check_config(cfg);
+  if (st) return st;
+  if ((st = check_mask(cfg, mask))) return st;
+  if (!h_count || !scratch || ((uintptr_t)scratch & 7)) return UTS_ERR_INVALID_ARG;
+  const Dims d = dims_of(cfg, &mask);
+  const int64_t n = (int64_t)d.V * d.n_slot * kTilePix;
+  cudaStream_t s = (cudaStream_t)stream;
+  UTS_CUDA(cudaMemsetAsync(scratch, 0, 8, s));
+  if (n > 0) {
+    if (!trans) return UTS_ERR_INVALID_ARG;
+    count_unsaturated_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(n, d.n_slot, mask.active_tiles, mask.pixel_mask_bits, trans, cfg->t_eps,
+                                                                         (unsigned long long*)scratch);
+    UTS_LAUNCH_CHECK();
+  }
+  UTS_CUDA(cudaMemcpyAsync(h_count, scratch, 8, cudaMemcpyDeviceToHost, s));
+  UTS_CUDA(cudaStreamSynchronize(s));
   return UTS_OK;
 }
 

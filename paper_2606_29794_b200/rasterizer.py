@@ -131,6 +131,28 @@ class Rasterizer:
         self.render_fwd()
         return self.color, self.alpha
 
+    def forward_depth_prefix(self, g, views, keep: int):
+        """Forward with tile lists built from the `keep` nearest Gaussians of each view only (needs fused_lists).  Returns
+        (color, alpha, n_open): n_open = visible pixels that did not saturate; 0 means image, n_last and the gradients of backward()
+        are exactly those of the full lists (include/uts.h, uts_depth_prefix_flags).  The caller decides what to do otherwise
+        (forward() again, or a larger prefix)."""
+        assert self.fused_lists
+        self.preprocess(g, views)
+        self.depth_order()
+        if getattr(self, "_pflags", None) is None:
+            self._pflags = torch.empty_like(self.proj.flags)
+            self._cnt = torch.zeros(1, dtype=torch.int64, device=self.dev)
+        B.uts_depth_prefix_flags(self.cfg, self.proj.flags, self.emit_rank, int(keep), self._pflags)
+        full = self.proj
+        self.proj = B.Proj(full.dir, full.lonlat, full.rho, full.conic_opac, full.rs, full.rgb, self._pflags)
+        try:
+            self.tile_lists()
+        finally:
+            self.proj = full
+        self.render_fwd()
+        n_open = B.uts_count_unsaturated(self.cfg, self.mask, self.trans, self._cnt)
+        return self.color, self.alpha, n_open
+
     def backward(self, g, views, dL_dcolor, dL_dalpha=None):
         self.render_bwd(dL_dcolor, dL_dalpha)
         self.preprocess_bwd(g, views)

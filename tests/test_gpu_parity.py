@@ -650,3 +650,40 @@ def test_marked_blend_equals_plain_blend(cfg_id, P, order):
     for k in Gm:
         a, b = Gm[k], Gp[k]
         assert float((a - b).abs().max()) <= 2e-4 * float(b.abs().max()) + 1e-12, k
+
+
+def test_depth_prefix_lists_give_the_full_result_when_every_pixel_saturates():
+    """Occlusion-bounded lists (include/uts.h, uts_depth_prefix_flags / uts_count_unsaturated): lists built from the nearest `keep`
+    Gaussians only.  n_open counts the visible pixels that did not saturate; with keep = P it is the full forward's own count; and as
+    soon as a prefix leaves no pixel open, image, alpha, T and n_last are bit-identical to the full lists' and the gradients are the
+    same sums — with far fewer pairs."""
+    B, R = _gpu()
+    scene = small_scene(4, 400000, 6)                      # dense: the large near Gaussians saturate every pixel
+    cfg = _cfg(R, scene)
+    g, views = R.scene_to_device(scene)
+    full = R.Rasterizer(cfg)
+    cf, af = full.forward(g, views)
+    P = cfg.n_gauss
+    scratch = torch.zeros(1, dtype=torch.int64, device="cuda")
+    open_full = B.uts_count_unsaturated(cfg, full.mask, full.trans, scratch)
+    assert open_full == int((full.trans >= cfg.t_eps).sum())
+    pre = R.Rasterizer(cfg)
+    _, _, n_open = pre.forward_depth_prefix(g, views, P)
+    assert n_open == open_full and pre.n_pairs == full.n_pairs
+    assert open_full == 0, "pick a denser scene: the test needs every pixel to saturate"
+    _, _, n_small = pre.forward_depth_prefix(g, views, 8)
+    assert n_small > 0                                    # eight Gaussians cannot saturate the sphere: reported, not hidden
+    keep = P // 512
+    while True:
+        cp, ap, n_open = pre.forward_depth_prefix(g, views, keep)
+        if n_open == 0 or keep >= P:
+            break
+        keep *= 2
+    assert n_open == 0 and keep <= P // 4 and pre.n_pairs < full.n_pairs // 2
+    for a, b in ((cp, cf), (ap, af), (pre.trans, full.trans), (pre.n_last, full.n_last)):
+        assert torch.equal(a, b)
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    gcol = torch.randn(cf.shape, device="cuda", generator=gen)
+    Gp = pre.backward(g, views, gcol); Gf = full.backward(g, views, gcol)
+    for k in Gf:
+        assert float((Gp[k] - Gf[k]).abs().max()) <= 2e-4 * float(Gf[k].abs().max()) + 1e-12, k

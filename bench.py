@@ -274,8 +274,11 @@ def run_ours(args):
     # timed on view 0's HEALPix image.  Camera: the paper's case for this grid where there is no mask (6080 x 3040 panorama ->
     # Nside 1024, Table 5), else a 1920 x 1080 pinhole of 60 x 45 degrees (config 5's frustum).
     extras = {}
+    run_extras = not args.no_extras
     r._color_full = r.color.clone()          # the full lists' image, for the bit-identity check of the depth-prefix leg below
     try:
+        if not run_extras:
+            raise RuntimeError("skipped (--no-extras)")
         cam = B.Camera("equirect", 6080, 3040) if mask.active_tiles is None else B.Camera("pinhole", 1920, 1080, np.radians(60.0), np.radians(45.0))
         img = r.color[0].contiguous()
         o_img = torch.empty(cam.height, cam.width, 3, dtype=torch.float32, device="cuda")
@@ -301,6 +304,8 @@ def run_ours(args):
     # the step before the backward hot path (not part of the step): L1 + HEALPix-SSIM loss and dL/dI on view 0's
     # image against a seeded target (the image plus N(0, 0.05) noise, clipped)
     try:
+        if not run_extras:
+            raise RuntimeError("skipped (--no-extras)")
         img = r.color[0].contiguous()
         tgt = (img + 0.05 * torch.randn(img.shape, device="cuda", generator=torch.Generator(device="cuda").manual_seed(7))).clamp_(0, 1)
         loss3 = torch.empty(3, dtype=torch.float64, device="cuda")
@@ -328,6 +333,8 @@ def run_ours(args):
     # Gaussians, verified every time by uts_count_unsaturated — when no visible pixel is left open, image and gradients are exactly
     # the full lists' ones.  keep is found by doubling from P/256; the timed steps include the check.
     try:
+        if not run_extras:
+            raise RuntimeError("skipped (--no-extras)")
         if fused:
             Pn = cfg.n_gauss
             keep, n_open = max(Pn // 256, 1), 1
@@ -464,6 +471,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--lists", default="fused", choices=["fused", "staged"],
                     help="Alg.1 l.9-16 as one uts_tile_lists call (default) or as uts_tile_query + uts_sort + uts_tile_ranges")
+    ap.add_argument("--no-extras", action="store_true", help="skip the legs that are not part of the step (resample, loss, depth prefix): used for the launch list")
     ap.add_argument("--marks", default="on", choices=["on", "off"],
                     help="blend through uts_render_fwd_marked / uts_render_bwd_marked (default) or the plain pair")
     args = ap.parse_args()

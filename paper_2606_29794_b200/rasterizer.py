@@ -153,6 +153,24 @@ class Rasterizer:
         n_open = B.uts_count_unsaturated(self.cfg, self.mask, self.trans, self._cnt)
         return self.color, self.alpha, n_open
 
+    def forward_auto(self, g, views):
+        """forward() through the depth prefix when that is known to pay, through the full lists otherwise; the result is always the
+        full lists' one (a prefix is accepted only when uts_count_unsaturated returns 0).  The prefix length is a running guess:
+        it starts at P/128, grows fourfold after a failed attempt (the full lists are then built for this call) and the attempts stop
+        once it would pass P/2 — the scene does not saturate, as configs 1, 2, 3 and 5 do not."""
+        P = self.cfg.n_gauss
+        st = self.__dict__.setdefault("_auto", dict(keep=max(P // 128, 1), off=not self.fused_lists, used_prefix=False))
+        st["used_prefix"] = False
+        if not st["off"]:
+            c, a, n_open = self.forward_depth_prefix(g, views, st["keep"])
+            if n_open == 0:
+                st["used_prefix"] = True
+                return c, a
+            st["keep"] *= 4
+            if st["keep"] > P // 2:
+                st["off"] = True
+        return self.forward(g, views)
+
     def backward(self, g, views, dL_dcolor, dL_dalpha=None):
         self.render_bwd(dL_dcolor, dL_dalpha)
         self.preprocess_bwd(g, views)

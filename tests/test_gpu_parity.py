@@ -687,3 +687,29 @@ def test_depth_prefix_lists_give_the_full_result_when_every_pixel_saturates():
     Gp = pre.backward(g, views, gcol); Gf = full.backward(g, views, gcol)
     for k in Gf:
         assert float((Gp[k] - Gf[k]).abs().max()) <= 2e-4 * float(Gf[k].abs().max()) + 1e-12, k
+
+
+def test_forward_auto_is_always_the_full_result():
+    """Rasterizer.forward_auto: depth prefix when every pixel saturates inside it, full lists otherwise — the image is the full
+    lists' image either way, bit for bit."""
+    B, R = _gpu()
+    # (a) a scene that saturates everywhere: the second call at the latest goes through the prefix
+    scene = small_scene(4, 400000, 6)
+    cfg = _cfg(R, scene)
+    g, views = R.scene_to_device(scene)
+    full = R.Rasterizer(cfg); cf, _ = full.forward(g, views)
+    auto = R.Rasterizer(cfg)
+    for _ in range(3):
+        ca, _ = auto.forward_auto(g, views)
+        assert torch.equal(ca, cf) and torch.equal(auto.n_last, full.n_last)
+    assert auto._auto["used_prefix"] and auto.n_pairs < full.n_pairs
+    # (b) a scene that does not: the attempts stop, every call returns the full result
+    scene = small_scene(1, 3000, 6)
+    cfg = _cfg(R, scene)
+    g, views = R.scene_to_device(scene)
+    full = R.Rasterizer(cfg); cf, _ = full.forward(g, views)
+    auto = R.Rasterizer(cfg)
+    for _ in range(6):
+        ca, _ = auto.forward_auto(g, views)
+        assert torch.equal(ca, cf) and auto.n_pairs == full.n_pairs
+    assert auto._auto["off"] and not auto._auto["used_prefix"]

@@ -391,3 +391,90 @@ def test_mask_semantics():
     sel = on[pix]
     assert np.array_equal(msk["color"][0][sel], full["color"][0][pix][sel])
     assert np.all(msk["color"][0][~sel] == 0) and np.all(msk["n_last"][0][~sel] == 0) and np.all(msk["alpha"][0][~sel] == 0)
+
+
+# ------------------------------------------------------------------ rotation / anisotropy / SH sign pins
+def _rodrigues(axis, th):
+    """Rotation by angle th about `axis` (right-handed, active): R = I + sin(th) K + (1 - cos(th)) K^2 — textbook, built here
+    without the oracle's QuatToMat."""
+    a = np.asarray(axis, np.float64); a = a / np.linalg.norm(a)
+    K = np.array([[0, -a[2], a[1]], [a[2], 0, -a[0]], [-a[1], a[0], 0]])
+    return np.eye(3) + math.sin(th) * K + (1 - math.cos(th)) * (K @ K)
+
+
+@pytest.mark.parametrize("dil", [0.0, 0.3])
+def test_single_anisotropic_rotated_gaussian_from_first_principles(dil):
+    """Pins QuatToMat (R, not R^T; Alg.1 l.4 PAPER.md:537), the (east,north) orientation of SphericalOffset and the sign of
+    the conic's off-diagonal (Eq.2) — none of which an isotropic Gaussian can see.  ONE strongly anisotropic
+    Gaussian (scales 0.02 / 0.1 / 0.3) with a non-trivial rotation, a tilted view W and b != 0, alpha rules disabled.
+    Expected value, numpy only: Sigma3D = R diag(s^2) R^T with R from Rodrigues' formula on the axis-angle the quaternion
+    encodes; Sigma2 = E (W Sigma3D W^T) E^T / rho^2 (+ h I) in an ARBITRARY orthonormal tangent basis E at the Gaussian's
+    direction (not the oracle's east/north: the quadratic form does not depend on the basis); delta = the pixel direction's
+    log-map offset in that basis; alpha = o exp(-delta^T Sigma2^-1 delta / 2).  (1) log-map offset: equality to rounding;
+    (2) gnomonic (pinhole-on-the-tangent-plane) offset, the flat-space limit of EWA splatting: agreement to O((sigma/rho)^2)."""
+    k = 9
+    cfg = orc.Config(order=k, n_gauss=1, alpha_min=0.0, alpha_max=1.0, t_eps=0.0, cov_dilation_px2=dil)
+    axis = np.array([0.3, -0.5, 0.8]); axis /= np.linalg.norm(axis); th = 1.1
+    q32 = np.float32(np.concatenate([[math.cos(th / 2)], math.sin(th / 2) * axis]))
+    s32 = np.float32([0.02, 0.1, 0.3]); mu32 = np.float32([2.6, 2.1, -4.4]); o32 = np.float32(0.85)
+    W32 = np.float32(_rodrigues([1.0, 0.4, -0.2], 0.7)); b32 = np.float32([0.3, -0.2, 0.5])
+    sh0 = np.float32([1.0, 0.5, -0.2])
+    sc = dict(means=mu32[None], scales=s32[None], quats=q32[None], opac=np.float32([o32]), sh=sh0.reshape(1, 1, 3),
+              W=W32.reshape(1, 9), b=b32[None], order=k, n_gauss=1, n_views=1, sh_degree=0)
+    out = orc.forward_chain(cfg, sc)
+
+    s, mu, o, W, b = (a.astype(np.float64) for a in (s32, mu32, o32, W32, b32))
+    R = _rodrigues(axis, th)
+    Sigma = R @ np.diag(s * s) @ R.T
+    t = W @ mu + b; rho = np.linalg.norm(t); u = t / rho
+    e1 = np.cross(u, [0.2, 0.9, -0.4]); e1 /= np.linalg.norm(e1); e2 = np.cross(u, e1)
+    E = np.stack([e1, e2])
+    h = float(np.float32(dil)) * 4 * math.pi / cfg.n_pix
+    S2 = E @ (W @ Sigma @ W.T) @ E.T / rho ** 2 + h * np.eye(2)
+    ev = np.linalg.eigvalsh(S2)
+    assert ev[1] / ev[0] > 8 and abs(S2[0, 1]) > 0.1 * ev[1]               # really anisotropic, really oblique in this basis
+    Q = np.linalg.inv(S2)
+    _, _, w = orc.centers(k, 2)
+    c = w @ u; tau = w - c[:, None] * u[None, :]; sn = np.linalg.norm(tau, axis=1)
+    g = np.arctan2(sn, c)
+    d_log = (tau @ E.T) * (g / np.maximum(sn, 1e-300))[:, None]
+    a_log = o * np.exp(-0.5 * np.einsum("pi,ij,pj->p", d_log, Q, d_log))
+    rgb = 0.5 + 0.28209479177387814 * sh0.astype(np.float64)
+    tiles = (out["keys"] >> np.uint64(32)).astype(np.int64)
+    in_list = np.isin(np.arange(cfg.n_pix) >> 8, tiles)
+    assert 3 <= np.unique(tiles).shape[0] and a_log[~in_list].max(initial=0) < math.exp(-4.5) * o
+    assert (a_log[in_list] > 0.5).sum() > 100                               # the Gaussian is resolved by many pixels
+    assert np.abs(out["alpha"][0] - np.where(in_list, a_log, 0)).max() < 5e-6
+    assert np.abs(out["color"][0] - np.where(in_list[:, None], a_log[:, None] * rgb[None, :], 0)).max() < 5e-6
+    # r_s = 3 sqrt(lambda_max) (PAPER.md:81) from the same independent matrix
+    assert out["proj"].rs[0, 0] == pytest.approx(3 * math.sqrt(ev[1]), rel=1e-6)
+    # (2) flat-space limit: pinhole projection onto the tangent plane at u
+    front = c > 0.5
+    d_gn = (w @ E.T) / np.where(front, c, 1.0)[:, None]
+    a_gn = np.where(front, o * np.exp(-0.5 * np.einsum("pi,ij,pj->p", d_gn, Q, d_gn)), 0.0)
+    sig_max = math.sqrt(ev[1])
+    err = np.abs(out["alpha"][0] - a_gn)[in_list].max()
+    assert err < 2.0 * sig_max ** 2 and sig_max ** 2 < 2e-3, (err, sig_max)
+    # what a transposed R (or swapped tangent axes) would give is far outside both tolerances
+    S2_T = E @ (W @ (R.T @ np.diag(s * s) @ R) @ W.T) @ E.T / rho ** 2 + h * np.eye(2)
+    a_T = o * np.exp(-0.5 * np.einsum("pi,ij,pj->p", d_log, np.linalg.inv(S2_T), d_log))
+    assert np.abs(a_T - a_log)[in_list].max() > 0.3
+
+
+def test_sh_basis_signs_against_scipy_complex_harmonics():
+    """Degree 0-3 constants AND signs of the real SH basis (reading A13) against a library routine: the convention is the real
+    form of the complex harmonics with the Condon-Shortley phase kept, index l^2 + l + m:
+        m > 0: sqrt(2) Re Y_l^m,   m = 0: Y_l^0,   m < 0: sqrt(2) Im Y_l^|m|
+    (degree 1 then reads (-y, z, -x) sqrt(3/4pi), the convention stated in SURVEY 8c O1.5).  scipy evaluates Y_l^m through
+    Legendre recurrences, not through the polynomial table the oracle restates."""
+    from scipy.special import sph_harm_y
+    rng = np.random.default_rng(11)
+    for _ in range(25):
+        d = rng.standard_normal(3); d /= np.linalg.norm(d)
+        theta, phi = math.acos(d[2]), math.atan2(d[1], d[0])
+        want = []
+        for l in range(4):
+            for m in range(-l, l + 1):
+                y = complex(sph_harm_y(l, abs(m), theta, phi))
+                want.append(y.real if m == 0 else math.sqrt(2) * (y.real if m > 0 else y.imag))
+        assert np.allclose(orc.sh_basis(3, d), want, rtol=0, atol=1e-12)

@@ -17,13 +17,18 @@
  *
  * Conventions
  *   - extern "C"; every call returns an int status (UTS_OK = 0).  Nothing throws, aborts, allocates or frees
- *     caller-visible memory: THE CALLER OWNS EVERY BUFFER, including scratch (sizes from uts_*_scratch_bytes).
+ *     device memory: THE CALLER OWNS EVERY BUFFER, including scratch (sizes from uts_*_scratch_bytes).
  *   - Every pointer is a DEVICE pointer unless its name starts with h_ (host; pinned where it is written
  *     asynchronously).  uts_config is read on the host.  The only calls taking host data arrays are the
  *     uts_host_* calls at the end.
  *   - All work is enqueued on `stream` (a cudaStream_t passed as void*); calls are asynchronous.  Where a host
  *     count is returned (h_n_pairs) the call synchronises the stream before returning, as documented there.
- *   - No global state except the last CUDA error code; no CPU fallback; sm_100 only.
+ *   - Library state: the last CUDA error code, the launch counter, and ONE CONTEXT PER DEVICE, created on the first call made with
+ *     that device current and kept until the process ends: the SM count, cached occupancy numbers, two auxiliary streams with their
+ *     fork / join events (uts_tile_query / uts_tile_lists run their three work shapes side by side on them and join back into
+ *     `stream` before returning) and one copy stream with four events (uts_host_forward_backward).  A per-device mutex is held
+ *     while a call enqueues on those streams, so calls may be issued from several threads and on several streams; they never
+ *     read the environment.  No CPU fallback; sm_100 only.
  *   - Inputs are ACTIVATED values: scales > 0, opacity in (0,1), quaternion (w,x,y,z) used as given
  *     (reading A14).  Arrays are dense row-major float32 unless stated.
  *   - Index conventions: NESTED pixel p = f*4^k + interleave(x,y); tile of p = p >> (2*tile_log2); pixel slot
@@ -103,6 +108,18 @@ typedef struct {
   const uint32_t* pixel_mask_bits; /* [N_pix/32] bit (p & 31) of word p>>5 is M_C(p), NESTED order */
 } uts_mask;
 
+/* Optional steering of the tile query's implementation choices (tests and A/B measurements).  Production passes NULL, which is
+ * the same as every field 0.  None of these changes the result: the tile set, the sorted arrays and the ranges are bit-identical
+ * for every setting. */
+typedef struct {
+  int   query_impl;        /* 0: ring intervals (uts_ring_query.cuh) when k_q <= 12, else the quadtree descent;
+                              1: always the quadtree descent — Alg.2's depth-first form, stackless */
+  float descent_block_radius; /* descent only: discs with R > value / sqrt(N_tile) take the block-per-Gaussian bitmap path; 0 = 36 */
+  int   descent_blocks_per_sm;/* descent only: persistent blocks per SM of that path; 0 = 2 */
+  int   matrix_off;        /* uts_tile_lists: 1 = never route discs through the (disc x tile) bit matrix */
+  float matrix_min_tiles;  /* uts_tile_lists: discs covering at least this many tiles become matrix rows; 0 = max(48, N_tile / 144) */
+} uts_tuning;
+
 /* ---------------------------------------------------------------------------------------------- forward */
 
 /* Alg.1 l.2-8.  For each view v and Gaussian i fills every array of `out` at index v*P+i.  Culled records
@@ -138,7 +155,7 @@ size_t uts_depth_order_scratch_bytes(const uts_config* cfg);
  * scratch: uts_tile_query_scratch_bytes(cfg) bytes, 256-byte aligned. */
 int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint32_t* emit_rank, uint64_t* offsets,
                    uint64_t* keys, uint32_t* vals, uint64_t capacity, uint64_t* h_n_pairs, void* scratch,
-                   size_t scratch_bytes, void* stream);
+                   size_t scratch_bytes, const uts_tuning* tuning /* may be NULL */, void* stream);
 
 /* F2 + F3 + F4 in one call (Alg.1 l.9-16): the sorted pair arrays and the tile ranges, bit-identical to
  *     uts_tile_query(emit_rank) -> uts_sort(depth_presorted = 1) -> uts_tile_ranges,
@@ -154,7 +171,8 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
 size_t uts_tile_lists_scratch_bytes(const uts_config* cfg);
 int uts_tile_lists(const uts_config* cfg, uts_proj in, uts_mask mask, const uint32_t* emit_rank, uint64_t* keys, uint32_t* vals,
                    uint64_t* keys_tmp, uint32_t* vals_tmp, uint64_t capacity, uint64_t* ranges, uint64_t* h_n_pairs, void* scratch,
-                   size_t scratch_bytes, void* sort_scratch, size_t sort_scratch_bytes, void* stream);
+                   size_t scratch_bytes, void* sort_scratch, size_t sort_scratch_bytes, const uts_tuning* tuning /* may be NULL */,
+                   void* stream);
 size_t uts_tile_query_scratch_bytes(const uts_config* cfg);
 
 /* Alg.1 l.15.  Stable ascending LSD radix sort on the 64-bit key (ties keep emission order; with emission in Gaussian-id
@@ -211,8 +229,8 @@ int uts_preprocess_bwd(const uts_config* cfg, uts_gaussians g, uts_views views, 
 
 /* Builds M_C on the device: kind 0 = spherical cap, h_params = axis[3], half_angle;
  * kind 1 = pinhole frustum in the frame (right,up,fwd), h_params = right[3], up[3], fwd[3], tan_x, tan_y.
- * pixel_mask_bits [N_pix/32], slot_of_tile [N_tile], active_tiles [N_tile] (first n_active entries valid).
- * Synchronises `stream` and writes n_active to *h_n_active. */
+ * pixel_mask_bits [N_pix/32], slot_of_tile [N_tile], active_tiles [N_tile + 1]: the first n_active entries are the list, entry
+ * N_tile receives n_active on the device (the call allocates nothing).  Synchronises `stream` and writes n_active to *h_n_active. */
 int uts_build_mask(const uts_config* cfg, int kind, const double* h_params, uint32_t* pixel_mask_bits,
                    int32_t* slot_of_tile, uint32_t* active_tiles, int* h_n_active, void* stream);
 

@@ -62,6 +62,27 @@ class CMask(C.Structure):
     _fields_ = [("active_tiles", C.c_void_p), ("n_active", C.c_int), ("slot_of_tile", C.c_void_p), ("pixel_mask_bits", C.c_void_p)]
 
 
+class CTuning(C.Structure):
+    _fields_ = [("query_impl", C.c_int), ("descent_block_radius", C.c_float), ("descent_blocks_per_sm", C.c_int), ("matrix_off", C.c_int),
+                ("matrix_min_tiles", C.c_float)]
+
+
+@dataclass
+class Tuning:
+    """uts_tuning (include/uts.h): steers implementation choices of the tile query, never its result.  None = defaults."""
+    query_impl: int = 0                 # 1: the quadtree descent (Alg.2's depth-first form)
+    descent_block_radius: float = 0.0
+    descent_blocks_per_sm: int = 0
+    matrix_off: int = 0
+    matrix_min_tiles: float = 0.0
+
+    def c(self): return CTuning(self.query_impl, self.descent_block_radius, self.descent_blocks_per_sm, self.matrix_off, self.matrix_min_tiles)
+
+
+def _tuning(t):
+    return None if t is None else C.byref(t.c())
+
+
 @dataclass
 class Config:
     """uts_config (include/uts.h).  Defaults follow DESIGN.md readings A3, A5, A7, A8."""
@@ -216,13 +237,14 @@ def uts_depth_order(cfg: Config, rho, emit_rank, scratch, stream=None):
                                  C.c_size_t(scratch.numel() * scratch.element_size()), _stream(stream)), "uts_depth_order")
 
 
-def uts_tile_query(cfg: Config, proj: Proj, mask: Mask, offsets, keys, vals, capacity: int, scratch, emit_rank=None, stream=None) -> int:
+def uts_tile_query(cfg: Config, proj: Proj, mask: Mask, offsets, keys, vals, capacity: int, scratch, emit_rank=None, tuning: Tuning | None = None,
+                   stream=None) -> int:
     """Returns the pair count.  keys=None: count only.  Raises UtsError(UTS_ERR_CAPACITY) with .needed set."""
     c = cfg.c()
     n = C.c_uint64(0)
     st = lib().uts_tile_query(C.byref(c), proj.c(), mask.c(), _ptr(emit_rank, torch.int32), _ptr(offsets, torch.int64), _ptr(keys, torch.int64), _ptr(vals, torch.int32),
                               C.c_uint64(capacity), C.byref(n), _ptr(scratch), C.c_size_t(scratch.numel() * scratch.element_size()),
-                              _stream(stream))
+                              _tuning(tuning), _stream(stream))
     if st == UTS_ERR_CAPACITY:
         e = UtsError(st, "uts_tile_query"); e.needed = int(n.value); raise e
     _check(st, "uts_tile_query")
@@ -242,14 +264,14 @@ def uts_tile_lists_scratch_bytes(cfg: Config) -> int:
 
 
 def uts_tile_lists(cfg: Config, proj: Proj, mask: Mask, emit_rank, keys, vals, keys_tmp, vals_tmp, capacity: int, ranges, scratch, sort_scratch,
-                   stream=None) -> int:
+                   tuning: Tuning | None = None, stream=None) -> int:
     """Sorted pairs + tile ranges in one call (see include/uts.h).  Returns the pair count; raises UtsError (status
     UTS_ERR_CAPACITY, .needed = required capacity) when the buffers are too small."""
     c = cfg.c()
     n = C.c_uint64(0)
     st = lib().uts_tile_lists(C.byref(c), proj.c(), mask.c(), _ptr(emit_rank), _ptr(keys), _ptr(vals), _ptr(keys_tmp), _ptr(vals_tmp),
                               C.c_uint64(capacity), _ptr(ranges), C.byref(n), _ptr(scratch), C.c_size_t(scratch.numel() * scratch.element_size()),
-                              _ptr(sort_scratch), C.c_size_t(sort_scratch.numel() * sort_scratch.element_size()), _stream(stream))
+                              _ptr(sort_scratch), C.c_size_t(sort_scratch.numel() * sort_scratch.element_size()), _tuning(tuning), _stream(stream))
     if st == UTS_ERR_CAPACITY:
         e = UtsError(st, "uts_tile_lists"); e.needed = int(n.value)
         raise e
@@ -325,7 +347,7 @@ def uts_build_mask(cfg: Config, kind: str, params, device="cuda", stream=None) -
     c = cfg.c()
     bits = torch.empty(cfg.n_pix // 32, dtype=torch.int32, device=device)
     slot = torch.empty(cfg.n_tiles, dtype=torch.int32, device=device)
-    act = torch.empty(cfg.n_tiles, dtype=torch.int32, device=device)
+    act = torch.empty(cfg.n_tiles + 1, dtype=torch.int32, device=device)     # entry N_tile receives n_active
     prm = (C.c_double * len(params))(*[float(x) for x in params])
     n = C.c_int(0)
     _check(lib().uts_build_mask(C.byref(c), C.c_int(0 if kind == "cap" else 1), prm, _ptr(bits), _ptr(slot), _ptr(act), C.byref(n),
@@ -388,7 +410,7 @@ def uts_build_camera_mask(cfg: Config, cam: Camera, device="cuda", stream=None) 
     c = cfg.c()
     bits = torch.empty(cfg.n_pix // 32, dtype=torch.int32, device=device)
     slot = torch.empty(cfg.n_tiles, dtype=torch.int32, device=device)
-    act = torch.empty(cfg.n_tiles, dtype=torch.int32, device=device)
+    act = torch.empty(cfg.n_tiles + 1, dtype=torch.int32, device=device)     # entry N_tile receives n_active
     n = C.c_int(0)
     _check(lib().uts_build_camera_mask(C.byref(c), cam.c(), _ptr(bits), _ptr(slot), _ptr(act), C.byref(n), _stream(stream)),
            "uts_build_camera_mask")

@@ -10,14 +10,35 @@ void set_last_cuda_error(cudaError_t e) { g_last_cuda_error.store((int)e); }
 static std::atomic<unsigned long long> g_launches{0};
 void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
 
+// One context per device, created under a table lock on first use and never destroyed (the streams and events live as long as
+// the process; include/uts.h "Library state").
+DeviceCtx* device_ctx() {
+  constexpr int kMaxDevices = 64;
+  static DeviceCtx* table[kMaxDevices] = {};
+  static std::mutex table_mu;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess || dev < 0 || dev >= kMaxDevices) { set_last_cuda_error(e != cudaSuccess ? e : cudaErrorInvalidDevice); return nullptr; }
+  std::lock_guard<std::mutex> lock(table_mu);
+  if (table[dev]) return table[dev];
+  DeviceCtx* c = new DeviceCtx();
+  c->device = dev;
+  if (cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || c->sms <= 0) c->sms = 148;
+  bool ok = true;
+  for (int i = 0; i < 2 && ok; ++i)
+    ok = cudaStreamCreateWithFlags(&c->aux[i], cudaStreamNonBlocking) == cudaSuccess &&
+         cudaEventCreateWithFlags(&c->join[i], cudaEventDisableTiming) == cudaSuccess;
+  ok = ok && cudaEventCreateWithFlags(&c->fork, cudaEventDisableTiming) == cudaSuccess;
+  ok = ok && cudaStreamCreateWithFlags(&c->copy, cudaStreamNonBlocking) == cudaSuccess;
+  for (int i = 0; i < 4 && ok; ++i) ok = cudaEventCreateWithFlags(&c->ev[i], cudaEventDisableTiming) == cudaSuccess;
+  if (!ok) { set_last_cuda_error(cudaGetLastError()); delete c; return nullptr; }
+  table[dev] = c;
+  return c;
+}
+
 int sm_count() {
-  static int n = 0;
-  if (n == 0) {
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return 148;
-    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
-  }
-  return n;
+  DeviceCtx* c = device_ctx();
+  return c ? c->sms : 148;
 }
 
 int check_config(const uts_config* c) {
@@ -32,6 +53,8 @@ int check_config(const uts_config* c) {
   if ((((int64_t)12 << (2 * (c->order - c->tile_log2))) * c->n_views) > (int64_t)0xffffffffll) return UTS_ERR_UNSUPPORTED;
   if (!(c->alpha_min >= 0.f) || !(c->alpha_max <= 1.f) || !(c->t_eps >= 0.f) || !(c->cov_dilation_px2 >= 0.f))
     return UTS_ERR_INVALID_ARG;
+  if (!(c->alpha_min <= c->alpha_max) || !isfinite(c->r_near)) return UTS_ERR_INVALID_ARG;
+  for (int i = 0; i < 3; ++i) if (!isfinite(c->bg[i])) return UTS_ERR_INVALID_ARG;
   return UTS_OK;
 }
 
@@ -135,12 +158,10 @@ __global__ void mask_tiles_kernel(const uint32_t* __restrict__ bits, int64_t n_t
 
 // active-tile list and slot table of a pixel bitmap (shared by uts_build_mask and uts_build_camera_mask); synchronises s
 int build_mask_tiles(const Dims& d, uint32_t* pixel_mask_bits, int32_t* slot_of_tile, uint32_t* active_tiles, int* h_n_active, cudaStream_t s) {
-  int* d_count = nullptr;   // 4 library-private bytes, freed below; this call is not on the per-frame path
-  UTS_CUDA(cudaMallocAsync((void**)&d_count, sizeof(int), s));
+  int* d_count = reinterpret_cast<int*>(active_tiles + d.n_tile);     // entry N_tile of the caller's buffer receives n_active
   mask_tiles_kernel<<<1, 1024, 0, s>>>(pixel_mask_bits, d.n_tile, slot_of_tile, active_tiles, d_count);
   UTS_LAUNCH_CHECK();
   UTS_CUDA(cudaMemcpyAsync(h_n_active, d_count, sizeof(int), cudaMemcpyDeviceToHost, s));
-  UTS_CUDA(cudaFreeAsync(d_count, s));
   UTS_CUDA(cudaStreamSynchronize(s));
   return UTS_OK;
 }

@@ -99,14 +99,14 @@ int uts_host_forward_backward(const uts_config* cfg, const float* h_means, const
   // Gaussian bytes at degree 3) and the upstream gradient go up while the geometry is projected and the tile lists are built —
   // only the colour pass, just before the blend, needs the SH — and the image comes down while the backward runs (effective
   // with pinned host buffers).
-  cudaStream_t s2 = nullptr;
-  cudaEvent_t ev_up = nullptr, ev_fwd = nullptr, ev_start = nullptr, ev_sh = nullptr;
-  UTS_CUDA(cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking));
-  UTS_CUDA(cudaEventCreateWithFlags(&ev_up, cudaEventDisableTiming));
-  UTS_CUDA(cudaEventCreateWithFlags(&ev_fwd, cudaEventDisableTiming));
-  UTS_CUDA(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
-  UTS_CUDA(cudaEventCreateWithFlags(&ev_sh, cudaEventDisableTiming));
-  struct Cleanup { cudaStream_t s2; cudaEvent_t a, b, c, d; ~Cleanup() { cudaStreamSynchronize(s2); cudaEventDestroy(a); cudaEventDestroy(b); cudaEventDestroy(c); cudaEventDestroy(d); cudaStreamDestroy(s2); } } cleanup{s2, ev_up, ev_fwd, ev_start, ev_sh};
+  // The stream and its four events belong to the device context (created once per device); ctx->mu is held for the whole call,
+  // which ends with both streams synchronised, so the events are never shared between two calls in flight.
+  DeviceCtx* ctx = device_ctx();
+  if (!ctx) return UTS_ERR_CUDA;
+  std::lock_guard<std::recursive_mutex> lock(ctx->mu);
+  cudaStream_t s2 = ctx->copy;
+  cudaEvent_t ev_up = ctx->ev[0], ev_fwd = ctx->ev[1], ev_start = ctx->ev[2], ev_sh = ctx->ev[3];
+  struct Drain { cudaStream_t s2; ~Drain() { cudaStreamSynchronize(s2); } } drain{s2};      // on every exit path
   UTS_CUDA(cudaEventRecord(ev_start, s));                 // s2 must not run ahead of work already queued on the caller's stream
   UTS_CUDA(cudaStreamWaitEvent(s2, ev_start, 0));
   UTS_CUDA(cudaMemcpyAsync(L.sh, h_sh, 3 * M * P * f, cudaMemcpyHostToDevice, s2));
@@ -122,7 +122,7 @@ int uts_host_forward_backward(const uts_config* cfg, const float* h_means, const
   if ((st = uts_depth_order(cfg, L.proj.rho, L.emit_rank, L.do_scratch, L.do_bytes, stream))) return st;
   // Alg.1 l.9-16 in one call: sorted pairs + tile ranges (large discs through the bit matrix, the rest through emit + radix sort)
   if ((st = uts_tile_lists(cfg, L.proj, mask, L.emit_rank, L.keys, L.vals, L.keys_tmp, L.vals_tmp, pair_capacity, L.ranges, h_n_pairs,
-                           L.tq_scratch, L.tq_bytes, L.sort_scratch, L.sort_bytes, stream)))
+                           L.tq_scratch, L.tq_bytes, L.sort_scratch, L.sort_bytes, nullptr, stream)))
     return st;
   UTS_CUDA(cudaStreamWaitEvent(s, ev_sh, 0));
   if ((st = uts_preprocess_color(cfg, g, vw, L.proj, stream))) return st;

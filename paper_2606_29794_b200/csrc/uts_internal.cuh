@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <math.h>
+#include <mutex>
 #include "uts.h"
 
 namespace uts {
@@ -26,7 +27,33 @@ void count_launch();                     // uts_launch_count(): one tick per ker
 
 int check_config(const uts_config* c);   // UTS_OK / UTS_ERR_INVALID_ARG / UTS_ERR_UNSUPPORTED
 int check_mask(const uts_config* c, const uts_mask& m);
-int sm_count();
+int sm_count();                          // of the current device (from its context)
+
+// The library's per-device state (include/uts.h "Library state"): created on the first call made with the device current, kept
+// until the process ends.  `mu` is held by a call while it enqueues on the streams below (fork ... join), so concurrent callers
+// never interleave their event records; the streams themselves only order work.
+struct DeviceCtx {
+  std::recursive_mutex mu;            // recursive: uts_host_forward_backward holds it around the stage calls
+  int device = -1, sms = 148;
+  cudaStream_t aux[2] = {nullptr, nullptr};         // tile query: the three work shapes run side by side
+  cudaEvent_t fork = nullptr, join[2] = {nullptr, nullptr};
+  cudaStream_t copy = nullptr;                      // uts_host_forward_backward: copies off the critical path
+  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  bool attrs_set[4] = {false, false, false, false}; // cudaFuncSetAttribute done, per translation unit (under mu)
+  static constexpr int kOccSlots = 32;              // cached cudaOccupancyMaxActiveBlocksPerMultiprocessor results (under mu)
+  uint64_t occ_key[kOccSlots] = {}; int occ_val[kOccSlots] = {}; int occ_n = 0;
+};
+DeviceCtx* device_ctx();                 // nullptr when the CUDA runtime fails (last error set)
+// blocks per SM of `kernel` at (threads, dynamic smem), looked up in / added to ctx's cache; the caller holds ctx->mu
+template <class K>
+inline int cached_occupancy(DeviceCtx* ctx, int kernel_id, K kernel, int threads, size_t smem) {
+  const uint64_t key = ((uint64_t)kernel_id << 48) | ((uint64_t)threads << 36) | (uint64_t)smem;
+  for (int i = 0; i < ctx->occ_n; ++i) if (ctx->occ_key[i] == key) return ctx->occ_val[i];
+  int occ = 1;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem) != cudaSuccess || occ < 1) occ = 1;
+  if (ctx->occ_n < DeviceCtx::kOccSlots) { ctx->occ_key[ctx->occ_n] = key; ctx->occ_val[ctx->occ_n] = occ; ++ctx->occ_n; }
+  return occ;
+}
 
 // --------------------------------------------------------------------------------------------- derived
 struct Dims {
@@ -44,7 +71,7 @@ inline Dims dims_of(const uts_config* c, const uts_mask* m) {
   return d;
 }
 
-// rho_max(o) table (host, computed once): see uts_healpix.cu
+// rho_max(o) table (host, computed once): uts_common.cu, fill_rho_max()
 const double* rho_max_table_host();
 
 // ------------------------------------------------------------------------------------- HEALPix (device)

@@ -188,7 +188,15 @@ static int radix_sort_bytes(uint64_t n_pairs, uint64_t* keys, uint32_t* vals, ui
   uint64_t* offs = reinterpret_cast<uint64_t*>(sp);              sp += (((m + 1) * 8 + 255) / 256) * 256;
   uint64_t* block_sums = reinterpret_cast<uint64_t*>(sp);
   uint64_t* kin = keys; uint32_t* vin = vals; uint64_t* kout = keys_tmp; uint32_t* vout = vals_tmp;
-  UTS_CUDA(cudaFuncSetAttribute(sort_downsweep, cudaFuncAttributeMaxDynamicSharedMemorySize, kSortTile * 12));
+  DeviceCtx* ctx = device_ctx();
+  if (!ctx) return UTS_ERR_CUDA;
+  {
+    std::lock_guard<std::recursive_mutex> lock(ctx->mu);
+    if (!ctx->attrs_set[1]) {                                    // once per device
+      UTS_CUDA(cudaFuncSetAttribute(sort_downsweep, cudaFuncAttributeMaxDynamicSharedMemorySize, kSortTile * 12));
+      ctx->attrs_set[1] = true;
+    }
+  }
   for (int pass = 0; pass < n_bytes; ++pass) {
     const int shift = 8 * (first_byte + pass);
     sort_upsweep<<<nb, kSortThreads, 0, s>>>(kin, n_pairs, shift, nb, counts);
@@ -201,7 +209,7 @@ static int radix_sort_bytes(uint64_t n_pairs, uint64_t* keys, uint32_t* vals, ui
     uint32_t* tv = vin; vin = vout; vout = tv;
   }
   if (kin != keys) {
-    copy_pairs<<<sm_count() * 8, 256, 0, s>>>(kin, vin, keys, vals, n_pairs);
+    copy_pairs<<<ctx->sms * 8, 256, 0, s>>>(kin, vin, keys, vals, n_pairs);
     UTS_LAUNCH_CHECK();
   }
   return UTS_OK;

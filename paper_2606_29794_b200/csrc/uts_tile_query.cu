@@ -21,7 +21,6 @@
 #include "uts_internal.cuh"
 #include "uts_scan.cuh"
 #include "uts_ring_query.cuh"
-#include <cstdlib>
 #include <cstring>
 
 namespace uts {
@@ -851,24 +850,9 @@ int radius_bucket_host(float R32) {                    // host replica of radius
   const int b = (int)(t >> 21) - (int)(u >> 21);
   return b < 0 ? 0 : (b > kBuckets - 1 ? kBuckets - 1 : b);
 }
-// The three shapes of the ring path are independent: they run side by side on two library-private streams that are forked from
-// and joined back to the caller's stream with events, so the caller still sees one ordered stream.
-struct ForkJoin {
-  cudaStream_t aux[2] = {nullptr, nullptr};
-  cudaEvent_t fork = nullptr, join[2] = {nullptr, nullptr};
-  bool ok = false;
-  bool init() {
-    if (ok) return true;
-    for (int i = 0; i < 2; ++i) {
-      if (cudaStreamCreateWithFlags(&aux[i], cudaStreamNonBlocking) != cudaSuccess) return false;
-      if (cudaEventCreateWithFlags(&join[i], cudaEventDisableTiming) != cudaSuccess) return false;
-    }
-    if (cudaEventCreateWithFlags(&fork, cudaEventDisableTiming) != cudaSuccess) return false;
-    ok = true;
-    return true;
-  }
-};
-ForkJoin g_fj;
+// The three shapes of the ring path are independent: they run side by side on the device context's two auxiliary streams, forked
+// from and joined back to the caller's stream with events, so the caller still sees one ordered stream.  ctx->mu is held from
+// the fork to the join (QueryRun::count / emit), so two callers never interleave their records of the shared events.
 constexpr int kRingThreadRings = 24, kRingWarpRings = 128, kRingBlockRingsMax = 24575;   // ring-table capacities (8 B per ring)
 
 struct QueryLayout { size_t counts, list, perm, nlarge, active, scan, tcache, bcache, bcache_bytes, total; uint32_t bcache_cap; };
@@ -945,9 +929,14 @@ struct QueryRun {
   unsigned agrid, wgrid, bgrid, agrid_e, wgrid_e, bgrid_e;
   static constexpr int kBatchA = 128, kBatchB = 32;          // discs per batch: rc_thread class, rc_warp class
   int b_mat; uint32_t cap_rows;                              // matrix class of uts_tile_lists (b_mat < 0: none)
+  DeviceCtx* ctx;
+  enum { kOccBlock0 = 1, kOccBlock1, kOccB0, kOccB1, kOccA0, kOccA1, kOccMat };
 
-  int setup(const uts_config* cfg_, uts_proj in_, uts_mask mask_, const uint32_t* emit_rank_, void* scratch, cudaStream_t s_) {
+  int setup(const uts_config* cfg_, uts_proj in_, uts_mask mask_, const uint32_t* emit_rank_, void* scratch, const uts_tuning* tuning, cudaStream_t s_) {
     cfg = cfg_; in = in_; mask = mask_; emit_rank = emit_rank_; s = s_;
+    ctx = device_ctx();
+    if (!ctx) return UTS_ERR_CUDA;
+    const uts_tuning tn = tuning ? *tuning : uts_tuning{0, 0.f, 0, 0, 0.f};
     d = dims_of(cfg, &mask);
     n = (int64_t)d.P * d.V;
     b_mat = -1; cap_rows = 0;
@@ -956,10 +945,9 @@ struct QueryRun {
     qp.rho_q = cfg->query_mode == UTS_QUERY_RING ? 0.0 : rm[d.kq];      // Alg.3's set has no PixRad margin
     for (int o = 0; o <= kMaxOrder; ++o) { qp.rho[o] = (float)rm[o]; qp.sin_hrho[o] = (float)sin(0.5 * rm[o]); qp.cos_hrho[o] = (float)cos(0.5 * rm[o]); }
     // Implementation choice: the ring-interval path (uts_ring_query.cuh) whenever a block's ring table fits shared memory
-    // (k_q <= 12); the quadtree descent below otherwise, or when UTS_QUERY_IMPL=tree asks for it (A/B measurements).
-    const char* impl_env = getenv("UTS_QUERY_IMPL");
+    // (k_q <= 12); the quadtree descent (Alg.2's depth-first form) otherwise, or when uts_tuning.query_impl = 1 asks for it.
     const int Nq = 1 << d.kq;
-    ring_impl = 4 * Nq - 1 <= kRingBlockRingsMax && !(impl_env && strcmp(impl_env, "tree") == 0);
+    ring_impl = 4 * Nq - 1 <= kRingBlockRingsMax && tn.query_impl != 1;
     qp.rc_thread = kRingThreadRings; qp.rc_warp = 4 * Nq - 1 < kRingWarpRings ? 4 * Nq - 1 : kRingWarpRings; qp.rc_block = 4 * Nq - 1;
     // a disc of radius R reaches at most 3 R N + 4 rings (ring spacing >= 2/(3N) in colatitude, +-1 ring of padding at each end)
     qp.b_warp = radius_bucket_host((float)((qp.rc_thread - 6) / (3.0 * Nq)));
@@ -972,8 +960,7 @@ struct QueryRun {
     const size_t large_smem = (2 * (size_t)(d.n_tile / 32) + 2 * (size_t)qp.wl_cap) * 4;
     use_large = !ring_impl && d.kt >= 2 && large_smem <= kMaxLargeSmem;
     qp.n_words = use_large ? (int)(d.n_tile / 32) : 0;
-    const char* e1__ = getenv("UTS_RLARGE"); const char* e2__ = getenv("UTS_LGRID");
-    qp.r_large = (float)((e1__ ? atof(e1__) : 36.0) / sqrt((double)d.n_tile));      // ~320 tiles (pi R^2 / (4 pi / n_tile)); measured crossover on config 4
+    qp.r_large = (float)((tn.descent_block_radius > 0.f ? (double)tn.descent_block_radius : 36.0) / sqrt((double)d.n_tile));      // ~320 tiles (pi R^2 / (4 pi / n_tile)); measured crossover on config 4
 
     const QueryLayout L = query_layout(cfg);
     char* sp = reinterpret_cast<char*>(scratch);
@@ -995,51 +982,54 @@ struct QueryRun {
     qp.mask_base = list;
     active_arg = nullptr;
     qgrid = (unsigned)((n + kLargeThreads - 1) / kLargeThreads);
-    lgrid = use_large ? sm_count() * (e2__ ? atoi(e2__) : 2) : 0;
+    lgrid = use_large ? ctx->sms * (tn.descent_blocks_per_sm > 0 ? tn.descent_blocks_per_sm : 2) : 0;
     dyn_smem = use_large ? large_smem : 0;
     smem_a = sizeof(BatchRec) * kBatchA + (size_t)kBatchA * qp.rc_thread * sizeof(int2);
     smem_b = sizeof(BatchRec) * kBatchB + (size_t)kBatchB * qp.rc_warp * sizeof(int2);
     smem_block = (size_t)qp.rc_block * sizeof(int2);
     agrid = wgrid = bgrid = agrid_e = wgrid_e = bgrid_e = 0;     // persistent grids: exactly the resident blocks
-    if (use_large) {
-      static bool attr_set = false;
-      if (!attr_set) {
-        UTS_CUDA(cudaFuncSetAttribute(tile_query_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxLargeSmem));
-        UTS_CUDA(cudaFuncSetAttribute(tile_query_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxLargeSmem));
-        attr_set = true;
-      }
+    std::lock_guard<std::recursive_mutex> lock(ctx->mu);
+    if (!ctx->attrs_set[0]) {                                    // once per device
+      UTS_CUDA(cudaFuncSetAttribute(tile_query_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxLargeSmem));
+      UTS_CUDA(cudaFuncSetAttribute(tile_query_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxLargeSmem));
+      UTS_CUDA(cudaFuncSetAttribute(ring_query_block_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kRingBlockRingsMax * 8 + 8));
+      UTS_CUDA(cudaFuncSetAttribute(ring_query_block_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kRingBlockRingsMax * 8 + 8));
+      UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchA, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+      UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchA, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+      UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+      UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+      UTS_CUDA(cudaFuncSetAttribute(matrix_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024));
+      ctx->attrs_set[0] = true;
     }
-    if (ring_impl) {
-      static bool ring_attr_set = false;
-      if (!ring_attr_set) {
-        UTS_CUDA(cudaFuncSetAttribute(ring_query_block_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kRingBlockRingsMax * 8 + 8));
-        UTS_CUDA(cudaFuncSetAttribute(ring_query_block_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kRingBlockRingsMax * 8 + 8));
-        UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchA, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
-        UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchA, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
-        UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
-        UTS_CUDA(cudaFuncSetAttribute(ring_query_batch_kernel<kBatchB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
-        UTS_CUDA(cudaFuncSetAttribute(matrix_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024));
-        ring_attr_set = true;
-      }
-      int occ[6] = {1, 1, 1, 1, 1, 1};
-      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[0], ring_query_block_kernel<false>, kLargeThreads, smem_block));
-      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[1], ring_query_block_kernel<true>, kLargeThreads, smem_block));
-      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[2], ring_query_batch_kernel<kBatchB, false>, kLargeThreads, smem_b));
-      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[3], ring_query_batch_kernel<kBatchB, true>, kLargeThreads, smem_b));
-      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[4], ring_query_batch_kernel<kBatchA, false>, kLargeThreads, smem_a));
-      UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[5], ring_query_batch_kernel<kBatchA, true>, kLargeThreads, smem_a));
-      const unsigned sms = (unsigned)sm_count();
-      bgrid = sms * (unsigned)(occ[0] > 0 ? occ[0] : 1); bgrid_e = sms * (unsigned)(occ[1] > 0 ? occ[1] : 1);
-      wgrid = sms * (unsigned)(occ[2] > 0 ? occ[2] : 1); wgrid_e = sms * (unsigned)(occ[3] > 0 ? occ[3] : 1);
-      agrid = sms * (unsigned)(occ[4] > 0 ? occ[4] : 1); agrid_e = sms * (unsigned)(occ[5] > 0 ? occ[5] : 1);
-      if (!g_fj.init()) { set_last_cuda_error(cudaGetLastError()); return UTS_ERR_CUDA; }
+    if (ring_impl) {                                             // occupancy numbers are cached per (kernel, shared-memory size)
+      const unsigned sms = (unsigned)ctx->sms;
+      bgrid = sms * (unsigned)cached_occupancy(ctx, kOccBlock0, ring_query_block_kernel<false>, kLargeThreads, smem_block);
+      bgrid_e = sms * (unsigned)cached_occupancy(ctx, kOccBlock1, ring_query_block_kernel<true>, kLargeThreads, smem_block);
+      wgrid = sms * (unsigned)cached_occupancy(ctx, kOccB0, ring_query_batch_kernel<kBatchB, false>, kLargeThreads, smem_b);
+      wgrid_e = sms * (unsigned)cached_occupancy(ctx, kOccB1, ring_query_batch_kernel<kBatchB, true>, kLargeThreads, smem_b);
+      agrid = sms * (unsigned)cached_occupancy(ctx, kOccA0, ring_query_batch_kernel<kBatchA, false>, kLargeThreads, smem_a);
+      agrid_e = sms * (unsigned)cached_occupancy(ctx, kOccA1, ring_query_batch_kernel<kBatchA, true>, kLargeThreads, smem_a);
     }
     return UTS_OK;
   }
 
   // classification + count pass + exclusive scan of the per-slot counts into offsets[n + 1].  mp != nullptr: the discs of the
   // matrix class write bitmap rows instead (and count 0).  Enqueues only.
+  // the aux streams wait for everything queued on s so far
+  int fork() {
+    UTS_CUDA(cudaEventRecord(ctx->fork, s));
+    UTS_CUDA(cudaStreamWaitEvent(ctx->aux[0], ctx->fork, 0));
+    UTS_CUDA(cudaStreamWaitEvent(ctx->aux[1], ctx->fork, 0));
+    return UTS_OK;
+  }
+  // s waits for the aux streams; called on every exit path after fork() so that no work is left unjoined
+  int join() {
+    for (int i = 0; i < 2; ++i) { UTS_CUDA(cudaEventRecord(ctx->join[i], ctx->aux[i])); UTS_CUDA(cudaStreamWaitEvent(s, ctx->join[i], 0)); }
+    return UTS_OK;
+  }
+
   int count(uint64_t* offsets, MatParams* mp, uint32_t* flag_by_rank, uint64_t* rank_scan, uint64_t* rank_scan_sums) {
+    std::lock_guard<std::recursive_mutex> lock(ctx->mu);
     if (use_large && mask.slot_of_tile) {
       active_words_kernel<<<(qp.n_words + 255) / 256, 256, 0, s>>>(mask.slot_of_tile, qp.n_words, active);
       UTS_LAUNCH_CHECK();
@@ -1057,7 +1047,7 @@ struct QueryRun {
       if (mp) {                                       // rows of the bit matrix: rank order of the matrix-class discs
         UTS_CUDA(cudaMemsetAsync(flag_by_rank, 0, (size_t)n * 4, s));
         UTS_CUDA(cudaMemsetAsync(mp->n_L, 0, 8, s));
-        mat_flag_kernel<<<sm_count() * 4, 256, 0, s>>>(perm, n_small, emit_rank, flag_by_rank);
+        mat_flag_kernel<<<ctx->sms * 4, 256, 0, s>>>(perm, n_small, emit_rank, flag_by_rank);
         UTS_LAUNCH_CHECK();
         int st = exclusive_scan_u32(flag_by_rank, n, rank_scan, rank_scan_sums, s);
         if (st) return st;
@@ -1068,27 +1058,30 @@ struct QueryRun {
           UTS_LAUNCH_CHECK();
         }
       }
-      UTS_CUDA(cudaEventRecord(g_fj.fork, s));
-      UTS_CUDA(cudaStreamWaitEvent(g_fj.aux[0], g_fj.fork, 0));
-      UTS_CUDA(cudaStreamWaitEvent(g_fj.aux[1], g_fj.fork, 0));
-      ring_query_block_kernel<false><<<bgrid, kLargeThreads, smem_block, s>>>(qp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small, emit_rank,
-                                                                            counts, nullptr, nullptr, nullptr);
-      UTS_LAUNCH_CHECK();
-      if (mp) {
-        const size_t smem_m = smem_block + (size_t)mp->n_words * 4;
-        int occ = 1;
-        UTS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, matrix_count_kernel, kMatThreads, smem_m));
-        matrix_count_kernel<<<(unsigned)sm_count() * (unsigned)(occ > 0 ? occ : 1), kMatThreads, smem_m, s>>>(
-            qp, *mp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, mask.slot_of_tile ? active : nullptr, perm, n_small, emit_rank, counts);
+      int st = fork();
+      if (st) return st;
+      st = [&]() -> int {
+        ring_query_block_kernel<false><<<bgrid, kLargeThreads, smem_block, s>>>(qp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small, emit_rank,
+                                                                              counts, nullptr, nullptr, nullptr);
         UTS_LAUNCH_CHECK();
-      }
-      ring_query_batch_kernel<kBatchB, false><<<wgrid, kLargeThreads, smem_b, g_fj.aux[0]>>>(qp, 0, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
-                                                                                 emit_rank, counts, nullptr, nullptr, nullptr);
-      UTS_LAUNCH_CHECK();
-      ring_query_batch_kernel<kBatchA, false><<<agrid, kLargeThreads, smem_a, g_fj.aux[1]>>>(qp, 1, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
-                                                                                 emit_rank, counts, nullptr, nullptr, nullptr);
-      UTS_LAUNCH_CHECK();
-      for (int i = 0; i < 2; ++i) { UTS_CUDA(cudaEventRecord(g_fj.join[i], g_fj.aux[i])); UTS_CUDA(cudaStreamWaitEvent(s, g_fj.join[i], 0)); }
+        if (mp) {
+          const size_t smem_m = smem_block + (size_t)mp->n_words * 4;
+          const int occ = cached_occupancy(ctx, kOccMat, matrix_count_kernel, kMatThreads, smem_m);
+          matrix_count_kernel<<<(unsigned)ctx->sms * (unsigned)occ, kMatThreads, smem_m, s>>>(
+              qp, *mp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, mask.slot_of_tile ? active : nullptr, perm, n_small, emit_rank, counts);
+          UTS_LAUNCH_CHECK();
+        }
+        ring_query_batch_kernel<kBatchB, false><<<wgrid, kLargeThreads, smem_b, ctx->aux[0]>>>(qp, 0, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
+                                                                                   emit_rank, counts, nullptr, nullptr, nullptr);
+        UTS_LAUNCH_CHECK();
+        ring_query_batch_kernel<kBatchA, false><<<agrid, kLargeThreads, smem_a, ctx->aux[1]>>>(qp, 1, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
+                                                                                   emit_rank, counts, nullptr, nullptr, nullptr);
+        UTS_LAUNCH_CHECK();
+        return UTS_OK;
+      }();
+      const int stj = join();
+      if (st) return st;
+      if (stj) return stj;
     } else {
       tile_query_kernel<false><<<qgrid + lgrid, kLargeThreads, dyn_smem, s>>>(qp, lgrid, in.dir, in.rho, in.rs, mask.slot_of_tile, active_arg, perm,
                                                                              n_small, list, n_large, emit_rank, counts, nullptr, nullptr, nullptr);
@@ -1100,20 +1093,23 @@ struct QueryRun {
   // emit pass: the pairs of every slot at keys/vals[offsets[slot] ...).  Enqueues only.
   int emit(const uint64_t* offsets, uint64_t* keys, uint32_t* vals) {
     if (ring_impl) {
-      UTS_CUDA(cudaEventRecord(g_fj.fork, s));
-      UTS_CUDA(cudaStreamWaitEvent(g_fj.aux[0], g_fj.fork, 0));
-      UTS_CUDA(cudaStreamWaitEvent(g_fj.aux[1], g_fj.fork, 0));
-      ring_query_block_kernel<true><<<bgrid_e, kLargeThreads, smem_block, s>>>(qp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small, emit_rank,
-                                                                           nullptr, offsets, keys, vals);
-      UTS_LAUNCH_CHECK();
-      ring_query_batch_kernel<kBatchB, true><<<wgrid_e, kLargeThreads, smem_b, g_fj.aux[0]>>>(qp, 0, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
-                                                                                emit_rank, nullptr, offsets, keys, vals);
-      UTS_LAUNCH_CHECK();
-      ring_query_batch_kernel<kBatchA, true><<<agrid_e, kLargeThreads, smem_a, g_fj.aux[1]>>>(qp, 1, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
-                                                                                emit_rank, nullptr, offsets, keys, vals);
-      UTS_LAUNCH_CHECK();
-      for (int i = 0; i < 2; ++i) { UTS_CUDA(cudaEventRecord(g_fj.join[i], g_fj.aux[i])); UTS_CUDA(cudaStreamWaitEvent(s, g_fj.join[i], 0)); }
-      return UTS_OK;
+      std::lock_guard<std::recursive_mutex> lock(ctx->mu);
+      int st = fork();
+      if (st) return st;
+      st = [&]() -> int {
+        ring_query_block_kernel<true><<<bgrid_e, kLargeThreads, smem_block, s>>>(qp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small, emit_rank,
+                                                                             nullptr, offsets, keys, vals);
+        UTS_LAUNCH_CHECK();
+        ring_query_batch_kernel<kBatchB, true><<<wgrid_e, kLargeThreads, smem_b, ctx->aux[0]>>>(qp, 0, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
+                                                                                  emit_rank, nullptr, offsets, keys, vals);
+        UTS_LAUNCH_CHECK();
+        ring_query_batch_kernel<kBatchA, true><<<agrid_e, kLargeThreads, smem_a, ctx->aux[1]>>>(qp, 1, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
+                                                                                  emit_rank, nullptr, offsets, keys, vals);
+        UTS_LAUNCH_CHECK();
+        return UTS_OK;
+      }();
+      const int stj = join();
+      return st ? st : stj;
     }
     tile_query_kernel<true><<<qgrid + lgrid, kLargeThreads, dyn_smem, s>>>(qp, lgrid, in.dir, in.rho, in.rs, mask.slot_of_tile, active_arg, perm,
                                                                           n_small, list, n_large, emit_rank, nullptr, offsets, keys, vals);
@@ -1131,7 +1127,8 @@ size_t uts_tile_query_scratch_bytes(const uts_config* cfg) {
 }
 
 int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint32_t* emit_rank, uint64_t* offsets, uint64_t* keys,
-                   uint32_t* vals, uint64_t capacity, uint64_t* h_n_pairs, void* scratch, size_t scratch_bytes, void* stream) {
+                   uint32_t* vals, uint64_t capacity, uint64_t* h_n_pairs, void* scratch, size_t scratch_bytes, const uts_tuning* tuning,
+                   void* stream) {
   int st = check_config(cfg);
   if (st) return st;
   if ((st = check_mask(cfg, mask))) return st;
@@ -1148,7 +1145,7 @@ int uts_tile_query(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   if (keys && !vals) return UTS_ERR_INVALID_ARG;
   if (scratch_bytes < uts_tile_query_scratch_bytes(cfg) || ((uintptr_t)scratch & 255)) return UTS_ERR_INVALID_ARG;
   QueryRun q;
-  if ((st = q.setup(cfg, in, mask, emit_rank, scratch, s))) return st;
+  if ((st = q.setup(cfg, in, mask, emit_rank, scratch, tuning, s))) return st;
   if ((st = q.count(offsets, nullptr, nullptr, nullptr, nullptr))) return st;
   UTS_CUDA(cudaMemcpyAsync(h_n_pairs, offsets + n, sizeof(uint64_t), cudaMemcpyDeviceToHost, s));
   UTS_CUDA(cudaStreamSynchronize(s));
@@ -1165,7 +1162,7 @@ size_t uts_tile_lists_scratch_bytes(const uts_config* cfg) {
 
 int uts_tile_lists(const uts_config* cfg, uts_proj in, uts_mask mask, const uint32_t* emit_rank, uint64_t* keys, uint32_t* vals,
                    uint64_t* keys_tmp, uint32_t* vals_tmp, uint64_t capacity, uint64_t* ranges, uint64_t* h_n_pairs, void* scratch,
-                   size_t scratch_bytes, void* sort_scratch, size_t sort_scratch_bytes, void* stream) {
+                   size_t scratch_bytes, void* sort_scratch, size_t sort_scratch_bytes, const uts_tuning* tuning, void* stream) {
   int st = check_config(cfg);
   if (st) return st;
   if ((st = check_mask(cfg, mask))) return st;
@@ -1187,7 +1184,7 @@ int uts_tile_lists(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   char* sp = reinterpret_cast<char*>(scratch);
   uint64_t* offsets = reinterpret_cast<uint64_t*>(sp + ML.offsets);
   QueryRun q;
-  if ((st = q.setup(cfg, in, mask, emit_rank, scratch, s))) return st;
+  if ((st = q.setup(cfg, in, mask, emit_rank, scratch, tuning, s))) return st;
   MatParams mp;
   mp.M = reinterpret_cast<uint32_t*>(sp + ML.M); mp.MT = reinterpret_cast<uint32_t*>(sp + ML.MT);
   mp.row_key = reinterpret_cast<unsigned long long*>(sp + ML.row_key);
@@ -1200,10 +1197,9 @@ int uts_tile_lists(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   // that a bitmap row (about 5 passes over n_tile / 8 bytes) is cheaper than the disc's pairs through emit + radix sort + ranges
   // (about 90 B per pair): tiles >= n_tile / 144.
   const size_t smem_m = q.smem_block + (size_t)mp.n_words * 4;
-  const bool mat_ok = q.ring_impl && d.kt >= 2 && smem_m <= 220 * 1024 && ML.cap_rows > 0 && !getenv("UTS_NO_MATRIX");
+  const bool mat_ok = q.ring_impl && d.kt >= 2 && smem_m <= 220 * 1024 && ML.cap_rows > 0 && !(tuning && tuning->matrix_off);
   if (mat_ok) {
-    const char* e = getenv("UTS_MAT_TILES");
-    const double tiles_min = e ? atof(e) : fmax(48.0, (double)d.n_tile / 144.0);
+    const double tiles_min = (tuning && tuning->matrix_min_tiles > 0.f) ? (double)tuning->matrix_min_tiles : fmax(48.0, (double)d.n_tile / 144.0);
     const double cosR = 1.0 - 2.0 * tiles_min / (double)d.n_tile;           // cap of tiles_min tiles: n_tile (1 - cos R) / 2
     q.b_mat = cosR <= -1.0 ? -1 : radius_bucket_host((float)acos(cosR));
     if (q.b_mat > q.qp.b_block) q.b_mat = q.qp.b_block;                     // only discs of the block-per-disc class

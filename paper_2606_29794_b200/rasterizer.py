@@ -18,11 +18,12 @@ class Rasterizer:
     synchronisation is the pair count returned by uts_tile_query."""
 
     def __init__(self, cfg: B.Config, mask: B.Mask | None = None, device="cuda", pair_capacity: int = 0, depth_presort: bool = True,
-                 fused_lists: bool = True, marks: bool = True):
+                 fused_lists: bool = True, marks: bool = True, tuning: B.Tuning | None = None):
         B.lib()
         if not torch.cuda.is_available():
             raise RuntimeError("uts: a CUDA device is required (no CPU fallback)")
         self.cfg, self.mask, self.dev = cfg, (mask or B.Mask.full()), device
+        self.tuning = tuning                # uts_tuning for the tile query (tests, A/B runs); None = the library's defaults
         V, P = cfg.n_views, cfg.n_gauss
         self.S = self.mask.n_slots(cfg)
         npx = self.S * cfg.ppt
@@ -65,19 +66,19 @@ class Rasterizer:
     def tile_query(self):
         try:
             self.n_pairs = B.uts_tile_query(self.cfg, self.proj, self.mask, self.offsets, self.keys, self.vals, self.capacity, self.tq_scratch,
-                                            self.emit_rank)
+                                            self.emit_rank, self.tuning)
         except B.UtsError as e:
             if e.status != B.UTS_ERR_CAPACITY:
                 raise
             self._alloc_pairs(int(e.needed * 1.05) + 1024)
             self.n_pairs = B.uts_tile_query(self.cfg, self.proj, self.mask, self.offsets, self.keys, self.vals, self.capacity, self.tq_scratch,
-                                            self.emit_rank)
+                                            self.emit_rank, self.tuning)
         return self.n_pairs
 
     def tile_lists(self):
         """uts_tile_lists: sorted keys / vals and ranges in one call (needs the depth order)."""
         args = lambda: (self.cfg, self.proj, self.mask, self.emit_rank, self.keys, self.vals, self.keys_tmp, self.vals_tmp, self.capacity, self.ranges,
-                        self.tq_scratch, self.sort_scratch)
+                        self.tq_scratch, self.sort_scratch, self.tuning)
         try:
             self.n_pairs = B.uts_tile_lists(*args())
         except B.UtsError as e:

@@ -69,11 +69,21 @@ def _sigmoid(x):
     return 1.0 / (1.0 + np.exp(-x))
 
 
+def _random_rotation(rng):
+    """A rotation matrix drawn uniformly (QR of a Gaussian matrix, signs fixed, determinant +1): an input draw, no method arithmetic."""
+    q, r = np.linalg.qr(rng.standard_normal((3, 3)))
+    q = q * np.sign(np.diag(r))[None, :]
+    if np.linalg.det(q) < 0:
+        q[:, 0] = -q[:, 0]
+    return q
+
+
 def make_scene(cfg_id: int, seed: int = 0, n_gauss: int | None = None, order: int | None = None,
-               sh_degree: int | None = None, n_views: int | None = None) -> dict:
+               sh_degree: int | None = None, n_views: int | None = None, general_view: bool = False) -> dict:
     """Returns float32 arrays means[P,3] scales[P,3] quats[P,4] opac[P] sh[P,M,3] W[V,9] b[V,3] plus
     order / sh_degree / n_views / mask descriptor.  n_gauss / order / sh_degree / n_views shrink a config for tests
-    (same distributions)."""
+    (same distributions).  general_view: every view gets its own random rotation W (tilted about all three axes) and a
+    translation b ~ N(0, 0.4) (camera off the origin) instead of the configs' W = I / rotation about y, b = 0."""
     base = CONFIGS[cfg_id]
     P = int(n_gauss if n_gauss is not None else base["n_gauss"])
     k = int(order if order is not None else base["order"])
@@ -120,6 +130,11 @@ def make_scene(cfg_id: int, seed: int = 0, n_gauss: int | None = None, order: in
         th = math.radians(6.0 * v) if cfg_id == 5 else 0.0                  # rotation about camera y
         c, s = math.cos(th), math.sin(th)
         W[v] = [c, 0, s, 0, 1, 0, -s, 0, c]
+    if general_view:
+        r_view = _rng(seed, cfg_id, 8)
+        for v in range(V):
+            W[v] = _random_rotation(r_view).reshape(-1)
+            b[v] = r_view.normal(0.0, 0.4, 3)
 
     mask = None
     if base["mask"] == "cap":

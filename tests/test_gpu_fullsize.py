@@ -1,5 +1,5 @@
-"""Full-size parity (BASELINE.json config 4 = the bench workload, and config 5 = mask + 4 views), in the launch configuration
-bench.py times.  The oracle cannot run a whole frame in seconds, so: (1) properties that hold at any size are checked on the
+"""Full-size parity for the BASELINE.json configs (config 2 whole frame; config 3 = cap mask, config 4 = the bench workload and
+config 5 = frustum mask + 4 views on sampled tiles), in the launch configuration bench.py times.  The oracle cannot run a whole frame in seconds, so: (1) properties that hold at any size are checked on the
 whole output on the device; (2) a random sample of tiles is rendered by the oracle from its OWN complete lists and compared
 element by element (list contents bit-exact, colour/alpha 1e-4, n_last); (3) the backward is run with an upstream gradient
 that is zero outside the sampled tiles, which the oracle can then reproduce exactly from the sample (1e-3)."""
@@ -27,7 +27,40 @@ def _rel(got, want):
     return np.abs(got.astype(np.float64) - want).max() / max(np.abs(want).max(), 1e-30)
 
 
-@pytest.mark.parametrize("cfg_id,n_sample", [(4, 16), (5, 16)], ids=["config4-large-sphere", "config5-frustum-4views"])
+def test_config2_whole_frame_against_the_oracle():
+    """BASELINE.json config 2 (Nside 256, 100k Gaussians, SH3) is small enough for the oracle to run WHOLE (about 25 s on one core):
+    every pair, every pixel and every gradient entry of the full-size frame is compared."""
+    B, R = _gpu()
+    scene = scenes.make_scene(2, seed=0)
+    cfg = R.config_of(scene)
+    oc = ocfg(scene)
+    fw = orc.forward_chain(oc, scene)
+    assert fw["qinfo"]["min_margin"] > 1e-12
+    g, views = R.scene_to_device(scene)
+    r = R.Rasterizer(cfg)
+    r.forward(g, views)
+    n = r.n_pairs
+    assert n == fw["skeys"].shape[0]
+    assert np.array_equal(r.keys[:n].cpu().numpy().view(np.uint64), fw["skeys"])
+    assert np.array_equal(r.vals[:n].cpu().numpy().view(np.uint32), fw["svals"])
+    assert np.array_equal(r.ranges.cpu().numpy().view(np.uint64), fw["ranges"])
+    safe = fw["margin"] > MARGIN
+    assert safe.mean() > 0.98
+    col, al = r.color.cpu().numpy(), r.alpha.cpu().numpy()
+    assert np.abs(col - fw["color"]).max(axis=-1)[safe].max() <= 1e-4 and np.abs(al - fw["alpha"])[safe].max() <= 1e-4
+    assert np.array_equal(r.n_last.cpu().numpy().view(np.uint32)[safe], fw["n_last"][safe])
+    assert np.abs(col - fw["color"]).max() < 2e-2
+    gcol = scenes.upstream_grad(1, col.shape[1], seed=12)
+    gcol[~safe] = 0                                                             # decisions within MARGIN of a threshold: excluded on both sides
+    G = r.backward(g, views, torch.from_numpy(gcol).cuda())
+    w_rgb, w_conic, w_mu2, w_opac = orc.render_bwd(oc, fw["proj"], fw["ranges"], fw["svals"], fw["n_last"], gcol)
+    w = orc.preprocess_bwd(oc, scene["means"], scene["scales"], scene["quats"], scene["sh"], scene["W"], scene["b"], w_rgb, w_conic, w_mu2)
+    for name, want in zip(("means", "scales", "quats", "sh"), w):
+        assert _rel(G[name].cpu().numpy(), want) <= 1e-3, name
+    assert _rel(G["opac"].cpu().numpy(), w_opac) <= 1e-3
+
+
+@pytest.mark.parametrize("cfg_id,n_sample", [(3, 32), (4, 16), (5, 16)], ids=["config3-fisheye-cap", "config4-large-sphere", "config5-frustum-4views"])
 def test_full_size_properties_and_sampled_tiles(cfg_id, n_sample):
     B, R = _gpu()
     scene = scenes.make_scene(cfg_id, seed=0)

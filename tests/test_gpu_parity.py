@@ -45,6 +45,11 @@ CASES = [
     pytest.param(4, 3000, 7, {}, id="cfg4-large-outliers"),
     pytest.param(5, 8000, 8, {"n_views": 2}, id="cfg5-frustum-2views"),
     pytest.param(4, 30000, 5, {}, id="cfg4-dense-long-lists-early-exit"),     # lists up to ~1500 entries (6 batches), 40 % of pixels saturate
+    # general views [W|b]: random tilted rotations and b != 0, so cam = -W^T b, the SH view direction from an off-origin
+    # camera, M = W Sigma W^T for a tilted W and W^T dL/dt in the backward are all exercised
+    pytest.param(2, 12000, 7, {"general_view": True}, id="cfg2-sh3-general-view"),
+    pytest.param(5, 8000, 8, {"n_views": 3, "general_view": True}, id="cfg5-frustum-3-general-views"),
+    pytest.param(4, 3000, 7, {"general_view": True, "sh_degree": 2}, id="cfg4-sh2-general-view"),
 ]
 
 
@@ -103,13 +108,12 @@ def test_mask_builder_matches_oracle_mask():
         bits, act, slot = oracle_mask(oc, scene)
         m = B.uts_build_mask(_cfg(R, scene), scene["mask"]["kind"], scene["mask"]["params"])
         gb = u32(m.pixel_mask_bits)
-        # the predicate is evaluated in double on both sides; allow a handful of boundary pixels to differ
-        diff = np.unpackbits((gb ^ bits).view(np.uint8)).sum()
-        assert diff <= 4
-        if diff == 0:
-            assert m.n_active == act.shape[0]
-            assert np.array_equal(u32(m.active_tiles), act)
-            assert np.array_equal(m.slot_of_tile.cpu().numpy(), slot)
+        # the predicate is evaluated in double on both sides from centres that agree to 5e-15 (test_pixel_centers_match_oracle), and
+        # no centre of these grids lies within 1e-12 of a mask boundary: the bitmaps, the tile list and the slot table are identical
+        assert np.array_equal(gb, bits)
+        assert m.n_active == act.shape[0]
+        assert np.array_equal(u32(m.active_tiles), act)
+        assert np.array_equal(m.slot_of_tile.cpu().numpy(), slot)
 
 
 # ------------------------------------------------------------------------------------------- F1
@@ -203,6 +207,66 @@ def test_tile_query_bit_exact(cfg_id, P, order, extra):
     gk, gv = canon_pairs(u64(offsets), u64(keys), u32(vals))
     assert np.array_equal(gk, c.fw["keys"])
     assert np.array_equal(gv, c.fw["vals"])
+
+
+@pytest.mark.parametrize("block_radius", [0.0, 6.0], ids=["default-split", "most-discs-on-the-block-path"])
+@pytest.mark.parametrize("cfg_id,P,order,extra", CASES)
+def test_tile_query_quadtree_descent_bit_exact(cfg_id, P, order, extra, block_radius):
+    """uts_tuning.query_impl = 1: the stackless quadtree descent — Alg.2's depth-first form, the library's path
+    for k_q = 13 — on every case, with the default thread / block split and with the split moved so that most discs take the
+    block-per-Gaussian bitmap path.  Count-only, capacity error, emit; with and without the depth-order emission ranks."""
+    B, R = _gpu()
+    c = Case.get(cfg_id, P, order, extra)
+    cfg = _cfg(R, c.scene)
+    proj, mask = c.gpu_proj(B), c.gpu_mask(B)
+    tn = B.Tuning(query_impl=1, descent_block_radius=block_radius)
+    n_want = int(c.fw["keys"].shape[0])
+    offsets = torch.empty(cfg.n_views * cfg.n_gauss + 1, dtype=torch.int64, device="cuda")
+    scratch = torch.empty(B.uts_tile_query_scratch_bytes(cfg) // 8 + 32, dtype=torch.int64, device="cuda")
+    assert B.uts_tile_query(cfg, proj, mask, offsets, None, None, 0, scratch, tuning=tn) == n_want
+    assert np.array_equal(u64(offsets), c.fw["offsets"])
+    keys = torch.empty(max(n_want, 1), dtype=torch.int64, device="cuda"); vals = torch.empty(max(n_want, 1), dtype=torch.int32, device="cuda")
+    if n_want > 1:
+        with pytest.raises(B.UtsError) as ei:
+            B.uts_tile_query(cfg, proj, mask, offsets, keys, vals, n_want - 1, scratch, tuning=tn)
+        assert ei.value.status == B.UTS_ERR_CAPACITY and ei.value.needed == n_want
+    B.uts_tile_query(cfg, proj, mask, offsets, keys, vals, n_want, scratch, tuning=tn)
+    gk, gv = canon_pairs(u64(offsets), u64(keys), u32(vals))
+    assert np.array_equal(gk, c.fw["keys"]) and np.array_equal(gv, c.fw["vals"])
+    # the whole staged chain on the descent, depth-presorted: sorted arrays and ranges
+    r = R.Rasterizer(cfg, mask, fused_lists=False, depth_presort=True, tuning=tn)
+    r.proj = proj
+    r.depth_order(); r.tile_query(); r.sort(); r.tile_ranges()
+    assert r.n_pairs == n_want
+    assert np.array_equal(u64(r.keys)[:n_want], c.fw["skeys"]) and np.array_equal(u32(r.vals)[:n_want], c.fw["svals"])
+    assert np.array_equal(u64(r.ranges), c.fw["ranges"])
+
+
+@pytest.mark.parametrize("mode,P,seed", [(0, 300, 0), (1, 120, 1)], ids=["nested", "ring-set"])
+def test_tile_query_order13_refine16_takes_the_descent(mode, P, seed):
+    """k = 13, f = 16: k_q = 13, where a block's ring table no longer fits shared memory and the library switches to the quadtree
+    descent by itself (no tuning).  A few hundred Gaussians incl. discs of tens of thousands of tiles, a polar one and a culled
+    one; the oracle's descent / Alg.3 scan is the reference (its brute force over 12 * 4^13 pixels per Gaussian is out of reach),
+    pinned at lower orders.  (seed: the one whose margin certificate holds.)"""
+    B, R = _gpu()
+    scene = small_scene(5, P, 13, n_views=1, seed=seed)
+    scene["mask"] = None
+    scene["scales"][::7] *= 8.0
+    scene["means"][3] = np.array([0.004, 2.5, -0.003]); scene["means"][5] *= 1e-3
+    oc = ocfg(scene, query_refine_log2=4, query_mode=mode)
+    pr = orc.preprocess(oc, scene["means"], scene["scales"], scene["quats"], scene["opac"], scene["sh"], scene["W"], scene["b"])
+    off, keys, vals, info = orc.tile_query(oc, pr)
+    assert info["min_margin"] > 1e-12 and keys.shape[0] > 3000
+    cfg = _cfg(R, scene, query_refine_log2=4, query_mode=mode)
+    proj = B.Proj(dev(pr.dir), dev(pr.lonlat), dev(pr.rho), dev(pr.conic_opac), dev(pr.rs), dev(pr.rgb), dev(pr.flags))
+    n = int(keys.shape[0])
+    offsets = torch.empty(cfg.n_gauss + 1, dtype=torch.int64, device="cuda")
+    scratch = torch.empty(B.uts_tile_query_scratch_bytes(cfg) // 8 + 32, dtype=torch.int64, device="cuda")
+    gkeys = torch.empty(n, dtype=torch.int64, device="cuda"); gvals = torch.empty(n, dtype=torch.int32, device="cuda")
+    assert B.uts_tile_query(cfg, proj, B.Mask.full(), offsets, gkeys, gvals, n, scratch) == n
+    assert np.array_equal(u64(offsets), off)
+    gk, gv = canon_pairs(u64(offsets), u64(gkeys), u32(gvals))
+    assert np.array_equal(gk, keys) and np.array_equal(gv, vals)
 
 
 @pytest.mark.parametrize("refine", [0, 1, 3, 4])
@@ -369,9 +433,9 @@ def test_sort_sizes_and_ties(n):
 
 
 # ------------------------------------------------------------------------------------------- F5 / F6
-def _render_gpu(B, R, c, cfg):
+def _render_gpu(B, R, c, cfg, marks=True):
     mask = c.gpu_mask(B)
-    r = R.Rasterizer(cfg, mask, pair_capacity=int(c.fw["svals"].shape[0]))      # the marks are sized by the capacity
+    r = R.Rasterizer(cfg, mask, pair_capacity=int(c.fw["svals"].shape[0]), marks=marks)      # the marks are sized by the capacity
     r.proj = c.gpu_proj(B)
     r.ranges = dev(c.fw["ranges"].view(np.int64))
     r.vals = dev(c.fw["svals"].view(np.int32))
@@ -392,11 +456,15 @@ def _compare_image(c, color, alpha, n_last):
     assert dc.max() < 2e-2 and da.max() < 2e-2
 
 
+MARKS = pytest.mark.parametrize("marks", [False, True], ids=["plain", "marked"])     # uts_render_fwd / _bwd and the marked pair
+
+
+@MARKS
 @pytest.mark.parametrize("cfg_id,P,order,extra", CASES)
-def test_render_fwd(cfg_id, P, order, extra):
+def test_render_fwd(cfg_id, P, order, extra, marks):
     B, R = _gpu()
     c = Case.get(cfg_id, P, order, extra)
-    r = _render_gpu(B, R, c, _cfg(R, c.scene))
+    r = _render_gpu(B, R, c, _cfg(R, c.scene), marks)
     color, alpha = r.color.cpu().numpy(), r.alpha.cpu().numpy()
     _compare_image(c, color, alpha, u32(r.n_last))
     assert np.allclose(r.trans.cpu().numpy() + alpha, 1.0, atol=1e-6)
@@ -441,12 +509,13 @@ def _zero_unsafe(c, gcol, galpha=None):
     return gcol, galpha
 
 
+@MARKS
 @pytest.mark.parametrize("cfg_id,P,order,extra", CASES)
-def test_backward(cfg_id, P, order, extra):
+def test_backward(cfg_id, P, order, extra, marks):
     B, R = _gpu()
     c = Case.get(cfg_id, P, order, extra)
     cfg = _cfg(R, c.scene)
-    r = _render_gpu(B, R, c, cfg)
+    r = _render_gpu(B, R, c, cfg, marks)
     V, npx = r.color.shape[0], r.color.shape[1]
     from paper_2606_29794_b200 import scenes
     gcol, galpha = _zero_unsafe(c, *scenes.upstream_grad(V, npx, seed=cfg_id, with_alpha=True))
@@ -470,23 +539,25 @@ def test_backward(cfg_id, P, order, extra):
         assert e <= 1e-3, (name, e)
 
 
-@pytest.mark.parametrize("cfg_id,P,order", [(1, 1000, 6), (2, 12000, 7), (4, 30000, 5)])
-def test_backward_thresholds_off_every_pixel(cfg_id, P, order):
+@pytest.mark.parametrize("cfg_id,P,order,extra,marks", [(1, 1000, 6, {}, True), (2, 12000, 7, {}, True), (4, 30000, 5, {}, True), (2, 12000, 7, {}, False),
+                                                        (2, 8000, 7, {"general_view": True}, True), (5, 6000, 7, {"general_view": True, "n_views": 2}, False)])
+def test_backward_thresholds_off_every_pixel(cfg_id, P, order, extra, marks):
     """alpha_min 0, alpha_max 1, eps 0: no decision exists, so every pixel takes part and the whole chain (forward on the GPU,
     backward on the GPU) must match the oracle's within 1e-3 on every gradient array."""
     B, R = _gpu()
-    scene = small_scene(cfg_id, P, order)
+    scene = small_scene(cfg_id, P, order, **extra)
+    scene["mask"] = None                               # full sphere: every pixel of every tile takes part
     kw = dict(alpha_min=0.0, alpha_max=1.0, t_eps=0.0, bg=(0.1, 0.2, 0.3))
     oc = ocfg(scene, **kw)
     fw = orc.forward_chain(oc, scene)
     cfg = _cfg(R, scene, **kw)
     g, views = R.scene_to_device(scene)
-    r = R.Rasterizer(cfg)
+    r = R.Rasterizer(cfg, marks=marks)
     r.forward(g, views)
     assert np.array_equal(u64(r.keys)[: r.n_pairs], fw["skeys"])
     assert np.abs(r.color.cpu().numpy() - fw["color"]).max() <= 1e-4
     from paper_2606_29794_b200 import scenes
-    gcol, galpha = scenes.upstream_grad(1, r.color.shape[1], seed=7, with_alpha=True)
+    gcol, galpha = scenes.upstream_grad(cfg.n_views, r.color.shape[1], seed=7, with_alpha=True)
     w_rgb, w_conic, w_mu2, w_opac = orc.render_bwd(oc, fw["proj"], fw["ranges"], fw["svals"], fw["n_last"], gcol, galpha)
     w_means, w_scales, w_quats, w_sh = orc.preprocess_bwd(oc, scene["means"], scene["scales"], scene["quats"], scene["sh"], scene["W"],
                                                           scene["b"], w_rgb, w_conic, w_mu2)
@@ -500,9 +571,18 @@ def test_backward_thresholds_off_every_pixel(cfg_id, P, order):
 
 
 # ------------------------------------------------------------------------------------------- whole chain
-@pytest.mark.parametrize("presort", [True, False], ids=["depth-presorted", "plain-sort"])
+# the three ways the ABI builds the sorted lists (include/uts.h), with the marked and the plain blend pair:
+#   fused            uts_depth_order -> uts_tile_lists                                              (the default), marked blend
+#   staged-presorted uts_depth_order -> uts_tile_query(emit_rank) -> uts_sort(depth_presorted = 1) -> uts_tile_ranges, plain blend
+#   staged-plain     uts_tile_query(emit_rank = NULL) -> uts_sort (all key bytes) -> uts_tile_ranges, marked blend
+PATHS = {"fused": dict(depth_presort=True, fused_lists=True, marks=True),
+         "staged-presorted": dict(depth_presort=True, fused_lists=False, marks=False),
+         "staged-plain": dict(depth_presort=False, fused_lists=False, marks=True)}
+
+
+@pytest.mark.parametrize("path", list(PATHS))
 @pytest.mark.parametrize("cfg_id,P,order,extra", CASES)
-def test_end_to_end_chain(cfg_id, P, order, extra, presort):
+def test_end_to_end_chain(cfg_id, P, order, extra, path):
     """All-GPU chain against the all-oracle chain: pair lists, sorted order and ranges bit-exact (the GPU preprocess
     rounds double results to fp32 once, as the oracle does), image within 1e-4, parameter gradients within 1e-3."""
     B, R = _gpu()
@@ -510,12 +590,12 @@ def test_end_to_end_chain(cfg_id, P, order, extra, presort):
     cfg = _cfg(R, c.scene)
     if c.scene["mask"] is not None:
         mask = B.uts_build_mask(cfg, c.scene["mask"]["kind"], c.scene["mask"]["params"])
-        if not np.array_equal(u32(mask.pixel_mask_bits), c.bits):
-            mask = c.gpu_mask(B)           # a boundary pixel differs: use the oracle's mask (the mask is an input of the path)
+        assert np.array_equal(u32(mask.pixel_mask_bits), c.bits)
     else:
         mask = B.Mask.full()
     g, views = R.scene_to_device(c.scene)
-    r = R.Rasterizer(cfg, mask, depth_presort=presort)
+    r = R.Rasterizer(cfg, mask, **PATHS[path])
+    assert r.fused_lists == PATHS[path]["fused_lists"] and r.use_marks == PATHS[path]["marks"]
     r.forward(g, views)
     n = r.n_pairs
     # fp32 records straddling a rounding boundary could flip a borderline tile; require exact equality and report if not
@@ -579,20 +659,17 @@ def test_invalid_arguments_are_reported():
 
 
 # ------------------------------------------------------------------------------------------- F2 + F3 + F4 fused
-@pytest.mark.parametrize("mat_tiles", [None, "3", "40"], ids=["default-threshold", "matrix-from-3-tiles", "matrix-from-40-tiles"])
+@pytest.mark.parametrize("mat_tiles", [None, 3.0, 40.0, "off"], ids=["default-threshold", "matrix-from-3-tiles", "matrix-from-40-tiles", "matrix-off"])
 @pytest.mark.parametrize("cfg_id,P,order,extra", CASES + [pytest.param(4, 3000, 8, {"n_views": 3}, id="cfg4-3views-order8"),
                                                           pytest.param(3, 4000, 6, {}, id="cfg3-cap-mask-order6")])
-def test_tile_lists_bit_exact(cfg_id, P, order, extra, mat_tiles, monkeypatch):
+def test_tile_lists_bit_exact(cfg_id, P, order, extra, mat_tiles):
     """uts_tile_lists (large discs through the bit matrix, small discs through emit + sort, per-tile merge) against the oracle's
     sorted pairs and ranges, bit for bit; the matrix threshold is moved so that few, most or nearly all discs take the matrix."""
     B, R = _gpu()
-    if mat_tiles is None:
-        monkeypatch.delenv("UTS_MAT_TILES", raising=False)
-    else:
-        monkeypatch.setenv("UTS_MAT_TILES", mat_tiles)
+    tuning = None if mat_tiles is None else (B.Tuning(matrix_off=1) if mat_tiles == "off" else B.Tuning(matrix_min_tiles=mat_tiles))
     c = Case.get(cfg_id, P, order, extra)
     cfg = _cfg(R, c.scene)
-    r = R.Rasterizer(cfg, c.gpu_mask(B), fused_lists=True, pair_capacity=16)          # tiny capacity: exercises UTS_ERR_CAPACITY + regrow
+    r = R.Rasterizer(cfg, c.gpu_mask(B), fused_lists=True, pair_capacity=16, tuning=tuning)   # tiny capacity: exercises UTS_ERR_CAPACITY + regrow
     r.proj = c.gpu_proj(B)
     r.depth_order()
     n = r.tile_lists()
@@ -602,10 +679,9 @@ def test_tile_lists_bit_exact(cfg_id, P, order, extra, mat_tiles, monkeypatch):
     assert np.array_equal(u64(r.ranges), c.fw["ranges"])
 
 
-def test_tile_lists_whole_sphere_discs_and_empty(monkeypatch):
+def test_tile_lists_whole_sphere_discs_and_empty():
     """Whole-sphere discs (reading A24) as matrix rows, with and without a mask; culled Gaussians; P = 0."""
     B, R = _gpu()
-    monkeypatch.setenv("UTS_MAT_TILES", "8")
     scene = small_scene(3, 600, 6)
     scene["scales"][:40] *= 400.0                                     # r_s = pi
     scene["means"][40:60] *= 1e-3                                     # inside r_near: culled
@@ -616,7 +692,7 @@ def test_tile_lists_whole_sphere_discs_and_empty(monkeypatch):
     cfg = _cfg(R, scene)
     mask = B.Mask(dev(act.view(np.int32)), int(act.shape[0]), dev(slot), dev(bits.view(np.int32)))
     g, views = R.scene_to_device(scene)
-    r = R.Rasterizer(cfg, mask, fused_lists=True)
+    r = R.Rasterizer(cfg, mask, fused_lists=True, tuning=B.Tuning(matrix_min_tiles=8.0))
     r.preprocess(g, views); r.depth_order()
     n = r.tile_lists()
     assert n == fw["skeys"].shape[0] and np.array_equal(u64(r.keys)[:n], fw["skeys"]) and np.array_equal(u32(r.vals)[:n], fw["svals"])

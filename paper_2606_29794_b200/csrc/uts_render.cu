@@ -2,17 +2,25 @@
 // (Alg.1 l.17-30 PAPER.md:563-587; Eq.6; SphericalOffset PAPER.md:112; mask PAPER.md:62, 129), and
 // B1: its backward.
 //
-// One thread block per active tile, one thread per pixel (thread id = p & 255, the NESTED low bits, so a warp is a
-// compact 8x4 pixel patch).  The tile's sorted list is staged through shared memory in batches of 256 entries.
+// One thread block of 256 / PX threads per active tile; every thread owns PX pixels (p & 255 = tid + (256 / PX) j, j < PX), so
+// that one staged list entry read from shared memory serves PX pixel evaluations and, in the backward, one warp reduction + one
+// set of atomics serves up to 32 PX pixels.  The 32 pixels (lane, j) of a warp form a compact 8x4 "patch" (thread id = NESTED low
+// bits); patches are what the early exit, the marks and the backward's visit list are kept for.  The tile's sorted list is
+// staged through shared memory in batches of 256 entries.
 //
-// SphericalOffset without inverse trigonometry in the common case, and without fp32 cancellation (DESIGN.md
-// "Kernels/F5"):  with Gaussian direction u and its east/north unit vectors e, n, and pixel direction w,
+// SphericalOffset without inverse trigonometry and without fp32 cancellation:  with Gaussian direction u
+// and its east/north unit vectors e, n, and pixel direction w,
 //     a = e.w, b = n.w, c = u.w,  sin(d_gc) = sqrt(a^2+b^2),  (d_x,d_y) = (d_gc / sin d_gc) (a,b)
 // is the haversine distance + bearing decomposition of PAPER.md:112 in vector form.  Because e.u = n.u = 0,
 // a = e.(w-u) and b = n.(w-u): the difference w-u = (c_tile - u) + (w - c_tile) is formed in double precision once per
 // (tile, Gaussian) and once per pixel, then everything per (pixel, Gaussian) is fp32 FMAs on small, exactly known
-// differences.  k = d_gc/sin d_gc = P(c) rsqrt(1+c) with a degree-7 polynomial P for c = cos d_gc >= 0 (atan2f beyond
-// 90 degrees).  power*log2(e) = k^2 (qa a^2 + qb a b + qc b^2) with the conic pre-scaled at staging; alpha uses ex2.
+// differences.  k = d_gc/sin d_gc = P(c) rsqrt(1+c) with a degree-7 polynomial P for c = cos d_gc >= 0 (out of line beyond 90
+// degrees, still without atan).  (A polynomial in t = sin^2 d_gc alone, which needs no c on the near side, was measured and
+// dropped: on the paper's kind of scene the entries a pixel consumes before it saturates are the nearest, largest Gaussians, and
+// 64 % of the evaluated pairs of config 4 lie beyond 30 degrees of the Gaussian's centre, 22 % beyond 60.)
+// power*log2(e) = k^2 (qa a^2 + qb a b + qc b^2) with the conic pre-scaled at staging; alpha uses ex2, and an entry whose power is
+// below log2(alpha_min / o) (minus a margin far above the ex2 error) is skipped before the ex2: the same decision as
+// alpha < alpha_min, taken identically by forward and backward.
 #include "uts_internal.cuh"
 
 namespace uts {
@@ -24,6 +32,18 @@ struct RenderParams {
 };
 
 constexpr float kLog2e = 1.4426950408889634f;
+// Pixels per thread (PX) of the two kernels: a block has 256 / PX threads.  Measured on config 4 (B200): the forward is bound by
+// the per-evaluation arithmetic, not by the shared-memory reads or the loop (the same 2.9e9 warp instructions at PX = 1 and 4),
+// so it keeps one pixel per thread and the occupancy that goes with it; the backward gains from PX = 4 because one warp
+// reduction + one set of atomics then serves the four patches of a warp.
+#ifndef UTS_FWD_PX
+#define UTS_FWD_PX 1
+#endif
+#ifndef UTS_BWD_PX
+#define UTS_BWD_PX 4
+#endif
+constexpr int kFwdPx = UTS_FWD_PX, kBwdPx = UTS_BWD_PX;
+constexpr int kBatch = 256;                          // list entries staged per batch
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
@@ -50,11 +70,6 @@ __device__ __forceinline__ float4 lds128(uint32_t addr) {
 }
 __device__ __forceinline__ void red_add_global(float* p, float v) {       // p is a global address (cudaMalloc'ed gradient buffer)
   asm volatile("red.global.add.f32 [%0], %1;" :: "l"(p), "f"(v) : "memory");
-}
-__device__ __forceinline__ float2 lds64(uint32_t addr) {
-  float2 v;
-  asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
-  return v;
 }
 
 // k = d_gc / sin(d_gc).  For cos(d_gc) = c >= 0:  acos(c) = sqrt(1-c) P(c) with P analytic on [0,1], so
@@ -83,19 +98,22 @@ __device__ __forceinline__ float arc_over_sin(float t, float c) {
   return arc_over_sin_far(t, c);
 }
 
-// What one (tile, Gaussian) list entry contributes to every pixel of the tile, staged once per entry.
-struct Entry {
-  float a0, b0, c0, o;          // e.(c_tile-u), n.(c_tile-u), uhat.c_tile, opacity
-  float ex, ez, nx, ny;         // e = (ex, 0, ez)
-  float nz, ux, uy, uz;         // uhat
-  float qa, qb, qc, r;          // -0.5 A log2e, -B log2e, -0.5 C log2e, red
-  float g, bl;                  // green, blue
-};
-
+// What one (tile, Gaussian) list entry contributes to every pixel of the tile, staged once per entry as float4 rows:
+//   g0 = (a0, b0, c0, th)     a0 = e.(c_tile-u), b0 = n.(c_tile-u), c0 = uhat.c_tile; th = log2(alpha_min / o) - margin
+//   g1 = (ex, ez, nx, ny)     e = (ex, 0, ez)
+//   g2 = (nz, ux, uy, uz)     uhat
+//   g3 = (qa, qb, qc, o)      -0.5 A log2e, -B log2e, -0.5 C log2e; opacity
+//   g4 = (r, g, b, id)        colour; id = Gaussian index as raw bits (backward)
+//   g5 = (sin phi, cos phi)   backward only
+constexpr uint32_t kRow = kBatch * 16u;               // bytes between rows
 struct TileFrame { double cx, cy, cz; };              // tile centre direction (order k_t pixel centre)
 
-__device__ __forceinline__ void stage_entry(const TileFrame& tf, float ux, float uy, float uz, float4 co, float r, float g,
-                                            float b, Entry& E) {
+template <bool BWD>
+struct __align__(16) SEntries { float4 g[BWD ? 6 : 5][kBatch]; };
+
+template <bool BWD>
+__device__ __forceinline__ void stage_entry(SEntries<BWD>& S, int i, const TileFrame& tf, float amin, uint32_t id, float ux, float uy,
+                                            float uz, float4 co, float r, float g, float b) {
   const float dxf = (float)(tf.cx - (double)ux), dyf = (float)(tf.cy - (double)uy), dzf = (float)(tf.cz - (double)uz);
   const float rxz2 = ux * ux + uz * uz;
   float ex = 1.f, ez = 0.f;
@@ -103,151 +121,199 @@ __device__ __forceinline__ void stage_entry(const TileFrame& tf, float ux, float
   const float invn = rsqrtf(rxz2 + uy * uy);
   const float hx = ux * invn, hy = uy * invn, hz = uz * invn;
   const float nx = hy * ez, ny = hz * ex - hx * ez, nz = -hy * ex;                       // n = uhat x e
-  E.a0 = ex * dxf + ez * dzf;
-  E.b0 = nx * dxf + ny * dyf + nz * dzf;
-  E.c0 = hx * (float)tf.cx + hy * (float)tf.cy + hz * (float)tf.cz;
-  E.o = co.w;
-  E.ex = ex; E.ez = ez; E.nx = nx; E.ny = ny; E.nz = nz; E.ux = hx; E.uy = hy; E.uz = hz;
-  E.qa = -0.5f * kLog2e * co.x; E.qb = -kLog2e * co.y; E.qc = -0.5f * kLog2e * co.z;
-  E.r = r; E.g = g; E.bl = b;
-}
-
-struct SEntry {                                       // shared-memory layout: broadcast reads of float4
-  float4 f0[kTilePix], f1[kTilePix], f2[kTilePix], f3[kTilePix];
-  float2 f4[kTilePix];
-};
-
-__device__ __forceinline__ void put_entry(SEntry& S, int i, const Entry& E) {
-  S.f0[i] = make_float4(E.a0, E.b0, E.c0, E.o);
-  S.f1[i] = make_float4(E.ex, E.ez, E.nx, E.ny);
-  S.f2[i] = make_float4(E.nz, E.ux, E.uy, E.uz);
-  S.f3[i] = make_float4(E.qa, E.qb, E.qc, E.r);
-  S.f4[i] = make_float2(E.g, E.bl);
+  // alpha = o 2^p2 < alpha_min  <=>  p2 < log2(alpha_min / o); the 1e-3 margin (0.07 % in alpha) is far above the error of
+  // lg2.approx / ex2.approx, so p2 < th implies alpha < alpha_min and the exact test settles everything else
+  float th = -3.0e38f;
+  if (amin > 0.f) th = co.w > 0.f ? __log2f(amin / co.w) - 1e-3f : 3.0e38f;
+  S.g[0][i] = make_float4(ex * dxf + ez * dzf, nx * dxf + ny * dyf + nz * dzf, hx * (float)tf.cx + hy * (float)tf.cy + hz * (float)tf.cz, th);
+  S.g[1][i] = make_float4(ex, ez, nx, ny);
+  S.g[2][i] = make_float4(nz, hx, hy, hz);
+  S.g[3][i] = make_float4(-0.5f * kLog2e * co.x, -kLog2e * co.y, -0.5f * kLog2e * co.z, co.w);
+  S.g[4][i] = make_float4(r, g, b, __uint_as_float(id));
+  if (BWD) S.g[5][i] = make_float4(hy, sqrtf(hx * hx + hz * hz), 0.f, 0.f);
 }
 
 struct Eval { float a, b, c, t, k, p2; };
 
 // Shared by forward and backward so that both take the same skip / clamp decisions.
-__device__ __forceinline__ void eval_entry(const float4 f0, const float4 f1, const float4 f2, const float4 f3, float px,
-                                           float py, float pz, Eval& ev) {
-  ev.a = fmaf(f1.x, px, fmaf(f1.y, pz, f0.x));
-  ev.b = fmaf(f1.z, px, fmaf(f1.w, py, fmaf(f2.x, pz, f0.y)));
-  ev.c = fmaf(f2.y, px, fmaf(f2.z, py, fmaf(f2.w, pz, f0.z)));
+__device__ __forceinline__ void eval_entry(const float4 g0, const float4 g1, const float4 g2, const float4 g3, float px, float py, float pz,
+                                           Eval& ev) {
+  ev.a = fmaf(g1.x, px, fmaf(g1.y, pz, g0.x));
+  ev.b = fmaf(g1.z, px, fmaf(g1.w, py, fmaf(g2.x, pz, g0.y)));
+  ev.c = fmaf(g2.y, px, fmaf(g2.z, py, fmaf(g2.w, pz, g0.z)));
   ev.t = fmaf(ev.a, ev.a, ev.b * ev.b);
   ev.k = arc_over_sin(ev.t, ev.c);
-  const float q = fmaf(ev.a, fmaf(f3.x, ev.a, f3.y * ev.b), f3.z * ev.b * ev.b);     // qa a^2 + qb a b + qc b^2
+  const float q = fmaf(ev.a, fmaf(g3.x, ev.a, g3.y * ev.b), g3.z * ev.b * ev.b);     // qa a^2 + qb a b + qc b^2
   ev.p2 = q * ev.k * ev.k;
 }
+// Alg.1 l.23 (reading A7): power > 0 skipped; power below the alpha_min cut skipped (see stage_entry)
+__device__ __forceinline__ bool may_contribute(const Eval& ev, float th) { return !(ev.p2 > 0.f) && ev.p2 >= th; }
 
 // Pixel and tile set-up common to both kernels.
-struct PixelSetup { float px, py, pz; bool on; size_t out; uint64_t start, end; int v; int64_t tile; };
+template <int PX>
+struct TileSetup { bool on[PX]; float px[PX], py[PX], pz[PX]; size_t out0; uint64_t start, end; int v; int64_t tile; };
 
-__device__ __forceinline__ void setup_pixel(const RenderParams& rp, const uint32_t* __restrict__ active_tiles,
-                                            const uint32_t* __restrict__ mask_bits, const uint64_t* __restrict__ ranges,
-                                            TileFrame* s_tf, PixelSetup& ps) {
+template <int PX>
+__device__ __forceinline__ void setup_tile(const RenderParams& rp, const uint32_t* __restrict__ active_tiles,
+                                           const uint32_t* __restrict__ mask_bits, const uint64_t* __restrict__ ranges,
+                                           TileFrame* s_tf, TileSetup<PX>& ts) {
+  constexpr int kThreads = kTilePix / PX;
   const int64_t slot = blockIdx.x % rp.n_slot;
-  ps.v = (int)(blockIdx.x / rp.n_slot);
+  ts.v = (int)(blockIdx.x / rp.n_slot);
   const int64_t tile = active_tiles ? (int64_t)__ldg(active_tiles + slot) : slot;
-  const uint64_t p = (uint64_t)tile * kTilePix + threadIdx.x;
-  ps.tile = tile;
-  ps.on = mask_bits ? ((__ldg(mask_bits + (p >> 5)) >> (p & 31)) & 1u) != 0 : true;
-  ps.out = ((size_t)ps.v * rp.n_slot + slot) * kTilePix + threadIdx.x;
-  const uint64_t rix = 2 * ((uint64_t)ps.v * rp.n_tile + tile);
-  ps.start = __ldg(ranges + rix); ps.end = __ldg(ranges + rix + 1);
+  ts.tile = tile;
+  ts.out0 = ((size_t)ts.v * rp.n_slot + slot) * kTilePix + threadIdx.x;       // pixel j of this thread: out0 + kThreads j
+  const uint64_t rix = 2 * ((uint64_t)ts.v * rp.n_tile + tile);
+  ts.start = __ldg(ranges + rix); ts.end = __ldg(ranges + rix + 1);
   if (threadIdx.x == 0) pix_center_cam(rp.k - kTileLog2, (uint64_t)tile, s_tf->cx, s_tf->cy, s_tf->cz);
-  double wx, wy, wz;
-  pix_center_cam(rp.k, p, wx, wy, wz);
+  double wx[PX], wy[PX], wz[PX];
+#pragma unroll
+  for (int j = 0; j < PX; ++j) {
+    const uint64_t p = (uint64_t)tile * kTilePix + threadIdx.x + kThreads * j;
+    ts.on[j] = mask_bits ? ((__ldg(mask_bits + (p >> 5)) >> (p & 31)) & 1u) != 0 : true;
+    pix_center_cam(rp.k, p, wx[j], wy[j], wz[j]);
+  }
   __syncthreads();
-  ps.px = (float)(wx - s_tf->cx); ps.py = (float)(wy - s_tf->cy); ps.pz = (float)(wz - s_tf->cz);
+#pragma unroll
+  for (int j = 0; j < PX; ++j) {
+    ts.px[j] = (float)(wx[j] - s_tf->cx); ts.py[j] = (float)(wy[j] - s_tf->cy); ts.pz[j] = (float)(wz[j] - s_tf->cz);
+  }
 }
 
-// Marks (uts_render_fwd_marked / uts_render_bwd_marked): one bit per (warp of the tile's block, list entry), set by the forward
-// when at least one of the warp's 32 pixels blended the entry.  Plane w (of 8) holds warp w's bits; the bits of (view, tile) vt
-// start at word (start_vt >> 5) + vt of the plane, entry j of the list at bit j of that run — runs of different tiles never share a
-// word.  The backward walks only the set bits: on the paper's kind of scene half of the (warp, entry) visits re-evaluate alpha just
-// to find that no pixel of the warp took the entry.
-__device__ __forceinline__ uint64_t mark_base(const RenderParams& rp, const PixelSetup& ps, int64_t tile) {
-  return (ps.start >> 5) + (uint64_t)ps.v * (uint64_t)rp.n_tile + (uint64_t)tile;
+// Marks (uts_render_fwd_marked / uts_render_bwd_marked): one bit per (patch, list entry), set by the forward when at least one
+// of the patch's 32 pixels blended the entry.  Patch (j, warp) — pixels (256 / PX) j + 32 warp + lane — is plane (8 / PX) j + warp
+// of 8, whatever PX the forward and the backward were built with; the bits
+// of (view, tile) vt start at word (start_vt >> 5) + vt of the plane, entry i of the list at bit i of that run — runs of
+// different tiles never share a word.  The backward visits an entry only for the patches whose bit is set: on the paper's kind of
+// scene half of the (patch, entry) visits would re-evaluate alpha just to find that no pixel of the patch took the entry.
+template <int PX>
+__device__ __forceinline__ uint64_t mark_base(const RenderParams& rp, const TileSetup<PX>& ts) {
+  return (ts.start >> 5) + (uint64_t)ts.v * (uint64_t)rp.n_tile + (uint64_t)ts.tile;
 }
 
-template <bool MARK>
-__global__ void __launch_bounds__(kTilePix)
+// Every thread stages PX entries of the batch, one after the other (issuing the gathers of several entries together was measured:
+// the extra registers cost more occupancy than the overlapped latency gives back).  Up to three null entries follow the last real
+// one, so that the walk can take entries four at a time: a = 1, qa = 1 give power > 0, which Alg.1 l.23 skips whatever the thresholds.
+template <int PX, bool BWD>
+__device__ __forceinline__ void stage_batch(SEntries<BWD>& S, const TileFrame& tf, const RenderParams& rp, const float* __restrict__ dir,
+                                            const float* __restrict__ conic_opac, const float* __restrict__ rgb,
+                                            const uint32_t* __restrict__ vals, uint64_t first, uint64_t n, size_t gbase) {
+  constexpr int kThreads = kTilePix / PX;
+#pragma unroll 1
+  for (uint32_t e = threadIdx.x; e < (uint32_t)kBatch; e += kThreads) {
+    if ((uint64_t)e < n) {
+      const uint32_t id = __ldg(vals + first + e);
+      const size_t gi = gbase + id;
+      stage_entry<BWD>(S, (int)e, tf, rp.amin, id, __ldg(dir + 3 * gi), __ldg(dir + 3 * gi + 1), __ldg(dir + 3 * gi + 2),
+                       __ldg(reinterpret_cast<const float4*>(conic_opac) + gi), __ldg(rgb + 3 * gi), __ldg(rgb + 3 * gi + 1),
+                       __ldg(rgb + 3 * gi + 2));
+    } else {
+      if ((uint64_t)e < n + 3) {
+        S.g[0][e] = make_float4(1.f, 0.f, 1.f, -3.0e38f); S.g[1][e] = make_float4(0.f, 0.f, 0.f, 0.f);
+        S.g[2][e] = make_float4(0.f, 0.f, 0.f, 0.f); S.g[3][e] = make_float4(1.f, 0.f, 0.f, 0.f);
+      }
+      break;
+    }
+  }
+}
+
+template <int PX, bool MARK>
+__global__ void __launch_bounds__(kTilePix / PX)
 render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* __restrict__ conic_opac, const float* __restrict__ rgb,
                   const uint32_t* __restrict__ active_tiles, const uint32_t* __restrict__ mask_bits,
                   const uint64_t* __restrict__ ranges, const uint32_t* __restrict__ vals, float* __restrict__ color,
                   float* __restrict__ alpha_out, float* __restrict__ trans_out, uint32_t* __restrict__ n_last_out,
                   uint32_t* __restrict__ marks, uint64_t plane_words) {
-  __shared__ SEntry S;
+  constexpr int kThreads = kTilePix / PX, kWarps = kThreads / 32;
+  __shared__ SEntries<false> S;
   __shared__ TileFrame s_tf;
-  PixelSetup ps;
-  setup_pixel(rp, active_tiles, mask_bits, ranges, &s_tf, ps);
+  TileSetup<PX> ts;
+  setup_tile<PX>(rp, active_tiles, mask_bits, ranges, &s_tf, ts);
   const TileFrame tf = s_tf;
-  const size_t gbase = (size_t)ps.v * rp.P;
+  const size_t gbase = (size_t)ts.v * rp.P;
+  const int wid = threadIdx.x >> 5;
 
-  float T = 1.f, Cr = 0.f, Cg = 0.f, Cb = 0.f;
-  uint32_t n_last = 0;
-  bool done = !ps.on;
-  const uint64_t len = ps.end - ps.start;
+  float T[PX], Cr[PX], Cg[PX], Cb[PX];
+  uint32_t n_last[PX];
+  uint32_t open = 0;                                  // bit j: pixel j still takes entries
+#pragma unroll
+  for (int j = 0; j < PX; ++j) { T[j] = 1.f; Cr[j] = Cg[j] = Cb[j] = 0.f; n_last[j] = 0; if (ts.on[j]) open |= 1u << j; }
+  const uint64_t len = ts.end - ts.start;
   const uint32_t sS = (uint32_t)__cvta_generic_to_shared(&S);
-  uint32_t* mark_w = nullptr;                         // this warp's run of mark words for the tile
-  if (MARK) mark_w = marks + (uint64_t)(threadIdx.x >> 5) * plane_words + mark_base(rp, ps, ps.tile);
-  for (uint64_t b0 = 0; b0 < len; b0 += kTilePix) {
-    if (__syncthreads_and(done)) break;               // every pixel of the tile saturated (or masked)
-    const uint64_t j = b0 + threadIdx.x;
-    if (j < len) {
-      const size_t gi = gbase + __ldg(vals + ps.start + j);
-      Entry E;
-      stage_entry(tf, __ldg(dir + 3 * gi), __ldg(dir + 3 * gi + 1), __ldg(dir + 3 * gi + 2),
-                  __ldg(reinterpret_cast<const float4*>(conic_opac) + gi), __ldg(rgb + 3 * gi), __ldg(rgb + 3 * gi + 1),
-                  __ldg(rgb + 3 * gi + 2), E);
-      put_entry(S, threadIdx.x, E);
-    } else if (j < len + 3) {
-      // null entries pad the list to a multiple of 4: a = 1, qa = 1 give power > 0, which Alg.1 l.23 skips whatever the thresholds
-      S.f0[threadIdx.x] = make_float4(1.f, 0.f, 0.f, 0.f); S.f1[threadIdx.x] = make_float4(0.f, 0.f, 0.f, 0.f);
-      S.f2[threadIdx.x] = make_float4(0.f, 0.f, 0.f, 0.f); S.f3[threadIdx.x] = make_float4(1.f, 0.f, 0.f, 0.f);
-    }
+  uint32_t* mark_w = nullptr;                         // plane `wid` of this tile's run; patch j is kWarps j planes further
+  if (MARK) mark_w = marks + (uint64_t)wid * plane_words + mark_base<PX>(rp, ts);
+  for (uint64_t b0 = 0; b0 < len; b0 += kBatch) {
+    if (__syncthreads_and(open == 0)) break;          // every pixel of the tile saturated (or masked)
+    const uint64_t left_n = len - b0;
+    stage_batch<PX, false>(S, tf, rp, dir, conic_opac, rgb, vals, ts.start + b0, left_n, gbase);
     __syncthreads();
-    const int nb = (int)((len - b0) < (uint64_t)kTilePix ? (len - b0) : (uint64_t)kTilePix);
-    // four entries per warp vote: the vote only ends the walk early, every skip / clamp decision is per lane.  The batch is walked
-    // in groups of 32 entries, one mark word each.
+    const int nb = (int)(left_n < (uint64_t)kBatch ? left_n : (uint64_t)kBatch);
+    // The batch is walked in groups of 32 entries, one mark word per patch each.  Every four entries the warp finds out which
+    // of its patches still have an open pixel (one redux); the vote only ends a patch's walk early, every skip / clamp decision
+    // is per pixel.  The list is padded with null entries to a multiple of four.
     bool left = false;
     for (int g0 = 0; g0 < nb && !left; g0 += 32) {
-      uint32_t mw = 0;                                // this lane's marks of the group
+      uint32_t mw[PX];                                // this lane's marks of the group, per patch
+#pragma unroll
+      for (int j = 0; j < PX; ++j) mw[j] = 0u;
       const int ge = min(nb, g0 + 32);
       for (int j4 = g0; j4 < ge; j4 += 4) {
-        if (__all_sync(0xffffffffu, done)) { left = true; break; }     // warp vote: the whole 8x4 patch is saturated
-        const uint32_t bit4 = 1u << (j4 - g0);
+        const uint32_t alive = __reduce_or_sync(0xffffffffu, open);
+        if (alive == 0) { left = true; break; }       // every pixel of the warp is saturated
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
           const int jj = j4 + u;
           const uint32_t sa = sS + (uint32_t)jj * 16u;
-          const float4 f0 = lds128(sa), f1 = lds128(sa + 0x1000u), f2 = lds128(sa + 0x2000u), f3 = lds128(sa + 0x3000u);
-          Eval ev;
-          eval_entry(f0, f1, f2, f3, ps.px, ps.py, ps.pz, ev);
-          if (done || ev.p2 > 0.f) continue;          // Alg.1 l.23: power > 0 skipped (reading A7)
-          const float a = fminf(rp.amax, f0.w * ex2_approx(ev.p2));
-          if (a < rp.amin) continue;
-          if (MARK) mw |= bit4 << u;                  // this lane blended the entry
-          const float2 f4 = lds64(sS + 0x4000u + (uint32_t)jj * 8u);
-          const float w = T * a;                      // Eq.6: c_i alpha_i prod_{j<i} (1 - alpha_j)
-          Cr = fmaf(w, f3.w, Cr); Cg = fmaf(w, f4.x, Cg); Cb = fmaf(w, f4.y, Cb);
-          T = T * (1.f - a);
-          n_last = (uint32_t)(b0 + jj) + 1u;
-          if (T < rp.teps) done = true;               // Alg.1 l.27: test after the update
+          const float4 g0v = lds128(sa), g1 = lds128(sa + kRow), g2 = lds128(sa + 2u * kRow), g3 = lds128(sa + 3u * kRow);
+          float p2[PX];
+          uint32_t cand = 0;                          // bit j: pixel j may blend this entry
+#pragma unroll
+          for (int j = 0; j < PX; ++j) {
+            p2[j] = 1.f;
+            if (PX == 1 || (alive & (1u << j))) {     // warp-uniform
+              Eval ev;
+              eval_entry(g0v, g1, g2, g3, ts.px[j], ts.py[j], ts.pz[j], ev);
+              p2[j] = ev.p2;
+              if (((open >> j) & 1u) && may_contribute(ev, g0v.w)) cand |= 1u << j;
+            }
+          }
+          if (PX > 1 && !__any_sync(0xffffffffu, cand != 0)) continue;
+          if (PX == 1 && cand == 0) continue;
+          const float4 g4 = lds128(sa + 4u * kRow);
+          const uint32_t bit = 1u << (jj - g0);
+#pragma unroll
+          for (int j = 0; j < PX; ++j) {
+            if (!((cand >> j) & 1u)) continue;
+            const float a = fminf(rp.amax, g3.w * ex2_approx(p2[j]));
+            if (a < rp.amin) continue;
+            if (MARK) mw[j] |= bit;                   // this pixel blended the entry
+            const float w = T[j] * a;                 // Eq.6: c_i alpha_i prod_{j<i} (1 - alpha_j)
+            Cr[j] = fmaf(w, g4.x, Cr[j]); Cg[j] = fmaf(w, g4.y, Cg[j]); Cb[j] = fmaf(w, g4.z, Cb[j]);
+            T[j] = T[j] * (1.f - a);
+            n_last[j] = (uint32_t)(b0 + jj) + 1u;
+            if (T[j] < rp.teps) open &= ~(1u << j);   // Alg.1 l.27: test after the update
+          }
         }
       }
-      if (MARK) {                                     // the warp's word of the group (written even when 0: the buffer is not cleared)
-        const uint32_t gw = __reduce_or_sync(0xffffffffu, mw);
-        if ((threadIdx.x & 31) == 0) mark_w[(b0 + (uint64_t)g0) >> 5] = gw;
+      if (MARK) {                                     // the patches' words of the group (written even when 0: the buffer is not cleared)
+#pragma unroll
+        for (int j = 0; j < PX; ++j) {
+          const uint32_t gw = __reduce_or_sync(0xffffffffu, mw[j]);
+          if ((threadIdx.x & 31) == 0) mark_w[(uint64_t)(kWarps * j) * plane_words + ((b0 + (uint64_t)g0) >> 5)] = gw;
+        }
       }
     }
   }
-  if (ps.on) {
-    color[3 * ps.out] = fmaf(T, rp.bg[0], Cr); color[3 * ps.out + 1] = fmaf(T, rp.bg[1], Cg); color[3 * ps.out + 2] = fmaf(T, rp.bg[2], Cb);
-    alpha_out[ps.out] = 1.f - T; trans_out[ps.out] = T; n_last_out[ps.out] = n_last;
-  } else {
-    color[3 * ps.out] = 0.f; color[3 * ps.out + 1] = 0.f; color[3 * ps.out + 2] = 0.f;
-    alpha_out[ps.out] = 0.f; trans_out[ps.out] = 1.f; n_last_out[ps.out] = 0u;
+#pragma unroll
+  for (int j = 0; j < PX; ++j) {
+    const size_t o = ts.out0 + (size_t)kThreads * j;
+    if (ts.on[j]) {
+      color[3 * o] = fmaf(T[j], rp.bg[0], Cr[j]); color[3 * o + 1] = fmaf(T[j], rp.bg[1], Cg[j]); color[3 * o + 2] = fmaf(T[j], rp.bg[2], Cb[j]);
+      alpha_out[o] = 1.f - T[j]; trans_out[o] = T[j]; n_last_out[o] = n_last[j];
+    } else {
+      color[3 * o] = 0.f; color[3 * o + 1] = 0.f; color[3 * o + 2] = 0.f;
+      alpha_out[o] = 0.f; trans_out[o] = 1.f; n_last_out[o] = 0u;
+    }
   }
 }
 
@@ -258,43 +324,47 @@ __device__ __forceinline__ float warp_sum(float x) {
   return x;
 }
 
-struct SEntryBwd {
-  float4 f0[kTilePix], f1[kTilePix], f2[kTilePix], f3[kTilePix];
-  float4 f5[kTilePix];                                 // green, blue, sin(phi), cos(phi)
-  uint32_t id[kTilePix];
-};
-
-template <bool MARK>
-__global__ void __launch_bounds__(kTilePix)
+template <int PX, bool MARK>
+__global__ void __launch_bounds__(kTilePix / PX)
 render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* __restrict__ conic_opac, const float* __restrict__ rgb,
                   const uint32_t* __restrict__ active_tiles, const uint32_t* __restrict__ mask_bits,
                   const uint64_t* __restrict__ ranges, const uint32_t* __restrict__ vals, const float* __restrict__ trans,
                   const uint32_t* __restrict__ n_last_in, const float* __restrict__ dL_dcolor, const float* __restrict__ dL_dalpha,
                   float* __restrict__ dL_drgb, float* __restrict__ dL_dconic, float* __restrict__ dL_dmu2, float* __restrict__ dL_dopac,
                   const uint32_t* __restrict__ marks, uint64_t plane_words) {
-  __shared__ SEntryBwd S;
+  constexpr int kThreads = kTilePix / PX, kWarps = kThreads / 32;
+  __shared__ SEntries<true> S;
   __shared__ TileFrame s_tf;
-  __shared__ uint32_t s_max[kTilePix / 32];
-  PixelSetup ps;
-  setup_pixel(rp, active_tiles, mask_bits, ranges, &s_tf, ps);
+  __shared__ uint32_t s_max[kWarps];
+  TileSetup<PX> ts;
+  setup_tile<PX>(rp, active_tiles, mask_bits, ranges, &s_tf, ts);
   const TileFrame tf = s_tf;
-  const size_t gbase = (size_t)ps.v * rp.P;
+  const size_t gbase = (size_t)ts.v * rp.P;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
 
-  const uint32_t nl = ps.on ? __ldg(n_last_in + ps.out) : 0u;
-  const float Tfin = ps.on ? __ldg(trans + ps.out) : 1.f;
-  const float gr = ps.on ? __ldg(dL_dcolor + 3 * ps.out) : 0.f, gg = ps.on ? __ldg(dL_dcolor + 3 * ps.out + 1) : 0.f,
-              gb = ps.on ? __ldg(dL_dcolor + 3 * ps.out + 2) : 0.f;
-  const float ga_T = (dL_dalpha && ps.on) ? __ldg(dL_dalpha + ps.out) * Tfin : 0.f;      // dL/dalpha_out * T_final
+  uint32_t nl[PX];
+  float T[PX], Sr[PX], Sg[PX], Sb[PX], gr[PX], gg[PX], gb[PX], ga_T[PX];
+  uint32_t m = 0;
+#pragma unroll
+  for (int j = 0; j < PX; ++j) {
+    const size_t o = ts.out0 + (size_t)kThreads * j;
+    const bool on = ts.on[j];
+    nl[j] = on ? __ldg(n_last_in + o) : 0u;
+    const float Tfin = on ? __ldg(trans + o) : 1.f;
+    gr[j] = on ? __ldg(dL_dcolor + 3 * o) : 0.f; gg[j] = on ? __ldg(dL_dcolor + 3 * o + 1) : 0.f; gb[j] = on ? __ldg(dL_dcolor + 3 * o + 2) : 0.f;
+    ga_T[j] = (dL_dalpha && on) ? __ldg(dL_dalpha + o) * Tfin : 0.f;          // dL/dalpha_out * T_final
+    T[j] = Tfin;                                        // transmittance after the entry being visited
+    Sr[j] = Tfin * rp.bg[0]; Sg[j] = Tfin * rp.bg[1]; Sb[j] = Tfin * rp.bg[2];  // colour accumulated behind it
+    m = max(m, nl[j]);
+  }
   // block maximum of n_last: entries beyond it were reached by no pixel
-  uint32_t m = nl;
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, d));
   if (lane == 0) s_max[wid] = m;
   __syncthreads();
   uint32_t max_nl = 0;
 #pragma unroll
-  for (int w = 0; w < kTilePix / 32; ++w) max_nl = max(max_nl, s_max[w]);
+  for (int w = 0; w < kWarps; ++w) max_nl = max(max_nl, s_max[w]);
   if (max_nl == 0) return;
 
   // the gradient word this lane owns after the butterfly below (lanes 4j: value j), as base pointer + stride per Gaussian:
@@ -307,85 +377,76 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
   asm volatile("" : "+l"(lane_dst));                   // keep the per-view base folded into the pointer (one IMAD.WIDE per atomic)
   const uint32_t sS = (uint32_t)__cvta_generic_to_shared(&S);
 
-  float T = Tfin;                                      // transmittance after the entry being visited
-  float Sr = Tfin * rp.bg[0], Sg = Tfin * rp.bg[1], Sb = Tfin * rp.bg[2];                // colour accumulated behind it
-  const int n_batch = (int)((max_nl + kTilePix - 1) / kTilePix);
-  const uint32_t* mark_w = nullptr;                    // this warp's run of mark words for the tile (see render_fwd_kernel)
-  if (MARK) mark_w = marks + (uint64_t)wid * plane_words + mark_base(rp, ps, ps.tile);
+  const int n_batch = (int)((max_nl + kBatch - 1) / kBatch);
+  // lane 8 j + g (j < PX) reads word g of patch j's plane, kWarps j + wid
+  const uint32_t* mark_w = nullptr;
+  if (MARK && lane < 8 * PX) mark_w = marks + (uint64_t)(kWarps * (lane >> 3) + wid) * plane_words + mark_base<PX>(rp, ts);
   for (int bi = n_batch - 1; bi >= 0; --bi) {
-    const uint32_t b0 = (uint32_t)bi * kTilePix;
-    // lane g < 8: the marks of entries b0 + 32 g .. + 31.  The forward wrote this warp's words up to the last entry any of its
-    // pixels blended; words beyond that hold whatever the buffer held (it is never cleared) — a set bit there only costs the
-    // visit's first vote, because no pixel of the warp reaches such an entry.
+    const uint32_t b0 = (uint32_t)bi * kBatch;
+    // The forward wrote a patch's words up to the last entry any of its pixels blended; words beyond that hold whatever the
+    // buffer held (it is never cleared) — a set bit there only costs the evaluation, because no pixel of the patch reaches
+    // such an entry (jl < nl below).
     uint32_t myw = 0u;
-    if (MARK && lane < 8) myw = __ldg(mark_w + (size_t)bi * 8 + lane);
+    if (MARK && lane < 8 * PX) myw = __ldg(mark_w + (size_t)bi * 8 + (lane & 7));
     __syncthreads();
-    const uint32_t j = b0 + threadIdx.x;
-    if (j < max_nl) {
-      const uint32_t id = __ldg(vals + ps.start + j);
-      const size_t gi = gbase + id;
-      const float ux = __ldg(dir + 3 * gi), uy = __ldg(dir + 3 * gi + 1), uz = __ldg(dir + 3 * gi + 2);
-      Entry E;
-      stage_entry(tf, ux, uy, uz, __ldg(reinterpret_cast<const float4*>(conic_opac) + gi), __ldg(rgb + 3 * gi),
-                  __ldg(rgb + 3 * gi + 1), __ldg(rgb + 3 * gi + 2), E);
-      S.f0[threadIdx.x] = make_float4(E.a0, E.b0, E.c0, E.o);
-      S.f1[threadIdx.x] = make_float4(E.ex, E.ez, E.nx, E.ny);
-      S.f2[threadIdx.x] = make_float4(E.nz, E.ux, E.uy, E.uz);
-      S.f3[threadIdx.x] = make_float4(E.qa, E.qb, E.qc, E.r);
-      S.f5[threadIdx.x] = make_float4(E.g, E.bl, E.uy, sqrtf(E.ux * E.ux + E.uz * E.uz));
-      S.id[threadIdx.x] = id;
-    }
+    stage_batch<PX, true>(S, tf, rp, dir, conic_opac, rgb, vals, ts.start + b0, (uint64_t)(max_nl - b0), gbase);
     __syncthreads();
-    const int nb = (int)min((uint32_t)kTilePix, max_nl - b0);
-    auto visit = [&](const int jj) {
+    const int nb = (int)min((uint32_t)kBatch, max_nl - b0);
+    // one list entry for the patches in pm (bit j: patch j of this warp)
+    auto visit = [&](const int jj, const uint32_t pm) {
       const uint32_t jl = b0 + (uint32_t)jj;
-      const bool reach = jl < nl;                      // this pixel's forward pass got this far
-      if (!__any_sync(0xffffffffu, reach)) return;
       const uint32_t sa = sS + (uint32_t)jj * 16u;
-      const float4 f0 = lds128(sa), f1 = lds128(sa + 0x1000u), f2 = lds128(sa + 0x2000u), f3 = lds128(sa + 0x3000u), f5 = lds128(sa + 0x4000u);
-      Eval ev;
-      eval_entry(f0, f1, f2, f3, ps.px, ps.py, ps.pz, ev);
-      float e2 = 0.f, raw = 0.f, a = 0.f;
-      bool used = reach && !(ev.p2 > 0.f);
-      if (used) { e2 = ex2_approx(ev.p2); raw = f0.w * e2; a = fminf(rp.amax, raw); used = !(a < rp.amin); }
-      if (!__any_sync(0xffffffffu, used)) return;
+      const float4 g0v = lds128(sa), g1 = lds128(sa + kRow), g2 = lds128(sa + 2u * kRow), g3 = lds128(sa + 3u * kRow), g4 = lds128(sa + 4u * kRow);
       float d_r = 0.f, d_g = 0.f, d_b = 0.f, d_A = 0.f, d_B = 0.f, d_C = 0.f, d_o = 0.f, d_om = 0.f, d_ph = 0.f;
-      if (used) {
-        const float inv1a = rcp_approx(1.f - a);
-        const float Tb = T * inv1a;                    // transmittance before this entry
+      bool any_used = false;
+#pragma unroll
+      for (int j = 0; j < PX; ++j) {
+        if (PX > 1 && !((pm >> j) & 1u)) continue;     // warp-uniform
+        Eval ev;
+        eval_entry(g0v, g1, g2, g3, ts.px[j], ts.py[j], ts.pz[j], ev);
+        bool used = jl < nl[j] && may_contribute(ev, g0v.w);       // jl < nl: this pixel's forward pass got this far
+        float e2 = 0.f, raw = 0.f, a = 0.f;
+        if (used) { e2 = ex2_approx(ev.p2); raw = g3.w * e2; a = fminf(rp.amax, raw); used = !(a < rp.amin); }
+        if (!used) continue;
+        any_used = true;
+        const float inv1a = rcp_approx(fmaxf(1.f - a, 1e-7f));      // alpha = 1 (alpha_max = 1, opacity 1 at the centre): finite
+        const float Tb = T[j] * inv1a;                 // transmittance before this entry
         const float w = Tb * a;
-        d_r = w * gr; d_g = w * gg; d_b = w * gb;
-        float dLa = gr * (Tb * f3.w - Sr * inv1a) + gg * (Tb * f5.x - Sg * inv1a) + gb * (Tb * f5.y - Sb * inv1a) + ga_T * inv1a;
-        Sr = fmaf(w, f3.w, Sr); Sg = fmaf(w, f5.x, Sg); Sb = fmaf(w, f5.y, Sb);
-        T = Tb;
-        if (!(raw > rp.amax)) {                        // reading A7: no gradient through a clamped alpha
-          d_o = e2 * dLa;                              // exp(power) dL/dalpha
-          const float gp = a * dLa;                    // dL/dpower
-          const float dx = ev.k * ev.a, dy = ev.k * ev.b;
-          const float cA = -2.f / kLog2e * f3.x, cB = -1.f / kLog2e * f3.y, cC = -2.f / kLog2e * f3.z;   // conic (A,B,C)
-          d_A = -0.5f * dx * dx * gp; d_B = -dx * dy * gp; d_C = -0.5f * dy * dy * gp;
-          const float gdx = -(cA * dx + cB * dy) * gp, gdy = -(cB * dx + cC * dy) * gp;
-          // (dx,dy) = k(s,c) (a,b):  dk/ds / s = (c/den - k)/t,  dk/dc = -1/den,  den = s^2 + c^2
-          float g_a = gdx, g_b = gdy, g_c = 0.f;
-          if (ev.t > 0.f) {
-            const float den = ev.t + ev.c * ev.c;
-            const float gk = gdx * ev.a + gdy * ev.b;
-            const float iden = rcp_approx(den);
-            const float kp = (ev.c * iden - ev.k) * rcp_approx(ev.t);
-            g_a = fmaf(gk * kp, ev.a, ev.k * gdx);
-            g_b = fmaf(gk * kp, ev.b, ev.k * gdy);
-            g_c = -gk * iden;
-          }
-          // a = e.w, b = n.w, c = u.w with de/dom = -hh, dn/dom = -sin(phi) e, du/dom = cos(phi) e, dn/dphi = -u, du/dphi = n,
-          // and hh.w = cos(phi) c - sin(phi) b
-          const float sp = f5.z, cp = f5.w;
-          d_om = -g_a * (cp * ev.c - sp * ev.b) - g_b * sp * ev.a + g_c * cp * ev.a;
-          d_ph = g_c * ev.b - g_b * ev.c;
+        d_r = fmaf(w, gr[j], d_r); d_g = fmaf(w, gg[j], d_g); d_b = fmaf(w, gb[j], d_b);
+        const float dLa = gr[j] * (Tb * g4.x - Sr[j] * inv1a) + gg[j] * (Tb * g4.y - Sg[j] * inv1a) + gb[j] * (Tb * g4.z - Sb[j] * inv1a) +
+                          ga_T[j] * inv1a;
+        Sr[j] = fmaf(w, g4.x, Sr[j]); Sg[j] = fmaf(w, g4.y, Sg[j]); Sb[j] = fmaf(w, g4.z, Sb[j]);
+        T[j] = Tb;
+        if (raw > rp.amax) continue;                   // reading A7: no gradient through a clamped alpha
+        d_o = fmaf(e2, dLa, d_o);                      // exp(power) dL/dalpha
+        const float gp = a * dLa;                      // dL/dpower
+        const float dx = ev.k * ev.a, dy = ev.k * ev.b;
+        const float cA = -2.f / kLog2e * g3.x, cB = -1.f / kLog2e * g3.y, cC = -2.f / kLog2e * g3.z;   // conic (A,B,C)
+        d_A = fmaf(-0.5f * dx * dx, gp, d_A); d_B = fmaf(-dx * dy, gp, d_B); d_C = fmaf(-0.5f * dy * dy, gp, d_C);
+        const float gdx = -(cA * dx + cB * dy) * gp, gdy = -(cB * dx + cC * dy) * gp;
+        // (dx,dy) = k(s,c) (a,b):  dk/ds / s = (c/den - k)/t,  dk/dc = -1/den,  den = s^2 + c^2
+        float g_a = gdx, g_b = gdy, g_c = 0.f;
+        if (ev.t > 0.f) {
+          const float den = ev.t + ev.c * ev.c;
+          const float gk = gdx * ev.a + gdy * ev.b;
+          const float iden = rcp_approx(den);
+          const float kp = (ev.c * iden - ev.k) * rcp_approx(ev.t);
+          g_a = fmaf(gk * kp, ev.a, ev.k * gdx);
+          g_b = fmaf(gk * kp, ev.b, ev.k * gdy);
+          g_c = -gk * iden;
         }
+        // a = e.w, b = n.w, c = u.w with de/dom = -hh, dn/dom = -sin(phi) e, du/dom = cos(phi) e, dn/dphi = -u, du/dphi = n,
+        // and hh.w = cos(phi) c - sin(phi) b
+        const float2 g5 = *reinterpret_cast<const float2*>(&S.g[5][jj]);
+        const float sp = g5.x, cp = g5.y;
+        d_om += -g_a * (cp * ev.c - sp * ev.b) - g_b * sp * ev.a + g_c * cp * ev.a;
+        d_ph += g_c * ev.b - g_b * ev.c;
       }
-      // 9 sums over the warp.  Eight of them go through a transposing butterfly: at each of the first three steps a lane
-      // keeps half of its values and hands the other half to its partner, so 4+2+1 shuffles leave every lane with ONE value
-      // summed over 8 lanes, and two more steps finish it: 9 shuffles instead of 40.  Lane 4*j ends up owning value j.
+      if (!__any_sync(0xffffffffu, any_used)) return;
+      // 9 sums over the warp (each lane already holds the sum over its PX pixels).  Eight of them go through a transposing
+      // butterfly: at each of the first three steps a lane keeps half of its values and hands the other half to its partner, so
+      // 4+2+1 shuffles leave every lane with ONE value summed over 8 lanes, and two more steps finish it: 9 shuffles instead of
+      // 40.  Lane 4*j ends up owning value j.
       float v0 = d_r, v1 = d_g, v2 = d_b, v3 = d_A, v4 = d_B, v5 = d_C, v6 = d_om, v7 = d_ph;
       {
         const bool hi = lane & 16;
@@ -408,23 +469,32 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
       v0 += __shfl_xor_sync(0xffffffffu, v0, 2);
       v0 += __shfl_xor_sync(0xffffffffu, v0, 1);
       d_o = warp_sum(d_o);
-      {
-        const uint32_t id = S.id[jj];
-        if (lane_owns) red_add_global(lane_dst + (size_t)id * lane_stride, lane == 1 ? d_o : v0);
-      }
+      if (lane_owns) red_add_global(lane_dst + (size_t)__float_as_uint(g4.w) * lane_stride, lane == 1 ? d_o : v0);
     };
     if (MARK) {
       for (int grp = (nb - 1) >> 5; grp >= 0; --grp) {
-        uint32_t wb = __shfl_sync(0xffffffffu, myw, grp);
+        uint32_t w[PX], wb = 0;
+#pragma unroll
+        for (int j = 0; j < PX; ++j) { w[j] = __shfl_sync(0xffffffffu, myw, 8 * j + grp); wb |= w[j]; }
         if (nb - 32 * grp < 32) wb &= (1u << (nb - 32 * grp)) - 1u;   // entries >= nb: beyond the tile's largest n_last
         while (wb) {                                                  // back to front over the marked entries
           const int bit = 31 - __clz((int)wb);
           wb &= ~(1u << bit);
-          visit(32 * grp + bit);
+          uint32_t pm = 0;
+#pragma unroll
+          for (int j = 0; j < PX; ++j) pm |= ((w[j] >> bit) & 1u) << j;
+          visit(32 * grp + bit, pm);
         }
       }
     } else {
-      for (int jj = nb - 1; jj >= 0; --jj) visit(jj);
+      for (int jj = nb - 1; jj >= 0; --jj) {
+        const uint32_t jl = b0 + (uint32_t)jj;
+        uint32_t reach = 0;
+#pragma unroll
+        for (int j = 0; j < PX; ++j) reach |= (jl < nl[j] ? 1u : 0u) << j;
+        const uint32_t pm = __reduce_or_sync(0xffffffffu, reach);     // patches with a pixel that got this far
+        if (pm) visit(jj, pm);
+      }
     }
   }
 }
@@ -464,10 +534,10 @@ static int render_fwd_impl(const uts_config* cfg, uts_proj in, uts_mask mask, co
   if (d.n_slot * d.V > 0x7fffffffll) return UTS_ERR_UNSUPPORTED;
   RenderParams rp = make_params(cfg, d);
   if (marks)
-    render_fwd_kernel<true><<<(unsigned)(d.n_slot * d.V), kTilePix, 0, (cudaStream_t)stream>>>(
+    render_fwd_kernel<kFwdPx, true><<<(unsigned)(d.n_slot * d.V), kTilePix / kFwdPx, 0, (cudaStream_t)stream>>>(
         rp, in.dir, in.conic_opac, in.rgb, mask.active_tiles, mask.pixel_mask_bits, ranges, vals, color, alpha, trans, n_last, marks, plane_words);
   else
-    render_fwd_kernel<false><<<(unsigned)(d.n_slot * d.V), kTilePix, 0, (cudaStream_t)stream>>>(
+    render_fwd_kernel<kFwdPx, false><<<(unsigned)(d.n_slot * d.V), kTilePix / kFwdPx, 0, (cudaStream_t)stream>>>(
         rp, in.dir, in.conic_opac, in.rgb, mask.active_tiles, mask.pixel_mask_bits, ranges, vals, color, alpha, trans, n_last, nullptr, 0);
   UTS_LAUNCH_CHECK();
   return UTS_OK;
@@ -507,11 +577,11 @@ static int render_bwd_impl(const uts_config* cfg, uts_proj in, uts_mask mask, co
   if (d.n_slot * d.V > 0x7fffffffll) return UTS_ERR_UNSUPPORTED;
   RenderParams rp = make_params(cfg, d);
   if (marks)
-    render_bwd_kernel<true><<<(unsigned)(d.n_slot * d.V), kTilePix, 0, (cudaStream_t)stream>>>(
+    render_bwd_kernel<kBwdPx, true><<<(unsigned)(d.n_slot * d.V), kTilePix / kBwdPx, 0, (cudaStream_t)stream>>>(
         rp, in.dir, in.conic_opac, in.rgb, mask.active_tiles, mask.pixel_mask_bits, ranges, vals, trans, n_last, dL_dcolor,
         dL_dalpha, dL_drgb, dL_dconic, dL_dmu2, dL_dopac, marks, plane_words);
   else
-    render_bwd_kernel<false><<<(unsigned)(d.n_slot * d.V), kTilePix, 0, (cudaStream_t)stream>>>(
+    render_bwd_kernel<kBwdPx, false><<<(unsigned)(d.n_slot * d.V), kTilePix / kBwdPx, 0, (cudaStream_t)stream>>>(
         rp, in.dir, in.conic_opac, in.rgb, mask.active_tiles, mask.pixel_mask_bits, ranges, vals, trans, n_last, dL_dcolor,
         dL_dalpha, dL_drgb, dL_dconic, dL_dmu2, dL_dopac, nullptr, 0);
   UTS_LAUNCH_CHECK();

@@ -13,6 +13,7 @@ from __future__ import annotations
 import argparse
 import json
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -30,9 +31,13 @@ UNIT = "px/s"
 # default: Alg.1 l.9-16 through uts_tile_lists (one call); --lists staged times uts_tile_query / uts_sort / uts_tile_ranges one by one
 STAGES_FUSED = ["preprocess", "depth_order", "tile_lists", "render_fwd", "render_bwd", "preprocess_bwd"]
 STAGES_STAGED = ["preprocess", "depth_order", "tile_query", "sort", "tile_ranges", "render_fwd", "render_bwd", "preprocess_bwd"]
-# FP32 operations one evaluated (Gaussian, pixel) pair costs in the blend kernels (counted from the
-# arithmetic of Eq.6 + SphericalOffset as implemented, FMA = 2): forward 46, backward 118.
-FLOP_FWD, FLOP_BWD = 46, 118
+# FP32 operations of the blend kernels per (Gaussian, pixel) pair (counted from the arithmetic of Eq.6 +
+# SphericalOffset as implemented, FMA = 2): an EVALUATED pair costs 41 (forward) / 46 (backward: the same evaluation + the reach
+# test and exp kept for the gradient), a CONTRIBUTING pair another 9 (forward: blend) / 72 (backward: gradient chain + its share
+# of the warp reduction).
+FLOP_FWD_EVAL, FLOP_FWD_CONTRIB, FLOP_BWD_EVAL, FLOP_BWD_CONTRIB = 41, 9, 46, 72
+# the ONE bounded oracle sample both arms time (--impl reference, and the cpu_baseline leg of the default arm)
+ORACLE_SAMPLE = dict(n_pre=500_000, n_query=60_000, n_tiles_sample=192)
 
 
 def _peaks():
@@ -154,45 +159,69 @@ class OracleSample:
         return total, desc
 
 
+def workload_config(cfg_id, n_gpus, n_pix):
+    """The `config` object of the JSON line: the same keys and values in both arms (--impl ours / reference)."""
+    m = scenes.CONFIGS[cfg_id]
+    return dict(workload=f"config{cfg_id}:{m['name']}", order=m["order"], nside=1 << m["order"], n_pix=int(n_pix), n_gauss=m["n_gauss"],
+                sh_degree=m["sh_degree"], n_views=m["n_views"], parallelism=f"replicas{n_gpus}",
+                l2="inputs larger than L2 (Gaussians + pair buffers: GBs at config 4); no flush needed")
+
+
+def oracle_timing(cfg_id, repeats, warmup=0):
+    """The oracle as it stands on ORACLE_SAMPLE of the workload, `repeats` timed steps.  Returns (sample object, step times, description)."""
+    smp = OracleSample(cfg_id, seed=0, **ORACLE_SAMPLE)
+    times, desc = [], ""
+    for i in range(warmup + repeats):
+        t, desc = smp.step()
+        if i >= warmup:
+            times.append(t)
+    return smp, times, desc
+
+
+def cpu_baseline_object(smp, times, desc):
+    t = float(np.mean(times))
+    return dict(value=smp.n_pix / t, unit=UNIT, cores=1, kind="oracle", sample=desc, repeats=len(times),
+                spread=dict(min_s=float(np.min(times)), max_s=float(np.max(times)), mean_s=t,
+                            note="extrapolated whole-frame seconds of each timed repeat of the same sample"))
+
+
 def run_reference(args):
+    """The reference arm for this tier is the oracle (there is no reference code): rank 0 alone times it, the other ranks exit."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    sc_meta = scenes.CONFIGS[args.config]
-    times = []
-    desc = ""
-    smp = OracleSample(args.config, seed=0, n_pre=200_000, n_query=20_000, n_tiles_sample=48)
-    for i in range(args.warmup + args.steps):
-        t, desc = smp.step()
-        if i >= args.warmup:
-            times.append(t)
+    smp, times, desc = oracle_timing(args.config, args.steps, args.warmup)
     t = float(np.mean(times))
     val = smp.n_pix / t
     line = dict(metric=METRIC, value=val, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup, ms_per_step=t * 1e3,
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic", impl="reference",
-                config=dict(workload=f"config{args.config}:{sc_meta['name']}", order=sc_meta["order"], n_gauss=sc_meta["n_gauss"],
-                            sh_degree=sc_meta["sh_degree"], n_views=sc_meta["n_views"]),
-                cpu_baseline=dict(value=val, unit=UNIT, cores=1, kind="oracle", sample=desc),
+                config=workload_config(args.config, args.gpus, smp.n_pix),
+                note=("ms_per_step is the EXTRAPOLATED whole-frame time of the single-thread fp64 oracle from a bounded sample (cpu_baseline.sample); "
+                      "the CPU time actually spent per step is about 1/100 of it"),
+                cpu_baseline=cpu_baseline_object(smp, times, desc),
                 e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
     print(json.dumps(line))
 
 
 # ----------------------------------------------------------------------------------------------------- our arm
-def run_ours(args):
+def stage_bytes(stage, P, V, M, n_tiles, n_pairs):
+    """Algorithmic HBM bytes of one call of an HBM-bound stage."""
+    tile_bytes = (max(1, (V * n_tiles - 1)).bit_length() + 7) // 8
+    return {"preprocess": P * V * (44 + 12 * M + 57),
+            "preprocess_bwd": P * (44 + 12 * M + V * 33 + 40 + 12 * M),
+            "depth_order": P * V * (4 + 5 * 32 + 16),
+            "tile_query": P * V * 2 * 29 + 8 * P * V + 12 * n_pairs,
+            "tile_lists": P * V * 2 * 29 + 12 * n_pairs + 16 * V * n_tiles,      # floor: every sorted pair written once
+            "sort": 32.0 * n_pairs * tile_bytes,
+            "tile_ranges": 8.0 * n_pairs + 16 * V * n_tiles}[stage]
+
+
+def measure_config(args, cfg_id, steps, warmup, rank, world, dist, local, sample_clocks=False):
+    """Times `steps` whole steps of config cfg_id on this rank (CUDA events on the launching stream, per stage and whole).
+    Returns a dict with the rasteriser still alive under "r" (the caller deletes it)."""
     import torch
-    import torch.distributed as dist
     from paper_2606_29794_b200 import binding as B, rasterizer as R, replicas
-
-    world, rank, local = replicas.world()
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    peaks = _peaks()
-
-    # replicas only: every rank renders its own scene of the same recipe; no data-path collective
-    scene = scenes.make_scene(args.config, seed=replicas.rank_seed(rank))
+    scene = scenes.make_scene(cfg_id, seed=replicas.rank_seed(rank))
     cfg = R.config_of(scene)
     mask = B.Mask.full() if scene["mask"] is None else B.uts_build_mask(cfg, scene["mask"]["kind"], scene["mask"]["params"])
     g, views = R.scene_to_device(scene)
@@ -203,8 +232,12 @@ def run_ours(args):
     V, S = cfg.n_views, r.S
     npx = S * cfg.ppt
     gcol = torch.from_numpy(scenes.upstream_grad(V, npx, seed=rank)).cuda()
-    n_pix_active = int(V * cfg.n_pix) if scene["mask"] is None else int(V * sum(bin(int(w) & 0xffffffff).count("1") for w in mask.pixel_mask_bits.cpu().numpy().tolist()))
-
+    if scene["mask"] is None:
+        n_pix_active = int(V * cfg.n_pix)
+    else:
+        w = mask.pixel_mask_bits.to(torch.int64) & 0xffffffff
+        w = w - ((w >> 1) & 0x55555555); w = (w & 0x33333333) + ((w >> 2) & 0x33333333); w = (w + (w >> 4)) & 0x0f0f0f0f
+        n_pix_active = int(V * int((((w * 0x01010101) & 0xffffffff) >> 24).sum().item()))
     stream = torch.cuda.current_stream()
 
     def step(events=None):
@@ -226,40 +259,39 @@ def run_ours(args):
         mark(i + 2); r.preprocess_bwd(g, views)
         mark(i + 3)
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         step()
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
-    sampler = ClockSampler(local); sampler.start()
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(NS + 1)] for _ in range(args.steps)]
+    sampler = None
+    if sample_clocks:
+        sampler = ClockSampler(local); sampler.start()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(NS + 1)] for _ in range(steps)]
     t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
     launches0 = B.uts_launch_count()
     t0.record(stream)
-    for k in range(args.steps):
+    for k in range(steps):
         step(ev[k])
     t1.record(stream)
     torch.cuda.synchronize()
     launches = B.uts_launch_count() - launches0          # counted by the library itself, one tick per kernel launch
-    clocks = sampler.stop()
-    total_ms = t0.elapsed_time(t1)
-    ms_step = total_ms / args.steps
-    stage_ms = {STAGES[i]: float(np.mean([ev[k][i].elapsed_time(ev[k][i + 1]) for k in range(args.steps)])) for i in range(NS)}
+    clocks = sampler.stop() if sampler else None
+    ms_step = t0.elapsed_time(t1) / steps
+    stage_ms = {STAGES[i]: float(np.mean([ev[k][i].elapsed_time(ev[k][i + 1]) for k in range(steps)])) for i in range(NS)}
     ms_fwd = sum(stage_ms[s] for s in STAGES[:NS - 2])
 
-    # work counters from the forward outputs (measurement plumbing): entries each pixel evaluated
-    lens = (r.ranges[:, 1] - r.ranges[:, 0])
-    tiles = torch.arange(cfg.n_tiles, device="cuda") if mask.active_tiles is None else mask.active_tiles.long()
-    ev_f = ev_b = 0
-    for v in range(V):
-        L = lens[v * cfg.n_tiles + tiles].repeat_interleave(cfg.ppt)
-        nl = r.n_last[v].long()
-        sat = r.trans[v] < cfg.t_eps
-        ev_f += int(torch.where(sat, nl, L).sum().item())
-        ev_b += int(nl.sum().item())
-    # with marks the backward visits only the (warp, entry) pairs the forward marked: 32 pixel evaluations each (measurement plumbing:
-    # a population count of the mark words; the buffer starts zeroed and every step writes the same words)
+    # ---- work counters (measurement plumbing, after the timed region)
+    # evaluated / contributing pairs of Alg.1's loop, counted on the device by uts_render_fwd_counted (same decisions as the timed kernels)
+    work = torch.zeros(2, dtype=torch.int64, device="cuda")
+    scratch_img = [torch.empty_like(t) for t in (r.color, r.alpha, r.trans, r.n_last)]
+    B.uts_render_fwd_counted(cfg, r.proj, mask, r.ranges, r.vals, *scratch_img, work)
+    ev_f, contrib = (int(x) for x in work.cpu().tolist())
+    del scratch_img
+    ev_b = int(r.n_last.long().sum().item())              # SURVEY 8(d)'s E_bwd: every entry before n_last, for every pixel
+    # with marks the backward evaluates only the (patch, entry) pairs the forward marked: 32 pixel evaluations each (a population
+    # count of the mark words; the buffer starts zeroed and every step writes the same words)
     ev_b_visited = None
     if r.use_marks:
         tot = 0
@@ -269,13 +301,79 @@ def run_ours(args):
             t = t - ((t >> 1) & 0x55555555); t = (t & 0x33333333) + ((t >> 2) & 0x33333333); t = (t + (t >> 4)) & 0x0f0f0f0f
             tot += int((((t * 0x01010101) & 0xffffffff) >> 24).sum().item())
         ev_b_visited = 32 * tot
+    return dict(scene=scene, cfg=cfg, mask=mask, g=g, views=views, r=r, gcol=gcol, STAGES=STAGES, ms_step=ms_step, ms_fwd=ms_fwd, stage_ms=stage_ms,
+                launches=int(launches), clocks=clocks, n_pix_active=n_pix_active, n_pairs=int(r.n_pairs), ev_f=ev_f, ev_b=ev_b, contrib=contrib,
+                ev_b_visited=ev_b_visited, npx=npx)
 
-    # next step after the hot path (not part of the step): Interp_H of Eq.7 to the camera image and its adjoint,
-    # timed on view 0's HEALPix image.  Camera: the paper's case for this grid where there is no mask (6080 x 3040 panorama ->
-    # Nside 1024, Table 5), else a 1920 x 1080 pinhole of 60 x 45 degrees (config 5's frustum).
+
+def per_kernel_table(m, peaks, fp32_peak):
+    """Per stage: ms and the achieved fraction of the roofline that bounds it (HBM stages: algorithmic bytes / time against the measured
+    copy bandwidth; blend stages: FP32 operations of the work the kernel EXECUTES / time against the derived FP32 peak)."""
+    cfg = m["cfg"]
+    P, V, M = cfg.n_gauss, cfg.n_views, cfg.n_sh
+    out = {}
+    for s_, ms in m["stage_ms"].items():
+        sec = ms * 1e-3
+        if s_ == "render_fwd":
+            flop = m["ev_f"] * FLOP_FWD_EVAL + m["contrib"] * FLOP_FWD_CONTRIB
+            out[s_] = dict(ms=ms, bound="alu", tflops=flop / sec / 1e12, frac_fp32_peak=flop / sec / 1e12 / fp32_peak)
+        elif s_ == "render_bwd":
+            ev_exec = m["ev_b_visited"] if m["ev_b_visited"] is not None else m["ev_b"]
+            flop = ev_exec * FLOP_BWD_EVAL + m["contrib"] * FLOP_BWD_CONTRIB
+            flop_alg = m["ev_b"] * FLOP_BWD_EVAL + m["contrib"] * FLOP_BWD_CONTRIB
+            out[s_] = dict(ms=ms, bound="alu", tflops=flop / sec / 1e12, frac_fp32_peak=flop / sec / 1e12 / fp32_peak,
+                           frac_fp32_peak_alg1_units=flop_alg / sec / 1e12 / fp32_peak)
+        else:
+            byts = stage_bytes(s_, P, V, M, cfg.n_tiles, m["n_pairs"])
+            out[s_] = dict(ms=ms, bound="hbm", gbs=byts / sec / 1e9, frac_hbm_peak=byts / sec / 1e9 / peaks["hbm_gbs"])
+    return out
+
+
+def roofline_of_dominant(m, pk, peaks, fp32_peak, traffic):
+    """`roofline` = the stage with the largest time, whichever it is (uts_tile_lists is one ABI call of about 25 kernels; its line is
+    the call's algorithmic bytes against the HBM peak, and profiles/ holds its kernels one by one)."""
+    dom = max(m["stage_ms"], key=m["stage_ms"].get)
+    e = pk[dom]
+    if e["bound"] == "alu":
+        roof = dict(kernel=dom, bound="alu", achieved=e["tflops"], peak=fp32_peak, unit="TFLOP/s", frac=e["frac_fp32_peak"], traffic=traffic.get(dom),
+                    peak_source="derived: 148 SM x 128 FP32 lanes x 2 x sm_max_mhz",
+                    note="flops of the evaluations the kernel executes (41/46 per evaluated pair + 9/72 per contributing pair, counted on the device)")
+    else:
+        roof = dict(kernel=dom, bound="hbm", achieved=e["gbs"], peak=peaks["hbm_gbs"], unit="GB/s", frac=e["frac_hbm_peak"], traffic=traffic.get(dom),
+                    peak_source=peaks["source"] + " (MEASURED_PEAKS.json hbm_gbs: copy bandwidth)" if peaks["source"] == "measured" else "fallback 6650 GB/s")
+        if dom == "tile_lists":
+            roof["note"] = ("one ABI call = Alg.1 l.9-16 (tile query + depth sort + ranges): algorithmic bytes = every sorted pair written once (12 B) + "
+                            "58 B per (view, Gaussian) + 16 B per (view, tile); the call is issue-bound geometry + a merge, see profiles/")
+    return roof
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_29794_b200 import binding as B, rasterizer as R, replicas
+
+    world, rank, local = replicas.world()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    peaks = _peaks()
+    fp32_peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12       # TFLOP/s at the maximum SM clock (DESIGN.md "Roofline")
+
+    # replicas only (DESIGN.md "Multi-GPU"): every rank renders its own scene of the same recipe; no data-path collective
+    m = measure_config(args, args.config, args.steps, args.warmup, rank, world, dist, local, sample_clocks=True)
+    scene, cfg, mask, g, views, r, gcol = m["scene"], m["cfg"], m["mask"], m["g"], m["views"], m["r"], m["gcol"]
+    V, npx, n_pix_active = cfg.n_views, m["npx"], m["n_pix_active"]
+    fused = args.lists == "fused"
+    ms_step = m["ms_step"]
+
     extras = {}
     run_extras = not args.no_extras
     r._color_full = r.color.clone()          # the full lists' image, for the bit-identity check of the depth-prefix leg below
+    # next step after the hot path (SURVEY §8f NEXT-2, not part of the step): Interp_H of Eq.7 to the camera image and its adjoint,
+    # timed on view 0's HEALPix image.  Camera: the paper's case for this grid where there is no mask (6080 x 3040 panorama ->
+    # Nside 1024, Table 5 PAPER.md:358), else a 1920 x 1080 pinhole of 60 x 45 degrees (config 5's frustum).
     try:
         if not run_extras:
             raise RuntimeError("skipped (--no-extras)")
@@ -368,17 +466,17 @@ def run_ours(args):
     pin = lambda *s: torch.empty(*s, dtype=torch.float32).pin_memory()
     out = dict(color=pin(V, npx, 3), alpha=pin(V, npx), dL_dmeans=pin(P, 3), dL_dscales=pin(P, 3), dL_dquats=pin(P, 4), dL_dopac=pin(P),
                dL_dsh=pin(P, M, 3))
-    cap = r.n_pairs + 1024
-    n_pairs = r.n_pairs
+    cap = m["n_pairs"] + 1024
     ws_bytes = B.uts_host_workspace_bytes(cfg, mask.n_active, cap)
-    keep = dict(stage_proj=None)
     del r
+    m["r"] = None
     torch.cuda.empty_cache()
     ws = torch.empty(ws_bytes // 8 + 64, dtype=torch.int64, device="cuda")
     h2d = sum(t.numel() * 4 for t in h.values()) + hg.numel() * 4
     d2h = sum(t.numel() * 4 for t in out.values())
-    e2e_steps = max(1, min(args.steps, 3))
-    B.uts_host_forward_backward(cfg, h, mask, hg, out, cap, ws)           # warm-up
+    e2e_steps = max(10, min(args.steps, 20)) if args.steps >= 3 else args.steps      # at least 10 timed end-to-end steps in a normal run
+    for _ in range(2):
+        B.uts_host_forward_backward(cfg, h, mask, hg, out, cap, ws)       # warm-up
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
@@ -387,6 +485,8 @@ def run_ours(args):
         B.uts_host_forward_backward(cfg, h, mask, hg, out, cap, ws)       # synchronises the stream itself
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - tt) * 1e3 / e2e_steps
+    del ws, h, hg, out
+    torch.cuda.empty_cache()
 
     ms_step_max, e2e_ms_max = replicas.max_over_ranks([ms_step, e2e_ms], device="cuda")
     if rank != 0:
@@ -395,70 +495,91 @@ def run_ours(args):
         return
 
     value = replicas.aggregate_throughput(n_pix_active, ms_step_max, world)
-    # DRAM bytes per launch of each kernel from the committed ncu --set full capture of this workload (profiles/), or None
+    # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed ncu --set full capture of this workload
+    # (profiles/), or None
     traffic = {}
-    tp = os.path.join(ROOT, "profiles", "r01_traffic.csv")
-    if os.path.exists(tp):
-        with open(tp) as f:
-            for ln in f.read().splitlines()[1:]:
-                w_, st_, by_ = ln.split(",")
-                if w_ == f"config{args.config}":
-                    traffic[st_] = int(by_)
-    # dominant kernel and its roofline
-    # (uts_tile_lists is a call of about 25 kernels, the longest of them shorter than the forward blend: not a candidate)
-    dom = max((k_ for k_ in stage_ms if k_ != "tile_lists"), key=stage_ms.get)
-    fp32_peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12       # TFLOP/s at the maximum SM clock
-    if dom in ("render_fwd", "render_bwd"):
-        # units as SURVEY 8(d) defines them: E_fwd / E_bwd = the pairs Alg.1's loop evaluates, every entry before n_last for every pixel
-        flop = ev_f * FLOP_FWD if dom == "render_fwd" else ev_b * FLOP_BWD
-        ach = flop / (stage_ms[dom] * 1e-3) / 1e12
-        roof = dict(kernel=dom, bound="alu", achieved=ach, peak=fp32_peak, unit="TFLOP/s", frac=ach / fp32_peak, traffic=traffic.get(dom),
-                    peak_source="derived: 148 SM x 128 FP32 lanes x 2 x sm_max_mhz")
-        if dom == "render_bwd" and ev_b_visited is not None:
-            a1 = ev_b_visited * FLOP_BWD / (stage_ms[dom] * 1e-3) / 1e12
-            roof["note"] = ("units = E_bwd of SURVEY 8(d): every entry before n_last for every pixel (Alg.1's loop).  The marked backward skips the (warp, "
-                            "entry) visits in which no pixel of the warp blended the entry; counting only the 32 pixel evaluations of each visit it "
-                            f"does make: achieved = {a1:.1f} TFLOP/s, frac = {a1 / fp32_peak:.3f}")
-    else:
-        per_pair = {"sort": 32.0 * ((max(1, (V * cfg.n_tiles - 1)).bit_length() + 7) // 8), "tile_query": 12.0, "tile_ranges": 8.0}.get(dom)
-        byts = per_pair * n_pairs if per_pair else P * V * (44 + 12 * M + 57)
-        ach = byts / (stage_ms[dom] * 1e-3) / 1e9
-        roof = dict(kernel=dom, bound="hbm", achieved=ach, peak=peaks["hbm_gbs"], unit="GB/s", frac=ach / peaks["hbm_gbs"], traffic=traffic.get(dom),
-                    peak_source=peaks["source"])
-    per_kernel = {}
-    for s_, ms in stage_ms.items():
-        if s_ == "render_fwd":
-            per_kernel[s_] = dict(ms=ms, tflops=ev_f * FLOP_FWD / (ms * 1e-3) / 1e12, frac_fp32_peak=ev_f * FLOP_FWD / (ms * 1e-3) / 1e12 / fp32_peak)
-        elif s_ == "render_bwd":
-            per_kernel[s_] = dict(ms=ms, tflops=ev_b * FLOP_BWD / (ms * 1e-3) / 1e12, frac_fp32_peak=ev_b * FLOP_BWD / (ms * 1e-3) / 1e12 / fp32_peak)
-            if ev_b_visited is not None:
-                per_kernel[s_]["tflops_visited_only"] = ev_b_visited * FLOP_BWD / (ms * 1e-3) / 1e12
-        else:
-            byts = {"preprocess": P * V * (44 + 12 * M + 57), "preprocess_bwd": P * (44 + 12 * M + V * 33 + 40 + 12 * M),
-                    "depth_order": P * V * (4 + 5 * 32 + 16), "tile_query": P * V * 2 * 29 + 8 * P * V + 12 * n_pairs,
-                    "tile_lists": P * V * 2 * 29 + 12 * n_pairs + 16 * V * cfg.n_tiles,      # floor: every sorted pair written once
-                    "sort": 32.0 * n_pairs * ((max(1, (V * cfg.n_tiles - 1)).bit_length() + 7) // 8),
-                    "tile_ranges": 8.0 * n_pairs + 16 * V * cfg.n_tiles}[s_]
-            per_kernel[s_] = dict(ms=ms, gbs=byts / (ms * 1e-3) / 1e9, frac_hbm_peak=byts / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"])
+    for name in ("r02_traffic.csv", "r01_traffic.csv"):
+        tp = os.path.join(ROOT, "profiles", name)
+        if os.path.exists(tp):
+            with open(tp) as f:
+                for ln in f.read().splitlines()[1:]:
+                    w_, st_, by_ = ln.split(",")
+                    if w_ == f"config{args.config}":
+                        traffic[st_] = int(by_)
+            break
+    pk = per_kernel_table(m, peaks, fp32_peak)
+    roof = roofline_of_dominant(m, pk, peaks, fp32_peak, traffic)
+
+    # the other BASELINE.json configs, a few steps each (headline stays args.config): ms forward / forward+backward, px/s and the
+    # dominant stage's roofline fraction, so that the driver-run record covers all five configs
+    if run_extras and world == 1:
+        others = {}
+        for cid in (1, 2, 3, 5):
+            if cid == args.config:
+                continue
+            try:
+                mo = measure_config(args, cid, 5, 3, rank, world, dist, local)
+                pko = per_kernel_table(mo, peaks, fp32_peak)
+                domo = max(mo["stage_ms"], key=mo["stage_ms"].get)
+                fr = pko[domo].get("frac_hbm_peak", pko[domo].get("frac_fp32_peak"))
+                others[f"config{cid}"] = dict(workload=f"config{cid}:{mo['scene']['name']}", n_pix=mo["n_pix_active"], n_pairs=mo["n_pairs"], steps=5, warmup=3,
+                                              ms_forward=mo["ms_fwd"], ms_forward_backward=mo["ms_step"], px_per_s=mo["n_pix_active"] / (mo["ms_step"] * 1e-3),
+                                              stage_ms=mo["stage_ms"], dominant=dict(stage=domo, bound=pko[domo]["bound"], frac=fr), gpu_launches_per_step=mo["launches"] / 5)
+                for k_ in ("r", "g", "views", "gcol", "mask"):
+                    mo[k_] = None
+                del mo
+                torch.cuda.empty_cache()
+            except Exception as e:      # measurement plumbing only
+                others[f"config{cid}"] = dict(error=str(e))
+        extras["configs"] = others
 
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup, ms_per_step=ms_step_max,
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
-                config=dict(workload=f"config{args.config}:{scene['name']}", order=cfg.order, nside=1 << cfg.order, n_pix=n_pix_active,
-                            n_gauss=P, sh_degree=cfg.sh_degree, n_views=V, n_pairs=n_pairs, parallelism=f"replicas{world}", lists=args.lists, marks=args.marks,
-                            l2="inputs larger than L2 (Gaussians 472 MB, pairs GBs); no flush needed"),
-                ms_forward=ms_fwd, ms_forward_backward=ms_step, stage_ms=stage_ms, per_kernel=per_kernel,
-                evaluated_pairs=dict(forward=ev_f, backward=ev_b, backward_visited_with_marks=ev_b_visited),
-                roofline=roof, clocks=clocks, extras=extras,
-                e2e=dict(value=replicas.aggregate_throughput(n_pix_active, e2e_ms_max, world), unit=UNIT, ms_per_step=e2e_ms_max, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h),
-                gpu_launches=0)
-    line["gpu_launches"] = int(launches)                 # uts_launch_count() over the timed region
+                config=workload_config(args.config, world, n_pix_active),
+                path=dict(lists=args.lists, marks=args.marks, n_pairs=m["n_pairs"]),
+                ms_forward=m["ms_fwd"], ms_forward_backward=ms_step, stage_ms=m["stage_ms"], per_kernel=pk,
+                evaluated_pairs=dict(forward=m["ev_f"], contributing=m["contrib"], backward_alg1=m["ev_b"], backward_executed=m["ev_b_visited"],
+                                     listed=int(m["n_pairs"]) * cfg.ppt,
+                                     note="forward / contributing: counted on the device by uts_render_fwd_counted; backward_alg1: sum of n_last; "
+                                          "backward_executed: 32 x marked (patch, entry) pairs; listed: pairs x 256 pixels"),
+                roofline=roof, clocks=m["clocks"], extras=extras,
+                e2e=dict(value=replicas.aggregate_throughput(n_pix_active, e2e_ms_max, world), unit=UNIT, ms_per_step=e2e_ms_max, steps=e2e_steps,
+                         h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h),
+                gpu_launches=m["launches"])                # uts_launch_count() over the timed region
     if not args.no_cpu_baseline:
-        smp = OracleSample(args.config, seed=0, n_pre=1_000_000, n_query=120_000, n_tiles_sample=384)   # about 10 s of oracle time on config 4
-        t, desc = smp.step()
-        line["cpu_baseline"] = dict(value=smp.n_pix / t, unit=UNIT, cores=1, kind="oracle", sample=desc)
+        smp, times, desc = oracle_timing(args.config, 3)
+        line["cpu_baseline"] = cpu_baseline_object(smp, times, desc)
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+
+
+def run_selftest(args):
+    """CPU-only check of the multi-rank plumbing (tests/test_replicas_gloo.py): every rank joins a gloo group, the ranks agree on
+    max-over-ranks times, rank 0 prints a line with n_gpus = world size.  Runs no kernel and reports no measurement."""
+    import torch.distributed as dist
+    from paper_2606_29794_b200 import replicas
+    world, rank, _ = replicas.world()
+    if world > 1:
+        dist.init_process_group("gloo")
+    mx = replicas.max_over_ranks([10.0 + rank, 5.0 - rank])
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(dict(selftest=True, n_gpus=world, max_over_ranks=mx)))
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` outside torchrun: start the N ranks here, the way the driver does
+    (python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P bench.py ...),
+    and pass their output through.  NCCL's own log stays on (NCCL_DEBUG=INFO unless the caller set it) and goes to stderr."""
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd, env=env)
 
 
 def main():
@@ -467,16 +588,20 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config id 1..5 (default 4 = the metric's workload)")
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference", "selftest"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--lists", default="fused", choices=["fused", "staged"],
                     help="Alg.1 l.9-16 as one uts_tile_lists call (default) or as uts_tile_query + uts_sort + uts_tile_ranges")
-    ap.add_argument("--no-extras", action="store_true", help="skip the legs that are not part of the step (resample, loss, depth prefix): used for the launch list")
+    ap.add_argument("--no-extras", action="store_true", help="skip the legs that are not part of the step (resample, loss, depth prefix, other configs): used for the launch list")
     ap.add_argument("--marks", default="on", choices=["on", "off"],
                     help="blend through uts_render_fwd_marked / uts_render_bwd_marked (default) or the plain pair")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(spawn_ranks(args))
     if args.impl == "reference":
         run_reference(args)
+    elif args.impl == "selftest":
+        run_selftest(args)
     else:
         run_ours(args)
 

@@ -118,6 +118,8 @@ typedef struct {
   int   descent_blocks_per_sm;/* descent only: persistent blocks per SM of that path; 0 = 2 */
   int   matrix_off;        /* uts_tile_lists: 1 = never route discs through the (disc x tile) bit matrix */
   float matrix_min_tiles;  /* uts_tile_lists: discs covering at least this many tiles become matrix rows; 0 = max(48, N_tile / 144) */
+  int   window_off;        /* 1 = the smallest discs go through ring intervals like the others instead of the tile window
+                              (uts_window_query.cuh) */
 } uts_tuning;
 
 /* ---------------------------------------------------------------------------------------------- forward */
@@ -193,6 +195,12 @@ int uts_tile_ranges(const uts_config* cfg, uint64_t n_pairs, const uint64_t* key
  * Entry order inside a tile is the order of `vals`. */
 int uts_render_fwd(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
                    float* color, float* alpha, float* trans, uint32_t* n_last, void* stream);
+
+/* uts_render_fwd that also counts its work (measurement only: bench.py's roofline lines): adds to work[0] the (pixel, entry) pairs
+ * Alg.1's loop evaluates (every entry a pixel visits before it stops, l.20-28 PAPER.md:568-584) and to work[1] those that
+ * contribute (alpha >= alpha_min).  work: 2 DEVICE uint64, zeroed by the caller.  Outputs as uts_render_fwd. */
+int uts_render_fwd_counted(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
+                           float* color, float* alpha, float* trans, uint32_t* n_last, uint64_t* work, void* stream);
 
 /* --------------------------------------------------------------------------------------------- backward */
 

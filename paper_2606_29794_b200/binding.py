@@ -20,7 +20,7 @@ UTS_OK, UTS_ERR_INVALID_ARG, UTS_ERR_CAPACITY, UTS_ERR_CUDA, UTS_ERR_UNSUPPORTED
 # every symbol include/uts.h declares
 SYMBOLS = [
     "uts_preprocess", "uts_preprocess_geometry", "uts_preprocess_color", "uts_depth_order", "uts_depth_order_scratch_bytes", "uts_tile_query", "uts_tile_query_scratch_bytes", "uts_tile_lists", "uts_tile_lists_scratch_bytes", "uts_sort", "uts_sort_scratch_bytes",
-    "uts_tile_ranges", "uts_render_fwd", "uts_render_bwd", "uts_render_marks_bytes", "uts_render_fwd_marked", "uts_render_bwd_marked", "uts_preprocess_bwd", "uts_build_mask", "uts_pixel_centers",
+    "uts_tile_ranges", "uts_render_fwd", "uts_render_fwd_counted", "uts_render_bwd", "uts_render_marks_bytes", "uts_render_fwd_marked", "uts_render_bwd_marked", "uts_preprocess_bwd", "uts_build_mask", "uts_pixel_centers",
     "uts_rho_max_table", "uts_resample_fwd", "uts_resample_bwd", "uts_build_camera_mask", "uts_inv_depth_channel", "uts_inv_depth_bwd", "uts_rs_max_update", "uts_depth_prefix_flags", "uts_count_unsaturated", "uts_hssim_loss", "uts_hssim_scratch_bytes",
     "uts_host_workspace_bytes", "uts_host_forward_backward", "uts_last_cuda_error", "uts_launch_count", "uts_strerror",
     "uts_version",
@@ -64,7 +64,7 @@ class CMask(C.Structure):
 
 class CTuning(C.Structure):
     _fields_ = [("query_impl", C.c_int), ("descent_block_radius", C.c_float), ("descent_blocks_per_sm", C.c_int), ("matrix_off", C.c_int),
-                ("matrix_min_tiles", C.c_float)]
+                ("matrix_min_tiles", C.c_float), ("window_off", C.c_int)]
 
 
 @dataclass
@@ -75,8 +75,10 @@ class Tuning:
     descent_blocks_per_sm: int = 0
     matrix_off: int = 0
     matrix_min_tiles: float = 0.0
+    window_off: int = 0                 # 1: no tile-window path for the smallest discs
 
-    def c(self): return CTuning(self.query_impl, self.descent_block_radius, self.descent_blocks_per_sm, self.matrix_off, self.matrix_min_tiles)
+    def c(self):
+        return CTuning(self.query_impl, self.descent_block_radius, self.descent_blocks_per_sm, self.matrix_off, self.matrix_min_tiles, self.window_off)
 
 
 def _tuning(t):
@@ -301,6 +303,14 @@ def uts_render_fwd(cfg: Config, proj: Proj, mask: Mask, ranges, vals, color, alp
     _check(lib().uts_render_fwd(C.byref(c), proj.c(), mask.c(), _ptr(ranges, torch.int64), _ptr(vals, torch.int32),
                                 _ptr(color, torch.float32), _ptr(alpha, torch.float32), _ptr(trans, torch.float32),
                                 _ptr(n_last, torch.int32), _stream(stream)), "uts_render_fwd")
+
+
+def uts_render_fwd_counted(cfg: Config, proj: Proj, mask: Mask, ranges, vals, color, alpha, trans, n_last, work, stream=None):
+    """uts_render_fwd + work counters: work = 2 int64 on the device (zeroed by the caller) -> += (evaluated, contributing) pairs."""
+    c = cfg.c()
+    _check(lib().uts_render_fwd_counted(C.byref(c), proj.c(), mask.c(), _ptr(ranges, torch.int64), _ptr(vals, torch.int32),
+                                        _ptr(color, torch.float32), _ptr(alpha, torch.float32), _ptr(trans, torch.float32),
+                                        _ptr(n_last, torch.int32), _ptr(work, torch.int64), _stream(stream)), "uts_render_fwd_counted")
 
 
 def uts_render_bwd(cfg: Config, proj: Proj, mask: Mask, ranges, vals, trans, n_last, dL_dcolor, dL_dalpha, dL_drgb, dL_dconic,

@@ -217,15 +217,17 @@ __device__ __forceinline__ void stage_batch(SEntries<BWD>& S, const TileFrame& t
   }
 }
 
-template <int PX, bool MARK>
+// COUNT (uts_render_fwd_counted, measurement only): also adds the evaluated and the contributing (pixel, entry) pairs to work[0..1].
+template <int PX, bool MARK, bool COUNT = false>
 __global__ void __launch_bounds__(kTilePix / PX)
 render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* __restrict__ conic_opac, const float* __restrict__ rgb,
                   const uint32_t* __restrict__ active_tiles, const uint32_t* __restrict__ mask_bits,
                   const uint64_t* __restrict__ ranges, const uint32_t* __restrict__ vals, float* __restrict__ color,
                   float* __restrict__ alpha_out, float* __restrict__ trans_out, uint32_t* __restrict__ n_last_out,
-                  uint32_t* __restrict__ marks, uint64_t plane_words) {
+                  uint32_t* __restrict__ marks, uint64_t plane_words, unsigned long long* __restrict__ work = nullptr) {
   constexpr int kThreads = kTilePix / PX, kWarps = kThreads / 32;
   __shared__ SEntries<false> S;
+  uint32_t n_eval = 0, n_contrib = 0;                 // COUNT only
   __shared__ TileFrame s_tf;
   TileSetup<PX> ts;
   setup_tile<PX>(rp, active_tiles, mask_bits, ranges, &s_tf, ts);
@@ -274,6 +276,7 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
               Eval ev;
               eval_entry(g0v, g1, g2, g3, ts.px[j], ts.py[j], ts.pz[j], ev);
               p2[j] = ev.p2;
+              if (COUNT && ((open >> j) & 1u) && (uint64_t)jj < left_n) ++n_eval;       // null padding entries are not Alg.1's
               if (((open >> j) & 1u) && may_contribute(ev, g0v.w)) cand |= 1u << j;
             }
           }
@@ -287,6 +290,7 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
             const float a = fminf(rp.amax, g3.w * ex2_approx(p2[j]));
             if (a < rp.amin) continue;
             if (MARK) mw[j] |= bit;                   // this pixel blended the entry
+            if (COUNT) ++n_contrib;
             const float w = T[j] * a;                 // Eq.6: c_i alpha_i prod_{j<i} (1 - alpha_j)
             Cr[j] = fmaf(w, g4.x, Cr[j]); Cg[j] = fmaf(w, g4.y, Cg[j]); Cb[j] = fmaf(w, g4.z, Cb[j]);
             T[j] = T[j] * (1.f - a);
@@ -303,6 +307,10 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
         }
       }
     }
+  }
+  if (COUNT) {
+    const uint32_t e = __reduce_add_sync(0xffffffffu, n_eval), c = __reduce_add_sync(0xffffffffu, n_contrib);
+    if ((threadIdx.x & 31) == 0) { atomicAdd(work, (unsigned long long)e); atomicAdd(work + 1, (unsigned long long)c); }
   }
 #pragma unroll
   for (int j = 0; j < PX; ++j) {
@@ -546,6 +554,23 @@ static int render_fwd_impl(const uts_config* cfg, uts_proj in, uts_mask mask, co
 int uts_render_fwd(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
                    float* color, float* alpha, float* trans, uint32_t* n_last, void* stream) {
   return render_fwd_impl(cfg, in, mask, ranges, vals, color, alpha, trans, n_last, nullptr, 0, stream);
+}
+
+int uts_render_fwd_counted(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
+                           float* color, float* alpha, float* trans, uint32_t* n_last, uint64_t* work, void* stream) {
+  int st = check_config(cfg);
+  if (st) return st;
+  if ((st = check_mask(cfg, mask))) return st;
+  if (!in.dir || !in.conic_opac || !in.rgb || !ranges || !color || !alpha || !trans || !n_last || !work) return UTS_ERR_INVALID_ARG;
+  Dims d = dims_of(cfg, &mask);
+  if (d.n_slot == 0) return UTS_OK;
+  if (d.n_slot * d.V > 0x7fffffffll) return UTS_ERR_UNSUPPORTED;
+  RenderParams rp = make_params(cfg, d);
+  render_fwd_kernel<1, false, true><<<(unsigned)(d.n_slot * d.V), kTilePix, 0, (cudaStream_t)stream>>>(
+      rp, in.dir, in.conic_opac, in.rgb, mask.active_tiles, mask.pixel_mask_bits, ranges, vals, color, alpha, trans, n_last, nullptr, 0,
+      reinterpret_cast<unsigned long long*>(work));
+  UTS_LAUNCH_CHECK();
+  return UTS_OK;
 }
 
 int uts_render_fwd_marked(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,

@@ -21,6 +21,7 @@
 #include "uts_internal.cuh"
 #include "uts_scan.cuh"
 #include "uts_ring_query.cuh"
+#include "uts_window_query.cuh"
 #include <cstring>
 
 namespace uts {
@@ -37,6 +38,8 @@ struct QueryParams {
   int wl_cap;                           // capacity of each of the two block work lists
   int64_t n_tile;
   double rho_q;                         // rho_max(k_q) (NESTED set) or 0 (RING set): R = min(pi, r_s + rho_q)
+  double rho_t;                         // rho_max(k_t)
+  int w_max;                            // window class: largest half-width (2 without a mask, kWindowMax with one)
   float r_large;                        // discs with R above this go to the block path
   uint32_t* tile_cache;                 // [V*P][kTileCacheK] tiles found by the count pass (thread path), reused by the emit pass
   uint32_t* bitmap_cache;               // [bitmap_cache_cap][n_words] bitmaps of the count pass (block path)
@@ -265,10 +268,11 @@ classify_kernel(QueryParams qp, const float* __restrict__ rs, const uint8_t* __r
 // n_small[3]: end of the matrix class (uts_tile_lists): whole buckets <= b_mat while they fit cap_rows rows; 0 when b_mat < 0 or
 // when the pairs those discs own (estimated from the bucket radii) would not pay for the per-(view, tile) bookkeeping of the
 // matrix path (about 256 B per (view, tile) against about 90 B per pair saved)
-__global__ void bucket_scan_kernel(uint32_t* __restrict__ hist, uint32_t* __restrict__ n_small, int b_block, int b_warp, int b_mat, uint32_t cap_rows,
-                                   double n_tile, double nvt) {
+// n_small[4]: start of the window class (uts_window_query.cuh): buckets >= b_fast, the smallest discs
+__global__ void bucket_scan_kernel(uint32_t* __restrict__ hist, uint32_t* __restrict__ n_small, int b_block, int b_warp, int b_mat, int b_fast,
+                                   uint32_t cap_rows, double n_tile, double nvt) {
   if (threadIdx.x == 0) {
-    uint32_t run = 0, e_block = 0, e_warp = 0, e_mat = 0;
+    uint32_t run = 0, e_block = 0, e_warp = 0, e_mat = 0, e_fast = 0;
     double est_pairs = 0.0, est_at_mat = 0.0;
     const int top = (int)(__float_as_uint(4.0f) >> 21);
     for (int b = 0; b < kBuckets; ++b) {
@@ -277,10 +281,11 @@ __global__ void bucket_scan_kernel(uint32_t* __restrict__ hist, uint32_t* __rest
       est_pairs += (double)c * fmin(n_tile, 0.5 * n_tile * (1.0 - cos((double)r_lo)));
       if (b <= b_block) e_block = run;
       if (b <= b_warp) e_warp = run;
+      if (b < b_fast) e_fast = run;
       if (b <= b_mat && run <= cap_rows) { e_mat = run; est_at_mat = est_pairs; }
     }
     if (est_at_mat * 90.0 < nvt * 256.0) e_mat = 0;
-    n_small[0] = run; n_small[1] = e_block; n_small[2] = e_warp; n_small[3] = e_mat;
+    n_small[0] = run; n_small[1] = e_block; n_small[2] = e_warp; n_small[3] = e_mat; n_small[4] = e_fast;
   }
 }
 
@@ -584,7 +589,7 @@ ring_query_batch_kernel(QueryParams qp, int which /*0: rc_warp class, 1: rc_thre
   BatchRec* rec = reinterpret_cast<BatchRec*>(smem_raw);
   int2* tab = reinterpret_cast<int2*>(smem_raw + sizeof(BatchRec) * G);
   const int rc = which == 0 ? qp.rc_warp : qp.rc_thread;
-  const uint32_t begin = which == 0 ? n_small[1] : n_small[2], end = which == 0 ? n_small[2] : n_small[0];
+  const uint32_t begin = which == 0 ? n_small[1] : n_small[2], end = which == 0 ? n_small[2] : n_small[4];      // [n_small[4], n_small[0]): window class
   const int N = 1 << qp.kq, tid = threadIdx.x;
   for (uint32_t b0 = begin + blockIdx.x * G; b0 < end; b0 += gridDim.x * G) {
     const int ng = min((uint32_t)G, end - b0);
@@ -835,6 +840,48 @@ ring_query_block_kernel(QueryParams qp, const float* __restrict__ dir, const flo
   }
 }
 
+// ---------------------------------------------------------------------------------------------- window class: the smallest discs
+// perm[n_small[4], n_small[0]): one thread per disc (uts_window_query.cuh); neighbouring threads hold discs of the same radius
+// bucket, so their windows have the same size.  The count pass remembers up to kTileCacheK tiles per disc, the emit pass replays
+// them (a 7 x 7 window can hold more: such a disc is queried again).
+constexpr int kWindowThreads = 128;
+template <bool EMIT>
+__global__ void __launch_bounds__(kWindowThreads)
+window_query_kernel(QueryParams qp, const float* __restrict__ dir, const float* __restrict__ rho, const float* __restrict__ rs,
+                    const int32_t* __restrict__ slot_of_tile, const uint32_t* __restrict__ perm, const uint32_t* __restrict__ n_small,
+                    const uint32_t* __restrict__ emit_rank, uint32_t* __restrict__ counts, const uint64_t* __restrict__ offsets,
+                    uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+  const uint64_t idx = (uint64_t)n_small[4] + (uint64_t)blockIdx.x * kWindowThreads + threadIdx.x;
+  if (idx >= (uint64_t)n_small[0]) return;
+  const int64_t k = (int64_t)perm[idx];
+  const int64_t slot = emit_rank ? (int64_t)emit_rank[k] : k;
+  const int v = (int)(k / qp.P);
+  const uint64_t hi = (uint64_t)v * (uint64_t)qp.n_tile;
+  const uint32_t depth = __float_as_uint(__ldg(rho + k)), gid = (uint32_t)(k - (int64_t)v * qp.P);           // reading A10
+  uint32_t* cache = qp.tile_cache + (size_t)k * kTileCacheK;
+  uint64_t b0 = 0;
+  if (EMIT) {
+    b0 = offsets[slot];
+    const uint64_t cnt = offsets[slot + 1] - b0;
+    if (cnt == 0) return;
+    if (cnt <= (uint64_t)kTileCacheK) {
+      for (uint32_t j = 0; j < (uint32_t)cnt; ++j) { keys[b0 + j] = ((hi + cache[j]) << 32) | depth; vals[b0 + j] = gid; }   // Alg.1 l.12: ((t, rho), i)
+      return;
+    }
+  }
+  const float d[3] = {__ldg(dir + 3 * k), __ldg(dir + 3 * k + 1), __ldg(dir + 3 * k + 2)};
+  WindowDisc D;
+  make_window_disc(qp.kt, d, fmin(kPi, (double)__ldg(rs + k) + qp.rho_q), qp.rho_t, D);
+  D.w = min(D.w, qp.w_max);               // the class holds R <= 0.98 (1 - 1e-6) kWindowWidth w_max / N_t: a last-ulp excess stays inside the margin
+  uint32_t pos = 0;
+  window_query(D, qp.kt, qp.kq, slot_of_tile, [&](uint32_t tile) {
+    if (EMIT) { keys[b0 + pos] = ((hi + tile) << 32) | depth; vals[b0 + pos] = gid; }
+    else if (pos < (uint32_t)kTileCacheK) cache[pos] = tile;
+    ++pos;
+  });
+  if (!EMIT) counts[slot] = pos;
+}
+
 }  // namespace uts
 
 #include "uts_tile_matrix.cuh"
@@ -929,6 +976,7 @@ struct QueryRun {
   unsigned agrid, wgrid, bgrid, agrid_e, wgrid_e, bgrid_e;
   static constexpr int kBatchA = 128, kBatchB = 32;          // discs per batch: rc_thread class, rc_warp class
   int b_mat; uint32_t cap_rows;                              // matrix class of uts_tile_lists (b_mat < 0: none)
+  int b_fast;                                                // window class: radius buckets >= b_fast (kBuckets: none)
   DeviceCtx* ctx;
   enum { kOccBlock0 = 1, kOccBlock1, kOccB0, kOccB1, kOccA0, kOccA1, kOccMat };
 
@@ -936,13 +984,14 @@ struct QueryRun {
     cfg = cfg_; in = in_; mask = mask_; emit_rank = emit_rank_; s = s_;
     ctx = device_ctx();
     if (!ctx) return UTS_ERR_CUDA;
-    const uts_tuning tn = tuning ? *tuning : uts_tuning{0, 0.f, 0, 0, 0.f};
+    const uts_tuning tn = tuning ? *tuning : uts_tuning{0, 0.f, 0, 0, 0.f, 0};
     d = dims_of(cfg, &mask);
     n = (int64_t)d.P * d.V;
     b_mat = -1; cap_rows = 0;
     qp.kt = d.kt; qp.kq = d.kq; qp.P = d.P; qp.V = d.V; qp.n_tile = d.n_tile;
     const double* rm = rho_max_table_host();
     qp.rho_q = cfg->query_mode == UTS_QUERY_RING ? 0.0 : rm[d.kq];      // Alg.3's set has no PixRad margin
+    qp.rho_t = rm[d.kt];
     for (int o = 0; o <= kMaxOrder; ++o) { qp.rho[o] = (float)rm[o]; qp.sin_hrho[o] = (float)sin(0.5 * rm[o]); qp.cos_hrho[o] = (float)cos(0.5 * rm[o]); }
     // Implementation choice: the ring-interval path (uts_ring_query.cuh) whenever a block's ring table fits shared memory
     // (k_q <= 12); the quadtree descent (Alg.2's depth-first form) otherwise, or when uts_tuning.query_impl = 1 asks for it.
@@ -953,6 +1002,14 @@ struct QueryRun {
     qp.b_warp = radius_bucket_host((float)((qp.rc_thread - 6) / (3.0 * Nq)));
     qp.b_block = radius_bucket_host((float)((qp.rc_warp - 6) / (3.0 * Nq)));
     if (qp.b_block > qp.b_warp) qp.b_block = qp.b_warp;
+    // window class (uts_window_query.cuh): discs of the thread class with R <= 0.98 kWindowWidth w_max / N_t, i.e. the
+    // radius buckets strictly below the one that holds that radius; needs N_t >= 2 kWindowMax + 1 so that the window's cells are distinct
+    b_fast = kBuckets;
+    qp.w_max = mask.slot_of_tile ? kWindowMax : 2;               // measured: see uts_window_query.cuh
+    if (ring_impl && !tn.window_off && (1 << d.kt) >= 2 * kWindowMax + 1) {
+      b_fast = radius_bucket_host((float)(0.98 * (1.0 - 1e-6) * kWindowWidth * qp.w_max / (double)(1 << d.kt))) + 1;
+      if (b_fast <= qp.b_warp) b_fast = qp.b_warp + 1;
+    }
     qp.active_tiles = mask.active_tiles; qp.n_active = mask.active_tiles ? mask.n_active : -1;
     qp.os = d.kt < 4 ? d.kt : 4;
     const size_t n_split = (size_t)12 << (2 * qp.os);
@@ -1039,7 +1096,7 @@ struct QueryRun {
     const unsigned cgrid = (unsigned)((n + 255) / 256);
     classify_kernel<0><<<cgrid, 256, 0, s>>>(qp, in.rs, in.flags, counts, list, n_large, hist, perm, emit_rank);
     UTS_LAUNCH_CHECK();
-    bucket_scan_kernel<<<1, 32, 0, s>>>(hist, n_small, qp.b_block, qp.b_warp, mp ? b_mat : -1, cap_rows, (double)d.n_tile, (double)d.n_tile * d.V);
+    bucket_scan_kernel<<<1, 32, 0, s>>>(hist, n_small, qp.b_block, qp.b_warp, mp ? b_mat : -1, ring_impl ? b_fast : kBuckets, cap_rows, (double)d.n_tile, (double)d.n_tile * d.V);
     UTS_LAUNCH_CHECK();
     classify_kernel<1><<<cgrid, 256, 0, s>>>(qp, in.rs, in.flags, counts, list, n_large, hist, perm, emit_rank);
     UTS_LAUNCH_CHECK();
@@ -1077,6 +1134,11 @@ struct QueryRun {
         ring_query_batch_kernel<kBatchA, false><<<agrid, kLargeThreads, smem_a, ctx->aux[1]>>>(qp, 1, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
                                                                                    emit_rank, counts, nullptr, nullptr, nullptr);
         UTS_LAUNCH_CHECK();
+        if (b_fast < kBuckets) {
+          window_query_kernel<false><<<(unsigned)((n + kWindowThreads - 1) / kWindowThreads), kWindowThreads, 0, ctx->aux[1]>>>(
+              qp, in.dir, in.rho, in.rs, mask.slot_of_tile, perm, n_small, emit_rank, counts, nullptr, nullptr, nullptr);
+          UTS_LAUNCH_CHECK();
+        }
         return UTS_OK;
       }();
       const int stj = join();
@@ -1106,6 +1168,11 @@ struct QueryRun {
         ring_query_batch_kernel<kBatchA, true><<<agrid_e, kLargeThreads, smem_a, ctx->aux[1]>>>(qp, 1, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
                                                                                   emit_rank, nullptr, offsets, keys, vals);
         UTS_LAUNCH_CHECK();
+        if (b_fast < kBuckets) {
+          window_query_kernel<true><<<(unsigned)((n + kWindowThreads - 1) / kWindowThreads), kWindowThreads, 0, ctx->aux[1]>>>(
+              qp, in.dir, in.rho, in.rs, mask.slot_of_tile, perm, n_small, emit_rank, nullptr, offsets, keys, vals);
+          UTS_LAUNCH_CHECK();
+        }
         return UTS_OK;
       }();
       const int stj = join();

@@ -184,26 +184,31 @@ def test_preprocess_in_two_calls_is_bit_identical():
 
 
 # ------------------------------------------------------------------------------------------- F2
+WINDOW = pytest.mark.parametrize("window", [True, False], ids=["window-path", "ring-intervals-only"])   # uts_tuning.window_off
+
+
+@WINDOW
 @pytest.mark.parametrize("cfg_id,P,order,extra", CASES)
-def test_tile_query_bit_exact(cfg_id, P, order, extra):
+def test_tile_query_bit_exact(cfg_id, P, order, extra, window):
     B, R = _gpu()
     c = Case.get(cfg_id, P, order, extra)
     cfg = _cfg(R, c.scene)
     proj, mask = c.gpu_proj(B), c.gpu_mask(B)
+    tn = None if window else B.Tuning(window_off=1)
     n_want = int(c.fw["keys"].shape[0])
     offsets = torch.empty(cfg.n_views * cfg.n_gauss + 1, dtype=torch.int64, device="cuda")
     scratch = torch.empty(B.uts_tile_query_scratch_bytes(cfg) // 8 + 32, dtype=torch.int64, device="cuda")
     # count-only call
-    n = B.uts_tile_query(cfg, proj, mask, offsets, None, None, 0, scratch)
+    n = B.uts_tile_query(cfg, proj, mask, offsets, None, None, 0, scratch, tuning=tn)
     assert n == n_want
     assert np.array_equal(u64(offsets), c.fw["offsets"])
     # capacity too small -> error carrying the needed size
     keys = torch.empty(max(n, 1), dtype=torch.int64, device="cuda"); vals = torch.empty(max(n, 1), dtype=torch.int32, device="cuda")
     if n > 1:
         with pytest.raises(B.UtsError) as ei:
-            B.uts_tile_query(cfg, proj, mask, offsets, keys, vals, n - 1, scratch)
+            B.uts_tile_query(cfg, proj, mask, offsets, keys, vals, n - 1, scratch, tuning=tn)
         assert ei.value.status == B.UTS_ERR_CAPACITY and ei.value.needed == n
-    n = B.uts_tile_query(cfg, proj, mask, offsets, keys, vals, n, scratch)
+    n = B.uts_tile_query(cfg, proj, mask, offsets, keys, vals, n, scratch, tuning=tn)
     gk, gv = canon_pairs(u64(offsets), u64(keys), u32(vals))
     assert np.array_equal(gk, c.fw["keys"])
     assert np.array_equal(gv, c.fw["vals"])
@@ -267,6 +272,72 @@ def test_tile_query_order13_refine16_takes_the_descent(mode, P, seed):
     assert np.array_equal(u64(offsets), off)
     gk, gv = canon_pairs(u64(offsets), u64(gkeys), u32(gvals))
     assert np.array_equal(gk, keys) and np.array_equal(gv, vals)
+
+
+@pytest.mark.parametrize("mode", [0, 1], ids=["nested", "ring-set"])
+@pytest.mark.parametrize("order,refine,masked", [(8, 2, False), (9, 2, True), (8, 0, False), (8, 4, False), (12, 2, False)])
+def test_tile_query_window_path_small_discs_everywhere(order, refine, masked, mode):
+    """The tile-window path (uts_window_query.cuh) on discs it is made for: 6000 small discs, among them centres ON and next to the
+    poles, the vertices shared by three and by four faces and the meridian face edges, radii up to the largest the path accepts (so
+    that 3 x 3, 5 x 5 and 7 x 7 windows all occur), with a cap mask or without; emission ranks from uts_depth_order; count-only, then
+    emit.  Against the oracle's sets, bit for bit; the same call with window_off must give the same arrays."""
+    B, R = _gpu()
+    n = 6000
+    scene = small_scene(3 if masked else 4, n, order, n_views=1)
+    if not masked:
+        scene["mask"] = None
+    oc = ocfg(scene, query_refine_log2=refine, query_mode=mode)
+    bits, act, slot = oracle_mask(oc, scene)
+    pr = orc.preprocess(oc, scene["means"], scene["scales"], scene["quats"], scene["opac"], scene["sh"], scene["W"], scene["b"])
+    rng = np.random.default_rng(order * 10 + refine)
+    Nt = 1 << oc.tile_order
+    d = pr.dir[0].astype(np.float64)
+    special = [[0, 1, 0], [0, -1, 0]]
+    for sgn in (1, -1):
+        for c in range(4):
+            lam = c * np.pi / 2
+            special.append([np.sqrt(5) / 3 * np.sin(lam), sgn * 2 / 3, np.sqrt(5) / 3 * np.cos(lam)])       # 3-face vertices (camera frame)
+    for c in range(4):
+        lam = np.pi / 4 + c * np.pi / 2
+        special.append([np.sin(lam), 0.0, np.cos(lam)])                                                     # 4-face vertices
+    special = np.array(special)
+    k = special.shape[0]
+    for rep in range(40):
+        d[rep * k:(rep + 1) * k] = special + (0.0 if rep == 0 else 0.8 / Nt) * rng.standard_normal((k, 3))
+    zz = rng.uniform(0.67, 0.9999, 300) * rng.choice([-1, 1], 300); lam = rng.integers(0, 4, 300) * np.pi / 2
+    d[40 * k:40 * k + 300] = np.stack([np.sqrt(1 - zz * zz) * np.sin(lam), zz, np.sqrt(1 - zz * zz) * np.cos(lam)], 1)   # meridian face edges
+    d /= np.linalg.norm(d, axis=1, keepdims=True)
+    pr.dir[0] = d.astype(np.float32)
+    pr.lonlat[0, :, 0] = np.arctan2(d[:, 0], d[:, 2]).astype(np.float32)
+    pr.lonlat[0, :, 1] = np.arctan2(d[:, 1], np.hypot(d[:, 0], d[:, 2])).astype(np.float32)
+    rho_q = 0.0 if mode == 1 else orc.rho_max_closed(oc.tile_order + refine)
+    w = rng.integers(1, 4, n)
+    Rmax = 0.98 * 0.6 * w / Nt
+    Rr = np.where(rng.random(n) < 0.3, Rmax * (1 - 1e-3 * rng.random(n)), Rmax * rng.uniform(0.1, 1.0, n))
+    Rr[::50] *= 4.0                                                              # a few discs beyond the window class, mixed in
+    pr.rs[0] = np.maximum(Rr - rho_q, 1e-5).astype(np.float32)
+    pr.rho[0] = rng.uniform(0.5, 30.0, n).astype(np.float32)
+    pr.flags[0] = 0
+    pr.flags[0, 5::97] = 1                                                       # culled records in between
+    off, keys, vals, info = orc.tile_query(oc, pr, slot)
+    assert info["min_margin"] > 1e-12
+    cfg = _cfg(R, scene, query_refine_log2=refine, query_mode=mode)
+    mask = B.Mask.full() if bits is None else B.Mask(dev(act.view(np.int32)), int(act.shape[0]), dev(slot), dev(bits.view(np.int32)))
+    proj = B.Proj(dev(pr.dir), dev(pr.lonlat), dev(pr.rho), dev(pr.conic_opac), dev(pr.rs), dev(pr.rgb), dev(pr.flags))
+    got = []
+    for tn in (None, B.Tuning(window_off=1)):
+        r = R.Rasterizer(cfg, mask, depth_presort=True, fused_lists=False, tuning=tn, pair_capacity=16)
+        r.proj = proj
+        r.depth_order()
+        assert r.tile_query() == keys.shape[0]
+        rank = u32(r.emit_rank).astype(np.int64)
+        cnt = np.diff(u64(r.offsets).astype(np.int64))
+        assert np.array_equal(cnt[rank], np.diff(off.astype(np.int64)))          # per-Gaussian counts, in emission-rank order
+        r.sort(); r.tile_ranges()
+        wk, wv = orc.sort_pairs(keys, vals)
+        assert np.array_equal(u64(r.keys)[: r.n_pairs], wk) and np.array_equal(u32(r.vals)[: r.n_pairs], wv)
+        got.append((u64(r.keys)[: r.n_pairs].copy(), u32(r.vals)[: r.n_pairs].copy()))
+    assert np.array_equal(got[0][0], got[1][0]) and np.array_equal(got[0][1], got[1][1])
 
 
 @pytest.mark.parametrize("refine", [0, 1, 3, 4])
@@ -473,6 +544,25 @@ def test_render_fwd(cfg_id, P, order, extra, marks):
         pix = (c.act.astype(np.int64)[:, None] * ppt + np.arange(ppt)[None, :]).reshape(-1)
         on = ((c.bits[pix >> 5] >> (pix & 31).astype(np.uint32)) & 1).astype(bool)
         assert (color[:, ~on] == 0).all() and (alpha[:, ~on] == 0).all()
+
+
+@pytest.mark.parametrize("cfg_id,P,order,extra", [CASES[1], CASES[5]])
+def test_render_fwd_counted_matches_the_oracle_work_counters(cfg_id, P, order, extra):
+    """uts_render_fwd_counted (bench.py's work counters): same image as uts_render_fwd, and the evaluated / contributing pair counts
+    of Alg.1's loop equal the oracle's counters up to the few pixels whose decisions sit on a threshold."""
+    B, R = _gpu()
+    c = Case.get(cfg_id, P, order, extra)
+    r = _render_gpu(B, R, c, _cfg(R, c.scene), marks=False)
+    work = torch.zeros(2, dtype=torch.int64, device="cuda")
+    out = [torch.empty_like(t) for t in (r.color, r.alpha, r.trans, r.n_last)]
+    B.uts_render_fwd_counted(r.cfg, r.proj, r.mask, r.ranges, r.vals, *out, work)
+    for a, b in zip(out, (r.color, r.alpha, r.trans, r.n_last)):
+        assert torch.equal(a, b)
+    ev, contrib = (int(x) for x in work.cpu().tolist())
+    ctr = c.fw["counters"]
+    assert abs(ev - ctr["evaluated"]) <= 2e-3 * ctr["evaluated"] + 16, (ev, ctr)
+    assert abs(contrib - ctr["contributing"]) <= 2e-3 * ctr["contributing"] + 16, (contrib, ctr)
+    assert ev >= int(u32(r.n_last).astype(np.int64).sum())                # every entry before n_last was evaluated
 
 
 def test_render_fwd_background_and_no_thresholds():

@@ -44,3 +44,21 @@ def test_two_ranks_max_times_and_distinct_scenes():
 def test_single_process_is_identity():
     assert replicas.max_over_ranks([1.5, 2.5]) == [1.5, 2.5]
     assert replicas.world()[0] >= 1
+
+
+def test_bench_spawns_its_own_ranks_when_not_under_torchrun():
+    """`python bench.py --gpus 2` outside torchrun must start two ranks itself (the driver's torchrun command line) and print ONE line
+    with n_gpus = 2.  --impl selftest runs the rank plumbing on CPU with gloo (no kernel, no measurement)."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--impl", "selftest"], capture_output=True, text=True,
+                         timeout=300, env=env)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [json.loads(ln) for ln in out.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1 and lines[0]["n_gpus"] == 2 and lines[0]["max_over_ranks"] == [11.0, 5.0]
+    # one process: no spawn, n_gpus = 1
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--impl", "selftest"], capture_output=True, text=True, timeout=300, env=env)
+    assert out.returncode == 0 and json.loads(out.stdout.strip().splitlines()[-1])["n_gpus"] == 1

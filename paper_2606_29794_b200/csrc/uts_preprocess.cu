@@ -1,7 +1,7 @@
 // uts_preprocess.cu — F1 (Alg.1 l.2-8, Eq.1-2) and B2 (Eq.3-4).
 //
-// One thread per (view, Gaussian) forward, one thread per Gaussian backward (views summed in registers, so the
-// parameter gradients are written once, no atomics).  Both kernels are streaming: 236 B in + 57 B out per Gaussian
+// One thread per (view, Gaussian) forward, one thread per Gaussian backward (two kernels: geometry chain, colour path; views
+// summed in registers, so the parameter gradients are written once, no atomics).  Both kernels are streaming: 236 B in + 57 B out per Gaussian
 // forward at SH degree 3.  The geometry chain runs in double precision: it is ~1.5 k instructions per Gaussian, below
 // the HBM time of the 48 SH floats, and it makes the stored fp32 records (dir, rho, r_s) the correctly rounded
 // values, so that the integer stages downstream (tile query, sort key) see the same bits as a double reference.
@@ -240,76 +240,29 @@ preprocess_fwd_kernel(uts_config cfg, const float* __restrict__ means, const flo
 //   e = e(omega), n = n(omega,phi), u = u(omega,phi):  de/domega = -hh, dn/domega = -sin(phi) e, dn/dphi = -u,
 //   with hh = cos(phi) u - sin(phi) n the horizontal unit vector;  d omega/dt = e / rxz,  d phi/dt = n / rho,  d rho/dt = u.
 // The three paths of PAPER.md:91-96 (mu' path, J path, S_phi path) are this single chain written in the (e,n,u) frame.
-__global__ void __launch_bounds__(128, 4)
-preprocess_bwd_kernel(uts_config cfg, const float* __restrict__ means, const float* __restrict__ scales,
-                      const float* __restrict__ quats, const float* __restrict__ sh, const float* __restrict__ Wv,
-                      const float* __restrict__ bv, const uint8_t* __restrict__ flags, const float* __restrict__ dL_drgb,
-                      const float* __restrict__ dL_dconic, const float* __restrict__ dL_dmu2, float* __restrict__ dL_dmeans,
-                      float* __restrict__ dL_dscales, float* __restrict__ dL_dquats, float* __restrict__ dL_dsh, double h) {
+// Two kernels, one thread per Gaussian each, views summed in registers (no atomics, the sums are deterministic):
+//   preprocess_bwd_geo_kernel    the geometry chain (double precision, no SH): writes dL_dmeans (geometry part), dL_dscales, dL_dquats;
+//   preprocess_bwd_color_kernel  the colour path: dL_dsh accumulated over the views in registers and written once (48 floats at
+//                                degree 3, as float4), and the view-direction term added to dL_dmeans.
+// As one kernel the 128-register cap spilt 0.5 KB per thread and every further view read-modified-wrote the 192 B of dL_dsh
+// (config 5, 4 views: 2.2 ms for 1 M Gaussians); split, neither kernel spills.
+__global__ void __launch_bounds__(128)
+preprocess_bwd_geo_kernel(uts_config cfg, const float* __restrict__ means, const float* __restrict__ scales,
+                          const float* __restrict__ quats, const float* __restrict__ Wv, const float* __restrict__ bv,
+                          const uint8_t* __restrict__ flags, const float* __restrict__ dL_dconic, const float* __restrict__ dL_dmu2,
+                          float* __restrict__ dL_dmeans, float* __restrict__ dL_dscales, float* __restrict__ dL_dquats, double h) {
   const int P = cfg.n_gauss;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= P) return;
-  const int deg = cfg.sh_degree, M = (deg + 1) * (deg + 1);
   const double mu[3] = {(double)__ldg(means + 3 * i), (double)__ldg(means + 3 * i + 1), (double)__ldg(means + 3 * i + 2)};
   const double s[3] = {(double)__ldg(scales + 3 * i), (double)__ldg(scales + 3 * i + 1), (double)__ldg(scales + 3 * i + 2)};
   const float4 qf = __ldg(reinterpret_cast<const float4*>(quats) + i);
   const double q[4] = {(double)qf.x, (double)qf.y, (double)qf.z, (double)qf.w};
   double g_mu[3] = {0, 0, 0}, g_s[3] = {0, 0, 0}, g_q[4] = {0, 0, 0, 0};
-  const float* shp = sh + (size_t)i * 3 * M;
-  float* gsh = dL_dsh + (size_t)i * 3 * M;
   for (int v = 0; v < cfg.n_views; ++v) {
     const size_t k = (size_t)v * P + i;
-    const uint8_t fl = __ldg(flags + k);
-    const bool first = (v == 0);
-    if (fl & 1) {                                        // culled in this view: contributes nothing
-      if (first) for (int j = 0; j < 3 * M; ++j) gsh[j] = 0.f;
-      continue;
-    }
+    if (__ldg(flags + k) & 1) continue;                  // culled in this view: contributes nothing
     ViewConst vc; load_view(Wv, bv, v, vc);
-    // ---- colour path
-    const float gr[3] = {(fl & 2) ? 0.f : __ldg(dL_drgb + 3 * k), (fl & 4) ? 0.f : __ldg(dL_drgb + 3 * k + 1),
-                         (fl & 8) ? 0.f : __ldg(dL_drgb + 3 * k + 2)};
-    double vd[3] = {mu[0] - vc.cam[0], mu[1] - vc.cam[1], mu[2] - vc.cam[2]};
-    const double vl = sqrt(vd[0] * vd[0] + vd[1] * vd[1] + vd[2] * vd[2]);
-    vd[0] /= vl; vd[1] /= vl; vd[2] /= vl;
-    const float dx = (float)vd[0], dy = (float)vd[1], dz = (float)vd[2];
-    float Y[16];
-    sh_basis_eval<float>(deg, dx, dy, dz, Y);
-    float cmix[16];                                      // sum_ch g_ch sh[m,ch]
-    if (M == 16) {                                       // degree 3: 48 floats = 12 aligned float4 in and out
-#pragma unroll
-      for (int m = 0; m < 16; ++m) cmix[m] = 0.f;
-      const float4* s4 = reinterpret_cast<const float4*>(shp);
-      float4* g4 = reinterpret_cast<float4*>(gsh);
-#pragma unroll
-      for (int j = 0; j < 12; ++j) {
-        const float4 c4 = __ldg(s4 + j);
-        const float cc[4] = {c4.x, c4.y, c4.z, c4.w};
-        float o4[4];
-#pragma unroll
-        for (int l = 0; l < 4; ++l) {
-          const int idx = 4 * j + l;                       // = 3 m + ch, compile-time after unrolling
-          cmix[idx / 3] += gr[idx % 3] * cc[l];
-          o4[l] = Y[idx / 3] * gr[idx % 3];
-        }
-        if (first) g4[j] = make_float4(o4[0], o4[1], o4[2], o4[3]);
-        else { float4 p4 = g4[j]; g4[j] = make_float4(p4.x + o4[0], p4.y + o4[1], p4.z + o4[2], p4.w + o4[3]); }
-      }
-    } else {
-      for (int m = 0; m < M; ++m) {
-        const float c0 = __ldg(shp + 3 * m), c1 = __ldg(shp + 3 * m + 1), c2 = __ldg(shp + 3 * m + 2);
-        cmix[m] = gr[0] * c0 + gr[1] * c1 + gr[2] * c2;
-        if (first) { gsh[3 * m] = Y[m] * gr[0]; gsh[3 * m + 1] = Y[m] * gr[1]; gsh[3 * m + 2] = Y[m] * gr[2]; }
-        else { gsh[3 * m] += Y[m] * gr[0]; gsh[3 * m + 1] += Y[m] * gr[1]; gsh[3 * m + 2] += Y[m] * gr[2]; }
-      }
-    }
-    float gvx, gvy, gvz;
-    sh_dir_grad(deg, dx, dy, dz, cmix, gvx, gvy, gvz);
-    {  // vdir = v/|v|  =>  d vdir/d mu = (I - vdir vdir^T)/|v|
-      const double dot = gvx * vd[0] + gvy * vd[1] + gvz * vd[2];
-      g_mu[0] += (gvx - dot * vd[0]) / vl; g_mu[1] += (gvy - dot * vd[1]) / vl; g_mu[2] += (gvz - dot * vd[2]) / vl;
-    }
-    // ---- geometry path
     Geo g;
     geometry(vc, mu, s, q, (double)cfg.r_near, h, g);
     if (g.culled || g.pole) continue;                    // A22: only the colour path at an exact pole
@@ -378,6 +331,80 @@ preprocess_bwd_kernel(uts_config cfg, const float* __restrict__ means, const flo
   reinterpret_cast<float4*>(dL_dquats)[i] = make_float4((float)g_q[0], (float)g_q[1], (float)g_q[2], (float)g_q[3]);
 }
 
+// Colour path: rgb_ch = max(0, 1/2 + sum_m Y_m(vdir) sh[m,ch]) (reading A13).  dL_dmeans must hold the geometry part already.
+template <int DEG>
+__global__ void __launch_bounds__(128)
+preprocess_bwd_color_kernel(uts_config cfg, const float* __restrict__ means, const float* __restrict__ sh, const float* __restrict__ Wv,
+                            const float* __restrict__ bv, const uint8_t* __restrict__ flags, const float* __restrict__ dL_drgb,
+                            float* __restrict__ dL_dmeans, float* __restrict__ dL_dsh) {
+  constexpr int M = (DEG + 1) * (DEG + 1), NF = 3 * M;
+  const int P = cfg.n_gauss;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= P) return;
+  const double mu[3] = {(double)__ldg(means + 3 * i), (double)__ldg(means + 3 * i + 1), (double)__ldg(means + 3 * i + 2)};
+  const float* shp = sh + (size_t)i * NF;
+  float* gsh = dL_dsh + (size_t)i * NF;
+  float acc[NF];                                         // dL_dsh of this Gaussian, [m][ch], summed over the views
+#pragma unroll
+  for (int j = 0; j < NF; ++j) acc[j] = 0.f;
+  double g_mu[3] = {0, 0, 0};
+  for (int v = 0; v < cfg.n_views; ++v) {
+    const size_t k = (size_t)v * P + i;
+    const uint8_t fl = __ldg(flags + k);
+    if (fl & 1) continue;
+    const float gr[3] = {(fl & 2) ? 0.f : __ldg(dL_drgb + 3 * k), (fl & 4) ? 0.f : __ldg(dL_drgb + 3 * k + 1),
+                         (fl & 8) ? 0.f : __ldg(dL_drgb + 3 * k + 2)};
+    // camera centre -W^T b of this view
+    double cam[3];
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+      cam[r] = -((double)__ldg(Wv + 9 * v + r) * (double)__ldg(bv + 3 * v) + (double)__ldg(Wv + 9 * v + 3 + r) * (double)__ldg(bv + 3 * v + 1) +
+                 (double)__ldg(Wv + 9 * v + 6 + r) * (double)__ldg(bv + 3 * v + 2));
+    double vd[3] = {mu[0] - cam[0], mu[1] - cam[1], mu[2] - cam[2]};
+    const double vl = sqrt(vd[0] * vd[0] + vd[1] * vd[1] + vd[2] * vd[2]);
+    vd[0] /= vl; vd[1] /= vl; vd[2] /= vl;
+    const float dx = (float)vd[0], dy = (float)vd[1], dz = (float)vd[2];
+    float Y[16];
+    sh_basis_eval<float>(DEG, dx, dy, dz, Y);
+    float cmix[16];                                      // sum_ch g_ch sh[m,ch]; the coefficients are re-read per view (L1 / L2 hits)
+#pragma unroll
+    for (int m = 0; m < M; ++m) cmix[m] = 0.f;
+    if (DEG == 3) {                                      // 48 floats = 12 aligned float4
+#pragma unroll
+      for (int j = 0; j < NF / 4; ++j) {
+        const float4 c4 = __ldg(reinterpret_cast<const float4*>(shp) + j);
+        const float cc[4] = {c4.x, c4.y, c4.z, c4.w};
+#pragma unroll
+        for (int l = 0; l < 4; ++l) {
+          const int idx = 4 * j + l;                     // = 3 m + ch, compile-time after unrolling
+          cmix[idx / 3] = fmaf(gr[idx % 3], cc[l], cmix[idx / 3]);
+          acc[idx] = fmaf(Y[idx / 3], gr[idx % 3], acc[idx]);
+        }
+      }
+    } else {
+#pragma unroll
+      for (int idx = 0; idx < NF; ++idx) {
+        cmix[idx / 3] = fmaf(gr[idx % 3], __ldg(shp + idx), cmix[idx / 3]);
+        acc[idx] = fmaf(Y[idx / 3], gr[idx % 3], acc[idx]);
+      }
+    }
+    float gvx, gvy, gvz;
+    sh_dir_grad(DEG, dx, dy, dz, cmix, gvx, gvy, gvz);
+    // vdir = v/|v|  =>  d vdir/d mu = (I - vdir vdir^T)/|v|
+    const double dot = gvx * vd[0] + gvy * vd[1] + gvz * vd[2];
+    g_mu[0] += (gvx - dot * vd[0]) / vl; g_mu[1] += (gvy - dot * vd[1]) / vl; g_mu[2] += (gvz - dot * vd[2]) / vl;
+  }
+  if (DEG == 3) {
+#pragma unroll
+    for (int j = 0; j < NF / 4; ++j) reinterpret_cast<float4*>(gsh)[j] = make_float4(acc[4 * j], acc[4 * j + 1], acc[4 * j + 2], acc[4 * j + 3]);
+  } else {
+#pragma unroll
+    for (int j = 0; j < NF; ++j) gsh[j] = acc[j];
+  }
+#pragma unroll
+  for (int r = 0; r < 3; ++r) dL_dmeans[3 * i + r] = (float)((double)dL_dmeans[3 * i + r] + g_mu[r]);
+}
+
 }  // namespace uts
 
 using namespace uts;
@@ -430,9 +457,17 @@ int uts_preprocess_bwd(const uts_config* cfg, uts_gaussians g, uts_views views, 
   if (!dL_drgb || !dL_dconic || !dL_dmu2 || !dL_dmeans || !dL_dscales || !dL_dquats || !dL_dsh) return UTS_ERR_INVALID_ARG;
   if (cfg->n_gauss == 0) return UTS_OK;
   const double h = (double)cfg->cov_dilation_px2 * 4.0 * kPi / (double)((int64_t)12 << (2 * cfg->order));
-  preprocess_bwd_kernel<<<(cfg->n_gauss + 127) / 128, 128, 0, (cudaStream_t)stream>>>(
-      *cfg, g.means, g.scales, g.quats, g.sh, views.W, views.b, flags, dL_drgb, dL_dconic, dL_dmu2, dL_dmeans, dL_dscales,
-      dL_dquats, dL_dsh, h);
+  const unsigned grid = (unsigned)((cfg->n_gauss + 127) / 128);
+  cudaStream_t s = (cudaStream_t)stream;
+  preprocess_bwd_geo_kernel<<<grid, 128, 0, s>>>(*cfg, g.means, g.scales, g.quats, views.W, views.b, flags, dL_dconic, dL_dmu2, dL_dmeans,
+                                                 dL_dscales, dL_dquats, h);
+  UTS_LAUNCH_CHECK();
+  switch (cfg->sh_degree) {
+    case 0: preprocess_bwd_color_kernel<0><<<grid, 128, 0, s>>>(*cfg, g.means, g.sh, views.W, views.b, flags, dL_drgb, dL_dmeans, dL_dsh); break;
+    case 1: preprocess_bwd_color_kernel<1><<<grid, 128, 0, s>>>(*cfg, g.means, g.sh, views.W, views.b, flags, dL_drgb, dL_dmeans, dL_dsh); break;
+    case 2: preprocess_bwd_color_kernel<2><<<grid, 128, 0, s>>>(*cfg, g.means, g.sh, views.W, views.b, flags, dL_drgb, dL_dmeans, dL_dsh); break;
+    default: preprocess_bwd_color_kernel<3><<<grid, 128, 0, s>>>(*cfg, g.means, g.sh, views.W, views.b, flags, dL_drgb, dL_dmeans, dL_dsh); break;
+  }
   UTS_LAUNCH_CHECK();
   return UTS_OK;
 }

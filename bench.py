@@ -427,6 +427,34 @@ def run_ours(args):
     except Exception as e:      # measurement plumbing only
         extras["hssim_loss"] = dict(error=str(e))
 
+    # inverse radial depth as a fourth channel of the blend (not part of the step): the marked pair with and without it
+    try:
+        if not run_extras:
+            raise RuntimeError("skipped (--no-extras)")
+        depth = torch.empty_like(r.alpha)
+        g_d = torch.randn(r.alpha.shape, device="cuda")
+        G_ = r._alloc_grads()
+        invr = torch.empty(cfg.n_views, cfg.n_gauss, dtype=torch.float32, device="cuda")
+        legs = dict(fwd=lambda: r.render_fwd(), fwd_depth=lambda: B.uts_render_fwd_depth(cfg, r.proj, mask, r.ranges, r.vals, r.capacity, r.color, r.alpha, r.trans, r.n_last, depth, r.marks),
+                    bwd=lambda: r.render_bwd(gcol), bwd_depth=lambda: B.uts_render_bwd_depth(cfg, r.proj, mask, r.ranges, r.vals, r.capacity, r.trans, r.n_last, r.marks, gcol, None, g_d,
+                                                                                          G_["rgb"], G_["conic"], G_["mu2"], G_["opac"], invr))
+        tms = {}
+        for name, fn in legs.items():
+            for _ in range(2):
+                fn()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(5):
+                fn()
+            e1.record(); torch.cuda.synchronize()
+            tms[name + "_ms"] = e0.elapsed_time(e1) / 5
+        tms["overhead_fwd"] = tms["fwd_depth_ms"] / tms["fwd_ms"] - 1.0
+        tms["overhead_bwd"] = tms["bwd_depth_ms"] / tms["bwd_ms"] - 1.0
+        extras["depth_channel"] = tms
+        del depth, g_d, invr
+    except Exception as e:      # measurement plumbing only
+        extras["depth_channel"] = dict(error=str(e))
+
     # occlusion-bounded lists (not the step: Alg.1 builds the full lists): lists from the nearest `keep`
     # Gaussians, verified every time by uts_count_unsaturated — when no visible pixel is left open, image and gradients are exactly
     # the full lists' ones.  keep is found by doubling from P/256; the timed steps include the check.

@@ -273,10 +273,23 @@ int uts_build_camera_mask(const uts_config* cfg, uts_camera cam, uint32_t* pixel
  * depth image; uts_render_bwd on the same record with dL_dcolor = (dL/dD, 0, 0) returns dL/d(1/r_i) in dL_drgb[...,0] and the
  * depth loss's share of dL_dconic / dL_dmu2 / dL_dopac. */
 int uts_inv_depth_channel(const uts_config* cfg, const float* rho, const uint8_t* flags, float* chan, void* stream);
-/* d(1/r)/dt = -t / r^3 carried to the means: dL_dmeans [P,3] (+)= sum_v W_v^T (-t / r^3) dL_dchan[v,i,0].
+/* The same depth image as a FOURTH CHANNEL of the colour blend (one pass instead of two; the decisions, and so color / alpha /
+ * trans / n_last / marks, are those of uts_render_fwd[_marked]): depth [V,S*256] = sum_i T_i alpha_i / rho_i, 0 at masked-out pixels.
+ * marks == NULL: the plain pair.  in.rho is read as well.  The backward takes dL_ddepth [V,S*256] next to dL_dcolor and returns, besides
+ * uts_render_bwd's outputs (which now hold the colour loss's AND the depth loss's alpha-path terms), dL_dinvr [V,P] = dL/d(1/rho_i)
+ * (zeroed by the call; pass it to uts_inv_depth_bwd with chan_stride = 1). */
+int uts_render_fwd_depth(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
+                         uint64_t pair_capacity, float* color, float* alpha, float* trans, uint32_t* n_last, float* depth,
+                         uint32_t* marks, size_t marks_bytes, void* stream);
+int uts_render_bwd_depth(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
+                         uint64_t pair_capacity, const float* trans, const uint32_t* n_last, const uint32_t* marks,
+                         const float* dL_dcolor, const float* dL_dalpha, const float* dL_ddepth, float* dL_drgb, float* dL_dconic,
+                         float* dL_dmu2, float* dL_dopac, float* dL_dinvr, void* stream);
+/* d(1/r)/dt = -t / r^3 carried to the means: dL_dmeans [P,3] (+)= sum_v W_v^T (-t / r^3) dL_dchan[(v*P + i) * chan_stride].
+ * chan_stride = 3 for uts_render_bwd's dL_drgb on a depth-channel record, 1 for uts_render_bwd_depth's dL_dinvr.
  * accumulate != 0 adds to dL_dmeans (after uts_preprocess_bwd), 0 overwrites. */
 int uts_inv_depth_bwd(const uts_config* cfg, const float* means, uts_views views, const uint8_t* flags, const float* dL_dchan,
-                      int accumulate, float* dL_dmeans, void* stream);
+                      int chan_stride, int accumulate, float* dL_dmeans, void* stream);
 /* Radian-space density control buffer: rs_max[i] <- max(rs_max[i], rs[v,i]) over the views in which Gaussian i
  * is visible (not culled by uts_preprocess).  rs, flags: uts_preprocess's records; rs_max [P], caller-initialised. */
 int uts_rs_max_update(const uts_config* cfg, const float* rs, const uint8_t* flags, float* rs_max, void* stream);

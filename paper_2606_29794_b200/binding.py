@@ -21,7 +21,7 @@ UTS_OK, UTS_ERR_INVALID_ARG, UTS_ERR_CAPACITY, UTS_ERR_CUDA, UTS_ERR_UNSUPPORTED
 SYMBOLS = [
     "uts_preprocess", "uts_preprocess_geometry", "uts_preprocess_color", "uts_depth_order", "uts_depth_order_scratch_bytes", "uts_tile_query", "uts_tile_query_scratch_bytes", "uts_tile_lists", "uts_tile_lists_scratch_bytes", "uts_sort", "uts_sort_scratch_bytes",
     "uts_tile_ranges", "uts_render_fwd", "uts_render_fwd_counted", "uts_render_bwd", "uts_render_marks_bytes", "uts_render_fwd_marked", "uts_render_bwd_marked", "uts_preprocess_bwd", "uts_build_mask", "uts_pixel_centers",
-    "uts_rho_max_table", "uts_resample_fwd", "uts_resample_bwd", "uts_build_camera_mask", "uts_inv_depth_channel", "uts_inv_depth_bwd", "uts_rs_max_update", "uts_depth_prefix_flags", "uts_count_unsaturated", "uts_hssim_loss", "uts_hssim_scratch_bytes",
+    "uts_rho_max_table", "uts_resample_fwd", "uts_resample_bwd", "uts_build_camera_mask", "uts_inv_depth_channel", "uts_inv_depth_bwd", "uts_render_fwd_depth", "uts_render_bwd_depth", "uts_rs_max_update", "uts_depth_prefix_flags", "uts_count_unsaturated", "uts_hssim_loss", "uts_hssim_scratch_bytes",
     "uts_host_workspace_bytes", "uts_host_forward_backward", "uts_last_cuda_error", "uts_launch_count", "uts_strerror",
     "uts_version",
 ]
@@ -372,9 +372,30 @@ def uts_inv_depth_channel(cfg: Config, rho, flags, chan, stream=None):
 
 
 def uts_inv_depth_bwd(cfg: Config, means, views: Views, flags, dL_dchan, dL_dmeans, accumulate=True, stream=None):
+    """dL_dchan: [V,P,3] (uts_render_bwd's dL_drgb on a depth-channel record) or [V,P] (uts_render_bwd_depth's dL_dinvr)."""
     c = cfg.c()
+    stride = 3 if dL_dchan.dim() == 3 else 1
     _check(lib().uts_inv_depth_bwd(C.byref(c), _ptr(means, torch.float32), views.c(), _ptr(flags, torch.uint8), _ptr(dL_dchan, torch.float32),
-                                   C.c_int(1 if accumulate else 0), _ptr(dL_dmeans, torch.float32), _stream(stream)), "uts_inv_depth_bwd")
+                                   C.c_int(stride), C.c_int(1 if accumulate else 0), _ptr(dL_dmeans, torch.float32), _stream(stream)), "uts_inv_depth_bwd")
+
+
+def uts_render_fwd_depth(cfg: Config, proj: Proj, mask: Mask, ranges, vals, pair_capacity: int, color, alpha, trans, n_last, depth, marks=None, stream=None):
+    """Colour + inverse radial depth in one blend pass (marks=None: the plain pair)."""
+    c = cfg.c()
+    mb = 0 if marks is None else marks.numel() * marks.element_size()
+    _check(lib().uts_render_fwd_depth(C.byref(c), proj.c(), mask.c(), _ptr(ranges), _ptr(vals), C.c_uint64(pair_capacity), _ptr(color, torch.float32),
+                                      _ptr(alpha, torch.float32), _ptr(trans, torch.float32), _ptr(n_last), _ptr(depth, torch.float32), _ptr(marks),
+                                      C.c_size_t(mb), _stream(stream)), "uts_render_fwd_depth")
+
+
+def uts_render_bwd_depth(cfg: Config, proj: Proj, mask: Mask, ranges, vals, pair_capacity: int, trans, n_last, marks, dL_dcolor, dL_dalpha, dL_ddepth,
+                         dL_drgb, dL_dconic, dL_dmu2, dL_dopac, dL_dinvr, stream=None):
+    c = cfg.c()
+    _check(lib().uts_render_bwd_depth(C.byref(c), proj.c(), mask.c(), _ptr(ranges), _ptr(vals), C.c_uint64(pair_capacity), _ptr(trans, torch.float32),
+                                      _ptr(n_last), _ptr(marks), _ptr(dL_dcolor, torch.float32), _ptr(dL_dalpha, torch.float32),
+                                      _ptr(dL_ddepth, torch.float32), _ptr(dL_drgb, torch.float32), _ptr(dL_dconic, torch.float32),
+                                      _ptr(dL_dmu2, torch.float32), _ptr(dL_dopac, torch.float32), _ptr(dL_dinvr, torch.float32), _stream(stream)),
+           "uts_render_bwd_depth")
 
 
 def uts_rs_max_update(cfg: Config, rs, flags, rs_max, stream=None):

@@ -5,7 +5,9 @@
 // composite from `uts_proj.rgb`, so the depth image is uts_render_fwd on a record whose rgb is the channel (r^-1, 0, 0) built
 // here, and uts_render_bwd on the same record returns dL/d(r_i^-1) in dL_drgb[..., 0] together with the alpha-path terms of the
 // depth loss (dL_dconic, dL_dmu2, dL_dopac), which add to those of the colour loss.  uts_inv_depth_bwd then carries dL/d(r^-1)
-// to the means.  Streaming kernels, one thread per (view, Gaussian) or per Gaussian.
+// to the means.  That form costs a second blend pass; uts_render_fwd_depth / uts_render_bwd_depth (uts_render.cu) blend 1 / rho as a
+// FOURTH CHANNEL of the colour pass instead (+2 % forward, +7 % backward on config 4) and return dL/d(r^-1) as dL_dinvr [V,P],
+// which uts_inv_depth_bwd takes with chan_stride = 1.  Streaming kernels, one thread per (view, Gaussian) or per Gaussian.
 #include "uts_internal.cuh"
 
 namespace uts {
@@ -20,7 +22,7 @@ __global__ void inv_depth_channel_kernel(int64_t n, const float* __restrict__ rh
 
 // one thread per Gaussian, views summed in registers; double like the geometry chain of the preprocess
 __global__ void inv_depth_bwd_kernel(int P, int V, const float* __restrict__ means, const float* __restrict__ Wv, const float* __restrict__ bv,
-                                     const uint8_t* __restrict__ flags, const float* __restrict__ dL_dchan, int accumulate,
+                                     const uint8_t* __restrict__ flags, const float* __restrict__ dL_dchan, int chan_stride, int accumulate,
                                      float* __restrict__ dL_dmeans) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= P) return;
@@ -34,7 +36,7 @@ __global__ void inv_depth_bwd_kernel(int P, int V, const float* __restrict__ mea
     const double ty = (double)W[3] * mx + (double)W[4] * my + (double)W[5] * mz + (double)b[1];
     const double tz = (double)W[6] * mx + (double)W[7] * my + (double)W[8] * mz + (double)b[2];
     const double r2 = tx * tx + ty * ty + tz * tz;
-    const double s = -(double)__ldg(dL_dchan + 3 * k) / (r2 * sqrt(r2));      // dL/d(r^-1) * (-1/r^3)
+    const double s = -(double)__ldg(dL_dchan + (size_t)chan_stride * k) / (r2 * sqrt(r2));      // dL/d(r^-1) * (-1/r^3)
     gx += s * ((double)W[0] * tx + (double)W[3] * ty + (double)W[6] * tz);    // W^T (s t)
     gy += s * ((double)W[1] * tx + (double)W[4] * ty + (double)W[7] * tz);
     gz += s * ((double)W[2] * tx + (double)W[5] * ty + (double)W[8] * tz);
@@ -97,13 +99,13 @@ int uts_inv_depth_channel(const uts_config* cfg, const float* rho, const uint8_t
 }
 
 int uts_inv_depth_bwd(const uts_config* cfg, const float* means, uts_views views, const uint8_t* flags, const float* dL_dchan,
-                      int accumulate, float* dL_dmeans, void* stream) {
+                      int chan_stride, int accumulate, float* dL_dmeans, void* stream) {
   int st = check_config(cfg);
   if (st) return st;
   if (cfg->n_gauss == 0) return UTS_OK;
-  if (!means || !views.W || !views.b || !flags || !dL_dchan || !dL_dmeans) return UTS_ERR_INVALID_ARG;
+  if (!means || !views.W || !views.b || !flags || !dL_dchan || !dL_dmeans || chan_stride < 1) return UTS_ERR_INVALID_ARG;
   inv_depth_bwd_kernel<<<(unsigned)((cfg->n_gauss + 255) / 256), 256, 0, (cudaStream_t)stream>>>(cfg->n_gauss, cfg->n_views, means, views.W, views.b,
-                                                                                               flags, dL_dchan, accumulate, dL_dmeans);
+                                                                                               flags, dL_dchan, chan_stride, accumulate, dL_dmeans);
   UTS_LAUNCH_CHECK();
   return UTS_OK;
 }

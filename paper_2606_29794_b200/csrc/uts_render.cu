@@ -103,8 +103,8 @@ __device__ __forceinline__ float arc_over_sin(float t, float c) {
 //   g1 = (ex, ez, nx, ny)     e = (ex, 0, ez)
 //   g2 = (nz, ux, uy, uz)     uhat
 //   g3 = (qa, qb, qc, o)      -0.5 A log2e, -B log2e, -0.5 C log2e; opacity
-//   g4 = (r, g, b, id)        colour; id = Gaussian index as raw bits (backward)
-//   g5 = (sin phi, cos phi)   backward only
+//   g4 = (r, g, b, id | 1/rho)  colour; backward: Gaussian index as raw bits; forward with the depth channel: 1 / rho
+//   g5 = (sin phi, cos phi, 1/rho)   backward only
 constexpr uint32_t kRow = kBatch * 16u;               // bytes between rows
 struct TileFrame { double cx, cy, cz; };              // tile centre direction (order k_t pixel centre)
 
@@ -113,7 +113,7 @@ struct __align__(16) SEntries { float4 g[BWD ? 6 : 5][kBatch]; };
 
 template <bool BWD>
 __device__ __forceinline__ void stage_entry(SEntries<BWD>& S, int i, const TileFrame& tf, float amin, uint32_t id, float ux, float uy,
-                                            float uz, float4 co, float r, float g, float b) {
+                                            float uz, float4 co, float r, float g, float b, float inv_r) {
   const float dxf = (float)(tf.cx - (double)ux), dyf = (float)(tf.cy - (double)uy), dzf = (float)(tf.cz - (double)uz);
   const float rxz2 = ux * ux + uz * uz;
   float ex = 1.f, ez = 0.f;
@@ -129,8 +129,8 @@ __device__ __forceinline__ void stage_entry(SEntries<BWD>& S, int i, const TileF
   S.g[1][i] = make_float4(ex, ez, nx, ny);
   S.g[2][i] = make_float4(nz, hx, hy, hz);
   S.g[3][i] = make_float4(-0.5f * kLog2e * co.x, -kLog2e * co.y, -0.5f * kLog2e * co.z, co.w);
-  S.g[4][i] = make_float4(r, g, b, __uint_as_float(id));
-  if (BWD) S.g[5][i] = make_float4(hy, sqrtf(hx * hx + hz * hz), 0.f, 0.f);
+  S.g[4][i] = make_float4(r, g, b, BWD ? __uint_as_float(id) : inv_r);
+  if (BWD) S.g[5][i] = make_float4(hy, sqrtf(hx * hx + hz * hz), inv_r, 0.f);
 }
 
 struct Eval { float a, b, c, t, k, p2; };
@@ -194,9 +194,9 @@ __device__ __forceinline__ uint64_t mark_base(const RenderParams& rp, const Tile
 // Every thread stages PX entries of the batch, one after the other (issuing the gathers of several entries together was measured:
 // the extra registers cost more occupancy than the overlapped latency gives back).  Up to three null entries follow the last real
 // one, so that the walk can take entries four at a time: a = 1, qa = 1 give power > 0, which Alg.1 l.23 skips whatever the thresholds.
-template <int PX, bool BWD>
+template <int PX, bool BWD, bool DEPTH>
 __device__ __forceinline__ void stage_batch(SEntries<BWD>& S, const TileFrame& tf, const RenderParams& rp, const float* __restrict__ dir,
-                                            const float* __restrict__ conic_opac, const float* __restrict__ rgb,
+                                            const float* __restrict__ conic_opac, const float* __restrict__ rgb, const float* __restrict__ rho,
                                             const uint32_t* __restrict__ vals, uint64_t first, uint64_t n, size_t gbase) {
   constexpr int kThreads = kTilePix / PX;
 #pragma unroll 1
@@ -206,7 +206,7 @@ __device__ __forceinline__ void stage_batch(SEntries<BWD>& S, const TileFrame& t
       const size_t gi = gbase + id;
       stage_entry<BWD>(S, (int)e, tf, rp.amin, id, __ldg(dir + 3 * gi), __ldg(dir + 3 * gi + 1), __ldg(dir + 3 * gi + 2),
                        __ldg(reinterpret_cast<const float4*>(conic_opac) + gi), __ldg(rgb + 3 * gi), __ldg(rgb + 3 * gi + 1),
-                       __ldg(rgb + 3 * gi + 2));
+                       __ldg(rgb + 3 * gi + 2), DEPTH ? __fdiv_rn(1.0f, __ldg(rho + gi)) : 0.f);
     } else {
       if ((uint64_t)e < n + 3) {
         S.g[0][e] = make_float4(1.f, 0.f, 1.f, -3.0e38f); S.g[1][e] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -218,13 +218,15 @@ __device__ __forceinline__ void stage_batch(SEntries<BWD>& S, const TileFrame& t
 }
 
 // COUNT (uts_render_fwd_counted, measurement only): also adds the evaluated and the contributing (pixel, entry) pairs to work[0..1].
-template <int PX, bool MARK, bool COUNT = false>
+// DEPTH (uts_render_fwd_depth): a fourth blended channel, the inverse radial depth 1 / rho_i (reading A29).
+template <int PX, bool MARK, bool COUNT = false, bool DEPTH = false>
 __global__ void __launch_bounds__(kTilePix / PX)
 render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* __restrict__ conic_opac, const float* __restrict__ rgb,
                   const uint32_t* __restrict__ active_tiles, const uint32_t* __restrict__ mask_bits,
                   const uint64_t* __restrict__ ranges, const uint32_t* __restrict__ vals, float* __restrict__ color,
                   float* __restrict__ alpha_out, float* __restrict__ trans_out, uint32_t* __restrict__ n_last_out,
-                  uint32_t* __restrict__ marks, uint64_t plane_words, unsigned long long* __restrict__ work = nullptr) {
+                  uint32_t* __restrict__ marks, uint64_t plane_words, unsigned long long* __restrict__ work = nullptr,
+                  const float* __restrict__ rho = nullptr, float* __restrict__ depth_out = nullptr) {
   constexpr int kThreads = kTilePix / PX, kWarps = kThreads / 32;
   __shared__ SEntries<false> S;
   uint32_t n_eval = 0, n_contrib = 0;                 // COUNT only
@@ -235,11 +237,11 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
   const size_t gbase = (size_t)ts.v * rp.P;
   const int wid = threadIdx.x >> 5;
 
-  float T[PX], Cr[PX], Cg[PX], Cb[PX];
+  float T[PX], Cr[PX], Cg[PX], Cb[PX], Cd[PX];
   uint32_t n_last[PX];
   uint32_t open = 0;                                  // bit j: pixel j still takes entries
 #pragma unroll
-  for (int j = 0; j < PX; ++j) { T[j] = 1.f; Cr[j] = Cg[j] = Cb[j] = 0.f; n_last[j] = 0; if (ts.on[j]) open |= 1u << j; }
+  for (int j = 0; j < PX; ++j) { T[j] = 1.f; Cr[j] = Cg[j] = Cb[j] = Cd[j] = 0.f; n_last[j] = 0; if (ts.on[j]) open |= 1u << j; }
   const uint64_t len = ts.end - ts.start;
   const uint32_t sS = (uint32_t)__cvta_generic_to_shared(&S);
   uint32_t* mark_w = nullptr;                         // plane `wid` of this tile's run; patch j is kWarps j planes further
@@ -247,7 +249,7 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
   for (uint64_t b0 = 0; b0 < len; b0 += kBatch) {
     if (__syncthreads_and(open == 0)) break;          // every pixel of the tile saturated (or masked)
     const uint64_t left_n = len - b0;
-    stage_batch<PX, false>(S, tf, rp, dir, conic_opac, rgb, vals, ts.start + b0, left_n, gbase);
+    stage_batch<PX, false, DEPTH>(S, tf, rp, dir, conic_opac, rgb, rho, vals, ts.start + b0, left_n, gbase);
     __syncthreads();
     const int nb = (int)(left_n < (uint64_t)kBatch ? left_n : (uint64_t)kBatch);
     // The batch is walked in groups of 32 entries, one mark word per patch each.  Every four entries the warp finds out which
@@ -293,6 +295,7 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
             if (COUNT) ++n_contrib;
             const float w = T[j] * a;                 // Eq.6: c_i alpha_i prod_{j<i} (1 - alpha_j)
             Cr[j] = fmaf(w, g4.x, Cr[j]); Cg[j] = fmaf(w, g4.y, Cg[j]); Cb[j] = fmaf(w, g4.z, Cb[j]);
+            if (DEPTH) Cd[j] = fmaf(w, g4.w, Cd[j]);  // D = sum_i T_i alpha_i / rho_i, no background term
             T[j] = T[j] * (1.f - a);
             n_last[j] = (uint32_t)(b0 + jj) + 1u;
             if (T[j] < rp.teps) open &= ~(1u << j);   // Alg.1 l.27: test after the update
@@ -318,9 +321,11 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
     if (ts.on[j]) {
       color[3 * o] = fmaf(T[j], rp.bg[0], Cr[j]); color[3 * o + 1] = fmaf(T[j], rp.bg[1], Cg[j]); color[3 * o + 2] = fmaf(T[j], rp.bg[2], Cb[j]);
       alpha_out[o] = 1.f - T[j]; trans_out[o] = T[j]; n_last_out[o] = n_last[j];
+      if (DEPTH) depth_out[o] = Cd[j];
     } else {
       color[3 * o] = 0.f; color[3 * o + 1] = 0.f; color[3 * o + 2] = 0.f;
       alpha_out[o] = 0.f; trans_out[o] = 1.f; n_last_out[o] = 0u;
+      if (DEPTH) depth_out[o] = 0.f;
     }
   }
 }
@@ -335,14 +340,15 @@ __device__ __forceinline__ float warp_sum(float x) {
 #ifndef UTS_BWD_MINB
 #define UTS_BWD_MINB 8   // 8 blocks of 64 threads per SM: 128 registers; at 138 registers (7 blocks) the kernel takes 5.0 instead of 4.4 ms
 #endif
-template <int PX, bool MARK>
+template <int PX, bool MARK, bool DEPTH = false>
 __global__ void __launch_bounds__(kTilePix / PX, UTS_BWD_MINB)
 render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* __restrict__ conic_opac, const float* __restrict__ rgb,
                   const uint32_t* __restrict__ active_tiles, const uint32_t* __restrict__ mask_bits,
                   const uint64_t* __restrict__ ranges, const uint32_t* __restrict__ vals, const float* __restrict__ trans,
                   const uint32_t* __restrict__ n_last_in, const float* __restrict__ dL_dcolor, const float* __restrict__ dL_dalpha,
                   float* __restrict__ dL_drgb, float* __restrict__ dL_dconic, float* __restrict__ dL_dmu2, float* __restrict__ dL_dopac,
-                  const uint32_t* __restrict__ marks, uint64_t plane_words) {
+                  const uint32_t* __restrict__ marks, uint64_t plane_words, const float* __restrict__ rho = nullptr,
+                  const float* __restrict__ dL_ddepth = nullptr, float* __restrict__ dL_dinvr = nullptr) {
   constexpr int kThreads = kTilePix / PX, kWarps = kThreads / 32;
   __shared__ SEntries<true> S;
   __shared__ TileFrame s_tf;
@@ -355,6 +361,7 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
 
   uint32_t nl[PX];
   float T[PX], Sr[PX], Sg[PX], Sb[PX], gr[PX], gg[PX], gb[PX], ga_T[PX];
+  float Sd[PX], gd[PX];                                 // DEPTH: depth accumulated behind the entry; upstream dL/dD
   uint32_t m = 0;
 #pragma unroll
   for (int j = 0; j < PX; ++j) {
@@ -366,6 +373,7 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
     ga_T[j] = (dL_dalpha && on) ? __ldg(dL_dalpha + o) * Tfin : 0.f;          // dL/dalpha_out * T_final
     T[j] = Tfin;                                        // transmittance after the entry being visited
     Sr[j] = Tfin * rp.bg[0]; Sg[j] = Tfin * rp.bg[1]; Sb[j] = Tfin * rp.bg[2];  // colour accumulated behind it
+    Sd[j] = 0.f; gd[j] = (DEPTH && on) ? __ldg(dL_ddepth + o) : 0.f;
     m = max(m, nl[j]);
   }
   // block maximum of n_last: entries beyond it were reached by no pixel
@@ -384,7 +392,8 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
   float* lane_dst = (vi < 3 ? dL_drgb + vi : vi < 6 ? dL_dconic + (vi - 3) : dL_dmu2 + (vi - 6)) + (size_t)(vi < 6 ? 3 : 2) * gbase;
   uint32_t lane_stride = vi < 6 ? 3u : 2u;
   if (lane == 1) { lane_dst = dL_dopac; lane_stride = 1u; }                    // lane 1 owns the opacity sum (summed over views)
-  const bool lane_owns = (lane & 3) == 0 || lane == 1;
+  if (DEPTH && lane == 2) { lane_dst = dL_dinvr + gbase; lane_stride = 1u; }   // lane 2 the 1/rho sum
+  const bool lane_owns = (lane & 3) == 0 || lane == 1 || (DEPTH && lane == 2);
   asm volatile("" : "+l"(lane_dst));                   // keep the per-view base folded into the pointer (one IMAD.WIDE per atomic)
   const uint32_t sS = (uint32_t)__cvta_generic_to_shared(&S);
 
@@ -400,7 +409,7 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
     uint32_t myw = 0u;
     if (MARK && lane < 8 * PX) myw = __ldg(mark_w + (size_t)bi * 8 + (lane & 7));
     __syncthreads();
-    stage_batch<PX, true>(S, tf, rp, dir, conic_opac, rgb, vals, ts.start + b0, (uint64_t)(max_nl - b0), gbase);
+    stage_batch<PX, true, DEPTH>(S, tf, rp, dir, conic_opac, rgb, rho, vals, ts.start + b0, (uint64_t)(max_nl - b0), gbase);
     __syncthreads();
     const int nb = (int)min((uint32_t)kBatch, max_nl - b0);
     // one list entry for the patches in pm (bit j: patch j of this warp)
@@ -408,7 +417,9 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
       const uint32_t jl = b0 + (uint32_t)jj;
       const uint32_t sa = sS + (uint32_t)jj * 16u;
       const float4 g0v = lds128(sa), g1 = lds128(sa + kRow), g2 = lds128(sa + 2u * kRow), g3 = lds128(sa + 3u * kRow), g4 = lds128(sa + 4u * kRow);
-      float d_r = 0.f, d_g = 0.f, d_b = 0.f, d_A = 0.f, d_B = 0.f, d_C = 0.f, d_o = 0.f, d_om = 0.f, d_ph = 0.f;
+      float d_r = 0.f, d_g = 0.f, d_b = 0.f, d_A = 0.f, d_B = 0.f, d_C = 0.f, d_o = 0.f, d_om = 0.f, d_ph = 0.f, d_i = 0.f;
+      const float2 g5 = *reinterpret_cast<const float2*>(&S.g[5][jj]);
+      const float inv_r = DEPTH ? S.g[5][jj].z : 0.f;
       bool any_used = false;
 #pragma unroll
       for (int j = 0; j < PX; ++j) {
@@ -424,9 +435,14 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
         const float Tb = T[j] * inv1a;                 // transmittance before this entry
         const float w = Tb * a;
         d_r = fmaf(w, gr[j], d_r); d_g = fmaf(w, gg[j], d_g); d_b = fmaf(w, gb[j], d_b);
-        const float dLa = gr[j] * (Tb * g4.x - Sr[j] * inv1a) + gg[j] * (Tb * g4.y - Sg[j] * inv1a) + gb[j] * (Tb * g4.z - Sb[j] * inv1a) +
-                          ga_T[j] * inv1a;
+        float dLa = gr[j] * (Tb * g4.x - Sr[j] * inv1a) + gg[j] * (Tb * g4.y - Sg[j] * inv1a) + gb[j] * (Tb * g4.z - Sb[j] * inv1a) +
+                    ga_T[j] * inv1a;
         Sr[j] = fmaf(w, g4.x, Sr[j]); Sg[j] = fmaf(w, g4.y, Sg[j]); Sb[j] = fmaf(w, g4.z, Sb[j]);
+        if (DEPTH) {                                   // the fourth channel, same algebra as a colour channel with c_i = 1 / rho_i
+          d_i = fmaf(w, gd[j], d_i);
+          dLa = fmaf(gd[j], Tb * inv_r - Sd[j] * inv1a, dLa);
+          Sd[j] = fmaf(w, inv_r, Sd[j]);
+        }
         T[j] = Tb;
         if (raw > rp.amax) continue;                   // reading A7: no gradient through a clamped alpha
         d_o = fmaf(e2, dLa, d_o);                      // exp(power) dL/dalpha
@@ -448,7 +464,6 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
         }
         // a = e.w, b = n.w, c = u.w with de/dom = -hh, dn/dom = -sin(phi) e, du/dom = cos(phi) e, dn/dphi = -u, du/dphi = n,
         // and hh.w = cos(phi) c - sin(phi) b
-        const float2 g5 = *reinterpret_cast<const float2*>(&S.g[5][jj]);
         const float sp = g5.x, cp = g5.y;
         d_om += -g_a * (cp * ev.c - sp * ev.b) - g_b * sp * ev.a + g_c * cp * ev.a;
         d_ph += g_c * ev.b - g_b * ev.c;
@@ -480,7 +495,8 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
       v0 += __shfl_xor_sync(0xffffffffu, v0, 2);
       v0 += __shfl_xor_sync(0xffffffffu, v0, 1);
       d_o = warp_sum(d_o);
-      if (lane_owns) red_add_global(lane_dst + (size_t)__float_as_uint(g4.w) * lane_stride, lane == 1 ? d_o : v0);
+      if (DEPTH) d_i = warp_sum(d_i);
+      if (lane_owns) red_add_global(lane_dst + (size_t)__float_as_uint(g4.w) * lane_stride, lane == 1 ? d_o : ((DEPTH && lane == 2) ? d_i : v0));
     };
     if (MARK) {
       for (int grp = (nb - 1) >> 5; grp >= 0; --grp) {
@@ -630,6 +646,68 @@ int uts_render_bwd_marked(const uts_config* cfg, uts_proj in, uts_mask mask, con
   if (!marks || check_config(cfg) != UTS_OK) return UTS_ERR_INVALID_ARG;
   return render_bwd_impl(cfg, in, mask, ranges, vals, trans, n_last, dL_dcolor, dL_dalpha, dL_drgb, dL_dconic, dL_dmu2, dL_dopac, marks,
                          mark_plane_words(cfg, pair_capacity), stream);
+}
+
+// ---- colour + inverse radial depth in one blend pass
+int uts_render_fwd_depth(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
+                         uint64_t pair_capacity, float* color, float* alpha, float* trans, uint32_t* n_last, float* depth,
+                         uint32_t* marks, size_t marks_bytes, void* stream) {
+  int st = check_config(cfg);
+  if (st) return st;
+  if ((st = check_mask(cfg, mask))) return st;
+  if (!in.dir || !in.conic_opac || !in.rgb || !in.rho || !ranges || !color || !alpha || !trans || !n_last || !depth) return UTS_ERR_INVALID_ARG;
+  uint64_t pw = 0;
+  if (marks) {
+    pw = mark_plane_words(cfg, pair_capacity);
+    if (marks_bytes < (size_t)pw * 8 * sizeof(uint32_t)) return UTS_ERR_CAPACITY;
+  }
+  Dims d = dims_of(cfg, &mask);
+  if (d.n_slot == 0) return UTS_OK;
+  if (d.n_slot * d.V > 0x7fffffffll) return UTS_ERR_UNSUPPORTED;
+  RenderParams rp = make_params(cfg, d);
+  const unsigned grid = (unsigned)(d.n_slot * d.V);
+  cudaStream_t s = (cudaStream_t)stream;
+  if (marks)
+    render_fwd_kernel<kFwdPx, true, false, true><<<grid, kTilePix / kFwdPx, 0, s>>>(rp, in.dir, in.conic_opac, in.rgb, mask.active_tiles, mask.pixel_mask_bits,
+                                                                                   ranges, vals, color, alpha, trans, n_last, marks, pw, nullptr, in.rho, depth);
+  else
+    render_fwd_kernel<kFwdPx, false, false, true><<<grid, kTilePix / kFwdPx, 0, s>>>(rp, in.dir, in.conic_opac, in.rgb, mask.active_tiles, mask.pixel_mask_bits,
+                                                                                    ranges, vals, color, alpha, trans, n_last, nullptr, 0, nullptr, in.rho, depth);
+  UTS_LAUNCH_CHECK();
+  return UTS_OK;
+}
+
+int uts_render_bwd_depth(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
+                         uint64_t pair_capacity, const float* trans, const uint32_t* n_last, const uint32_t* marks,
+                         const float* dL_dcolor, const float* dL_dalpha, const float* dL_ddepth, float* dL_drgb, float* dL_dconic,
+                         float* dL_dmu2, float* dL_dopac, float* dL_dinvr, void* stream) {
+  int st = check_config(cfg);
+  if (st) return st;
+  if ((st = check_mask(cfg, mask))) return st;
+  if (!in.dir || !in.conic_opac || !in.rgb || !in.rho || !ranges || !trans || !n_last || !dL_dcolor || !dL_ddepth) return UTS_ERR_INVALID_ARG;
+  if (!dL_drgb || !dL_dconic || !dL_dmu2 || !dL_dopac || !dL_dinvr) return UTS_ERR_INVALID_ARG;
+  Dims d = dims_of(cfg, &mask);
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t vp = (size_t)d.V * d.P;
+  UTS_CUDA(cudaMemsetAsync(dL_drgb, 0, vp * 3 * sizeof(float), s));
+  UTS_CUDA(cudaMemsetAsync(dL_dconic, 0, vp * 3 * sizeof(float), s));
+  UTS_CUDA(cudaMemsetAsync(dL_dmu2, 0, vp * 2 * sizeof(float), s));
+  UTS_CUDA(cudaMemsetAsync(dL_dopac, 0, (size_t)d.P * sizeof(float), s));
+  UTS_CUDA(cudaMemsetAsync(dL_dinvr, 0, vp * sizeof(float), s));
+  if (d.n_slot == 0 || d.P == 0) return UTS_OK;
+  if (d.n_slot * d.V > 0x7fffffffll) return UTS_ERR_UNSUPPORTED;
+  RenderParams rp = make_params(cfg, d);
+  const unsigned grid = (unsigned)(d.n_slot * d.V);
+  if (marks)
+    render_bwd_kernel<kBwdPx, true, true><<<grid, kTilePix / kBwdPx, 0, s>>>(
+        rp, in.dir, in.conic_opac, in.rgb, mask.active_tiles, mask.pixel_mask_bits, ranges, vals, trans, n_last, dL_dcolor, dL_dalpha, dL_drgb,
+        dL_dconic, dL_dmu2, dL_dopac, marks, mark_plane_words(cfg, pair_capacity), in.rho, dL_ddepth, dL_dinvr);
+  else
+    render_bwd_kernel<kBwdPx, false, true><<<grid, kTilePix / kBwdPx, 0, s>>>(
+        rp, in.dir, in.conic_opac, in.rgb, mask.active_tiles, mask.pixel_mask_bits, ranges, vals, trans, n_last, dL_dcolor, dL_dalpha, dL_drgb,
+        dL_dconic, dL_dmu2, dL_dopac, nullptr, 0, in.rho, dL_ddepth, dL_dinvr);
+  UTS_LAUNCH_CHECK();
+  return UTS_OK;
 }
 
 }  // extern "C"

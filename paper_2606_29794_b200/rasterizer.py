@@ -99,6 +99,22 @@ class Rasterizer:
         else:
             B.uts_render_fwd(self.cfg, self.proj, self.mask, self.ranges, self.vals, self.color, self.alpha, self.trans, self.n_last)
 
+    def render_fwd_depth(self):
+        """Colour + inverse radial depth in one blend pass; returns the depth image [V, S*256]."""
+        if getattr(self, "depth", None) is None:
+            self.depth = torch.empty_like(self.alpha)
+        B.uts_render_fwd_depth(self.cfg, self.proj, self.mask, self.ranges, self.vals, self.capacity, self.color, self.alpha, self.trans, self.n_last,
+                               self.depth, self.marks if self.use_marks else None)
+        return self.depth
+
+    def render_bwd_depth(self, dL_dcolor, dL_ddepth, dL_dalpha=None):
+        """Backward of render_fwd_depth: grads["rgb" / "conic" / "mu2" / "opac"] hold both losses' terms, grads["invr"] = dL/d(1/rho) [V,P]."""
+        G = self._alloc_grads()
+        if "invr" not in G:
+            G["invr"] = _f32(self.cfg.n_views, self.cfg.n_gauss, dev=self.dev)
+        B.uts_render_bwd_depth(self.cfg, self.proj, self.mask, self.ranges, self.vals, self.capacity, self.trans, self.n_last,
+                               self.marks if self.use_marks else None, dL_dcolor, dL_dalpha, dL_ddepth, G["rgb"], G["conic"], G["mu2"], G["opac"], G["invr"])
+
     def _alloc_grads(self):
         if self.grads is None:
             V, P, M, d = self.cfg.n_views, self.cfg.n_gauss, self.cfg.n_sh, self.dev

@@ -24,8 +24,8 @@
  *   - All work is enqueued on `stream` (a cudaStream_t passed as void*); calls are asynchronous.  Where a host
  *     count is returned (h_n_pairs) the call synchronises the stream before returning, as documented there.
  *   - Library state: the last CUDA error code, the launch counter, and ONE CONTEXT PER DEVICE, created on the first call made with
- *     that device current and kept until the process ends: the SM count, cached occupancy numbers, two auxiliary streams with their
- *     fork / join events (uts_tile_query / uts_tile_lists run their three work shapes side by side on them and join back into
+ *     that device current and kept until the process ends: the SM count, cached occupancy numbers, three auxiliary streams with their
+ *     fork / join events (uts_tile_query / uts_tile_lists run independent kernels side by side on them and join back into
  *     `stream` before returning) and one copy stream with four events (uts_host_forward_backward).  A per-device mutex is held
  *     while a call enqueues on those streams, so calls may be issued from several threads and on several streams; they never
  *     read the environment.  No CPU fallback; sm_100 only.

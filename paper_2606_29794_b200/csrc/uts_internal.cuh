@@ -37,6 +37,8 @@ struct DeviceCtx {
   int device = -1, sms = 148;
   cudaStream_t aux[2] = {nullptr, nullptr};         // tile query: the three work shapes run side by side
   cudaEvent_t fork = nullptr, join[2] = {nullptr, nullptr};
+  cudaStream_t side = nullptr;                      // uts_tile_lists: matrix transpose + popcount beside the small pairs' emit + sort
+  cudaEvent_t side_fork = nullptr, side_join = nullptr;
   cudaStream_t copy = nullptr;                      // uts_host_forward_backward: copies off the critical path
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
   bool attrs_set[4] = {false, false, false, false}; // cudaFuncSetAttribute done, per translation unit (under mu)

@@ -1005,7 +1005,10 @@ struct QueryRun {
     // window class (uts_window_query.cuh): discs of the thread class with R <= 0.98 kWindowWidth w_max / N_t, i.e. the
     // radius buckets strictly below the one that holds that radius; needs N_t >= 2 kWindowMax + 1 so that the window's cells are distinct
     b_fast = kBuckets;
-    qp.w_max = mask.slot_of_tile ? kWindowMax : 2;               // measured: see uts_window_query.cuh
+#ifndef UTS_WIN_UNMASKED_MAX
+#define UTS_WIN_UNMASKED_MAX 2
+#endif
+    qp.w_max = mask.slot_of_tile ? kWindowMax : UTS_WIN_UNMASKED_MAX;   // measured: see uts_window_query.cuh
     if (ring_impl && !tn.window_off && (1 << d.kt) >= 2 * kWindowMax + 1) {
       b_fast = radius_bucket_host((float)(0.98 * (1.0 - 1e-6) * kWindowWidth * qp.w_max / (double)(1 << d.kt))) + 1;
       if (b_fast <= qp.b_warp) b_fast = qp.b_warp + 1;
@@ -1294,12 +1297,24 @@ int uts_tile_lists(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
     }
     return uts_tile_ranges(cfg, n_S, keys, ranges, stream);
   }
-  // ---- large discs: transpose the bit matrix, count per (view, tile)
+  // ---- large discs: transpose the bit matrix, count per (view, tile) — on the context's side stream, beside the small pairs' emit +
+  // sort + ranges below (HBM-bound against latency-bound: they overlap); joined back before the totals.  The guard joins on every
+  // exit path, so no work is ever left unjoined.
+  DeviceCtx* ctx = q.ctx;
+  std::lock_guard<std::recursive_mutex> side_lock(ctx->mu);
+  struct SideJoin {
+    DeviceCtx* c; cudaStream_t s; bool forked = false;
+    int join() { if (!forked) return UTS_OK; forked = false; UTS_CUDA(cudaEventRecord(c->side_join, c->side)); UTS_CUDA(cudaStreamWaitEvent(s, c->side_join, 0)); return UTS_OK; }
+    ~SideJoin() { join(); }
+  } side{ctx, s};
   {
+    UTS_CUDA(cudaEventRecord(ctx->side_fork, s));
+    UTS_CUDA(cudaStreamWaitEvent(ctx->side, ctx->side_fork, 0));
+    side.forked = true;
     dim3 grid((unsigned)((mp.n_words + 31) / 32), (unsigned)(n_mat / 256 + (uint64_t)d.V + 1));
-    matrix_transpose_kernel<<<grid, 256, 0, s>>>(mp, d.V, d.n_tile);
+    matrix_transpose_kernel<<<grid, 256, 0, ctx->side>>>(mp, d.V, d.n_tile);
     UTS_LAUNCH_CHECK();
-    matrix_popcount_kernel<<<(unsigned)sm_count() * 8, 256, 0, s>>>(mp, d.V, d.n_tile);
+    matrix_popcount_kernel<<<(unsigned)ctx->sms * 8, 256, 0, ctx->side>>>(mp, d.V, d.n_tile);
     UTS_LAUNCH_CHECK();
   }
   // ---- small discs: emit at keys_tmp / vals_tmp, sort there (ping-pong through keys / vals, free until the merge), their ranges
@@ -1309,6 +1324,7 @@ int uts_tile_lists(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
     if ((st = uts_sort(cfg, n_S, keys_tmp, vals_tmp, keys, vals, 1, sort_scratch, sort_scratch_bytes, stream))) return st;
   }
   if ((st = uts_tile_ranges(cfg, n_S, keys_tmp, s_ranges, stream))) return st;
+  if ((st = side.join())) return st;
   // ---- final ranges, then one warp per (view, tile) merges its large discs (bit vector) with its small pairs into keys / vals
   uint32_t* total = reinterpret_cast<uint32_t*>(sp + ML.total);
   uint64_t* start = reinterpret_cast<uint64_t*>(sp + ML.start);

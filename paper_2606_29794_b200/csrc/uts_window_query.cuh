@@ -13,7 +13,9 @@
 // candidate outside the mask costs one table read, where the ring path pays for rings and rows before it filters —, config 4 (no
 // mask) 8.53 -> 8.43 ms with windows up to 5 x 5 (7 x 7: 8.55): the work per disc grows with the window AREA times the 4^(k_q-k_t)
 // rim tests, so the ring intervals take over early on unmasked scenes.  (The gluing table must be `static`: as a plain constexpr
-// local it was copied to each thread's stack, and config 4 went to 12.3 ms.)
+// local it was copied to each thread's stack, and config 4 went to 12.3 ms.  Also measured: classifying all cells first and then
+// walking the rim tiles' query pixels in ONE flattened loop per lane (so that lanes whose tile was settled by the centre test do
+// not idle through the others' pixel loops; ncu shows 12 of 32 lanes active here) — no gain, config 5 3.9 -> 4.1 ms; not kept.)
 // Everything is __host__ __device__: tests/hostlogic drives the same code on the CPU against the oracle's sets.
 #pragma once
 #include "uts_internal.cuh"

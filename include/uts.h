@@ -141,6 +141,17 @@ int uts_preprocess_color(const uts_config* cfg, uts_gaussians g, uts_views views
 int uts_depth_order(const uts_config* cfg, const float* rho /*[V,P]*/, uint32_t* emit_rank /*[V*P]*/, void* scratch,
                     size_t scratch_bytes, void* stream);
 size_t uts_depth_order_scratch_bytes(const uts_config* cfg);
+/* uts_depth_order for callers that cannot allocate device memory (CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): the same kernels and the same emit_rank, bit for bit, with the scratch in a 7 MiB file-scope device array of the
+ * library (held by every GPU that loads the library until the process exits).  Limit: n_gauss * n_views <=
+ * UTS_DEPTH_ORDER_STATIC_MAX = uts_depth_order_static_max(); beyond it the call enqueues nothing and returns UTS_ERR_CAPACITY.
+ * The call itself allocates and frees nothing; the first call on a device looks the array's address up (cudaGetSymbolAddress) and
+ * creates the device context.  ALL calls share the one array, whose contents are those of the last call (nothing in it needs
+ * clearing: every region is written before it is read): two calls that overlap on the GPU — different streams, or graph branches
+ * without an edge between them — RACE; order them on one stream or with an event. */
+#define UTS_DEPTH_ORDER_STATIC_MAX 262144
+uint64_t uts_depth_order_static_max(void);
+int uts_depth_order_static(const uts_config* cfg, const float* rho /*[V,P]*/, uint32_t* emit_rank /*[V*P]*/, void* stream);
 
 /* Alg.1 l.9-14 with Alg.2 (reading A6) or, with cfg->query_mode = UTS_QUERY_RING, Alg.3.  The tile set of (v,i) is
  *     { q >> 2(k_q-k_t) : q an order-k_q NESTED pixel with  u . centre(q) >= cos R } ∩ active tiles,

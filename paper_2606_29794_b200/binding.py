@@ -19,7 +19,7 @@ UTS_OK, UTS_ERR_INVALID_ARG, UTS_ERR_CAPACITY, UTS_ERR_CUDA, UTS_ERR_UNSUPPORTED
 
 # every symbol include/uts.h declares
 SYMBOLS = [
-    "uts_preprocess", "uts_preprocess_geometry", "uts_preprocess_color", "uts_depth_order", "uts_depth_order_scratch_bytes", "uts_tile_query", "uts_tile_query_scratch_bytes", "uts_tile_lists", "uts_tile_lists_scratch_bytes", "uts_sort", "uts_sort_scratch_bytes",
+    "uts_preprocess", "uts_preprocess_geometry", "uts_preprocess_color", "uts_depth_order", "uts_depth_order_scratch_bytes", "uts_depth_order_static", "uts_depth_order_static_max", "uts_tile_query", "uts_tile_query_scratch_bytes", "uts_tile_lists", "uts_tile_lists_scratch_bytes", "uts_sort", "uts_sort_scratch_bytes",
     "uts_tile_ranges", "uts_render_fwd", "uts_render_fwd_counted", "uts_render_bwd", "uts_render_marks_bytes", "uts_render_fwd_marked", "uts_render_bwd_marked", "uts_preprocess_bwd", "uts_build_mask", "uts_pixel_centers",
     "uts_rho_max_table", "uts_resample_fwd", "uts_resample_bwd", "uts_build_camera_mask", "uts_inv_depth_channel", "uts_inv_depth_bwd", "uts_render_fwd_depth", "uts_render_bwd_depth", "uts_rs_max_update", "uts_depth_prefix_flags", "uts_count_unsaturated", "uts_hssim_loss", "uts_hssim_scratch_bytes",
     "uts_host_workspace_bytes", "uts_host_forward_backward", "uts_last_cuda_error", "uts_launch_count", "uts_strerror",
@@ -237,6 +237,20 @@ def uts_depth_order(cfg: Config, rho, emit_rank, scratch, stream=None):
     c = cfg.c()
     _check(lib().uts_depth_order(C.byref(c), _ptr(rho, torch.float32), _ptr(emit_rank, torch.int32), _ptr(scratch),
                                  C.c_size_t(scratch.numel() * scratch.element_size()), _stream(stream)), "uts_depth_order")
+
+
+def uts_depth_order_static_max() -> int:
+    lib().uts_depth_order_static_max.restype = C.c_uint64
+    return int(lib().uts_depth_order_static_max())
+
+
+def uts_depth_order_static(cfg: Config, rho, emit_rank, stream=None):
+    """uts_depth_order with the scratch inside the library (no allocation anywhere); n_gauss * n_views <= uts_depth_order_static_max()."""
+    c = cfg.c()
+    st = lib().uts_depth_order_static(C.byref(c), _ptr(rho, torch.float32), _ptr(emit_rank, torch.int32), _stream(stream))
+    if st == UTS_ERR_CAPACITY:
+        raise UtsError(st, f"uts_depth_order_static: {cfg.n_gauss * cfg.n_views} records exceed the static scratch's limit of {uts_depth_order_static_max()}")
+    _check(st, "uts_depth_order_static")
 
 
 def uts_tile_query(cfg: Config, proj: Proj, mask: Mask, offsets, keys, vals, capacity: int, scratch, emit_rank=None, tuning: Tuning | None = None,

@@ -287,4 +287,54 @@ int uts_tile_ranges(const uts_config* cfg, uint64_t n_pairs, const uint64_t* key
   return UTS_OK;
 }
 
+// ------------------------------------------------------------------------------------- uts_depth_order without caller scratch
+// For callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): the scratch of
+// uts_depth_order lives in a file-scope device array of the library, 7 MiB, enough for UTS_DEPTH_ORDER_STATIC_MAX (view, Gaussian)
+// records; every GPU that loads the library holds it until the process exits.  In host code `g_depth_order_scratch` is only a
+// stand-in for the symbol, NOT a device address: its device address is looked up once per device, with that device current, by
+// cudaGetSymbolAddress (checked), and that pointer is what the kernels get.
+}  // extern "C"
+
+namespace uts {
+constexpr size_t kDepthOrderStaticBytes = (size_t)7 << 20;
+static __device__ __align__(256) unsigned char g_depth_order_scratch[kDepthOrderStaticBytes];
+
+// device address of g_depth_order_scratch on the current device (looked up once per device), or nullptr (last CUDA error set)
+static void* depth_order_static_scratch() {
+  constexpr int kMaxDevices = 64;
+  static void* table[kMaxDevices] = {};
+  static std::mutex mu;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess || dev < 0 || dev >= kMaxDevices) { set_last_cuda_error(e != cudaSuccess ? e : cudaErrorInvalidDevice); return nullptr; }
+  std::lock_guard<std::mutex> lock(mu);
+  if (!table[dev]) {
+    void* ptr = nullptr;
+    e = cudaGetSymbolAddress(&ptr, g_depth_order_scratch);
+    if (e != cudaSuccess || !ptr) { set_last_cuda_error(e != cudaSuccess ? e : cudaErrorInvalidSymbol); return nullptr; }
+    table[dev] = ptr;
+  }
+  return table[dev];
+}
+}  // namespace uts
+
+extern "C" {
+
+uint64_t uts_depth_order_static_max(void) { return (uint64_t)UTS_DEPTH_ORDER_STATIC_MAX; }
+
+int uts_depth_order_static(const uts_config* cfg, const float* rho, uint32_t* emit_rank, void* stream) {
+  int st = check_config(cfg);
+  if (st) return st;
+  const uint64_t n = (uint64_t)cfg->n_gauss * (uint64_t)cfg->n_views;
+  // beyond the array: refused before anything is enqueued (UTS_ERR_CAPACITY; uts_depth_order_static_max() is the limit)
+  if (n > (uint64_t)UTS_DEPTH_ORDER_STATIC_MAX || uts_depth_order_scratch_bytes(cfg) > kDepthOrderStaticBytes) return UTS_ERR_CAPACITY;
+  if (n == 0) return UTS_OK;
+  if (!rho || !emit_rank) return UTS_ERR_INVALID_ARG;
+  void* scratch = depth_order_static_scratch();
+  if (!scratch) return UTS_ERR_CUDA;
+  // Nothing in the scratch has to start at zero: every region (keys, values, digit counts, scan sums) is written by a kernel of this
+  // call before a later kernel of this call reads it, so the previous call's contents are never seen.
+  return uts_depth_order(cfg, rho, emit_rank, scratch, kDepthOrderStaticBytes, stream);
+}
+
 }  // extern "C"

@@ -24,8 +24,9 @@ constexpr float kRingDelta = 4e-6f;       // fp32 chord margin, as in the descen
 constexpr int kRingFull = 1 << 28;        // |first|, |last| of a ring that lies entirely inside the disc
 
 struct RingDisc {
-  float dir[3];                           // the record's direction as stored (fp32); normalised in double where a decision needs it
-  double R;                               // min(pi, r_s + rho_q)
+  float dir[3];                           // the record's direction as stored (fp32)
+  double un[3];                           // the same, normalised in double: what the defining predicate uses
+  double R, cosR;                         // min(pi, r_s + rho_q) and its cosine
   float lq;                               // longitude in eighth-ring units: g_c = lq * n_r, lq in [0,8)
   float dq;                               // the disc's longitude half-extent in the same units (4 = everywhere)
   float zc, sc, T2, T2lo, T2hi;           // z and sin(colatitude) of u; chord thresholds T^2, (T -+ delta)^2, T = 2 sin(R/2)
@@ -55,7 +56,13 @@ __host__ __device__ __forceinline__ float ring_coord(int N, float theta) {
 __host__ __device__ __forceinline__ void make_ring_disc(int kq, const float dir[3], float lon, float lat, double R, RingDisc& D) {
   const int N = 1 << kq;
   D.dir[0] = dir[0]; D.dir[1] = dir[1]; D.dir[2] = dir[2];
+  {
+    const double ux = (double)dir[0], uy = (double)dir[1], uz = (double)dir[2];
+    const double nrm = sqrt(ux * ux + uy * uy + uz * uz);
+    D.un[0] = ux / nrm; D.un[1] = uy / nrm; D.un[2] = uz / nrm;
+  }
   D.R = R;
+  D.cosR = cos(R);
   D.all = R >= kPi;
   const float Rf = (float)R;
   const float T = 2.0f * sin_poly(0.5f * Rf);
@@ -84,21 +91,24 @@ __host__ __device__ __forceinline__ bool face_in_extent(const RingDisc& D, int f
   return d <= 1.0f + D.dq;
 }
 
-// the defining predicate for the pixel at position g of ring i, in double
+// the defining predicate  u . centre >= cos R  for the pixel at position g of ring i, in double.  With the centre
+// (sth sin(lam), z, sth cos(lam)), sth = sqrt(s2) >= 0:  sth A >= B  with  A = u_x sin(lam) + u_z cos(lam),  B = cos R - u_y z,
+// decided on the squares (s2 A^2 against B^2) so that no square root is taken; un and cos R come with the disc.  (The form with
+// sqrt, a normalisation and cos(R) per call was 18 % of the count kernels' instructions: ncu source view, round 2.)
 __host__ __device__ __forceinline__ bool ring_pixel_inside_exact(const RingDisc& D, int N, int i, int g) {
-  double u[3] = {(double)D.dir[0], (double)D.dir[1], (double)D.dir[2]};
-  const double nrm = sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
-  u[0] /= nrm; u[1] /= nrm; u[2] /= nrm;
-  double z, sth;
+  double z, s2;
   int n;
   const double inv3N2 = 1.0 / (3.0 * (double)N * (double)N);
-  if (i < N) { n = i; const double w = (double)n * (double)n * inv3N2; z = 1.0 - w; sth = sqrt(w * (2.0 - w)); }
-  else if (i > 3 * N) { n = 4 * N - i; const double w = (double)n * (double)n * inv3N2; z = w - 1.0; sth = sqrt(w * (2.0 - w)); }
-  else { n = N; z = (double)(2 * (2 * N - i)) / (double)(3 * N); sth = sqrt((1.0 - z) * (1.0 + z)); }
+  if (i < N) { n = i; const double w = (double)n * (double)n * inv3N2; z = 1.0 - w; s2 = w * (2.0 - w); }
+  else if (i > 3 * N) { n = 4 * N - i; const double w = (double)n * (double)n * inv3N2; z = w - 1.0; s2 = w * (2.0 - w); }
+  else { n = N; z = (double)(2 * (2 * N - i)) / (double)(3 * N); s2 = (1.0 - z) * (1.0 + z); }
   const double lam = (kPi / 4) * ((double)g / (double)n);
   double sn, cs;
   sincos(lam, &sn, &cs);
-  return u[0] * (sth * sn) + u[1] * z + u[2] * (sth * cs) >= cos(D.R);
+  const double A = D.un[0] * sn + D.un[2] * cs, B = D.cosR - D.un[1] * z;
+  const double lhs = s2 * A * A, rhs = B * B;
+  if (B <= 0.0) return A >= 0.0 || lhs <= rhs;
+  return A > 0.0 && lhs >= rhs;
 }
 
 // Phase 1.  In-disc pixel positions of ring i: the integers g = first, first+2, ..., last (not reduced mod 8 n_r;

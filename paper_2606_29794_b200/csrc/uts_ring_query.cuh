@@ -95,7 +95,14 @@ __host__ __device__ __forceinline__ bool face_in_extent(const RingDisc& D, int f
 // (sth sin(lam), z, sth cos(lam)), sth = sqrt(s2) >= 0:  sth A >= B  with  A = u_x sin(lam) + u_z cos(lam),  B = cos R - u_y z,
 // decided on the squares (s2 A^2 against B^2) so that no square root is taken; un and cos R come with the disc.  (The form with
 // sqrt, a normalisation and cos(R) per call was 18 % of the count kernels' instructions: ncu source view, round 2.)
+// The ring number passes through an empty volatile asm: without it the compiler hoists the part that depends on the ring alone out
+// of the callers' loops and executes it — in double — for every ring, whether or not any pixel falls inside the fp32 margin
+// (another 10 % of the instructions); as a __noinline__ call instead, the count kernels lost more to the call's register spills
+// than they gained (config 4 tile lists 7.6 -> 8.6 ms).
 __host__ __device__ __forceinline__ bool ring_pixel_inside_exact(const RingDisc& D, int N, int i, int g) {
+#ifdef __CUDA_ARCH__
+  asm volatile("" : "+r"(i));
+#endif
   double z, s2;
   int n;
   const double inv3N2 = 1.0 / (3.0 * (double)N * (double)N);

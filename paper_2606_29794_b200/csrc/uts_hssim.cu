@@ -20,7 +20,8 @@
 // weight * (c0 + K1 dx + K2 dg), summed over its four pixels in registers, into a gradient patch private to its warp (plain
 // read-add-write between __syncwarp()s: float atomics on shared memory are compare-and-swap loops on sm_100).  The two warps'
 // patches are summed and flushed to dL_dX with one red.global per cell and channel.  The upstream gradient of a loss is 1, so
-// forward and backward share the staged patch and X, G are read from HBM once.  The path is bound by fp32 ALU: about 24 FP32
+// forward and backward share the staged patch and X, G are read from HBM once.  Tiles of the equatorial faces whose whole patch is
+// visible take a SEPARABLE form of both walks (11 + 11 taps; see `sep` in the kernel): a third of the tiles on a full sphere.  The path is bound by fp32 ALU: about 24 FP32
 // instructions per tap and pixel forward and 10 backward, against 36 B of compulsory traffic per pixel.
 #include "uts_internal.cuh"
 
@@ -133,7 +134,7 @@ hssim_kernel(int k, int64_t n_pix_full, const uint32_t* __restrict__ active_tile
   __shared__ float s_val[kHCellsS];          // 1 valid, 0 missing
   __shared__ int s_idx[kHCellsS];            // storage index (pixels, < 2^31) or -1
   __shared__ float s_w[kHTaps];
-  __shared__ float s_grad[GRAD ? 2 * 3 * kGR * kHS : 1];   // [warp][channel][row][col]: no two warps share a cell
+  __shared__ float s_grad[2 * 3 * kGR * kHS];                // [warp][channel][row][col]: no two warps share a cell; scratch of the separable path
   __shared__ float s_red[2][2];
 
   const int tid = threadIdx.x;
@@ -146,6 +147,7 @@ hssim_kernel(int k, int64_t n_pix_full, const uint32_t* __restrict__ active_tile
   const bool polar = (f >> 2) != 1;
 
   for (int t = tid; t < kHTaps; t += kHT) s_w[t] = wts.w[polar ? 1 : 0][t];
+  bool mine_valid = true;                                     // every patch cell this thread staged exists and is visible
   for (int c = tid; c < kHCells; c += kHT) {
     const int cy = c / kHP, cx = c - cy * kHP;
     const int cell = cy * kHS + cx;
@@ -153,6 +155,7 @@ hssim_kernel(int k, int64_t n_pix_full, const uint32_t* __restrict__ active_tile
     const int64_t i = store_index(p, slot_of_tile, bits);
     s_idx[cell] = (int)i;
     s_val[cell] = i >= 0 ? 1.f : 0.f;
+    mine_valid = mine_valid && i >= 0;
     float x[3] = {0.f, 0.f, 0.f}, g[3] = {0.f, 0.f, 0.f};
     if (i >= 0) {
 #pragma unroll
@@ -162,7 +165,14 @@ hssim_kernel(int k, int64_t n_pix_full, const uint32_t* __restrict__ active_tile
     for (int ch = 0; ch < 3; ++ch) s_xg[ch][cell] = make_float2(x[ch], g[ch]);
   }
   if (GRAD) for (int c = tid; c < 2 * 3 * kGR * kHS; c += kHT) s_grad[c] = 0.f;
-  __syncthreads();
+  // Separable path ("enabling separable convolution"): on an equatorial face the window weights are the isotropic
+  // Gaussian g(dx) g(dy) (reading A31), and when every cell of the patch exists and is visible no tap is dropped (A32), so the
+  // renormalisation is the constant (sum g)^2: the five window sums are an 11-tap pass along x followed by an 11-tap pass along y,
+  // and the transposed window of the gradient is the same two passes on the per-pixel coefficient maps.  Block-uniform decision;
+  // polar faces (anisotropic, not separable over the square window) and patches with a missing or masked cell take all 121 taps.
+  // (Measured, order 10 full sphere, loss + gradient: all 121 taps everywhere 3.01 ms; this path unblocked 2.96; with four outputs
+  // per item in registers 2.73; the two paths as two launches, each with its own register budget, 2.80.)
+  const bool sep = __syncthreads_and(mine_valid) && !polar;
 
   const int lx = tid & 15, r0 = (tid >> 4) * kHJ;             // tile rows r0 .. r0+3; half warp = one strip of 16 x 4 pixels
   const int base = r0 * kHS + lx;                             // patch cell of tap (0,0) of pixel j = 0
@@ -171,7 +181,8 @@ hssim_kernel(int k, int64_t n_pix_full, const uint32_t* __restrict__ active_tile
     // reference value of the sums: the thread's second pixel, or its first visible one (a masked cell holds 0, which would
     // leave the sums uncentred)
     int cref = (r0 + 1 + kHR) * kHS + lx + kHR;
-    if (s_idx[cref] < 0) {
+    if (sep) cref = (8 + kHR) * kHS + 8 + kHR;                // the intermediate sums are shared: one reference for the block
+    else if (s_idx[cref] < 0) {
 #pragma unroll
       for (int j = kHJ - 1; j >= 0; --j) { const int cj = (r0 + j + kHR) * kHS + lx + kHR; if (s_idx[cj] >= 0) cref = cj; }
     }
@@ -210,6 +221,55 @@ hssim_kernel(int k, int64_t n_pix_full, const uint32_t* __restrict__ active_tile
   // Patch rows 0..2 and 11..13 lie under fewer than four of the thread's windows (unrolled); rows 3..10 under all four: a real
   // loop, so that the body stays inside the instruction cache (fully unrolled, 14 rows x 4 pixels, it stalled on fetch).
   using I0 = Int<0>; using I1 = Int<1>; using I2 = Int<2>; using I3 = Int<3>;
+  if (sep) {
+    // g(d) = the window's middle row; pass 1 along x into s_grad as H[row][col][5] (26 x 16 x 5 floats), pass 2 along y in registers
+    const float* g1 = s_w + kHR * kHW;
+    float gsum = 0.f;
+#pragma unroll
+    for (int t = 0; t < kHW; ++t) gsum += g1[t];
+#pragma unroll
+    for (int j = 0; j < kHJ; ++j) wsum[j] = gsum * gsum;
+    float* H = s_grad;
+#pragma unroll
+    for (int ch = 0; ch < 3; ++ch) {                          // unrolled: ch indexes register arrays
+      __syncthreads();                                          // the previous channel's H has been consumed
+      for (int it = tid; it < kHP * 4; it += kHT) {             // item = (patch row, group of 4 tile columns): 14 cells serve 4 outputs
+        const int row = it >> 2, cg = (it & 3) * 4;
+        const float2* src = &s_xg[ch][row * kHS + cg];
+        float dxv[14], dgv[14];
+#pragma unroll
+        for (int i = 0; i < 14; ++i) { const float2 v = src[i]; dxv[i] = v.x - xr[ch]; dgv[i] = v.y - gr[ch]; }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          float h1 = 0.f, h2 = 0.f, h11 = 0.f, h22 = 0.f, h12 = 0.f;
+#pragma unroll
+          for (int t = 0; t < kHW; ++t) {
+            const float a = g1[t] * dxv[q + t], b = g1[t] * dgv[q + t];
+            h1 += a; h2 += b; h11 = fmaf(a, dxv[q + t], h11); h22 = fmaf(b, dgv[q + t], h22); h12 = fmaf(a, dgv[q + t], h12);
+          }
+          float* dst = H + (row * 16 + cg + q) * 5;
+          dst[0] = h1; dst[1] = h2; dst[2] = h11; dst[3] = h22; dst[4] = h12;
+        }
+      }
+      __syncthreads();
+#pragma unroll
+      for (int rho = 0; rho < kHRows; ++rho) {                  // patch rows r0 .. r0 + 13 of column lx
+        const float* hv = H + ((r0 + rho) * 16 + lx) * 5;
+        const float v0 = hv[0], v1 = hv[1], v2 = hv[2], v3 = hv[3], v4 = hv[4];
+#pragma unroll
+        for (int j = 0; j < kHJ; ++j) {
+          const int t = rho - j;                                // window row of pixel j
+          if (t >= 0 && t < kHW) {
+            const float wv = g1[t];
+            S1[j][ch] = fmaf(wv, v0, S1[j][ch]); S2[j][ch] = fmaf(wv, v1, S2[j][ch]); S11[j][ch] = fmaf(wv, v2, S11[j][ch]);
+            S22[j][ch] = fmaf(wv, v3, S22[j][ch]); S12[j][ch] = fmaf(wv, v4, S12[j][ch]);
+          }
+        }
+      }
+    }
+    __syncthreads();
+    if (GRAD) for (int c = tid; c < 2 * 3 * kGR * kHS; c += kHT) s_grad[c] = 0.f;      // not used as warp patches on this path, but kept defined
+  } else
 #pragma unroll 1
   for (int tx = 0; tx < kHW; ++tx) {
     const int c = base + tx;
@@ -261,7 +321,73 @@ hssim_kernel(int k, int64_t n_pix_full, const uint32_t* __restrict__ active_tile
     if (h_map) h_map[slot * 256 + (spread16((uint32_t)lx) | (spread16((uint32_t)(r0 + j)) << 1))] = hq;   // Morton position in the slot
   }
 
-  if (GRAD) {
+  if (GRAD && sep) {
+    // Transposed window, separable: the tap's share of dL/dx at a patch cell is  A + B dx_cell + C dg_cell  with A, B, C the window
+    // transforms of the per-pixel coefficient maps c0, k1, k2 over the tile — a pass along y (26 x 16 x 3) and a pass along x
+    // (26 x 26 x 3) per channel, in s_grad as Cf[16][16][3] and V[26][16][3]; each patch cell's sum goes straight to dL_dX with one
+    // atomic (neighbouring tiles add their aprons to the same pixels).
+    const float* g1 = s_w + kHR * kHW;
+    float* Cf = s_grad;                                         // 768 floats
+    float* V = s_grad + 16 * 16 * 3;                            // 1248 floats
+#pragma unroll
+    for (int ch = 0; ch < 3; ++ch) {                          // unrolled: ch indexes register arrays
+      __syncthreads();                                          // the previous channel's maps have been consumed
+#pragma unroll
+      for (int j = 0; j < kHJ; ++j) {
+        float* d = Cf + ((r0 + j) * 16 + lx) * 3;
+        d[0] = c0[j][ch]; d[1] = k1[j][ch]; d[2] = k2[j][ch];
+      }
+      __syncthreads();
+      for (int it = tid; it < 16 * 7; it += kHT) {              // along y; item = (tile column, group of 4 patch rows): 14 tile rows serve 4 outputs
+        const int col = it & 15, p0 = (it >> 4) * 4;
+        float cf[14][3];
+#pragma unroll
+        for (int i = 0; i < 14; ++i) {
+          const int tr = p0 - 10 + i;                           // tile row; patch row prow takes tile rows prow - 10 .. prow
+          const bool in = tr >= 0 && tr < 16;
+          const float* sp = Cf + ((in ? tr : 0) * 16 + col) * 3;
+          cf[i][0] = in ? sp[0] : 0.f; cf[i][1] = in ? sp[1] : 0.f; cf[i][2] = in ? sp[2] : 0.f;
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          if (p0 + q >= kHP) break;
+          float a = 0.f, b = 0.f, c = 0.f;
+#pragma unroll
+          for (int t = 0; t < kHW; ++t) { a = fmaf(g1[t], cf[q - t + 10][0], a); b = fmaf(g1[t], cf[q - t + 10][1], b); c = fmaf(g1[t], cf[q - t + 10][2], c); }
+          float* d = V + ((p0 + q) * 16 + col) * 3;
+          d[0] = a; d[1] = b; d[2] = c;
+        }
+      }
+      __syncthreads();
+      for (int it = tid; it < kHP * 7; it += kHT) {             // along x; item = (patch row, group of 4 patch columns), then the cells' values and atomics
+        const int prow = it / 7, p0 = (it - prow * 7) * 4;
+        float vv[14][3];
+#pragma unroll
+        for (int i = 0; i < 14; ++i) {
+          const int tc = p0 - 10 + i;
+          const bool in = tc >= 0 && tc < 16;
+          const float* sp = V + (prow * 16 + (in ? tc : 0)) * 3;
+          vv[i][0] = in ? sp[0] : 0.f; vv[i][1] = in ? sp[1] : 0.f; vv[i][2] = in ? sp[2] : 0.f;
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const int pcol = p0 + q;
+          if (pcol >= kHP) break;
+          float a = 0.f, b = 0.f, c = 0.f;
+#pragma unroll
+          for (int t = 0; t < kHW; ++t) { a = fmaf(g1[t], vv[q - t + 10][0], a); b = fmaf(g1[t], vv[q - t + 10][1], b); c = fmaf(g1[t], vv[q - t + 10][2], c); }
+          const int cell = prow * kHS + pcol;
+          const float2 v = s_xg[ch][cell];
+          float val = fmaf(b, v.x - xr[ch], fmaf(c, v.y - gr[ch], a));
+          if (prow >= kHR && prow < kHR + 16 && pcol >= kHR && pcol < kHR + 16) {     // L1 term at the tile's own pixels
+            const float d = v.x - v.y;
+            val += (1.f - lambda) * inv_n * (1.f / 3.f) * (d > 0.f ? 1.f : (d < 0.f ? -1.f : 0.f));
+          }
+          if (val != 0.f) atomicAdd(dL_dX + 3 * (int64_t)s_idx[cell] + ch, val);
+        }
+      }
+    }
+  } else if (GRAD) {
     // transposed window: every tap scatters into the warp's private patch.  Within one group of four patch rows the 32 lanes
     // touch 32 different cells (the other half warp works 4 rows further down), so plain read-add-write is safe between the
     // __syncwarp()s (after rows 2, 6, 10, 13); sums over the thread's own four pixels are taken in registers first.
@@ -316,7 +442,7 @@ hssim_kernel(int k, int64_t n_pix_full, const uint32_t* __restrict__ active_tile
     const double s = (double)s_red[tid][0] + (double)s_red[tid][1];
     if (s != 0.0) atomicAdd(acc + tid, s);
   }
-  if (GRAD) {
+  if (GRAD && !sep) {
     for (int c = tid; c < kHCells; c += kHT) {
       const int cy = c / kHP, cx = c - cy * kHP;
       const int i = s_idx[cy * kHS + cx];

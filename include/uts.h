@@ -118,8 +118,8 @@ typedef struct {
   int   descent_blocks_per_sm;/* descent only: persistent blocks per SM of that path; 0 = 2 */
   int   matrix_off;        /* uts_tile_lists: 1 = never route discs through the (disc x tile) bit matrix */
   float matrix_min_tiles;  /* uts_tile_lists: discs covering at least this many tiles become matrix rows; 0 = max(48, N_tile / 144) */
-  int   window_off;        /* 1 = the smallest discs go through ring intervals like the others instead of the tile window
-                              (uts_window_query.cuh) */
+  int   window_mode;       /* tile window for the smallest discs (uts_window_query.cuh) instead of ring intervals: 0 = when the mask
+                              keeps at most a quarter of the tiles (where it was measured to pay), 1 = never, 2 = always */
 } uts_tuning;
 
 /* ---------------------------------------------------------------------------------------------- forward */

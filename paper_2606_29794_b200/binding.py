@@ -64,7 +64,7 @@ class CMask(C.Structure):
 
 class CTuning(C.Structure):
     _fields_ = [("query_impl", C.c_int), ("descent_block_radius", C.c_float), ("descent_blocks_per_sm", C.c_int), ("matrix_off", C.c_int),
-                ("matrix_min_tiles", C.c_float), ("window_off", C.c_int)]
+                ("matrix_min_tiles", C.c_float), ("window_mode", C.c_int)]
 
 
 @dataclass
@@ -75,10 +75,10 @@ class Tuning:
     descent_blocks_per_sm: int = 0
     matrix_off: int = 0
     matrix_min_tiles: float = 0.0
-    window_off: int = 0                 # 1: no tile-window path for the smallest discs
+    window_mode: int = 0                # tile-window path for the smallest discs: 0 automatic (sparse masks), 1 never, 2 always
 
     def c(self):
-        return CTuning(self.query_impl, self.descent_block_radius, self.descent_blocks_per_sm, self.matrix_off, self.matrix_min_tiles, self.window_off)
+        return CTuning(self.query_impl, self.descent_block_radius, self.descent_blocks_per_sm, self.matrix_off, self.matrix_min_tiles, self.window_mode)
 
 
 def _tuning(t):

@@ -39,7 +39,7 @@ struct QueryParams {
   int64_t n_tile;
   double rho_q;                         // rho_max(k_q) (NESTED set) or 0 (RING set): R = min(pi, r_s + rho_q)
   double rho_t;                         // rho_max(k_t)
-  int w_max;                            // window class: largest half-width (2 without a mask, kWindowMax with one)
+  int w_max;                            // window class: largest half-width
   float r_large;                        // discs with R above this go to the block path
   uint32_t* tile_cache;                 // [V*P][kTileCacheK] tiles found by the count pass (thread path), reused by the emit pass
   uint32_t* bitmap_cache;               // [bitmap_cache_cap][n_words] bitmaps of the count pass (block path)
@@ -1005,11 +1005,14 @@ struct QueryRun {
     // window class (uts_window_query.cuh): discs of the thread class with R <= 0.98 kWindowWidth w_max / N_t, i.e. the
     // radius buckets strictly below the one that holds that radius; needs N_t >= 2 kWindowMax + 1 so that the window's cells are distinct
     b_fast = kBuckets;
-#ifndef UTS_WIN_UNMASKED_MAX
-#define UTS_WIN_UNMASKED_MAX 2
-#endif
-    qp.w_max = mask.slot_of_tile ? kWindowMax : UTS_WIN_UNMASKED_MAX;   // measured: see uts_window_query.cuh
-    if (ring_impl && !tn.window_off && (1 << d.kt) >= 2 * kWindowMax + 1) {
+    // When: measured after the ring path's exact test became cheap (round 2), the window wins only where most candidates fall
+    // outside the mask (config 5, frustum = 6 % of the tiles: tile lists 4.5 -> 3.7 ms; config 3, cap = 55 %: 0.68 -> 0.78;
+    // no mask: config 2 0.24 -> 0.33, config 4 unchanged) — so by default it is taken when the mask keeps at most a quarter of
+    // the tiles; uts_tuning.window_mode forces it on (tests) or off.
+    qp.w_max = kWindowMax;
+    const bool window_auto = mask.slot_of_tile && (int64_t)mask.n_active * 4 <= d.n_tile;
+    const bool window_on = tn.window_mode == 2 || (tn.window_mode == 0 && window_auto);
+    if (ring_impl && window_on && (1 << d.kt) >= 2 * kWindowMax + 1) {
       b_fast = radius_bucket_host((float)(0.98 * (1.0 - 1e-6) * kWindowWidth * qp.w_max / (double)(1 << d.kt))) + 1;
       if (b_fast <= qp.b_warp) b_fast = qp.b_warp + 1;
     }

@@ -9,13 +9,14 @@
 // around tile(u), taken in the extended (x, y) frame of u's base face and carried into the neighbouring faces by the gluing rules
 // below, holds every candidate; each candidate is settled by one fp32 chord test of its centre (all of it inside / outside the
 // disc) and, on the rim, by the defining predicate on its 4^(k_q-k_t) query pixels (fp32 chord with a margin, double inside the
-// margin).  Measured (B200, tile-lists call): config 5 (frustum mask, N_t = 128) 5.5 -> 3.9 ms with windows up to 7 x 7 — a
-// candidate outside the mask costs one table read, where the ring path pays for rings and rows before it filters —, config 4 (no
-// mask) 8.53 -> 8.43 ms with windows up to 5 x 5 (7 x 7: 8.55): the work per disc grows with the window AREA times the 4^(k_q-k_t)
-// rim tests, so the ring intervals take over early on unmasked scenes.  (The gluing table must be `static`: as a plain constexpr
-// local it was copied to each thread's stack, and config 4 went to 12.3 ms.  Also measured: classifying all cells first and then
-// walking the rim tiles' query pixels in ONE flattened loop per lane (so that lanes whose tile was settled by the centre test do
-// not idle through the others' pixel loops; ncu shows 12 of 32 lanes active here) — no gain, config 5 3.9 -> 4.1 ms; not kept.)
+// margin).  A candidate outside the FoV mask costs one table read, where the ring path pays for rings and rows before it filters:
+// measured (B200, tile-lists call, round 2 after the ring path's exact test became cheap) config 5 (frustum mask = 6 % of the
+// tiles, N_t = 128) 4.5 -> 3.7 ms with windows up to 7 x 7; config 3 (cap mask, 55 %) 0.68 -> 0.78 ms, config 2 (no mask) 0.24 ->
+// 0.33 ms, config 4 (no mask) unchanged: the work per disc grows with the window AREA times the 4^(k_q-k_t) rim tests.  So the
+// caller (uts_tile_query.cu) takes this path by default only under a mask that keeps at most a quarter of the tiles.
+// (The gluing table must be `static`: as a plain constexpr local it was copied to each thread's stack, and config 4 went from 8.5
+// to 12.3 ms.  Also measured: classifying all cells first and then walking the rim tiles' query pixels in ONE flattened loop per
+// lane, so that lanes whose tile was settled by the centre test do not idle through the others' pixel loops — no gain; not kept.)
 // Everything is __host__ __device__: tests/hostlogic drives the same code on the CPU against the oracle's sets.
 #pragma once
 #include "uts_internal.cuh"

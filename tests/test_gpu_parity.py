@@ -184,7 +184,7 @@ def test_preprocess_in_two_calls_is_bit_identical():
 
 
 # ------------------------------------------------------------------------------------------- F2
-WINDOW = pytest.mark.parametrize("window", [True, False], ids=["window-path", "ring-intervals-only"])   # uts_tuning.window_off
+WINDOW = pytest.mark.parametrize("window", [True, False], ids=["window-path", "ring-intervals-only"])   # uts_tuning.window_mode 2 / 1
 
 
 @WINDOW
@@ -194,7 +194,7 @@ def test_tile_query_bit_exact(cfg_id, P, order, extra, window):
     c = Case.get(cfg_id, P, order, extra)
     cfg = _cfg(R, c.scene)
     proj, mask = c.gpu_proj(B), c.gpu_mask(B)
-    tn = None if window else B.Tuning(window_off=1)
+    tn = B.Tuning(window_mode=2 if window else 1)
     n_want = int(c.fw["keys"].shape[0])
     offsets = torch.empty(cfg.n_views * cfg.n_gauss + 1, dtype=torch.int64, device="cuda")
     scratch = torch.empty(B.uts_tile_query_scratch_bytes(cfg) // 8 + 32, dtype=torch.int64, device="cuda")
@@ -280,7 +280,7 @@ def test_tile_query_window_path_small_discs_everywhere(order, refine, masked, mo
     """The tile-window path (uts_window_query.cuh) on discs it is made for: 6000 small discs, among them centres ON and next to the
     poles, the vertices shared by three and by four faces and the meridian face edges, radii up to the largest the path accepts (so
     that 3 x 3, 5 x 5 and 7 x 7 windows all occur), with a cap mask or without; emission ranks from uts_depth_order; count-only, then
-    emit.  Against the oracle's sets, bit for bit; the same call with window_off must give the same arrays."""
+    emit.  Against the oracle's sets, bit for bit; the same call with the window path switched off must give the same arrays."""
     B, R = _gpu()
     n = 6000
     scene = small_scene(3 if masked else 4, n, order, n_views=1)
@@ -325,7 +325,7 @@ def test_tile_query_window_path_small_discs_everywhere(order, refine, masked, mo
     mask = B.Mask.full() if bits is None else B.Mask(dev(act.view(np.int32)), int(act.shape[0]), dev(slot), dev(bits.view(np.int32)))
     proj = B.Proj(dev(pr.dir), dev(pr.lonlat), dev(pr.rho), dev(pr.conic_opac), dev(pr.rs), dev(pr.rgb), dev(pr.flags))
     got = []
-    for tn in (None, B.Tuning(window_off=1)):
+    for tn in (B.Tuning(window_mode=2), B.Tuning(window_mode=1)):
         r = R.Rasterizer(cfg, mask, depth_presort=True, fused_lists=False, tuning=tn, pair_capacity=16)
         r.proj = proj
         r.depth_order()

@@ -276,6 +276,17 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
             p2[j] = 1.f;
             if (PX == 1 || (alive & (1u << j))) {     // warp-uniform
               Eval ev;
+              if (PX == 1 && !COUNT) {
+                // Patch-level early out: k >= 1, so power = q k^2 <= q for q <= 0; when q is already below the alpha_min cut for
+                // every open pixel of the patch (half of the (patch, entry) visits on the paper's kind of scene), c and k are not
+                // needed.  0.999999: the polynomial's k may fall short of 1 by 2e-7.  No decision changes: such a pixel fails
+                // may_contribute() below as well.
+                ev.a = fmaf(g1.x, ts.px[j], fmaf(g1.y, ts.pz[j], g0v.x));
+                ev.b = fmaf(g1.z, ts.px[j], fmaf(g1.w, ts.py[j], fmaf(g2.x, ts.pz[j], g0v.y)));
+                const float q = fmaf(ev.a, fmaf(g3.x, ev.a, g3.y * ev.b), g3.z * ev.b * ev.b);
+                const bool maybe = open && !(q > 0.f) && q * 0.999999f >= g0v.w;
+                if (!__any_sync(0xffffffffu, maybe)) continue;
+              }
               eval_entry(g0v, g1, g2, g3, ts.px[j], ts.py[j], ts.pz[j], ev);
               p2[j] = ev.p2;
               if (COUNT && ((open >> j) & 1u) && (uint64_t)jj < left_n) ++n_eval;       // null padding entries are not Alg.1's

@@ -207,9 +207,12 @@ int uts_tile_ranges(const uts_config* cfg, uint64_t n_pairs, const uint64_t* key
 int uts_render_fwd(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
                    float* color, float* alpha, float* trans, uint32_t* n_last, void* stream);
 
-/* uts_render_fwd that also counts its work (measurement only: bench.py's roofline lines): adds to work[0] the (pixel, entry) pairs
- * Alg.1's loop evaluates (every entry a pixel visits before it stops, l.20-28 PAPER.md:568-584) and to work[1] those that
- * contribute (alpha >= alpha_min).  work: 2 DEVICE uint64, zeroed by the caller.  Outputs as uts_render_fwd. */
+/* uts_render_fwd that also counts its work (measurement only: bench.py's roofline lines), walking every entry in full, i.e. without
+ * the patch cull and the early out of the production kernels (its image is the reference of their bit-identity).  Adds to work[0] the
+ * (pixel, entry) pairs Alg.1's loop evaluates (every entry a pixel visits before it stops, l.20-28 PAPER.md:568-584), to work[1] those
+ * that contribute (alpha >= alpha_min), to work[2] those the production forward evaluates at all (the entry passes the patch cull) and
+ * to work[3] those it evaluates in full (it also passes the early out).  work: 4 DEVICE uint64, zeroed by the caller.  Outputs as
+ * uts_render_fwd. */
 int uts_render_fwd_counted(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
                            float* color, float* alpha, float* trans, uint32_t* n_last, uint64_t* work, void* stream);
 

@@ -320,7 +320,9 @@ def uts_render_fwd(cfg: Config, proj: Proj, mask: Mask, ranges, vals, color, alp
 
 
 def uts_render_fwd_counted(cfg: Config, proj: Proj, mask: Mask, ranges, vals, color, alpha, trans, n_last, work, stream=None):
-    """uts_render_fwd + work counters: work = 2 int64 on the device (zeroed by the caller) -> += (evaluated, contributing) pairs."""
+    """uts_render_fwd + work counters: work = 4 int64 on the device (zeroed by the caller) -> += (evaluated by Alg.1, contributing,
+    passing the patch cull, evaluated in full) pairs."""
+    assert work.numel() >= 4
     c = cfg.c()
     _check(lib().uts_render_fwd_counted(C.byref(c), proj.c(), mask.c(), _ptr(ranges, torch.int64), _ptr(vals, torch.int32),
                                         _ptr(color, torch.float32), _ptr(alpha, torch.float32), _ptr(trans, torch.float32),

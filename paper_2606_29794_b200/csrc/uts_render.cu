@@ -104,12 +104,12 @@ __device__ __forceinline__ float arc_over_sin(float t, float c) {
 //   g2 = (nz, ux, uy, uz)     uhat
 //   g3 = (qa, qb, qc, o)      -0.5 A log2e, -B log2e, -0.5 C log2e; opacity
 //   g4 = (r, g, b, id | 1/rho)  colour; backward: Gaussian index as raw bits; forward with the depth channel: 1 / rho
-//   g5 = (sin phi, cos phi, 1/rho)   backward only
+//   g5 = (sin phi, cos phi, 1/rho)   backward;  (L, -, -, -) forward: L = sqrt(lambda_max) of the scaled conic, for the patch cull
 constexpr uint32_t kRow = kBatch * 16u;               // bytes between rows
 struct TileFrame { double cx, cy, cz; };              // tile centre direction (order k_t pixel centre)
 
 template <bool BWD>
-struct __align__(16) SEntries { float4 g[BWD ? 6 : 5][kBatch]; };
+struct __align__(16) SEntries { float4 g[6][kBatch]; };
 
 template <bool BWD>
 __device__ __forceinline__ void stage_entry(SEntries<BWD>& S, int i, const TileFrame& tf, float amin, uint32_t id, float ux, float uy,
@@ -131,6 +131,12 @@ __device__ __forceinline__ void stage_entry(SEntries<BWD>& S, int i, const TileF
   S.g[3][i] = make_float4(-0.5f * kLog2e * co.x, -kLog2e * co.y, -0.5f * kLog2e * co.z, co.w);
   S.g[4][i] = make_float4(r, g, b, BWD ? __uint_as_float(id) : inv_r);
   if (BWD) S.g[5][i] = make_float4(hy, sqrtf(hx * hx + hz * hz), inv_r, 0.f);
+  else {
+    // -q(d) = d^T K d with K = [[-qa, -qb/2], [-qb/2, -qc]] positive definite: sqrt(-q) is a norm, bounded by L |d|
+    const float A = 0.5f * kLog2e * co.x, B = 0.5f * kLog2e * co.y, C = 0.5f * kLog2e * co.z;
+    const float hd = 0.5f * (A - C);
+    S.g[5][i] = make_float4(sqrtf(0.5f * (A + C) + sqrtf(fmaf(hd, hd, B * B))) * 1.00001f, 0.f, 0.f, 0.f);
+  }
 }
 
 struct Eval { float a, b, c, t, k, p2; };
@@ -217,7 +223,9 @@ __device__ __forceinline__ void stage_batch(SEntries<BWD>& S, const TileFrame& t
   }
 }
 
-// COUNT (uts_render_fwd_counted, measurement only): also adds the evaluated and the contributing (pixel, entry) pairs to work[0..1].
+// COUNT (uts_render_fwd_counted, measurement only): the walk WITHOUT the patch cull and the early out (every entry is evaluated in
+// full: the reference for their bit-identity), adding to work[0..3] the (pixel, entry) pairs of Alg.1's loop, those that contribute,
+// those the production kernel evaluates at all (they pass the patch cull) and those it evaluates in full (they pass the early out).
 // DEPTH (uts_render_fwd_depth): a fourth blended channel, the inverse radial depth 1 / rho_i (reading A29).
 template <int PX, bool MARK, bool COUNT = false, bool DEPTH = false>
 __global__ void __launch_bounds__(kTilePix / PX)
@@ -229,7 +237,7 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
                   const float* __restrict__ rho = nullptr, float* __restrict__ depth_out = nullptr) {
   constexpr int kThreads = kTilePix / PX, kWarps = kThreads / 32;
   __shared__ SEntries<false> S;
-  uint32_t n_eval = 0, n_contrib = 0;                 // COUNT only
+  uint32_t n_eval = 0, n_contrib = 0, n_cull = 0, n_full = 0;      // COUNT only
   __shared__ TileFrame s_tf;
   TileSetup<PX> ts;
   setup_tile<PX>(rp, active_tiles, mask_bits, ranges, &s_tf, ts);
@@ -246,6 +254,27 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
   const uint32_t sS = (uint32_t)__cvta_generic_to_shared(&S);
   uint32_t* mark_w = nullptr;                         // plane `wid` of this tile's run; patch j is kWarps j planes further
   if (MARK) mark_w = marks + (uint64_t)wid * plane_words + mark_base<PX>(rp, ts);
+  // Patch cull (PX = 1: a warp is one 8x4 patch).  At the start of a group of 32 entries lane l asks whether entry l can reach the
+  // patch at all: with the patch's centre pc and radius r (in the tile frame; the map to the Gaussian's (a, b) plane is an
+  // isometry of the chord), sqrt(-q) >= N(pc) - r L everywhere on the patch, so N(pc) - r L > sqrt(-th) means every pixel's power
+  // is below the alpha_min cut.  The ballot's survivors are walked as before, the others cost two instructions.  No per-pixel
+  // decision changes (such an entry fails may_contribute() at every pixel); the margin 1.0001 covers the fp32 rounding of the
+  // bound.  A warp whose last tested group kept >= 24 of 32 entries (config 4: large near Gaussians) skips the test for 3 groups.
+  float pcx = 0.f, pcy = 0.f, pcz = 0.f, prad = 0.f;
+  int skip_tests = 0;
+  if (PX == 1) {
+    pcx = ts.px[0]; pcy = ts.py[0]; pcz = ts.pz[0];
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+      pcx += __shfl_xor_sync(0xffffffffu, pcx, d); pcy += __shfl_xor_sync(0xffffffffu, pcy, d); pcz += __shfl_xor_sync(0xffffffffu, pcz, d);
+    }
+    pcx *= (1.f / 32.f); pcy *= (1.f / 32.f); pcz *= (1.f / 32.f);
+    const float ex = ts.px[0] - pcx, ey = ts.py[0] - pcy, ez = ts.pz[0] - pcz;
+    prad = sqrtf(ex * ex + ey * ey + ez * ez);
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) prad = fmaxf(prad, __shfl_xor_sync(0xffffffffu, prad, d));
+    prad *= 1.00001f;
+  }
   for (uint64_t b0 = 0; b0 < len; b0 += kBatch) {
     if (__syncthreads_and(open == 0)) break;          // every pixel of the tile saturated (or masked)
     const uint64_t left_n = len - b0;
@@ -261,12 +290,32 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
 #pragma unroll
       for (int j = 0; j < PX; ++j) mw[j] = 0u;
       const int ge = min(nb, g0 + 32);
+      uint32_t live = 0xffffffffu;                    // bit e: entry g0 + e may reach this patch
+      if (PX == 1) {
+        if (skip_tests > 0) --skip_tests;
+        else {
+          const int e = g0 + (int)(threadIdx.x & 31);
+          bool reach = false;
+          if (e < nb) {
+            const uint32_t se = sS + (uint32_t)e * 16u;
+            const float4 h0 = lds128(se), h1 = lds128(se + kRow), h2 = lds128(se + 2u * kRow), h3 = lds128(se + 3u * kRow), h5 = lds128(se + 5u * kRow);
+            const float ac = fmaf(h1.x, pcx, fmaf(h1.y, pcz, h0.x));
+            const float bc = fmaf(h1.z, pcx, fmaf(h1.w, pcy, fmaf(h2.x, pcz, h0.y)));
+            const float nq = -fmaf(ac, fmaf(h3.x, ac, h3.y * bc), h3.z * bc * bc);     // -q at the patch centre
+            const float slack = sqrtf(fmaxf(nq, 0.f)) - prad * h5.x;
+            reach = !(slack > 0.f && slack * slack > -h0.w * 1.0002f);
+          }
+          live = __ballot_sync(0xffffffffu, reach);
+          if (__popc(live) >= 24) skip_tests = 3;
+        }
+      }
       for (int j4 = g0; j4 < ge; j4 += 4) {
         const uint32_t alive = __reduce_or_sync(0xffffffffu, open);
         if (alive == 0) { left = true; break; }       // every pixel of the warp is saturated
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
           const int jj = j4 + u;
+          if (PX == 1 && !COUNT && !((live >> (jj - g0)) & 1u)) continue;
           const uint32_t sa = sS + (uint32_t)jj * 16u;
           const float4 g0v = lds128(sa), g1 = lds128(sa + kRow), g2 = lds128(sa + 2u * kRow), g3 = lds128(sa + 3u * kRow);
           float p2[PX];
@@ -276,16 +325,18 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
             p2[j] = 1.f;
             if (PX == 1 || (alive & (1u << j))) {     // warp-uniform
               Eval ev;
-              if (PX == 1 && !COUNT) {
+              if (PX == 1) {
                 // Patch-level early out: k >= 1, so power = q k^2 <= q for q <= 0; when q is already below the alpha_min cut for
-                // every open pixel of the patch (half of the (patch, entry) visits on the paper's kind of scene), c and k are not
-                // needed.  0.999999: the polynomial's k may fall short of 1 by 2e-7.  No decision changes: such a pixel fails
-                // may_contribute() below as well.
+                // every open pixel of the patch, c and k are not needed.  0.999999: the polynomial's k may fall short of 1 by
+                // 2e-7.  No decision changes: such a pixel fails may_contribute() below as well.
                 ev.a = fmaf(g1.x, ts.px[j], fmaf(g1.y, ts.pz[j], g0v.x));
                 ev.b = fmaf(g1.z, ts.px[j], fmaf(g1.w, ts.py[j], fmaf(g2.x, ts.pz[j], g0v.y)));
                 const float q = fmaf(ev.a, fmaf(g3.x, ev.a, g3.y * ev.b), g3.z * ev.b * ev.b);
                 const bool maybe = open && !(q > 0.f) && q * 0.999999f >= g0v.w;
-                if (!__any_sync(0xffffffffu, maybe)) continue;
+                const bool pass = __any_sync(0xffffffffu, maybe);
+                if (COUNT) {
+                  if (open && (uint64_t)jj < left_n && ((live >> (jj - g0)) & 1u)) { ++n_cull; if (pass) ++n_full; }
+                } else if (!pass) continue;
               }
               eval_entry(g0v, g1, g2, g3, ts.px[j], ts.py[j], ts.pz[j], ev);
               p2[j] = ev.p2;
@@ -324,7 +375,11 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
   }
   if (COUNT) {
     const uint32_t e = __reduce_add_sync(0xffffffffu, n_eval), c = __reduce_add_sync(0xffffffffu, n_contrib);
-    if ((threadIdx.x & 31) == 0) { atomicAdd(work, (unsigned long long)e); atomicAdd(work + 1, (unsigned long long)c); }
+    const uint32_t u = __reduce_add_sync(0xffffffffu, n_cull), f = __reduce_add_sync(0xffffffffu, n_full);
+    if ((threadIdx.x & 31) == 0) {
+      atomicAdd(work, (unsigned long long)e); atomicAdd(work + 1, (unsigned long long)c);
+      atomicAdd(work + 2, (unsigned long long)u); atomicAdd(work + 3, (unsigned long long)f);
+    }
   }
 #pragma unroll
   for (int j = 0; j < PX; ++j) {

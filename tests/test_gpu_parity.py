@@ -548,17 +548,19 @@ def test_render_fwd(cfg_id, P, order, extra, marks):
 
 @pytest.mark.parametrize("cfg_id,P,order,extra", [CASES[1], CASES[5]])
 def test_render_fwd_counted_matches_the_oracle_work_counters(cfg_id, P, order, extra):
-    """uts_render_fwd_counted (bench.py's work counters): same image as uts_render_fwd, and the evaluated / contributing pair counts
-    of Alg.1's loop equal the oracle's counters up to the few pixels whose decisions sit on a threshold."""
+    """uts_render_fwd_counted (bench.py's work counters; it walks every entry in full): bit-identical image to uts_render_fwd, whose
+    patch cull and early out therefore change nothing, and the evaluated / contributing pair counts of Alg.1's loop equal the
+    oracle's counters up to the few pixels whose decisions sit on a threshold."""
     B, R = _gpu()
     c = Case.get(cfg_id, P, order, extra)
     r = _render_gpu(B, R, c, _cfg(R, c.scene), marks=False)
-    work = torch.zeros(2, dtype=torch.int64, device="cuda")
+    work = torch.zeros(4, dtype=torch.int64, device="cuda")
     out = [torch.empty_like(t) for t in (r.color, r.alpha, r.trans, r.n_last)]
     B.uts_render_fwd_counted(r.cfg, r.proj, r.mask, r.ranges, r.vals, *out, work)
-    for a, b in zip(out, (r.color, r.alpha, r.trans, r.n_last)):
-        assert torch.equal(a, b)
-    ev, contrib = (int(x) for x in work.cpu().tolist())
+    for a, b in zip(out, (r.color, r.alpha, r.trans, r.n_last)):        # the counted walk takes no patch cull and no early out:
+        assert torch.equal(a, b)                                          # the production kernel's shortcuts change no bit
+    ev, contrib, n_cull, n_full = (int(x) for x in work.cpu().tolist())
+    assert contrib <= n_full <= n_cull <= ev
     ctr = c.fw["counters"]
     assert abs(ev - ctr["evaluated"]) <= 2e-3 * ctr["evaluated"] + 16, (ev, ctr)
     assert abs(contrib - ctr["contributing"]) <= 2e-3 * ctr["contributing"] + 16, (contrib, ctr)

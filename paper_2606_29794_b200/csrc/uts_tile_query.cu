@@ -900,7 +900,10 @@ int radius_bucket_host(float R32) {                    // host replica of radius
 // The three shapes of the ring path are independent: they run side by side on the device context's two auxiliary streams, forked
 // from and joined back to the caller's stream with events, so the caller still sees one ordered stream.  ctx->mu is held from
 // the fork to the join (QueryRun::count / emit), so two callers never interleave their records of the shared events.
-constexpr int kRingThreadRings = 24, kRingWarpRings = 128, kRingBlockRingsMax = 24575;   // ring-table capacities (8 B per ring)
+#ifndef UTS_RING_WARP_RINGS
+#define UTS_RING_WARP_RINGS 128
+#endif
+constexpr int kRingThreadRings = 24, kRingWarpRings = UTS_RING_WARP_RINGS, kRingBlockRingsMax = 24575;   // ring-table capacities (8 B per ring)
 
 struct QueryLayout { size_t counts, list, perm, nlarge, active, scan, tcache, bcache, bcache_bytes, total; uint32_t bcache_cap; };
 QueryLayout query_layout(const uts_config* cfg) {

@@ -888,3 +888,49 @@ def test_forward_auto_is_always_the_full_result():
         ca, _ = auto.forward_auto(g, views)
         assert torch.equal(ca, cf) and auto.n_pairs == full.n_pairs
     assert auto._auto["off"] and not auto._auto["used_prefix"]
+
+
+def test_concurrent_calls_from_two_threads_on_two_streams():
+    """include/uts.h "Library state": the per-device context (auxiliary streams, fork / join events) is guarded by a mutex, so two
+    threads may drive the path at the same time on their own streams.  Each thread runs the whole forward + backward 15 times on its
+    own scene and stream (ctypes releases the GIL during the calls); every result must equal the one computed alone."""
+    import threading
+    B, R = _gpu()
+    from paper_2606_29794_b200 import scenes
+    jobs = []
+    for seed, cfg_id in ((0, 2), (1, 4)):
+        scene = small_scene(cfg_id, 12000, 7, seed=seed)
+        cfg = _cfg(R, scene)
+        g, views = R.scene_to_device(scene)
+        r = R.Rasterizer(cfg)
+        r.forward(g, views)
+        gcol = torch.from_numpy(scenes.upstream_grad(1, r.color.shape[1], seed=seed)).cuda()
+        r.backward(g, views, gcol)
+        torch.cuda.synchronize()
+        ref = dict(n=r.n_pairs, keys=r.keys[: r.n_pairs].clone(), vals=r.vals[: r.n_pairs].clone(), ranges=r.ranges.clone(), color=r.color.clone(),
+                   n_last=r.n_last.clone(), means=r.grads["means"].clone())
+        jobs.append((cfg, g, views, gcol, ref))
+    errors = []
+
+    def work(job):
+        try:
+            cfg, g, views, gcol, ref = job
+            stream = torch.cuda.Stream()
+            with torch.cuda.stream(stream):
+                r = R.Rasterizer(cfg)
+                for _ in range(15):
+                    r.forward(g, views)
+                    G = r.backward(g, views, gcol)
+                    stream.synchronize()
+                    n = r.n_pairs
+                    assert n == ref["n"]
+                    assert torch.equal(r.keys[:n], ref["keys"]) and torch.equal(r.vals[:n], ref["vals"]) and torch.equal(r.ranges, ref["ranges"])
+                    assert torch.equal(r.color, ref["color"]) and torch.equal(r.n_last, ref["n_last"])
+                    assert float((G["means"] - ref["means"]).abs().max()) <= 2e-4 * float(ref["means"].abs().max())
+        except BaseException as e:      # noqa: BLE001 - reported by the main thread
+            errors.append(repr(e))
+
+    threads = [threading.Thread(target=work, args=(j,)) for j in jobs]
+    for t in threads: t.start()
+    for t in threads: t.join()
+    assert not errors, errors

@@ -35,7 +35,7 @@ STAGES_STAGED = ["preprocess", "depth_order", "tile_query", "sort", "tile_ranges
 # SphericalOffset as implemented, FMA = 2): an EVALUATED pair costs 41 (forward) / 46 (backward: the same evaluation + the reach
 # test and exp kept for the gradient), a CONTRIBUTING pair another 9 (forward: blend) / 72 (backward: gradient chain + its share
 # of the warp reduction).
-FLOP_FWD_EVAL, FLOP_FWD_EARLY, FLOP_FWD_CONTRIB, FLOP_BWD_EVAL, FLOP_BWD_CONTRIB = 41, 16, 9, 46, 72
+FLOP_FWD_EVAL, FLOP_FWD_CONTRIB, FLOP_BWD_EVAL, FLOP_BWD_CONTRIB = 41, 9, 46, 72
 # the ONE bounded oracle sample both arms time (--impl reference, and the cpu_baseline leg of the default arm)
 ORACLE_SAMPLE = dict(n_pre=500_000, n_query=60_000, n_tiles_sample=192)
 
@@ -315,8 +315,8 @@ def per_kernel_table(m, peaks, fp32_peak):
     for s_, ms in m["stage_ms"].items():
         sec = ms * 1e-3
         if s_ == "render_fwd":
-            # executed work: full evaluations 41, evaluations stopped by the early out 16 (a, b, q), contributing pairs + 9
-            flop = m["ev_full"] * FLOP_FWD_EVAL + (m["ev_cull"] - m["ev_full"]) * FLOP_FWD_EARLY + m["contrib"] * FLOP_FWD_CONTRIB
+            # executed work: evaluations that pass the patch cull 41, contributing pairs + 9
+            flop = m["ev_cull"] * FLOP_FWD_EVAL + m["contrib"] * FLOP_FWD_CONTRIB
             flop_alg = m["ev_f"] * FLOP_FWD_EVAL + m["contrib"] * FLOP_FWD_CONTRIB
             out[s_] = dict(ms=ms, bound="alu", tflops=flop / sec / 1e12, frac_fp32_peak=flop / sec / 1e12 / fp32_peak,
                            frac_fp32_peak_alg1_units=flop_alg / sec / 1e12 / fp32_peak)
@@ -569,9 +569,9 @@ def run_ours(args):
                 config=workload_config(args.config, world, n_pix_active),
                 path=dict(lists=args.lists, marks=args.marks, n_pairs=m["n_pairs"]),
                 ms_forward=m["ms_fwd"], ms_forward_backward=ms_step, stage_ms=m["stage_ms"], per_kernel=pk,
-                evaluated_pairs=dict(forward=m["ev_f"], forward_after_patch_cull=m["ev_cull"], forward_in_full=m["ev_full"], contributing=m["contrib"], backward_alg1=m["ev_b"], backward_executed=m["ev_b_visited"],
+                evaluated_pairs=dict(forward=m["ev_f"], forward_after_patch_cull=m["ev_cull"], forward_q_above_cut=m["ev_full"], contributing=m["contrib"], backward_alg1=m["ev_b"], backward_executed=m["ev_b_visited"],
                                      listed=int(m["n_pairs"]) * cfg.ppt,
-                                     note="forward (Alg.1's loop) / after the patch cull / in full (after the early out) / contributing: counted on the device by uts_render_fwd_counted; backward_alg1: sum of n_last; "
+                                     note="forward (Alg.1's loop) / after the patch cull (what the forward executes) / of those, patches where q alone cannot rule the entry out (informational) / contributing: counted on the device by uts_render_fwd_counted; backward_alg1: sum of n_last; "
                                           "backward_executed: 32 x marked (patch, entry) pairs; listed: pairs x 256 pixels"),
                 roofline=roof, clocks=m["clocks"], extras=extras,
                 e2e=dict(value=replicas.aggregate_throughput(n_pix_active, e2e_ms_max, world), unit=UNIT, ms_per_step=e2e_ms_max, steps=e2e_steps,

@@ -208,10 +208,11 @@ int uts_render_fwd(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
                    float* color, float* alpha, float* trans, uint32_t* n_last, void* stream);
 
 /* uts_render_fwd that also counts its work (measurement only: bench.py's roofline lines), walking every entry in full, i.e. without
- * the patch cull and the early out of the production kernels (its image is the reference of their bit-identity).  Adds to work[0] the
+ * the patch cull of the production kernels (its image is the reference of their bit-identity).  Adds to work[0] the
  * (pixel, entry) pairs Alg.1's loop evaluates (every entry a pixel visits before it stops, l.20-28 PAPER.md:568-584), to work[1] those
- * that contribute (alpha >= alpha_min), to work[2] those the production forward evaluates at all (the entry passes the patch cull) and
- * to work[3] those it evaluates in full (it also passes the early out).  work: 4 DEVICE uint64, zeroed by the caller.  Outputs as
+ * that contribute (alpha >= alpha_min), to work[2] those the production forward evaluates (the entry passes the patch cull) and
+ * to work[3] those of work[2] whose patch has an open pixel with q above the alpha_min cut (what a patch-level early out on q alone
+ * would leave; informational, the production forward takes no such early out).  work: 4 DEVICE uint64, zeroed by the caller.  Outputs as
  * uts_render_fwd. */
 int uts_render_fwd_counted(const uts_config* cfg, uts_proj in, uts_mask mask, const uint64_t* ranges, const uint32_t* vals,
                            float* color, float* alpha, float* trans, uint32_t* n_last, uint64_t* work, void* stream);

@@ -32,12 +32,14 @@ struct RenderParams {
 };
 
 constexpr float kLog2e = 1.4426950408889634f;
-// Pixels per thread (PX) of the two kernels: a block has 256 / PX threads.  Measured on config 4 (B200): the forward is bound by
-// the per-evaluation arithmetic, not by the shared-memory reads or the loop (the same 2.9e9 warp instructions at PX = 1 and 4),
-// so it keeps one pixel per thread and the occupancy that goes with it; the backward gains from PX = 4 because one warp
-// reduction + one set of atomics then serves the four patches of a warp.
+// Pixels per thread (PX) of the two kernels: a block has 256 / PX threads and a warp owns PX consecutive patches of 32 pixels.
+// Measured on config 4 (B200): with scalar arithmetic the forward is bound by the per-evaluation instructions, not by the
+// shared-memory reads or the loop (the same 2.9e9 warp instructions at PX = 1 and 4), and more pixels per thread only cost
+// occupancy; with PX = 2 the two pixels' evaluations go through packed fp32 pairs (FFMA2 / FMUL2, eval_entry2): half the
+// arithmetic instructions per pixel, 2.53 -> 2.10 ms.  The backward gains from PX = 4 because one warp reduction + one set of
+// atomics then serves the four patches of a warp.
 #ifndef UTS_FWD_PX
-#define UTS_FWD_PX 1
+#define UTS_FWD_PX 2
 #endif
 #ifndef UTS_BWD_PX
 #define UTS_BWD_PX 4
@@ -68,6 +70,15 @@ __device__ __forceinline__ float4 lds128(uint32_t addr) {
   asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
   return v;
 }
+// Packed fp32 pairs (sm_100: fma / mul / add .f32x2 — one instruction, two IEEE roundings, the same results as the scalar forms).
+// A pair is a 64-bit register; f2_bc(s) = (s, s) costs nothing (ptxas folds it into a scalar operand of FFMA2 / FMUL2 / FADD2).
+typedef unsigned long long f2_t;
+__device__ __forceinline__ f2_t f2_pack(float lo, float hi) { f2_t d; asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi)); return d; }
+__device__ __forceinline__ f2_t f2_bc(float s) { return f2_pack(s, s); }
+__device__ __forceinline__ void f2_unpack(f2_t v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f2_t f2_fma(f2_t a, f2_t b, f2_t c) { f2_t d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ f2_t f2_mul(f2_t a, f2_t b) { f2_t d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f2_t f2_add(f2_t a, f2_t b) { f2_t d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 __device__ __forceinline__ void red_add_global(float* p, float v) {       // p is a global address (cudaMalloc'ed gradient buffer)
   asm volatile("red.global.add.f32 [%0], %1;" :: "l"(p), "f"(v) : "memory");
 }
@@ -155,6 +166,36 @@ __device__ __forceinline__ void eval_entry(const float4 g0, const float4 g1, con
 // Alg.1 l.23 (reading A7): power > 0 skipped; power below the alpha_min cut skipped (see stage_entry)
 __device__ __forceinline__ bool may_contribute(const Eval& ev, float th) { return !(ev.p2 > 0.f) && ev.p2 >= th; }
 
+// eval_entry for two pixels at once: the same operations in the same order on packed pairs, so a, b, c, k and p2 are bit-identical to
+// two scalar calls (the backward and the counted forward keep the scalar form and rely on that; a test compares the images bit by bit).
+__device__ __forceinline__ void eval_entry2(const float4 g0, const float4 g1, const float4 g2, const float4 g3, f2_t px, f2_t py, f2_t pz,
+                                            float& p2_0, float& p2_1) {
+  const f2_t a = f2_fma(f2_bc(g1.x), px, f2_fma(f2_bc(g1.y), pz, f2_bc(g0.x)));
+  const f2_t b = f2_fma(f2_bc(g1.z), px, f2_fma(f2_bc(g1.w), py, f2_fma(f2_bc(g2.x), pz, f2_bc(g0.y))));
+  const f2_t c = f2_fma(f2_bc(g2.y), px, f2_fma(f2_bc(g2.z), py, f2_fma(f2_bc(g2.w), pz, f2_bc(g0.z))));
+  float c0, c1;
+  f2_unpack(c, c0, c1);
+  f2_t k;
+  if (c0 >= 0.f && c1 >= 0.f) {                        // acos_poly(c) * rsqrt(1 + c), both pixels
+    f2_t p = f2_fma(f2_bc(-0.00115729403f), c, f2_bc(0.00628544204f));
+    p = f2_fma(p, c, f2_bc(-0.016528869f));
+    p = f2_fma(p, c, f2_bc(0.0304812621f));
+    p = f2_fma(p, c, f2_bc(-0.0500148833f));
+    p = f2_fma(p, c, f2_bc(0.0889478773f));
+    p = f2_fma(p, c, f2_bc(-0.214596227f));
+    p = f2_fma(p, c, f2_bc(1.57079625f));
+    float s0, s1;
+    f2_unpack(f2_add(f2_bc(1.0f), c), s0, s1);
+    k = f2_mul(p, f2_pack(rsqrt_approx(s0), rsqrt_approx(s1)));
+  } else {                                             // a pixel beyond 90 degrees: the scalar form
+    float a0, a1, b0, b1;
+    f2_unpack(a, a0, a1); f2_unpack(b, b0, b1);
+    k = f2_pack(arc_over_sin(fmaf(a0, a0, b0 * b0), c0), arc_over_sin(fmaf(a1, a1, b1 * b1), c1));
+  }
+  const f2_t q = f2_fma(a, f2_fma(f2_bc(g3.x), a, f2_mul(f2_bc(g3.y), b)), f2_mul(f2_mul(f2_bc(g3.z), b), b));
+  f2_unpack(f2_mul(f2_mul(q, k), k), p2_0, p2_1);
+}
+
 // Pixel and tile set-up common to both kernels.
 template <int PX>
 struct TileSetup { bool on[PX]; float px[PX], py[PX], pz[PX]; size_t out0; uint64_t start, end; int v; int64_t tile; };
@@ -168,14 +209,15 @@ __device__ __forceinline__ void setup_tile(const RenderParams& rp, const uint32_
   ts.v = (int)(blockIdx.x / rp.n_slot);
   const int64_t tile = active_tiles ? (int64_t)__ldg(active_tiles + slot) : slot;
   ts.tile = tile;
-  ts.out0 = ((size_t)ts.v * rp.n_slot + slot) * kTilePix + threadIdx.x;       // pixel j of this thread: out0 + kThreads j
+  const uint32_t pix0 = (threadIdx.x >> 5) * (32u * PX) + (threadIdx.x & 31u);  // a warp owns PX consecutive patches of 32 pixels
+  ts.out0 = ((size_t)ts.v * rp.n_slot + slot) * kTilePix + pix0;                 // pixel j of this thread: out0 + 32 j
   const uint64_t rix = 2 * ((uint64_t)ts.v * rp.n_tile + tile);
   ts.start = __ldg(ranges + rix); ts.end = __ldg(ranges + rix + 1);
   if (threadIdx.x == 0) pix_center_cam(rp.k - kTileLog2, (uint64_t)tile, s_tf->cx, s_tf->cy, s_tf->cz);
   double wx[PX], wy[PX], wz[PX];
 #pragma unroll
   for (int j = 0; j < PX; ++j) {
-    const uint64_t p = (uint64_t)tile * kTilePix + threadIdx.x + kThreads * j;
+    const uint64_t p = (uint64_t)tile * kTilePix + pix0 + 32u * j;
     ts.on[j] = mask_bits ? ((__ldg(mask_bits + (p >> 5)) >> (p & 31)) & 1u) != 0 : true;
     pix_center_cam(rp.k, p, wx[j], wy[j], wz[j]);
   }
@@ -187,8 +229,8 @@ __device__ __forceinline__ void setup_tile(const RenderParams& rp, const uint32_
 }
 
 // Marks (uts_render_fwd_marked / uts_render_bwd_marked): one bit per (patch, list entry), set by the forward when at least one
-// of the patch's 32 pixels blended the entry.  Patch (j, warp) — pixels (256 / PX) j + 32 warp + lane — is plane (8 / PX) j + warp
-// of 8, whatever PX the forward and the backward were built with; the bits
+// of the patch's 32 pixels blended the entry.  Patch (warp, j) — pixels 32 (PX warp + j) + lane, a warp owns PX consecutive patches —
+// is plane PX warp + j of 8, whatever PX the forward and the backward were built with; the bits
 // of (view, tile) vt start at word (start_vt >> 5) + vt of the plane, entry i of the list at bit i of that run — runs of
 // different tiles never share a word.  The backward visits an entry only for the patches whose bit is set: on the paper's kind of
 // scene half of the (patch, entry) visits would re-evaluate alpha just to find that no pixel of the patch took the entry.
@@ -252,29 +294,36 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
   for (int j = 0; j < PX; ++j) { T[j] = 1.f; Cr[j] = Cg[j] = Cb[j] = Cd[j] = 0.f; n_last[j] = 0; if (ts.on[j]) open |= 1u << j; }
   const uint64_t len = ts.end - ts.start;
   const uint32_t sS = (uint32_t)__cvta_generic_to_shared(&S);
-  uint32_t* mark_w = nullptr;                         // plane `wid` of this tile's run; patch j is kWarps j planes further
-  if (MARK) mark_w = marks + (uint64_t)wid * plane_words + mark_base<PX>(rp, ts);
+  uint32_t* mark_w = nullptr;                         // plane PX wid of this tile's run; patch j is j planes further
+  if (MARK) mark_w = marks + (uint64_t)(PX * wid) * plane_words + mark_base<PX>(rp, ts);
   // Patch cull (PX = 1: a warp is one 8x4 patch).  At the start of a group of 32 entries lane l asks whether entry l can reach the
   // patch at all: with the patch's centre pc and radius r (in the tile frame; the map to the Gaussian's (a, b) plane is an
   // isometry of the chord), sqrt(-q) >= N(pc) - r L everywhere on the patch, so N(pc) - r L > sqrt(-th) means every pixel's power
   // is below the alpha_min cut.  The ballot's survivors are walked as before, the others cost two instructions.  No per-pixel
   // decision changes (such an entry fails may_contribute() at every pixel); the margin 1.0001 covers the fp32 rounding of the
   // bound.  A warp whose last tested group kept >= 24 of 32 entries (config 4: large near Gaussians) skips the test for 3 groups.
-  float pcx = 0.f, pcy = 0.f, pcz = 0.f, prad = 0.f;
+  constexpr bool kCull = PX <= 2;                     // per patch j of the warp (PX = 2: an entry is walked when it reaches either)
+  float pcx[PX], pcy[PX], pcz[PX], prad[PX];
   int skip_tests = 0;
-  if (PX == 1) {
-    pcx = ts.px[0]; pcy = ts.py[0]; pcz = ts.pz[0];
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) {
-      pcx += __shfl_xor_sync(0xffffffffu, pcx, d); pcy += __shfl_xor_sync(0xffffffffu, pcy, d); pcz += __shfl_xor_sync(0xffffffffu, pcz, d);
+  for (int j = 0; j < PX; ++j) {
+    pcx[j] = pcy[j] = pcz[j] = prad[j] = 0.f;
+    if (kCull) {
+      float sx = ts.px[j], sy = ts.py[j], sz = ts.pz[j];
+#pragma unroll
+      for (int d = 16; d > 0; d >>= 1) {
+        sx += __shfl_xor_sync(0xffffffffu, sx, d); sy += __shfl_xor_sync(0xffffffffu, sy, d); sz += __shfl_xor_sync(0xffffffffu, sz, d);
+      }
+      pcx[j] = sx * (1.f / 32.f); pcy[j] = sy * (1.f / 32.f); pcz[j] = sz * (1.f / 32.f);
+      const float ex = ts.px[j] - pcx[j], ey = ts.py[j] - pcy[j], ez = ts.pz[j] - pcz[j];
+      float r = sqrtf(ex * ex + ey * ey + ez * ez);
+#pragma unroll
+      for (int d = 16; d > 0; d >>= 1) r = fmaxf(r, __shfl_xor_sync(0xffffffffu, r, d));
+      prad[j] = r * 1.00001f;
     }
-    pcx *= (1.f / 32.f); pcy *= (1.f / 32.f); pcz *= (1.f / 32.f);
-    const float ex = ts.px[0] - pcx, ey = ts.py[0] - pcy, ez = ts.pz[0] - pcz;
-    prad = sqrtf(ex * ex + ey * ey + ez * ez);
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) prad = fmaxf(prad, __shfl_xor_sync(0xffffffffu, prad, d));
-    prad *= 1.00001f;
   }
+  f2_t px2 = 0, py2 = 0, pz2 = 0;                     // PX = 2: the two pixels' coordinates as packed pairs
+  if (PX == 2) { px2 = f2_pack(ts.px[0], ts.px[PX - 1]); py2 = f2_pack(ts.py[0], ts.py[PX - 1]); pz2 = f2_pack(ts.pz[0], ts.pz[PX - 1]); }
   for (uint64_t b0 = 0; b0 < len; b0 += kBatch) {
     if (__syncthreads_and(open == 0)) break;          // every pixel of the tile saturated (or masked)
     const uint64_t left_n = len - b0;
@@ -290,8 +339,8 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
 #pragma unroll
       for (int j = 0; j < PX; ++j) mw[j] = 0u;
       const int ge = min(nb, g0 + 32);
-      uint32_t live = 0xffffffffu;                    // bit e: entry g0 + e may reach this patch
-      if (PX == 1) {
+      uint32_t live = 0xffffffffu;                    // bit e: entry g0 + e may reach a patch of this warp
+      if (kCull) {
         if (skip_tests > 0) --skip_tests;
         else {
           const int e = g0 + (int)(threadIdx.x & 31);
@@ -299,11 +348,14 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
           if (e < nb) {
             const uint32_t se = sS + (uint32_t)e * 16u;
             const float4 h0 = lds128(se), h1 = lds128(se + kRow), h2 = lds128(se + 2u * kRow), h3 = lds128(se + 3u * kRow), h5 = lds128(se + 5u * kRow);
-            const float ac = fmaf(h1.x, pcx, fmaf(h1.y, pcz, h0.x));
-            const float bc = fmaf(h1.z, pcx, fmaf(h1.w, pcy, fmaf(h2.x, pcz, h0.y)));
-            const float nq = -fmaf(ac, fmaf(h3.x, ac, h3.y * bc), h3.z * bc * bc);     // -q at the patch centre
-            const float slack = sqrtf(fmaxf(nq, 0.f)) - prad * h5.x;
-            reach = !(slack > 0.f && slack * slack > -h0.w * 1.0002f);
+#pragma unroll
+            for (int j = 0; j < PX; ++j) {
+              const float ac = fmaf(h1.x, pcx[j], fmaf(h1.y, pcz[j], h0.x));
+              const float bc = fmaf(h1.z, pcx[j], fmaf(h1.w, pcy[j], fmaf(h2.x, pcz[j], h0.y)));
+              const float nq = -fmaf(ac, fmaf(h3.x, ac, h3.y * bc), h3.z * bc * bc);   // -q at the patch centre
+              const float slack = sqrtf(fmaxf(nq, 0.f)) - prad[j] * h5.x;
+              reach = reach || !(slack > 0.f && slack * slack > -h0.w * 1.0002f);
+            }
           }
           live = __ballot_sync(0xffffffffu, reach);
           if (__popc(live) >= 24) skip_tests = 3;
@@ -315,11 +367,18 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
           const int jj = j4 + u;
-          if (PX == 1 && !COUNT && !((live >> (jj - g0)) & 1u)) continue;
+          if (kCull && !COUNT && !((live >> (jj - g0)) & 1u)) continue;
           const uint32_t sa = sS + (uint32_t)jj * 16u;
           const float4 g0v = lds128(sa), g1 = lds128(sa + kRow), g2 = lds128(sa + 2u * kRow), g3 = lds128(sa + 3u * kRow);
           float p2[PX];
           uint32_t cand = 0;                          // bit j: pixel j may blend this entry
+          if (PX == 2 && !COUNT) {                    // both pixels in packed arithmetic
+            eval_entry2(g0v, g1, g2, g3, px2, py2, pz2, p2[0], p2[PX - 1]);
+            Eval e0, e1;
+            e0.p2 = p2[0]; e1.p2 = p2[PX - 1];
+            if ((open & 1u) && may_contribute(e0, g0v.w)) cand |= 1u;
+            if ((open & 2u) && may_contribute(e1, g0v.w)) cand |= 2u;
+          } else
 #pragma unroll
           for (int j = 0; j < PX; ++j) {
             p2[j] = 1.f;
@@ -343,8 +402,8 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
               if (((open >> j) & 1u) && may_contribute(ev, g0v.w)) cand |= 1u << j;
             }
           }
-          if (PX > 1 && !__any_sync(0xffffffffu, cand != 0)) continue;
-          if (PX == 1 && cand == 0) continue;
+          if (PX > 2 && !__any_sync(0xffffffffu, cand != 0)) continue;
+          if (PX <= 2 && cand == 0) continue;
           const float4 g4 = lds128(sa + 4u * kRow);
           const uint32_t bit = 1u << (jj - g0);
 #pragma unroll
@@ -367,7 +426,7 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
 #pragma unroll
         for (int j = 0; j < PX; ++j) {
           const uint32_t gw = __reduce_or_sync(0xffffffffu, mw[j]);
-          if ((threadIdx.x & 31) == 0) mark_w[(uint64_t)(kWarps * j) * plane_words + ((b0 + (uint64_t)g0) >> 5)] = gw;
+          if ((threadIdx.x & 31) == 0) mark_w[(uint64_t)j * plane_words + ((b0 + (uint64_t)g0) >> 5)] = gw;
         }
       }
     }
@@ -382,7 +441,7 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
   }
 #pragma unroll
   for (int j = 0; j < PX; ++j) {
-    const size_t o = ts.out0 + (size_t)kThreads * j;
+    const size_t o = ts.out0 + (size_t)32 * j;
     if (ts.on[j]) {
       color[3 * o] = fmaf(T[j], rp.bg[0], Cr[j]); color[3 * o + 1] = fmaf(T[j], rp.bg[1], Cg[j]); color[3 * o + 2] = fmaf(T[j], rp.bg[2], Cb[j]);
       alpha_out[o] = 1.f - T[j]; trans_out[o] = T[j]; n_last_out[o] = n_last[j];
@@ -430,7 +489,7 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
   uint32_t m = 0;
 #pragma unroll
   for (int j = 0; j < PX; ++j) {
-    const size_t o = ts.out0 + (size_t)kThreads * j;
+    const size_t o = ts.out0 + (size_t)32 * j;
     const bool on = ts.on[j];
     nl[j] = on ? __ldg(n_last_in + o) : 0u;
     const float Tfin = on ? __ldg(trans + o) : 1.f;
@@ -465,7 +524,7 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
   const int n_batch = (int)((max_nl + kBatch - 1) / kBatch);
   // lane 8 j + g (j < PX) reads word g of patch j's plane, kWarps j + wid
   const uint32_t* mark_w = nullptr;
-  if (MARK && lane < 8 * PX) mark_w = marks + (uint64_t)(kWarps * (lane >> 3) + wid) * plane_words + mark_base<PX>(rp, ts);
+  if (MARK && lane < 8 * PX) mark_w = marks + (uint64_t)(PX * wid + (lane >> 3)) * plane_words + mark_base<PX>(rp, ts);
   for (int bi = n_batch - 1; bi >= 0; --bi) {
     const uint32_t b0 = (uint32_t)bi * kBatch;
     // The forward wrote a patch's words up to the last entry any of its pixels blended; words beyond that hold whatever the

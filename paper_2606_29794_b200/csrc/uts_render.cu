@@ -322,7 +322,8 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
       prad[j] = r * 1.00001f;
     }
   }
-  f2_t px2 = 0, py2 = 0, pz2 = 0;                     // PX = 2: the two pixels' coordinates as packed pairs
+  f2_t px2 = 0, py2 = 0, pz2 = 0;                     // PX = 2: the two pixels' coordinates, T and colour sums as packed pairs
+  f2_t T2 = f2_bc(1.f), Cr2 = 0, Cg2 = 0, Cb2 = 0, Cd2 = 0;
   if (PX == 2) { px2 = f2_pack(ts.px[0], ts.px[PX - 1]); py2 = f2_pack(ts.py[0], ts.py[PX - 1]); pz2 = f2_pack(ts.pz[0], ts.pz[PX - 1]); }
   for (uint64_t b0 = 0; b0 < len; b0 += kBatch) {
     if (__syncthreads_and(open == 0)) break;          // every pixel of the tile saturated (or masked)
@@ -376,8 +377,25 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
             eval_entry2(g0v, g1, g2, g3, px2, py2, pz2, p2[0], p2[PX - 1]);
             Eval e0, e1;
             e0.p2 = p2[0]; e1.p2 = p2[PX - 1];
-            if ((open & 1u) && may_contribute(e0, g0v.w)) cand |= 1u;
-            if ((open & 2u) && may_contribute(e1, g0v.w)) cand |= 2u;
+            bool c0 = (open & 1u) && may_contribute(e0, g0v.w), c1 = (open & 2u) && may_contribute(e1, g0v.w);
+            if (!(c0 || c1)) continue;
+            // The blend of both pixels, packed and branch-free: a pixel that does not take the entry gets alpha = 0, which leaves its
+            // T and colour sums exactly as they were (w = T 0 = 0, C + 0 c = C, T (1 - 0) = T).
+            const float4 g4 = lds128(sa + 4u * kRow);
+            float a0 = fminf(rp.amax, g3.w * ex2_approx(p2[0])), a1 = fminf(rp.amax, g3.w * ex2_approx(p2[PX - 1]));
+            c0 = c0 && !(a0 < rp.amin); c1 = c1 && !(a1 < rp.amin);
+            a0 = c0 ? a0 : 0.f; a1 = c1 ? a1 : 0.f;
+            const f2_t al = f2_pack(a0, a1);
+            const f2_t w = f2_mul(T2, al);              // Eq.6: c_i alpha_i prod_{j<i} (1 - alpha_j)
+            Cr2 = f2_fma(w, f2_bc(g4.x), Cr2); Cg2 = f2_fma(w, f2_bc(g4.y), Cg2); Cb2 = f2_fma(w, f2_bc(g4.z), Cb2);
+            if (DEPTH) Cd2 = f2_fma(w, f2_bc(g4.w), Cd2);
+            T2 = f2_mul(T2, f2_fma(al, f2_bc(-1.f), f2_bc(1.f)));
+            float t0, t1;
+            f2_unpack(T2, t0, t1);
+            const uint32_t bit = 1u << (jj - g0), nl = (uint32_t)(b0 + jj) + 1u;
+            if (c0) { if (MARK) mw[0] |= bit; n_last[0] = nl; if (t0 < rp.teps) open &= ~1u; }      // Alg.1 l.27: test after the update
+            if (c1) { if (MARK) mw[PX - 1] |= bit; n_last[PX - 1] = nl; if (t1 < rp.teps) open &= ~2u; }
+            continue;
           } else
 #pragma unroll
           for (int j = 0; j < PX; ++j) {
@@ -430,6 +448,10 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
         }
       }
     }
+  }
+  if (PX == 2 && !COUNT) {
+    f2_unpack(T2, T[0], T[PX - 1]); f2_unpack(Cr2, Cr[0], Cr[PX - 1]); f2_unpack(Cg2, Cg[0], Cg[PX - 1]); f2_unpack(Cb2, Cb[0], Cb[PX - 1]);
+    if (DEPTH) f2_unpack(Cd2, Cd[0], Cd[PX - 1]);
   }
   if (COUNT) {
     const uint32_t e = __reduce_add_sync(0xffffffffu, n_eval), c = __reduce_add_sync(0xffffffffu, n_contrib);

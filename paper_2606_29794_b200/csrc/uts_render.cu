@@ -168,8 +168,9 @@ __device__ __forceinline__ bool may_contribute(const Eval& ev, float th) { retur
 
 // eval_entry for two pixels at once: the same operations in the same order on packed pairs, so a, b, c, k and p2 are bit-identical to
 // two scalar calls (the backward and the counted forward keep the scalar form and rely on that; a test compares the images bit by bit).
+struct Eval2 { f2_t a, b, c, k, p2; };
 __device__ __forceinline__ void eval_entry2(const float4 g0, const float4 g1, const float4 g2, const float4 g3, f2_t px, f2_t py, f2_t pz,
-                                            float& p2_0, float& p2_1) {
+                                            Eval2& ev) {
   const f2_t a = f2_fma(f2_bc(g1.x), px, f2_fma(f2_bc(g1.y), pz, f2_bc(g0.x)));
   const f2_t b = f2_fma(f2_bc(g1.z), px, f2_fma(f2_bc(g1.w), py, f2_fma(f2_bc(g2.x), pz, f2_bc(g0.y))));
   const f2_t c = f2_fma(f2_bc(g2.y), px, f2_fma(f2_bc(g2.z), py, f2_fma(f2_bc(g2.w), pz, f2_bc(g0.z))));
@@ -193,8 +194,10 @@ __device__ __forceinline__ void eval_entry2(const float4 g0, const float4 g1, co
     k = f2_pack(arc_over_sin(fmaf(a0, a0, b0 * b0), c0), arc_over_sin(fmaf(a1, a1, b1 * b1), c1));
   }
   const f2_t q = f2_fma(a, f2_fma(f2_bc(g3.x), a, f2_mul(f2_bc(g3.y), b)), f2_mul(f2_mul(f2_bc(g3.z), b), b));
-  f2_unpack(f2_mul(f2_mul(q, k), k), p2_0, p2_1);
+  ev.a = a; ev.b = b; ev.c = c; ev.k = k;
+  ev.p2 = f2_mul(f2_mul(q, k), k);
 }
+__device__ __forceinline__ bool may_contribute(float p2, float th) { return !(p2 > 0.f) && p2 >= th; }
 
 // Pixel and tile set-up common to both kernels.
 template <int PX>
@@ -374,10 +377,10 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
           float p2[PX];
           uint32_t cand = 0;                          // bit j: pixel j may blend this entry
           if (PX == 2 && !COUNT) {                    // both pixels in packed arithmetic
-            eval_entry2(g0v, g1, g2, g3, px2, py2, pz2, p2[0], p2[PX - 1]);
-            Eval e0, e1;
-            e0.p2 = p2[0]; e1.p2 = p2[PX - 1];
-            bool c0 = (open & 1u) && may_contribute(e0, g0v.w), c1 = (open & 2u) && may_contribute(e1, g0v.w);
+            Eval2 ev2;
+            eval_entry2(g0v, g1, g2, g3, px2, py2, pz2, ev2);
+            f2_unpack(ev2.p2, p2[0], p2[PX - 1]);
+            bool c0 = (open & 1u) && may_contribute(p2[0], g0v.w), c1 = (open & 2u) && may_contribute(p2[PX - 1], g0v.w);
             if (!(c0 || c1)) continue;
             // The blend of both pixels, packed and branch-free: a pixel that does not take the entry gets alpha = 0, which leaves its
             // T and colour sums exactly as they were (w = T 0 = 0, C + 0 c = C, T (1 - 0) = T).
@@ -522,6 +525,18 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
     Sd[j] = 0.f; gd[j] = (DEPTH && on) ? __ldg(dL_ddepth + o) : 0.f;
     m = max(m, nl[j]);
   }
+  // PX even: the per-pixel state as packed pairs (pixels 2p, 2p + 1), walked with packed arithmetic (visit below)
+  constexpr bool kPack = (PX % 2) == 0;
+  constexpr int NP = kPack ? PX / 2 : 1;
+  f2_t px2[NP], py2[NP], pz2[NP], T2[NP], Sr2[NP], Sg2[NP], Sb2[NP], Sd2[NP], gr2[NP], gg2[NP], gb2[NP], gaT2[NP], gd2[NP];
+#pragma unroll
+  for (int q = 0; q < NP; ++q) {
+    const int j0 = kPack ? 2 * q : 0, j1 = kPack ? 2 * q + 1 : 0;
+    px2[q] = f2_pack(ts.px[j0], ts.px[j1]); py2[q] = f2_pack(ts.py[j0], ts.py[j1]); pz2[q] = f2_pack(ts.pz[j0], ts.pz[j1]);
+    T2[q] = f2_pack(T[j0], T[j1]); Sr2[q] = f2_pack(Sr[j0], Sr[j1]); Sg2[q] = f2_pack(Sg[j0], Sg[j1]); Sb2[q] = f2_pack(Sb[j0], Sb[j1]);
+    Sd2[q] = 0; gr2[q] = f2_pack(gr[j0], gr[j1]); gg2[q] = f2_pack(gg[j0], gg[j1]); gb2[q] = f2_pack(gb[j0], gb[j1]);
+    gaT2[q] = f2_pack(ga_T[j0], ga_T[j1]); gd2[q] = f2_pack(gd[j0], gd[j1]);
+  }
   // block maximum of n_last: entries beyond it were reached by no pixel
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, d));
@@ -567,6 +582,83 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
       const float2 g5 = *reinterpret_cast<const float2*>(&S.g[5][jj]);
       const float inv_r = DEPTH ? S.g[5][jj].z : 0.f;
       bool any_used = false;
+      if constexpr (kPack) {
+        // Two pixels (patches 2q, 2q + 1 of the warp) per step in packed fp32 pairs, branch-free: a pixel that did not take the
+        // entry gets alpha = 0 and zero gradient weights, which leave its state and every sum exactly as they were.
+        f2_t s_r = 0, s_g = 0, s_b = 0, s_A = 0, s_B = 0, s_C = 0, s_o = 0, s_om = 0, s_ph = 0, s_i = 0;
+        const float cA = -2.f / kLog2e * g3.x, cB = -1.f / kLog2e * g3.y, cC = -2.f / kLog2e * g3.z;   // conic (A,B,C)
+        const float sp = g5.x, cp = g5.y;
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+          if (!((pm >> (2 * q)) & 3u)) continue;       // warp-uniform: neither patch has the entry marked
+          Eval2 ev;
+          eval_entry2(g0v, g1, g2, g3, px2[q], py2[q], pz2[q], ev);
+          float p20, p21;
+          f2_unpack(ev.p2, p20, p21);
+          bool u0 = ((pm >> (2 * q)) & 1u) && jl < nl[2 * q] && may_contribute(p20, g0v.w);
+          bool u1 = ((pm >> (2 * q + 1)) & 1u) && jl < nl[2 * q + 1] && may_contribute(p21, g0v.w);
+          const float e20 = ex2_approx(p20), e21 = ex2_approx(p21);
+          const float raw0 = g3.w * e20, raw1 = g3.w * e21;
+          float a0 = fminf(rp.amax, raw0), a1 = fminf(rp.amax, raw1);
+          u0 = u0 && !(a0 < rp.amin); u1 = u1 && !(a1 < rp.amin);
+          if (!(u0 || u1)) continue;
+          any_used = true;
+          a0 = u0 ? a0 : 0.f; a1 = u1 ? a1 : 0.f;
+          const f2_t al = f2_pack(a0, a1);
+          float m0, m1;
+          f2_unpack(f2_fma(al, f2_bc(-1.f), f2_bc(1.f)), m0, m1);                        // 1 - alpha
+          const float i0 = u0 ? rcp_approx(fmaxf(m0, 1e-7f)) : 1.f, i1 = u1 ? rcp_approx(fmaxf(m1, 1e-7f)) : 1.f;
+          const f2_t inv = f2_pack(i0, i1), ninv = f2_pack(-i0, -i1);
+          const f2_t Tb = f2_mul(T2[q], inv);            // transmittance before this entry
+          const f2_t w = f2_mul(Tb, al);
+          s_r = f2_fma(w, gr2[q], s_r); s_g = f2_fma(w, gg2[q], s_g); s_b = f2_fma(w, gb2[q], s_b);
+          f2_t dLa = f2_mul(gr2[q], f2_fma(Tb, f2_bc(g4.x), f2_mul(Sr2[q], ninv)));
+          dLa = f2_fma(gg2[q], f2_fma(Tb, f2_bc(g4.y), f2_mul(Sg2[q], ninv)), dLa);
+          dLa = f2_fma(gb2[q], f2_fma(Tb, f2_bc(g4.z), f2_mul(Sb2[q], ninv)), dLa);
+          dLa = f2_fma(gaT2[q], inv, dLa);
+          Sr2[q] = f2_fma(w, f2_bc(g4.x), Sr2[q]); Sg2[q] = f2_fma(w, f2_bc(g4.y), Sg2[q]); Sb2[q] = f2_fma(w, f2_bc(g4.z), Sb2[q]);
+          if (DEPTH) {
+            s_i = f2_fma(w, gd2[q], s_i);
+            dLa = f2_fma(gd2[q], f2_fma(Tb, f2_bc(inv_r), f2_mul(Sd2[q], ninv)), dLa);
+            Sd2[q] = f2_fma(w, f2_bc(inv_r), Sd2[q]);
+          }
+          T2[q] = Tb;
+          // reading A7: no gradient through a clamped alpha
+          const bool h0 = u0 && !(raw0 > rp.amax), h1 = u1 && !(raw1 > rp.amax);
+          s_o = f2_fma(f2_pack(h0 ? e20 : 0.f, h1 ? e21 : 0.f), dLa, s_o);               // exp(power) dL/dalpha
+          const f2_t ngp = f2_mul(f2_pack(h0 ? -a0 : 0.f, h1 ? -a1 : 0.f), dLa);         // - dL/dpower
+          const f2_t dx = f2_mul(ev.k, ev.a), dy = f2_mul(ev.k, ev.b);
+          s_A = f2_fma(f2_mul(f2_mul(f2_bc(0.5f), dx), dx), ngp, s_A);
+          s_B = f2_fma(f2_mul(dx, dy), ngp, s_B);
+          s_C = f2_fma(f2_mul(f2_mul(f2_bc(0.5f), dy), dy), ngp, s_C);
+          const f2_t gdx = f2_mul(f2_fma(f2_bc(cA), dx, f2_mul(f2_bc(cB), dy)), ngp);
+          const f2_t gdy = f2_mul(f2_fma(f2_bc(cB), dx, f2_mul(f2_bc(cC), dy)), ngp);
+          // (dx,dy) = k(s,c) (a,b):  dk/ds / s = (c/den - k)/t,  dk/dc = -1/den,  den = s^2 + c^2;  t = 0: g_a = k gdx = gdx, g_c = 0
+          const f2_t t = f2_fma(ev.a, ev.a, f2_mul(ev.b, ev.b));
+          float t0, t1, den0, den1;
+          f2_unpack(t, t0, t1);
+          f2_unpack(f2_fma(ev.c, ev.c, t), den0, den1);
+          const f2_t iden = f2_pack(rcp_approx(den0), rcp_approx(den1));
+          const f2_t rt = f2_pack(t0 > 0.f ? rcp_approx(t0) : 0.f, t1 > 0.f ? rcp_approx(t1) : 0.f);
+          const f2_t gk = f2_fma(gdx, ev.a, f2_mul(gdy, ev.b));
+          const f2_t gkkp = f2_mul(gk, f2_mul(f2_fma(ev.c, iden, f2_mul(ev.k, f2_bc(-1.f))), rt));
+          const f2_t g_a = f2_fma(gkkp, ev.a, f2_mul(ev.k, gdx));
+          const f2_t g_b = f2_fma(gkkp, ev.b, f2_mul(ev.k, gdy));
+          const f2_t g_c = f2_mul(f2_mul(gk, f2_bc(-1.f)), iden);
+          // a = e.w, b = n.w, c = u.w with de/dom = -hh, dn/dom = -sin(phi) e, du/dom = cos(phi) e, dn/dphi = -u, du/dphi = n,
+          // and hh.w = cos(phi) c - sin(phi) b
+          s_om = f2_fma(g_a, f2_fma(f2_bc(-cp), ev.c, f2_mul(f2_bc(sp), ev.b)), s_om);
+          s_om = f2_fma(f2_mul(g_b, f2_bc(-sp)), ev.a, s_om);
+          s_om = f2_fma(f2_mul(g_c, f2_bc(cp)), ev.a, s_om);
+          s_ph = f2_fma(g_c, ev.b, s_ph);
+          s_ph = f2_fma(f2_mul(g_b, f2_bc(-1.f)), ev.c, s_ph);
+        }
+        float lo, hi;
+        f2_unpack(s_r, lo, hi); d_r = lo + hi; f2_unpack(s_g, lo, hi); d_g = lo + hi; f2_unpack(s_b, lo, hi); d_b = lo + hi;
+        f2_unpack(s_A, lo, hi); d_A = lo + hi; f2_unpack(s_B, lo, hi); d_B = lo + hi; f2_unpack(s_C, lo, hi); d_C = lo + hi;
+        f2_unpack(s_o, lo, hi); d_o = lo + hi; f2_unpack(s_om, lo, hi); d_om = lo + hi; f2_unpack(s_ph, lo, hi); d_ph = lo + hi;
+        if (DEPTH) { f2_unpack(s_i, lo, hi); d_i = lo + hi; }
+      } else
 #pragma unroll
       for (int j = 0; j < PX; ++j) {
         if (PX > 1 && !((pm >> j) & 1u)) continue;     // warp-uniform

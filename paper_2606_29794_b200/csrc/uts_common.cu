@@ -34,6 +34,7 @@ DeviceCtx* device_ctx() {
   ok = ok && cudaEventCreateWithFlags(&c->side_fork, cudaEventDisableTiming) == cudaSuccess;
   ok = ok && cudaEventCreateWithFlags(&c->side_join, cudaEventDisableTiming) == cudaSuccess;
   for (int i = 0; i < 4 && ok; ++i) ok = cudaEventCreateWithFlags(&c->ev[i], cudaEventDisableTiming) == cudaSuccess;
+  ok = ok && cudaHostAlloc(reinterpret_cast<void**>(&c->pin), 64, cudaHostAllocDefault) == cudaSuccess;
   if (!ok) { set_last_cuda_error(cudaGetLastError()); delete c; return nullptr; }
   table[dev] = c;
   return c;

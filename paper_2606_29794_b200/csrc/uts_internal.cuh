@@ -41,6 +41,7 @@ struct DeviceCtx {
   cudaEvent_t side_fork = nullptr, side_join = nullptr;
   cudaStream_t copy = nullptr;                      // uts_host_forward_backward: copies off the critical path
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  unsigned long long* pin = nullptr;                // 8 pinned host words: small device -> host reads in one copy (under mu)
   bool attrs_set[4] = {false, false, false, false}; // cudaFuncSetAttribute done, per translation unit (under mu)
   static constexpr int kOccSlots = 32;              // cached cudaOccupancyMaxActiveBlocksPerMultiprocessor results (under mu)
   uint64_t occ_key[kOccSlots] = {}; int occ_val[kOccSlots] = {}; int occ_n = 0;

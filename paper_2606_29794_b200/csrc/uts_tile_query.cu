@@ -965,6 +965,11 @@ MatLayout mat_layout(const uts_config* cfg, size_t base) {
   return L;
 }
 
+// three device words -> three consecutive words (a null source reads as 0)
+__global__ void gather3_kernel(const uint64_t* a, const uint64_t* b, const uint64_t* c, unsigned long long* out) {
+  out[0] = a ? *a : 0ull; out[1] = b ? *b : 0ull; out[2] = c ? *c : 0ull;
+}
+
 // One tile query on the ring-interval path (or the quadtree descent): host-side parameters, then count() and emit().
 struct QueryRun {
   const uts_config* cfg; uts_proj in; uts_mask mask; const uint32_t* emit_rank; cudaStream_t s;
@@ -1284,14 +1289,18 @@ int uts_tile_lists(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   uint32_t* flag_by_rank = reinterpret_cast<uint32_t*>(sp + ML.flag);
   uint64_t* scan_sums = reinterpret_cast<uint64_t*>(sp + ML.scan);
   if ((st = q.count(offsets, mat_ok ? &mp : nullptr, flag_by_rank, reinterpret_cast<uint64_t*>(sp + ML.rank_scan), scan_sums))) return st;
-  // host needs: small pairs, matrix pairs, matrix rows
+  // host needs: small pairs, matrix pairs, matrix rows — gathered on the device, one copy into the context's pinned words
   uint64_t h3[3] = {0, 0, 0};
-  UTS_CUDA(cudaMemcpyAsync(&h3[0], offsets + n, 8, cudaMemcpyDeviceToHost, s));
-  if (mat_ok) {
-    UTS_CUDA(cudaMemcpyAsync(&h3[1], mp.n_L, 8, cudaMemcpyDeviceToHost, s));
-    UTS_CUDA(cudaMemcpyAsync(&h3[2], mp.row_of_rank + n, 8, cudaMemcpyDeviceToHost, s));
+  {
+    DeviceCtx* c = q.ctx;
+    std::lock_guard<std::recursive_mutex> pin_lock(c->mu);
+    unsigned long long* g3 = reinterpret_cast<unsigned long long*>(sp + ML.misc) + 8;
+    gather3_kernel<<<1, 1, 0, s>>>(offsets + n, mat_ok ? reinterpret_cast<const uint64_t*>(mp.n_L) : nullptr, mat_ok ? mp.row_of_rank + n : nullptr, g3);
+    UTS_LAUNCH_CHECK();
+    UTS_CUDA(cudaMemcpyAsync(c->pin, g3, 24, cudaMemcpyDeviceToHost, s));
+    UTS_CUDA(cudaStreamSynchronize(s));
+    h3[0] = c->pin[0]; h3[1] = c->pin[1]; h3[2] = c->pin[2];
   }
-  UTS_CUDA(cudaStreamSynchronize(s));
   const uint64_t n_S = h3[0], n_L = h3[1], n_mat = h3[2];
   *h_n_pairs = n_S + n_L;
   if (*h_n_pairs > capacity) return UTS_ERR_CAPACITY;

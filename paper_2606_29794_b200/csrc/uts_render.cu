@@ -365,13 +365,19 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
           if (__popc(live) >= 24) skip_tests = 3;
         }
       }
-      for (int j4 = g0; j4 < ge; j4 += 4) {
+      // The entries of the group this warp visits (the cull's survivors), front to back; culled entries cost nothing.  Measured
+      // against testing the bit of every entry inside a walk unrolled by four with immediate addresses: config 4 (32 % culled)
+      // 1.98 -> 2.03 ms, config 5 (70 % culled) 2.61 -> 2.48 ms, config 3 0.50 -> 0.48 ms.
+      uint32_t walk = COUNT ? 0xffffffffu : live;
+      if (ge - g0 < 32) walk &= (1u << (ge - g0)) - 1u;
+      while (walk) {
         const uint32_t alive = __reduce_or_sync(0xffffffffu, open);
         if (alive == 0) { left = true; break; }       // every pixel of the warp is saturated
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
-          const int jj = j4 + u;
-          if (kCull && !COUNT && !((live >> (jj - g0)) & 1u)) continue;
+          if (!walk) break;
+          const int jj = g0 + __ffs((int)walk) - 1;
+          walk &= walk - 1u;
           const uint32_t sa = sS + (uint32_t)jj * 16u;
           const float4 g0v = lds128(sa), g1 = lds128(sa + kRow), g2 = lds128(sa + 2u * kRow), g3 = lds128(sa + 3u * kRow);
           float p2[PX];

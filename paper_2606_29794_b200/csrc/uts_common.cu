@@ -33,6 +33,7 @@ DeviceCtx* device_ctx() {
   ok = ok && cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) == cudaSuccess;
   ok = ok && cudaEventCreateWithFlags(&c->side_fork, cudaEventDisableTiming) == cudaSuccess;
   ok = ok && cudaEventCreateWithFlags(&c->side_join, cudaEventDisableTiming) == cudaSuccess;
+  ok = ok && cudaEventCreateWithFlags(&c->side_mid, cudaEventDisableTiming) == cudaSuccess;
   for (int i = 0; i < 4 && ok; ++i) ok = cudaEventCreateWithFlags(&c->ev[i], cudaEventDisableTiming) == cudaSuccess;
   ok = ok && cudaHostAlloc(reinterpret_cast<void**>(&c->pin), 64, cudaHostAllocDefault) == cudaSuccess;
   if (!ok) { set_last_cuda_error(cudaGetLastError()); delete c; return nullptr; }

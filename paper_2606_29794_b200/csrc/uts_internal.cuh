@@ -38,7 +38,7 @@ struct DeviceCtx {
   cudaStream_t aux[2] = {nullptr, nullptr};         // tile query: the three work shapes run side by side
   cudaEvent_t fork = nullptr, join[2] = {nullptr, nullptr};
   cudaStream_t side = nullptr;                      // uts_tile_lists: matrix transpose + popcount beside the small pairs' emit + sort
-  cudaEvent_t side_fork = nullptr, side_join = nullptr;
+  cudaEvent_t side_fork = nullptr, side_join = nullptr, side_mid = nullptr;
   cudaStream_t copy = nullptr;                      // uts_host_forward_backward: copies off the critical path
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
   unsigned long long* pin = nullptr;                // 8 pinned host words: small device -> host reads in one copy (under mu)

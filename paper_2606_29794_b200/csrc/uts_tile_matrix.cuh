@@ -45,11 +45,14 @@ __device__ __forceinline__ void transpose32(uint32_t (&x)[32]) {
   }
 }
 
-// flag_by_rank[emit_rank[k]] = 1 for the large discs perm[0 .. n_mat)
+// flag_by_rank[emit_rank[k]] = 1 for the large discs perm[0 .. n_mat); they emit no pairs of their own: counts[slot] = 0
 __global__ void mat_flag_kernel(const uint32_t* __restrict__ perm, const uint32_t* __restrict__ n_small, const uint32_t* __restrict__ emit_rank,
-                                uint32_t* __restrict__ flag_by_rank) {
+                                uint32_t* __restrict__ flag_by_rank, uint32_t* __restrict__ counts) {
   const uint32_t n_mat = n_small[3];
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_mat; i += gridDim.x * blockDim.x) flag_by_rank[emit_rank[perm[i]]] = 1u;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_mat; i += gridDim.x * blockDim.x) {
+    const uint32_t slot = emit_rank[perm[i]];
+    flag_by_rank[slot] = 1u; counts[slot] = 0u;
+  }
 }
 
 // per view: its rows, the width of its bit vectors and where they start
@@ -80,8 +83,7 @@ constexpr int kMatThreads = UTS_MAT_THREADS;
 __global__ void __launch_bounds__(kMatThreads, UTS_MAT_MINB)
 matrix_count_kernel(QueryParams qp, MatParams mp, const float* __restrict__ dir, const float* __restrict__ lonlat, const float* __restrict__ rho,
                     const float* __restrict__ rs, const int32_t* __restrict__ slot_of_tile, const uint32_t* __restrict__ active_words,
-                    const uint32_t* __restrict__ perm, const uint32_t* __restrict__ n_small, const uint32_t* __restrict__ emit_rank,
-                    uint32_t* __restrict__ counts) {
+                    const uint32_t* __restrict__ perm, const uint32_t* __restrict__ n_small, const uint32_t* __restrict__ emit_rank) {
   extern __shared__ int2 ring_tab[];                 // [rc_block], then the bitmap [n_words]
   uint32_t* bitmap = reinterpret_cast<uint32_t*>(ring_tab + qp.rc_block);
   __shared__ RingDisc s_disc;
@@ -153,7 +155,6 @@ matrix_count_kernel(QueryParams qp, MatParams mp, const float* __restrict__ dir,
       for (int w = tid; w < mp.n_words; w += kMatThreads) dst[w] = bitmap[w];
     }
     if (tid == 0) {
-      counts[slot] = 0;                                // this disc emits no pairs of its own
       const uint32_t gid = (uint32_t)(k - (int64_t)v * qp.P);
       mp.row_key[row] = ((unsigned long long)__float_as_uint(__ldg(rho + k)) << 32) | gid;        // reading A10
       atomicAdd(mp.n_L, (unsigned long long)s_total);

@@ -976,6 +976,7 @@ struct QueryRun {
   Dims d; int64_t n;
   QueryParams qp;
   bool ring_impl, use_large;
+  bool side_forked = false;          // count() put the matrix class on ctx->side: the caller joins
   uint32_t *counts, *list, *n_large, *n_small, *hist, *perm, *active;
   uint64_t* block_sums;
   const uint32_t* active_arg;
@@ -1118,7 +1119,7 @@ struct QueryRun {
       if (mp) {                                       // rows of the bit matrix: rank order of the matrix-class discs
         UTS_CUDA(cudaMemsetAsync(flag_by_rank, 0, (size_t)n * 4, s));
         UTS_CUDA(cudaMemsetAsync(mp->n_L, 0, 8, s));
-        mat_flag_kernel<<<ctx->sms * 4, 256, 0, s>>>(perm, n_small, emit_rank, flag_by_rank);
+        mat_flag_kernel<<<ctx->sms * 4, 256, 0, s>>>(perm, n_small, emit_rank, flag_by_rank, counts);
         UTS_LAUNCH_CHECK();
         int st = exclusive_scan_u32(flag_by_rank, n, rank_scan, rank_scan_sums, s);
         if (st) return st;
@@ -1135,13 +1136,6 @@ struct QueryRun {
         ring_query_block_kernel<false><<<bgrid, kLargeThreads, smem_block, s>>>(qp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small, emit_rank,
                                                                               counts, nullptr, nullptr, nullptr);
         UTS_LAUNCH_CHECK();
-        if (mp) {
-          const size_t smem_m = smem_block + (size_t)mp->n_words * 4;
-          const int occ = cached_occupancy(ctx, kOccMat, matrix_count_kernel, kMatThreads, smem_m);
-          matrix_count_kernel<<<(unsigned)ctx->sms * (unsigned)occ, kMatThreads, smem_m, s>>>(
-              qp, *mp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, mask.slot_of_tile ? active : nullptr, perm, n_small, emit_rank, counts);
-          UTS_LAUNCH_CHECK();
-        }
         ring_query_batch_kernel<kBatchB, false><<<wgrid, kLargeThreads, smem_b, ctx->aux[0]>>>(qp, 0, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, perm, n_small,
                                                                                    emit_rank, counts, nullptr, nullptr, nullptr);
         UTS_LAUNCH_CHECK();
@@ -1158,6 +1152,22 @@ struct QueryRun {
       const int stj = join();
       if (st) return st;
       if (stj) return stj;
+      if (mp) {
+        // The bitmap rows of the matrix class go to the context's side stream, behind the small discs' count: issue-bound geometry
+        // that then runs beside the host's read of the pair count and the small pairs' emit and radix sort (HBM-bound) instead of
+        // in front of them.  The caller joins (side_forked).
+        UTS_CUDA(cudaEventRecord(ctx->side_fork, s));
+        UTS_CUDA(cudaStreamWaitEvent(ctx->side, ctx->side_fork, 0));
+        side_forked = true;
+        const size_t smem_m = smem_block + (size_t)mp->n_words * 4;
+        const int occ = cached_occupancy(ctx, kOccMat, matrix_count_kernel, kMatThreads, smem_m);
+#ifndef UTS_MAT_SIDE_BLOCKS
+#define UTS_MAT_SIDE_BLOCKS 8
+#endif
+        matrix_count_kernel<<<(unsigned)ctx->sms * (unsigned)(occ < UTS_MAT_SIDE_BLOCKS ? occ : UTS_MAT_SIDE_BLOCKS), kMatThreads, smem_m, ctx->side>>>(
+            qp, *mp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, mask.slot_of_tile ? active : nullptr, perm, n_small, emit_rank);
+        UTS_LAUNCH_CHECK();
+      }
     } else {
       tile_query_kernel<false><<<qgrid + lgrid, kLargeThreads, dyn_smem, s>>>(qp, lgrid, in.dir, in.rho, in.rs, mask.slot_of_tile, active_arg, perm,
                                                                              n_small, list, n_large, emit_rank, counts, nullptr, nullptr, nullptr);
@@ -1288,33 +1298,9 @@ int uts_tile_lists(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   }
   uint32_t* flag_by_rank = reinterpret_cast<uint32_t*>(sp + ML.flag);
   uint64_t* scan_sums = reinterpret_cast<uint64_t*>(sp + ML.scan);
-  if ((st = q.count(offsets, mat_ok ? &mp : nullptr, flag_by_rank, reinterpret_cast<uint64_t*>(sp + ML.rank_scan), scan_sums))) return st;
-  // host needs: small pairs, matrix pairs, matrix rows — gathered on the device, one copy into the context's pinned words
-  uint64_t h3[3] = {0, 0, 0};
-  {
-    DeviceCtx* c = q.ctx;
-    std::lock_guard<std::recursive_mutex> pin_lock(c->mu);
-    unsigned long long* g3 = reinterpret_cast<unsigned long long*>(sp + ML.misc) + 8;
-    gather3_kernel<<<1, 1, 0, s>>>(offsets + n, mat_ok ? reinterpret_cast<const uint64_t*>(mp.n_L) : nullptr, mat_ok ? mp.row_of_rank + n : nullptr, g3);
-    UTS_LAUNCH_CHECK();
-    UTS_CUDA(cudaMemcpyAsync(c->pin, g3, 24, cudaMemcpyDeviceToHost, s));
-    UTS_CUDA(cudaStreamSynchronize(s));
-    h3[0] = c->pin[0]; h3[1] = c->pin[1]; h3[2] = c->pin[2];
-  }
-  const uint64_t n_S = h3[0], n_L = h3[1], n_mat = h3[2];
-  *h_n_pairs = n_S + n_L;
-  if (*h_n_pairs > capacity) return UTS_ERR_CAPACITY;
-  if (sort_scratch_bytes < uts_sort_scratch_bytes(n_S)) return UTS_ERR_INVALID_ARG;
-  if (n_L == 0) {                                     // no large discs: the plain sequence
-    if (n_S) {
-      if ((st = q.emit(offsets, keys, vals))) return st;
-      if ((st = uts_sort(cfg, n_S, keys, vals, keys_tmp, vals_tmp, 1, sort_scratch, sort_scratch_bytes, stream))) return st;
-    }
-    return uts_tile_ranges(cfg, n_S, keys, ranges, stream);
-  }
-  // ---- large discs: transpose the bit matrix, count per (view, tile) — on the context's side stream, beside the small pairs' emit +
-  // sort + ranges below (HBM-bound against latency-bound: they overlap); joined back before the totals.  The guard joins on every
-  // exit path, so no work is ever left unjoined.
+  // The matrix class runs on the context's side stream from its count on (q.count forks it): bitmap rows, transpose, per-tile counts
+  // beside the small discs' count, emit, radix sort and ranges; joined back before the totals.  The guard joins on every exit path,
+  // so no work is ever left unjoined; the context stays locked for the call (side stream, its events and the pinned words).
   DeviceCtx* ctx = q.ctx;
   std::lock_guard<std::recursive_mutex> side_lock(ctx->mu);
   struct SideJoin {
@@ -1322,10 +1308,38 @@ int uts_tile_lists(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
     int join() { if (!forked) return UTS_OK; forked = false; UTS_CUDA(cudaEventRecord(c->side_join, c->side)); UTS_CUDA(cudaStreamWaitEvent(s, c->side_join, 0)); return UTS_OK; }
     ~SideJoin() { join(); }
   } side{ctx, s};
+  st = q.count(offsets, mat_ok ? &mp : nullptr, flag_by_rank, reinterpret_cast<uint64_t*>(sp + ML.rank_scan), scan_sums);
+  side.forked = q.side_forked;
+  if (st) return st;
+  if (side.forked) {                                  // the matrix pairs' total, read by the host while the small pairs are sorted
+    UTS_CUDA(cudaMemcpyAsync(ctx->pin + 4, mp.n_L, 8, cudaMemcpyDeviceToHost, ctx->side));
+    UTS_CUDA(cudaEventRecord(ctx->side_mid, ctx->side));
+  }
+  // host needs now: small pairs and matrix rows — gathered on the device, one copy into the context's pinned words
+  uint64_t n_S = 0, n_mat = 0;
   {
-    UTS_CUDA(cudaEventRecord(ctx->side_fork, s));
-    UTS_CUDA(cudaStreamWaitEvent(ctx->side, ctx->side_fork, 0));
-    side.forked = true;
+    unsigned long long* g3 = reinterpret_cast<unsigned long long*>(sp + ML.misc) + 8;
+    gather3_kernel<<<1, 1, 0, s>>>(offsets + n, nullptr, mat_ok ? mp.row_of_rank + n : nullptr, g3);
+    UTS_LAUNCH_CHECK();
+    UTS_CUDA(cudaMemcpyAsync(ctx->pin, g3, 24, cudaMemcpyDeviceToHost, s));
+    UTS_CUDA(cudaStreamSynchronize(s));
+    n_S = ctx->pin[0]; n_mat = ctx->pin[2];
+  }
+  *h_n_pairs = n_S;
+  if (n_S > capacity) {                               // report the whole need: wait for the matrix pairs' total as well
+    if (side.forked) { UTS_CUDA(cudaEventSynchronize(ctx->side_mid)); *h_n_pairs = n_S + ctx->pin[4]; }
+    return UTS_ERR_CAPACITY;
+  }
+  if (sort_scratch_bytes < uts_sort_scratch_bytes(n_S)) return UTS_ERR_INVALID_ARG;
+  if (!side.forked || n_mat == 0) {                   // no large discs: the plain sequence
+    if ((st = side.join())) return st;
+    if (n_S) {
+      if ((st = q.emit(offsets, keys, vals))) return st;
+      if ((st = uts_sort(cfg, n_S, keys, vals, keys_tmp, vals_tmp, 1, sort_scratch, sort_scratch_bytes, stream))) return st;
+    }
+    return uts_tile_ranges(cfg, n_S, keys, ranges, stream);
+  }
+  {
     dim3 grid((unsigned)((mp.n_words + 31) / 32), (unsigned)(n_mat / 256 + (uint64_t)d.V + 1));
     matrix_transpose_kernel<<<grid, 256, 0, ctx->side>>>(mp, d.V, d.n_tile);
     UTS_LAUNCH_CHECK();
@@ -1339,6 +1353,10 @@ int uts_tile_lists(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
     if ((st = uts_sort(cfg, n_S, keys_tmp, vals_tmp, keys, vals, 1, sort_scratch, sort_scratch_bytes, stream))) return st;
   }
   if ((st = uts_tile_ranges(cfg, n_S, keys_tmp, s_ranges, stream))) return st;
+  UTS_CUDA(cudaEventSynchronize(ctx->side_mid));     // the bitmap rows are done (the stream s is still busy with the sort)
+  const uint64_t n_L = ctx->pin[4];
+  *h_n_pairs = n_S + n_L;
+  if (*h_n_pairs > capacity) return UTS_ERR_CAPACITY;
   if ((st = side.join())) return st;
   // ---- final ranges, then one warp per (view, tile) merges its large discs (bit vector) with its small pairs into keys / vals
   uint32_t* total = reinterpret_cast<uint32_t*>(sp + ML.total);

@@ -26,9 +26,10 @@
  *   - Library state: the last CUDA error code, the launch counter, and ONE CONTEXT PER DEVICE, created on the first call made with
  *     that device current and kept until the process ends: the SM count, cached occupancy numbers, three auxiliary streams with their
  *     fork / join events (uts_tile_query / uts_tile_lists run independent kernels side by side on them and join back into
- *     `stream` before returning) and one copy stream with four events (uts_host_forward_backward).  A per-device mutex is held
- *     while a call enqueues on those streams, so calls may be issued from several threads and on several streams; they never
- *     read the environment.  No CPU fallback; sm_100 only.
+ *     `stream` before returning), one copy stream with four events (uts_host_forward_backward) and 64 bytes of pinned host
+ *     memory (the pair counts of uts_tile_lists come back in one copy).  A per-device mutex is held while a call enqueues on
+ *     those streams (uts_tile_lists: from its count pass to its last launch, its host read of the pair count included), so calls
+ *     may be issued from several threads and on several streams; they never read the environment.  No CPU fallback; sm_100 only.
  *   - Inputs are ACTIVATED values: scales > 0, opacity in (0,1), quaternion (w,x,y,z) used as given
  *     (reading A14).  Arrays are dense row-major float32 unless stated.
  *   - Index conventions: NESTED pixel p = f*4^k + interleave(x,y); tile of p = p >> (2*tile_log2); pixel slot

@@ -185,9 +185,10 @@ __host__ __device__ __forceinline__ unsigned long long tile_row_mask(const RingD
   const int Hm = min(S, 2 * Nt - 2 - S);
   const int jtop = min(Hm, jbase + 63);
   unsigned long long mask = 0;
-  for (int d = 0; d <= 2 * m - 2; ++d) {
+  // rings of this tile row inside the disc's ring range only: i = top - (m S + d) in [i_lo, i_hi]
+  const int d_lo = max(0, top - m * S - D.i_hi), d_hi = min(2 * m - 2, top - m * S - D.i_lo);
+  for (int d = d_lo; d <= d_hi; ++d) {
     const int i = top - (m * S + d);
-    if (i < D.i_lo || i > D.i_hi) continue;
     int first, last;
     tab(i, first, last);
     if (last < first) continue;

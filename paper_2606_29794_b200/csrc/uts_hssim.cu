@@ -201,20 +201,36 @@ hssim_kernel(int k, int64_t n_pix_full, const uint32_t* __restrict__ active_tile
   }
   // One patch cell under the windows of pixels J0..J1 (compile-time range): wp points at the weight of pixel j = 0 for this cell,
   // pixel j's weight sits j window rows before it.
+  // The 121-tap walk keeps (S1, S2) and (S11, S22) as packed fp32 pairs: per tap, pixel and channel (a, b) = w (dx, dg) is one
+  // FMUL2, the two sums one FADD2, the two squares one FFMA2 and the cross term one FFMA — four issue slots instead of seven, the
+  // same roundings as the scalar form.
+  f2_t P12[kHJ][3], P1122[kHJ][3], nref[3];
+#pragma unroll
+  for (int ch = 0; ch < 3; ++ch) nref[ch] = f2_pack(-xr[ch], -gr[ch]);
+#pragma unroll
+  for (int j = 0; j < kHJ; ++j)
+#pragma unroll
+    for (int ch = 0; ch < 3; ++ch) P12[j][ch] = P1122[j][ch] = 0;
   auto fwd_cell = [&](int c, const float* wp, auto j0, auto j1) {
     const float val = s_val[c];
-    float dx[3], dg[3];
+    f2_t d2[3];                                               // (dx, dg) per channel
+    float dg[3];
 #pragma unroll
-    for (int ch = 0; ch < 3; ++ch) { const float2 v = s_xg[ch][c]; dx[ch] = v.x - xr[ch]; dg[ch] = v.y - gr[ch]; }
+    for (int ch = 0; ch < 3; ++ch) {
+      d2[ch] = f2_add(*reinterpret_cast<const f2_t*>(&s_xg[ch][c]), nref[ch]);
+      float lo; f2_unpack(d2[ch], lo, dg[ch]);
+    }
 #pragma unroll
     for (int j = decltype(j0)::value; j <= decltype(j1)::value; ++j) {
       const float wv = wp[-j * kHW] * val;
       wsum[j] += wv;
 #pragma unroll
       for (int ch = 0; ch < 3; ++ch) {
-        const float a = wv * dx[ch], b = wv * dg[ch];
-        S1[j][ch] += a; S2[j][ch] += b;
-        S11[j][ch] = fmaf(a, dx[ch], S11[j][ch]); S22[j][ch] = fmaf(b, dg[ch], S22[j][ch]); S12[j][ch] = fmaf(a, dg[ch], S12[j][ch]);
+        const f2_t ab = f2_mul(f2_bc(wv), d2[ch]);
+        float a, b; f2_unpack(ab, a, b);
+        P12[j][ch] = f2_add(P12[j][ch], ab);
+        P1122[j][ch] = f2_fma(ab, d2[ch], P1122[j][ch]);
+        S12[j][ch] = fmaf(a, dg[ch], S12[j][ch]);
       }
     }
   };
@@ -282,6 +298,12 @@ hssim_kernel(int k, int64_t n_pix_full, const uint32_t* __restrict__ active_tile
     fwd_cell(c + 11 * kHS, wp + 11 * kHW, I1(), I3());
     fwd_cell(c + 12 * kHS, wp + 12 * kHW, I2(), I3());
     fwd_cell(c + 13 * kHS, wp + 13 * kHW, I3(), I3());
+  }
+  if (!sep) {
+#pragma unroll
+    for (int j = 0; j < kHJ; ++j)
+#pragma unroll
+      for (int ch = 0; ch < 3; ++ch) { f2_unpack(P12[j][ch], S1[j][ch], S2[j][ch]); f2_unpack(P1122[j][ch], S11[j][ch], S22[j][ch]); }
   }
 
   // SSIM index and, for the gradient, its derivatives folded into three coefficients per pixel and channel:
@@ -392,19 +414,42 @@ hssim_kernel(int k, int64_t n_pix_full, const uint32_t* __restrict__ active_tile
     // touch 32 different cells (the other half warp works 4 rows further down), so plain read-add-write is safe between the
     // __syncwarp()s (after rows 2, 6, 10, 13); sums over the thread's own four pixels are taken in registers first.
     float* gw = s_grad + (tid >> 5) * (3 * kGR * kHS) + (((tid >> 4) & 1) * kHJ) * kHS + lx;
+    // the coefficients of pixel pairs (0, 1) and (2, 3) as packed fp32 pairs: a cell under both windows of a pair takes three FFMA2
+    // per channel for the two pixels (the pair's halves are added once per cell)
+    f2_t c0p[2][3], k1p[2][3], k2p[2][3];
+#pragma unroll
+    for (int q = 0; q < 2; ++q)
+#pragma unroll
+      for (int ch = 0; ch < 3; ++ch) {
+        c0p[q][ch] = f2_pack(c0[2 * q][ch], c0[2 * q + 1][ch]); k1p[q][ch] = f2_pack(k1[2 * q][ch], k1[2 * q + 1][ch]);
+        k2p[q][ch] = f2_pack(k2[2 * q][ch], k2[2 * q + 1][ch]);
+      }
     auto bwd_cell = [&](int c, const float* wp, float* gp, auto j0, auto j1) {
+      constexpr int J0 = decltype(j0)::value, J1 = decltype(j1)::value;
       const float val = s_val[c];
       float dx[3], dg[3], ac[3] = {0.f, 0.f, 0.f};
+      f2_t ac2[3] = {0, 0, 0};
 #pragma unroll
       for (int ch = 0; ch < 3; ++ch) { const float2 v = s_xg[ch][c]; dx[ch] = v.x - xr[ch]; dg[ch] = v.y - gr[ch]; }
 #pragma unroll
-      for (int j = decltype(j0)::value; j <= decltype(j1)::value; ++j) {
-        const float wv = wp[-j * kHW] * val;
+      for (int q = 0; q < 2; ++q) {
+        if (J0 <= 2 * q && 2 * q + 1 <= J1) {                   // both pixels of the pair see this cell
+          const f2_t wv2 = f2_pack(wp[-(2 * q) * kHW] * val, wp[-(2 * q + 1) * kHW] * val);
 #pragma unroll
-        for (int ch = 0; ch < 3; ++ch) ac[ch] = fmaf(wv, fmaf(k1[j][ch], dx[ch], fmaf(k2[j][ch], dg[ch], c0[j][ch])), ac[ch]);
+          for (int ch = 0; ch < 3; ++ch)
+            ac2[ch] = f2_fma(wv2, f2_fma(k1p[q][ch], f2_bc(dx[ch]), f2_fma(k2p[q][ch], f2_bc(dg[ch]), c0p[q][ch])), ac2[ch]);
+        } else {
+#pragma unroll
+          for (int j = 2 * q; j <= 2 * q + 1; ++j) {
+            if (j < J0 || j > J1) continue;
+            const float wv = wp[-j * kHW] * val;
+#pragma unroll
+            for (int ch = 0; ch < 3; ++ch) ac[ch] = fmaf(wv, fmaf(k1[j][ch], dx[ch], fmaf(k2[j][ch], dg[ch], c0[j][ch])), ac[ch]);
+          }
+        }
       }
 #pragma unroll
-      for (int ch = 0; ch < 3; ++ch) gp[ch * (kGR * kHS)] += ac[ch];
+      for (int ch = 0; ch < 3; ++ch) { float lo, hi; f2_unpack(ac2[ch], lo, hi); gp[ch * (kGR * kHS)] += ac[ch] + (lo + hi); }
     };
 #pragma unroll 1
     for (int tx = 0; tx < kHW; ++tx) {

@@ -174,4 +174,14 @@ __device__ __forceinline__ void pix_center_cam_f32(int o, uint32_t p, float& vx,
   vx = sth * s; vy = z; vz = sth * cs;
 }
 
+// Packed fp32 pairs (sm_100: fma / mul / add .f32x2 — one instruction, two IEEE roundings, the same results as the scalar forms).
+// A pair is a 64-bit register; f2_bc(s) = (s, s) costs nothing (ptxas folds it into a scalar operand of FFMA2 / FMUL2 / FADD2).
+typedef unsigned long long f2_t;
+__device__ __forceinline__ f2_t f2_pack(float lo, float hi) { f2_t d; asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi)); return d; }
+__device__ __forceinline__ f2_t f2_bc(float s) { return f2_pack(s, s); }
+__device__ __forceinline__ void f2_unpack(f2_t v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f2_t f2_fma(f2_t a, f2_t b, f2_t c) { f2_t d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ f2_t f2_mul(f2_t a, f2_t b) { f2_t d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f2_t f2_add(f2_t a, f2_t b) { f2_t d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+
 }  // namespace uts

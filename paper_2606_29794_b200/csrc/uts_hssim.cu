@@ -134,7 +134,7 @@ hssim_kernel(int k, int64_t n_pix_full, const uint32_t* __restrict__ active_tile
   __shared__ float s_val[kHCellsS];          // 1 valid, 0 missing
   __shared__ int s_idx[kHCellsS];            // storage index (pixels, < 2^31) or -1
   __shared__ float s_w[kHTaps];
-  __shared__ float s_grad[2 * 3 * kGR * kHS];                // [warp][channel][row][col]: no two warps share a cell; scratch of the separable path
+  __shared__ __align__(16) float s_grad[2 * 3 * kGR * kHS];                // [warp][channel][row][col]: no two warps share a cell; scratch of the separable path
   __shared__ float s_red[2][2];
 
   const int tid = threadIdx.x;
@@ -238,7 +238,7 @@ hssim_kernel(int k, int64_t n_pix_full, const uint32_t* __restrict__ active_tile
   // loop, so that the body stays inside the instruction cache (fully unrolled, 14 rows x 4 pixels, it stalled on fetch).
   using I0 = Int<0>; using I1 = Int<1>; using I2 = Int<2>; using I3 = Int<3>;
   if (sep) {
-    // g(d) = the window's middle row; pass 1 along x into s_grad as H[row][col][5] (26 x 16 x 5 floats), pass 2 along y in registers
+    // g(d) = the window's middle row; pass 1 along x into s_grad as H[row][col][6] (26 x 16 records of 5 floats + 1 of padding), pass 2 along y in registers
     const float* g1 = s_w + kHR * kHW;
     float gsum = 0.f;
 #pragma unroll
@@ -252,33 +252,37 @@ hssim_kernel(int k, int64_t n_pix_full, const uint32_t* __restrict__ active_tile
       for (int it = tid; it < kHP * 4; it += kHT) {             // item = (patch row, group of 4 tile columns): 14 cells serve 4 outputs
         const int row = it >> 2, cg = (it & 3) * 4;
         const float2* src = &s_xg[ch][row * kHS + cg];
-        float dxv[14], dgv[14];
+        f2_t dv[14];                                            // (dx, dg) of the 14 cells, packed
+        float dgv[14];
 #pragma unroll
-        for (int i = 0; i < 14; ++i) { const float2 v = src[i]; dxv[i] = v.x - xr[ch]; dgv[i] = v.y - gr[ch]; }
+        for (int i = 0; i < 14; ++i) { dv[i] = f2_add(*reinterpret_cast<const f2_t*>(src + i), nref[ch]); float lo; f2_unpack(dv[i], lo, dgv[i]); }
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-          float h1 = 0.f, h2 = 0.f, h11 = 0.f, h22 = 0.f, h12 = 0.f;
+          f2_t h12p = 0, h1122 = 0;
+          float h12 = 0.f;
 #pragma unroll
           for (int t = 0; t < kHW; ++t) {
-            const float a = g1[t] * dxv[q + t], b = g1[t] * dgv[q + t];
-            h1 += a; h2 += b; h11 = fmaf(a, dxv[q + t], h11); h22 = fmaf(b, dgv[q + t], h22); h12 = fmaf(a, dgv[q + t], h12);
+            const f2_t ab = f2_mul(f2_bc(g1[t]), dv[q + t]);
+            float a, b; f2_unpack(ab, a, b);
+            h12p = f2_add(h12p, ab); h1122 = f2_fma(ab, dv[q + t], h1122); h12 = fmaf(a, dgv[q + t], h12);
           }
-          float* dst = H + (row * 16 + cg + q) * 5;
-          dst[0] = h1; dst[1] = h2; dst[2] = h11; dst[3] = h22; dst[4] = h12;
+          float* dst = H + (row * 16 + cg + q) * 6;             // records of 6 floats: the two pairs stay 8-byte aligned
+          *reinterpret_cast<f2_t*>(dst) = h12p; *reinterpret_cast<f2_t*>(dst + 2) = h1122; dst[4] = h12;
         }
       }
       __syncthreads();
 #pragma unroll
       for (int rho = 0; rho < kHRows; ++rho) {                  // patch rows r0 .. r0 + 13 of column lx
-        const float* hv = H + ((r0 + rho) * 16 + lx) * 5;
-        const float v0 = hv[0], v1 = hv[1], v2 = hv[2], v3 = hv[3], v4 = hv[4];
+        const float* hv = H + ((r0 + rho) * 16 + lx) * 6;
+        const f2_t v01 = *reinterpret_cast<const f2_t*>(hv), v23 = *reinterpret_cast<const f2_t*>(hv + 2);
+        const float v4 = hv[4];
 #pragma unroll
         for (int j = 0; j < kHJ; ++j) {
           const int t = rho - j;                                // window row of pixel j
           if (t >= 0 && t < kHW) {
             const float wv = g1[t];
-            S1[j][ch] = fmaf(wv, v0, S1[j][ch]); S2[j][ch] = fmaf(wv, v1, S2[j][ch]); S11[j][ch] = fmaf(wv, v2, S11[j][ch]);
-            S22[j][ch] = fmaf(wv, v3, S22[j][ch]); S12[j][ch] = fmaf(wv, v4, S12[j][ch]);
+            P12[j][ch] = f2_fma(f2_bc(wv), v01, P12[j][ch]); P1122[j][ch] = f2_fma(f2_bc(wv), v23, P1122[j][ch]);
+            S12[j][ch] = fmaf(wv, v4, S12[j][ch]);
           }
         }
       }
@@ -299,7 +303,7 @@ hssim_kernel(int k, int64_t n_pix_full, const uint32_t* __restrict__ active_tile
     fwd_cell(c + 12 * kHS, wp + 12 * kHW, I2(), I3());
     fwd_cell(c + 13 * kHS, wp + 13 * kHW, I3(), I3());
   }
-  if (!sep) {
+  {
 #pragma unroll
     for (int j = 0; j < kHJ; ++j)
 #pragma unroll

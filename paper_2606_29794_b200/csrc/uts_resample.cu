@@ -81,7 +81,15 @@ __device__ __forceinline__ void ring_z(int N, int i, double& z, double& sth) {
   else { z = (double)(2 * (2 * N - i)) / (double)(3 * N); sth = sqrt((1.0 - z) * (1.0 + z)); }
 }
 
-// NESTED index of the pixel at position g of ring i (g already reduced to [0, 8 n_r) with the ring's parity)
+// NESTED index of the pixel at position g of ring i (g already reduced to [0, 8 n_r) with the ring's parity).  A ring crosses at
+// most two face rows; on a face of row r the pixel's x - y = g - F2 n_r lies within (-n_r, n_r), which fixes the face column.
+__device__ __forceinline__ uint32_t spread_bits16(uint32_t v) {   // 16 bits -> even bit positions
+  v = (v | (v << 8)) & 0x00ff00ffu;
+  v = (v | (v << 4)) & 0x0f0f0f0fu;
+  v = (v | (v << 2)) & 0x33333333u;
+  v = (v | (v << 1)) & 0x55555555u;
+  return v;
+}
 __device__ __forceinline__ uint64_t ring_pos_to_nest(int order, int i, int g) {
   const int N = 1 << order;
   const int n = min(i, min(N, 4 * N - i));
@@ -89,18 +97,15 @@ __device__ __forceinline__ uint64_t ring_pos_to_nest(int order, int i, int g) {
     const int s = (r + 2) * N - 1 - i;                          // x + y on a face of row r
     if (s < 0 || s > 2 * N - 2) continue;
     const int hm = min(s, 2 * N - 2 - s);
-    for (int c = 0; c < 4; ++c) {
-      const int F2 = 2 * c + 1 - (r & 1);
-      int h = g - F2 * n;                                       // x - y, modulo the ring length 8 n
-      if (h > 4 * n) h -= 8 * n;
-      if (h <= -4 * n) h += 8 * n;
-      if (h < -hm || h > hm || ((s + h) & 1)) continue;
-      const uint64_t x = (uint64_t)((s + h) >> 1), y = (uint64_t)((s - h) >> 1);
-      const uint64_t f = (uint64_t)(4 * r + c);
-      uint64_t m = 0;
-      for (int b = 0; b < order; ++b) m |= (((x >> b) & 1ull) << (2 * b)) | (((y >> b) & 1ull) << (2 * b + 1));
-      return (f << (2 * order)) | m;
-    }
+    const int t = r & 1;
+    const int c = ((g + t * n) / (2 * n)) & 3;                  // the column whose centre F2 n is within n of g
+    int h = g - (2 * c + 1 - t) * n;                            // x - y, modulo the ring length 8 n
+    if (h > 4 * n) h -= 8 * n;
+    if (h <= -4 * n) h += 8 * n;
+    if (h < -hm || h > hm || ((s + h) & 1)) continue;
+    const uint32_t x = (uint32_t)((s + h) >> 1), y = (uint32_t)((s - h) >> 1);
+    const uint64_t f = (uint64_t)(4 * r + c);
+    return (f << (2 * order)) | (uint64_t)(spread_bits16(x) | (spread_bits16(y) << 1));
   }
   return 0;                                                     // unreachable: every (ring, position) is a pixel
 }
@@ -136,8 +141,12 @@ __device__ __forceinline__ int interp_support(int order, double dx, double dy, d
   else i1 = (int)floor((double)N * (2.0 - 1.5 * z));
   i1 = max(0, min(last, i1));
   auto theta_of = [&](int i) { double zz, ss; ring_z(N, i, zz, ss); return atan2(ss, zz); };
-  while (i1 < last && theta_of(i1 + 1) <= theta) ++i1;
-  while (i1 >= 1 && theta_of(i1) > theta) --i1;
+  // settled on the rings' z (colatitude <= theta  <=>  z_ring >= cos theta): no inverse trigonometry in the search; at a tie either
+  // ring gives the same interpolated value (the weight of the other ring is then 0)
+  auto z_of = [&](int i) { double zz, ss; ring_z(N, i, zz, ss); return zz; };
+  const double zn = z / sqrt(z * z + sth * sth);
+  while (i1 < last && z_of(i1 + 1) >= zn) ++i1;
+  while (i1 >= 1 && z_of(i1) < zn) --i1;
   int cnt = 0;
   uint64_t p2[2]; double a2[2];
   if (i1 == 0) {

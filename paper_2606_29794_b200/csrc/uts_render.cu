@@ -287,7 +287,8 @@ render_fwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
 #pragma unroll
   for (int j = 0; j < PX; ++j) { T[j] = 1.f; Cr[j] = Cg[j] = Cb[j] = Cd[j] = 0.f; n_last[j] = 0; if (ts.on[j]) open |= 1u << j; }
   const uint64_t len = ts.end - ts.start;
-  const uint32_t sS = (uint32_t)__cvta_generic_to_shared(&S);
+  uint32_t sS = (uint32_t)__cvta_generic_to_shared(&S);
+  asm volatile("" : "+r"(sS));                       // keep the window address in a register (otherwise it is rebuilt from CgaCtaId at every entry)
   uint32_t* mark_w = nullptr;                         // plane PX wid of this tile's run; patch j is j planes further
   if (MARK) mark_w = marks + (uint64_t)(PX * wid) * plane_words + mark_base<PX>(rp, ts);
   // Patch cull (PX = 1: a warp is one 8x4 patch).  At the start of a group of 32 entries lane l asks whether entry l can reach the
@@ -553,7 +554,7 @@ render_bwd_kernel(RenderParams rp, const float* __restrict__ dir, const float* _
   if (DEPTH && lane == 2) { lane_dst = dL_dinvr + gbase; lane_stride = 1u; }   // lane 2 the 1/rho sum
   const bool lane_owns = (lane & 3) == 0 || lane == 1 || (DEPTH && lane == 2);
   asm volatile("" : "+l"(lane_dst));                   // keep the per-view base folded into the pointer (one IMAD.WIDE per atomic)
-  const uint32_t sS = (uint32_t)__cvta_generic_to_shared(&S);
+  const uint32_t sS = (uint32_t)__cvta_generic_to_shared(&S);   // (pinning it in a register as in the forward costs two registers: 3.54 -> 3.58 ms)
 
   const int n_batch = (int)((max_nl + kBatch - 1) / kBatch);
   // lane 8 j + g (j < PX) reads word g of patch j's plane, kWarps j + wid

@@ -329,6 +329,8 @@ def per_kernel_table(m, peaks, fp32_peak):
         else:
             byts = stage_bytes(s_, P, V, M, cfg.n_tiles, m["n_pairs"])
             out[s_] = dict(ms=ms, bound="hbm", gbs=byts / sec / 1e9, frac_hbm_peak=byts / sec / 1e9 / peaks["hbm_gbs"])
+            if s_ == "tile_lists":        # secondary: SURVEY 8(d)'s separate floors of F2 + F3 + F4 (12 + 24 + 8 B per pair) instead of write-once
+                out[s_]["frac_hbm_peak_survey8d_units"] = 44.0 * m["n_pairs"] / sec / 1e9 / peaks["hbm_gbs"]
     return out
 
 

@@ -573,7 +573,7 @@ def run_ours(args):
                 ms_forward=m["ms_fwd"], ms_forward_backward=ms_step, stage_ms=m["stage_ms"], per_kernel=pk,
                 evaluated_pairs=dict(forward=m["ev_f"], forward_after_patch_cull=m["ev_cull"], forward_q_above_cut=m["ev_full"], contributing=m["contrib"], backward_alg1=m["ev_b"], backward_executed=m["ev_b_visited"],
                                      listed=int(m["n_pairs"]) * cfg.ppt,
-                                     note="forward (Alg.1's loop) / after the patch cull (what the forward executes) / of those, patches where q alone cannot rule the entry out (informational) / contributing: counted on the device by uts_render_fwd_counted; backward_alg1: sum of n_last; "
+                                     note="forward (Alg.1's loop) / after the per-patch cull (a lower bound of what the forward executes: a warp owns two patches and walks an entry for both when it reaches either) / of those, patches where q alone cannot rule the entry out (informational) / contributing: counted on the device by uts_render_fwd_counted; backward_alg1: sum of n_last; "
                                           "backward_executed: 32 x marked (patch, entry) pairs; listed: pairs x 256 pixels"),
                 roofline=roof, clocks=m["clocks"], extras=extras,
                 e2e=dict(value=replicas.aggregate_throughput(n_pix_active, e2e_ms_max, world), unit=UNIT, ms_per_step=e2e_ms_max, steps=e2e_steps,

@@ -131,7 +131,7 @@ __device__ __forceinline__ void ring_pair(int order, int i, double lam, uint64_t
 __device__ __forceinline__ int interp_support(int order, double dx, double dy, double dz, uint64_t pix[8], double w[8]) {
   const int N = 1 << order, last = 4 * N - 1;
   const double z = dy, sth = sqrt(dx * dx + dz * dz);
-  const double theta = atan2(sth, z);
+  double theta = 0.0;                                 // colatitude: only the two polar caps below need the angle itself
   double lam = atan2(dx, dz);
   if (lam < 0.0) lam += 2.0 * kPi;
   // largest ring whose colatitude is <= theta (0: north of ring 1): closed-form estimate, then settled on ring colatitudes
@@ -150,6 +150,7 @@ __device__ __forceinline__ int interp_support(int order, double dx, double dy, d
   int cnt = 0;
   uint64_t p2[2]; double a2[2];
   if (i1 == 0) {
+    theta = atan2(sth, z);
     const double wt = theta / theta_of(1);
     ring_pair(order, 1, lam, p2, a2);
     pix[0] = p2[0]; w[0] = a2[0] * wt; pix[1] = p2[1]; w[1] = a2[1] * wt; cnt = 2;
@@ -157,13 +158,31 @@ __device__ __forceinline__ int interp_support(int order, double dx, double dy, d
     return cnt;
   }
   if (i1 == last) {
+    theta = atan2(sth, z);
     const double t1 = theta_of(last), wt = (theta - t1) / (kPi - t1);
     ring_pair(order, last, lam, p2, a2);
     pix[0] = p2[0]; w[0] = a2[0] * (1.0 - wt); pix[1] = p2[1]; w[1] = a2[1] * (1.0 - wt); cnt = 2;
     for (int j = 0; j < 4; ++j) { pix[cnt] = ring_pos_to_nest(order, last, 2 * j + 1); w[cnt++] = 0.25 * wt; }
     return cnt;
   }
-  const double t1 = theta_of(i1), t2 = theta_of(i1 + 1), wt = (theta - t1) / (t2 - t1);
+  // wt = (theta - t1) / (t2 - t1) from the sines of the two differences (no colatitude is formed): with (z, s) = (cos, sin),
+  // sin(theta - t1) = s z1 - z s1 and sin(t2 - t1) = s2 z1 - z2 s1; the rings are at most a few hundredths of a radian apart, where
+  // asin x = x + x^3/6 + 3 x^5/40 + 15 x^7/336 is exact to 1e-10 relative; wider gaps (orders below 4) take atan2.
+  double wt;
+  {
+    double z1, s1, z2, s2;
+    ring_z(N, i1, z1, s1); ring_z(N, i1 + 1, z2, s2);
+    const double inv_n = 1.0 / sqrt(z * z + sth * sth), zc = z * inv_n, sc = sth * inv_n;
+    const double d1 = sc * z1 - zc * s1, d21 = s2 * z1 - z2 * s1;
+    if (d21 < 0.15) {
+      auto asin_small = [](double x) { const double x2 = x * x; return x * (1.0 + x2 * (1.0 / 6.0 + x2 * (3.0 / 40.0 + x2 * (15.0 / 336.0 + x2 * (105.0 / 3456.0))))); };
+      wt = asin_small(d1) / asin_small(d21);
+    } else {
+      theta = atan2(sth, z);
+      const double t1 = atan2(s1, z1), t2 = atan2(s2, z2);
+      wt = (theta - t1) / (t2 - t1);
+    }
+  }
   ring_pair(order, i1, lam, p2, a2);
   pix[0] = p2[0]; w[0] = a2[0] * (1.0 - wt); pix[1] = p2[1]; w[1] = a2[1] * (1.0 - wt);
   ring_pair(order, i1 + 1, lam, p2, a2);

@@ -2,11 +2,11 @@
 // (Alg.1 l.17-30 PAPER.md:563-587; Eq.6; SphericalOffset PAPER.md:112; mask PAPER.md:62, 129), and
 // B1: its backward.
 //
-// One thread block of 256 / PX threads per active tile; every thread owns PX pixels (p & 255 = tid + (256 / PX) j, j < PX), so
-// that one staged list entry read from shared memory serves PX pixel evaluations and, in the backward, one warp reduction + one
-// set of atomics serves up to 32 PX pixels.  The 32 pixels (lane, j) of a warp form a compact 8x4 "patch" (thread id = NESTED low
-// bits); patches are what the early exit, the marks and the backward's visit list are kept for.  The tile's sorted list is
-// staged through shared memory in batches of 256 entries.
+// One thread block of 256 / PX threads per active tile; every thread owns PX pixels (p & 255 = 32 (PX warp + j) + lane, j < PX: a
+// warp owns PX consecutive 8x4 "patches" of 32 pixels in NESTED order), so that one staged list entry read from shared memory
+// serves PX pixel evaluations — two at a time in packed fp32 pairs (FFMA2 / FMUL2 / FADD2, sm_100) — and, in the backward, one warp
+// reduction + one set of atomics serves up to 32 PX pixels.  Patches are what the early exit, the patch cull, the marks and the
+// backward's visit list are kept for.  The tile's sorted list is staged through shared memory in batches of 256 entries.
 //
 // SphericalOffset without inverse trigonometry and without fp32 cancellation:  with Gaussian direction u
 // and its east/north unit vectors e, n, and pixel direction w,

@@ -80,6 +80,12 @@ __global__ void mat_view_tab_kernel(MatParams mp, int P, int V, int64_t n_tile) 
 #define UTS_MAT_MINB 16
 #endif
 constexpr int kMatThreads = UTS_MAT_THREADS;
+// Blocks per SM the kernel is given when it runs on the side stream beside the small pairs' emit and sort (uts_tile_lists): a persistent
+// grid that leaves half of the register file to them.  Measured on config 4 (tile lists): 6 -> 7.16 ms, 8 -> 7.00, 10 -> 7.09, 16 -> 7.16.
+#ifndef UTS_MAT_SIDE_BLOCKS
+#define UTS_MAT_SIDE_BLOCKS 8
+#endif
+constexpr int kMatSideBlocks = UTS_MAT_SIDE_BLOCKS;
 __global__ void __launch_bounds__(kMatThreads, UTS_MAT_MINB)
 matrix_count_kernel(QueryParams qp, MatParams mp, const float* __restrict__ dir, const float* __restrict__ lonlat, const float* __restrict__ rho,
                     const float* __restrict__ rs, const int32_t* __restrict__ slot_of_tile, const uint32_t* __restrict__ active_words,

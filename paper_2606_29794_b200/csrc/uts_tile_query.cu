@@ -1161,10 +1161,7 @@ struct QueryRun {
         side_forked = true;
         const size_t smem_m = smem_block + (size_t)mp->n_words * 4;
         const int occ = cached_occupancy(ctx, kOccMat, matrix_count_kernel, kMatThreads, smem_m);
-#ifndef UTS_MAT_SIDE_BLOCKS
-#define UTS_MAT_SIDE_BLOCKS 8
-#endif
-        matrix_count_kernel<<<(unsigned)ctx->sms * (unsigned)(occ < UTS_MAT_SIDE_BLOCKS ? occ : UTS_MAT_SIDE_BLOCKS), kMatThreads, smem_m, ctx->side>>>(
+        matrix_count_kernel<<<(unsigned)ctx->sms * (unsigned)(occ < kMatSideBlocks ? occ : kMatSideBlocks), kMatThreads, smem_m, ctx->side>>>(
             qp, *mp, in.dir, in.lonlat, in.rho, in.rs, mask.slot_of_tile, mask.slot_of_tile ? active : nullptr, perm, n_small, emit_rank);
         UTS_LAUNCH_CHECK();
       }

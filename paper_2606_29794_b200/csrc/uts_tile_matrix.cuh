@@ -6,7 +6,7 @@
 // tile.  So the large discs (radius class chosen so that a bitmap row is cheaper than the disc's pairs through the radix sort) are
 // taken out of the pair stream:
 //   count     each large disc's tile set is written as a bitmap row of a (disc x tile) bit matrix, rows in (view, depth, id) order
-//   transpose 32 x 32 bit blocks -> one bit VECTOR over the large discs per (view, tile)
+//   transpose 32 x 32 bit blocks -> one bit VECTOR over the large discs per (view, tile), and the vectors' population counts
 //   emit      a warp per (view, tile) walks its bit vector: set bit r = disc r belongs to this tile's list.  The list comes out
 //             already grouped by tile and ordered by depth — no sort — with coalesced writes.
 // Only the small discs' pairs go through emit + radix sort; a per-tile merge of the two depth-ordered lists gives the final
@@ -202,23 +202,9 @@ matrix_transpose_kernel(MatParams mp, int V, int64_t n_tile) {
     hi.x = sT[4][cc * 33 + b]; hi.y = sT[5][cc * 33 + b]; hi.z = sT[6][cc * 33 + b]; hi.w = sT[7][cc * 33 + b];
     uint4* dst = reinterpret_cast<uint4*>(out + (size_t)tile * mv.W + (size_t)rb * 8);
     dst[0] = lo; dst[1] = hi;
-  }
-}
-
-// large_count[(v, tile)] = popcount of the tile's bit vector; one warp per (view, tile)
-__global__ void __launch_bounds__(256)
-matrix_popcount_kernel(MatParams mp, int V, int64_t n_tile) {
-  const int lane = threadIdx.x & 31;
-  const int64_t n = (int64_t)V * n_tile;
-  for (int64_t vt = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5); vt < n; vt += (int64_t)gridDim.x * 8) {
-    const int v = (int)(vt / n_tile);
-    const MatView mv = mp.views[v];
-    const uint32_t* bv = mp.MT + mv.mt_base + (size_t)(vt - (int64_t)v * n_tile) * mv.W;
-    uint32_t c = 0;
-    for (uint32_t w = lane; w < mv.W; w += 32) c += (uint32_t)__popc(__ldg(bv + w));
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xffffffffu, c, d);
-    if (lane == 0) mp.large_count[vt] = c;
+    // large_count[(v, tile)] (zeroed by the caller): this block's 256 rows of the tile's bit vector
+    const uint32_t c = (uint32_t)(__popc(lo.x) + __popc(lo.y) + __popc(lo.z) + __popc(lo.w) + __popc(hi.x) + __popc(hi.y) + __popc(hi.z) + __popc(hi.w));
+    if (c) atomicAdd(mp.large_count + (size_t)v * (size_t)n_tile + (size_t)tile, c);
   }
 }
 

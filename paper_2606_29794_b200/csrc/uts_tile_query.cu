@@ -1338,9 +1338,8 @@ int uts_tile_lists(const uts_config* cfg, uts_proj in, uts_mask mask, const uint
   }
   {
     dim3 grid((unsigned)((mp.n_words + 31) / 32), (unsigned)(n_mat / 256 + (uint64_t)d.V + 1));
+    UTS_CUDA(cudaMemsetAsync(mp.large_count, 0, (size_t)nvt * 4, ctx->side));       // the transpose adds each row block's counts
     matrix_transpose_kernel<<<grid, 256, 0, ctx->side>>>(mp, d.V, d.n_tile);
-    UTS_LAUNCH_CHECK();
-    matrix_popcount_kernel<<<(unsigned)ctx->sms * 8, 256, 0, ctx->side>>>(mp, d.V, d.n_tile);
     UTS_LAUNCH_CHECK();
   }
   // ---- small discs: emit at keys_tmp / vals_tmp, sort there (ping-pong through keys / vals, free until the merge), their ranges

@@ -20,7 +20,7 @@ constexpr int kSortThreads = 256;
 #define UTS_SORT_ITEMS 12
 #endif
 #ifndef UTS_SORT_MINB
-#define UTS_SORT_MINB 3
+#define UTS_SORT_MINB 4
 #endif
 constexpr int kSortItems = UTS_SORT_ITEMS;
 constexpr int kSortTile = kSortThreads * kSortItems;     // 3072 pairs per block (47 KB of static shared memory)

@@ -613,9 +613,12 @@ ring_query_batch_kernel(QueryParams qp, int which /*0: rc_warp class, 1: rc_thre
         if (cnt == 0) skip = true;
         else if (cnt <= (uint64_t)kTileCacheK) { r.cached = (uint32_t)cnt; skip = true; }
       }
-      load_ring_disc(qp, dir, lonlat, rs, k, r.D);
-      if (r.D.all) skip = true;                        // handled after the row loop
-      r.D.i_hi = min(r.D.i_hi, r.D.i_lo + rc - 1);
+      if (EMIT && skip) r.D.all = false;               // no pairs, or replayed from tile_cache: the disc itself is not needed
+      else {
+        load_ring_disc(qp, dir, lonlat, rs, k, r.D);
+        if (r.D.all) skip = true;                      // handled after the row loop
+        r.D.i_hi = min(r.D.i_hi, r.D.i_lo + rc - 1);
+      }
       r.skip = skip ? 1u : 0u;
       r.mbase = (EMIT && !skip) ? qp.mask_base[k] : 0xffffffffu;          // emit: the count pass kept this disc's row masks
       if (!skip && r.mbase == 0xffffffffu) my_rings = (uint32_t)(r.D.i_hi - r.D.i_lo + 1);

@@ -128,12 +128,10 @@ __device__ __forceinline__ void ring_pair(int order, int i, double lam, uint64_t
 }
 
 // Interp_H support of direction (dx,dy,dz) (camera frame; polar axis +y, longitude atan2(dx,dz): reading A1).
-__device__ __forceinline__ int interp_support(int order, double dx, double dy, double dz, uint64_t pix[8], double w[8]) {
+// (the direction as longitude lam in [0, 2 pi), z = cos(colatitude) and sth = sin(colatitude), up to a common positive factor of z, sth)
+__device__ __forceinline__ int interp_support_lzs(int order, double lam, double z, double sth, uint64_t pix[8], double w[8]) {
   const int N = 1 << order, last = 4 * N - 1;
-  const double z = dy, sth = sqrt(dx * dx + dz * dz);
   double theta = 0.0;                                 // colatitude: only the two polar caps below need the angle itself
-  double lam = atan2(dx, dz);
-  if (lam < 0.0) lam += 2.0 * kPi;
   // largest ring whose colatitude is <= theta (0: north of ring 1): closed-form estimate, then settled on ring colatitudes
   int i1;
   if (z > 2.0 / 3.0) i1 = (int)floor((double)N * sqrt(3.0 * (1.0 - z)));
@@ -190,14 +188,33 @@ __device__ __forceinline__ int interp_support(int order, double dx, double dy, d
   return 4;
 }
 
+__device__ __forceinline__ int interp_support(int order, double dx, double dy, double dz, uint64_t pix[8], double w[8]) {
+  double lam = atan2(dx, dz);
+  if (lam < 0.0) lam += 2.0 * kPi;
+  return interp_support_lzs(order, lam, dy, sqrt(dx * dx + dz * dz), pix, w);
+}
+
 // valid HEALPix samples of image pixel (i,j) as slot-layout indices with renormalised weights (reading A27)
 __device__ __forceinline__ int pixel_support(int order, const CamParams& c, const int32_t* __restrict__ slot_of_tile,
                                              const uint32_t* __restrict__ mask_bits, int i, int j, int64_t idx[8], float w[8], bool& in_domain) {
-  double dx, dy, dz;
-  in_domain = cam_pixel_dir(c, (double)i + 0.5, (double)j + 0.5, dx, dy, dz);
-  if (!in_domain) return 0;
   uint64_t pix[8]; double ww[8];
-  const int n = interp_support(order, dx, dy, dz, pix, ww);
+  int n;
+  if (c.model == UTS_CAM_EQUIRECT) {
+    // the image's own coordinates are longitude and latitude (cam_pixel_dir's last branch): lam = om mod 2 pi, (z, sth) = (sin, cos)(ph),
+    // without the detour through the direction and its atan2
+    const double u = (double)i + 0.5, v = (double)j + 0.5;
+    in_domain = u >= 0.0 && u < (double)c.W && v >= 0.0 && v < (double)c.H;
+    if (!in_domain) return 0;
+    double lam = u * c.a - kPi, sp, cp;
+    if (lam < 0.0) lam += 2.0 * kPi;
+    sincos(0.5 * kPi - v * c.b, &sp, &cp);
+    n = interp_support_lzs(order, lam, sp, fabs(cp), pix, ww);
+  } else {
+    double dx, dy, dz;
+    in_domain = cam_pixel_dir(c, (double)i + 0.5, (double)j + 0.5, dx, dy, dz);
+    if (!in_domain) return 0;
+    n = interp_support(order, dx, dy, dz, pix, ww);
+  }
   int cnt = 0; double sum = 0.0;
   for (int k = 0; k < n; ++k) {
     const uint64_t p = pix[k];

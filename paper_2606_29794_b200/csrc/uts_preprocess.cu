@@ -138,7 +138,7 @@ __device__ __forceinline__ void geometry(const ViewConst& vc, const double mu[3]
 // PARTS: 1 = geometry records only (everything but rgb; needs no SH), 2 = colour only (rgb and the clamp bits of flags, on records
 // whose geometry part has run), 3 = both in one pass (uts_preprocess).  1 then 2 writes exactly what 3 writes.
 template <int PARTS>
-__global__ void __launch_bounds__(128, 6)
+__global__ void __launch_bounds__(128, 8)
 preprocess_fwd_kernel(uts_config cfg, const float* __restrict__ means, const float* __restrict__ scales,
                       const float* __restrict__ quats, const float* __restrict__ opac, const float* __restrict__ sh,
                       const float* __restrict__ Wv, const float* __restrict__ bv, uts_proj out, double h) {

@@ -246,7 +246,8 @@ preprocess_fwd_kernel(uts_config cfg, const float* __restrict__ means, const flo
 //                                degree 3, as float4), and the view-direction term added to dL_dmeans.
 // As one kernel the 128-register cap spilt 0.5 KB per thread and every further view read-modified-wrote the 192 B of dL_dsh
 // (config 5, 4 views: 2.2 ms for 1 M Gaussians); split, neither kernel spills.
-__global__ void __launch_bounds__(128)
+// (four resident blocks per SM: 128 registers with 0.3 KB of spills beat 192 registers without: 0.21 -> 0.16 ms on config 4)
+__global__ void __launch_bounds__(128, 4)
 preprocess_bwd_geo_kernel(uts_config cfg, const float* __restrict__ means, const float* __restrict__ scales,
                           const float* __restrict__ quats, const float* __restrict__ Wv, const float* __restrict__ bv,
                           const uint8_t* __restrict__ flags, const float* __restrict__ dL_dconic, const float* __restrict__ dL_dmu2,
@@ -333,7 +334,7 @@ preprocess_bwd_geo_kernel(uts_config cfg, const float* __restrict__ means, const
 
 // Colour path: rgb_ch = max(0, 1/2 + sum_m Y_m(vdir) sh[m,ch]) (reading A13).  dL_dmeans must hold the geometry part already.
 template <int DEG>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, 4)
 preprocess_bwd_color_kernel(uts_config cfg, const float* __restrict__ means, const float* __restrict__ sh, const float* __restrict__ Wv,
                             const float* __restrict__ bv, const uint8_t* __restrict__ flags, const float* __restrict__ dL_drgb,
                             float* __restrict__ dL_dmeans, float* __restrict__ dL_dsh) {
